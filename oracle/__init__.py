@@ -1,0 +1,134 @@
+"""TEST INFRASTRUCTURE ONLY -- the CPU oracle for out-of-core DGEMM (C = alpha*A*B + beta*C, FP64).
+
+Plain C (oracle/dgemm_oracle.c, see its header for the definition and the PAPER.md citations),
+compiled with `gcc -O2 -ffp-contract=off -fopenmp` and called through ctypes.  It shares nothing
+with the CUDA path in paper_1808_05056_b200/ and must never be imported by it: only tests/,
+__graft_entry__.smoke() and bench.py's cpu_baseline / `--impl reference` legs use it.
+
+Pinned by tests/test_oracle_pins.py (brute force, int64 exactness, closed forms, exact-sum error
+bound, numpy cross-check, the paper's 44-element partition example) -- nothing here is
+"parity unpinned".
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "dgemm_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+
+# the gate of BASELINE.json north_star as read in DESIGN.md (G14): |C - C_ref| <= RTOL * D
+RTOL = 1e-13
+
+
+def build(force: bool = False) -> str:
+    """Compile liboracle.so if missing or stale.  Never -ffast-math, never contraction."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
+                               "-o", _LIB, _SRC, "-lm"])
+    return _LIB
+
+
+_lib = None
+_i64 = ctypes.c_int64
+_dbl = ctypes.c_double
+_ptr = ctypes.c_void_p
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        lib.oracle_dgemm.restype = ctypes.c_int
+        lib.oracle_dgemm.argtypes = [_i64, _i64, _i64, _dbl, _ptr, _i64, _ptr, _i64, _dbl, _ptr, _i64, _ptr, _i64]
+        lib.oracle_dgemm_sub.restype = ctypes.c_int
+        lib.oracle_dgemm_sub.argtypes = [_i64, _i64, _i64, _dbl, _ptr, _i64, _ptr, _i64, _dbl, _ptr, _i64,
+                                         _i64, _ptr, _i64, _ptr, _ptr, _ptr]
+        lib.oracle_partition.restype = ctypes.c_int
+        lib.oracle_partition.argtypes = [_i64, _i64, _i64, _i64, ctypes.POINTER(_i64), ctypes.POINTER(_i64)]
+        _lib = lib
+    return _lib
+
+
+def _chk2d(x, name):
+    assert isinstance(x, np.ndarray) and x.dtype == np.float64 and x.ndim == 2 and x.strides[1] == 8 \
+        and x.strides[0] % 8 == 0, f"{name}: need a row-major float64 2-D array"
+    return x.ctypes.data, x.strides[0] // 8
+
+
+def dgemm_ptr(M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, D=0, ldd=0) -> None:
+    """Raw-address form (host pointers as ints), for multi-GB buffers not owned by numpy."""
+    rc = _load().oracle_dgemm(M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, D or None, ldd)
+    if rc != 0:
+        raise RuntimeError(f"oracle_dgemm failed: {rc}")
+
+
+def dgemm(alpha, A, B, beta, C, want_denominator=False):
+    """C <- alpha*A*B + beta*C in place (numpy row-major views; M, N, K from C and A).
+    Returns D (the tolerance denominator) when asked, else None."""
+    M, N = C.shape
+    K = A.shape[1] if A is not None else 0
+    cp, ldc = _chk2d(C, "C")
+    ap, lda = _chk2d(A, "A") if A is not None and A.size else (None, max(K, 1))
+    bp, ldb = _chk2d(B, "B") if B is not None and B.size else (None, max(N, 1))
+    if A is not None and A.size:
+        assert A.shape[0] == M and B.shape == (K, N)
+    D = np.empty((M, N)) if want_denominator else None
+    rc = _load().oracle_dgemm(M, N, K, alpha, ap, lda, bp, ldb, beta, cp, ldc,
+                              D.ctypes.data if D is not None else None, N)
+    if rc != 0:
+        raise RuntimeError(f"oracle_dgemm failed: {rc}")
+    return D
+
+
+def dgemm_sub_ptr(M, N, K, alpha, A, lda, B, ldb, beta, C0, ldc, rows=None, cols=None,
+                  want_denominator=True):
+    """Sampled outputs from raw host addresses: the sub-matrix rows x cols of the updated C (dense),
+    plus its denominator.  rows/cols: 1-D int arrays or None for all."""
+    rows_a = None if rows is None else np.ascontiguousarray(rows, dtype=np.int64)
+    cols_a = None if cols is None else np.ascontiguousarray(cols, dtype=np.int64)
+    nr = M if rows_a is None else rows_a.size
+    nc = N if cols_a is None else cols_a.size
+    out = np.empty((nr, nc))
+    dout = np.empty((nr, nc)) if want_denominator else None
+    rc = _load().oracle_dgemm_sub(M, N, K, alpha, A or None, lda, B or None, ldb, beta, C0 or None, ldc,
+                                  nr, rows_a.ctypes.data if rows_a is not None else None,
+                                  nc, cols_a.ctypes.data if cols_a is not None else None,
+                                  out.ctypes.data, dout.ctypes.data if dout is not None else None)
+    if rc != 0:
+        raise RuntimeError(f"oracle_dgemm_sub failed: {rc}")
+    return out, dout
+
+
+def dgemm_sub(alpha, A, B, beta, C0, rows=None, cols=None, want_denominator=True):
+    """numpy-view form of dgemm_sub_ptr; C0 may be None when beta == 0."""
+    M, K = A.shape
+    N = B.shape[1]
+    ap, lda = _chk2d(A, "A") if A.size else (0, max(K, 1))
+    bp, ldb = _chk2d(B, "B") if B.size else (0, max(N, 1))
+    cp, ldc = _chk2d(C0, "C0") if C0 is not None else (0, N)
+    return dgemm_sub_ptr(M, N, K, alpha, ap, lda, bp, ldb, beta, cp, ldc, rows, cols, want_denominator)
+
+
+def partition(M, N, K, S):
+    """(h, w) of the paper's hclMatrixPartitioner rule by enumeration, or None if nothing fits."""
+    h, w = _i64(), _i64()
+    rc = _load().oracle_partition(M, N, K, S, ctypes.byref(h), ctypes.byref(w))
+    if rc == 1:
+        return None
+    if rc != 0:
+        raise ValueError("oracle_partition: bad argument")
+    return h.value, w.value
+
+
+def within_gate(C_test: np.ndarray, C_ref: np.ndarray, D: np.ndarray, rtol: float = RTOL):
+    """Elementwise gate |C_test - C_ref| <= rtol * D (G14).  Returns (ok, worst ratio)."""
+    err = np.abs(C_test - C_ref)
+    bad = ~(err <= rtol * D)          # NaN-safe: NaN fails
+    with np.errstate(divide="ignore", invalid="ignore"):
+        ratio = np.where(D > 0, err / D, np.where(err == 0, 0.0, np.inf))
+    return (not bad.any()), float(np.nanmax(ratio)) if ratio.size else 0.0

@@ -1,0 +1,293 @@
+"""Pins for the CPU oracle (oracle/dgemm_oracle.c) against things other than itself.
+
+What fixes the answer here is the definition C = alpha*A*B + beta*C and
+mathematics: brute force in pure Python, exact int64 arithmetic, closed forms, exactly rounded sums
+(math.fsum), a library matmul within the gate, and the paper's printed partition example
+(tests/golden/paper_partition_example.txt).  A dropped k term, a swapped index,
+a transposed operand, a fused multiply-add or a wrong epilogue sign fails at least one of them.
+"""
+import itertools
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import synthgen
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def padded(rng, rows, cols, pad, fill="uniform"):
+    """rows x cols view into a wider NaN-padded buffer (leading dimension cols + pad)."""
+    buf = np.full((max(rows, 1), cols + pad), np.nan)
+    v = buf[:rows, :cols]
+    if fill == "uniform":
+        v[...] = rng.uniform(-1, 1, (rows, cols))
+    elif fill == "int":
+        v[...] = rng.integers(-4, 5, (rows, cols)).astype(np.float64)
+    return buf, v
+
+
+def naive_ijk(alpha, A, B, beta, C0):
+    """The definition in pure Python floats (IEEE double, no fma): i-j-k, in-order k."""
+    M, N = C0.shape
+    K = A.shape[1]
+    out = np.empty((M, N))
+    for i in range(M):
+        for j in range(N):
+            acc = 0.0
+            if alpha != 0.0:
+                for k in range(K):
+                    acc = acc + float(A[i, k]) * float(B[k, j])
+            if beta == 0.0:
+                out[i, j] = alpha * acc
+            else:
+                out[i, j] = alpha * acc + beta * float(C0[i, j])
+    return out
+
+
+def bits(x):
+    return np.ascontiguousarray(x).view(np.uint64)
+
+
+# ---------------------------------------------------------------- brute force, bit-identical
+def test_brute_force_all_tiny_shapes_bit_identical():
+    rng = np.random.default_rng(1)
+    for M, N, K in itertools.product(range(0, 6), range(0, 6), [0, 1, 2, 3, 5, 9]):
+        pad = int(rng.integers(0, 4))
+        _, A = padded(rng, M, K, pad)
+        _, B = padded(rng, K, N, pad + 1)
+        cbuf, C = padded(rng, M, N, pad + 2)
+        alpha, beta = float(rng.uniform(-2, 2)), float(rng.choice([0.0, 1.0, -0.75, 0.5]))
+        want = naive_ijk(alpha, A, B, beta, C.copy())
+        oracle.dgemm(alpha, A, B, beta, C)
+        assert np.array_equal(bits(C), bits(want)), (M, N, K)
+        if M:
+            assert np.isnan(cbuf[:M, N:]).all()          # padding of C untouched
+
+
+def test_brute_force_spans_blocks_and_ragged_tail():
+    # sizes beyond the oracle's 32-row / 128-k blocking with ragged tails, still bit-identical
+    rng = np.random.default_rng(2)
+    M, N, K = 37, 11, 263
+    _, A = padded(rng, M, K, 3)
+    _, B = padded(rng, K, N, 5)
+    _, C = padded(rng, M, N, 2)
+    want = naive_ijk(-1.25, A, B, 0.5, C.copy())
+    oracle.dgemm(-1.25, A, B, 0.5, C)
+    assert np.array_equal(bits(C), bits(want))
+
+
+def test_no_fused_multiply_add():
+    # (1+e)*(1-e) = 1 - e^2 rounds to 1.0 as a separate product, so acc = 1.0 - 1.0 = 0 exactly;
+    # an fma would keep -e^2.  Catches -ffp-contract / FMA code generation in the oracle.
+    e = 2.0 ** -30
+    A = np.array([[1.0 + e, 1.0]])
+    B = np.array([[1.0 - e], [-1.0]])
+    C = np.zeros((1, 1))
+    oracle.dgemm(1.0, A, B, 0.0, C)
+    assert C[0, 0] == 0.0
+
+
+# ---------------------------------------------------------------- exact integer arithmetic
+@pytest.mark.parametrize("M,N,K,alpha,beta", [(33, 47, 129, 1.0, 0.5), (64, 64, 512, 2.0, -1.0),
+                                              (5, 130, 1000, -3.0, 1.0), (70, 3, 77, 1.0, 0.0)])
+def test_integer_inputs_equal_int64_reference(M, N, K, alpha, beta):
+    rng = np.random.default_rng(M * 1000 + N)
+    _, A = padded(rng, M, K, 1, "int")
+    _, B = padded(rng, K, N, 2, "int")
+    _, C = padded(rng, M, N, 3, "int")
+    Ai, Bi, Ci = A.astype(np.int64), B.astype(np.int64), C.astype(np.int64)
+    # everything in exact integers scaled by 2 (beta may be a half-integer)
+    want2 = int(round(alpha * 2)) * (Ai @ Bi) + int(round(beta * 2)) * Ci
+    assert np.abs(want2).max() < 2 ** 52
+    oracle.dgemm(alpha, A, B, beta, C)
+    assert np.array_equal(C * 2.0, want2.astype(np.float64))
+
+
+def test_generator_integer_variant_exact():
+    M = N = K = 96
+    A = synthgen.fill(np.empty((M, K)), 7, "A", "int")
+    B = synthgen.fill(np.empty((K, N)), 7, "B", "int")
+    C = synthgen.fill(np.empty((M, N)), 7, "C", "int")
+    assert A.min() >= -4 and A.max() <= 4 and not np.signbit(A[A == 0]).any()
+    want2 = 2 * (A.astype(np.int64) @ B.astype(np.int64)) + C.astype(np.int64)
+    oracle.dgemm(1.0, A, B, 0.5, C)
+    assert np.array_equal(C * 2.0, want2.astype(np.float64))
+
+
+# ---------------------------------------------------------------- closed forms
+def test_identity_A_gives_alpha_B_plus_beta_C():
+    rng = np.random.default_rng(3)
+    K = N = 41
+    B = rng.uniform(-1, 1, (K, N))
+    C0 = rng.uniform(-1, 1, (K, N))
+    C = C0.copy()
+    oracle.dgemm(1.5, np.eye(K), B, -0.25, C)
+    assert np.array_equal(C, 1.5 * B + (-0.25) * C0)     # adding exact zeros changes nothing
+
+
+def test_permutation_matrices_permute_rows_and_columns():
+    rng = np.random.default_rng(4)
+    n = 29
+    p = rng.permutation(n)
+    P = np.zeros((n, n)); P[np.arange(n), p] = 1.0        # (P @ X)[i] = X[p[i]]
+    X = rng.uniform(-1, 1, (n, 17))
+    C = np.zeros((n, 17))
+    oracle.dgemm(1.0, P, X, 0.0, C)
+    assert np.array_equal(C, X[p])
+    Y = rng.uniform(-1, 1, (13, n))
+    C = np.zeros((13, n))
+    oracle.dgemm(1.0, Y, P, 0.0, C)                       # (Y @ P)[:, p[i]] = Y[:, i]
+    want = np.zeros((13, n)); want[:, p] = Y
+    assert np.array_equal(C, want)
+
+
+def test_rank_one_outer_product_exact_rounding_sequence():
+    rng = np.random.default_rng(5)
+    u = rng.uniform(-1, 1, (23, 1)); v = rng.uniform(-1, 1, (1, 31))
+    C0 = rng.uniform(-1, 1, (23, 31)); C = C0.copy()
+    oracle.dgemm(0.75, u, v, 1.25, C)
+    want = 0.75 * (0.0 + u * v) + 1.25 * C0               # same three roundings per element
+    assert np.array_equal(bits(C), bits(want))
+
+
+def test_all_ones_and_index_products():
+    M, N, K = 19, 21, 300
+    C = np.full((M, N), 2.0)
+    oracle.dgemm(3.0, np.ones((M, K)), np.ones((K, N)), 0.5, C)
+    assert np.array_equal(C, np.full((M, N), 3.0 * K + 1.0))
+    A = np.repeat(np.arange(1.0, M + 1)[:, None], K, axis=1)
+    B = np.repeat(np.arange(1.0, N + 1)[None, :], K, axis=0)
+    C = np.zeros((M, N))
+    oracle.dgemm(1.0, A, B, 0.0, C)
+    assert np.array_equal(C, np.outer(np.arange(1.0, M + 1), np.arange(1.0, N + 1)) * K)
+
+
+def test_non_symmetric_shape_catches_transposed_operands():
+    # A_ik = 10*i + k, B_kj = k - 3*j : sum_k has a closed form that is not symmetric in (i, j)
+    M, N, K = 7, 5, 9
+    i = np.arange(M)[:, None]; k = np.arange(K)[None, :]
+    A = (10.0 * i + k)
+    B = (np.arange(K)[:, None] - 3.0 * np.arange(N)[None, :])
+    C = np.zeros((M, N))
+    oracle.dgemm(1.0, A, B, 0.0, C)
+    kk = np.arange(K)
+    want = np.array([[float(sum((10 * ii + q) * (q - 3 * jj) for q in kk)) for jj in range(N)] for ii in range(M)])
+    assert np.array_equal(C, want)
+
+
+def test_alpha_zero_does_not_read_A_B_and_beta_zero_does_not_read_C():
+    rng = np.random.default_rng(6)
+    M, N, K = 9, 8, 7
+    nanA, nanB = np.full((M, K), np.nan), np.full((K, N), np.nan)
+    C0 = rng.uniform(-1, 1, (M, N)); C = C0.copy()
+    oracle.dgemm(0.0, nanA, nanB, -2.0, C)
+    assert np.array_equal(C, -2.0 * C0)
+    A = rng.uniform(-1, 1, (M, K)); B = rng.uniform(-1, 1, (K, N))
+    C = np.full((M, N), np.nan)
+    oracle.dgemm(1.0, A, B, 0.0, C)
+    assert np.isfinite(C).all() and np.array_equal(bits(C), bits(naive_ijk(1.0, A, B, 0.0, np.zeros((M, N)))))
+    C = np.full((M, N), np.nan)
+    oracle.dgemm(0.0, nanA, nanB, 0.0, C)
+    assert np.array_equal(bits(C), bits(np.zeros((M, N))))        # +0 everywhere, sign included
+    C = C0.copy()
+    oracle.dgemm(1.0, np.empty((M, 0)), np.empty((0, N)), 0.5, C)  # K == 0
+    assert np.array_equal(C, 0.5 * C0)
+
+
+# ---------------------------------------------------------------- error bound vs exactly rounded sums
+@pytest.mark.parametrize("K,dist", [(512, "uniform"), (4096, "uniform"), (2048, "normal")])
+def test_error_against_exact_sum_is_far_below_gate(K, dist):
+    M, N = 6, 5
+    A = synthgen.fill(np.empty((M, K)), 11, "A", dist)
+    B = synthgen.fill(np.empty((K, N)), 11, "B", dist)
+    C0 = synthgen.fill(np.empty((M, N)), 11, "C", dist)
+    alpha, beta = 1.0, 0.5        # powers of two: the epilogue scaling is exact, so fsum is THE answer
+    C = C0.copy()
+    D = oracle.dgemm(alpha, A, B, beta, C, want_denominator=True)
+    from fractions import Fraction
+    for i in range(M):
+        for j in range(N):
+            exact = sum((Fraction(float(A[i, k])) * Fraction(float(B[k, j])) for k in range(K)), Fraction(0))
+            exact = alpha * exact + Fraction(beta) * Fraction(float(C0[i, j]))
+            dexact = sum((abs(Fraction(float(A[i, k])) * Fraction(float(B[k, j]))) for k in range(K)), Fraction(0))
+            dexact = dexact + Fraction(beta) * abs(Fraction(float(C0[i, j])))
+            err = abs(Fraction(float(C[i, j])) - exact)
+            u = Fraction(1, 2 ** 53)
+            assert err <= (K + 2) * u * dexact * Fraction(101, 100)      # classical gamma_K bound
+            assert float(err) <= 2e-15 * float(dexact)                   # ~50x below the 1e-13 gate
+            assert abs(float(D[i, j]) - float(dexact)) <= 1e-12 * float(dexact)   # pins D itself
+
+
+def test_library_matmul_agrees_within_gate():
+    M, N, K = 150, 170, 700
+    A = synthgen.fill(np.empty((M, K)), 12, "A", "uniform")
+    B = synthgen.fill(np.empty((K, N)), 12, "B", "uniform")
+    C0 = synthgen.fill(np.empty((M, N)), 12, "C", "uniform")
+    C = C0.copy()
+    D = oracle.dgemm(2.0, A, B, -1.0, C, want_denominator=True)
+    ok, worst = oracle.within_gate(2.0 * (A @ B) - C0, C, D)
+    assert ok and worst < 1e-14
+    # the denominator is what it says
+    assert np.allclose(D, 2.0 * (np.abs(A) @ np.abs(B)) + np.abs(C0), rtol=1e-12, atol=0)
+    # and the gate is sharp enough to see one dropped k term
+    Cbad = 2.0 * (A[:, :-1] @ B[:-1]) - C0
+    ok_bad, _ = oracle.within_gate(Cbad, C, D)
+    assert not ok_bad
+
+
+# ---------------------------------------------------------------- sampled form == full form
+def test_sub_matches_full_bit_for_bit():
+    M, N, K = 45, 52, 301
+    rng = np.random.default_rng(8)
+    _, A = padded(rng, M, K, 2); _, B = padded(rng, K, N, 1); _, C0 = padded(rng, M, N, 4)
+    C = C0.copy()
+    D = oracle.dgemm(1.0, A, B, 0.5, C, want_denominator=True)
+    rows = np.array([0, 44, 31, 32, 7]); cols = np.array([51, 0, 13])
+    s, d = oracle.dgemm_sub(1.0, A, B, 0.5, C0, rows=rows, cols=None)
+    assert np.array_equal(bits(s), bits(C[rows])) and np.array_equal(bits(d), bits(D[rows]))
+    s, d = oracle.dgemm_sub(1.0, A, B, 0.5, C0, rows=None, cols=cols)
+    assert np.array_equal(bits(s), bits(C[:, cols])) and np.array_equal(bits(d), bits(D[:, cols]))
+    s, d = oracle.dgemm_sub(1.0, A, B, 0.5, C0, rows=rows, cols=cols)
+    assert np.array_equal(bits(s), bits(C[np.ix_(rows, cols)]))
+    s, _ = oracle.dgemm_sub(1.0, A, B, 0.0, None, rows=rows, cols=cols)      # beta == 0: C0 not needed
+    assert np.array_equal(bits(s), bits(naive_ijk(1.0, A, B, 0.0, np.zeros((M, N)))[np.ix_(rows, cols)]))
+
+
+# ---------------------------------------------------------------- the paper's partition example
+def test_paper_partition_example_golden():
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "paper_partition_example.txt")) if l.strip() and not l.startswith("#")]
+    assert len(rows) == 1
+    M, N, K, S, total, h, w, blocks, steps = map(int, rows[0])
+    assert M * K + K * N + M * N == total and total > S             # "80 exceeds 44"
+    assert oracle.partition(M, N, K, S) == (h, w)                   # Figure 3
+    assert h * w == blocks == steps                                  # "w x h main steps"
+    # the reading is discriminating: both rival readings of PAPER.md:289 contradict Figure 3
+    feas = [(hh, ww) for hh in (1, 2, 4) for ww in (1, 2, 4)
+            if K * (N // ww) + 2 * (M // hh) * K + 2 * (M // hh) * (N // ww) <= S]
+    assert sorted(feas) == [(2, 4), (4, 2), (4, 4)]
+    assert oracle.partition(M, N, K, 19) is None                     # (4,4) needs 8+16+2 = 26 > 19
+    assert oracle.partition(M, N, K, 80 * 2) == (1, 1)               # everything fits: in-core
+
+
+# ---------------------------------------------------------------- generator twins agree
+@pytest.mark.parametrize("dist", ["uniform", "int", "normal"])
+def test_generator_c_and_numpy_twins_agree(dist):
+    a = np.full((9, 20), np.nan)
+    synthgen.fill(a, 99, "C", dist, cols=17, row0=5, col0=3, logical_cols=1000)
+    b = synthgen.fill_numpy(9, 17, 99, "C", dist, row0=5, col0=3, logical_cols=1000)
+    if dist == "normal":
+        assert np.allclose(a[:, :17], b, rtol=1e-14, atol=1e-15)      # libm vs numpy log/cos: last ulps
+    else:
+        assert np.array_equal(a[:, :17], b)
+    assert np.isnan(a[:, 17:]).all()
+    # a sub-block regenerates the same values as the whole
+    whole = synthgen.fill(np.empty((14, 1000)), 99, "C", dist)
+    assert np.array_equal(a[:, :17], whole[5:14, 3:20])
+    if dist == "uniform":
+        assert whole.min() >= -1.0 and whole.max() < 1.0 and abs(whole.mean()) < 0.02
+    if dist == "normal":
+        assert abs(whole.mean()) < 0.03 and abs(whole.std() - 1.0) < 0.03
