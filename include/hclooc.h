@@ -1,0 +1,192 @@
+/* hclooc.h -- C ABI of libhclooc_b200: out-of-core FP64 matrix multiplication on one NVIDIA B200.
+ *
+ * The operation is the paper's MMOOC (arXiv 1808.05056; citations are PAPER.md:<line>):
+ *
+ *     C = alpha * A * B + beta * C        A is M x K, B is K x N, C is M x N, FP64   (:180, :275)
+ *
+ * with A, B and C resident in (pinned) host memory and the device restricted to a stated memory
+ * budget (:277 "dMemSize", :289).  The library cuts A into horizontal slices, B into vertical slices
+ * and C into blocks (:289, Figure 3 :281), streams them through device buffers on separate
+ * host-to-device, compute and device-to-host CUDA streams synchronised with events (:291, :303-313),
+ * and runs a hand-written sm_100a FP64 tile kernel per step (the "in-core DGEMM" of :308).
+ *
+ * Conventions for every function
+ *   - Storage is ROW-MAJOR, no transposes; leading dimensions are in ELEMENTS (doubles).
+ *   - All functions return an int status: 0 = success; a NEGATIVE value -k means the k-th argument
+ *     (1-based, in the order of the C prototype) is invalid (LAPACK "info" convention); POSITIVE
+ *     values are the HCLOOC_ERR_* codes below.  Nothing aborts and nothing throws across this ABI.
+ *   - "host" pointers must be page-locked (hclooc_host_alloc / hclooc_host_register / cudaHostAlloc)
+ *     and "device" pointers must come from hclMalloc / cudaMalloc on the current device.  There is no
+ *     pageable or CPU fallback.
+ *   - The library never takes ownership of caller memory.
+ */
+#ifndef HCLOOC_H
+#define HCLOOC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ------------------------------------------------------------------ status codes */
+#define HCLOOC_OK               0
+#define HCLOOC_ERR_BUDGET       1   /* device budget below the minimum working set of the planner   */
+#define HCLOOC_ERR_NOT_PINNED   2   /* A, B or C is pageable host memory (no silent fallback)       */
+#define HCLOOC_ERR_CUDA         3   /* a CUDA call failed; see hclooc_last_cuda_error()             */
+#define HCLOOC_ERR_NOMEM        4   /* device or host allocation failed                             */
+#define HCLOOC_ERR_ALIGN        5   /* device operand not 16-byte aligned / odd leading dimension   */
+#define HCLOOC_ERR_INTERNAL     6   /* planner/executor invariant violated (a bug)                  */
+
+/* ------------------------------------------------------------------ handles */
+typedef struct hclooc_ctx hclooc_ctx;   /* opaque: device, streams, events, workspace              */
+typedef void* hclStream;                /* a cudaStream_t (the paper's hclStream, :144)            */
+typedef void* hclEvent;                 /* a cudaEvent_t  (the paper's hclEvent,  :146)            */
+
+/* copy direction, the paper's enum Direction {H2D, D2H} (:136) */
+#define HCL_H2D 0
+#define HCL_D2H 1
+
+/* ------------------------------------------------------------------ the plan (hclMatrixPartitioner, :186, :289)
+ * Loop structure:  for p < kpanels:  for j < w:  for i < h:  one step computes the C block
+ * (rows i*mb .., cols j*nb ..) with the K panel p (k0 = p*kb):   c_ij = alpha*a_i*b_j + beta'*c_ij   (:308)
+ * where beta' = beta for p == 0 and 1 afterwards.  Step index idx = i + h*(j + w*p) (:191 for p = 0).
+ * Edge slices are ragged (ceil division; the paper only treats equal slices).                       */
+typedef struct hclooc_plan_t {
+    int64_t  M, N, K;
+    int64_t  mb, nb, kb;          /* rows of an A slice, columns of a B slice, depth of a K panel   */
+    int64_t  h, w, kpanels;       /* ceil(M/mb), ceil(N/nb), ceil(K/kb)                             */
+    int64_t  n_steps;             /* h * w * kpanels                                                */
+    int32_t  n_sets;              /* (A slice, C block) device buffer pairs, round-robin by step    */
+    int32_t  n_bbuf;              /* B slice device buffers (1 = paper's single buffer, 2 = prefetch) */
+    int32_t  beta_nonzero;        /* C blocks are uploaded only when 1 (or for K panels p > 0)      */
+    int32_t  scale_only;          /* alpha == 0 or K == 0: C = beta*C, A and B never referenced     */
+    int64_t  lda_dev, ldb_dev, ldc_dev;  /* leading dimensions of the device buffers (elements)    */
+    uint64_t bytes_a_buf, bytes_b_buf, bytes_c_buf;   /* one buffer of each kind                   */
+    uint64_t workspace_bytes;     /* n_bbuf*b + n_sets*(a + c), <= the budget                       */
+    uint64_t bytes_h2d, bytes_d2h;/* exactly what the executor enqueues over the host link          */
+    uint64_t n_copies_h2d, n_copies_d2h;
+    double   flops;               /* 2*M*N*K (:368)                                                 */
+    double   t_flop_s, t_link_s, t_model_s;  /* cost model terms used to pick this plan             */
+} hclooc_plan_t;
+
+/* Plan only (pure host arithmetic, needs no GPU).  alpha_zero != 0 plans the scale-only pass.
+ * Errors: -1..-3 negative dimension, -7 NULL out, HCLOOC_ERR_BUDGET.                               */
+int hclooc_plan(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zero,
+                size_t device_budget_bytes, hclooc_plan_t* out);
+
+/* The paper's own rule, kept for reference and tests (:289, worked example :301): EQUAL slices only,
+ * working set K*nb + 2*mb*K + 2*mb*nb <= budget_elements, least host-to-device traffic
+ * w*M*K + K*N + M*N; ties: fewest steps, then smallest h.  Returns HCLOOC_ERR_BUDGET if nothing fits. */
+int hclMatrixPartitioner(int64_t M, int64_t N, int64_t K, int64_t budget_elements, int64_t* h, int64_t* w);
+
+/* ------------------------------------------------------------------ the schedule (S2-S7 as a list of stream operations)
+ * hclooc_schedule() expands a plan into the exact sequence of operations the executor enqueues, in
+ * host issue order: copies, kernels, and the event records/waits that order them across streams
+ * (the paper's five event families eA, rA, rB, eC, rC, :187-188, :291, :311).  The executor issues this
+ * very list, so tests can check coverage, byte counts and hazard freedom without a GPU.            */
+#define HCLOOC_OP_H2D_A   0   /* S(a_i)  :306  host A[r0:r0+nr, c0:c0+nc] -> device buffer `buf`            */
+#define HCLOOC_OP_H2D_B   1   /* S(b_j)  :305  host B[r0.., c0..] -> rows dev_r0.. of device buffer `buf`   */
+#define HCLOOC_OP_H2D_C   2   /* S(c_ij) :307  host C[r0.., c0..] -> device buffer `buf`                    */
+#define HCLOOC_OP_GEMM    3   /* DGEMM   :308  buf3(C) = alpha*buf(A)*buf2(B) + beta*buf3(C); nr x nc x kk  */
+#define HCLOOC_OP_D2H_C   4   /* R(c_ij) :309  device buffer `buf` -> host C[r0.., c0..]                    */
+#define HCLOOC_OP_WAIT    5   /* stream waits for event (hclWaitEvent, :116)                              */
+#define HCLOOC_OP_RECORD  6   /* event recorded in stream (Rec(x), :311)                                  */
+/* streams: 0 = H2D copy stream, 1 = D2H copy stream, 2 + c = compute stream c.
+ * buffers: A slice of set s = s; C block of set s = n_sets + s; B slice b = 2*n_sets + b.            */
+typedef struct hclooc_op_t {
+    int32_t kind, stream, event;
+    int32_t buf, buf2, buf3;
+    int64_t r0, nr, c0, nc;       /* region of the host matrix (GEMM: nr x nc output block)          */
+    int64_t dev_r0;               /* first row inside the device buffer (B prefetch chunks)          */
+    int64_t k0, kk;               /* GEMM: K panel                                                    */
+    int64_t step;                 /* idx = i + h*(j + w*p)                                            */
+    double  beta;                 /* GEMM: effective beta of this step                                */
+} hclooc_op_t;
+
+/* Writes up to max_ops operations to ops (may be NULL to only count) and the total count to *n_ops.
+ * n_compute = number of compute streams the executor will round-robin over (>= 1).                  */
+int hclooc_schedule(const hclooc_plan_t* plan, int n_compute, hclooc_op_t* ops, size_t max_ops, size_t* n_ops);
+
+/* ------------------------------------------------------------------ statistics of one call */
+typedef struct hclooc_stats {
+    hclooc_plan_t plan;
+    uint64_t bytes_h2d, bytes_d2h;      /* counted at enqueue time; equal plan.bytes_*              */
+    uint64_t n_kernels, n_copies_h2d, n_copies_d2h;
+    double   t_total_s;                 /* wall time of the call, entry to return (:368 "including transfers") */
+    double   t_enqueue_s;               /* host time spent enqueueing                               */
+} hclooc_stats;
+
+/* ------------------------------------------------------------------ context
+ * device: CUDA ordinal.  d_workspace/workspace_bytes: caller-owned device memory (e.g. a PyTorch
+ * tensor) the context carves all its buffers from, or NULL/0 to let the library cudaMalloc (and grow)
+ * its own.  stream_h2d / stream_d2h: caller-owned cudaStream_t or NULL for library-owned.
+ * compute_streams[n_compute]: caller-owned compute streams, or NULL/0 for 4 library-owned ones.    */
+int hclooc_ctx_create(hclooc_ctx** ctx, int device, void* d_workspace, size_t workspace_bytes,
+                      hclStream stream_h2d, hclStream stream_d2h, hclStream* compute_streams, int n_compute);
+int hclooc_ctx_destroy(hclooc_ctx* ctx);
+
+/* ------------------------------------------------------------------ the operation
+ * hclooc_dgemm: C = alpha*A*B + beta*C, synchronous: C is complete in host memory on return.
+ *   A: M x K, lda >= K;  B: K x N, ldb >= N;  C: M x N, ldc >= N, updated IN PLACE; A, B read-only.
+ *   A, B, C: pinned HOST pointers (the product path).  Device pointers are also accepted (the copies
+ *   become device-to-device); that is what bench.py's HBM-resident `value` leg uses.
+ *   device_budget_bytes bounds the sum of all device buffers the call uses (0 = all free HBM minus a
+ *   1 GiB margin).  Uses a process-wide default context created on first use.
+ *   beta == 0: C is never read (NaN/Inf in C are overwritten).  alpha == 0 or K == 0: A and B are not
+ *   referenced, C = beta*C streamed through the device.  M == 0 or N == 0: returns 0, touches nothing.
+ * Errors: -1/-2/-3 negative M/N/K; -5 A NULL; -6 lda < K; -7 B NULL; -8 ldb < N; -10 C NULL or C
+ *   overlaps A or B; -11 ldc < N; HCLOOC_ERR_BUDGET; HCLOOC_ERR_NOT_PINNED; HCLOOC_ERR_NOMEM;
+ *   HCLOOC_ERR_CUDA.  Validation errors leave C untouched; after HCLOOC_ERR_CUDA C is unspecified.  */
+int hclooc_dgemm(int64_t M, int64_t N, int64_t K, double alpha, const double* A, int64_t lda,
+                 const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
+                 size_t device_budget_bytes);
+
+/* Same with an explicit context (NULL = default) and optional statistics (argument numbers in error
+ * codes are those of hclooc_dgemm).  If the context has a caller-owned workspace the budget is
+ * min(device_budget_bytes or workspace size, workspace size).                                      */
+int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
+                    int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
+                    size_t device_budget_bytes, hclooc_stats* stats_out);
+
+/* ------------------------------------------------------------------ the runtime the paper abstracts (:109-116, :212)
+ * CUDA only, plain functions (no virtual dispatch, cf. :164).                                      */
+int hclMalloc(void** dptr, size_t bytes);                         /* :109  device memory            */
+int hclFree(void* dptr);                                          /* :110                           */
+int hclGetMemSize(int device, size_t* free_bytes);                /* :111  free device memory       */
+int hclStreamCreate(hclStream* s);                                /* hclStreamFactory::create, :144 */
+int hclStreamDestroy(hclStream s);
+int hclEventDestroy(hclEvent e);
+int hclMemcpy(void* dst, const void* src, size_t bytes, int dir);                         /* :112   */
+/* Async calls take a stream and optionally create+record an event tied to the call (:140-146):
+ * if ev != NULL and *ev == NULL a new event is created; the event is recorded after the operation. */
+int hclMemcpyAsync(void* dst, const void* src, size_t bytes, int dir, hclStream s, hclEvent* ev);   /* :113 */
+/* 2-D strided copy (rows x width_bytes, pitches in bytes): needed for row-major column slices; not in the paper. */
+int hclMemcpy2DAsync(void* dst, size_t dpitch, const void* src, size_t spitch, size_t width_bytes,
+                     size_t rows, int dir, hclStream s, hclEvent* ev);
+/* In-core DGEMM on DEVICE pointers -- the tile kernel, one step of the pipeline (:212, :308):
+ *   dC = alpha*dA*dB + beta*dC, row-major.  dA, dB, dC 16-byte aligned, lda/ldb/ldc even, else
+ *   HCLOOC_ERR_ALIGN.  beta == 0: dC is not read.  K == 0 or alpha == 0: dC = beta*dC.              */
+int hclDgemmAsync(int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda,
+                  const double* dB, int64_t ldb, double beta, double* dC, int64_t ldc,
+                  hclStream s, hclEvent* ev);
+int hclWaitEvent(hclStream s, hclEvent e);                        /* :116  stream waits for event   */
+int hclStreamSynchronize(hclStream s);                            /* :115                           */
+int hclDeviceSynchronize(int device);                             /* :114                           */
+
+/* ------------------------------------------------------------------ pinned host memory */
+void* hclooc_host_alloc(size_t bytes);                 /* cudaHostAlloc; NULL on failure            */
+int   hclooc_host_free(void* p);
+int   hclooc_host_register(void* p, size_t bytes);     /* pin caller memory in place                */
+int   hclooc_host_unregister(void* p);
+
+/* ------------------------------------------------------------------ diagnostics */
+const char* hclooc_strerror(int status);
+int         hclooc_last_cuda_error(void);              /* last cudaError_t seen by this thread      */
+const char* hclooc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HCLOOC_H */

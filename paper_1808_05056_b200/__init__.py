@@ -1,0 +1,18 @@
+"""hclooc-b200: out-of-core FP64 matrix multiplication (the MMOOC of arXiv 1808.05056) on one B200.
+
+Thin ctypes binding over the C ABI in include/hclooc.h -- same names, argument marshalling only;
+every step of the hot path (plan, schedule, copies, events, the DMMA tile kernel) runs inside
+libhclooc_b200.so.  There is no CPU fallback: if the library cannot be built or loaded, importing
+the binding's functions raises.
+"""
+from ._binding import (  # noqa: F401
+    HclError, lib, HostMatrix, Plan, Stats,
+    hclooc_plan, hclooc_schedule, hclMatrixPartitioner,
+    hclooc_ctx_create, hclooc_ctx_destroy, hclooc_dgemm, hclooc_dgemm_ex,
+    hclMalloc, hclFree, hclGetMemSize, hclStreamCreate, hclStreamDestroy, hclEventDestroy,
+    hclMemcpy, hclMemcpyAsync, hclMemcpy2DAsync, hclDgemmAsync, hclWaitEvent,
+    hclStreamSynchronize, hclDeviceSynchronize,
+    hclooc_host_alloc, hclooc_host_free, hclooc_host_register, hclooc_host_unregister,
+    hclooc_strerror, hclooc_last_cuda_error, hclooc_version,
+    HCL_H2D, HCL_D2H, EXPORTS, OP_DTYPE,
+)

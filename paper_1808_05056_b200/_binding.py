@@ -1,0 +1,306 @@
+"""ctypes marshalling for include/hclooc.h.  No arithmetic of the method lives here."""
+from __future__ import annotations
+
+import ctypes
+from ctypes import POINTER, byref, c_char_p, c_double, c_int, c_int32, c_int64, c_size_t, c_uint64, c_void_p
+
+import numpy as np
+
+from . import build as _build
+
+HCL_H2D, HCL_D2H = 0, 1
+
+# every symbol include/hclooc.h declares (tests check the .so exports all of them)
+EXPORTS = [
+    "hclooc_plan", "hclMatrixPartitioner", "hclooc_schedule", "hclooc_ctx_create", "hclooc_ctx_destroy",
+    "hclooc_dgemm", "hclooc_dgemm_ex", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
+    "hclStreamDestroy", "hclEventDestroy", "hclMemcpy", "hclMemcpyAsync", "hclMemcpy2DAsync",
+    "hclDgemmAsync", "hclWaitEvent", "hclStreamSynchronize", "hclDeviceSynchronize",
+    "hclooc_host_alloc", "hclooc_host_free", "hclooc_host_register", "hclooc_host_unregister",
+    "hclooc_strerror", "hclooc_last_cuda_error", "hclooc_version",
+]
+
+
+class Plan(ctypes.Structure):
+    _fields_ = [("M", c_int64), ("N", c_int64), ("K", c_int64),
+                ("mb", c_int64), ("nb", c_int64), ("kb", c_int64),
+                ("h", c_int64), ("w", c_int64), ("kpanels", c_int64), ("n_steps", c_int64),
+                ("n_sets", c_int32), ("n_bbuf", c_int32), ("beta_nonzero", c_int32), ("scale_only", c_int32),
+                ("lda_dev", c_int64), ("ldb_dev", c_int64), ("ldc_dev", c_int64),
+                ("bytes_a_buf", c_uint64), ("bytes_b_buf", c_uint64), ("bytes_c_buf", c_uint64),
+                ("workspace_bytes", c_uint64), ("bytes_h2d", c_uint64), ("bytes_d2h", c_uint64),
+                ("n_copies_h2d", c_uint64), ("n_copies_d2h", c_uint64),
+                ("flops", c_double), ("t_flop_s", c_double), ("t_link_s", c_double), ("t_model_s", c_double)]
+
+    def asdict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class Stats(ctypes.Structure):
+    _fields_ = [("plan", Plan), ("bytes_h2d", c_uint64), ("bytes_d2h", c_uint64), ("n_kernels", c_uint64),
+                ("n_copies_h2d", c_uint64), ("n_copies_d2h", c_uint64), ("t_total_s", c_double), ("t_enqueue_s", c_double)]
+
+    def asdict(self):
+        d = {k: getattr(self, k) for k, _ in self._fields_ if k != "plan"}
+        d["plan"] = self.plan.asdict()
+        return d
+
+
+OP_DTYPE = np.dtype([("kind", "<i4"), ("stream", "<i4"), ("event", "<i4"), ("buf", "<i4"), ("buf2", "<i4"), ("buf3", "<i4"),
+                     ("r0", "<i8"), ("nr", "<i8"), ("c0", "<i8"), ("nc", "<i8"), ("dev_r0", "<i8"),
+                     ("k0", "<i8"), ("kk", "<i8"), ("step", "<i8"), ("beta", "<f8")], align=True)
+
+
+class HclError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = lib().hclooc_strerror(status).decode()
+        extra = f", cuda error {lib().hclooc_last_cuda_error()}" if status == 3 else ""
+        super().__init__(f"{where}: status {status} ({msg}{extra})")
+
+
+_lib = None
+
+
+def lib():
+    """Load (building first if stale) libhclooc_b200.so.  Raises if that is impossible."""
+    global _lib
+    if _lib is None:
+        L = ctypes.CDLL(_build.build())
+        i64, dbl, vp, sz = c_int64, c_double, c_void_p, c_size_t
+        L.hclooc_plan.argtypes = [i64, i64, i64, c_int, c_int, sz, POINTER(Plan)]
+        L.hclMatrixPartitioner.argtypes = [i64, i64, i64, i64, POINTER(i64), POINTER(i64)]
+        L.hclooc_schedule.argtypes = [POINTER(Plan), c_int, vp, sz, POINTER(sz)]
+        L.hclooc_ctx_create.argtypes = [POINTER(vp), c_int, vp, sz, vp, vp, POINTER(vp), c_int]
+        L.hclooc_ctx_destroy.argtypes = [vp]
+        L.hclooc_dgemm.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz]
+        L.hclooc_dgemm_ex.argtypes = [vp, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
+        L.hclMalloc.argtypes = [POINTER(vp), sz]
+        L.hclFree.argtypes = [vp]
+        L.hclGetMemSize.argtypes = [c_int, POINTER(sz)]
+        L.hclStreamCreate.argtypes = [POINTER(vp)]
+        L.hclStreamDestroy.argtypes = [vp]
+        L.hclEventDestroy.argtypes = [vp]
+        L.hclMemcpy.argtypes = [vp, vp, sz, c_int]
+        L.hclMemcpyAsync.argtypes = [vp, vp, sz, c_int, vp, POINTER(vp)]
+        L.hclMemcpy2DAsync.argtypes = [vp, sz, vp, sz, sz, sz, c_int, vp, POINTER(vp)]
+        L.hclDgemmAsync.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, vp, POINTER(vp)]
+        L.hclWaitEvent.argtypes = [vp, vp]
+        L.hclStreamSynchronize.argtypes = [vp]
+        L.hclDeviceSynchronize.argtypes = [c_int]
+        L.hclooc_host_alloc.argtypes = [sz]
+        L.hclooc_host_alloc.restype = vp
+        L.hclooc_host_free.argtypes = [vp]
+        L.hclooc_host_register.argtypes = [vp, sz]
+        L.hclooc_host_unregister.argtypes = [vp]
+        L.hclooc_strerror.argtypes = [c_int]
+        L.hclooc_strerror.restype = c_char_p
+        L.hclooc_last_cuda_error.argtypes = []
+        L.hclooc_version.restype = c_char_p
+        for name in EXPORTS:
+            if name not in ("hclooc_host_alloc", "hclooc_strerror", "hclooc_version"):
+                getattr(L, name).restype = c_int
+        _lib = L
+    return _lib
+
+
+def _ptr(x) -> int | None:
+    """Address of a host/device buffer: int, None, numpy array, torch tensor or HostMatrix."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if isinstance(x, HostMatrix):
+        return x.ptr
+    if isinstance(x, np.ndarray):
+        return x.ctypes.data
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    if hasattr(x, "cuda_stream"):      # torch.cuda.Stream
+        return x.cuda_stream
+    raise TypeError(type(x))
+
+
+def _check(status: int, where: str) -> None:
+    if status != 0:
+        raise HclError(status, where)
+
+
+# ------------------------------------------------------------------ pinned host memory
+def hclooc_host_alloc(nbytes: int) -> int:
+    p = lib().hclooc_host_alloc(nbytes)
+    if not p:
+        raise HclError(4, "hclooc_host_alloc")
+    return p
+
+
+def hclooc_host_free(p) -> None:
+    _check(lib().hclooc_host_free(_ptr(p)), "hclooc_host_free")
+
+
+def hclooc_host_register(p, nbytes: int) -> None:
+    _check(lib().hclooc_host_register(_ptr(p), nbytes), "hclooc_host_register")
+
+
+def hclooc_host_unregister(p) -> None:
+    _check(lib().hclooc_host_unregister(_ptr(p)), "hclooc_host_unregister")
+
+
+class HostMatrix:
+    """A rows x cols FP64 row-major matrix in pinned host memory (leading dimension ld >= cols),
+    allocated with hclooc_host_alloc; `.array` is a numpy view of the whole rows x ld buffer and
+    `.view` of the logical rows x cols part."""
+
+    def __init__(self, rows: int, cols: int, ld: int | None = None):
+        self.rows, self.cols, self.ld = rows, cols, (cols if ld is None else ld)
+        assert self.ld >= cols
+        self.nbytes = max(1, rows * self.ld) * 8
+        self.ptr = hclooc_host_alloc(self.nbytes)
+        buf = (ctypes.c_double * max(1, rows * self.ld)).from_address(self.ptr)
+        self.array = np.frombuffer(buf, dtype=np.float64)[: rows * self.ld].reshape(rows, self.ld)
+        self.view = self.array[:, :cols]
+
+    def free(self):
+        if self.ptr:
+            self.array = self.view = None
+            hclooc_host_free(self.ptr)
+            self.ptr = 0
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+
+# ------------------------------------------------------------------ planner / schedule
+def hclooc_plan(M, N, K, beta_nonzero, alpha_zero, device_budget_bytes) -> Plan:
+    p = Plan()
+    _check(lib().hclooc_plan(M, N, K, int(bool(beta_nonzero)), int(bool(alpha_zero)), device_budget_bytes, byref(p)), "hclooc_plan")
+    return p
+
+
+def hclMatrixPartitioner(M, N, K, budget_elements):
+    h, w = c_int64(), c_int64()
+    _check(lib().hclMatrixPartitioner(M, N, K, budget_elements, byref(h), byref(w)), "hclMatrixPartitioner")
+    return h.value, w.value
+
+
+def hclooc_schedule(plan: Plan, n_compute: int = 8) -> np.ndarray:
+    n = c_size_t()
+    _check(lib().hclooc_schedule(byref(plan), n_compute, None, 0, byref(n)), "hclooc_schedule")
+    ops = np.zeros(n.value, dtype=OP_DTYPE)
+    assert OP_DTYPE.itemsize == 96
+    _check(lib().hclooc_schedule(byref(plan), n_compute, ops.ctypes.data if n.value else None, n.value, byref(n)), "hclooc_schedule")
+    return ops
+
+
+# ------------------------------------------------------------------ context and the operation
+def hclooc_ctx_create(device=0, d_workspace=None, workspace_bytes=0, stream_h2d=None, stream_d2h=None, compute_streams=None) -> int:
+    ctx = c_void_p()
+    n = len(compute_streams) if compute_streams else 0
+    arr = (c_void_p * n)(*[_ptr(s) for s in compute_streams]) if n else None
+    _check(lib().hclooc_ctx_create(byref(ctx), device, _ptr(d_workspace), workspace_bytes, _ptr(stream_h2d),
+                                   _ptr(stream_d2h), arr, n), "hclooc_ctx_create")
+    return ctx.value
+
+
+def hclooc_ctx_destroy(ctx) -> None:
+    _check(lib().hclooc_ctx_destroy(ctx), "hclooc_ctx_destroy")
+
+
+def hclooc_dgemm(M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes) -> None:
+    _check(lib().hclooc_dgemm(M, N, K, alpha, _ptr(A), lda, _ptr(B), ldb, beta, _ptr(C), ldc, device_budget_bytes), "hclooc_dgemm")
+
+
+def hclooc_dgemm_ex(ctx, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes, want_stats=True):
+    st = Stats()
+    _check(lib().hclooc_dgemm_ex(ctx, M, N, K, alpha, _ptr(A), lda, _ptr(B), ldb, beta, _ptr(C), ldc,
+                                 device_budget_bytes, byref(st) if want_stats else None), "hclooc_dgemm_ex")
+    return st if want_stats else None
+
+
+# ------------------------------------------------------------------ the runtime the paper abstracts
+def hclMalloc(nbytes: int) -> int:
+    p = c_void_p()
+    _check(lib().hclMalloc(byref(p), nbytes), "hclMalloc")
+    return p.value or 0
+
+
+def hclFree(dptr) -> None:
+    _check(lib().hclFree(_ptr(dptr)), "hclFree")
+
+
+def hclGetMemSize(device: int = 0) -> int:
+    n = c_size_t()
+    _check(lib().hclGetMemSize(device, byref(n)), "hclGetMemSize")
+    return n.value
+
+
+def hclStreamCreate() -> int:
+    s = c_void_p()
+    _check(lib().hclStreamCreate(byref(s)), "hclStreamCreate")
+    return s.value
+
+
+def hclStreamDestroy(s) -> None:
+    _check(lib().hclStreamDestroy(_ptr(s)), "hclStreamDestroy")
+
+
+def hclEventDestroy(e) -> None:
+    _check(lib().hclEventDestroy(e), "hclEventDestroy")
+
+
+def hclMemcpy(dst, src, nbytes, direction) -> None:
+    _check(lib().hclMemcpy(_ptr(dst), _ptr(src), nbytes, direction), "hclMemcpy")
+
+
+def _ev(want_event, event):
+    if event is not None:
+        return c_void_p(event)
+    return c_void_p() if want_event else None
+
+
+def hclMemcpyAsync(dst, src, nbytes, direction, stream, want_event=False, event=None):
+    """Returns the event handle (int) tied to this call when want_event or event is given, else None."""
+    ev = _ev(want_event, event)
+    _check(lib().hclMemcpyAsync(_ptr(dst), _ptr(src), nbytes, direction, _ptr(stream), byref(ev) if ev is not None else None), "hclMemcpyAsync")
+    return ev.value if ev is not None else None
+
+
+def hclMemcpy2DAsync(dst, dpitch, src, spitch, width_bytes, rows, direction, stream, want_event=False, event=None):
+    ev = _ev(want_event, event)
+    _check(lib().hclMemcpy2DAsync(_ptr(dst), dpitch, _ptr(src), spitch, width_bytes, rows, direction, _ptr(stream),
+                                  byref(ev) if ev is not None else None), "hclMemcpy2DAsync")
+    return ev.value if ev is not None else None
+
+
+def hclDgemmAsync(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, stream=None, want_event=False, event=None):
+    ev = _ev(want_event, event)
+    _check(lib().hclDgemmAsync(M, N, K, alpha, _ptr(dA), lda, _ptr(dB), ldb, beta, _ptr(dC), ldc, _ptr(stream),
+                               byref(ev) if ev is not None else None), "hclDgemmAsync")
+    return ev.value if ev is not None else None
+
+
+def hclWaitEvent(stream, event) -> None:
+    _check(lib().hclWaitEvent(_ptr(stream), event), "hclWaitEvent")
+
+
+def hclStreamSynchronize(stream=None) -> None:
+    _check(lib().hclStreamSynchronize(_ptr(stream)), "hclStreamSynchronize")
+
+
+def hclDeviceSynchronize(device: int = 0) -> None:
+    _check(lib().hclDeviceSynchronize(device), "hclDeviceSynchronize")
+
+
+def hclooc_strerror(status: int) -> str:
+    return lib().hclooc_strerror(status).decode()
+
+
+def hclooc_last_cuda_error() -> int:
+    return lib().hclooc_last_cuda_error()
+
+
+def hclooc_version() -> str:
+    return lib().hclooc_version().decode()

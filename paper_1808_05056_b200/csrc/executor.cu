@@ -1,0 +1,395 @@
+// executor.cu -- S0 (validate), S2-S4/S6 (copies), S7 (events) of the hot path, and the context.
+//
+// The pipeline of PAPER.md:303-313 (five stages S(b_j), S(a_i), S(c_ij), DGEMM, R(c_ij)) on three
+// role streams -- one host-to-device copy stream, one device-to-host copy stream, several compute
+// streams -- ordered by CUDA events.  The paper's Figure 2 (:182-271) uses two round-robin streams,
+// double-buffered A/C and a single B buffer; here a schedule is generated from the plan as an
+// explicit operation list (hclooc_schedule) and then issued verbatim, so the hazard rule of :311
+// ("data stored in device buffers is not overwritten until kernel executions that operate on the
+// data have completed") can be checked on the list itself without a GPU.
+#include <chrono>
+#include <cstring>
+#include <mutex>
+#include <vector>
+#include "internal.h"
+
+namespace hclooc {
+
+static thread_local int g_last_cuda_error = 0;
+void set_last_cuda_error(int e) { g_last_cuda_error = e; }
+
+namespace {
+
+constexpr int DEFAULT_COMPUTE_STREAMS = 8;
+constexpr int MAX_COMPUTE_STREAMS = 16;
+
+// event ids inside a schedule
+struct EventIds {
+    int n_sets, n_bbuf;
+    int set_ready(int s) const { return s; }                 // rA/rC: A slice (and C block) of set s received
+    int kernel_done(int s) const { return n_sets + s; }      // eA: kernel that used set s finished
+    int c_stored(int s) const { return 2 * n_sets + s; }     // eC: C block of set s is back on the host
+    int b_ready(int b) const { return 3 * n_sets + b; }      // rB: B slice b received
+    int count() const { return 3 * n_sets + n_bbuf; }
+};
+
+int64_t chunks_for(int64_t h, int64_t kk) { return std::max<int64_t>(1, std::min(h, kk)); }
+
+// Expand the plan into the operation list.  This is the single source of truth for the executor.
+void build_schedule(const hclooc_plan_t& P, int ncs, std::vector<hclooc_op_t>& ops) {
+    ops.clear();
+    if (P.n_steps == 0) return;
+    const EventIds ev{P.n_sets, P.n_bbuf};
+    const bool scale_only = P.scale_only != 0;
+    std::vector<char> set_used(P.n_sets, 0), set_stored(P.n_sets, 0);
+    auto push = [&](int kind, int stream, int event) -> hclooc_op_t& {
+        hclooc_op_t o;
+        std::memset(&o, 0, sizeof(o));
+        o.kind = kind; o.stream = stream; o.event = event; o.buf = o.buf2 = o.buf3 = -1; o.step = -1;
+        ops.push_back(o);
+        return ops.back();
+    };
+    auto bbuf_id = [&](int b) { return 2 * P.n_sets + b; };
+    // wait until every kernel issued so far has finished (latest record of each set's kernel_done)
+    auto wait_all_kernels = [&](int stream) {
+        for (int s = 0; s < P.n_sets; ++s)
+            if (set_used[s]) push(HCLOOC_OP_WAIT, stream, ev.kernel_done(s));
+    };
+    auto load_b = [&](int64_t p, int64_t j, int b, int64_t kr0, int64_t krows) {
+        hclooc_op_t& o = push(HCLOOC_OP_H2D_B, 0, -1);
+        o.buf = bbuf_id(b);
+        o.r0 = p * P.kb + kr0; o.nr = krows;
+        o.c0 = j * P.nb; o.nc = std::min(P.nb, P.N - j * P.nb);
+        o.dev_r0 = kr0;
+    };
+    const int64_t slabs = P.w * P.kpanels;
+    int64_t step = 0;
+    for (int64_t sl = 0; sl < slabs; ++sl) {
+        const int64_t p = sl / P.w, j = sl % P.w;
+        const int64_t k0 = p * P.kb, kk = scale_only ? 0 : std::min(P.kb, P.K - k0);
+        const int64_t j0 = j * P.nb, nj = std::min(P.nb, P.N - j0);
+        const int b = (int)(sl % P.n_bbuf);
+        const bool cload = P.beta_nonzero || p > 0;
+        const double beta_flag = (p > 0) ? 1.0 : -1.0;   // -1: "use the caller's beta" (resolved by the executor)
+        if (!scale_only && (P.n_bbuf == 1 || sl == 0)) {
+            // S(b_j): whole slice; with a single buffer every kernel of the previous column must be done (:236-242)
+            if (sl > 0) wait_all_kernels(0);
+            load_b(p, j, b, 0, kk);
+            push(HCLOOC_OP_RECORD, 0, ev.b_ready(b));
+        }
+        // next slice (prefetched in chunks during this column when there are two B buffers)
+        const bool prefetch = !scale_only && P.n_bbuf == 2 && sl + 1 < slabs;
+        const int64_t np = (sl + 1) / P.w, nj_idx = (sl + 1) % P.w;
+        const int64_t nkk = prefetch ? std::min(P.kb, P.K - np * P.kb) : 0;
+        const int64_t nchunks = prefetch ? chunks_for(P.h, nkk) : 0;
+        for (int64_t i = 0; i < P.h; ++i, ++step) {
+            const int set = (int)(step % P.n_sets);
+            const int cs = 2 + (int)(step % ncs);
+            const int64_t i0 = i * P.mb, mi = std::min(P.mb, P.M - i0);
+            // ---- uploads for this step on the H2D stream
+            if (!scale_only) {
+                if (set_used[set]) push(HCLOOC_OP_WAIT, 0, ev.kernel_done(set));     // Wait(eA): buffer free
+                hclooc_op_t& o = push(HCLOOC_OP_H2D_A, 0, -1);                       // S(a_i)
+                o.buf = set; o.r0 = i0; o.nr = mi; o.c0 = k0; o.nc = kk; o.step = step;
+            }
+            if (cload) {
+                if (set_stored[set]) push(HCLOOC_OP_WAIT, 0, ev.c_stored(set));      // Wait(eC): block is back on the host
+                hclooc_op_t& o = push(HCLOOC_OP_H2D_C, 0, -1);                       // S(c_ij)
+                o.buf = P.n_sets + set; o.r0 = i0; o.nr = mi; o.c0 = j0; o.nc = nj; o.step = step;
+            }
+            if (!scale_only || cload) push(HCLOOC_OP_RECORD, 0, ev.set_ready(set));  // Rec(rA), Rec(rC)
+            // ---- one chunk of the next B slice, interleaved with the uploads
+            if (prefetch && i < nchunks) {
+                if (i == 0) wait_all_kernels(0);   // the other B buffer was last read by the previous column's kernels
+                const int64_t r_lo = nkk * i / nchunks, r_hi = nkk * (i + 1) / nchunks;
+                load_b(np, nj_idx, (int)((sl + 1) % P.n_bbuf), r_lo, r_hi - r_lo);
+                if (i == nchunks - 1) push(HCLOOC_OP_RECORD, 0, ev.b_ready((int)((sl + 1) % P.n_bbuf)));
+            }
+            // ---- DGEMM on a compute stream
+            if (!scale_only || cload) push(HCLOOC_OP_WAIT, cs, ev.set_ready(set));   // Wait(rA), Wait(rC)
+            if (!scale_only) push(HCLOOC_OP_WAIT, cs, ev.b_ready(b));                // Wait(rB)
+            if (!cload && set_stored[set]) push(HCLOOC_OP_WAIT, cs, ev.c_stored(set));  // C buffer still draining
+            {
+                hclooc_op_t& o = push(HCLOOC_OP_GEMM, cs, -1);
+                o.buf = scale_only ? -1 : set; o.buf2 = scale_only ? -1 : bbuf_id(b); o.buf3 = P.n_sets + set;
+                o.r0 = i0; o.nr = mi; o.c0 = j0; o.nc = nj; o.k0 = k0; o.kk = kk; o.step = step; o.beta = beta_flag;
+            }
+            push(HCLOOC_OP_RECORD, cs, ev.kernel_done(set));                          // Rec(eA)
+            set_used[set] = 1;
+            // ---- download on the D2H stream
+            push(HCLOOC_OP_WAIT, 1, ev.kernel_done(set));
+            {
+                hclooc_op_t& o = push(HCLOOC_OP_D2H_C, 1, -1);                        // R(c_ij)
+                o.buf = P.n_sets + set; o.r0 = i0; o.nr = mi; o.c0 = j0; o.nc = nj; o.step = step;
+            }
+            push(HCLOOC_OP_RECORD, 1, ev.c_stored(set));                              // Rec(eC)
+            set_stored[set] = 1;
+        }
+    }
+}
+
+}  // namespace
+}  // namespace hclooc
+
+using namespace hclooc;
+
+struct hclooc_ctx {
+    int device = 0;
+    void* workspace = nullptr;
+    size_t workspace_bytes = 0;
+    bool owns_workspace = false;
+    cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
+    bool owns_h2d = false, owns_d2h = false;
+    cudaStream_t s_compute[MAX_COMPUTE_STREAMS] = {};
+    int n_compute = 0;
+    bool owns_compute = false;
+    std::vector<cudaEvent_t> events;
+    std::vector<hclooc_op_t> ops;
+    std::mutex mu;
+};
+
+extern "C" int hclooc_schedule(const hclooc_plan_t* plan, int n_compute, hclooc_op_t* ops, size_t max_ops, size_t* n_ops) {
+    if (!plan) return -1;
+    if (n_compute < 1 || n_compute > MAX_COMPUTE_STREAMS) return -2;
+    if (!n_ops) return -5;
+    std::vector<hclooc_op_t> v;
+    build_schedule(*plan, n_compute, v);
+    *n_ops = v.size();
+    if (ops) std::memcpy(ops, v.data(), std::min(max_ops, v.size()) * sizeof(hclooc_op_t));
+    return HCLOOC_OK;
+}
+
+extern "C" int hclooc_ctx_create(hclooc_ctx** out, int device, void* d_workspace, size_t workspace_bytes,
+                                 hclStream stream_h2d, hclStream stream_d2h, hclStream* compute_streams, int n_compute) {
+    if (!out) return -1;
+    if (device < 0) return -2;
+    if ((d_workspace == nullptr) != (workspace_bytes == 0)) return -4;
+    if (n_compute < 0 || n_compute > MAX_COMPUTE_STREAMS || ((compute_streams == nullptr) != (n_compute == 0))) return -8;
+    HCL_CUDA(cudaSetDevice(device));
+    hclooc_ctx* c = new (std::nothrow) hclooc_ctx();
+    if (!c) return HCLOOC_ERR_NOMEM;
+    c->device = device;
+    c->workspace = d_workspace;
+    c->workspace_bytes = workspace_bytes;
+    c->owns_workspace = false;
+    auto mk = [](cudaStream_t* s) { return cudaStreamCreateWithFlags(s, cudaStreamNonBlocking); };
+    cudaError_t e = cudaSuccess;
+    if (stream_h2d) c->s_h2d = (cudaStream_t)stream_h2d; else { e = mk(&c->s_h2d); c->owns_h2d = true; }
+    if (e == cudaSuccess) { if (stream_d2h) c->s_d2h = (cudaStream_t)stream_d2h; else { e = mk(&c->s_d2h); c->owns_d2h = true; } }
+    if (e == cudaSuccess) {
+        if (compute_streams) {
+            c->n_compute = n_compute;
+            for (int i = 0; i < n_compute; ++i) c->s_compute[i] = (cudaStream_t)compute_streams[i];
+        } else {
+            c->n_compute = DEFAULT_COMPUTE_STREAMS;
+            c->owns_compute = true;
+            for (int i = 0; i < c->n_compute && e == cudaSuccess; ++i) e = mk(&c->s_compute[i]);
+        }
+    }
+    if (e != cudaSuccess) { hclooc_ctx_destroy(c); return cuda_fail(e); }
+    *out = c;
+    return HCLOOC_OK;
+}
+
+extern "C" int hclooc_ctx_destroy(hclooc_ctx* c) {
+    if (!c) return HCLOOC_OK;
+    cudaSetDevice(c->device);
+    cudaDeviceSynchronize();
+    for (cudaEvent_t e : c->events) cudaEventDestroy(e);
+    if (c->owns_h2d && c->s_h2d) cudaStreamDestroy(c->s_h2d);
+    if (c->owns_d2h && c->s_d2h) cudaStreamDestroy(c->s_d2h);
+    if (c->owns_compute) for (int i = 0; i < c->n_compute; ++i) if (c->s_compute[i]) cudaStreamDestroy(c->s_compute[i]);
+    if (c->owns_workspace && c->workspace) cudaFree(c->workspace);
+    delete c;
+    return HCLOOC_OK;
+}
+
+namespace {
+
+hclooc_ctx* g_default_ctx = nullptr;
+std::mutex g_default_mu;
+
+int default_ctx(hclooc_ctx** out) {
+    std::lock_guard<std::mutex> lk(g_default_mu);
+    if (!g_default_ctx) {
+        int dev = 0;
+        HCL_CUDA(cudaGetDevice(&dev));
+        int rc = hclooc_ctx_create(&g_default_ctx, dev, nullptr, 0, nullptr, nullptr, nullptr, 0);
+        if (rc) return rc;
+    }
+    *out = g_default_ctx;
+    return HCLOOC_OK;
+}
+
+// 0 = ok, HCLOOC_ERR_NOT_PINNED if pageable host memory
+int check_resident(const void* p) {
+    cudaPointerAttributes at;
+    cudaError_t e = cudaPointerGetAttributes(&at, p);
+    if (e != cudaSuccess) { cudaGetLastError(); return HCLOOC_ERR_NOT_PINNED; }
+    if (at.type == cudaMemoryTypeUnregistered) return HCLOOC_ERR_NOT_PINNED;
+    return HCLOOC_OK;
+}
+
+bool overlaps(const double* a, int64_t rows_a, int64_t cols_a, int64_t lda, const double* b, int64_t rows_b, int64_t cols_b, int64_t ldb) {
+    if (rows_a == 0 || cols_a == 0 || rows_b == 0 || cols_b == 0) return false;
+    const uintptr_t a0 = (uintptr_t)a, a1 = a0 + 8 * (uintptr_t)((rows_a - 1) * lda + cols_a);
+    const uintptr_t b0 = (uintptr_t)b, b1 = b0 + 8 * (uintptr_t)((rows_b - 1) * ldb + cols_b);
+    return a0 < b1 && b0 < a1;
+}
+
+int copy2d(void* dst, size_t dpitch, const void* src, size_t spitch, size_t width, size_t rows, cudaStream_t s) {
+    if (width == 0 || rows == 0) return HCLOOC_OK;
+    if (dpitch == width && spitch == width) HCL_CUDA(cudaMemcpyAsync(dst, src, width * rows, cudaMemcpyDefault, s));
+    else HCL_CUDA(cudaMemcpy2DAsync(dst, dpitch, src, spitch, width, rows, cudaMemcpyDefault, s));
+    return HCLOOC_OK;
+}
+
+}  // namespace
+
+extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
+                               int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
+                               size_t device_budget_bytes, hclooc_stats* stats) {
+    const auto t_begin = std::chrono::steady_clock::now();
+    // ---------------------------------------------------------------- S0 validate (argument numbers of hclooc_dgemm)
+    if (M < 0) return -1;
+    if (N < 0) return -2;
+    if (K < 0) return -3;
+    if (stats) std::memset(stats, 0, sizeof(*stats));
+    if (M == 0 || N == 0) return HCLOOC_OK;
+    const bool scale_only = (alpha == 0.0 || K == 0);
+    if (!scale_only) {
+        if (!A) return -5;
+        if (lda < K) return -6;
+        if (!B) return -7;
+        if (ldb < N) return -8;
+    }
+    if (!C) return -10;
+    if (ldc < N) return -11;
+    if (!scale_only && (overlaps(C, M, N, ldc, A, M, K, lda) || overlaps(C, M, N, ldc, B, K, N, ldb))) return -10;
+    if (scale_only && beta == 1.0) return HCLOOC_OK;            // C = 1*C
+    int rc;
+    if (!ctx && (rc = default_ctx(&ctx))) return rc;
+    std::lock_guard<std::mutex> lk(ctx->mu);
+    HCL_CUDA(cudaSetDevice(ctx->device));
+    if ((rc = check_resident(C))) return rc;
+    if (!scale_only && ((rc = check_resident(A)) || (rc = check_resident(B)))) return rc;
+
+    // ---------------------------------------------------------------- S1 plan
+    size_t budget = device_budget_bytes;
+    if (!ctx->owns_workspace && ctx->workspace) {
+        budget = (budget == 0) ? ctx->workspace_bytes : std::min(budget, ctx->workspace_bytes);
+    } else if (budget == 0) {
+        size_t fr = 0, tot = 0;
+        HCL_CUDA(cudaMemGetInfo(&fr, &tot));
+        fr += ctx->workspace_bytes;                                // what we already hold counts as free
+        const size_t margin = (size_t)1 << 30;
+        budget = fr > 2 * margin ? fr - margin : fr / 2;
+    }
+    hclooc_plan_t P;
+    rc = hclooc_plan(M, N, K, beta != 0.0, alpha == 0.0, budget, &P);
+    if (rc) return rc;
+    if (P.workspace_bytes > ctx->workspace_bytes) {
+        if (ctx->workspace && !ctx->owns_workspace) return HCLOOC_ERR_BUDGET;
+        if (ctx->workspace) { HCL_CUDA(cudaDeviceSynchronize()); cudaFree(ctx->workspace); ctx->workspace = nullptr; ctx->workspace_bytes = 0; }
+        void* p = nullptr;
+        cudaError_t e = cudaMalloc(&p, P.workspace_bytes);
+        if (e != cudaSuccess) { set_last_cuda_error((int)e); cudaGetLastError(); return HCLOOC_ERR_NOMEM; }
+        ctx->workspace = p; ctx->workspace_bytes = P.workspace_bytes; ctx->owns_workspace = true;
+    }
+    // ---------------------------------------------------------------- buffers carved from the workspace
+    uint8_t* base = (uint8_t*)ctx->workspace;
+    const uintptr_t mis = (uintptr_t)base & 1023u;
+    if (mis) {   // caller workspace not 1 KiB aligned: shift (costs < 1 KiB, checked against the size)
+        base += 1024 - mis;
+        if (P.workspace_bytes + 1024 - mis > ctx->workspace_bytes) return HCLOOC_ERR_BUDGET;
+    }
+    std::vector<double*> bufs(2 * P.n_sets + P.n_bbuf);
+    {
+        uint8_t* q = base;
+        for (int b = 0; b < P.n_bbuf; ++b) { bufs[2 * P.n_sets + b] = (double*)q; q += P.bytes_b_buf; }
+        for (int s = 0; s < P.n_sets; ++s) {
+            bufs[s] = (double*)q; q += P.bytes_a_buf;
+            bufs[P.n_sets + s] = (double*)q; q += P.bytes_c_buf;
+        }
+        if ((size_t)(q - base) != P.workspace_bytes) return HCLOOC_ERR_INTERNAL;
+    }
+    // ---------------------------------------------------------------- events
+    const size_t n_events = 3 * (size_t)P.n_sets + P.n_bbuf;
+    while (ctx->events.size() < n_events) {
+        cudaEvent_t e;
+        HCL_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        ctx->events.push_back(e);
+    }
+    // ---------------------------------------------------------------- S2-S7: issue the schedule
+    build_schedule(P, ctx->n_compute, ctx->ops);
+    auto stream_of = [&](int s) { return s == 0 ? ctx->s_h2d : (s == 1 ? ctx->s_d2h : ctx->s_compute[s - 2]); };
+    uint64_t bytes_h2d = 0, bytes_d2h = 0, n_h2d = 0, n_d2h = 0, n_kernels = 0;
+    const auto t_enq0 = std::chrono::steady_clock::now();
+    rc = HCLOOC_OK;
+    for (const hclooc_op_t& o : ctx->ops) {
+        cudaStream_t st = stream_of(o.stream);
+        switch (o.kind) {
+            case HCLOOC_OP_WAIT: {
+                cudaError_t e = cudaStreamWaitEvent(st, ctx->events[o.event], 0);
+                if (e != cudaSuccess) rc = cuda_fail(e);
+                break;
+            }
+            case HCLOOC_OP_RECORD: {
+                cudaError_t e = cudaEventRecord(ctx->events[o.event], st);
+                if (e != cudaSuccess) rc = cuda_fail(e);
+                break;
+            }
+            case HCLOOC_OP_H2D_A:
+                rc = copy2d(bufs[o.buf], (size_t)P.lda_dev * 8, A + o.r0 * lda + o.c0, (size_t)lda * 8, (size_t)o.nc * 8, (size_t)o.nr, st);
+                bytes_h2d += (uint64_t)o.nr * o.nc * 8; ++n_h2d;
+                break;
+            case HCLOOC_OP_H2D_B:
+                rc = copy2d(bufs[o.buf] + o.dev_r0 * P.ldb_dev, (size_t)P.ldb_dev * 8, B + o.r0 * ldb + o.c0, (size_t)ldb * 8, (size_t)o.nc * 8, (size_t)o.nr, st);
+                bytes_h2d += (uint64_t)o.nr * o.nc * 8; ++n_h2d;
+                break;
+            case HCLOOC_OP_H2D_C:
+                rc = copy2d(bufs[o.buf], (size_t)P.ldc_dev * 8, C + o.r0 * ldc + o.c0, (size_t)ldc * 8, (size_t)o.nc * 8, (size_t)o.nr, st);
+                bytes_h2d += (uint64_t)o.nr * o.nc * 8; ++n_h2d;
+                break;
+            case HCLOOC_OP_D2H_C:
+                rc = copy2d(C + o.r0 * ldc + o.c0, (size_t)ldc * 8, bufs[o.buf], (size_t)P.ldc_dev * 8, (size_t)o.nc * 8, (size_t)o.nr, st);
+                bytes_d2h += (uint64_t)o.nr * o.nc * 8; ++n_d2h;
+                break;
+            case HCLOOC_OP_GEMM: {
+                const double b_eff = (o.beta < 0.0) ? beta : o.beta;
+                rc = launch_dgemm_tiles(o.nr, o.nc, o.kk, scale_only ? 0.0 : alpha, o.buf >= 0 ? bufs[o.buf] : nullptr, P.lda_dev,
+                                        o.buf2 >= 0 ? bufs[o.buf2] : nullptr, P.ldb_dev, b_eff, bufs[o.buf3], P.ldc_dev, st);
+                ++n_kernels;
+                break;
+            }
+            default: rc = HCLOOC_ERR_INTERNAL;
+        }
+        if (rc) break;
+    }
+    const auto t_enq1 = std::chrono::steady_clock::now();
+    // ---------------------------------------------------------------- final synchronisation (:268-269)
+    cudaError_t e1 = cudaStreamSynchronize(ctx->s_d2h);
+    cudaError_t e2 = cudaStreamSynchronize(ctx->s_h2d);
+    cudaError_t e3 = cudaSuccess;
+    for (int i = 0; i < ctx->n_compute && e3 == cudaSuccess; ++i) e3 = cudaStreamSynchronize(ctx->s_compute[i]);
+    if (rc) return rc;
+    if (e1 != cudaSuccess) return cuda_fail(e1);
+    if (e2 != cudaSuccess) return cuda_fail(e2);
+    if (e3 != cudaSuccess) return cuda_fail(e3);
+    if (bytes_h2d != P.bytes_h2d || bytes_d2h != P.bytes_d2h || n_h2d != P.n_copies_h2d || n_d2h != P.n_copies_d2h) return HCLOOC_ERR_INTERNAL;
+    if (stats) {
+        stats->plan = P;
+        stats->bytes_h2d = bytes_h2d; stats->bytes_d2h = bytes_d2h;
+        stats->n_kernels = n_kernels; stats->n_copies_h2d = n_h2d; stats->n_copies_d2h = n_d2h;
+        stats->t_enqueue_s = std::chrono::duration<double>(t_enq1 - t_enq0).count();
+        stats->t_total_s = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_begin).count();
+    }
+    return HCLOOC_OK;
+}
+
+extern "C" int hclooc_dgemm(int64_t M, int64_t N, int64_t K, double alpha, const double* A, int64_t lda,
+                            const double* B, int64_t ldb, double beta, double* C, int64_t ldc, size_t device_budget_bytes) {
+    return hclooc_dgemm_ex(nullptr, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes, nullptr);
+}
+
+extern "C" int hclooc_last_cuda_error(void) { return g_last_cuda_error; }

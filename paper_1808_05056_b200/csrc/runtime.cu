@@ -1,0 +1,178 @@
+// runtime.cu -- the uniform runtime the paper abstracts, CUDA only,
+// as plain C functions: no factory, no virtual dispatch (the paper attributes part of its 4-10 %
+// overhead to the virtual-table lookups, :164).
+#include <cstring>
+#include "internal.h"
+
+using namespace hclooc;
+
+namespace {
+int finish_async(cudaStream_t s, hclEvent* ev) {
+    if (!ev) return HCLOOC_OK;
+    if (*ev == nullptr) {   // "an uninitialised hclEvent ... will create and initialise the event" (:146)
+        cudaEvent_t e;
+        HCL_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        *ev = (hclEvent)e;
+    }
+    HCL_CUDA(cudaEventRecord((cudaEvent_t)*ev, s));
+    return HCLOOC_OK;
+}
+cudaMemcpyKind kind_of(int dir) { return dir == HCL_H2D ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToHost; }
+}  // namespace
+
+extern "C" {
+
+int hclMalloc(void** dptr, size_t bytes) {
+    if (!dptr) return -1;
+    *dptr = nullptr;
+    if (bytes == 0) return HCLOOC_OK;
+    cudaError_t e = cudaMalloc(dptr, bytes);
+    if (e == cudaErrorMemoryAllocation) { set_last_cuda_error((int)e); cudaGetLastError(); return HCLOOC_ERR_NOMEM; }
+    if (e != cudaSuccess) return cuda_fail(e);
+    return HCLOOC_OK;
+}
+int hclFree(void* dptr) {
+    if (!dptr) return HCLOOC_OK;
+    HCL_CUDA(cudaFree(dptr));
+    return HCLOOC_OK;
+}
+int hclGetMemSize(int device, size_t* free_bytes) {
+    if (device < 0) return -1;
+    if (!free_bytes) return -2;
+    int cur = 0;
+    HCL_CUDA(cudaGetDevice(&cur));
+    if (cur != device) HCL_CUDA(cudaSetDevice(device));
+    size_t fr = 0, tot = 0;
+    cudaError_t e = cudaMemGetInfo(&fr, &tot);
+    if (cur != device) cudaSetDevice(cur);
+    if (e != cudaSuccess) return cuda_fail(e);
+    *free_bytes = fr;
+    return HCLOOC_OK;
+}
+int hclStreamCreate(hclStream* s) {
+    if (!s) return -1;
+    cudaStream_t st;
+    HCL_CUDA(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
+    *s = (hclStream)st;
+    return HCLOOC_OK;
+}
+int hclStreamDestroy(hclStream s) {
+    if (!s) return HCLOOC_OK;
+    HCL_CUDA(cudaStreamDestroy((cudaStream_t)s));
+    return HCLOOC_OK;
+}
+int hclEventDestroy(hclEvent e) {
+    if (!e) return HCLOOC_OK;
+    HCL_CUDA(cudaEventDestroy((cudaEvent_t)e));
+    return HCLOOC_OK;
+}
+int hclMemcpy(void* dst, const void* src, size_t bytes, int dir) {
+    if (bytes == 0) return HCLOOC_OK;
+    if (!dst) return -1;
+    if (!src) return -2;
+    if (dir != HCL_H2D && dir != HCL_D2H) return -4;
+    HCL_CUDA(cudaMemcpy(dst, src, bytes, kind_of(dir)));
+    return HCLOOC_OK;
+}
+int hclMemcpyAsync(void* dst, const void* src, size_t bytes, int dir, hclStream s, hclEvent* ev) {
+    if (bytes != 0) {
+        if (!dst) return -1;
+        if (!src) return -2;
+        if (dir != HCL_H2D && dir != HCL_D2H) return -4;
+        HCL_CUDA(cudaMemcpyAsync(dst, src, bytes, kind_of(dir), (cudaStream_t)s));
+    }
+    return finish_async((cudaStream_t)s, ev);
+}
+int hclMemcpy2DAsync(void* dst, size_t dpitch, const void* src, size_t spitch, size_t width_bytes, size_t rows,
+                     int dir, hclStream s, hclEvent* ev) {
+    if (width_bytes != 0 && rows != 0) {
+        if (!dst) return -1;
+        if (dpitch < width_bytes) return -2;
+        if (!src) return -3;
+        if (spitch < width_bytes) return -4;
+        if (dir != HCL_H2D && dir != HCL_D2H) return -7;
+        HCL_CUDA(cudaMemcpy2DAsync(dst, dpitch, src, spitch, width_bytes, rows, kind_of(dir), (cudaStream_t)s));
+    }
+    return finish_async((cudaStream_t)s, ev);
+}
+int hclDgemmAsync(int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda, const double* dB,
+                  int64_t ldb, double beta, double* dC, int64_t ldc, hclStream s, hclEvent* ev) {
+    if (M < 0) return -1;
+    if (N < 0) return -2;
+    if (K < 0) return -3;
+    const bool noab = (alpha == 0.0 || K == 0);
+    if (M > 0 && N > 0) {
+        if (!noab) {
+            if (!dA) return -5;
+            if (lda < K) return -6;
+            if (!dB) return -7;
+            if (ldb < N) return -8;
+            if (((uintptr_t)dA & 15u) || ((uintptr_t)dB & 15u) || (lda & 1) || (ldb & 1)) return HCLOOC_ERR_ALIGN;
+        }
+        if (!dC) return -10;
+        if (ldc < N) return -11;
+        int rc = launch_dgemm_tiles(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, (cudaStream_t)s);
+        if (rc) return rc;
+    }
+    return finish_async((cudaStream_t)s, ev);
+}
+int hclWaitEvent(hclStream s, hclEvent e) {
+    if (!e) return -2;
+    HCL_CUDA(cudaStreamWaitEvent((cudaStream_t)s, (cudaEvent_t)e, 0));
+    return HCLOOC_OK;
+}
+int hclStreamSynchronize(hclStream s) {
+    HCL_CUDA(cudaStreamSynchronize((cudaStream_t)s));
+    return HCLOOC_OK;
+}
+int hclDeviceSynchronize(int device) {
+    if (device < 0) return -1;
+    int cur = 0;
+    HCL_CUDA(cudaGetDevice(&cur));
+    if (cur != device) HCL_CUDA(cudaSetDevice(device));
+    cudaError_t e = cudaDeviceSynchronize();
+    if (cur != device) cudaSetDevice(cur);
+    if (e != cudaSuccess) return cuda_fail(e);
+    return HCLOOC_OK;
+}
+
+void* hclooc_host_alloc(size_t bytes) {
+    void* p = nullptr;
+    if (bytes == 0) return nullptr;
+    cudaError_t e = cudaHostAlloc(&p, bytes, cudaHostAllocDefault);
+    if (e != cudaSuccess) { set_last_cuda_error((int)e); cudaGetLastError(); return nullptr; }
+    return p;
+}
+int hclooc_host_free(void* p) {
+    if (!p) return HCLOOC_OK;
+    HCL_CUDA(cudaFreeHost(p));
+    return HCLOOC_OK;
+}
+int hclooc_host_register(void* p, size_t bytes) {
+    if (!p) return -1;
+    if (bytes == 0) return -2;
+    HCL_CUDA(cudaHostRegister(p, bytes, cudaHostRegisterDefault));
+    return HCLOOC_OK;
+}
+int hclooc_host_unregister(void* p) {
+    if (!p) return -1;
+    HCL_CUDA(cudaHostUnregister(p));
+    return HCLOOC_OK;
+}
+
+const char* hclooc_strerror(int status) {
+    if (status == HCLOOC_OK) return "success";
+    if (status < 0) return "invalid argument (the value is minus the 1-based argument number)";
+    switch (status) {
+        case HCLOOC_ERR_BUDGET: return "device budget below the minimum working set";
+        case HCLOOC_ERR_NOT_PINNED: return "A, B or C is pageable host memory (pin it: hclooc_host_alloc / hclooc_host_register)";
+        case HCLOOC_ERR_CUDA: return "a CUDA call failed (see hclooc_last_cuda_error)";
+        case HCLOOC_ERR_NOMEM: return "out of device or host memory";
+        case HCLOOC_ERR_ALIGN: return "device operand must be 16-byte aligned with an even leading dimension";
+        case HCLOOC_ERR_INTERNAL: return "internal invariant violated";
+        default: return "unknown status";
+    }
+}
+const char* hclooc_version(void) { return "hclooc-b200 0.1 (sm_100a, DMMA tile kernel)"; }
+
+}  // extern "C"

@@ -1,0 +1,310 @@
+"""GPU parity: the CUDA path (through the C ABI binding) against the CPU oracle, element by element.
+
+Bar (BASELINE.json north_star, G14): bit-exact (by value) on small-integer inputs whose
+products and sums are exact in FP64; |C_gpu - C_ref| <= 1e-13 * D elsewhere, with
+D = |alpha| * sum_k |A_ik||B_kj| + |beta||C0_ij| computed by the oracle.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import synthgen
+
+pytestmark = pytest.mark.gpu
+
+RTOL = 1e-13          # the gate, written out as the task requires
+MiB = 1 << 20
+
+
+@pytest.fixture(scope="module")
+def H():
+    import paper_1808_05056_b200 as H
+    import torch
+    assert torch.cuda.is_available()
+    torch.cuda.init()
+    return H
+
+
+def host_inputs(H, M, N, K, seed, dist, pads=(0, 0, 0), poison_c=False):
+    A = H.HostMatrix(M, K, K + pads[0])
+    B = H.HostMatrix(K, N, N + pads[1])
+    C = H.HostMatrix(M, N, N + pads[2])
+    for X in (A, B, C):
+        X.array[...] = np.nan                        # padding is NaN: reading it would show
+    synthgen.fill(A.array, seed, "A", dist, cols=K)
+    synthgen.fill(B.array, seed, "B", dist, cols=N)
+    if poison_c:
+        C.view[...] = np.nan
+    else:
+        synthgen.fill(C.array, seed, "C", dist, cols=N)
+    return A, B, C
+
+
+def check(C_gpu, C_ref, D, exact):
+    assert not np.isnan(C_gpu).any()
+    if exact:
+        assert np.array_equal(C_gpu, C_ref), f"{np.count_nonzero(C_gpu != C_ref)} elements differ"
+        assert not (np.signbit(C_gpu) != np.signbit(C_ref)).any()       # sign of zero too (G15)
+    else:
+        ok, worst = oracle.within_gate(C_gpu, C_ref, D, RTOL)
+        assert ok, f"worst |err|/D = {worst:.3e} > {RTOL}"
+
+
+# ------------------------------------------------------------------ S5: the tile kernel on device pointers
+@pytest.mark.parametrize("M,N,K,alpha,beta,dist", [
+    (128, 128, 16, 1.0, 0.0, "uniform"),          # exactly one tile, one k step
+    (1, 1, 1, 2.0, 0.5, "uniform"),
+    (300, 260, 200, 1.0, 0.5, "uniform"),         # several tiles, ragged in m, n and k
+    (129, 257, 33, -1.5, 1.0, "normal"),
+    (517, 389, 1000, 2.0, -1.0, "uniform"),
+    (256, 384, 512, 1.0, 0.5, "int"),
+    (131, 77, 97, 3.0, 2.0, "int"),               # primes
+    (64, 1024, 8, 1.0, 0.0, "int"),
+])
+def test_tile_kernel_matches_oracle(H, M, N, K, alpha, beta, dist):
+    import torch
+    lda, ldb, ldc = K + (K % 2) + 4, N + (N % 2) + 2, N + (N % 2) + 6      # even, padded
+    A = np.full((M, lda), np.nan); B = np.full((K, ldb), np.nan); C0 = np.full((M, ldc), np.nan)
+    synthgen.fill(A, 21, "A", dist, cols=K); synthgen.fill(B, 21, "B", dist, cols=N); synthgen.fill(C0, 21, "C", dist, cols=N)
+    if beta == 0.0:
+        C0[:, :N] = np.nan                                                       # must not be read
+    dA, dB, dC = (torch.from_numpy(x).cuda() for x in (A, B, C0))
+    H.hclDgemmAsync(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    got = dC.cpu().numpy()
+    ref = C0[:, :N].copy()
+    D = oracle.dgemm(alpha, A[:, :K], B[:, :N], beta, ref, want_denominator=True)
+    check(got[:, :N], ref, D, exact=(dist == "int"))
+    assert np.isnan(got[:, N:]).all()                                            # padding of C untouched
+
+
+def test_tile_kernel_alpha_zero_and_k_zero(H):
+    import torch
+    M, N = 200, 136
+    C0 = synthgen.fill(np.empty((M, N)), 22, "C", "uniform")
+    nan = torch.full((M, 64), float("nan"), dtype=torch.float64, device="cuda")
+    nanb = torch.full((64, N), float("nan"), dtype=torch.float64, device="cuda")
+    dC = torch.from_numpy(C0).cuda()
+    H.hclDgemmAsync(M, N, 64, 0.0, nan, 64, nanb, N, -2.0, dC, N, torch.cuda.current_stream())    # alpha == 0: A, B not read
+    torch.cuda.synchronize()
+    assert np.array_equal(dC.cpu().numpy(), -2.0 * C0)
+    dC = torch.from_numpy(C0).cuda()
+    H.hclDgemmAsync(M, N, 0, 1.0, None, 2, None, N, 0.5, dC, N, torch.cuda.current_stream())      # K == 0
+    torch.cuda.synchronize()
+    assert np.array_equal(dC.cpu().numpy(), 0.5 * C0)
+    with pytest.raises(H.HclError) as e:
+        H.hclDgemmAsync(M, N, 64, 1.0, nan, 63, nanb, N, 0.0, dC, N, torch.cuda.current_stream())
+    assert e.value.status == -6
+    with pytest.raises(H.HclError) as e:
+        H.hclDgemmAsync(M, N, 63, 1.0, nan, 65, nanb, N, 0.0, dC, N, torch.cuda.current_stream())
+    assert e.value.status == 5                                                                     # odd ld: HCLOOC_ERR_ALIGN
+
+
+# ------------------------------------------------------------------ the whole path: configs[0]
+@pytest.mark.parametrize("dist,exact", [("uniform", False), ("int", True)])
+def test_config1_every_tile_streams(H, dist, exact):
+    """BASELINE.json configs[0]: 512^3, alpha 1, beta 0.5, budget 1 MiB; float and {-4..4} variants."""
+    M = N = K = 512
+    A, B, C = host_inputs(H, M, N, K, synthgen.BASE_SEED + 1, dist)
+    ref = C.view.copy()
+    D = oracle.dgemm(1.0, A.view, B.view, 0.5, ref, want_denominator=True)
+    st = H.hclooc_dgemm_ex(None, M, N, K, 1.0, A, A.ld, B, B.ld, 0.5, C, C.ld, 1 * MiB)
+    assert st.plan.workspace_bytes <= 1 * MiB and st.plan.n_steps > 4
+    assert st.bytes_h2d == st.plan.bytes_h2d and st.bytes_d2h == st.plan.bytes_d2h == M * N * 8
+    check(C.view, ref, D, exact)
+
+
+def test_budget_invariance_bitwise(H):
+    """K is never split here, so every budget must give the same bits (SURVEY 8(c) invariant (i))."""
+    M, N, K = 515, 389, 301
+    outs = []
+    for budget in (1 * MiB, 4 * MiB, 64 * MiB, 0):
+        A, B, C = host_inputs(H, M, N, K, 33, "uniform", pads=(3, 5, 7))
+        st = H.hclooc_dgemm_ex(None, M, N, K, -0.75, A, A.ld, B, B.ld, 1.25, C, C.ld, budget)
+        assert st.plan.kpanels == 1
+        assert np.isnan(C.array[:, N:]).all()                  # host padding of C untouched
+        outs.append(C.view.copy())
+    for o in outs[1:]:
+        assert np.array_equal(o.view(np.uint64), outs[0].view(np.uint64))
+    A, B, C = host_inputs(H, M, N, K, 33, "uniform", pads=(3, 5, 7))
+    ref = C.view.copy()
+    D = oracle.dgemm(-0.75, A.view, B.view, 1.25, ref, want_denominator=True)
+    check(outs[0], ref, D, exact=False)
+
+
+def test_k_split_when_budget_is_tiny(H):
+    """A budget too small for one K-deep B slice forces K panels; integers stay exact."""
+    M, N, K = 96, 112, 4096
+    A, B, C = host_inputs(H, M, N, K, 34, "int")
+    ref = C.view.copy()
+    D = oracle.dgemm(2.0, A.view, B.view, -1.0, ref, want_denominator=True)
+    st = H.hclooc_dgemm_ex(None, M, N, K, 2.0, A, A.ld, B, B.ld, -1.0, C, C.ld, 600 * 1024)
+    assert st.plan.kpanels > 1
+    check(C.view, ref, D, exact=True)
+    A, B, C = host_inputs(H, M, N, K, 34, "uniform")
+    ref = C.view.copy()
+    D = oracle.dgemm(2.0, A.view, B.view, -1.0, ref, want_denominator=True)
+    H.hclooc_dgemm(M, N, K, 2.0, A, A.ld, B, B.ld, -1.0, C, C.ld, 600 * 1024)
+    check(C.view, ref, D, exact=False)
+
+
+@pytest.mark.parametrize("M,N,K", [(1, 1, 1), (7, 1000, 3), (1000, 7, 3), (257, 131, 1031), (640, 640, 64)])
+def test_ragged_and_degenerate_shapes(H, M, N, K):
+    A, B, C = host_inputs(H, M, N, K, 35, "int", pads=(1, 2, 3))
+    ref = C.view.copy()
+    D = oracle.dgemm(1.0, A.view, B.view, 0.5, ref, want_denominator=True)
+    H.hclooc_dgemm(M, N, K, 1.0, A, A.ld, B, B.ld, 0.5, C, C.ld, 2 * MiB)
+    check(C.view, ref, D, exact=True)
+    assert np.isnan(C.array[:, N:]).all()
+
+
+def test_beta_zero_overwrites_nan_and_alpha_zero_skips_a_b(H):
+    M, N, K = 300, 200, 150
+    A, B, C = host_inputs(H, M, N, K, 36, "uniform", poison_c=True)
+    ref = np.zeros((M, N))
+    D = oracle.dgemm(1.0, A.view, B.view, 0.0, ref, want_denominator=True)
+    st = H.hclooc_dgemm_ex(None, M, N, K, 1.0, A, A.ld, B, B.ld, 0.0, C, C.ld, 1 * MiB)
+    assert st.bytes_h2d == st.plan.bytes_h2d and st.plan.beta_nonzero == 0           # no C upload
+    check(C.view, ref, D, exact=False)
+    # alpha == 0: C = beta*C streamed through the device; A and B are NaN and must not matter
+    A.array[...] = np.nan; B.array[...] = np.nan
+    C0 = synthgen.fill(np.empty((M, N)), 36, "C", "uniform")
+    C.view[...] = C0
+    st = H.hclooc_dgemm_ex(None, M, N, K, 0.0, A, A.ld, B, B.ld, -2.0, C, C.ld, 1 * MiB)
+    assert st.plan.scale_only == 1 and st.bytes_h2d == M * N * 8
+    assert np.array_equal(C.view, -2.0 * C0)
+    # alpha == beta == 0: +0 everywhere
+    C.view[...] = np.nan
+    H.hclooc_dgemm(M, N, K, 0.0, A, A.ld, B, B.ld, 0.0, C, C.ld, 1 * MiB)
+    assert np.array_equal(C.view, np.zeros((M, N))) and not np.signbit(C.view).any()
+    # K == 0 and beta == 1: nothing to do
+    C.view[...] = C0
+    H.hclooc_dgemm(M, N, 0, 1.0, None, 1, None, N, 1.0, C, C.ld, 1 * MiB)
+    assert np.array_equal(C.view, C0)
+    # M == 0: touches nothing, pointers may be NULL
+    H.hclooc_dgemm(0, N, K, 1.0, None, K, None, N, 1.0, None, N, 1 * MiB)
+
+
+def test_k_split_identity_and_linearity_on_integers(H):
+    """Two calls on K halves (beta = 1 on the second) == one call; alpha scales linearly (exact on integers)."""
+    M, N, K = 200, 168, 256
+    A, B, C = host_inputs(H, M, N, K, 37, "int")
+    H.hclooc_dgemm(M, N, K, 1.0, A, A.ld, B, B.ld, 0.5, C, C.ld, 1 * MiB)
+    one = C.view.copy()
+    synthgen.fill(C.array, 37, "C", "int", cols=N)
+    H.hclooc_dgemm(M, N, K // 2, 1.0, A, A.ld, B, B.ld, 0.5, C, C.ld, 1 * MiB)
+    H.hclooc_dgemm(M, N, K - K // 2, 1.0, A.ptr + 8 * (K // 2), A.ld, B.ptr + 8 * (K // 2) * B.ld, B.ld, 1.0, C, C.ld, 1 * MiB)
+    assert np.array_equal(C.view, one)
+    C.view[...] = 0.0
+    H.hclooc_dgemm(M, N, K, 3.0, A, A.ld, B, B.ld, 0.0, C, C.ld, 1 * MiB)
+    three = C.view.copy()
+    H.hclooc_dgemm(M, N, K, 1.0, A, A.ld, B, B.ld, 0.0, C, C.ld, 1 * MiB)
+    assert np.array_equal(three, 3.0 * C.view)
+
+
+def test_argument_errors_leave_c_untouched(H):
+    M, N, K = 64, 64, 64
+    A, B, C = host_inputs(H, M, N, K, 38, "uniform")
+    before = C.view.copy()
+    cases = [((-1, N, K, 1.0, A, K, B, N, 1.0, C, N), -1), ((M, N, K, 1.0, None, K, B, N, 1.0, C, N), -5),
+             ((M, N, K, 1.0, A, K - 1, B, N, 1.0, C, N), -6), ((M, N, K, 1.0, A, K, None, N, 1.0, C, N), -7),
+             ((M, N, K, 1.0, A, K, B, N - 1, 1.0, C, N), -8), ((M, N, K, 1.0, A, K, B, N, 1.0, None, N), -10),
+             ((M, N, K, 1.0, A, K, B, N, 1.0, C, N - 1), -11), ((M, N, K, 1.0, C, K, B, N, 1.0, C, N), -10)]
+    for args, want in cases:
+        with pytest.raises(H.HclError) as e:
+            H.hclooc_dgemm(*args, 1 * MiB)
+        assert e.value.status == want, (args, e.value.status)
+    with pytest.raises(H.HclError) as e:
+        H.hclooc_dgemm(M, N, K, 1.0, A, K, B, N, 1.0, C, N, 4096)               # budget below the minimum working set
+    assert e.value.status == 1
+    pageable = np.ones((M, K))
+    with pytest.raises(H.HclError) as e:
+        H.hclooc_dgemm(M, N, K, 1.0, pageable, K, B, N, 1.0, C, N, 1 * MiB)      # no pageable fallback
+    assert e.value.status == 2
+    assert np.array_equal(C.view, before)
+    H.hclooc_host_register(pageable, pageable.nbytes)                             # pinned in place: now accepted
+    try:
+        H.hclooc_dgemm(M, N, K, 1.0, pageable, K, B, N, 0.0, C, N, 1 * MiB)
+    finally:
+        H.hclooc_host_unregister(pageable)
+    assert np.allclose(C.view, pageable @ B.view)
+
+
+def test_caller_owned_workspace_and_streams_from_torch(H):
+    """PyTorch supplies device memory and streams (north_star); the library carves its buffers from it."""
+    import torch
+    ws = torch.empty(8 * MiB, dtype=torch.uint8, device="cuda")
+    streams = [torch.cuda.Stream() for _ in range(5)]
+    ctx = H.hclooc_ctx_create(0, ws, ws.numel(), streams[0], streams[1], streams[2:])
+    try:
+        M, N, K = 700, 520, 384
+        A, B, C = host_inputs(H, M, N, K, 39, "int")
+        ref = C.view.copy()
+        oracle.dgemm(1.0, A.view, B.view, 0.5, ref)
+        st = H.hclooc_dgemm_ex(ctx, M, N, K, 1.0, A, A.ld, B, B.ld, 0.5, C, C.ld, 0)
+        assert st.plan.workspace_bytes <= ws.numel()
+        assert np.array_equal(C.view, ref)
+    finally:
+        H.hclooc_ctx_destroy(ctx)
+
+
+def test_runtime_calls_compose_a_manual_step(H):
+    """The paper's runtime calls (hclMalloc .. hclWaitEvent, :109-116, :212) used directly for one step."""
+    M, N, K = 192, 160, 96
+    A, B, C = host_inputs(H, M, N, K, 40, "int")
+    ref = C.view.copy()
+    oracle.dgemm(1.0, A.view, B.view, 1.0, ref)
+    assert H.hclGetMemSize(0) > (1 << 30)
+    dA, dB, dC = H.hclMalloc(M * K * 8), H.hclMalloc(K * N * 8), H.hclMalloc(M * N * 8)
+    s0, s1 = H.hclStreamCreate(), H.hclStreamCreate()
+    rB = H.hclMemcpyAsync(dB, B, K * N * 8, H.HCL_H2D, s0, want_event=True)
+    rA = H.hclMemcpyAsync(dA, A, M * K * 8, H.HCL_H2D, s0, want_event=True)
+    rC = H.hclMemcpy2DAsync(dC, N * 8, C, C.ld * 8, N * 8, M, H.HCL_H2D, s0, want_event=True)
+    for e in (rB, rA, rC):
+        H.hclWaitEvent(s1, e)
+    eA = H.hclDgemmAsync(M, N, K, 1.0, dA, K, dB, N, 1.0, dC, N, s1, want_event=True)
+    H.hclWaitEvent(s0, eA)
+    H.hclMemcpyAsync(C, dC, M * N * 8, H.HCL_D2H, s0)
+    H.hclStreamSynchronize(s0)
+    H.hclDeviceSynchronize(0)
+    assert np.array_equal(C.view, ref)
+    for e in (rB, rA, rC, eA):
+        H.hclEventDestroy(e)
+    for s in (s0, s1):
+        H.hclStreamDestroy(s)
+    for d in (dA, dB, dC):
+        H.hclFree(d)
+
+
+# ------------------------------------------------------------------ configs[1] at full size, sampled outputs
+def test_config2_full_size_sampled_rows_and_columns(H):
+    """BASELINE.json configs[1] (the bench workload): 8192^3, alpha 1, beta 1, budget 256 MiB, in the
+    launch configuration bench.py times.  The oracle computes complete rows and columns on both sides
+    of every slab boundary of the plan, plus random ones; integer variant bit-exact as well."""
+    M = N = K = 8192
+    for dist, exact in (("uniform", False), ("int", True)):
+        A, B, C = host_inputs(H, M, N, K, synthgen.BASE_SEED + 2, dist)
+        plan = H.hclooc_plan(M, N, K, 1, 0, 256 * MiB)
+        rng = np.random.default_rng(5)
+        rows = {0, M - 1} | {int(x) for x in rng.integers(0, M, 6)}
+        cols = {0, N - 1} | {int(x) for x in rng.integers(0, N, 6)}
+        for i in range(1, plan.h):
+            if i in (1, plan.h // 2, plan.h - 1):
+                rows |= {i * plan.mb - 1, i * plan.mb}
+        for j in range(1, plan.w):
+            cols |= {j * plan.nb - 1, j * plan.nb}
+        rows, cols = np.array(sorted(rows)), np.array(sorted(cols))
+        C0 = C.view.copy()
+        ref_r, D_r = oracle.dgemm_sub(1.0, A.view, B.view, 1.0, C0, rows=rows)
+        ref_c, D_c = oracle.dgemm_sub(1.0, A.view, B.view, 1.0, C0, cols=cols)
+        st = H.hclooc_dgemm_ex(None, M, N, K, 1.0, A, A.ld, B, B.ld, 1.0, C, C.ld, 256 * MiB)
+        assert st.plan.workspace_bytes <= 256 * MiB and st.bytes_h2d == st.plan.bytes_h2d
+        check(C.view[rows], ref_r, D_r, exact)
+        check(C.view[:, cols], ref_c, D_c, exact)
+        if exact:
+            # exact checksums over the WHOLE matrix (SURVEY 8(c) V-large (2)): C x and y^T C
+            x = synthgen.fill_numpy(N, 1, 77, "A", "int"); y = synthgen.fill_numpy(1, M, 77, "B", "int")
+            assert np.array_equal(C.view @ x, A.view @ (B.view @ x) + C0 @ x)
+            assert np.array_equal(y @ C.view, (y @ A.view) @ B.view + y @ C0)
+        for X in (A, B, C):
+            X.free()
