@@ -134,7 +134,7 @@ def test_budget_invariance_bitwise(H):
 
 def test_k_split_when_budget_is_tiny(H):
     """A budget too small for one K-deep B slice forces K panels; integers stay exact."""
-    M, N, K = 96, 112, 4096
+    M, N, K = 96, 112, 20000
     A, B, C = host_inputs(H, M, N, K, 34, "int")
     ref = C.view.copy()
     D = oracle.dgemm(2.0, A.view, B.view, -1.0, ref, want_denominator=True)

@@ -1,0 +1,256 @@
+"""Host logic without a GPU: the C ABI exports, the planner (S1) and the schedule (S2-S7).
+
+The schedule is the exact operation list the executor issues, so coverage, byte counts and the
+hazard rule of PAPER.md:311 ("data stored in device buffers is not overwritten until kernel
+executions that operate on the data have completed") are checked here by simulating stream/event
+semantics on the list itself.
+"""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_1808_05056_b200 as H
+
+MiB = 1 << 20
+GiB = 1 << 30
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+K_H2D_A, K_H2D_B, K_H2D_C, K_GEMM, K_D2H_C, K_WAIT, K_RECORD = range(7)
+
+
+# ------------------------------------------------------------------ the boundary
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "hclooc.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(hcl\w+|hclooc_\w+)\s*\(", hdr))
+    declared -= {"hclooc_ctx"}
+    assert declared == set(H.EXPORTS), declared ^ set(H.EXPORTS)
+    L = ctypes.CDLL(H.lib()._name)
+    for name in declared:
+        assert hasattr(L, name), name
+    assert "sm_100a" in H.hclooc_version()
+    assert "pageable" in H.hclooc_strerror(2) and H.hclooc_strerror(0) == "success"
+
+
+def test_binding_does_not_touch_the_oracle():
+    pkg = os.path.join(ROOT, "paper_1808_05056_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cpp", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in src and "from oracle" not in src and "liboracle" not in src, f
+
+
+# ------------------------------------------------------------------ the paper's partitioner rule
+def test_paper_example_partition():
+    # PAPER.md:301 / Figure 3 (:281): A 4x8, B 8x4, C 4x4, 44 elements -> 4 slices of A, 2 of B, 8 blocks
+    assert H.hclMatrixPartitioner(4, 4, 8, 44) == (4, 2)
+    assert H.hclMatrixPartitioner(4, 4, 8, 1000) == (1, 1)
+    with pytest.raises(H.HclError) as e:
+        H.hclMatrixPartitioner(4, 4, 8, 19)
+    assert e.value.status == 1
+
+
+def test_partitioner_agrees_with_brute_force_enumeration():
+    rng = np.random.default_rng(0)
+    for _ in range(200):
+        M, N, K = (int(x) for x in rng.integers(1, 25, 3))
+        S = int(rng.integers(1, 3 * (M * K + K * N + M * N)))
+        best = None
+        for h in range(1, M + 1):
+            if M % h:
+                continue
+            for w in range(1, N + 1):
+                if N % w:
+                    continue
+                mb, nb = M // h, N // w
+                if K * nb + 2 * mb * K + 2 * mb * nb > S:
+                    continue
+                key = (w * M * K + K * N + M * N, h * w, h)
+                if best is None or key < best[0]:
+                    best = (key, (h, w))
+        if best is None:
+            with pytest.raises(H.HclError):
+                H.hclMatrixPartitioner(M, N, K, S)
+        else:
+            assert H.hclMatrixPartitioner(M, N, K, S) == best[1], (M, N, K, S)
+
+
+# ------------------------------------------------------------------ hclooc_plan invariants
+CONFIGS = {  # BASELINE.json configs: (M, N, K, beta != 0, budget)
+    "cfg1": (512, 512, 512, 1, 1 * MiB),
+    "cfg2": (8192, 8192, 8192, 1, 256 * MiB),
+    "cfg3": (32768, 32768, 32768, 0, 4 * GiB),
+    "cfg4": (65536, 65536, 16384, 1, 16 * GiB),
+    "cfg5": (163840, 163840, 8192, 1, 178 * GiB),
+}
+
+
+def plan_checks(p, M, N, K, bnz, budget):
+    assert p.workspace_bytes <= budget
+    assert p.workspace_bytes == p.n_bbuf * p.bytes_b_buf + p.n_sets * (p.bytes_a_buf + p.bytes_c_buf)
+    assert p.h == -(-M // p.mb) and p.w == -(-N // p.nb)
+    assert p.n_steps == p.h * p.w * p.kpanels and p.n_sets >= 2
+    assert p.ldc_dev >= p.nb and p.ldc_dev % 2 == 0 and p.bytes_c_buf >= p.mb * p.ldc_dev * 8
+    if not p.scale_only:
+        assert p.kpanels == -(-K // p.kb)
+        assert p.lda_dev >= p.kb and p.lda_dev % 2 == 0 and p.ldb_dev >= p.nb and p.ldb_dev % 2 == 0
+        assert p.bytes_a_buf >= p.mb * p.lda_dev * 8 and p.bytes_b_buf >= p.kb * p.ldb_dev * 8
+        want_h2d = 8 * (p.w * M * K + K * N + (M * N if bnz else 0) + (p.kpanels - 1) * M * N)
+    else:
+        want_h2d = 8 * (M * N if bnz else 0)
+    assert p.bytes_h2d == want_h2d
+    assert p.bytes_d2h == 8 * p.kpanels * M * N
+
+
+@pytest.mark.parametrize("name", list(CONFIGS))
+def test_plans_for_the_baseline_configs(name):
+    M, N, K, bnz, budget = CONFIGS[name]
+    p = H.hclooc_plan(M, N, K, bnz, 0, budget)
+    plan_checks(p, M, N, K, bnz, budget)
+    assert p.kpanels == 1                       # none of the configs needs a K split
+    if name in ("cfg1", "cfg2"):                # link-bound: least traffic the budget allows
+        assert p.t_link_s > p.t_flop_s
+    else:                                       # FP64-bound
+        assert p.t_flop_s > p.t_link_s
+    if name == "cfg2":
+        assert p.w == 3 and p.bytes_h2d == 8 * 5 * 8192 * 8192
+
+
+def test_plans_for_random_shapes_and_budgets():
+    rng = np.random.default_rng(1)
+    n_ok = 0
+    for _ in range(300):
+        M, N, K = (int(x) for x in rng.integers(1, 3000, 3))
+        budget = int(rng.integers(64 * 1024, 64 * MiB))
+        bnz, az = int(rng.integers(0, 2)), int(rng.integers(0, 8) == 0)
+        try:
+            p = H.hclooc_plan(M, N, K, bnz, az, budget)
+        except H.HclError as e:
+            assert e.status == 1
+            continue
+        n_ok += 1
+        plan_checks(p, M, N, K, bnz, budget)
+    assert n_ok > 250
+    with pytest.raises(H.HclError):
+        H.hclooc_plan(100, 100, 100, 1, 0, 1024)
+    assert H.hclooc_plan(0, 5, 5, 1, 0, MiB).n_steps == 0
+    assert H.hclooc_plan(64, 64, 100000, 1, 0, 600 * 1024).kpanels > 1     # K split only when forced
+
+
+# ------------------------------------------------------------------ schedule: coverage, bytes, hazards
+def simulate(plan, ops, alpha_zero=False):
+    """Vector-clock simulation of CUDA stream/event semantics over the op list.
+    Returns nothing; asserts coverage, byte counts and that conflicting buffer accesses are ordered."""
+    n_streams = int(ops["stream"].max()) + 1
+    clock = [np.zeros(n_streams, dtype=np.int64) for _ in range(n_streams)]   # per-stream vector clocks
+    event_clock = {}
+    accesses = {}          # buffer -> list of (vector clock at completion, stream, is_write, row range, tag)
+    covered = np.zeros((plan.kpanels, plan.M, plan.N), dtype=np.int8) if plan.M * plan.N * plan.kpanels <= 4e6 else None
+    h2d = d2h = n_h2d = n_d2h = 0
+    content = {}           # buffer -> what it currently holds (for data-flow checks)
+
+    def access(buf, s, write, lo, hi, tag):
+        vc = clock[s].copy()
+        for (ovc, os_, ow, olo, ohi, otag) in accesses.setdefault(buf, []):
+            if not (write or ow):
+                continue
+            if hi <= olo or ohi <= lo:
+                continue
+            # the earlier access must happen-before this one: its clock entry on its own stream <= ours
+            assert ovc[os_] <= vc[os_], f"hazard on buffer {buf}: {otag} vs {tag}"
+        accesses[buf].append((vc, s, write, lo, hi, tag))
+        if len(accesses[buf]) > 64:
+            del accesses[buf][:32]
+
+    for idx, o in enumerate(ops):
+        s, kind = int(o["stream"]), int(o["kind"])
+        clock[s][s] += 1
+        if kind == K_RECORD:
+            event_clock[int(o["event"])] = clock[s].copy()
+        elif kind == K_WAIT:
+            assert int(o["event"]) in event_clock, "wait on an event never recorded"
+            clock[s] = np.maximum(clock[s], event_clock[int(o["event"])])
+        elif kind in (K_H2D_A, K_H2D_B, K_H2D_C):
+            assert s == 0
+            lo = int(o["dev_r0"]); hi = lo + int(o["nr"])
+            access(int(o["buf"]), s, True, lo, hi, (idx, "h2d", kind))
+            h2d += int(o["nr"]) * int(o["nc"]) * 8; n_h2d += 1
+            key = (kind, int(o["r0"]), int(o["nr"]), int(o["c0"]), int(o["nc"]))
+            if kind == K_H2D_B:
+                held = content.setdefault(int(o["buf"]), {})
+                for old in [r for r in held if not (r[1] <= lo or hi <= r[0])]:
+                    del held[old]                      # overwritten rows
+                held[(lo, hi)] = key
+            else:
+                content[int(o["buf"])] = key
+        elif kind == K_GEMM:
+            assert s >= 2
+            i0, mi, j0, nj, k0, kk = (int(o[f]) for f in ("r0", "nr", "c0", "nc", "k0", "kk"))
+            p = k0 // plan.kb if plan.kb else 0
+            if not plan.scale_only:
+                access(int(o["buf"]), s, False, 0, mi, (idx, "gemm-A"))
+                access(int(o["buf2"]), s, False, 0, kk, (idx, "gemm-B"))
+                assert content[int(o["buf"])] == (K_H2D_A, i0, mi, k0, kk)          # the right A slice is resident
+                rows = sorted(content[int(o["buf2"])].items())
+                got = [v for (lo, hi), v in rows if lo < kk]
+                assert sum(v[2] for v in got) == kk and all(v[3] == j0 and v[4] == nj for v in got)
+                assert min(v[1] for v in got) == k0 and max(v[1] + v[2] for v in got) == k0 + kk
+            cload = plan.beta_nonzero or p > 0
+            if cload:
+                assert content[int(o["buf3"])] == (K_H2D_C, i0, mi, j0, nj)
+            access(int(o["buf3"]), s, True, 0, mi, (idx, "gemm-C"))
+            content[int(o["buf3"])] = ("result", i0, mi, j0, nj, p)
+            assert (o["beta"] == 1.0) == (p > 0)
+            if covered is not None:
+                covered[p, i0:i0 + mi, j0:j0 + nj] += 1
+        elif kind == K_D2H_C:
+            assert s == 1
+            access(int(o["buf"]), s, False, 0, int(o["nr"]), (idx, "d2h"))
+            c = content[int(o["buf"])]
+            assert c[0] == "result" and c[1:5] == (int(o["r0"]), int(o["nr"]), int(o["c0"]), int(o["nc"]))
+            d2h += int(o["nr"]) * int(o["nc"]) * 8; n_d2h += 1
+    assert h2d == plan.bytes_h2d and d2h == plan.bytes_d2h
+    assert n_h2d == plan.n_copies_h2d and n_d2h == plan.n_copies_d2h
+    assert int((ops["kind"] == K_GEMM).sum()) == plan.n_steps
+    if covered is not None:
+        assert (covered == 1).all()            # every C element computed exactly once per K panel
+
+
+@pytest.mark.parametrize("shape", [
+    (512, 512, 512, 1, 0, 1 * MiB), (515, 389, 301, 1, 0, 1 * MiB), (515, 389, 301, 0, 0, 4 * MiB),
+    (96, 112, 20000, 1, 0, 600 * 1024), (300, 200, 150, 1, 1, 1 * MiB), (300, 200, 150, 0, 1, 1 * MiB),
+    (2000, 1500, 700, 1, 0, 6 * MiB), (2000, 1500, 700, 0, 0, 64 * MiB), (1, 1, 1, 1, 0, 1 * MiB),
+])
+@pytest.mark.parametrize("n_compute", [1, 3, 8])
+def test_schedule_is_complete_and_hazard_free(shape, n_compute):
+    M, N, K, bnz, az, budget = shape
+    p = H.hclooc_plan(M, N, K, bnz, az, budget)
+    ops = H.hclooc_schedule(p, n_compute)
+    simulate(p, ops)
+
+
+def test_schedule_with_two_b_buffers_prefetches_in_chunks(monkeypatch):
+    monkeypatch.setenv("HCLOOC_FORCE_BBUF", "2")     # experiment knob of the planner: two B buffers
+    p = H.hclooc_plan(4096, 4096, 2048, 0, 0, 40 * MiB)
+    assert p.n_bbuf == 2 and p.w > 1
+    ops = H.hclooc_schedule(p, 4)
+    simulate(p, ops)
+    b_loads = ops[ops["kind"] == K_H2D_B]
+    assert len(b_loads) > p.w                   # later slices arrive in several chunks
+
+
+def test_simulator_catches_a_missing_wait():
+    """The checker is not vacuous: dropping the Wait(eA) before an A upload is reported."""
+    p = H.hclooc_plan(515, 389, 301, 1, 0, 1 * MiB)
+    ops = H.hclooc_schedule(p, 4)
+    first_kernel_done = p.n_sets                # event ids: kernel_done(s) = n_sets + s
+    idx = [i for i, o in enumerate(ops) if o["kind"] == K_WAIT and o["stream"] == 0
+           and p.n_sets <= o["event"] < 2 * p.n_sets]
+    assert idx
+    broken = np.delete(ops, idx)
+    with pytest.raises(AssertionError, match="hazard"):
+        simulate(p, broken)
+    assert first_kernel_done >= 2
