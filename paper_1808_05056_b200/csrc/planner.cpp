@@ -98,7 +98,11 @@ void cost(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool scale_onl
     const double flops = scale_only ? 0.0 : 2.0 * (double)M * (double)N * (double)K;
     // tile padding and SM fill
     const double tiles_step = (double)ceil_div(c.mb, TILE) * (double)ceil_div(c.nb, TILE);
-    const double pad_eff = ((double)c.mb / (ceil_div(c.mb, TILE) * TILE)) * ((double)c.nb / (ceil_div(c.nb, TILE) * TILE));
+    // exact share of useful work in the 128 x 128 tiles the kernel launches (ragged last slices included)
+    const int64_t m_last = M - (c.h - 1) * c.mb, n_last = N - (c.w - 1) * c.nb;
+    const double tile_rows = (double)((c.h - 1) * ceil_div(c.mb, TILE) + ceil_div(m_last, TILE));
+    const double tile_cols = (double)((c.w - 1) * ceil_div(c.nb, TILE) + ceil_div(n_last, TILE));
+    const double pad_eff = ((double)M * (double)N) / (tile_rows * tile_cols * (double)(TILE * TILE));
     const double in_flight = std::max(1, c.n_sets - 2) * tiles_step;
     double fill = std::min(1.0, in_flight / NUM_SMS);
     if (tiles_step >= NUM_SMS) fill = std::min(fill, 0.98);
@@ -155,8 +159,10 @@ extern "C" int hclooc_plan(int64_t M, int64_t N, int64_t K, int beta_nonzero, in
         const int64_t kp = scale_only ? 1 : ceil_div(Keff, kb);
         int64_t last_nb = -1;
         const int64_t wmax = ceil_div(N, 16);
-        for (int64_t w = 1; w <= wmax; w = (w < 64 ? w + 1 : w + w / 8)) {
-            const int64_t nb = std::min(N, round_up(ceil_div(N, w), 16));
+        for (int64_t wi = 2; wi <= 2 * wmax + 1; wi = (wi < 128 ? wi + 1 : wi + wi / 8)) {
+            // two slice widths per w: the thinnest multiple of 16 and the thinnest multiple of the tile edge
+            const int64_t w = wi / 2;
+            const int64_t nb = std::min(N, round_up(ceil_div(N, w), (wi & 1) ? TILE : 16));
             if (nb == last_nb) continue;
             last_nb = nb;
             if (force_nb && nb != std::min(N, round_up(force_nb, 16))) continue;
