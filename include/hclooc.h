@@ -127,6 +127,20 @@ int hclooc_ctx_create(hclooc_ctx** ctx, int device, void* d_workspace, size_t wo
                       hclStream stream_h2d, hclStream stream_d2h, hclStream* compute_streams, int n_compute);
 int hclooc_ctx_destroy(hclooc_ctx* ctx);
 
+/* Tracing (debug aid): when enabled, the next hclooc_dgemm_ex calls on this context
+ * bracket every copy and kernel with timing events; hclooc_ctx_get_trace returns, for the LAST call, one
+ * record per operation with start/end in milliseconds relative to the first operation of that call.
+ * ctx == NULL addresses the default context.  Tracing costs two event records per operation.       */
+typedef struct hclooc_trace_rec {
+    int32_t  kind, stream;        /* HCLOOC_OP_* and stream index as in hclooc_op_t                  */
+    int64_t  step;
+    uint64_t bytes;               /* bytes moved (copies) or 0                                        */
+    double   flops;               /* 2*m*n*k (kernels) or 0                                           */
+    double   t_start_ms, t_end_ms;
+} hclooc_trace_rec;
+int hclooc_ctx_set_trace(hclooc_ctx* ctx, int enable);
+int hclooc_ctx_get_trace(hclooc_ctx* ctx, hclooc_trace_rec* recs, size_t max_recs, size_t* n_recs);
+
 /* ------------------------------------------------------------------ the operation
  * hclooc_dgemm: C = alpha*A*B + beta*C, synchronous: C is complete in host memory on return.
  *   A: M x K, lda >= K;  B: K x N, ldb >= N;  C: M x N, ldc >= N, updated IN PLACE; A, B read-only.

@@ -13,6 +13,7 @@ HCL_H2D, HCL_D2H = 0, 1
 # every symbol include/hclooc.h declares (tests check the .so exports all of them)
 EXPORTS = [
     "hclooc_plan", "hclMatrixPartitioner", "hclooc_schedule", "hclooc_ctx_create", "hclooc_ctx_destroy",
+    "hclooc_ctx_set_trace", "hclooc_ctx_get_trace",
     "hclooc_dgemm", "hclooc_dgemm_ex", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
     "hclStreamDestroy", "hclEventDestroy", "hclMemcpy", "hclMemcpyAsync", "hclMemcpy2DAsync",
     "hclDgemmAsync", "hclWaitEvent", "hclStreamSynchronize", "hclDeviceSynchronize",
@@ -73,6 +74,8 @@ def lib():
         L.hclooc_schedule.argtypes = [POINTER(Plan), c_int, vp, sz, POINTER(sz)]
         L.hclooc_ctx_create.argtypes = [POINTER(vp), c_int, vp, sz, vp, vp, POINTER(vp), c_int]
         L.hclooc_ctx_destroy.argtypes = [vp]
+        L.hclooc_ctx_set_trace.argtypes = [vp, c_int]
+        L.hclooc_ctx_get_trace.argtypes = [vp, vp, sz, POINTER(sz)]
         L.hclooc_dgemm.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz]
         L.hclooc_dgemm_ex.argtypes = [vp, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
         L.hclMalloc.argtypes = [POINTER(vp), sz]
@@ -207,6 +210,24 @@ def hclooc_ctx_create(device=0, d_workspace=None, workspace_bytes=0, stream_h2d=
 
 def hclooc_ctx_destroy(ctx) -> None:
     _check(lib().hclooc_ctx_destroy(ctx), "hclooc_ctx_destroy")
+
+
+TRACE_DTYPE = np.dtype([("kind", "<i4"), ("stream", "<i4"), ("step", "<i8"), ("bytes", "<u8"), ("flops", "<f8"),
+                        ("t_start_ms", "<f8"), ("t_end_ms", "<f8")], align=True)
+
+
+def hclooc_ctx_set_trace(ctx, enable: bool) -> None:
+    _check(lib().hclooc_ctx_set_trace(ctx, int(bool(enable))), "hclooc_ctx_set_trace")
+
+
+def hclooc_ctx_get_trace(ctx) -> np.ndarray:
+    n = c_size_t()
+    _check(lib().hclooc_ctx_get_trace(ctx, None, 0, byref(n)), "hclooc_ctx_get_trace")
+    recs = np.zeros(n.value, dtype=TRACE_DTYPE)
+    assert TRACE_DTYPE.itemsize == 48
+    if n.value:
+        _check(lib().hclooc_ctx_get_trace(ctx, recs.ctypes.data, n.value, byref(n)), "hclooc_ctx_get_trace")
+    return recs
 
 
 def hclooc_dgemm(M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes) -> None:

@@ -145,6 +145,9 @@ struct hclooc_ctx {
     bool owns_compute = false;
     std::vector<cudaEvent_t> events;
     std::vector<hclooc_op_t> ops;
+    bool trace = false;
+    std::vector<cudaEvent_t> trace_events;        // 2 per traced op (+1 base), timing enabled
+    std::vector<hclooc_trace_rec> trace_recs;     // filled after the final synchronisation
     std::mutex mu;
 };
 
@@ -196,6 +199,7 @@ extern "C" int hclooc_ctx_destroy(hclooc_ctx* c) {
     cudaSetDevice(c->device);
     cudaDeviceSynchronize();
     for (cudaEvent_t e : c->events) cudaEventDestroy(e);
+    for (cudaEvent_t e : c->trace_events) cudaEventDestroy(e);
     if (c->owns_h2d && c->s_h2d) cudaStreamDestroy(c->s_h2d);
     if (c->owns_d2h && c->s_d2h) cudaStreamDestroy(c->s_d2h);
     if (c->owns_compute) for (int i = 0; i < c->n_compute; ++i) if (c->s_compute[i]) cudaStreamDestroy(c->s_compute[i]);
@@ -326,8 +330,31 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
     uint64_t bytes_h2d = 0, bytes_d2h = 0, n_h2d = 0, n_d2h = 0, n_kernels = 0;
     const auto t_enq0 = std::chrono::steady_clock::now();
     rc = HCLOOC_OK;
+    const bool trace = ctx->trace;
+    size_t n_traced = 0;
+    if (trace) {
+        size_t need = 1;
+        for (const hclooc_op_t& o : ctx->ops) if (o.kind != HCLOOC_OP_WAIT && o.kind != HCLOOC_OP_RECORD) need += 2;
+        while (ctx->trace_events.size() < need) {
+            cudaEvent_t e;
+            HCL_CUDA(cudaEventCreate(&e));
+            ctx->trace_events.push_back(e);
+        }
+        ctx->trace_recs.clear();
+        HCL_CUDA(cudaEventRecord(ctx->trace_events[0], ctx->s_h2d));
+    }
     for (const hclooc_op_t& o : ctx->ops) {
         cudaStream_t st = stream_of(o.stream);
+        const bool traced = trace && o.kind != HCLOOC_OP_WAIT && o.kind != HCLOOC_OP_RECORD;
+        if (traced) {
+            cudaEventRecord(ctx->trace_events[1 + 2 * n_traced], st);
+            hclooc_trace_rec r;
+            std::memset(&r, 0, sizeof(r));
+            r.kind = o.kind; r.stream = o.stream; r.step = o.step;
+            if (o.kind == HCLOOC_OP_GEMM) r.flops = 2.0 * (double)o.nr * (double)o.nc * (double)o.kk;
+            else r.bytes = (uint64_t)o.nr * (uint64_t)o.nc * 8;
+            ctx->trace_recs.push_back(r);
+        }
         switch (o.kind) {
             case HCLOOC_OP_WAIT: {
                 cudaError_t e = cudaStreamWaitEvent(st, ctx->events[o.event], 0);
@@ -364,6 +391,7 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
             }
             default: rc = HCLOOC_ERR_INTERNAL;
         }
+        if (traced) { cudaEventRecord(ctx->trace_events[2 + 2 * n_traced], st); ++n_traced; }
         if (rc) break;
     }
     const auto t_enq1 = std::chrono::steady_clock::now();
@@ -376,6 +404,15 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
     if (e1 != cudaSuccess) return cuda_fail(e1);
     if (e2 != cudaSuccess) return cuda_fail(e2);
     if (e3 != cudaSuccess) return cuda_fail(e3);
+    if (trace) {
+        for (size_t i = 0; i < n_traced && i < ctx->trace_recs.size(); ++i) {
+            float a = 0, b = 0;
+            cudaEventElapsedTime(&a, ctx->trace_events[0], ctx->trace_events[1 + 2 * i]);
+            cudaEventElapsedTime(&b, ctx->trace_events[0], ctx->trace_events[2 + 2 * i]);
+            ctx->trace_recs[i].t_start_ms = a;
+            ctx->trace_recs[i].t_end_ms = b;
+        }
+    }
     if (bytes_h2d != P.bytes_h2d || bytes_d2h != P.bytes_d2h || n_h2d != P.n_copies_h2d || n_d2h != P.n_copies_d2h) return HCLOOC_ERR_INTERNAL;
     if (stats) {
         stats->plan = P;
@@ -390,6 +427,24 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
 extern "C" int hclooc_dgemm(int64_t M, int64_t N, int64_t K, double alpha, const double* A, int64_t lda,
                             const double* B, int64_t ldb, double beta, double* C, int64_t ldc, size_t device_budget_bytes) {
     return hclooc_dgemm_ex(nullptr, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes, nullptr);
+}
+
+extern "C" int hclooc_ctx_set_trace(hclooc_ctx* ctx, int enable) {
+    int rc;
+    if (!ctx && (rc = default_ctx(&ctx))) return rc;
+    std::lock_guard<std::mutex> lk(ctx->mu);
+    ctx->trace = enable != 0;
+    return HCLOOC_OK;
+}
+
+extern "C" int hclooc_ctx_get_trace(hclooc_ctx* ctx, hclooc_trace_rec* recs, size_t max_recs, size_t* n_recs) {
+    int rc;
+    if (!n_recs) return -4;
+    if (!ctx && (rc = default_ctx(&ctx))) return rc;
+    std::lock_guard<std::mutex> lk(ctx->mu);
+    *n_recs = ctx->trace_recs.size();
+    if (recs) std::memcpy(recs, ctx->trace_recs.data(), std::min(max_recs, ctx->trace_recs.size()) * sizeof(hclooc_trace_rec));
+    return HCLOOC_OK;
 }
 
 extern "C" int hclooc_last_cuda_error(void) { return g_last_cuda_error; }

@@ -308,3 +308,28 @@ def test_config2_full_size_sampled_rows_and_columns(H):
             assert np.array_equal(y @ C.view, (y @ A.view) @ B.view + y @ C0)
         for X in (A, B, C):
             X.free()
+
+
+def test_trace_records_every_copy_and_kernel(H):
+    """hclooc_ctx_set_trace / get_trace: one record per copy and kernel of the last call, ordered in time."""
+    M, N, K = 515, 389, 301
+    A, B, C = host_inputs(H, M, N, K, 41, "int")
+    ref = C.view.copy()
+    oracle.dgemm(1.0, A.view, B.view, 0.5, ref)
+    ctx = H.hclooc_ctx_create(0)
+    try:
+        H.hclooc_ctx_set_trace(ctx, True)
+        st = H.hclooc_dgemm_ex(ctx, M, N, K, 1.0, A, A.ld, B, B.ld, 0.5, C, C.ld, 1 * MiB)
+        tr = H.hclooc_ctx_get_trace(ctx)
+        assert np.array_equal(C.view, ref)
+        assert len(tr) == st.n_kernels + st.n_copies_h2d + st.n_copies_d2h
+        assert int(tr["bytes"][tr["kind"] <= 2].sum()) == st.bytes_h2d and int(tr["bytes"][tr["kind"] == 4].sum()) == st.bytes_d2h
+        assert tr["flops"].sum() == 2.0 * M * N * K
+        assert (tr["t_end_ms"] >= tr["t_start_ms"]).all() and tr["t_start_ms"].min() >= 0.0
+        for step in range(st.plan.n_steps):      # per step: uploads end before the kernel ends before the download ends
+            r = tr[tr["step"] == step]
+            k = r[r["kind"] == 3][0]
+            assert (r[r["kind"] < 3]["t_end_ms"] <= k["t_end_ms"]).all()
+            assert k["t_end_ms"] <= r[r["kind"] == 4][0]["t_end_ms"]
+    finally:
+        H.hclooc_ctx_destroy(ctx)
