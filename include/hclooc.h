@@ -62,6 +62,8 @@ typedef struct hclooc_plan_t {
     int32_t  n_bbuf;              /* B slice device buffers (1 = paper's single buffer, 2 = prefetch) */
     int32_t  beta_nonzero;        /* C blocks are uploaded only when 1 (or for K panels p > 0)      */
     int32_t  scale_only;          /* alpha == 0 or K == 0: C = beta*C, A and B never referenced     */
+    int32_t  ksplit;              /* CTAs per cluster sharing one tile's K range in the kernel (1, 2, 4) */
+    int32_t  reserved0;
     int64_t  lda_dev, ldb_dev, ldc_dev;  /* leading dimensions of the device buffers (elements)    */
     uint64_t bytes_a_buf, bytes_b_buf, bytes_c_buf;   /* one buffer of each kind                   */
     uint64_t workspace_bytes;     /* n_bbuf*b + n_sets*(a + c), <= the budget                       */

@@ -27,6 +27,7 @@ class Plan(ctypes.Structure):
                 ("mb", c_int64), ("nb", c_int64), ("kb", c_int64),
                 ("h", c_int64), ("w", c_int64), ("kpanels", c_int64), ("n_steps", c_int64),
                 ("n_sets", c_int32), ("n_bbuf", c_int32), ("beta_nonzero", c_int32), ("scale_only", c_int32),
+                ("ksplit", c_int32), ("reserved0", c_int32),
                 ("lda_dev", c_int64), ("ldb_dev", c_int64), ("ldc_dev", c_int64),
                 ("bytes_a_buf", c_uint64), ("bytes_b_buf", c_uint64), ("bytes_c_buf", c_uint64),
                 ("workspace_bytes", c_uint64), ("bytes_h2d", c_uint64), ("bytes_d2h", c_uint64),

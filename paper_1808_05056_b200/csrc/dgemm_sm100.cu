@@ -75,7 +75,25 @@ __device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
                  : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
 }
 
-// One CTA computes one 128 x 128 tile of C over the whole K range.
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void ld_dsmem128(double& x, double& y, uint32_t local_addr, uint32_t rank) {
+    uint32_t remote;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local_addr), "r"(rank));
+    asm volatile("ld.shared::cluster.v2.f64 {%0, %1}, [%2];" : "=d"(x), "=d"(y) : "r"(remote) : "memory");
+}
+
+// One CTA computes one 128 x 128 tile of C over the whole K range (KSPLIT == 1), or a cluster of KSPLIT
+// CTAs shares the tile: CTA r of the cluster takes the r-th share of the k blocks, the partial
+// accumulators are reduced through distributed shared memory in rank order (deterministic) and CTA 0
+// runs the epilogue.  Used when a pipeline step has too few tiles to fill 148 SMs.
+template <int KSPLIT>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 hclooc_dgemm_tile_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                          double* __restrict__ C, long long ldc, int M, int N, int K,
@@ -91,8 +109,9 @@ hclooc_dgemm_tile_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_c
     int tile_m, tile_n;
     {
         const int per_group = RASTER_GROUP * tiles_n;
-        const int grp = blockIdx.x / per_group;
-        const int rem = blockIdx.x - grp * per_group;
+        const int tile = (KSPLIT == 1) ? (int)blockIdx.x : (int)(blockIdx.x / KSPLIT);
+        const int grp = tile / per_group;
+        const int rem = tile - grp * per_group;
         const int gm0 = grp * RASTER_GROUP;
         const int gsz = min(RASTER_GROUP, tiles_m - gm0);
         tile_m = gm0 + rem % gsz;
@@ -100,7 +119,11 @@ hclooc_dgemm_tile_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_c
     }
     const int m0 = tile_m * BM;
     const int n0 = tile_n * BN;
-    const int num_kb = (K + BK - 1) / BK;
+    const int num_kb_all = (K + BK - 1) / BK;
+    const uint32_t crank = (KSPLIT == 1) ? 0u : cluster_ctarank();
+    const int kb_begin = (KSPLIT == 1) ? 0 : (int)(((long long)num_kb_all * crank) / KSPLIT);
+    const int kb_end = (KSPLIT == 1) ? num_kb_all : (int)(((long long)num_kb_all * (crank + 1)) / KSPLIT);
+    const int num_kb = kb_end - kb_begin;
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; ++s) {
@@ -125,13 +148,17 @@ hclooc_dgemm_tile_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_c
                 mbar_expect_tx(full, STAGE_BYTES);
                 const uint32_t sa = smem_base + stage * STAGE_BYTES;
                 const uint32_t sb = sa + A_STAGE_BYTES;
-                const int k0 = kb * BK;
+                const int k0 = (kb_begin + kb) * BK;
                 tma_load_2d(sa, &tmA, k0, m0, full);
                 #pragma unroll
                 for (int b = 0; b < BN / 16; ++b) tma_load_2d(sb + b * B_BOX_BYTES, &tmB, n0 + 16 * b, k0, full);
                 if (++stage == STAGES) { stage = 0; phase ^= 1u; }
             }
         }
+        if (KSPLIT == 1) return;
+        __syncwarp();
+        cluster_sync_all();      // partials written
+        cluster_sync_all();      // partials read: peers may exit
         return;
     }
 
@@ -187,6 +214,44 @@ hclooc_dgemm_tile_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_c
             if (lane == 0) mbar_arrive(bar_base + 8 * (STAGES + stage));
             if (++stage == STAGES) { stage = 0; phase ^= 1u; }
         }
+    }
+
+    // ---------------------------------------------------------------- split-K reduction over the cluster (DSMEM)
+    if (KSPLIT > 1) {
+        // every consumer warp of this CTA is done reading the stage buffers before they are reused
+        asm volatile("bar.sync 1, %0;" ::"n"(NUM_CONSUMER_WARPS * 32) : "memory");
+        const uint32_t slot = smem_base + threadIdx.x * 16;          // [i][tid] double2 layout: conflict free
+        if (crank != 0) {
+            #pragma unroll
+            for (int u = 0; u < 4; ++u)
+                #pragma unroll
+                for (int bx = 0; bx < 4; ++bx)
+                    #pragma unroll
+                    for (int v = 0; v < 2; ++v)
+                        asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(slot + ((u * 4 + bx) * 2 + v) * (NUM_CONSUMER_WARPS * 32 * 16)),
+                                     "d"(acc[u][bx][v][0]), "d"(acc[u][bx][v][1]) : "memory");
+        }
+        __syncwarp();
+        cluster_sync_all();
+        if (crank == 0) {
+            #pragma unroll 1
+            for (uint32_t r = 1; r < (uint32_t)KSPLIT; ++r) {
+                #pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    #pragma unroll
+                    for (int bx = 0; bx < 4; ++bx)
+                        #pragma unroll
+                        for (int v = 0; v < 2; ++v) {
+                            double p0, p1;
+                            ld_dsmem128(p0, p1, slot + ((u * 4 + bx) * 2 + v) * (NUM_CONSUMER_WARPS * 32 * 16), r);
+                            acc[u][bx][v][0] += p0;
+                            acc[u][bx][v][1] += p1;
+                        }
+            }
+        }
+        __syncwarp();
+        cluster_sync_all();
+        if (crank != 0) return;
     }
 
     // ---------------------------------------------------------------- fused epilogue
@@ -259,18 +324,46 @@ int ensure_kernel_attr() {
     static int status = -1;
     static std::once_flag once;
     std::call_once(once, [] {
-        cudaError_t e = cudaFuncSetAttribute(hclooc_dgemm_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+        cudaError_t e = cudaFuncSetAttribute(hclooc_dgemm_tile_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(hclooc_dgemm_tile_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(hclooc_dgemm_tile_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
         status = (e == cudaSuccess) ? 0 : cuda_fail(e);
     });
     return status;
+}
+
+template <int KSPLIT>
+cudaError_t launch_split(unsigned tiles, cudaStream_t stream, const CUtensorMap& tmA, const CUtensorMap& tmB, double* dC,
+                         long long ldc, int M, int N, int K, double alpha, double beta, int tm, int tn) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(tiles * KSPLIT, 1, 1);
+    cfg.blockDim = dim3(NUM_THREADS, 1, 1);
+    cfg.dynamicSmemBytes = SMEM_BYTES;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = KSPLIT;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, hclooc_dgemm_tile_kernel<KSPLIT>, tmA, tmB, dC, ldc, M, N, K, alpha, beta, tm, tn);
 }
 
 }  // namespace
 
 int64_t dgemm_tile_count(int64_t M, int64_t N) { return ((M + BM - 1) / BM) * ((N + BN - 1) / BN); }
 
+int dgemm_auto_ksplit(int64_t tiles_in_flight, int64_t K) {
+    // split K over a 2- or 4-CTA cluster when the tiles that can run together leave most SMs idle
+    if (K >= 2048 && tiles_in_flight * 4 <= 148) return 4;
+    if (K >= 1024 && tiles_in_flight * 2 <= 148) return 2;
+    return 1;
+}
+
 int launch_dgemm_tiles(int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda,
-                       const double* dB, int64_t ldb, double beta, double* dC, int64_t ldc, cudaStream_t stream) {
+                       const double* dB, int64_t ldb, double beta, double* dC, int64_t ldc, cudaStream_t stream,
+                       int ksplit) {
     if (M == 0 || N == 0) return HCLOOC_OK;
     if (alpha == 0.0) K = 0;                       // A and B are not referenced (BLAS convention)
     int rc = ensure_kernel_attr();
@@ -285,9 +378,16 @@ int launch_dgemm_tiles(int64_t M, int64_t N, int64_t K, double alpha, const doub
     }
     const int64_t tm = (M + BM - 1) / BM, tn = (N + BN - 1) / BN;
     if (tm * tn > 0x7fffffffLL || M > 0x7fffffffLL || N > 0x7fffffffLL || K > 0x7fffffffLL) return HCLOOC_ERR_INTERNAL;
-    hclooc_dgemm_tile_kernel<<<(unsigned)(tm * tn), NUM_THREADS, SMEM_BYTES, stream>>>(
-        tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn);
-    cudaError_t e = cudaGetLastError();
+    if (ksplit <= 0) ksplit = dgemm_auto_ksplit(tm * tn, K);
+    if (K == 0) ksplit = 1;
+    cudaError_t e;
+    if (ksplit >= 4) e = launch_split<4>((unsigned)(tm * tn), stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn);
+    else if (ksplit >= 2) e = launch_split<2>((unsigned)(tm * tn), stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn);
+    else {
+        hclooc_dgemm_tile_kernel<1><<<(unsigned)(tm * tn), NUM_THREADS, SMEM_BYTES, stream>>>(
+            tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn);
+        e = cudaGetLastError();
+    }
     if (e != cudaSuccess) return cuda_fail(e);
     return HCLOOC_OK;
 }

@@ -385,7 +385,7 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
             case HCLOOC_OP_GEMM: {
                 const double b_eff = (o.beta < 0.0) ? beta : o.beta;
                 rc = launch_dgemm_tiles(o.nr, o.nc, o.kk, scale_only ? 0.0 : alpha, o.buf >= 0 ? bufs[o.buf] : nullptr, P.lda_dev,
-                                        o.buf2 >= 0 ? bufs[o.buf2] : nullptr, P.ldb_dev, b_eff, bufs[o.buf3], P.ldc_dev, st);
+                                        o.buf2 >= 0 ? bufs[o.buf2] : nullptr, P.ldb_dev, b_eff, bufs[o.buf3], P.ldc_dev, st, P.ksplit > 0 ? P.ksplit : 1);
                 ++n_kernels;
                 break;
             }

@@ -33,7 +33,10 @@ const MachineModel& machine_model();
 // Preconditions (checked by callers): pointers 16-byte aligned, leading dimensions even.
 int launch_dgemm_tiles(int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda,
                        const double* dB, int64_t ldb, double beta, double* dC, int64_t ldc,
-                       cudaStream_t stream);
+                       cudaStream_t stream, int ksplit);   // ksplit: 1, 2, 4, or 0 = choose from the tile count
+
+// K split (cluster size) worth using when `tiles_in_flight` tiles can run concurrently
+int dgemm_auto_ksplit(int64_t tiles_in_flight, int64_t K);
 
 // number of CTAs the tile kernel uses for an M x N output (for stats / tests)
 int64_t dgemm_tile_count(int64_t M, int64_t N);

@@ -52,7 +52,7 @@ namespace {
 
 struct Cand {
     int64_t mb, nb, kb, h, w, kpanels;
-    int n_sets, n_bbuf;
+    int n_sets, n_bbuf, ksplit;
     int64_t lda_dev, ldb_dev, ldc_dev;
     uint64_t a_bytes, b_bytes, c_bytes, ws_bytes;
     uint64_t bytes_h2d, bytes_d2h, n_h2d, n_d2h;
@@ -103,7 +103,10 @@ void cost(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool scale_onl
     const double tile_rows = (double)((c.h - 1) * ceil_div(c.mb, TILE) + ceil_div(m_last, TILE));
     const double tile_cols = (double)((c.w - 1) * ceil_div(c.nb, TILE) + ceil_div(n_last, TILE));
     const double pad_eff = ((double)M * (double)N) / (tile_rows * tile_cols * (double)(TILE * TILE));
-    const double in_flight = std::max(1, c.n_sets - 2) * tiles_step;
+    // too few tiles in flight to fill the SMs: a cluster of 2 or 4 CTAs shares each tile's K range
+    const int force_ks = (int)env_or("HCLOOC_FORCE_KSPLIT", 0);
+    c.ksplit = scale_only ? 1 : (force_ks ? force_ks : dgemm_auto_ksplit((int64_t)(std::max(1, c.n_sets - 2) * tiles_step), c.kb));
+    const double in_flight = std::max(1, c.n_sets - 2) * tiles_step * c.ksplit;
     double fill = std::min(1.0, in_flight / NUM_SMS);
     if (tiles_step >= NUM_SMS) fill = std::min(fill, 0.98);
     c.t_flop = flops / mm.fp64_flops;
@@ -218,7 +221,7 @@ extern "C" int hclooc_plan(int64_t M, int64_t N, int64_t K, int beta_nonzero, in
     out->mb = best.mb; out->nb = best.nb; out->kb = best.kb;
     out->h = best.h; out->w = best.w; out->kpanels = best.kpanels;
     out->n_steps = best.h * best.w * best.kpanels;
-    out->n_sets = best.n_sets; out->n_bbuf = best.n_bbuf;
+    out->n_sets = best.n_sets; out->n_bbuf = best.n_bbuf; out->ksplit = best.ksplit;
     out->lda_dev = best.lda_dev; out->ldb_dev = best.ldb_dev; out->ldc_dev = best.ldc_dev;
     out->bytes_a_buf = best.a_bytes; out->bytes_b_buf = best.b_bytes; out->bytes_c_buf = best.c_bytes;
     out->workspace_bytes = best.ws_bytes;

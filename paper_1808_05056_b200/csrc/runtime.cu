@@ -111,7 +111,7 @@ int hclDgemmAsync(int64_t M, int64_t N, int64_t K, double alpha, const double* d
         }
         if (!dC) return -10;
         if (ldc < N) return -11;
-        int rc = launch_dgemm_tiles(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, (cudaStream_t)s);
+        int rc = launch_dgemm_tiles(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, (cudaStream_t)s, 0);
         if (rc) return rc;
     }
     return finish_async((cudaStream_t)s, ev);

@@ -60,6 +60,10 @@ def check(C_gpu, C_ref, D, exact):
     (256, 384, 512, 1.0, 0.5, "int"),
     (131, 77, 97, 3.0, 2.0, "int"),               # primes
     (64, 1024, 8, 1.0, 0.0, "int"),
+    (128, 256, 4096, 1.0, 0.5, "uniform"),        # 2 tiles, deep K: 4-CTA cluster split-K (DSMEM reduction)
+    (200, 300, 2061, -1.0, 2.0, "int"),           # 6 tiles, ragged K not a multiple of the split
+    (640, 1024, 1040, 1.0, 0.0, "uniform"),       # 40 tiles: 2-CTA cluster split-K
+    (640, 1024, 1040, 2.0, 1.0, "int"),
 ])
 def test_tile_kernel_matches_oracle(H, M, N, K, alpha, beta, dist):
     import torch
