@@ -52,21 +52,23 @@ typedef void* hclEvent;                 /* a cudaEvent_t  (the paper's hclEvent,
  * Loop structure:  for p < kpanels:  for j < w:  for i < h:  one step computes the C block
  * (rows i*mb .., cols j*nb ..) with the K panel p (k0 = p*kb):   c_ij = alpha*a_i*b_j + beta'*c_ij   (:308)
  * where beta' = beta for p == 0 and 1 afterwards.  Step index idx = i + h*(j + w*p) (:191 for p = 0).
+ * Rows are visited in serpentine order (down the even columns of blocks, up the odd ones) so the A slices
+ * still resident at the end of a column are reused by the next one instead of being uploaded again.
  * Edge slices are ragged (ceil division; the paper only treats equal slices).                       */
 typedef struct hclooc_plan_t {
     int64_t  M, N, K;
     int64_t  mb, nb, kb;          /* rows of an A slice, columns of a B slice, depth of a K panel   */
     int64_t  h, w, kpanels;       /* ceil(M/mb), ceil(N/nb), ceil(K/kb)                             */
     int64_t  n_steps;             /* h * w * kpanels                                                */
-    int32_t  n_sets;              /* (A slice, C block) device buffer pairs, round-robin by step    */
+    int32_t  n_sets;              /* C block device buffers, round-robin by step (the paper has 2)  */
     int32_t  n_bbuf;              /* B slice device buffers (1 = paper's single buffer, 2 = prefetch) */
     int32_t  beta_nonzero;        /* C blocks are uploaded only when 1 (or for K panels p > 0)      */
     int32_t  scale_only;          /* alpha == 0 or K == 0: C = beta*C, A and B never referenced     */
     int32_t  ksplit;              /* CTAs per cluster sharing one tile's K range in the kernel (1, 2, 4) */
-    int32_t  reserved0;
+    int32_t  n_abuf;              /* A slice device buffers: an LRU cache keyed by (row slice, K panel) */
     int64_t  lda_dev, ldb_dev, ldc_dev;  /* leading dimensions of the device buffers (elements)    */
     uint64_t bytes_a_buf, bytes_b_buf, bytes_c_buf;   /* one buffer of each kind                   */
-    uint64_t workspace_bytes;     /* n_bbuf*b + n_sets*(a + c), <= the budget                       */
+    uint64_t workspace_bytes;     /* n_bbuf*b + n_abuf*a + n_sets*c, <= the budget                  */
     uint64_t bytes_h2d, bytes_d2h;/* exactly what the executor enqueues over the host link          */
     uint64_t n_copies_h2d, n_copies_d2h;
     double   flops;               /* 2*M*N*K (:368)                                                 */
@@ -77,6 +79,13 @@ typedef struct hclooc_plan_t {
  * Errors: -1..-3 negative dimension, -7 NULL out, HCLOOC_ERR_BUDGET.                               */
 int hclooc_plan(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zero,
                 size_t device_budget_bytes, hclooc_plan_t* out);
+/* Same, saying where A, B and C live: 0 = pinned host memory (what hclooc_plan assumes), 1 = all three in
+ * device memory: the in-core case (:130, :368) -- nothing is staged, the plan is one step over the caller's
+ * matrices (h = w = 1, no buffers, no traffic).  hclooc_dgemm_ex picks this from the pointers it is given
+ * (device operands that are not 16-byte aligned with even leading dimensions are staged like host ones).
+ * -8: NULL out. */
+int hclooc_plan_ex(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zero,
+                   size_t device_budget_bytes, int operands_on_device, hclooc_plan_t* out);
 
 /* The paper's own rule, kept for reference and tests (:289, worked example :301): EQUAL slices only,
  * working set K*nb + 2*mb*K + 2*mb*nb <= budget_elements, least host-to-device traffic
@@ -96,7 +105,11 @@ int hclMatrixPartitioner(int64_t M, int64_t N, int64_t K, int64_t budget_element
 #define HCLOOC_OP_WAIT    5   /* stream waits for event (hclWaitEvent, :116)                              */
 #define HCLOOC_OP_RECORD  6   /* event recorded in stream (Rec(x), :311)                                  */
 /* streams: 0 = H2D copy stream, 1 = D2H copy stream, 2 + c = compute stream c.
- * buffers: A slice of set s = s; C block of set s = n_sets + s; B slice b = 2*n_sets + b.            */
+ * buffers: A slice buffer a = a; C block buffer c = n_abuf + c; B slice buffer b = n_abuf + n_sets + b.
+ * events:  c = uploads of the step using C buffer c arrived (rA/rC); n_sets + c = its kernel finished (eA);
+ *          2*n_sets + c = C buffer c stored on the host (eC); 3*n_sets + b = B buffer b received (rB);
+ *          3*n_sets + n_bbuf + b = every kernel of the column that read B buffer b finished;
+ *          3*n_sets + 2*n_bbuf + a = the latest kernel that read A buffer a finished.                 */
 typedef struct hclooc_op_t {
     int32_t kind, stream, event;
     int32_t buf, buf2, buf3;
@@ -146,8 +159,9 @@ int hclooc_ctx_get_trace(hclooc_ctx* ctx, hclooc_trace_rec* recs, size_t max_rec
 /* ------------------------------------------------------------------ the operation
  * hclooc_dgemm: C = alpha*A*B + beta*C, synchronous: C is complete in host memory on return.
  *   A: M x K, lda >= K;  B: K x N, ldb >= N;  C: M x N, ldc >= N, updated IN PLACE; A, B read-only.
- *   A, B, C: pinned HOST pointers (the product path).  Device pointers are also accepted (the copies
- *   become device-to-device); that is what bench.py's HBM-resident `value` leg uses.
+ *   A, B, C: pinned HOST pointers (the product path).  Device pointers are also accepted: if all three are
+ *   device memory the call is in-core (one DGEMM on the caller's matrices, nothing staged) -- bench.py's
+ *   HBM-resident `value` leg; a mix is staged through the workspace with device-to-device copies.
  *   device_budget_bytes bounds the sum of all device buffers the call uses (0 = all free HBM minus a
  *   1 GiB margin).  Uses a process-wide default context created on first use.
  *   beta == 0: C is never read (NaN/Inf in C are overwritten).  alpha == 0 or K == 0: A and B are not

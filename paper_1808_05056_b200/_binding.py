@@ -12,7 +12,7 @@ HCL_H2D, HCL_D2H = 0, 1
 
 # every symbol include/hclooc.h declares (tests check the .so exports all of them)
 EXPORTS = [
-    "hclooc_plan", "hclMatrixPartitioner", "hclooc_schedule", "hclooc_ctx_create", "hclooc_ctx_destroy",
+    "hclooc_plan", "hclooc_plan_ex", "hclMatrixPartitioner", "hclooc_schedule", "hclooc_ctx_create", "hclooc_ctx_destroy",
     "hclooc_ctx_set_trace", "hclooc_ctx_get_trace",
     "hclooc_dgemm", "hclooc_dgemm_ex", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
     "hclStreamDestroy", "hclEventDestroy", "hclMemcpy", "hclMemcpyAsync", "hclMemcpy2DAsync",
@@ -27,7 +27,7 @@ class Plan(ctypes.Structure):
                 ("mb", c_int64), ("nb", c_int64), ("kb", c_int64),
                 ("h", c_int64), ("w", c_int64), ("kpanels", c_int64), ("n_steps", c_int64),
                 ("n_sets", c_int32), ("n_bbuf", c_int32), ("beta_nonzero", c_int32), ("scale_only", c_int32),
-                ("ksplit", c_int32), ("reserved0", c_int32),
+                ("ksplit", c_int32), ("n_abuf", c_int32),
                 ("lda_dev", c_int64), ("ldb_dev", c_int64), ("ldc_dev", c_int64),
                 ("bytes_a_buf", c_uint64), ("bytes_b_buf", c_uint64), ("bytes_c_buf", c_uint64),
                 ("workspace_bytes", c_uint64), ("bytes_h2d", c_uint64), ("bytes_d2h", c_uint64),
@@ -71,6 +71,7 @@ def lib():
         L = ctypes.CDLL(_build.build())
         i64, dbl, vp, sz = c_int64, c_double, c_void_p, c_size_t
         L.hclooc_plan.argtypes = [i64, i64, i64, c_int, c_int, sz, POINTER(Plan)]
+        L.hclooc_plan_ex.argtypes = [i64, i64, i64, c_int, c_int, sz, c_int, POINTER(Plan)]
         L.hclMatrixPartitioner.argtypes = [i64, i64, i64, i64, POINTER(i64), POINTER(i64)]
         L.hclooc_schedule.argtypes = [POINTER(Plan), c_int, vp, sz, POINTER(sz)]
         L.hclooc_ctx_create.argtypes = [POINTER(vp), c_int, vp, sz, vp, vp, POINTER(vp), c_int]
@@ -181,6 +182,13 @@ class HostMatrix:
 def hclooc_plan(M, N, K, beta_nonzero, alpha_zero, device_budget_bytes) -> Plan:
     p = Plan()
     _check(lib().hclooc_plan(M, N, K, int(bool(beta_nonzero)), int(bool(alpha_zero)), device_budget_bytes, byref(p)), "hclooc_plan")
+    return p
+
+
+def hclooc_plan_ex(M, N, K, beta_nonzero, alpha_zero, device_budget_bytes, operands_on_device) -> Plan:
+    p = Plan()
+    _check(lib().hclooc_plan_ex(M, N, K, int(bool(beta_nonzero)), int(bool(alpha_zero)), device_budget_bytes,
+                                int(bool(operands_on_device)), byref(p)), "hclooc_plan_ex")
     return p
 
 

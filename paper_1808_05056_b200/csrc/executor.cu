@@ -7,6 +7,7 @@
 // explicit operation list (hclooc_schedule) and then issued verbatim, so the hazard rule of :311
 // ("data stored in device buffers is not overwritten until kernel executions that operate on the
 // data have completed") can be checked on the list itself without a GPU.
+#include <algorithm>
 #include <chrono>
 #include <cstring>
 #include <mutex>
@@ -25,23 +26,32 @@ constexpr int MAX_COMPUTE_STREAMS = 16;
 
 // event ids inside a schedule
 struct EventIds {
-    int n_sets, n_bbuf;
-    int set_ready(int s) const { return s; }                 // rA/rC: A slice (and C block) of set s received
-    int kernel_done(int s) const { return n_sets + s; }      // eA: kernel that used set s finished
-    int c_stored(int s) const { return 2 * n_sets + s; }     // eC: C block of set s is back on the host
-    int b_ready(int b) const { return 3 * n_sets + b; }      // rB: B slice b received
-    int count() const { return 3 * n_sets + n_bbuf; }
+    int n_sets, n_bbuf, n_abuf;
+    int up_ready(int c) const { return c; }                  // rA/rC: the uploads of the step using C buffer c have arrived
+    int kernel_done(int c) const { return n_sets + c; }      // eA: the kernel writing C buffer c finished
+    int c_stored(int c) const { return 2 * n_sets + c; }     // eC: C buffer c is back on the host
+    int b_ready(int b) const { return 3 * n_sets + b; }      // rB: B slice buffer b received
+    int b_free(int b) const { return 3 * n_sets + n_bbuf + b; }  // every kernel of the column that read B buffer b finished
+    int a_free(int a) const { return 3 * n_sets + 2 * n_bbuf + a; }  // the latest kernel that read A buffer a finished
+    int count() const { return 3 * n_sets + 2 * n_bbuf + n_abuf; }
 };
 
-int64_t chunks_for(int64_t h, int64_t kk) { return std::max<int64_t>(1, std::min(h, kk)); }
-
 // Expand the plan into the operation list.  This is the single source of truth for the executor.
+//
+// Order of the steps: columns of blocks one after the other (:189-190), rows in SERPENTINE order (down
+// the even columns, up the odd ones) so that the A slices still resident when a column ends are the
+// first ones the next column needs.  A slices live in an LRU cache of n_abuf device buffers keyed by
+// (row slice, K panel); C blocks use n_sets buffers round-robin by step.
 void build_schedule(const hclooc_plan_t& P, int ncs, std::vector<hclooc_op_t>& ops) {
     ops.clear();
     if (P.n_steps == 0) return;
-    const EventIds ev{P.n_sets, P.n_bbuf};
+    const int n_sets = P.n_sets, n_abuf = std::max(1, (int)P.n_abuf);
+    const EventIds ev{n_sets, P.n_bbuf, n_abuf};
     const bool scale_only = P.scale_only != 0;
-    std::vector<char> set_used(P.n_sets, 0), set_stored(P.n_sets, 0);
+    std::vector<char> set_used(n_sets, 0), set_stored(n_sets, 0);
+    // A-slice cache
+    struct ABuf { int64_t row = -1, panel = -1; int64_t last_use = -1; int ready_ev = -1; bool read = false; };
+    std::vector<ABuf> acache(n_abuf);
     auto push = [&](int kind, int stream, int event) -> hclooc_op_t& {
         hclooc_op_t o;
         std::memset(&o, 0, sizeof(o));
@@ -49,11 +59,13 @@ void build_schedule(const hclooc_plan_t& P, int ncs, std::vector<hclooc_op_t>& o
         ops.push_back(o);
         return ops.back();
     };
-    auto bbuf_id = [&](int b) { return 2 * P.n_sets + b; };
-    // wait until every kernel issued so far has finished (latest record of each set's kernel_done)
+    auto cbuf_id = [&](int c) { return n_abuf + c; };
+    auto bbuf_id = [&](int b) { return n_abuf + n_sets + b; };
+    // wait until every kernel issued so far has finished (the latest kernel of a C buffer finishes after
+    // all earlier kernels of that buffer: each waited for the download of its predecessor)
     auto wait_all_kernels = [&](int stream) {
-        for (int s = 0; s < P.n_sets; ++s)
-            if (set_used[s]) push(HCLOOC_OP_WAIT, stream, ev.kernel_done(s));
+        for (int c = 0; c < n_sets; ++c)
+            if (set_used[c]) push(HCLOOC_OP_WAIT, stream, ev.kernel_done(c));
     };
     auto load_b = [&](int64_t p, int64_t j, int b, int64_t kr0, int64_t krows) {
         hclooc_op_t& o = push(HCLOOC_OP_H2D_B, 0, -1);
@@ -62,68 +74,129 @@ void build_schedule(const hclooc_plan_t& P, int ncs, std::vector<hclooc_op_t>& o
         o.c0 = j * P.nb; o.nc = std::min(P.nb, P.N - j * P.nb);
         o.dev_r0 = kr0;
     };
+    struct Step { int64_t sl, p, j, i, t, seq; int abuf; bool a_hit; bool uploaded; };
     const int64_t slabs = P.w * P.kpanels;
-    int64_t step = 0;
+    auto make_step = [&](int64_t sl, int64_t t, int64_t seq) {
+        Step s{};
+        s.sl = sl; s.p = sl / P.w; s.j = sl % P.w; s.t = t; s.seq = seq;
+        s.i = (sl & 1) ? P.h - 1 - t : t;
+        s.abuf = -1; s.a_hit = false; s.uploaded = false;
+        return s;
+    };
+    // ---- the uploads of one step on the H2D stream: S(a_i) unless the slice is cached, S(c_ij) if C is read
+    auto issue_uploads = [&](Step& s) {
+        const int c = (int)(s.seq % n_sets);
+        const int64_t k0 = s.p * P.kb, kk = scale_only ? 0 : std::min(P.kb, P.K - k0);
+        const int64_t i0 = s.i * P.mb, mi = std::min(P.mb, P.M - i0);
+        const int64_t j0 = s.j * P.nb, nj = std::min(P.nb, P.N - j0);
+        const bool cload = P.beta_nonzero || s.p > 0;
+        const int64_t idx = s.i + P.h * (s.j + P.w * s.p);
+        bool any = false;
+        if (!scale_only) {
+            int hit = -1, victim = 0;
+            for (int a = 0; a < n_abuf; ++a) {
+                if (acache[a].row == s.i && acache[a].panel == s.p) hit = a;
+                if (acache[a].last_use < acache[victim].last_use) victim = a;
+            }
+            if (hit >= 0) { s.abuf = hit; s.a_hit = true; }
+            else {
+                ABuf& ab = acache[victim];
+                if (ab.read) push(HCLOOC_OP_WAIT, 0, ev.a_free(victim));                  // Wait(eA): buffer free (:311)
+                ab.read = false;
+                hclooc_op_t& o = push(HCLOOC_OP_H2D_A, 0, -1);                            // S(a_i)
+                o.buf = victim; o.r0 = i0; o.nr = mi; o.c0 = k0; o.nc = kk; o.step = idx;
+                ab.row = s.i; ab.panel = s.p; ab.ready_ev = ev.up_ready(c);
+                s.abuf = victim;
+                any = true;
+            }
+            acache[s.abuf].last_use = s.seq;
+        }
+        if (cload) {
+            if (set_stored[c]) push(HCLOOC_OP_WAIT, 0, ev.c_stored(c));                  // Wait(eC): block is back on the host
+            hclooc_op_t& o = push(HCLOOC_OP_H2D_C, 0, -1);                                // S(c_ij)
+            o.buf = cbuf_id(c); o.r0 = i0; o.nr = mi; o.c0 = j0; o.nc = nj; o.step = idx;
+            any = true;
+        }
+        if (any) push(HCLOOC_OP_RECORD, 0, ev.up_ready(c));                               // Rec(rA), Rec(rC)
+        s.uploaded = any;
+        return any;
+    };
+    // ---- DGEMM on a compute stream, then R(c_ij) on the D2H stream
+    auto issue_compute = [&](Step& s, bool any_upload, int b, bool last_of_slab) {
+        const int c = (int)(s.seq % n_sets);
+        const int cs = 2 + (int)(s.seq % ncs);
+        const int64_t k0 = s.p * P.kb, kk = scale_only ? 0 : std::min(P.kb, P.K - k0);
+        const int64_t i0 = s.i * P.mb, mi = std::min(P.mb, P.M - i0);
+        const int64_t j0 = s.j * P.nb, nj = std::min(P.nb, P.N - j0);
+        const bool cload = P.beta_nonzero || s.p > 0;
+        const int64_t idx = s.i + P.h * (s.j + P.w * s.p);
+        if (any_upload) push(HCLOOC_OP_WAIT, cs, ev.up_ready(c));                         // Wait(rA), Wait(rC)
+        if (!scale_only && s.a_hit) {
+            // cached slice: its upload arrived, and this kernel is ordered after the previous reader so that
+            // the latest record of a_free covers every kernel that read the buffer
+            if (acache[s.abuf].ready_ev != ev.up_ready(c)) push(HCLOOC_OP_WAIT, cs, acache[s.abuf].ready_ev);
+            if (acache[s.abuf].read) push(HCLOOC_OP_WAIT, cs, ev.a_free(s.abuf));
+        }
+        if (!scale_only) push(HCLOOC_OP_WAIT, cs, ev.b_ready(b));                         // Wait(rB)
+        if (!cload && set_stored[c]) push(HCLOOC_OP_WAIT, cs, ev.c_stored(c));            // C buffer still draining
+        {
+            hclooc_op_t& o = push(HCLOOC_OP_GEMM, cs, -1);
+            o.buf = scale_only ? -1 : s.abuf; o.buf2 = scale_only ? -1 : bbuf_id(b); o.buf3 = cbuf_id(c);
+            o.r0 = i0; o.nr = mi; o.c0 = j0; o.nc = nj; o.k0 = k0; o.kk = kk; o.step = idx;
+            o.beta = (s.p > 0) ? 1.0 : -1.0;             // -1: "use the caller's beta" (resolved by the executor)
+        }
+        push(HCLOOC_OP_RECORD, cs, ev.kernel_done(c));                                    // Rec(eA)
+        set_used[c] = 1;
+        if (!scale_only) { push(HCLOOC_OP_RECORD, cs, ev.a_free(s.abuf)); acache[s.abuf].read = true; }
+        push(HCLOOC_OP_WAIT, 1, ev.kernel_done(c));
+        if (last_of_slab && P.n_bbuf == 2 && !scale_only) push(HCLOOC_OP_RECORD, 1, ev.b_free(b));  // the column's kernels are done
+        {
+            hclooc_op_t& o = push(HCLOOC_OP_D2H_C, 1, -1);                                // R(c_ij)
+            o.buf = cbuf_id(c); o.r0 = i0; o.nr = mi; o.c0 = j0; o.nc = nj; o.step = idx;
+        }
+        push(HCLOOC_OP_RECORD, 1, ev.c_stored(c));                                        // Rec(eC)
+        set_stored[c] = 1;
+    };
+
+    // With one B buffer the uploads of the first steps of a column go out BEFORE the B reload, so the link
+    // has work while the kernels of the previous column drain (the paper leaves that reload exposed, :236-242).
+    const int64_t pre = (P.n_bbuf == 1 && !scale_only) ? early_uploads(P.h, n_sets, n_abuf) : 0;
+    std::vector<Step> early;
+    int64_t seq = 0;
     for (int64_t sl = 0; sl < slabs; ++sl) {
         const int64_t p = sl / P.w, j = sl % P.w;
-        const int64_t k0 = p * P.kb, kk = scale_only ? 0 : std::min(P.kb, P.K - k0);
-        const int64_t j0 = j * P.nb, nj = std::min(P.nb, P.N - j0);
+        const int64_t kk = scale_only ? 0 : std::min(P.kb, P.K - p * P.kb);
         const int b = (int)(sl % P.n_bbuf);
-        const bool cload = P.beta_nonzero || p > 0;
-        const double beta_flag = (p > 0) ? 1.0 : -1.0;   // -1: "use the caller's beta" (resolved by the executor)
+        early.clear();
         if (!scale_only && (P.n_bbuf == 1 || sl == 0)) {
-            // S(b_j): whole slice; with a single buffer every kernel of the previous column must be done (:236-242)
-            if (sl > 0) wait_all_kernels(0);
+            if (sl > 0) {
+                for (int64_t t = 0; t < pre; ++t) {
+                    early.push_back(make_step(sl, t, seq + t));
+                    issue_uploads(early.back());
+                }
+                wait_all_kernels(0);             // S(b_j) overwrites the single buffer: every kernel of the previous column is done
+            }
             load_b(p, j, b, 0, kk);
             push(HCLOOC_OP_RECORD, 0, ev.b_ready(b));
         }
-        // next slice (prefetched in chunks during this column when there are two B buffers)
+        // next slice, prefetched in chunks during this column when there are two B buffers
         const bool prefetch = !scale_only && P.n_bbuf == 2 && sl + 1 < slabs;
         const int64_t np = (sl + 1) / P.w, nj_idx = (sl + 1) % P.w;
         const int64_t nkk = prefetch ? std::min(P.kb, P.K - np * P.kb) : 0;
-        const int64_t nchunks = prefetch ? chunks_for(P.h, nkk) : 0;
-        for (int64_t i = 0; i < P.h; ++i, ++step) {
-            const int set = (int)(step % P.n_sets);
-            const int cs = 2 + (int)(step % ncs);
-            const int64_t i0 = i * P.mb, mi = std::min(P.mb, P.M - i0);
-            // ---- uploads for this step on the H2D stream
-            if (!scale_only) {
-                if (set_used[set]) push(HCLOOC_OP_WAIT, 0, ev.kernel_done(set));     // Wait(eA): buffer free
-                hclooc_op_t& o = push(HCLOOC_OP_H2D_A, 0, -1);                       // S(a_i)
-                o.buf = set; o.r0 = i0; o.nr = mi; o.c0 = k0; o.nc = kk; o.step = step;
+        int64_t pf_i0 = 0, nchunks = 0;
+        if (prefetch) prefetch_layout(P.h, nkk, n_sets, &pf_i0, &nchunks);
+        const int nb_buf = (int)((sl + 1) % P.n_bbuf);
+        for (int64_t t = 0; t < P.h; ++t, ++seq) {
+            Step s = (t < (int64_t)early.size()) ? early[t] : make_step(sl, t, seq);
+            const bool any = (t < (int64_t)early.size()) ? s.uploaded : issue_uploads(s);
+            if (prefetch && t >= pf_i0 && t < pf_i0 + nchunks) {
+                const int64_t ci = t - pf_i0;
+                if (ci == 0 && sl >= 1) push(HCLOOC_OP_WAIT, 0, ev.b_free(nb_buf));   // last read by the column before this one
+                const int64_t r_lo = nkk * ci / nchunks, r_hi = nkk * (ci + 1) / nchunks;
+                load_b(np, nj_idx, nb_buf, r_lo, r_hi - r_lo);
+                if (ci == nchunks - 1) push(HCLOOC_OP_RECORD, 0, ev.b_ready(nb_buf));
             }
-            if (cload) {
-                if (set_stored[set]) push(HCLOOC_OP_WAIT, 0, ev.c_stored(set));      // Wait(eC): block is back on the host
-                hclooc_op_t& o = push(HCLOOC_OP_H2D_C, 0, -1);                       // S(c_ij)
-                o.buf = P.n_sets + set; o.r0 = i0; o.nr = mi; o.c0 = j0; o.nc = nj; o.step = step;
-            }
-            if (!scale_only || cload) push(HCLOOC_OP_RECORD, 0, ev.set_ready(set));  // Rec(rA), Rec(rC)
-            // ---- one chunk of the next B slice, interleaved with the uploads
-            if (prefetch && i < nchunks) {
-                if (i == 0) wait_all_kernels(0);   // the other B buffer was last read by the previous column's kernels
-                const int64_t r_lo = nkk * i / nchunks, r_hi = nkk * (i + 1) / nchunks;
-                load_b(np, nj_idx, (int)((sl + 1) % P.n_bbuf), r_lo, r_hi - r_lo);
-                if (i == nchunks - 1) push(HCLOOC_OP_RECORD, 0, ev.b_ready((int)((sl + 1) % P.n_bbuf)));
-            }
-            // ---- DGEMM on a compute stream
-            if (!scale_only || cload) push(HCLOOC_OP_WAIT, cs, ev.set_ready(set));   // Wait(rA), Wait(rC)
-            if (!scale_only) push(HCLOOC_OP_WAIT, cs, ev.b_ready(b));                // Wait(rB)
-            if (!cload && set_stored[set]) push(HCLOOC_OP_WAIT, cs, ev.c_stored(set));  // C buffer still draining
-            {
-                hclooc_op_t& o = push(HCLOOC_OP_GEMM, cs, -1);
-                o.buf = scale_only ? -1 : set; o.buf2 = scale_only ? -1 : bbuf_id(b); o.buf3 = P.n_sets + set;
-                o.r0 = i0; o.nr = mi; o.c0 = j0; o.nc = nj; o.k0 = k0; o.kk = kk; o.step = step; o.beta = beta_flag;
-            }
-            push(HCLOOC_OP_RECORD, cs, ev.kernel_done(set));                          // Rec(eA)
-            set_used[set] = 1;
-            // ---- download on the D2H stream
-            push(HCLOOC_OP_WAIT, 1, ev.kernel_done(set));
-            {
-                hclooc_op_t& o = push(HCLOOC_OP_D2H_C, 1, -1);                        // R(c_ij)
-                o.buf = P.n_sets + set; o.r0 = i0; o.nr = mi; o.c0 = j0; o.nc = nj; o.step = step;
-            }
-            push(HCLOOC_OP_RECORD, 1, ev.c_stored(set));                              // Rec(eC)
-            set_stored[set] = 1;
+            issue_compute(s, any, b, t == P.h - 1);
         }
     }
 }
@@ -225,12 +298,13 @@ int default_ctx(hclooc_ctx** out) {
     return HCLOOC_OK;
 }
 
-// 0 = ok, HCLOOC_ERR_NOT_PINNED if pageable host memory
-int check_resident(const void* p) {
+// 0 = ok, HCLOOC_ERR_NOT_PINNED if pageable host memory; *on_device is cleared unless p is device memory
+int check_resident(const void* p, bool* on_device) {
     cudaPointerAttributes at;
     cudaError_t e = cudaPointerGetAttributes(&at, p);
     if (e != cudaSuccess) { cudaGetLastError(); return HCLOOC_ERR_NOT_PINNED; }
     if (at.type == cudaMemoryTypeUnregistered) return HCLOOC_ERR_NOT_PINNED;
+    if (at.type != cudaMemoryTypeDevice) *on_device = false;
     return HCLOOC_OK;
 }
 
@@ -275,8 +349,9 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
     if (!ctx && (rc = default_ctx(&ctx))) return rc;
     std::lock_guard<std::mutex> lk(ctx->mu);
     HCL_CUDA(cudaSetDevice(ctx->device));
-    if ((rc = check_resident(C))) return rc;
-    if (!scale_only && ((rc = check_resident(A)) || (rc = check_resident(B)))) return rc;
+    bool on_device = true;
+    if ((rc = check_resident(C, &on_device))) return rc;
+    if (!scale_only && ((rc = check_resident(A, &on_device)) || (rc = check_resident(B, &on_device)))) return rc;
 
     // ---------------------------------------------------------------- S1 plan
     size_t budget = device_budget_bytes;
@@ -290,8 +365,28 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
         budget = fr > 2 * margin ? fr - margin : fr / 2;
     }
     hclooc_plan_t P;
-    rc = hclooc_plan(M, N, K, beta != 0.0, alpha == 0.0, budget, &P);
+    // in-core case: every operand already in device memory and addressable by the tile kernel as it is
+    const bool aligned = (((uintptr_t)C & 15u) == 0) && (ldc % 2 == 0) &&
+                         (scale_only || ((((uintptr_t)A | (uintptr_t)B) & 15u) == 0 && lda % 2 == 0 && ldb % 2 == 0));
+    const bool in_core = on_device && aligned && M <= 0x7fffffffLL && N <= 0x7fffffffLL && K <= 0x7fffffffLL;
+    rc = hclooc_plan_ex(M, N, K, beta != 0.0, alpha == 0.0, budget, in_core ? 1 : 0, &P);
     if (rc) return rc;
+    if (in_core) {
+        const auto t0 = std::chrono::steady_clock::now();
+        rc = launch_dgemm_tiles(M, N, scale_only ? 0 : K, scale_only ? 0.0 : alpha, A, lda, B, ldb, beta, C, ldc, ctx->s_compute[0], P.ksplit);
+        const auto t1 = std::chrono::steady_clock::now();
+        cudaError_t e = cudaStreamSynchronize(ctx->s_compute[0]);
+        if (rc) return rc;
+        if (e != cudaSuccess) return cuda_fail(e);
+        ctx->trace_recs.clear();
+        if (stats) {
+            stats->plan = P;
+            stats->n_kernels = 1;
+            stats->t_enqueue_s = std::chrono::duration<double>(t1 - t0).count();
+            stats->t_total_s = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_begin).count();
+        }
+        return HCLOOC_OK;
+    }
     if (P.workspace_bytes > ctx->workspace_bytes) {
         if (ctx->workspace && !ctx->owns_workspace) return HCLOOC_ERR_BUDGET;
         if (ctx->workspace) { HCL_CUDA(cudaDeviceSynchronize()); cudaFree(ctx->workspace); ctx->workspace = nullptr; ctx->workspace_bytes = 0; }
@@ -307,18 +402,16 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
         base += 1024 - mis;
         if (P.workspace_bytes + 1024 - mis > ctx->workspace_bytes) return HCLOOC_ERR_BUDGET;
     }
-    std::vector<double*> bufs(2 * P.n_sets + P.n_bbuf);
+    std::vector<double*> bufs(P.n_abuf + P.n_sets + P.n_bbuf);
     {
         uint8_t* q = base;
-        for (int b = 0; b < P.n_bbuf; ++b) { bufs[2 * P.n_sets + b] = (double*)q; q += P.bytes_b_buf; }
-        for (int s = 0; s < P.n_sets; ++s) {
-            bufs[s] = (double*)q; q += P.bytes_a_buf;
-            bufs[P.n_sets + s] = (double*)q; q += P.bytes_c_buf;
-        }
+        for (int b = 0; b < P.n_bbuf; ++b) { bufs[P.n_abuf + P.n_sets + b] = (double*)q; q += P.bytes_b_buf; }
+        for (int a = 0; a < P.n_abuf; ++a) { bufs[a] = (double*)q; q += P.bytes_a_buf; }
+        for (int c = 0; c < P.n_sets; ++c) { bufs[P.n_abuf + c] = (double*)q; q += P.bytes_c_buf; }
         if ((size_t)(q - base) != P.workspace_bytes) return HCLOOC_ERR_INTERNAL;
     }
     // ---------------------------------------------------------------- events
-    const size_t n_events = 3 * (size_t)P.n_sets + P.n_bbuf;
+    const size_t n_events = 3 * (size_t)P.n_sets + 2 * (size_t)P.n_bbuf + (size_t)P.n_abuf;
     while (ctx->events.size() < n_events) {
         cudaEvent_t e;
         HCL_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));

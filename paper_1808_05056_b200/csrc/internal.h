@@ -38,6 +38,29 @@ int launch_dgemm_tiles(int64_t M, int64_t N, int64_t K, double alpha, const doub
 // K split (cluster size) worth using when `tiles_in_flight` tiles can run concurrently
 int dgemm_auto_ksplit(int64_t tiles_in_flight, int64_t K);
 
+// Where the chunks of a prefetched B slice sit inside the previous column of steps (two B buffers): the
+// first chunk goes out with the i0-th step of that column -- late enough that the kernels of the column
+// before it, the last readers of the target buffer, have normally drained -- and one chunk follows per step.
+// Shared by the planner (copy counts) and the executor (the schedule) so the two cannot disagree.
+inline void prefetch_layout(int64_t h, int64_t kk, int n_sets, int64_t* i0, int64_t* nchunks) {
+    const int64_t first = h > 1 ? (h - 1 < (int64_t)n_sets ? h - 1 : (int64_t)n_sets) : 0;
+    int64_t n = h - first;
+    if (n > kk) n = kk;
+    if (n < 1) n = 1;
+    *i0 = first;
+    *nchunks = n;
+}
+
+// With a single B buffer, the uploads of this many steps of the next column are issued BEFORE the B reload
+// (they keep the link busy while the previous column's kernels drain); the rest of the C buffers stay free so
+// that uploads can continue right after the reload while those first kernels run.
+inline int64_t early_uploads(int64_t h, int n_sets, int n_abuf) {
+    int64_t pre = n_sets - 4;
+    if (pre > n_abuf - 1) pre = n_abuf - 1;
+    if (pre > h) pre = h;
+    return pre < 0 ? 0 : pre;
+}
+
 // number of CTAs the tile kernel uses for an M x N output (for stats / tests)
 int64_t dgemm_tile_count(int64_t M, int64_t N);
 

@@ -42,7 +42,7 @@ const MachineModel& machine_model() {
         env_or("HCLOOC_H2D_GBPS", 55.5) * 1e9,
         env_or("HCLOOC_D2H_GBPS", 51.5) * 1e9,
         env_or("HCLOOC_DUPLEX_GBPS", 88.0) * 1e9,
-        env_or("HCLOOC_COPY_LATENCY_US", 4.0) * 1e-6,
+        env_or("HCLOOC_COPY_LATENCY_US", 8.0) * 1e-6, // per copy inside the pipeline (event waits between copies); 4-5 us back to back
         env_or("HCLOOC_LAUNCH_LATENCY_US", 5.0) * 1e-6,
     };
     return mm;
@@ -52,38 +52,50 @@ namespace {
 
 struct Cand {
     int64_t mb, nb, kb, h, w, kpanels;
-    int n_sets, n_bbuf, ksplit;
+    int n_sets, n_abuf, n_bbuf, ksplit;
     int64_t lda_dev, ldb_dev, ldc_dev;
     uint64_t a_bytes, b_bytes, c_bytes, ws_bytes;
     uint64_t bytes_h2d, bytes_d2h, n_h2d, n_d2h;
     double t_flop, t_link, t_model;
 };
 
-// Number of chunks the executor splits a prefetched B slice into (one per step of the previous
-// column, so the prefetch interleaves with that column's A/C uploads).
-int64_t prefetch_chunks(int64_t h, int64_t kk) { return std::max<int64_t>(1, std::min(h, kk)); }
-
+// Exact host<->device traffic of the schedule the executor builds from this candidate (executor.cu
+// build_schedule): columns of blocks in order, rows in serpentine order, A slices in an LRU cache of
+// n_abuf buffers -- so at every column switch inside a K panel the min(n_abuf, h) slices at the turning
+// end are reused, not uploaded again.
 void fill_traffic(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool scale_only) {
     const uint64_t MN = (uint64_t)M * (uint64_t)N;
     const uint64_t steps = (uint64_t)c.h * c.w * c.kpanels;
-    const bool cload0 = beta_nz;
     uint64_t el_h2d = 0, n_h2d = 0;
     if (!scale_only) {
-        el_h2d += (uint64_t)c.w * (uint64_t)M * (uint64_t)K;       // every A slice once per column of blocks
-        el_h2d += (uint64_t)K * (uint64_t)N;                       // every B slice once
-        n_h2d += steps;                                            // one A copy per step
+        const int64_t reuse = std::min<int64_t>(c.n_abuf, c.h);                 // slices reused per column switch
+        const int64_t rows_top = std::min<int64_t>(M, reuse * c.mb);            // rows of the first `reuse` slices
+        const int64_t rows_bottom = M - (c.h - reuse) * c.mb;                   // rows of the last `reuse` slices
+        for (int64_t sl = 0; sl < c.w * c.kpanels; ++sl) {
+            const int64_t p = sl / c.w, j = sl % c.w;
+            const int64_t kk = std::min(c.kb, K - p * c.kb);
+            if (j == 0) { el_h2d += (uint64_t)M * kk; n_h2d += c.h; }           // first column of a panel: every slice
+            else {
+                // column sl-1 ended at the bottom when it ran downwards (even), at the top otherwise
+                const int64_t kept = ((sl - 1) & 1) ? rows_top : rows_bottom;
+                el_h2d += (uint64_t)(M - kept) * kk;
+                n_h2d += c.h - reuse;
+            }
+        }
+        el_h2d += (uint64_t)K * (uint64_t)N;                                    // every B slice once
         const uint64_t slabs = (uint64_t)c.w * c.kpanels;
         if (c.n_bbuf == 1) n_h2d += slabs;
         else {
-            n_h2d += 1;                                            // first slice in one piece
-            for (int64_t p = 0; p < c.kpanels; ++p) {
-                const int64_t kk = std::min(c.kb, K - p * c.kb);
-                n_h2d += (uint64_t)c.w * prefetch_chunks(c.h, kk);
+            n_h2d += 1;                                                         // first slice in one piece
+            for (uint64_t sl = 1; sl < slabs; ++sl) {
+                const int64_t kk = std::min(c.kb, K - (int64_t)(sl / c.w) * c.kb);
+                int64_t i0, nch;
+                prefetch_layout(c.h, kk, c.n_sets, &i0, &nch);
+                n_h2d += nch;
             }
-            n_h2d -= prefetch_chunks(c.h, std::min(c.kb, K));      // slice 0 was counted as chunks too
         }
     }
-    if (cload0) { el_h2d += MN; n_h2d += (uint64_t)c.h * c.w; }
+    if (beta_nz) { el_h2d += MN; n_h2d += (uint64_t)c.h * c.w; }
     if (c.kpanels > 1) { el_h2d += (uint64_t)(c.kpanels - 1) * MN; n_h2d += (uint64_t)(c.kpanels - 1) * c.h * c.w; }
     c.bytes_h2d = 8 * el_h2d;
     c.n_h2d = n_h2d;
@@ -91,8 +103,7 @@ void fill_traffic(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool s
     c.n_d2h = steps;
 }
 
-void cost(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool scale_only) {
-    const MachineModel& mm = machine_model();
+void cost(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool scale_only, const MachineModel& mm) {
     fill_traffic(c, M, N, K, beta_nz, scale_only);
     const double steps = (double)c.h * c.w * c.kpanels;
     const double flops = scale_only ? 0.0 : 2.0 * (double)M * (double)N * (double)K;
@@ -103,28 +114,41 @@ void cost(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool scale_onl
     const double tile_rows = (double)((c.h - 1) * ceil_div(c.mb, TILE) + ceil_div(m_last, TILE));
     const double tile_cols = (double)((c.w - 1) * ceil_div(c.nb, TILE) + ceil_div(n_last, TILE));
     const double pad_eff = ((double)M * (double)N) / (tile_rows * tile_cols * (double)(TILE * TILE));
-    // too few tiles in flight to fill the SMs: a cluster of 2 or 4 CTAs shares each tile's K range
+    // too few tiles in flight to fill the SMs: a cluster of 2 or 4 CTAs shares each tile's K range.  When the
+    // link is the bound the kernels of successive steps hardly overlap, so one step's tiles are all there is.
     const int force_ks = (int)env_or("HCLOOC_FORCE_KSPLIT", 0);
-    c.ksplit = scale_only ? 1 : (force_ks ? force_ks : dgemm_auto_ksplit((int64_t)(std::max(1, c.n_sets - 2) * tiles_step), c.kb));
-    const double in_flight = std::max(1, c.n_sets - 2) * tiles_step * c.ksplit;
-    double fill = std::min(1.0, in_flight / NUM_SMS);
-    if (tiles_step >= NUM_SMS) fill = std::min(fill, 0.98);
     c.t_flop = flops / mm.fp64_flops;
-    const double t_compute = c.t_flop / std::max(1e-3, pad_eff * fill) + steps * 1e-6;
     const double t_in = c.bytes_h2d / mm.h2d_Bps + c.n_h2d * mm.copy_latency_s;
     const double t_out = c.bytes_d2h / mm.d2h_Bps + c.n_d2h * mm.copy_latency_s;
     c.t_link = std::max(std::max(t_in, t_out), (double)(c.bytes_h2d + c.bytes_d2h) / mm.duplex_Bps);
+    const bool link_bound = c.t_link > c.t_flop / std::max(1e-3, pad_eff);
+    const double steps_in_flight = link_bound ? 1.0 : (double)std::max(1, c.n_sets - 2);
+    c.ksplit = scale_only ? 1 : (force_ks ? force_ks : dgemm_auto_ksplit((int64_t)(steps_in_flight * tiles_step), c.kb));
+    const double in_flight = std::max(1, c.n_sets - 2) * tiles_step * c.ksplit;
+    double fill = std::min(1.0, in_flight / NUM_SMS);
+    if (tiles_step >= NUM_SMS) fill = std::min(fill, 0.98);
+    const double t_compute = c.t_flop / std::max(1e-3, pad_eff * fill) + steps * 1e-6;
     const bool cload = beta_nz || c.kpanels > 1;
     const double t_pro = ((double)c.b_bytes + (double)c.a_bytes + (cload ? (double)c.c_bytes : 0.0)) / mm.h2d_Bps + 3 * mm.copy_latency_s;
-    const double t_step = t_compute / std::max(1.0, steps);
+    // one step's kernel running alone: what the link waits for when a column drains, and the tail of the call
+    const double sms_step = std::min<double>(NUM_SMS, tiles_step * c.ksplit);
+    const double t_kernel = (flops / std::max(1.0, steps)) / (mm.fp64_flops * sms_step / NUM_SMS) + mm.launch_latency_s;
     const double switches = (double)c.w * c.kpanels - 1.0;
     double comp_path = t_pro + t_compute;
     double link_path = c.t_link;
     if (c.n_bbuf == 1) {
         comp_path += switches * ((double)c.b_bytes / mm.h2d_Bps);   // compute idles while the next B slice loads
-        link_path += switches * t_step * std::min<double>(c.n_sets, 3);  // link idles while the column drains
+        // the link idles (a) while the last kernels of a column drain before S(b_j) may overwrite the buffer,
+        // less the uploads issued ahead of the reload, and (b) after the reload once every C buffer is held by
+        // a step whose kernel has only just started
+        const double t_up = ((double)c.bytes_h2d - 8.0 * (double)K * (double)N) / std::max(1.0, steps) / mm.h2d_Bps + mm.copy_latency_s;
+        const double t_cup = cload ? (double)c.c_bytes / mm.h2d_Bps + mm.copy_latency_s : t_up;
+        const double pre = (double)early_uploads(c.h, c.n_sets, c.n_abuf);
+        const double drain = std::max(0.0, t_kernel - pre * t_cup);
+        const double refill = std::max(0.0, t_kernel + (double)c.c_bytes / mm.d2h_Bps - std::max(0.0, c.n_sets - pre - 1.0) * t_up);
+        link_path += switches * (drain + refill);
     }
-    const double t_tail = t_step * std::max(1.0, tiles_step / NUM_SMS > 1 ? 1.0 : 1.0) + (double)c.c_bytes / mm.d2h_Bps + mm.copy_latency_s;
+    const double t_tail = t_kernel + (double)c.c_bytes / mm.d2h_Bps + mm.copy_latency_s;
     // imperfect overlap: the shorter path still costs a fraction of its length (bursty uploads, shared
     // DMA/HBM resources), which also keeps plans away from the edge where link time ~ compute time
     c.t_model = std::max(comp_path, link_path) + OVERLAP_PENALTY * std::min(comp_path, link_path) + t_tail + mm.launch_latency_s;
@@ -137,16 +161,33 @@ using namespace hclooc;
 
 extern "C" int hclooc_plan(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zero,
                            size_t device_budget_bytes, hclooc_plan_t* out) {
+    return hclooc_plan_ex(M, N, K, beta_nonzero, alpha_zero, device_budget_bytes, 0, out);
+}
+
+extern "C" int hclooc_plan_ex(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zero,
+                              size_t device_budget_bytes, int operands_on_device, hclooc_plan_t* out) {
+    const MachineModel& mm = machine_model();
     if (M < 0) return -1;
     if (N < 0) return -2;
     if (K < 0) return -3;
-    if (!out) return -7;
+    if (!out) return operands_on_device ? -8 : -7;
     std::memset(out, 0, sizeof(*out));
     out->M = M; out->N = N; out->K = K;
     out->beta_nonzero = beta_nonzero ? 1 : 0;
     const bool scale_only = (alpha_zero != 0) || (K == 0);
     out->scale_only = scale_only ? 1 : 0;
     if (M == 0 || N == 0) return HCLOOC_OK;                       // nothing to do: zero steps
+    if (operands_on_device) {
+        // the in-core case (the switch to out-of-core happens only when the matrices do not
+        // fit): nothing to stage, one DGEMM over the caller's matrices, no workspace
+        out->mb = M; out->nb = N; out->kb = scale_only ? 0 : K;
+        out->h = out->w = out->kpanels = out->n_steps = 1;
+        out->ksplit = scale_only ? 1 : dgemm_auto_ksplit(dgemm_tile_count(M, N), K);
+        out->flops = scale_only ? 0.0 : 2.0 * (double)M * (double)N * (double)K;
+        out->t_flop_s = out->flops / mm.fp64_flops;
+        out->t_model_s = out->t_flop_s + mm.launch_latency_s;
+        return HCLOOC_OK;
+    }
     const bool beta_nz = beta_nonzero != 0;
     const int64_t Keff = scale_only ? 0 : K;
     const uint64_t S = (uint64_t)device_budget_bytes;
@@ -154,6 +195,7 @@ extern "C" int hclooc_plan(int64_t M, int64_t N, int64_t K, int beta_nonzero, in
     // experiment knobs (not part of the ABI): force parts of the plan
     const int64_t force_nb = (int64_t)env_or("HCLOOC_FORCE_NB", 0), force_mb = (int64_t)env_or("HCLOOC_FORCE_MB", 0);
     const int force_sets = (int)env_or("HCLOOC_FORCE_SETS", 0), force_bbuf = (int)env_or("HCLOOC_FORCE_BBUF", 0);
+    const int64_t force_abuf = (int64_t)env_or("HCLOOC_FORCE_ABUF", 0);
     bool found = false;
     Cand best{};
     static const int set_choices[] = {2, 3, 4, 5, 6, 7, 8, 10, 12};
@@ -203,9 +245,16 @@ extern "C" int hclooc_plan(int64_t M, int64_t N, int64_t K, int beta_nonzero, in
                         c.a_bytes = scale_only ? 0 : round_up((uint64_t)c.mb * lda_dev * 8, BUF_ALIGN);
                         c.b_bytes = b_bytes;
                         c.c_bytes = round_up((uint64_t)c.mb * ldc_dev * 8, BUF_ALIGN);
+                        c.n_abuf = scale_only ? 0 : c.n_sets;
                         c.ws_bytes = (uint64_t)n_bbuf * b_bytes + (uint64_t)c.n_sets * (c.a_bytes + c.c_bytes);
                         if (c.ws_bytes > S) continue;
-                        cost(c, M, N, Keff, beta_nz, scale_only);
+                        if (!scale_only && c.w > 1 && c.a_bytes > 0) {
+                            // spare budget holds more A slices: more reuse at every column switch
+                            const int64_t extra = std::min<int64_t>((int64_t)((S - c.ws_bytes) / c.a_bytes), std::max<int64_t>(0, c.h - c.n_abuf));
+                            const int64_t capped = std::min<int64_t>(extra, force_abuf ? std::max<int64_t>(0, force_abuf - c.n_abuf) : 256 - c.n_abuf);
+                            if (capped > 0) { c.n_abuf += (int)capped; c.ws_bytes += (uint64_t)capped * c.a_bytes; }
+                        }
+                        cost(c, M, N, Keff, beta_nz, scale_only, mm);
                         const double steps = (double)c.h * c.w * c.kpanels, bsteps = (double)best.h * best.w * best.kpanels;
                         if (!found || c.t_model < best.t_model * (1 - 1e-9) ||
                             (c.t_model <= best.t_model * (1 + 1e-9) && steps < bsteps)) {
@@ -221,7 +270,7 @@ extern "C" int hclooc_plan(int64_t M, int64_t N, int64_t K, int beta_nonzero, in
     out->mb = best.mb; out->nb = best.nb; out->kb = best.kb;
     out->h = best.h; out->w = best.w; out->kpanels = best.kpanels;
     out->n_steps = best.h * best.w * best.kpanels;
-    out->n_sets = best.n_sets; out->n_bbuf = best.n_bbuf; out->ksplit = best.ksplit;
+    out->n_sets = best.n_sets; out->n_abuf = best.n_abuf; out->n_bbuf = best.n_bbuf; out->ksplit = best.ksplit;
     out->lda_dev = best.lda_dev; out->ldb_dev = best.ldb_dev; out->ldc_dev = best.ldc_dev;
     out->bytes_a_buf = best.a_bytes; out->bytes_b_buf = best.b_bytes; out->bytes_c_buf = best.c_bytes;
     out->workspace_bytes = best.ws_bytes;

@@ -337,3 +337,30 @@ def test_trace_records_every_copy_and_kernel(H):
             assert k["t_end_ms"] <= r[r["kind"] == 4][0]["t_end_ms"]
     finally:
         H.hclooc_ctx_destroy(ctx)
+
+
+def test_device_resident_operands_run_in_core(H):
+    """All three operands in device memory: the in-core case -- one DGEMM on the caller's
+    matrices, nothing staged; a host operand or an unaligned device operand goes through the staged pipeline."""
+    import torch
+    M, N, K = 645, 518, 776
+    A, B, C = host_inputs(H, M, N, K, 51, "int")
+    ref = C.view.copy()
+    oracle.dgemm(2.0, A.view, B.view, -1.0, ref)
+    dA, dB = torch.from_numpy(A.view.copy()).cuda(), torch.from_numpy(B.view.copy()).cuda()
+    dC = torch.from_numpy(C.view.copy()).cuda()
+    st = H.hclooc_dgemm_ex(None, M, N, K, 2.0, dA, K, dB, N, -1.0, dC, N, 1 * MiB)
+    assert st.n_kernels == 1 and st.bytes_h2d == 0 and st.bytes_d2h == 0 and st.plan.workspace_bytes == 0
+    assert st.plan.h == 1 and st.plan.w == 1
+    assert np.array_equal(dC.cpu().numpy(), ref)
+    # mixed residency: A on the host, B and C on the device -> staged, same values
+    dC2 = torch.from_numpy(C.view.copy()).cuda()
+    st = H.hclooc_dgemm_ex(None, M, N, K, 2.0, A, A.ld, dB, N, -1.0, dC2, N, 1 * MiB)
+    assert st.n_kernels > 1 and st.plan.workspace_bytes <= 1 * MiB
+    assert np.array_equal(dC2.cpu().numpy(), ref)
+    # odd leading dimension of C on the device: not addressable by the vector epilogue/TMA rules -> staged
+    dC3 = torch.zeros(M, N + 1, dtype=torch.float64, device="cuda")
+    dC3[:, :N] = torch.from_numpy(C.view.copy()).cuda()
+    st = H.hclooc_dgemm_ex(None, M, N, K, 2.0, dA, K, dB, N, -1.0, dC3, N + 1, 1 * MiB)
+    assert st.n_kernels > 1
+    assert np.array_equal(dC3[:, :N].cpu().numpy(), ref) and float(dC3[:, N].abs().max()) == 0.0

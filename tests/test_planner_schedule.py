@@ -90,7 +90,7 @@ CONFIGS = {  # BASELINE.json configs: (M, N, K, beta != 0, budget)
 
 def plan_checks(p, M, N, K, bnz, budget):
     assert p.workspace_bytes <= budget
-    assert p.workspace_bytes == p.n_bbuf * p.bytes_b_buf + p.n_sets * (p.bytes_a_buf + p.bytes_c_buf)
+    assert p.workspace_bytes == p.n_bbuf * p.bytes_b_buf + p.n_abuf * p.bytes_a_buf + p.n_sets * p.bytes_c_buf
     assert p.h == -(-M // p.mb) and p.w == -(-N // p.nb)
     assert p.n_steps == p.h * p.w * p.kpanels and p.n_sets >= 2
     assert p.ldc_dev >= p.nb and p.ldc_dev % 2 == 0 and p.bytes_c_buf >= p.mb * p.ldc_dev * 8
@@ -98,7 +98,20 @@ def plan_checks(p, M, N, K, bnz, budget):
         assert p.kpanels == -(-K // p.kb)
         assert p.lda_dev >= p.kb and p.lda_dev % 2 == 0 and p.ldb_dev >= p.nb and p.ldb_dev % 2 == 0
         assert p.bytes_a_buf >= p.mb * p.lda_dev * 8 and p.bytes_b_buf >= p.kb * p.ldb_dev * 8
-        want_h2d = 8 * (p.w * M * K + K * N + (M * N if bnz else 0) + (p.kpanels - 1) * M * N)
+        assert p.n_abuf >= p.n_sets
+        # A slices: once per column of blocks, minus the min(n_abuf, h) slices the serpentine order finds
+        # still resident at each of the (w - 1) column switches of every K panel (restated here)
+        a_el = 0
+        reuse = min(p.n_abuf, p.h)
+        for sl in range(p.w * p.kpanels):
+            kk = min(p.kb, K - (sl // p.w) * p.kb)
+            if sl % p.w == 0:
+                a_el += M * kk
+            else:
+                kept = min(M, reuse * p.mb) if (sl - 1) % 2 else M - (p.h - reuse) * p.mb
+                a_el += (M - kept) * kk
+        assert M * K <= a_el <= p.w * M * K
+        want_h2d = 8 * (a_el + K * N + (M * N if bnz else 0) + (p.kpanels - 1) * M * N)
     else:
         want_h2d = 8 * (M * N if bnz else 0)
     assert p.bytes_h2d == want_h2d
@@ -116,7 +129,7 @@ def test_plans_for_the_baseline_configs(name):
     else:                                       # FP64-bound
         assert p.t_flop_s > p.t_link_s
     if name == "cfg2":
-        assert p.w == 3 and p.bytes_h2d == 8 * 5 * 8192 * 8192
+        assert p.w == 3 and p.bytes_h2d < 8 * 5 * 8192 * 8192     # 5 matrix volumes minus the reused A slices
 
 
 def test_plans_for_random_shapes_and_budgets():
@@ -138,6 +151,14 @@ def test_plans_for_random_shapes_and_budgets():
         H.hclooc_plan(100, 100, 100, 1, 0, 1024)
     assert H.hclooc_plan(0, 5, 5, 1, 0, MiB).n_steps == 0
     assert H.hclooc_plan(64, 64, 100000, 1, 0, 600 * 1024).kpanels > 1     # K split only when forced
+
+
+def test_in_core_plan_for_device_resident_operands():
+    p = H.hclooc_plan_ex(8192, 8192, 8192, 1, 0, 256 * MiB, 1)
+    assert (p.h, p.w, p.kpanels, p.n_steps) == (1, 1, 1, 1) and (p.mb, p.nb, p.kb) == (8192, 8192, 8192)
+    assert p.workspace_bytes == 0 and p.bytes_h2d == 0 and p.bytes_d2h == 0 and p.flops == 2.0 * 8192 ** 3
+    q = H.hclooc_plan_ex(8192, 8192, 8192, 1, 0, 256 * MiB, 0)
+    assert q.asdict() == H.hclooc_plan(8192, 8192, 8192, 1, 0, 256 * MiB).asdict()
 
 
 # ------------------------------------------------------------------ schedule: coverage, bytes, hazards
@@ -243,14 +264,64 @@ def test_schedule_with_two_b_buffers_prefetches_in_chunks(monkeypatch):
 
 
 def test_simulator_catches_a_missing_wait():
-    """The checker is not vacuous: dropping the Wait(eA) before an A upload is reported."""
+    """The checker is not vacuous: dropping the Wait(eA) before the A uploads (buffer free) or
+    the waits before a B reload is reported."""
     p = H.hclooc_plan(515, 389, 301, 1, 0, 1 * MiB)
     ops = H.hclooc_schedule(p, 4)
-    first_kernel_done = p.n_sets                # event ids: kernel_done(s) = n_sets + s
-    idx = [i for i, o in enumerate(ops) if o["kind"] == K_WAIT and o["stream"] == 0
-           and p.n_sets <= o["event"] < 2 * p.n_sets]
+    a_free0 = 3 * p.n_sets + 2 * p.n_bbuf              # event ids: a_free(a) = 3*n_sets + 2*n_bbuf + a
+    idx = [i for i, o in enumerate(ops) if o["kind"] == K_WAIT and o["stream"] == 0 and o["event"] >= a_free0]
     assert idx
-    broken = np.delete(ops, idx)
     with pytest.raises(AssertionError, match="hazard"):
-        simulate(p, broken)
-    assert first_kernel_done >= 2
+        simulate(p, np.delete(ops, idx))
+    if p.n_bbuf == 1 and p.w > 1:
+        idx = [i for i, o in enumerate(ops) if o["kind"] == K_WAIT and o["stream"] == 0
+               and p.n_sets <= o["event"] < 2 * p.n_sets]      # kernel_done waits before S(b_j)
+        assert idx
+        with pytest.raises(AssertionError, match="hazard"):
+            simulate(p, np.delete(ops, idx))
+
+
+def test_serpentine_order_reuses_resident_a_slices():
+    """Rows run down the even columns of blocks and up the odd ones; the A slices still in the cache when a
+    column ends are not uploaded again (hits need no S(a_i)), and every kernel still finds the right slice."""
+    p = H.hclooc_plan(2000, 1500, 700, 1, 0, 6 * MiB)
+    assert p.w >= 3 and p.h > p.n_abuf
+    ops = H.hclooc_schedule(p, 4)
+    simulate(p, ops)
+    gemms = ops[ops["kind"] == K_GEMM]
+    rows = (gemms["r0"] // p.mb).reshape(p.w, p.h)
+    assert (rows[0] == np.arange(p.h)).all() and (rows[1] == np.arange(p.h)[::-1]).all() and (rows[2] == rows[0]).all()
+    n_a = int((ops["kind"] == K_H2D_A).sum())
+    assert n_a == p.h * p.w - (p.w - 1) * p.n_abuf
+    # with everything cached (h <= n_abuf) A is uploaded exactly once
+    q = H.hclooc_plan(256, 4096, 64, 0, 0, 3 * MiB)
+    if q.w > 1 and q.h <= q.n_abuf and q.kpanels == 1:
+        assert int((H.hclooc_schedule(q, 2)["kind"] == K_H2D_A).sum()) == q.h
+
+
+@pytest.mark.parametrize("bbuf", [0, 1, 2])
+def test_random_plans_simulate_clean(monkeypatch, bbuf):
+    """Fuzz: random shapes, budgets, stream counts and buffer counts; every schedule must cover C exactly
+    once per K panel, move exactly the plan's bytes and order every conflicting buffer access."""
+    if bbuf:
+        monkeypatch.setenv("HCLOOC_FORCE_BBUF", str(bbuf))
+    rng = np.random.default_rng(100 + bbuf)
+    done = 0
+    for _ in range(120):
+        M, N, K = (int(x) for x in rng.integers(1, 1200, 3))
+        budget = int(rng.integers(128 * 1024, 6 * MiB))
+        bnz, az = int(rng.integers(0, 2)), int(rng.integers(0, 10) == 0)
+        sets = int(rng.choice([0, 2, 3, 5]))
+        if sets:
+            monkeypatch.setenv("HCLOOC_FORCE_SETS", str(sets))
+        else:
+            monkeypatch.delenv("HCLOOC_FORCE_SETS", raising=False)
+        try:
+            p = H.hclooc_plan(M, N, K, bnz, az, budget)
+        except H.HclError:
+            continue
+        if p.n_steps > 600:
+            continue
+        simulate(p, H.hclooc_schedule(p, int(rng.integers(1, 9))))
+        done += 1
+    assert done > 40
