@@ -9,8 +9,10 @@ S6 download, S7 events) over one synthetic problem: hclooc_dgemm(M,N,K,alpha,A,l
           throughput with inputs resident when the timed region starts.
   e2e   : the same call through the C ABI with pinned HOST buffers (the product path): host->device and
           device->host copies inside the timed region.  Its roofline is max(flops / FP64 peak, link time).
-  roofline : the dominant kernel (hclooc_dgemm_tile_kernel, FP64 DMMA) timed alone with CUDA events on its
-          launch stream at a GPU-filling launch of the plan's B-slice shape (M x nb x K).
+  roofline : the FP64 DMMA kernel timed alone with CUDA events on its launch stream at a GPU-filling launch of the
+          plan's B-slice shape (M x nb x K; hclDgemmAsync picks the persistent stream-K variant for it);
+          `pipeline_step` inside it is one step of the plan launched exactly as the pipeline launches it
+          (mb x nb x K with plan.ksplit CTAs per tile), against the peak of the SMs that launch occupies.
   cpu_baseline : the oracle, as it stands, on the host cores, on a bounded row sample of the same workload.
 
 `--impl reference` times the oracle (the reference arm of this tier).  Under torchrun every rank runs an
@@ -85,6 +87,17 @@ class ClockSampler:
                         reasons.add(name)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
                 "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def ncu_traffic(launch):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the roofline-leg launch from the committed ncu capture
+    (profiles/r01_traffic.json, written from `ncu --set full`), or None if that capture is of another launch."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "r01_traffic.json")) as f:
+            t = json.load(f)
+        return t["dram_bytes"] if t.get("launch") == launch else None
+    except (OSError, ValueError, KeyError):
+        return None
 
 
 def link_roofline_s(flops, bytes_h2d, bytes_d2h):
@@ -217,7 +230,22 @@ def run_ours(args, wl, name):
             k1.synchronize()
             if it >= max(args.warmup, 3):
                 kt.append(k0.elapsed_time(k1))
+        # ---- one pipeline step, launched as the executor launches it (it need not fill the GPU: steps overlap)
+        mb = min(plan.mb, M)
+        stt = []
+        for it in range(max(args.warmup, 3) + max(args.steps, 10)):
+            k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            k0.record(cur)
+            H.hclDgemmAsyncEx(mb, nb, K, alpha, dA, K, dB, N, beta, dC, N, cur, variant=max(1, plan.ksplit))
+            k1.record(cur)
+            k1.synchronize()
+            if it >= max(args.warmup, 3):
+                stt.append(k0.elapsed_time(k1))
         clocks = clk.summary()
+    ms_step = float(np.mean(stt))
+    step_ctas = min(148, -(-mb // 128) * -(-nb // 128) * max(1, plan.ksplit))
+    step_achieved = 2.0 * mb * nb * K / (ms_step * 1e-3) / 1e12
+    step_peak = FP64_PEAK_TFLOPS * step_ctas / 148.0
     ms_kernel = float(np.mean(kt))
     kflops = 2.0 * M * nb * K
     achieved = kflops / (ms_kernel * 1e-3) / 1e12
@@ -243,12 +271,17 @@ def run_ours(args, wl, name):
                 "h2d_bytes_per_step": int(st_e2e.bytes_h2d), "d2h_bytes_per_step": int(st_e2e.bytes_d2h),
                 "roofline_s": t_roof, "t_flop_s": t_flop, "t_link_s": t_link, "bound": "link" if t_link > t_flop else "fp64",
                 "frac_of_roofline": t_roof / (ms_e2e * 1e-3), "link_peaks": LINK},
-        "gpu_launches": int((st_res.n_kernels + st_e2e.n_kernels) * args.steps + len(kt)),
+        "gpu_launches": int((st_res.n_kernels + st_e2e.n_kernels) * args.steps + len(kt) + len(stt)),
         "clocks": clocks,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                     "frac": achieved / FP64_PEAK_TFLOPS, "traffic": None, "kernel": "hclooc_dgemm_tile_kernel",
+                     "frac": achieved / FP64_PEAK_TFLOPS, "traffic": ncu_traffic(f"{M}x{nb}x{K}"),
+                     "kernel": "hclooc_dgemm_streamk_kernel" if -(-M // 128) * -(-nb // 128) >= 148 else "hclooc_dgemm_tile_kernel",
                      "launch": f"{M}x{nb}x{K} (one B slice of the plan, all rows)", "ms_per_launch": ms_kernel,
-                     "peak_source": "derived 148 SM x 128 FP64 flop/clk x 1.965 GHz; DMMA microbenchmark measured 37.17"},
+                     "peak_source": "derived 148 SM x 128 FP64 flop/clk x 1.965 GHz; DMMA microbenchmark measured 37.17",
+                     "pipeline_step": {"kernel": f"hclooc_dgemm_tile_kernel<{max(1, plan.ksplit)}>", "launch": f"{mb}x{nb}x{K}",
+                                       "ctas": step_ctas, "ms_per_launch": ms_step, "achieved": step_achieved,
+                                       "peak": step_peak, "frac": step_achieved / step_peak,
+                                       "note": "peak = 37.2 TFLOP/s x CTAs/148: a step occupies only its own CTAs, other steps run beside it"}},
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         rows = min(M, args.cpu_rows if args.cpu_rows > 0 else max(128, int(1.0e12 / (2.0 * N * K)) // 128 * 128))

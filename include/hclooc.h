@@ -64,15 +64,19 @@ typedef struct hclooc_plan_t {
     int32_t  n_bbuf;              /* B slice device buffers (1 = paper's single buffer, 2 = prefetch) */
     int32_t  beta_nonzero;        /* C blocks are uploaded only when 1 (or for K panels p > 0)      */
     int32_t  scale_only;          /* alpha == 0 or K == 0: C = beta*C, A and B never referenced     */
-    int32_t  ksplit;              /* CTAs per cluster sharing one tile's K range in the kernel (1, 2, 4) */
+    int32_t  ksplit;              /* CTAs per cluster sharing one tile's K range in the kernel (1, 2, 4), or -1:
+                                     every step is one persistent stream-K launch that fills the GPU by itself */
     int32_t  n_abuf;              /* A slice device buffers: an LRU cache keyed by (row slice, K panel) */
     int64_t  lda_dev, ldb_dev, ldc_dev;  /* leading dimensions of the device buffers (elements)    */
     uint64_t bytes_a_buf, bytes_b_buf, bytes_c_buf;   /* one buffer of each kind                   */
-    uint64_t workspace_bytes;     /* n_bbuf*b + n_abuf*a + n_sets*c, <= the budget                  */
+    uint64_t workspace_bytes;     /* n_bbuf*b + n_abuf*a + n_sets*c + n_scratch*bytes_scratch, <= the budget */
     uint64_t bytes_h2d, bytes_d2h;/* exactly what the executor enqueues over the host link          */
     uint64_t n_copies_h2d, n_copies_d2h;
     double   flops;               /* 2*M*N*K (:368)                                                 */
     double   t_flop_s, t_link_s, t_model_s;  /* cost model terms used to pick this plan             */
+    int32_t  n_scratch;           /* stream-K scratch buffers (ksplit == -1): one per compute stream used       */
+    int32_t  reserved1;
+    uint64_t bytes_scratch;       /* one of them (partial-tile slots + counters)                                */
 } hclooc_plan_t;
 
 /* Plan only (pure host arithmetic, needs no GPU).  alpha_zero != 0 plans the scale-only pass.
@@ -109,7 +113,7 @@ int hclMatrixPartitioner(int64_t M, int64_t N, int64_t K, int64_t budget_element
  * events:  c = uploads of the step using C buffer c arrived (rA/rC); n_sets + c = its kernel finished (eA);
  *          2*n_sets + c = C buffer c stored on the host (eC); 3*n_sets + b = B buffer b received (rB);
  *          3*n_sets + n_bbuf + b = every kernel of the column that read B buffer b finished;
- *          3*n_sets + 2*n_bbuf + a = the latest kernel that read A buffer a finished.                 */
+ *          3*n_sets + 2*n_bbuf + 2*a + (0|1) = the kernels that read A buffer a finished (readers alternate). */
 typedef struct hclooc_op_t {
     int32_t kind, stream, event;
     int32_t buf, buf2, buf3;
@@ -201,6 +205,14 @@ int hclMemcpy2DAsync(void* dst, size_t dpitch, const void* src, size_t spitch, s
 int hclDgemmAsync(int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda,
                   const double* dB, int64_t ldb, double beta, double* dC, int64_t ldc,
                   hclStream s, hclEvent* ev);
+/* Same with the launch variant spelled out: HCL_DGEMM_AUTO (what hclDgemmAsync does: the persistent stream-K
+ * kernel when the output has at least 148 tiles of 128 x 128, else one CTA -- or a cluster of 2 or 4 CTAs
+ * splitting K -- per tile), 1 / 2 / 4 = that many CTAs per tile (what a pipeline step launches, plan.ksplit),
+ * -1 = persistent stream-K.  -14: unknown variant.                                                    */
+#define HCL_DGEMM_AUTO 0
+int hclDgemmAsyncEx(int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda,
+                    const double* dB, int64_t ldb, double beta, double* dC, int64_t ldc,
+                    hclStream s, hclEvent* ev, int variant);
 int hclWaitEvent(hclStream s, hclEvent e);                        /* :116  stream waits for event   */
 int hclStreamSynchronize(hclStream s);                            /* :115                           */
 int hclDeviceSynchronize(int device);                             /* :114                           */

@@ -10,7 +10,7 @@ from ._binding import (  # noqa: F401
     hclooc_plan, hclooc_plan_ex, hclooc_schedule, hclMatrixPartitioner,
     hclooc_ctx_create, hclooc_ctx_destroy, hclooc_ctx_set_trace, hclooc_ctx_get_trace, TRACE_DTYPE, hclooc_dgemm, hclooc_dgemm_ex,
     hclMalloc, hclFree, hclGetMemSize, hclStreamCreate, hclStreamDestroy, hclEventDestroy,
-    hclMemcpy, hclMemcpyAsync, hclMemcpy2DAsync, hclDgemmAsync, hclWaitEvent,
+    hclMemcpy, hclMemcpyAsync, hclMemcpy2DAsync, hclDgemmAsync, hclDgemmAsyncEx, hclWaitEvent,
     hclStreamSynchronize, hclDeviceSynchronize,
     hclooc_host_alloc, hclooc_host_free, hclooc_host_register, hclooc_host_unregister,
     hclooc_strerror, hclooc_last_cuda_error, hclooc_version,

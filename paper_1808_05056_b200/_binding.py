@@ -16,7 +16,7 @@ EXPORTS = [
     "hclooc_ctx_set_trace", "hclooc_ctx_get_trace",
     "hclooc_dgemm", "hclooc_dgemm_ex", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
     "hclStreamDestroy", "hclEventDestroy", "hclMemcpy", "hclMemcpyAsync", "hclMemcpy2DAsync",
-    "hclDgemmAsync", "hclWaitEvent", "hclStreamSynchronize", "hclDeviceSynchronize",
+    "hclDgemmAsync", "hclDgemmAsyncEx", "hclWaitEvent", "hclStreamSynchronize", "hclDeviceSynchronize",
     "hclooc_host_alloc", "hclooc_host_free", "hclooc_host_register", "hclooc_host_unregister",
     "hclooc_strerror", "hclooc_last_cuda_error", "hclooc_version",
 ]
@@ -32,7 +32,8 @@ class Plan(ctypes.Structure):
                 ("bytes_a_buf", c_uint64), ("bytes_b_buf", c_uint64), ("bytes_c_buf", c_uint64),
                 ("workspace_bytes", c_uint64), ("bytes_h2d", c_uint64), ("bytes_d2h", c_uint64),
                 ("n_copies_h2d", c_uint64), ("n_copies_d2h", c_uint64),
-                ("flops", c_double), ("t_flop_s", c_double), ("t_link_s", c_double), ("t_model_s", c_double)]
+                ("flops", c_double), ("t_flop_s", c_double), ("t_link_s", c_double), ("t_model_s", c_double),
+                ("n_scratch", c_int32), ("reserved1", c_int32), ("bytes_scratch", c_uint64)]
 
     def asdict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -90,6 +91,7 @@ def lib():
         L.hclMemcpyAsync.argtypes = [vp, vp, sz, c_int, vp, POINTER(vp)]
         L.hclMemcpy2DAsync.argtypes = [vp, sz, vp, sz, sz, sz, c_int, vp, POINTER(vp)]
         L.hclDgemmAsync.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, vp, POINTER(vp)]
+        L.hclDgemmAsyncEx.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, vp, POINTER(vp), c_int]
         L.hclWaitEvent.argtypes = [vp, vp]
         L.hclStreamSynchronize.argtypes = [vp]
         L.hclDeviceSynchronize.argtypes = [c_int]
@@ -302,6 +304,13 @@ def hclMemcpy2DAsync(dst, dpitch, src, spitch, width_bytes, rows, direction, str
     ev = _ev(want_event, event)
     _check(lib().hclMemcpy2DAsync(_ptr(dst), dpitch, _ptr(src), spitch, width_bytes, rows, direction, _ptr(stream),
                                   byref(ev) if ev is not None else None), "hclMemcpy2DAsync")
+    return ev.value if ev is not None else None
+
+
+def hclDgemmAsyncEx(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, stream=None, want_event=False, event=None, variant=0):
+    ev = _ev(want_event, event)
+    _check(lib().hclDgemmAsyncEx(M, N, K, alpha, _ptr(dA), lda, _ptr(dB), ldb, beta, _ptr(dC), ldc, _ptr(stream),
+                                 byref(ev) if ev is not None else None, variant), "hclDgemmAsyncEx")
     return ev.value if ev is not None else None
 
 

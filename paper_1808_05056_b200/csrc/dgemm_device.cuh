@@ -1,0 +1,187 @@
+// dgemm_device.cuh -- device-side building blocks shared by the two S5 kernels (dgemm_sm100.cu: one tile or one
+// cluster per tile; dgemm_streamk_sm100.cu: persistent stream-K): tile geometry, mbarrier/TMA/DMMA wrappers,
+// the permuted fragment layout and the fused alpha/beta epilogue.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace hclooc {
+namespace dev {
+
+constexpr int BM = 128;
+constexpr int BN = 128;
+constexpr int BK = 16;
+constexpr int STAGES = 6;
+constexpr int A_STAGE_BYTES = BM * BK * 8;          // 16 KiB: 128 rows x 128 B
+constexpr int B_BOX_BYTES = BK * 16 * 8;            // 2 KiB: 16 k-rows x 128 B (16 columns)
+constexpr int B_STAGE_BYTES = (BN / 16) * B_BOX_BYTES;  // 16 KiB
+constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;
+constexpr int NUM_CONSUMER_WARPS = 8;
+// Two consumer warpgroups + one producer warpgroup of which only warp 0 works.  The register file is split per
+// SM sub-partition (16384 registers for its 3 warps), so a flat allocation caps every thread at 168 registers
+// and the 128 accumulator registers of a consumer leave too little for the loop state: the producer warpgroup
+// gives its registers back (setmaxnreg.dec) and the consumers take them (setmaxnreg.inc).
+constexpr int NUM_PRODUCER_WARPS = 4;
+constexpr int NUM_THREADS = (NUM_CONSUMER_WARPS + NUM_PRODUCER_WARPS) * 32;
+constexpr int PRODUCER_REGS = 40;
+constexpr int CONSUMER_REGS = 232;
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align slack*/ + 2 * STAGES * 8;
+constexpr int RASTER_GROUP = 16;                     // m-tiles per rasterisation group
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "DONE:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+        ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void lds128(double& x, double& y, uint32_t addr) {
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(x), "=d"(y) : "r"(addr));
+}
+__device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+                 : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
+}
+
+__device__ __forceinline__ void regs_release_producer() {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(PRODUCER_REGS));
+}
+__device__ __forceinline__ void regs_take_consumer() {
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(CONSUMER_REGS));
+}
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void ld_dsmem128(double& x, double& y, uint32_t local_addr, uint32_t rank) {
+    uint32_t remote;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local_addr), "r"(rank));
+    asm volatile("ld.shared::cluster.v2.f64 {%0, %1}, [%2];" : "=d"(x), "=d"(y) : "r"(remote) : "memory");
+}
+
+
+// Tile rasterisation: groups of RASTER_GROUP m-tiles, m fastest inside a group, so CTAs that run together share
+// B column panels and a bounded set of A row panels in L2.
+__device__ __forceinline__ void tile_coords(int tile, int tiles_m, int tiles_n, int& tile_m, int& tile_n) {
+    const int per_group = RASTER_GROUP * tiles_n;
+    const int grp = tile / per_group;
+    const int rem = tile - grp * per_group;
+    const int gm0 = grp * RASTER_GROUP;
+    const int gsz = min(RASTER_GROUP, tiles_m - gm0);
+    tile_m = gm0 + rem % gsz;
+    tile_n = rem / gsz;
+}
+
+// Per-lane shared-memory byte offsets of the DMMA fragments inside a stage.  Inside a tile the 8 rows of an
+// m-tile, the 4 k indices of a k-step and the 8 columns of an n-tile are permuted (row g <-> 4(g&1)+(g>>1),
+// k index t <-> 2t+e, columns interleaved in pairs) so that with the 128-byte swizzle every LDS.128 of a
+// quarter warp hits distinct banks and feeds two DMMAs.
+struct FragLanes {
+    uint32_t a_lane, b_lane[2];
+    int rp, t, wm, wn;
+    __device__ __forceinline__ void init(int warp, int lane) {
+        const int g = lane >> 2;
+        t = lane & 3;
+        rp = 4 * (g & 1) + (g >> 1);
+        wm = warp & 3;
+        wn = warp >> 2;
+        a_lane = (uint32_t)((wm * 32 + rp) * 128 + ((t ^ rp) << 4));
+        #pragma unroll
+        for (int e = 0; e < 2; ++e)
+            b_lane[e] = (uint32_t)(A_STAGE_BYTES + wn * 4 * B_BOX_BYTES + (2 * t + e) * 128 + ((g ^ (2 * t + e)) << 4));
+    }
+};
+
+// One k block (16 deep) of the 32 x 64 warp tile: 12 LDS.128 feed 64 DMMA.8x8x4.
+__device__ __forceinline__ void mma_kblock(double (&acc)[4][4][2][2], uint32_t sbase, const FragLanes& f) {
+    #pragma unroll
+    for (int kg = 0; kg < 2; ++kg) {
+        double a[4][2];
+        #pragma unroll
+        for (int u = 0; u < 4; ++u) lds128(a[u][0], a[u][1], sbase + ((f.a_lane ^ (kg << 6)) + u * 1024));
+        #pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            double b[4][2];
+            #pragma unroll
+            for (int bx = 0; bx < 4; ++bx)
+                lds128(b[bx][0], b[bx][1], sbase + f.b_lane[e] + kg * 1024 + bx * B_BOX_BYTES);
+            #pragma unroll
+            for (int u = 0; u < 4; ++u)
+                #pragma unroll
+                for (int bx = 0; bx < 4; ++bx) {
+                    dmma(acc[u][bx][0], a[u][e], b[bx][0]);
+                    dmma(acc[u][bx][1], a[u][e], b[bx][1]);
+                }
+        }
+    }
+}
+
+// How many 8-row groups / 16-column boxes of this warp's 32 x 64 tile lie inside the matrix (0..4 each).  A warp
+// whose part of an edge tile is entirely zero fill skips its DMMAs (nobody reads those products).
+__device__ __forceinline__ int edge_groups(int extent, int origin, int unit) {
+    const int left = extent - origin;
+    return left <= 0 ? 0 : (left >= 4 * unit ? 4 : (left + unit - 1) / unit);
+}
+
+// Fused epilogue: C = alpha*acc + beta*C straight from registers; C is not read when beta == 0.
+__device__ __forceinline__ void epilogue_store(const double (&acc)[4][4][2][2], double* __restrict__ C, long long ldc,
+                                               int M, int N, int m0, int n0, double alpha, double beta, const FragLanes& f) {
+    const bool read_c = (beta != 0.0);
+    const bool vec_ok = ((ldc & 1LL) == 0) && ((reinterpret_cast<uintptr_t>(C) & 15u) == 0);
+    #pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const int row = m0 + f.wm * 32 + u * 8 + f.rp;
+        if (row >= M) continue;
+        double* crow = C + (long long)row * ldc;
+        #pragma unroll
+        for (int bx = 0; bx < 4; ++bx) {
+            const int col = n0 + f.wn * 64 + bx * 16 + 4 * f.t;
+            // lane holds 4 consecutive columns: (v=0,c0) (v=1,c0) (v=0,c1) (v=1,c1)
+            double x0 = alpha * acc[u][bx][0][0], x1 = alpha * acc[u][bx][1][0];
+            double x2 = alpha * acc[u][bx][0][1], x3 = alpha * acc[u][bx][1][1];
+            if (col + 3 < N && vec_ok) {
+                double2* p = reinterpret_cast<double2*>(crow + col);
+                if (read_c) {
+                    const double2 c01 = p[0], c23 = p[1];
+                    x0 += beta * c01.x; x1 += beta * c01.y; x2 += beta * c23.x; x3 += beta * c23.y;
+                }
+                p[0] = make_double2(x0, x1);
+                p[1] = make_double2(x2, x3);
+            } else {
+                const double xs[4] = {x0, x1, x2, x3};
+                #pragma unroll
+                for (int q = 0; q < 4; ++q)
+                    if (col + q < N) crow[col + q] = read_c ? xs[q] + beta * crow[col + q] : xs[q];
+            }
+        }
+    }
+}
+
+}  // namespace dev
+}  // namespace hclooc

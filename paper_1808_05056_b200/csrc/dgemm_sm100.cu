@@ -20,74 +20,16 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <mutex>
+#include <cstdlib>
+#include <cstring>
 #include "internal.h"
+#include "dgemm_device.cuh"
 
 namespace hclooc {
 
 namespace {
 
-constexpr int BM = 128;
-constexpr int BN = 128;
-constexpr int BK = 16;
-constexpr int STAGES = 6;
-constexpr int A_STAGE_BYTES = BM * BK * 8;          // 16 KiB: 128 rows x 128 B
-constexpr int B_BOX_BYTES = BK * 16 * 8;            // 2 KiB: 16 k-rows x 128 B (16 columns)
-constexpr int B_STAGE_BYTES = (BN / 16) * B_BOX_BYTES;  // 16 KiB
-constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;
-constexpr int NUM_CONSUMER_WARPS = 8;
-constexpr int NUM_THREADS = (NUM_CONSUMER_WARPS + 1) * 32;
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*align slack*/ + 2 * STAGES * 8;
-constexpr int RASTER_GROUP = 16;                     // m-tiles per rasterisation group
-
-__device__ __forceinline__ uint32_t smem_u32(const void* p) {
-    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
-}
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_LOOP:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE;\n"
-        "bra WAIT_LOOP;\n"
-        "DONE:\n"
-        "}\n" ::"r"(bar), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar) {
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
-        ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar) : "memory");
-}
-__device__ __forceinline__ void lds128(double& x, double& y, uint32_t addr) {
-    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(x), "=d"(y) : "r"(addr));
-}
-__device__ __forceinline__ void dmma(double (&c)[2], double a, double b) {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
-                 : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
-}
-
-__device__ __forceinline__ uint32_t cluster_ctarank() {
-    uint32_t r;
-    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
-    return r;
-}
-__device__ __forceinline__ void cluster_sync_all() {
-    asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void ld_dsmem128(double& x, double& y, uint32_t local_addr, uint32_t rank) {
-    uint32_t remote;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local_addr), "r"(rank));
-    asm volatile("ld.shared::cluster.v2.f64 {%0, %1}, [%2];" : "=d"(x), "=d"(y) : "r"(remote) : "memory");
-}
+using namespace dev;
 
 // One CTA computes one 128 x 128 tile of C over the whole K range (KSPLIT == 1), or a cluster of KSPLIT
 // CTAs shares the tile: CTA r of the cluster takes the r-th share of the k blocks, the partial
@@ -104,19 +46,8 @@ hclooc_dgemm_tile_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_c
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
 
-    // tile rasterisation: groups of RASTER_GROUP m-tiles, m fastest inside a group, so CTAs that run
-    // together share B column panels and a bounded set of A row panels in L2
     int tile_m, tile_n;
-    {
-        const int per_group = RASTER_GROUP * tiles_n;
-        const int tile = (KSPLIT == 1) ? (int)blockIdx.x : (int)(blockIdx.x / KSPLIT);
-        const int grp = tile / per_group;
-        const int rem = tile - grp * per_group;
-        const int gm0 = grp * RASTER_GROUP;
-        const int gsz = min(RASTER_GROUP, tiles_m - gm0);
-        tile_m = gm0 + rem % gsz;
-        tile_n = rem / gsz;
-    }
+    tile_coords((KSPLIT == 1) ? (int)blockIdx.x : (int)(blockIdx.x / KSPLIT), tiles_m, tiles_n, tile_m, tile_n);
     const int m0 = tile_m * BM;
     const int n0 = tile_n * BN;
     const int num_kb_all = (K + BK - 1) / BK;
@@ -134,9 +65,10 @@ hclooc_dgemm_tile_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_c
     }
     __syncthreads();
 
-    if (warp == NUM_CONSUMER_WARPS) {
-        // ------------------------------------------------------------ producer warp: TMA
-        if (lane == 0 && num_kb > 0) {
+    if (warp >= NUM_CONSUMER_WARPS) {
+        // ------------------------------------------------------------ producer warpgroup: warp 0 drives TMA
+        regs_release_producer();
+        if (warp == NUM_CONSUMER_WARPS && lane == 0 && num_kb > 0) {
             asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA) : "memory");
             asm volatile("prefetch.tensormap [%0];" ::"l"(&tmB) : "memory");
             int stage = 0;
@@ -163,18 +95,9 @@ hclooc_dgemm_tile_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_c
     }
 
     // ---------------------------------------------------------------- consumer warps: DMMA
-    const int g = lane >> 2;                  // fragment row group
-    const int t = lane & 3;                   // fragment k / column-pair index
-    const int rp = 4 * (g & 1) + (g >> 1);    // row permutation inside an 8-row m-tile
-    const int wm = warp & 3;                  // warp row   (32 rows each)
-    const int wn = warp >> 2;                 // warp column (64 columns each)
-
-    // per-lane shared-memory byte offsets inside a stage (see the header comment for the layout)
-    const uint32_t a_lane = (uint32_t)((wm * 32 + rp) * 128 + ((t ^ rp) << 4));
-    uint32_t b_lane[2];
-    #pragma unroll
-    for (int e = 0; e < 2; ++e)
-        b_lane[e] = (uint32_t)(A_STAGE_BYTES + wn * 4 * B_BOX_BYTES + (2 * t + e) * 128 + ((g ^ (2 * t + e)) << 4));
+    regs_take_consumer();
+    FragLanes f;
+    f.init(warp, lane);
 
     double acc[4][4][2][2];
     #pragma unroll
@@ -187,32 +110,22 @@ hclooc_dgemm_tile_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_c
     {
         int stage = 0;
         uint32_t phase = 0;
-        for (int kb = 0; kb < num_kb; ++kb) {
-            mbar_wait(bar_base + 8 * stage, phase);
-            const uint32_t sbase = smem_base + stage * STAGE_BYTES;
-            #pragma unroll
-            for (int kg = 0; kg < 2; ++kg) {
-                double a[4][2];
-                #pragma unroll
-                for (int u = 0; u < 4; ++u) lds128(a[u][0], a[u][1], sbase + ((a_lane ^ (kg << 6)) + u * 1024));
-                #pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    double b[4][2];
-                    #pragma unroll
-                    for (int bx = 0; bx < 4; ++bx)
-                        lds128(b[bx][0], b[bx][1], sbase + b_lane[e] + kg * 1024 + bx * B_BOX_BYTES);
-                    #pragma unroll
-                    for (int u = 0; u < 4; ++u)
-                        #pragma unroll
-                        for (int bx = 0; bx < 4; ++bx) {
-                            dmma(acc[u][bx][0], a[u][e], b[bx][0]);
-                            dmma(acc[u][bx][1], a[u][e], b[bx][1]);
-                        }
-                }
+        const int nu = edge_groups(M, m0 + f.wm * 32, 8), nbx = edge_groups(N, n0 + f.wn * 64, 16);
+        if (nu != 0 && nbx != 0) {
+            for (int kb = 0; kb < num_kb; ++kb) {
+                mbar_wait(bar_base + 8 * stage, phase);
+                mma_kblock(acc, smem_base + stage * STAGE_BYTES, f);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_base + 8 * (STAGES + stage));
+                if (++stage == STAGES) { stage = 0; phase ^= 1u; }
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(bar_base + 8 * (STAGES + stage));
-            if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+        } else {                                  // this warp's part of the tile lies outside C: only keep the ring moving
+            for (int kb = 0; kb < num_kb; ++kb) {
+                mbar_wait(bar_base + 8 * stage, phase);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_base + 8 * (STAGES + stage));
+                if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+            }
         }
     }
 
@@ -255,35 +168,7 @@ hclooc_dgemm_tile_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_c
     }
 
     // ---------------------------------------------------------------- fused epilogue
-    const bool read_c = (beta != 0.0);
-    const bool vec_ok = ((ldc & 1LL) == 0) && ((reinterpret_cast<uintptr_t>(C) & 15u) == 0);
-    #pragma unroll
-    for (int u = 0; u < 4; ++u) {
-        const int row = m0 + wm * 32 + u * 8 + rp;
-        if (row >= M) continue;
-        double* crow = C + (long long)row * ldc;
-        #pragma unroll
-        for (int bx = 0; bx < 4; ++bx) {
-            const int col = n0 + wn * 64 + bx * 16 + 4 * t;
-            // lane holds 4 consecutive columns: (v=0,c0) (v=1,c0) (v=0,c1) (v=1,c1)
-            double x0 = alpha * acc[u][bx][0][0], x1 = alpha * acc[u][bx][1][0];
-            double x2 = alpha * acc[u][bx][0][1], x3 = alpha * acc[u][bx][1][1];
-            if (col + 3 < N && vec_ok) {
-                double2* p = reinterpret_cast<double2*>(crow + col);
-                if (read_c) {
-                    const double2 c01 = p[0], c23 = p[1];
-                    x0 += beta * c01.x; x1 += beta * c01.y; x2 += beta * c23.x; x3 += beta * c23.y;
-                }
-                p[0] = make_double2(x0, x1);
-                p[1] = make_double2(x2, x3);
-            } else {
-                const double xs[4] = {x0, x1, x2, x3};
-                #pragma unroll
-                for (int q = 0; q < 4; ++q)
-                    if (col + q < N) crow[col + q] = read_c ? xs[q] + beta * crow[col + q] : xs[q];
-            }
-        }
-    }
+    epilogue_store(acc, C, ldc, M, N, m0, n0, alpha, beta, f);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -363,7 +248,7 @@ int dgemm_auto_ksplit(int64_t tiles_in_flight, int64_t K) {
 
 int launch_dgemm_tiles(int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda,
                        const double* dB, int64_t ldb, double beta, double* dC, int64_t ldc, cudaStream_t stream,
-                       int ksplit) {
+                       int ksplit, void* streamk_scratch) {
     if (M == 0 || N == 0) return HCLOOC_OK;
     if (alpha == 0.0) K = 0;                       // A and B are not referenced (BLAS convention)
     int rc = ensure_kernel_attr();
@@ -378,6 +263,12 @@ int launch_dgemm_tiles(int64_t M, int64_t N, int64_t K, double alpha, const doub
     }
     const int64_t tm = (M + BM - 1) / BM, tn = (N + BN - 1) / BN;
     if (tm * tn > 0x7fffffffLL || M > 0x7fffffffLL || N > 0x7fffffffLL || K > 0x7fffffffLL) return HCLOOC_ERR_INTERNAL;
+    static const bool no_streamk = getenv("HCLOOC_NO_STREAMK") != nullptr;   // experiment knob
+    if (ksplit < 0 && K > 0 && !no_streamk) {
+        // a launch that has the GPU to itself: persistent stream-K kernel (falls through if no scratch is free)
+        rc = launch_dgemm_streamk(M, N, K, alpha, tmA, tmB, beta, dC, ldc, stream, streamk_scratch);
+        if (rc != 1) return rc;
+    }
     if (ksplit <= 0) ksplit = dgemm_auto_ksplit(tm * tn, K);
     if (K == 0) ksplit = 1;
     cudaError_t e;

@@ -32,8 +32,10 @@ struct EventIds {
     int c_stored(int c) const { return 2 * n_sets + c; }     // eC: C buffer c is back on the host
     int b_ready(int b) const { return 3 * n_sets + b; }      // rB: B slice buffer b received
     int b_free(int b) const { return 3 * n_sets + n_bbuf + b; }  // every kernel of the column that read B buffer b finished
-    int a_free(int a) const { return 3 * n_sets + 2 * n_bbuf + a; }  // the latest kernel that read A buffer a finished
-    int count() const { return 3 * n_sets + 2 * n_bbuf + n_abuf; }
+    // readers of A buffer a record alternately into two events; reader r waits for reader r-2 (same event) first,
+    // so the latest record of each event covers every earlier reader of its parity
+    int a_free(int a, int parity) const { return 3 * n_sets + 2 * n_bbuf + 2 * a + parity; }
+    int count() const { return 3 * n_sets + 2 * n_bbuf + 2 * n_abuf; }
 };
 
 // Expand the plan into the operation list.  This is the single source of truth for the executor.
@@ -45,12 +47,13 @@ struct EventIds {
 void build_schedule(const hclooc_plan_t& P, int ncs, std::vector<hclooc_op_t>& ops) {
     ops.clear();
     if (P.n_steps == 0) return;
+    if (P.ksplit < 0) ncs = std::max(1, std::min(ncs, (int)P.n_scratch));   // stream-K steps: one scratch buffer per compute stream
     const int n_sets = P.n_sets, n_abuf = std::max(1, (int)P.n_abuf);
     const EventIds ev{n_sets, P.n_bbuf, n_abuf};
     const bool scale_only = P.scale_only != 0;
     std::vector<char> set_used(n_sets, 0), set_stored(n_sets, 0);
     // A-slice cache
-    struct ABuf { int64_t row = -1, panel = -1; int64_t last_use = -1; int ready_ev = -1; bool read = false; };
+    struct ABuf { int64_t row = -1, panel = -1; int64_t last_use = -1; int ready_ev = -1; int64_t readers = 0; };
     std::vector<ABuf> acache(n_abuf);
     auto push = [&](int kind, int stream, int event) -> hclooc_op_t& {
         hclooc_op_t o;
@@ -101,8 +104,9 @@ void build_schedule(const hclooc_plan_t& P, int ncs, std::vector<hclooc_op_t>& o
             if (hit >= 0) { s.abuf = hit; s.a_hit = true; }
             else {
                 ABuf& ab = acache[victim];
-                if (ab.read) push(HCLOOC_OP_WAIT, 0, ev.a_free(victim));                  // Wait(eA): buffer free (:311)
-                ab.read = false;
+                for (int par = 0; par < 2 && par < ab.readers; ++par)
+                    push(HCLOOC_OP_WAIT, 0, ev.a_free(victim, par));                      // Wait(eA): buffer free (:311)
+                ab.readers = 0;
                 hclooc_op_t& o = push(HCLOOC_OP_H2D_A, 0, -1);                            // S(a_i)
                 o.buf = victim; o.r0 = i0; o.nr = mi; o.c0 = k0; o.nc = kk; o.step = idx;
                 ab.row = s.i; ab.panel = s.p; ab.ready_ev = ev.up_ready(c);
@@ -132,10 +136,10 @@ void build_schedule(const hclooc_plan_t& P, int ncs, std::vector<hclooc_op_t>& o
         const int64_t idx = s.i + P.h * (s.j + P.w * s.p);
         if (any_upload) push(HCLOOC_OP_WAIT, cs, ev.up_ready(c));                         // Wait(rA), Wait(rC)
         if (!scale_only && s.a_hit) {
-            // cached slice: its upload arrived, and this kernel is ordered after the previous reader so that
-            // the latest record of a_free covers every kernel that read the buffer
+            // cached slice: its upload arrived; and this kernel is ordered after the reader before the previous
+            // one (at least a column of steps ago), whose event it is about to record over
             if (acache[s.abuf].ready_ev != ev.up_ready(c)) push(HCLOOC_OP_WAIT, cs, acache[s.abuf].ready_ev);
-            if (acache[s.abuf].read) push(HCLOOC_OP_WAIT, cs, ev.a_free(s.abuf));
+            if (acache[s.abuf].readers >= 2) push(HCLOOC_OP_WAIT, cs, ev.a_free(s.abuf, (int)(acache[s.abuf].readers & 1)));
         }
         if (!scale_only) push(HCLOOC_OP_WAIT, cs, ev.b_ready(b));                         // Wait(rB)
         if (!cload && set_stored[c]) push(HCLOOC_OP_WAIT, cs, ev.c_stored(c));            // C buffer still draining
@@ -147,7 +151,7 @@ void build_schedule(const hclooc_plan_t& P, int ncs, std::vector<hclooc_op_t>& o
         }
         push(HCLOOC_OP_RECORD, cs, ev.kernel_done(c));                                    // Rec(eA)
         set_used[c] = 1;
-        if (!scale_only) { push(HCLOOC_OP_RECORD, cs, ev.a_free(s.abuf)); acache[s.abuf].read = true; }
+        if (!scale_only) { push(HCLOOC_OP_RECORD, cs, ev.a_free(s.abuf, (int)(acache[s.abuf].readers & 1))); ++acache[s.abuf].readers; }
         push(HCLOOC_OP_WAIT, 1, ev.kernel_done(c));
         if (last_of_slab && P.n_bbuf == 2 && !scale_only) push(HCLOOC_OP_RECORD, 1, ev.b_free(b));  // the column's kernels are done
         {
@@ -373,7 +377,7 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
     if (rc) return rc;
     if (in_core) {
         const auto t0 = std::chrono::steady_clock::now();
-        rc = launch_dgemm_tiles(M, N, scale_only ? 0 : K, scale_only ? 0.0 : alpha, A, lda, B, ldb, beta, C, ldc, ctx->s_compute[0], P.ksplit);
+        rc = launch_dgemm_tiles(M, N, scale_only ? 0 : K, scale_only ? 0.0 : alpha, A, lda, B, ldb, beta, C, ldc, ctx->s_compute[0], -1);
         const auto t1 = std::chrono::steady_clock::now();
         cudaError_t e = cudaStreamSynchronize(ctx->s_compute[0]);
         if (rc) return rc;
@@ -403,15 +407,18 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
         if (P.workspace_bytes + 1024 - mis > ctx->workspace_bytes) return HCLOOC_ERR_BUDGET;
     }
     std::vector<double*> bufs(P.n_abuf + P.n_sets + P.n_bbuf);
+    uint8_t* scratch[MAX_COMPUTE_STREAMS] = {};
+    if (P.n_scratch > MAX_COMPUTE_STREAMS) return HCLOOC_ERR_INTERNAL;
     {
         uint8_t* q = base;
         for (int b = 0; b < P.n_bbuf; ++b) { bufs[P.n_abuf + P.n_sets + b] = (double*)q; q += P.bytes_b_buf; }
         for (int a = 0; a < P.n_abuf; ++a) { bufs[a] = (double*)q; q += P.bytes_a_buf; }
         for (int c = 0; c < P.n_sets; ++c) { bufs[P.n_abuf + c] = (double*)q; q += P.bytes_c_buf; }
+        for (int i = 0; i < P.n_scratch; ++i) { scratch[i] = q; q += P.bytes_scratch; }
         if ((size_t)(q - base) != P.workspace_bytes) return HCLOOC_ERR_INTERNAL;
     }
     // ---------------------------------------------------------------- events
-    const size_t n_events = 3 * (size_t)P.n_sets + 2 * (size_t)P.n_bbuf + (size_t)P.n_abuf;
+    const size_t n_events = 3 * (size_t)P.n_sets + 2 * (size_t)P.n_bbuf + 2 * (size_t)P.n_abuf;
     while (ctx->events.size() < n_events) {
         cudaEvent_t e;
         HCL_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
@@ -419,6 +426,8 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
     }
     // ---------------------------------------------------------------- S2-S7: issue the schedule
     build_schedule(P, ctx->n_compute, ctx->ops);
+    for (int i = 0; i < P.n_scratch && i < ctx->n_compute; ++i)   // stream-K tile counters start at zero
+        HCL_CUDA(cudaMemsetAsync(scratch[i] + streamk_counter_offset(), 0, streamk_counter_bytes(), ctx->s_compute[i]));
     auto stream_of = [&](int s) { return s == 0 ? ctx->s_h2d : (s == 1 ? ctx->s_d2h : ctx->s_compute[s - 2]); };
     uint64_t bytes_h2d = 0, bytes_d2h = 0, n_h2d = 0, n_d2h = 0, n_kernels = 0;
     const auto t_enq0 = std::chrono::steady_clock::now();
@@ -478,7 +487,8 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
             case HCLOOC_OP_GEMM: {
                 const double b_eff = (o.beta < 0.0) ? beta : o.beta;
                 rc = launch_dgemm_tiles(o.nr, o.nc, o.kk, scale_only ? 0.0 : alpha, o.buf >= 0 ? bufs[o.buf] : nullptr, P.lda_dev,
-                                        o.buf2 >= 0 ? bufs[o.buf2] : nullptr, P.ldb_dev, b_eff, bufs[o.buf3], P.ldc_dev, st, P.ksplit > 0 ? P.ksplit : 1);
+                                        o.buf2 >= 0 ? bufs[o.buf2] : nullptr, P.ldb_dev, b_eff, bufs[o.buf3], P.ldc_dev, st,
+                                        P.ksplit != 0 ? P.ksplit : 1, P.ksplit < 0 ? scratch[o.stream - 2] : nullptr);
                 ++n_kernels;
                 break;
             }

@@ -5,6 +5,8 @@
 #include <stddef.h>
 #include "../../include/hclooc.h"
 
+struct CUtensorMap_st;   // <cuda.h>
+
 namespace hclooc {
 
 // last CUDA error seen on this thread (hclooc_last_cuda_error)
@@ -33,7 +35,19 @@ const MachineModel& machine_model();
 // Preconditions (checked by callers): pointers 16-byte aligned, leading dimensions even.
 int launch_dgemm_tiles(int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda,
                        const double* dB, int64_t ldb, double beta, double* dC, int64_t ldc,
-                       cudaStream_t stream, int ksplit);   // ksplit: 1, 2, 4, or 0 = choose from the tile count
+                       cudaStream_t stream, int ksplit,    // ksplit: 1, 2, 4; 0 = choose from the tile count;
+                       void* streamk_scratch = nullptr);   // -1 = the launch has the GPU to itself: persistent stream-K
+                                                           //      (scratch: streamk_scratch_bytes(), or NULL = library pool)
+
+// The persistent stream-K kernel (dgemm_streamk_sm100.cu).  Returns 1 if it does not apply (no scratch buffer
+// free, shape out of range): the caller then launches one CTA per tile.
+int launch_dgemm_streamk(int64_t M, int64_t N, int64_t K, double alpha, const ::CUtensorMap_st& tmA, const ::CUtensorMap_st& tmB,
+                         double beta, double* dC, int64_t ldc, cudaStream_t stream, void* scratch);
+size_t streamk_scratch_bytes();     // one scratch buffer (partial-tile slots + counters), rounded to 1 KiB
+size_t streamk_counter_offset();    // the counters inside it must be zero before the first launch
+size_t streamk_counter_bytes();
+// Work split of a stream-K launch: G persistent CTAs, dp_waves whole-tile waves, tail_tiles tiles cut along K.
+bool streamk_layout(int64_t M, int64_t N, int64_t K, int num_sms, int* G, int* dp_waves, int* tail_tiles);
 
 // K split (cluster size) worth using when `tiles_in_flight` tiles can run concurrently
 int dgemm_auto_ksplit(int64_t tiles_in_flight, int64_t K);

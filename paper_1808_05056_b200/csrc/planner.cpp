@@ -34,6 +34,7 @@ constexpr int64_t LD_ALIGN = 16;       // device leading dimensions are multiple
 constexpr uint64_t BUF_ALIGN = 1024;   // every device buffer starts on a 1 KiB boundary
 constexpr int NUM_SMS = 148;
 constexpr double OVERLAP_PENALTY = 0.10;
+constexpr double STREAMK_MIN_TILES = 32;
 }  // namespace
 
 const MachineModel& machine_model() {
@@ -52,12 +53,18 @@ namespace {
 
 struct Cand {
     int64_t mb, nb, kb, h, w, kpanels;
-    int n_sets, n_abuf, n_bbuf, ksplit;
+    int n_sets, n_abuf, n_bbuf, ksplit, n_scratch;
     int64_t lda_dev, ldb_dev, ldc_dev;
     uint64_t a_bytes, b_bytes, c_bytes, ws_bytes;
     uint64_t bytes_h2d, bytes_d2h, n_h2d, n_d2h;
     double t_flop, t_link, t_model;
 };
+
+// Budget share kept free for the two stream-K scratch buffers (only when that is at most 5 % of the budget).
+uint64_t streamk_reserve(uint64_t budget) {
+    const uint64_t need = 2 * (uint64_t)streamk_scratch_bytes();
+    return need * 20 <= budget ? need : 0;
+}
 
 // Exact host<->device traffic of the schedule the executor builds from this candidate (executor.cu
 // build_schedule): columns of blocks in order, rows in serpentine order, A slices in an LRU cache of
@@ -103,7 +110,7 @@ void fill_traffic(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool s
     c.n_d2h = steps;
 }
 
-void cost(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool scale_only, const MachineModel& mm) {
+void cost(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool scale_only, const MachineModel& mm, uint64_t budget) {
     fill_traffic(c, M, N, K, beta_nz, scale_only);
     const double steps = (double)c.h * c.w * c.kpanels;
     const double flops = scale_only ? 0.0 : 2.0 * (double)M * (double)N * (double)K;
@@ -124,20 +131,45 @@ void cost(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool scale_onl
     const bool link_bound = c.t_link > c.t_flop / std::max(1e-3, pad_eff);
     const double steps_in_flight = link_bound ? 1.0 : (double)std::max(1, c.n_sets - 2);
     c.ksplit = scale_only ? 1 : (force_ks ? force_ks : dgemm_auto_ksplit((int64_t)(steps_in_flight * tiles_step), c.kb));
-    const double in_flight = std::max(1, c.n_sets - 2) * tiles_step * c.ksplit;
+    // Optional (HCLOOC_STREAMK_STEPS=1): compute-bound plans run every step as ONE persistent stream-K launch on
+    // all SMs, two compute streams alternating; costs two scratch buffers inside the budget and ~10 us per step.
+    // Measured on config 4: 0.969 of the FP64 peak against 0.976 for well-shaped steps whose one-CTA-per-tile
+    // kernels overlap on several streams, so it is not the default.
+    static const bool streamk_steps = std::getenv("HCLOOC_STREAMK_STEPS") != nullptr;   // off by default: measured 0.7 % behind
+    const bool want_streamk = streamk_steps && !scale_only && !link_bound && !force_ks && tiles_step >= STREAMK_MIN_TILES &&
+                              c.kb >= 256 && streamk_reserve(budget) > 0 && c.ws_bytes + streamk_reserve(budget) <= budget;
+    c.n_scratch = want_streamk ? 2 : 0;
+    if (want_streamk) c.ksplit = -1;
+    const double in_flight = want_streamk ? (double)NUM_SMS : std::max(1, c.n_sets - 2) * tiles_step * c.ksplit;
     double fill = std::min(1.0, in_flight / NUM_SMS);
-    if (tiles_step >= NUM_SMS) fill = std::min(fill, 0.98);
-    const double t_compute = c.t_flop / std::max(1e-3, pad_eff * fill) + steps * 1e-6;
+    if (!want_streamk && tiles_step >= NUM_SMS) fill = std::min(fill, 0.98);
+    if (!want_streamk && fill >= 1.0 && tiles_step < NUM_SMS) fill = 0.975;     // measured: kernels of several steps interleave imperfectly
+    if (!want_streamk && c.n_sets < 4) fill *= (c.n_sets == 2 ? 0.96 : 0.985);  // too few C blocks in flight to fill the wave tails
+    const double t_compute = c.t_flop / std::max(1e-3, pad_eff * fill) + steps * (want_streamk ? 10e-6 : 1e-6);
     const bool cload = beta_nz || c.kpanels > 1;
     const double t_pro = ((double)c.b_bytes + (double)c.a_bytes + (cload ? (double)c.c_bytes : 0.0)) / mm.h2d_Bps + 3 * mm.copy_latency_s;
     // one step's kernel running alone: what the link waits for when a column drains, and the tail of the call
-    const double sms_step = std::min<double>(NUM_SMS, tiles_step * c.ksplit);
+    const double sms_step = c.ksplit < 0 ? (double)NUM_SMS : std::min<double>(NUM_SMS, tiles_step * c.ksplit);
     const double t_kernel = (flops / std::max(1.0, steps)) / (mm.fp64_flops * sms_step / NUM_SMS) + mm.launch_latency_s;
     const double switches = (double)c.w * c.kpanels - 1.0;
-    double comp_path = t_pro + t_compute;
-    double link_path = c.t_link;
+    // Column by column: the first column of a K panel uploads every A slice, the later ones only what the cache
+    // lost, so the link demand is front-loaded -- a plan with many thin columns is link-bound in its first column
+    // even when the whole call is compute-bound (measured: config 4 with 47 columns lost 2 % there).
+    const double n_cols = (double)c.w * c.kpanels;
+    const double comp_col = t_compute / n_cols;
+    const double a_first = scale_only ? 0.0 : 8.0 * (double)M * (double)c.kb;
+    const double a_all = (double)c.bytes_h2d - 8.0 * (double)K * (double)N - (beta_nz ? 8.0 * (double)M * (double)N : 0.0) -
+                         (c.kpanels > 1 ? 8.0 * (double)(c.kpanels - 1) * (double)M * (double)N : 0.0);
+    const double a_later = n_cols > c.kpanels ? std::max(0.0, a_all - a_first * c.kpanels) / (n_cols - c.kpanels) : 0.0;
+    const double c_col = 8.0 * (double)M * (double)c.nb;
+    auto link_col = [&](double a_bytes) {
+        const double up = a_bytes + (scale_only ? 0.0 : (double)c.b_bytes) + (cload ? c_col : 0.0);
+        const double lat = (double)c.h * 2.0 * mm.copy_latency_s;
+        return std::max(std::max(up / mm.h2d_Bps, c_col / mm.d2h_Bps), (up + c_col) / mm.duplex_Bps) + lat;
+    };
+    double stall_comp = 0.0, stall_link = 0.0;      // per column switch, with a single B buffer
     if (c.n_bbuf == 1) {
-        comp_path += switches * ((double)c.b_bytes / mm.h2d_Bps);   // compute idles while the next B slice loads
+        stall_comp = (double)c.b_bytes / mm.h2d_Bps;                  // compute idles while the next B slice loads
         // the link idles (a) while the last kernels of a column drain before S(b_j) may overwrite the buffer,
         // less the uploads issued ahead of the reload, and (b) after the reload once every C buffer is held by
         // a step whose kernel has only just started
@@ -146,12 +178,19 @@ void cost(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool scale_onl
         const double pre = (double)early_uploads(c.h, c.n_sets, c.n_abuf);
         const double drain = std::max(0.0, t_kernel - pre * t_cup);
         const double refill = std::max(0.0, t_kernel + (double)c.c_bytes / mm.d2h_Bps - std::max(0.0, c.n_sets - pre - 1.0) * t_up);
-        link_path += switches * (drain + refill);
+        stall_link = drain + refill;
     }
+    const double l_first = link_col(a_first), l_later = link_col(a_later);
+    const double body = c.kpanels * std::max(comp_col + stall_comp, l_first + stall_link) +
+                        (n_cols - c.kpanels) * std::max(comp_col + stall_comp, l_later + stall_link);
+    const double comp_path = t_pro + t_compute, link_path = c.t_link;
     const double t_tail = t_kernel + (double)c.c_bytes / mm.d2h_Bps + mm.copy_latency_s;
     // imperfect overlap: the shorter path still costs a fraction of its length (bursty uploads, shared
     // DMA/HBM resources), which also keeps plans away from the edge where link time ~ compute time
-    c.t_model = std::max(comp_path, link_path) + OVERLAP_PENALTY * std::min(comp_path, link_path) + t_tail + mm.launch_latency_s;
+    c.t_model = t_pro + body + OVERLAP_PENALTY * std::min(comp_path, link_path) + t_tail + mm.launch_latency_s;
+    // between near-equal plans take the one whose slices are whole tiles: padded tiles burn FP64 issue slots and
+    // power for nothing even when the link hides their time
+    c.t_model *= 1.0 + 0.15 * (1.0 - pad_eff);
 }
 
 }  // namespace
@@ -250,11 +289,13 @@ extern "C" int hclooc_plan_ex(int64_t M, int64_t N, int64_t K, int beta_nonzero,
                         if (c.ws_bytes > S) continue;
                         if (!scale_only && c.w > 1 && c.a_bytes > 0) {
                             // spare budget holds more A slices: more reuse at every column switch
-                            const int64_t extra = std::min<int64_t>((int64_t)((S - c.ws_bytes) / c.a_bytes), std::max<int64_t>(0, c.h - c.n_abuf));
+                            const uint64_t room = S - c.ws_bytes > streamk_reserve(S) ? S - c.ws_bytes - streamk_reserve(S) : 0;
+                            const int64_t extra = std::min<int64_t>((int64_t)(room / c.a_bytes), std::max<int64_t>(0, c.h - c.n_abuf));
                             const int64_t capped = std::min<int64_t>(extra, force_abuf ? std::max<int64_t>(0, force_abuf - c.n_abuf) : 256 - c.n_abuf);
                             if (capped > 0) { c.n_abuf += (int)capped; c.ws_bytes += (uint64_t)capped * c.a_bytes; }
                         }
-                        cost(c, M, N, Keff, beta_nz, scale_only, mm);
+                        cost(c, M, N, Keff, beta_nz, scale_only, mm, S);
+                        c.ws_bytes += (uint64_t)c.n_scratch * streamk_scratch_bytes();
                         const double steps = (double)c.h * c.w * c.kpanels, bsteps = (double)best.h * best.w * best.kpanels;
                         if (!found || c.t_model < best.t_model * (1 - 1e-9) ||
                             (c.t_model <= best.t_model * (1 + 1e-9) && steps < bsteps)) {
@@ -274,6 +315,7 @@ extern "C" int hclooc_plan_ex(int64_t M, int64_t N, int64_t K, int beta_nonzero,
     out->lda_dev = best.lda_dev; out->ldb_dev = best.ldb_dev; out->ldc_dev = best.ldc_dev;
     out->bytes_a_buf = best.a_bytes; out->bytes_b_buf = best.b_bytes; out->bytes_c_buf = best.c_bytes;
     out->workspace_bytes = best.ws_bytes;
+    out->n_scratch = best.n_scratch; out->bytes_scratch = best.n_scratch ? streamk_scratch_bytes() : 0;
     out->bytes_h2d = best.bytes_h2d; out->bytes_d2h = best.bytes_d2h;
     out->n_copies_h2d = best.n_h2d; out->n_copies_d2h = best.n_d2h;
     out->flops = scale_only ? 0.0 : 2.0 * (double)M * (double)N * (double)K;

@@ -95,11 +95,12 @@ int hclMemcpy2DAsync(void* dst, size_t dpitch, const void* src, size_t spitch, s
     }
     return finish_async((cudaStream_t)s, ev);
 }
-int hclDgemmAsync(int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda, const double* dB,
-                  int64_t ldb, double beta, double* dC, int64_t ldc, hclStream s, hclEvent* ev) {
+int hclDgemmAsyncEx(int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda, const double* dB,
+                  int64_t ldb, double beta, double* dC, int64_t ldc, hclStream s, hclEvent* ev, int variant) {
     if (M < 0) return -1;
     if (N < 0) return -2;
     if (K < 0) return -3;
+    if (variant != HCL_DGEMM_AUTO && variant != -1 && variant != 1 && variant != 2 && variant != 4) return -14;
     const bool noab = (alpha == 0.0 || K == 0);
     if (M > 0 && N > 0) {
         if (!noab) {
@@ -111,10 +112,15 @@ int hclDgemmAsync(int64_t M, int64_t N, int64_t K, double alpha, const double* d
         }
         if (!dC) return -10;
         if (ldc < N) return -11;
-        int rc = launch_dgemm_tiles(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, (cudaStream_t)s, 0);
+        int rc = launch_dgemm_tiles(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, (cudaStream_t)s,
+                                    variant == HCL_DGEMM_AUTO ? (dgemm_tile_count(M, N) >= 148 ? -1 : 0) : variant);
         if (rc) return rc;
     }
     return finish_async((cudaStream_t)s, ev);
+}
+int hclDgemmAsync(int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda, const double* dB, int64_t ldb,
+                  double beta, double* dC, int64_t ldc, hclStream s, hclEvent* ev) {
+    return hclDgemmAsyncEx(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, s, ev, HCL_DGEMM_AUTO);
 }
 int hclWaitEvent(hclStream s, hclEvent e) {
     if (!e) return -2;

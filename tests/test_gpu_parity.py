@@ -364,3 +364,54 @@ def test_device_resident_operands_run_in_core(H):
     st = H.hclooc_dgemm_ex(None, M, N, K, 2.0, dA, K, dB, N, -1.0, dC3, N + 1, 1 * MiB)
     assert st.n_kernels > 1
     assert np.array_equal(dC3[:, :N].cpu().numpy(), ref) and float(dC3[:, N].abs().max()) == 0.0
+
+
+@pytest.mark.parametrize("M,N,K,dist", [
+    (1700, 1500, 1040, "int"),        # 14 x 12 = 168 tiles >= 148 SMs: one wave joins the stream-K tail, ragged edges
+    (1700, 1500, 1040, "uniform"),
+    (2048, 2432, 512, "int"),         # 16 x 19 = 304 tiles = 2 waves + 8: data-parallel wave + tail
+    (384, 640, 4100, "int"),          # 15 tiles < 148: every tile is cut along K among several CTAs
+    (128, 128, 70000, "uniform"),     # one tile shared by 148 CTAs
+    (130, 120, 16, "int"),            # a single k block per tile: nothing to split
+])
+def test_streamk_kernel_matches_oracle(H, M, N, K, dist):
+    """The persistent stream-K kernel (in-core path of hclooc_dgemm_ex on device operands): partial tiles are
+    summed in k order by whichever CTA arrives last, so the result is deterministic -- launched three times on
+    the same inputs (the scratch counters must reset themselves) and compared with the oracle each time."""
+    import torch
+    A = synthgen.fill(np.empty((M, K)), 61, "A", dist)
+    B = synthgen.fill(np.empty((K, N)), 61, "B", dist)
+    C0 = synthgen.fill(np.empty((M, N)), 61, "C", dist)
+    ref = C0.copy()
+    D = oracle.dgemm(1.5, A, B, -0.5, ref, want_denominator=True)
+    dA, dB = torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda()
+    outs = []
+    for rep in range(3):
+        dC = torch.from_numpy(C0).cuda()
+        st = H.hclooc_dgemm_ex(None, M, N, K, 1.5, dA, K, dB, N, -0.5, dC, N, 0)
+        assert st.n_kernels == 1
+        outs.append(dC.cpu().numpy())
+        check(outs[-1], ref, D, exact=(dist == "int"))
+    assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])      # bitwise repeatable
+
+
+def test_streamk_launches_on_two_streams_do_not_share_scratch(H):
+    """Concurrent stream-K launches (hclDgemmAsync on two streams) each get a scratch buffer of their own."""
+    import torch
+    M, N, K = 1700, 1500, 1040
+    A = synthgen.fill(np.empty((M, K)), 62, "A", "int")
+    B = synthgen.fill(np.empty((K, N)), 62, "B", "int")
+    C0 = synthgen.fill(np.empty((M, N)), 62, "C", "int")
+    ref = C0.copy()
+    oracle.dgemm(1.0, A, B, 1.0, ref)
+    dA, dB = torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda()
+    streams = [torch.cuda.Stream() for _ in range(3)]
+    dCs = [[torch.from_numpy(C0).cuda() for _ in range(4)] for _ in streams]
+    torch.cuda.synchronize()
+    for r in range(4):
+        for s, row in zip(streams, dCs):
+            H.hclDgemmAsync(M, N, K, 1.0, dA, K, dB, N, 1.0, row[r], N, s)
+    torch.cuda.synchronize()
+    for row in dCs:
+        for dC in row:
+            assert np.array_equal(dC.cpu().numpy(), ref)

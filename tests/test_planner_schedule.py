@@ -90,7 +90,7 @@ CONFIGS = {  # BASELINE.json configs: (M, N, K, beta != 0, budget)
 
 def plan_checks(p, M, N, K, bnz, budget):
     assert p.workspace_bytes <= budget
-    assert p.workspace_bytes == p.n_bbuf * p.bytes_b_buf + p.n_abuf * p.bytes_a_buf + p.n_sets * p.bytes_c_buf
+    assert p.workspace_bytes == p.n_bbuf * p.bytes_b_buf + p.n_abuf * p.bytes_a_buf + p.n_sets * p.bytes_c_buf + p.n_scratch * p.bytes_scratch
     assert p.h == -(-M // p.mb) and p.w == -(-N // p.nb)
     assert p.n_steps == p.h * p.w * p.kpanels and p.n_sets >= 2
     assert p.ldc_dev >= p.nb and p.ldc_dev % 2 == 0 and p.bytes_c_buf >= p.mb * p.ldc_dev * 8
@@ -128,6 +128,9 @@ def test_plans_for_the_baseline_configs(name):
         assert p.t_link_s > p.t_flop_s
     else:                                       # FP64-bound
         assert p.t_flop_s > p.t_link_s
+    assert p.n_scratch == 0 and p.ksplit >= 1
+    if name in ("cfg3", "cfg4"):
+        simulate(p, H.hclooc_schedule(p, 8))
     if name == "cfg2":
         assert p.w == 3 and p.bytes_h2d < 8 * 5 * 8192 * 8192     # 5 matrix volumes minus the reused A slices
 
@@ -325,3 +328,35 @@ def test_random_plans_simulate_clean(monkeypatch, bbuf):
         simulate(p, H.hclooc_schedule(p, int(rng.integers(1, 9))))
         done += 1
     assert done > 40
+
+
+def test_cached_slices_read_by_many_columns_then_overwritten(monkeypatch):
+    """All A slices of a K panel stay cached and are read by every column of blocks (3+ readers per buffer,
+    recorded alternately into two events); the next K panel then overwrites them.  The upload must wait for
+    every reader, not just the last one."""
+    monkeypatch.setenv("HCLOOC_FORCE_MB", "32")          # experiment knob: two row slices, both cached
+    found = 0
+    for budget in (1 * MiB, 1536 * 1024, 2 * MiB, 3 * MiB):
+        p = H.hclooc_plan(64, 1500, 9000, 1, 0, budget)
+        assert p.kpanels > 1 and p.w >= 3 and p.h <= p.n_abuf
+        for ncs in (1, 4, 8):
+            ops = H.hclooc_schedule(p, ncs)
+            simulate(p, ops)
+            assert int((ops["kind"] == K_H2D_A).sum()) == p.h * p.kpanels      # one upload per slice and panel
+        found += 1
+    assert found == 4
+
+
+def test_streamk_steps_use_one_scratch_buffer_per_compute_stream():
+    """Experiment knob HCLOOC_STREAMK_STEPS (read once per process, so in a subprocess): compute-bound plans run
+    each step as one persistent stream-K launch; the schedule then uses as many compute streams as the plan has
+    scratch buffers, and the scratch is part of the workspace."""
+    import subprocess, sys
+    code = ("import paper_1808_05056_b200 as H, numpy as np\n"
+            "p = H.hclooc_plan(65536, 65536, 16384, 1, 0, 16 << 30)\n"
+            "ops = H.hclooc_schedule(p, 8)\n"
+            "print(p.ksplit, p.n_scratch, int(p.bytes_scratch > 0), sorted(set(int(x) for x in ops['stream'][ops['kind'] == 3])),"
+            " int(p.workspace_bytes == p.n_bbuf * p.bytes_b_buf + p.n_abuf * p.bytes_a_buf + p.n_sets * p.bytes_c_buf + p.n_scratch * p.bytes_scratch))")
+    out = subprocess.run([sys.executable, "-c", code], cwd=ROOT, env=dict(os.environ, HCLOOC_STREAMK_STEPS="1"),
+                         capture_output=True, text=True, check=True).stdout.strip()
+    assert out == "-1 2 1 [2, 3] 1", out
