@@ -184,6 +184,18 @@ int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K, double alp
                     int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
                     size_t device_budget_bytes, hclooc_stats* stats_out);
 
+/* The paper's own pipeline, Figure 2 (:182-271), written against the hcl* runtime calls below and kept for
+ * comparison with the tuned scheduler: hclMatrixPartitioner's equal slices (h | M, w | N),
+ * steps in column-major order, TWO round-robin streams, five event families (eA, rA, rB, eC, rC), double
+ * buffered A slice and C block, a single B buffer reloaded un-overlapped at i == h-1; in-core (one upload,
+ * one DGEMM, one download) when A, B and C fit device_budget_bytes together (:130, :368).  Same arguments,
+ * result and error codes as hclooc_dgemm (M, N, K > 0 required: -1/-2/-3); allocates its device buffers with
+ * hclMalloc per call (at most device_budget_bytes; 0 = free HBM minus 1 GiB).  stats (nullable): plan.h/w/mb/nb,
+ * byte and copy counts, n_kernels; t_total_s runs from the first enqueue to both streams drained.        */
+int hclooc_dgemm_fig2(int64_t M, int64_t N, int64_t K, double alpha, const double* A, int64_t lda,
+                      const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
+                      size_t device_budget_bytes, hclooc_stats* stats);
+
 /* ------------------------------------------------------------------ the runtime the paper abstracts (:109-116, :212)
  * CUDA only, plain functions (no virtual dispatch, cf. :164).                                      */
 int hclMalloc(void** dptr, size_t bytes);                         /* :109  device memory            */

@@ -14,7 +14,7 @@ HCL_H2D, HCL_D2H = 0, 1
 EXPORTS = [
     "hclooc_plan", "hclooc_plan_ex", "hclMatrixPartitioner", "hclooc_schedule", "hclooc_ctx_create", "hclooc_ctx_destroy",
     "hclooc_ctx_set_trace", "hclooc_ctx_get_trace",
-    "hclooc_dgemm", "hclooc_dgemm_ex", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
+    "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_fig2", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
     "hclStreamDestroy", "hclEventDestroy", "hclMemcpy", "hclMemcpyAsync", "hclMemcpy2DAsync",
     "hclDgemmAsync", "hclDgemmAsyncEx", "hclWaitEvent", "hclStreamSynchronize", "hclDeviceSynchronize",
     "hclooc_host_alloc", "hclooc_host_free", "hclooc_host_register", "hclooc_host_unregister",
@@ -81,6 +81,7 @@ def lib():
         L.hclooc_ctx_get_trace.argtypes = [vp, vp, sz, POINTER(sz)]
         L.hclooc_dgemm.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz]
         L.hclooc_dgemm_ex.argtypes = [vp, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
+        L.hclooc_dgemm_fig2.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
         L.hclMalloc.argtypes = [POINTER(vp), sz]
         L.hclFree.argtypes = [vp]
         L.hclGetMemSize.argtypes = [c_int, POINTER(sz)]
@@ -249,6 +250,14 @@ def hclooc_dgemm_ex(ctx, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_bu
     st = Stats()
     _check(lib().hclooc_dgemm_ex(ctx, M, N, K, alpha, _ptr(A), lda, _ptr(B), ldb, beta, _ptr(C), ldc,
                                  device_budget_bytes, byref(st) if want_stats else None), "hclooc_dgemm_ex")
+    return st if want_stats else None
+
+
+def hclooc_dgemm_fig2(M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes, want_stats=True):
+    """The paper's Figure 2 pipeline over the hcl* runtime calls (two streams, five event families)."""
+    st = Stats()
+    _check(lib().hclooc_dgemm_fig2(M, N, K, alpha, _ptr(A), lda, _ptr(B), ldb, beta, _ptr(C), ldc,
+                                   device_budget_bytes, byref(st) if want_stats else None), "hclooc_dgemm_fig2")
     return st if want_stats else None
 
 

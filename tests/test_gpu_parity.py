@@ -415,3 +415,30 @@ def test_streamk_launches_on_two_streams_do_not_share_scratch(H):
     for row in dCs:
         for dC in row:
             assert np.array_equal(dC.cpu().numpy(), ref)
+
+
+@pytest.mark.parametrize("M,N,K,alpha,beta,budget,dist", [
+    (512, 512, 512, 1.0, 0.5, 1 * MiB, "int"),          # configs[0]: every block streams
+    (512, 512, 512, 1.0, 0.5, 1 * MiB, "uniform"),
+    (4, 4, 8, 1.0, 1.0, 44 * 8, "int"),                 # the paper's worked example (:301): h = 4, w = 2, 8 steps
+    (768, 640, 300, 2.0, 0.0, 2 * MiB, "int"),          # beta == 0: C is not uploaded, NaN in C is overwritten
+    (384, 1030, 257, -1.0, 1.0, 3 * MiB, "int"),        # odd slice widths (device leading dimensions padded)
+    (300, 200, 100, 1.0, 1.0, 64 * MiB, "int"),         # fits: the in-core case, one step
+])
+def test_fig2_pipeline_matches_oracle(H, M, N, K, alpha, beta, budget, dist):
+    """hclooc_dgemm_fig2: the paper's Figure 2 (two round-robin streams, eA/rA/rB/eC/rC events, single B buffer)
+    over the hcl* runtime calls gives the oracle's values; its traffic is the paper's w*M*K + K*N + M*N."""
+    A, B, C = host_inputs(H, M, N, K, 71, dist, poison_c=(beta == 0.0))
+    ref = C.view.copy() if beta != 0.0 else np.zeros((M, N))
+    D = oracle.dgemm(alpha, A.view, B.view, beta, ref, want_denominator=True)
+    st = H.hclooc_dgemm_fig2(M, N, K, alpha, A, A.ld, B, B.ld, beta, C, C.ld, budget)
+    check(C.view, ref, D, exact=(dist == "int"))
+    h, w = st.plan.h, st.plan.w
+    if 8 * (M * K + K * N + M * N) <= budget:
+        assert (h, w) == (1, 1) and st.n_kernels == 1
+    else:
+        assert (h, w) == H.hclMatrixPartitioner(M, N, K, budget // 8) and st.n_kernels == h * w
+    assert st.bytes_h2d == 8 * (w * M * K + K * N + (M * N if beta != 0.0 else 0)) and st.bytes_d2h == 8 * M * N
+    assert st.plan.workspace_bytes <= budget
+    if (M, N, K) == (4, 4, 8):
+        assert (h, w) == (4, 2)                           # Figure 3 (:281)
