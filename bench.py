@@ -15,8 +15,9 @@ S6 download, S7 events) over one synthetic problem: hclooc_dgemm(M,N,K,alpha,A,l
           (mb x nb x K with plan.ksplit CTAs per tile), against the peak of the SMs that launch occupies.
   cpu_baseline : the oracle, as it stands, on the host cores, on a bounded row sample of the same workload.
 
-`--impl reference` times the oracle (the reference arm of this tier).  Under torchrun every rank runs an
-independent replica on its own GPU ("replicas only": the path is single-GPU, DESIGN.md multi-GPU).
+`--impl reference` times the oracle (the reference arm of this tier).  Under torchrun the problem grows to
+world*M rows cut into one row band of C per GPU (independent bands, B on every rank, no collective: weak
+scaling; DESIGN.md "Multi-GPU").
 """
 import argparse
 import json
@@ -168,13 +169,18 @@ def run_ours(args, wl, name):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     M, N, K, alpha, beta, budget = wl["M"], wl["N"], wl["K"], wl["alpha"], wl["beta"], wl["budget"]
-    seed = synthgen.BASE_SEED + wl["seed_idx"] + 1000 * rank
+    seed = synthgen.BASE_SEED + wl["seed_idx"]
     flops = 2.0 * M * N * K
+    # N > 1: ONE problem of world*M rows cut into row bands of C (hclooc_shard_rows): rank r owns rows r*M .. of A
+    # and C, every rank holds all of B; the bands are independent, so no collective is on
+    # the data path and per-GPU work is fixed as N grows (weak scaling).
+    row0, rows = H.hclooc_shard_rows(world * M, world, rank, 128)
+    assert (row0, rows) == (rank * M, M) or M % 128
 
     # ---- inputs: pinned host matrices (the product path) and HBM-resident copies (the `value` leg)
     A, B, C = H.HostMatrix(M, K), H.HostMatrix(K, N), H.HostMatrix(M, N)
-    synthgen.fill(A.array, seed, "A", wl["dist"]); synthgen.fill(B.array, seed, "B", wl["dist"])
-    synthgen.fill(C.array, seed, "C", wl["dist"])
+    synthgen.fill(A.array, seed, "A", wl["dist"], row0=rank * M); synthgen.fill(B.array, seed, "B", wl["dist"])
+    synthgen.fill(C.array, seed, "C", wl["dist"], row0=rank * M)
     dA, dB, dC = (torch.from_numpy(X.array).cuda() for X in (A, B, C))
 
     # ---- PyTorch owns device memory and streams; the library carves its buffers from this workspace
@@ -263,7 +269,8 @@ def run_ours(args, wl, name):
         "warmup": max(args.warmup, 3), "ms_per_step": ms_res, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": f"{name}: {wl['desc']}", "M": M, "N": N, "K": K, "alpha": alpha, "beta": beta,
-                   "device_budget_bytes": budget, "dist": wl["dist"], "parallelism": "replicas only" if world > 1 else "1 GPU",
+                   "device_budget_bytes": budget, "dist": wl["dist"], "parallelism": (f"{world} row bands of C of {M} rows each, one per GPU (hclooc_shard_rows), B on every rank, no collective"
+                                   if world > 1 else "1 GPU"), "M_global": world * M,
                    "plan": {k: getattr(plan, k) for k in ("mb", "nb", "kb", "h", "w", "kpanels", "n_steps", "n_sets", "n_bbuf", "workspace_bytes")},
                    "l2": "inputs (A+B+C = %.2f GB) exceed the 126 MB L2; no flush needed" % ((M * K + K * N + M * N) * 8 / 1e9),
                    "value_leg": "A,B,C resident in HBM: in-core case, one tile-kernel launch over the whole problem, nothing staged"},

@@ -184,6 +184,14 @@ int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K, double alp
                     int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
                     size_t device_budget_bytes, hclooc_stats* stats_out);
 
+/* Multi-GPU (SURVEY 8(e); the paper's future work, :414): the row blocks of C are independent (:289, :293), so
+ * G processes, one per GPU, each take a contiguous band of the rows of A and C and all of B, and call
+ * hclooc_dgemm on their band -- no exchange step, no collective.  This returns the band of `rank`: the M rows
+ * are cut into `world` near-equal bands whose sizes are multiples of `align` rows (128 = the kernel's tile
+ * edge; 1 = any), the remainder going to the last non-empty band; trailing ranks may get rows = 0.
+ * Errors: -1 M < 0, -2 world < 1, -3 rank outside [0, world), -4 align < 1, -5/-6 NULL.              */
+int hclooc_shard_rows(int64_t M, int world, int rank, int64_t align, int64_t* row0, int64_t* rows);
+
 /* The paper's own pipeline, Figure 2 (:182-271), written against the hcl* runtime calls below and kept for
  * comparison with the tuned scheduler: hclMatrixPartitioner's equal slices (h | M, w | N),
  * steps in column-major order, TWO round-robin streams, five event families (eA, rA, rB, eC, rC), double

@@ -12,7 +12,7 @@ HCL_H2D, HCL_D2H = 0, 1
 
 # every symbol include/hclooc.h declares (tests check the .so exports all of them)
 EXPORTS = [
-    "hclooc_plan", "hclooc_plan_ex", "hclMatrixPartitioner", "hclooc_schedule", "hclooc_ctx_create", "hclooc_ctx_destroy",
+    "hclooc_plan", "hclooc_plan_ex", "hclooc_shard_rows", "hclMatrixPartitioner", "hclooc_schedule", "hclooc_ctx_create", "hclooc_ctx_destroy",
     "hclooc_ctx_set_trace", "hclooc_ctx_get_trace",
     "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_fig2", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
     "hclStreamDestroy", "hclEventDestroy", "hclMemcpy", "hclMemcpyAsync", "hclMemcpy2DAsync",
@@ -72,6 +72,7 @@ def lib():
         L = ctypes.CDLL(_build.build())
         i64, dbl, vp, sz = c_int64, c_double, c_void_p, c_size_t
         L.hclooc_plan.argtypes = [i64, i64, i64, c_int, c_int, sz, POINTER(Plan)]
+        L.hclooc_shard_rows.argtypes = [i64, c_int, c_int, i64, POINTER(i64), POINTER(i64)]
         L.hclooc_plan_ex.argtypes = [i64, i64, i64, c_int, c_int, sz, c_int, POINTER(Plan)]
         L.hclMatrixPartitioner.argtypes = [i64, i64, i64, i64, POINTER(i64), POINTER(i64)]
         L.hclooc_schedule.argtypes = [POINTER(Plan), c_int, vp, sz, POINTER(sz)]
@@ -193,6 +194,13 @@ def hclooc_plan_ex(M, N, K, beta_nonzero, alpha_zero, device_budget_bytes, opera
     _check(lib().hclooc_plan_ex(M, N, K, int(bool(beta_nonzero)), int(bool(alpha_zero)), device_budget_bytes,
                                 int(bool(operands_on_device)), byref(p)), "hclooc_plan_ex")
     return p
+
+
+def hclooc_shard_rows(M, world, rank, align=128):
+    """(row0, rows) of the band of C (and A) that process `rank` of `world` owns."""
+    r0, n = c_int64(), c_int64()
+    _check(lib().hclooc_shard_rows(M, world, rank, align, byref(r0), byref(n)), "hclooc_shard_rows")
+    return r0.value, n.value
 
 
 def hclMatrixPartitioner(M, N, K, budget_elements):

@@ -356,3 +356,21 @@ extern "C" int hclMatrixPartitioner(int64_t M, int64_t N, int64_t K, int64_t bud
     *h = bh; *w = bw;
     return HCLOOC_OK;
 }
+
+// Row bands for one process per GPU: independent C row blocks, no exchange step.
+extern "C" int hclooc_shard_rows(int64_t M, int world, int rank, int64_t align, int64_t* row0, int64_t* rows) {
+    if (M < 0) return -1;
+    if (world < 1) return -2;
+    if (rank < 0 || rank >= world) return -3;
+    if (align < 1) return -4;
+    if (!row0) return -5;
+    if (!rows) return -6;
+    const int64_t units = ceil_div(M, align);                  // bands are whole units of `align` rows
+    const int64_t base = units / world, extra = units % world; // the first `extra` ranks get one unit more
+    const int64_t u0 = rank * base + std::min<int64_t>(rank, extra);
+    const int64_t un = base + (rank < extra ? 1 : 0);
+    const int64_t r0 = std::min(M, u0 * align), r1 = std::min(M, (u0 + un) * align);
+    *row0 = r0;
+    *rows = r1 - r0;
+    return HCLOOC_OK;
+}
