@@ -11,11 +11,12 @@ namespace dev {
 
 constexpr int BM = 128;
 constexpr int BN = 128;
-constexpr int BK = 16;
-constexpr int STAGES = 6;
-constexpr int A_STAGE_BYTES = BM * BK * 8;          // 16 KiB: 128 rows x 128 B
-constexpr int B_BOX_BYTES = BK * 16 * 8;            // 2 KiB: 16 k-rows x 128 B (16 columns)
-constexpr int B_STAGE_BYTES = (BN / 16) * B_BOX_BYTES;  // 16 KiB
+constexpr int BK = 32;                              // k depth of a stage: two 128-byte k halves of A, 32 k-rows of B
+constexpr int STAGES = 3;
+constexpr int A_HALF_BYTES = BM * 16 * 8;           // 16 KiB: one TMA box of A, 128 rows x 128 B (16 k)
+constexpr int A_STAGE_BYTES = (BK / 16) * A_HALF_BYTES;
+constexpr int B_BOX_BYTES = BK * 16 * 8;            // 4 KiB: one TMA box of B, 32 k-rows x 128 B (16 columns)
+constexpr int B_STAGE_BYTES = (BN / 16) * B_BOX_BYTES;
 constexpr int STAGE_BYTES = A_STAGE_BYTES + B_STAGE_BYTES;
 constexpr int NUM_CONSUMER_WARPS = 8;
 // Two consumer warpgroups + one producer warpgroup of which only warp 0 works.  The register file is split per
@@ -118,13 +119,14 @@ struct FragLanes {
     }
 };
 
-// One k block (16 deep) of the 32 x 64 warp tile: 12 LDS.128 feed 64 DMMA.8x8x4.
+// One k block (BK deep) of the 32 x 64 warp tile: per group of 8 k, 12 LDS.128 feed 64 DMMA.8x8x4.
 __device__ __forceinline__ void mma_kblock(double (&acc)[4][4][2][2], uint32_t sbase, const FragLanes& f) {
     #pragma unroll
-    for (int kg = 0; kg < 2; ++kg) {
+    for (int kg = 0; kg < BK / 8; ++kg) {
         double a[4][2];
+        const uint32_t abase = sbase + (kg >> 1) * A_HALF_BYTES + (f.a_lane ^ ((kg & 1) << 6));
         #pragma unroll
-        for (int u = 0; u < 4; ++u) lds128(a[u][0], a[u][1], sbase + ((f.a_lane ^ (kg << 6)) + u * 1024));
+        for (int u = 0; u < 4; ++u) lds128(a[u][0], a[u][1], abase + u * 1024);
         #pragma unroll
         for (int e = 0; e < 2; ++e) {
             double b[4][2];

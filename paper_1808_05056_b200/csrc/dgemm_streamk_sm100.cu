@@ -12,7 +12,7 @@
 //     Every sharer stores its partial accumulators to a scratch slot and bumps the tile's counter; the CTA
 //     that arrives LAST adds the partials up in k order (so the result does not depend on who is last) and
 //     runs the epilogue.  Nobody ever waits for another CTA, so no co-residency is needed.
-//   * the TMA producer warp runs through the same work list and keeps the 6-stage ring full across tile
+//   * the TMA producer warp runs through the same work list and keeps the 3-stage ring full across tile
 //     boundaries: the loads of the next tile overlap the epilogue of this one.
 // Inner loop, fragment layout and epilogue are those of dgemm_sm100.cu (dgemm_device.cuh).
 #include <cuda.h>
@@ -32,7 +32,7 @@ constexpr int SK_SLOT_BYTES = BM * BN * 8;                 // one partial tile: 
 constexpr int SK_MAX_CTAS = 148;
 constexpr int SK_MAX_TAIL_TILES = 2 * SK_MAX_CTAS;
 constexpr size_t SK_SCRATCH_BYTES = (size_t)2 * SK_MAX_CTAS * SK_SLOT_BYTES + SK_MAX_TAIL_TILES * sizeof(unsigned);
-constexpr int SK_MIN_KBLOCKS = 16;                         // do not cut pieces shorter than 16 k blocks (256 deep)
+constexpr int SK_MIN_KBLOCKS = 256 / BK;                   // do not cut pieces shorter than 256 deep
 
 struct SkParams {
     int tiles_m, tiles_n, nk;        // tile grid and k blocks per tile
@@ -121,7 +121,8 @@ hclooc_dgemm_streamk_kernel(const __grid_constant__ CUtensorMap tmA, const __gri
                     const uint32_t sa = smem_base + stage * STAGE_BYTES;
                     const uint32_t sb = sa + A_STAGE_BYTES;
                     const int k0 = kb * BK;
-                    tma_load_2d(sa, &tmA, k0, m0, full);
+                    #pragma unroll
+                for (int hk = 0; hk < BK / 16; ++hk) tma_load_2d(sa + hk * A_HALF_BYTES, &tmA, k0 + 16 * hk, m0, full);
                     #pragma unroll
                     for (int b = 0; b < BN / 16; ++b) tma_load_2d(sb + b * B_BOX_BYTES, &tmB, n0 + 16 * b, k0, full);
                     if (++stage == STAGES) { stage = 0; phase ^= 1u; }

@@ -442,3 +442,35 @@ def test_fig2_pipeline_matches_oracle(H, M, N, K, alpha, beta, budget, dist):
     assert st.plan.workspace_bytes <= budget
     if (M, N, K) == (4, 4, 8):
         assert (h, w) == (4, 2)                           # Figure 3 (:281)
+
+
+def test_repeated_identical_call_replays_a_cuda_graph(H):
+    """A short, latency-bound schedule (configs[0]) is captured as a CUDA graph when the very same call comes a
+    second time and replayed from the third on; every repetition must equal the oracle bit for bit and report
+    the same traffic, and a different call in between must not reuse the graph."""
+    M = N = K = 512
+    A, B, C = host_inputs(H, M, N, K, 81, "int")
+    C0 = C.view.copy()
+    ref = C0.copy()
+    oracle.dgemm(1.0, A.view, B.view, 0.5, ref)
+    ctx = H.hclooc_ctx_create(0)
+    try:
+        stats = []
+        for rep in range(4):                              # ordinary, capture + launch, replay, replay
+            C.view[...] = C0
+            stats.append(H.hclooc_dgemm_ex(ctx, M, N, K, 1.0, A, A.ld, B, B.ld, 0.5, C, C.ld, 1 * MiB))
+            check(C.view, ref, None, exact=True)
+        assert len({(s.bytes_h2d, s.bytes_d2h, s.n_kernels, s.n_copies_h2d, s.n_copies_d2h) for s in stats}) == 1
+        # another alpha: not the captured call
+        ref2 = C0.copy()
+        oracle.dgemm(-2.0, A.view, B.view, 0.5, ref2)
+        C.view[...] = C0
+        H.hclooc_dgemm_ex(ctx, M, N, K, -2.0, A, A.ld, B, B.ld, 0.5, C, C.ld, 1 * MiB)
+        check(C.view, ref2, None, exact=True)
+        # and back: seen before, but the graph belongs to the call before the last one -> captured afresh
+        for rep in range(3):
+            C.view[...] = C0
+            H.hclooc_dgemm_ex(ctx, M, N, K, 1.0, A, A.ld, B, B.ld, 0.5, C, C.ld, 1 * MiB)
+            check(C.view, ref, None, exact=True)
+    finally:
+        H.hclooc_ctx_destroy(ctx)
