@@ -193,8 +193,20 @@ def run_ours(args, wl, name):
             dist.barrier()
         torch.cuda.synchronize()
 
+    def ci95_rel(xs):
+        """Half-width of the 95 % confidence interval of the mean over the mean (Student t; PAPER.md:362 asks
+        for 2.5 %)."""
+        n = len(xs)
+        if n < 2:
+            return None
+        t95 = {2: 12.71, 3: 4.303, 4: 3.182, 5: 2.776, 6: 2.571, 7: 2.447, 8: 2.365, 9: 2.306, 10: 2.262}.get(n, 2.0 if n > 30 else 2.2)
+        return float(t95 * np.std(xs, ddof=1) / np.sqrt(n) / np.mean(xs))
+
+    per_call = []
+
     def timed(fn, steps, warmup):
         st = None
+        per_call.clear()
         for _ in range(warmup):
             st = fn()
         barrier()
@@ -202,6 +214,7 @@ def run_ours(args, wl, name):
         e0.record()
         for _ in range(steps):
             st = fn()
+            per_call.append(st.t_total_s)
         e1.record()
         barrier()
         ms = e0.elapsed_time(e1)
@@ -209,7 +222,7 @@ def run_ours(args, wl, name):
             t = torch.tensor([ms], device="cuda", dtype=torch.float64)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             ms = float(t.item())
-        return ms / steps, st
+        return ms / steps, (st, ci95_rel(list(per_call)))
 
     def resident():
         return H.hclooc_dgemm_ex(ctx, M, N, K, alpha, dA, K, dB, N, beta, dC, N, budget)
@@ -221,8 +234,8 @@ def run_ours(args, wl, name):
         if args.kernel_only:
             plan = H.hclooc_plan(M, N, K, beta != 0.0, 0, budget)
         else:
-            ms_res, st_res = timed(resident, args.steps, max(args.warmup, 3))
-            ms_e2e, st_e2e = timed(host, args.steps, max(args.warmup, 3))
+            ms_res, (st_res, ci_res) = timed(resident, args.steps, max(args.warmup, 3))
+            ms_e2e, (st_e2e, ci_e2e) = timed(host, args.steps, max(args.warmup, 3))
             plan = st_e2e.plan
         # ---- roofline leg: the tile kernel alone, one GPU-filling launch of the plan's B-slice shape
         nb = min(plan.nb, N)
@@ -267,7 +280,7 @@ def run_ours(args, wl, name):
         "metric": "end-to-end out-of-core DGEMM TFLOP/s (host-resident A,B,C) and % of roofline",
         "value": world * flops / (ms_res * 1e-3) / 1e12, "unit": "TFLOP/s", "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_res, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic", "ci95_rel": ci_res,
         "config": {"workload": f"{name}: {wl['desc']}", "M": M, "N": N, "K": K, "alpha": alpha, "beta": beta,
                    "device_budget_bytes": budget, "dist": wl["dist"], "parallelism": (f"{world} row bands of C of {M} rows each, one per GPU (hclooc_shard_rows), B on every rank, no collective"
                                    if world > 1 else "1 GPU"), "M_global": world * M,
@@ -277,7 +290,7 @@ def run_ours(args, wl, name):
         "e2e": {"value": world * flops / (ms_e2e * 1e-3) / 1e12, "unit": "TFLOP/s", "ms_per_step": ms_e2e,
                 "h2d_bytes_per_step": int(st_e2e.bytes_h2d), "d2h_bytes_per_step": int(st_e2e.bytes_d2h),
                 "roofline_s": t_roof, "t_flop_s": t_flop, "t_link_s": t_link, "bound": "link" if t_link > t_flop else "fp64",
-                "frac_of_roofline": t_roof / (ms_e2e * 1e-3), "link_peaks": LINK},
+                "frac_of_roofline": t_roof / (ms_e2e * 1e-3), "link_peaks": LINK, "ci95_rel": ci_e2e},
         "gpu_launches": int((st_res.n_kernels + st_e2e.n_kernels) * args.steps + len(kt) + len(stt)),
         "clocks": clocks,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",

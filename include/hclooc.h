@@ -75,7 +75,8 @@ typedef struct hclooc_plan_t {
     double   flops;               /* 2*M*N*K (:368)                                                 */
     double   t_flop_s, t_link_s, t_model_s;  /* cost model terms used to pick this plan             */
     int32_t  n_scratch;           /* stream-K scratch buffers (ksplit == -1): one per compute stream used       */
-    int32_t  reserved1;
+    int32_t  c_on_device;         /* C lives in device memory: its block copies are device-to-device and are not
+                                     counted in bytes_h2d / bytes_d2h (host-link bytes)                         */
     uint64_t bytes_scratch;       /* one of them (partial-tile slots + counters)                                */
 } hclooc_plan_t;
 
@@ -86,8 +87,9 @@ int hclooc_plan(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zer
 /* Same, saying where A, B and C live: 0 = pinned host memory (what hclooc_plan assumes), 1 = all three in
  * device memory: the in-core case (:130, :368) -- nothing is staged, the plan is one step over the caller's
  * matrices (h = w = 1, no buffers, no traffic).  hclooc_dgemm_ex picks this from the pointers it is given
- * (device operands that are not 16-byte aligned with even leading dimensions are staged like host ones).
- * -8: NULL out. */
+ * (device operands that are not 16-byte aligned with even leading dimensions are staged like host ones);
+ * 2 = A and B in pinned host memory, C in device memory (the nsteps mode below): C blocks move device to
+ * device, so they cost no host-link time and are not counted in bytes_h2d / bytes_d2h.  -8: NULL out. */
 int hclooc_plan_ex(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zero,
                    size_t device_budget_bytes, int operands_on_device, hclooc_plan_t* out);
 
@@ -183,6 +185,20 @@ int hclooc_dgemm(int64_t M, int64_t N, int64_t K, double alpha, const double* A,
 int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
                     int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
                     size_t device_budget_bytes, hclooc_stats* stats_out);
+
+/* nsteps mode (:277-283): MMOOC as a subroutine of a blocked algorithm (SUMMA, HSUMMA) that updates the same C
+ * `nsteps` times: C = alpha*A_p*B_p + beta_p*C for p = *step = 0 .. nsteps-1, one call per p.  C is uploaded once
+ * at step 0 (if beta != 0), stays in device memory between the calls, and is downloaded once at the last step, so
+ * every call moves only its A and B over the host link (the paper's listing of this logic is garbled, :245,
+ * :259-263; this is its stated intent).  C (M x N, must fit the budget beside a working set) counts against
+ * device_budget_bytes; host C is untouched until the last step.  *step is incremented on success (the caller
+ * starts a sequence with *step = 0); a failed call ends the sequence and releases the device copy.
+ * Errors as hclooc_dgemm, plus -13 nsteps < 1, -14 step NULL or outside [0, nsteps), -10 also when C, M, N or ldc
+ * differ from the running sequence; HCLOOC_ERR_BUDGET when C does not fit.  stats as hclooc_dgemm_ex; the one
+ * upload / download of C is added to the byte counts of the first / last call.                          */
+int hclooc_dgemm_nsteps(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
+                        int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
+                        size_t device_budget_bytes, int nsteps, int* step, hclooc_stats* stats);
 
 /* Multi-GPU (SURVEY 8(e); the paper's future work, :414): the row blocks of C are independent (:289, :293), so
  * G processes, one per GPU, each take a contiguous band of the rows of A and C and all of B, and call

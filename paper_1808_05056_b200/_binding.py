@@ -14,7 +14,7 @@ HCL_H2D, HCL_D2H = 0, 1
 EXPORTS = [
     "hclooc_plan", "hclooc_plan_ex", "hclooc_shard_rows", "hclMatrixPartitioner", "hclooc_schedule", "hclooc_ctx_create", "hclooc_ctx_destroy",
     "hclooc_ctx_set_trace", "hclooc_ctx_get_trace",
-    "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_fig2", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
+    "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_fig2", "hclooc_dgemm_nsteps", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
     "hclStreamDestroy", "hclEventDestroy", "hclMemcpy", "hclMemcpyAsync", "hclMemcpy2DAsync",
     "hclDgemmAsync", "hclDgemmAsyncEx", "hclWaitEvent", "hclStreamSynchronize", "hclDeviceSynchronize",
     "hclooc_host_alloc", "hclooc_host_free", "hclooc_host_register", "hclooc_host_unregister",
@@ -33,7 +33,7 @@ class Plan(ctypes.Structure):
                 ("workspace_bytes", c_uint64), ("bytes_h2d", c_uint64), ("bytes_d2h", c_uint64),
                 ("n_copies_h2d", c_uint64), ("n_copies_d2h", c_uint64),
                 ("flops", c_double), ("t_flop_s", c_double), ("t_link_s", c_double), ("t_model_s", c_double),
-                ("n_scratch", c_int32), ("reserved1", c_int32), ("bytes_scratch", c_uint64)]
+                ("n_scratch", c_int32), ("c_on_device", c_int32), ("bytes_scratch", c_uint64)]
 
     def asdict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -82,6 +82,7 @@ def lib():
         L.hclooc_ctx_get_trace.argtypes = [vp, vp, sz, POINTER(sz)]
         L.hclooc_dgemm.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz]
         L.hclooc_dgemm_ex.argtypes = [vp, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
+        L.hclooc_dgemm_nsteps.argtypes = [vp, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, c_int, POINTER(c_int), POINTER(Stats)]
         L.hclooc_dgemm_fig2.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
         L.hclMalloc.argtypes = [POINTER(vp), sz]
         L.hclFree.argtypes = [vp]
@@ -192,7 +193,7 @@ def hclooc_plan(M, N, K, beta_nonzero, alpha_zero, device_budget_bytes) -> Plan:
 def hclooc_plan_ex(M, N, K, beta_nonzero, alpha_zero, device_budget_bytes, operands_on_device) -> Plan:
     p = Plan()
     _check(lib().hclooc_plan_ex(M, N, K, int(bool(beta_nonzero)), int(bool(alpha_zero)), device_budget_bytes,
-                                int(bool(operands_on_device)), byref(p)), "hclooc_plan_ex")
+                                int(operands_on_device), byref(p)), "hclooc_plan_ex")
     return p
 
 
@@ -259,6 +260,14 @@ def hclooc_dgemm_ex(ctx, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_bu
     _check(lib().hclooc_dgemm_ex(ctx, M, N, K, alpha, _ptr(A), lda, _ptr(B), ldb, beta, _ptr(C), ldc,
                                  device_budget_bytes, byref(st) if want_stats else None), "hclooc_dgemm_ex")
     return st if want_stats else None
+
+
+def hclooc_dgemm_nsteps(ctx, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes, nsteps, step):
+    """One call of an nsteps sequence; returns (next step, Stats)."""
+    st, sp = Stats(), c_int(step)
+    _check(lib().hclooc_dgemm_nsteps(ctx, M, N, K, alpha, _ptr(A), lda, _ptr(B), ldb, beta, _ptr(C), ldc,
+                                     device_budget_bytes, nsteps, byref(sp), byref(st)), "hclooc_dgemm_nsteps")
+    return sp.value, st
 
 
 def hclooc_dgemm_fig2(M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes, want_stats=True):

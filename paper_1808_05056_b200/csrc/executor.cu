@@ -232,6 +232,11 @@ struct hclooc_ctx {
     bool graph_valid = false;                     // graph_exec is the schedule of graph_key
     std::vector<int64_t> graph_key;               // the previous call
     std::vector<cudaEvent_t> join_events;
+    // nsteps mode (hclooc_dgemm_nsteps): C kept in device memory between the calls of one sequence
+    double* res_c = nullptr;
+    int64_t res_ld = 0, res_M = 0, res_N = 0, res_ldc = 0;
+    const double* res_host = nullptr;
+    size_t res_bytes = 0;
     std::mutex mu;
 };
 
@@ -290,6 +295,7 @@ extern "C" int hclooc_ctx_destroy(hclooc_ctx* c) {
     if (c->owns_d2h && c->s_d2h) cudaStreamDestroy(c->s_d2h);
     if (c->owns_compute) for (int i = 0; i < c->n_compute; ++i) if (c->s_compute[i]) cudaStreamDestroy(c->s_compute[i]);
     if (c->owns_workspace && c->workspace) cudaFree(c->workspace);
+    if (c->res_c) cudaFree(c->res_c);
     delete c;
     return HCLOOC_OK;
 }
@@ -362,9 +368,10 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
     if (!ctx && (rc = default_ctx(&ctx))) return rc;
     std::lock_guard<std::mutex> lk(ctx->mu);
     HCL_CUDA(cudaSetDevice(ctx->device));
-    bool on_device = true;
-    if ((rc = check_resident(C, &on_device))) return rc;
-    if (!scale_only && ((rc = check_resident(A, &on_device)) || (rc = check_resident(B, &on_device)))) return rc;
+    bool on_device = true, c_dev = true, ab_dev = true;
+    if ((rc = check_resident(C, &c_dev))) return rc;
+    if (!scale_only && ((rc = check_resident(A, &ab_dev)) || (rc = check_resident(B, &ab_dev)))) return rc;
+    on_device = c_dev && ab_dev;
 
     // ---------------------------------------------------------------- S1 plan
     size_t budget = device_budget_bytes;
@@ -382,7 +389,7 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
     const bool aligned = (((uintptr_t)C & 15u) == 0) && (ldc % 2 == 0) &&
                          (scale_only || ((((uintptr_t)A | (uintptr_t)B) & 15u) == 0 && lda % 2 == 0 && ldb % 2 == 0));
     const bool in_core = on_device && aligned && M <= 0x7fffffffLL && N <= 0x7fffffffLL && K <= 0x7fffffffLL;
-    rc = hclooc_plan_ex(M, N, K, beta != 0.0, alpha == 0.0, budget, in_core ? 1 : 0, &P);
+    rc = hclooc_plan_ex(M, N, K, beta != 0.0, alpha == 0.0, budget, in_core ? 1 : (c_dev ? 2 : 0), &P);
     if (rc) return rc;
     if (in_core) {
         const auto t0 = std::chrono::steady_clock::now();
@@ -518,11 +525,13 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
                 break;
             case HCLOOC_OP_H2D_C:
                 rc = copy2d(bufs[o.buf], (size_t)P.ldc_dev * 8, C + o.r0 * ldc + o.c0, (size_t)ldc * 8, (size_t)o.nc * 8, (size_t)o.nr, st);
-                bytes_h2d += (uint64_t)o.nr * o.nc * 8; ++n_h2d;
+                if (!c_dev) bytes_h2d += (uint64_t)o.nr * o.nc * 8;   // device-resident C: not link traffic
+                ++n_h2d;
                 break;
             case HCLOOC_OP_D2H_C:
                 rc = copy2d(C + o.r0 * ldc + o.c0, (size_t)ldc * 8, bufs[o.buf], (size_t)P.ldc_dev * 8, (size_t)o.nc * 8, (size_t)o.nr, st);
-                bytes_d2h += (uint64_t)o.nr * o.nc * 8; ++n_d2h;
+                if (!c_dev) bytes_d2h += (uint64_t)o.nr * o.nc * 8;
+                ++n_d2h;
                 break;
             case HCLOOC_OP_GEMM: {
                 const double b_eff = (o.beta < 0.0) ? beta : o.beta;
@@ -604,6 +613,85 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
 extern "C" int hclooc_dgemm(int64_t M, int64_t N, int64_t K, double alpha, const double* A, int64_t lda,
                             const double* B, int64_t ldb, double beta, double* C, int64_t ldc, size_t device_budget_bytes) {
     return hclooc_dgemm_ex(nullptr, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes, nullptr);
+}
+
+// ---------------------------------------------------------------------------------------------
+// nsteps mode: MMOOC as a subroutine of a blocked algorithm (SUMMA, HSUMMA) that updates the
+// same C `nsteps` times.  The paper uploads C only at step 0 and downloads it only at the last step; its listing
+// of that logic is garbled (:245, :259-263, G17), so the stated intent is implemented: C lives in device
+// memory between the calls of one sequence, and every call streams only its A and B.
+extern "C" int hclooc_dgemm_nsteps(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
+                                   int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
+                                   size_t device_budget_bytes, int nsteps, int* step, hclooc_stats* stats) {
+    const auto t_begin = std::chrono::steady_clock::now();
+    if (M <= 0) return -1;
+    if (N <= 0) return -2;
+    if (K < 0) return -3;
+    if (!C) return -10;
+    if (ldc < N) return -11;
+    if (nsteps < 1) return -13;
+    if (!step || *step < 0 || *step >= nsteps) return -14;
+    int rc;
+    if (!ctx && (rc = default_ctx(&ctx))) return rc;
+    const bool first = (*step == 0), last = (*step == nsteps - 1);
+    size_t budget = device_budget_bytes;
+    uint64_t up = 0, down = 0;
+    {
+        std::lock_guard<std::mutex> lk(ctx->mu);
+        HCL_CUDA(cudaSetDevice(ctx->device));
+        if (budget == 0) {
+            if (ctx->workspace && !ctx->owns_workspace) budget = ctx->workspace_bytes + ctx->res_bytes;
+            else {
+                size_t fr = 0, tot = 0;
+                HCL_CUDA(cudaMemGetInfo(&fr, &tot));
+                fr += ctx->workspace_bytes + ctx->res_bytes;
+                budget = fr > ((size_t)2 << 30) ? fr - ((size_t)1 << 30) : fr / 2;
+            }
+        }
+        if (first) {
+            if (ctx->res_c) { cudaFree(ctx->res_c); ctx->res_c = nullptr; ctx->res_bytes = 0; }   // an abandoned sequence
+            bool dummy = true;
+            if ((rc = check_resident(C, &dummy))) return rc;
+            const int64_t ld = (N + 15) / 16 * 16;
+            const size_t bytes = (size_t)M * ld * 8;
+            if (bytes >= budget) return HCLOOC_ERR_BUDGET;          // C itself does not fit: this mode does not apply
+            void* p = nullptr;
+            cudaError_t e = cudaMalloc(&p, bytes);
+            if (e != cudaSuccess) { set_last_cuda_error((int)e); cudaGetLastError(); return HCLOOC_ERR_NOMEM; }
+            ctx->res_c = (double*)p; ctx->res_ld = ld; ctx->res_M = M; ctx->res_N = N; ctx->res_host = C; ctx->res_ldc = ldc;
+            ctx->res_bytes = bytes;
+            if (beta != 0.0) {                                      // S(C) once, at step 0 (:277)
+                rc = copy2d(ctx->res_c, (size_t)ld * 8, C, (size_t)ldc * 8, (size_t)N * 8, (size_t)M, ctx->s_h2d);
+                cudaError_t es = cudaStreamSynchronize(ctx->s_h2d);
+                if (!rc && es != cudaSuccess) rc = cuda_fail(es);
+                if (rc) { cudaFree(ctx->res_c); ctx->res_c = nullptr; ctx->res_bytes = 0; return rc; }
+                up = (uint64_t)M * N * 8;
+            }
+        } else if (!ctx->res_c || ctx->res_M != M || ctx->res_N != N || ctx->res_host != C || ctx->res_ldc != ldc) {
+            return -10;                                             // not the C of the running sequence
+        }
+        if (ctx->res_bytes >= budget) return HCLOOC_ERR_BUDGET;
+        budget -= ctx->res_bytes;
+    }
+    rc = hclooc_dgemm_ex(ctx, M, N, K, alpha, A, lda, B, ldb, beta, ctx->res_c, ctx->res_ld, budget, stats);
+    {
+        std::lock_guard<std::mutex> lk(ctx->mu);
+        if (!rc && last) {                                          // R(C) once, at the last step
+            rc = copy2d(C, (size_t)ldc * 8, ctx->res_c, (size_t)ctx->res_ld * 8, (size_t)N * 8, (size_t)M, ctx->s_d2h);
+            cudaError_t es = cudaStreamSynchronize(ctx->s_d2h);
+            if (!rc && es != cudaSuccess) rc = cuda_fail(es);
+            down = (uint64_t)M * N * 8;
+        }
+        if (rc || last) { cudaFree(ctx->res_c); ctx->res_c = nullptr; ctx->res_bytes = 0; }
+    }
+    if (rc) return rc;
+    ++*step;
+    if (stats) {
+        stats->bytes_h2d += up; stats->bytes_d2h += down;
+        stats->n_copies_h2d += up ? 1 : 0; stats->n_copies_d2h += down ? 1 : 0;
+        stats->t_total_s = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_begin).count();
+    }
+    return HCLOOC_OK;
 }
 
 extern "C" int hclooc_ctx_set_trace(hclooc_ctx* ctx, int enable) {

@@ -54,6 +54,7 @@ namespace {
 struct Cand {
     int64_t mb, nb, kb, h, w, kpanels;
     int n_sets, n_abuf, n_bbuf, ksplit, n_scratch;
+    bool c_dev;           // C lives in device memory: its block copies are device-to-device, not host-link traffic
     int64_t lda_dev, ldb_dev, ldc_dev;
     uint64_t a_bytes, b_bytes, c_bytes, ws_bytes;
     uint64_t bytes_h2d, bytes_d2h, n_h2d, n_d2h;
@@ -102,11 +103,12 @@ void fill_traffic(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool s
             }
         }
     }
-    if (beta_nz) { el_h2d += MN; n_h2d += (uint64_t)c.h * c.w; }
-    if (c.kpanels > 1) { el_h2d += (uint64_t)(c.kpanels - 1) * MN; n_h2d += (uint64_t)(c.kpanels - 1) * c.h * c.w; }
+    const uint64_t MNlink = c.c_dev ? 0 : MN;                                   // copies are still enqueued, bytes are not link bytes
+    if (beta_nz) { el_h2d += MNlink; n_h2d += (uint64_t)c.h * c.w; }
+    if (c.kpanels > 1) { el_h2d += (uint64_t)(c.kpanels - 1) * MNlink; n_h2d += (uint64_t)(c.kpanels - 1) * c.h * c.w; }
     c.bytes_h2d = 8 * el_h2d;
     c.n_h2d = n_h2d;
-    c.bytes_d2h = 8 * (uint64_t)c.kpanels * MN;
+    c.bytes_d2h = 8 * (uint64_t)c.kpanels * MNlink;
     c.n_d2h = steps;
 }
 
@@ -158,10 +160,11 @@ void cost(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool scale_onl
     const double n_cols = (double)c.w * c.kpanels;
     const double comp_col = t_compute / n_cols;
     const double a_first = scale_only ? 0.0 : 8.0 * (double)M * (double)c.kb;
-    const double a_all = (double)c.bytes_h2d - 8.0 * (double)K * (double)N - (beta_nz ? 8.0 * (double)M * (double)N : 0.0) -
-                         (c.kpanels > 1 ? 8.0 * (double)(c.kpanels - 1) * (double)M * (double)N : 0.0);
+    const double mn_link = c.c_dev ? 0.0 : 8.0 * (double)M * (double)N;
+    const double a_all = (double)c.bytes_h2d - 8.0 * (double)K * (double)N - (beta_nz ? mn_link : 0.0) -
+                         (c.kpanels > 1 ? (double)(c.kpanels - 1) * mn_link : 0.0);
     const double a_later = n_cols > c.kpanels ? std::max(0.0, a_all - a_first * c.kpanels) / (n_cols - c.kpanels) : 0.0;
-    const double c_col = 8.0 * (double)M * (double)c.nb;
+    const double c_col = c.c_dev ? 0.0 : 8.0 * (double)M * (double)c.nb;
     auto link_col = [&](double a_bytes) {
         const double up = a_bytes + (scale_only ? 0.0 : (double)c.b_bytes) + (cload ? c_col : 0.0);
         const double lat = (double)c.h * 2.0 * mm.copy_latency_s;
@@ -174,10 +177,11 @@ void cost(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool scale_onl
         // less the uploads issued ahead of the reload, and (b) after the reload once every C buffer is held by
         // a step whose kernel has only just started
         const double t_up = ((double)c.bytes_h2d - 8.0 * (double)K * (double)N) / std::max(1.0, steps) / mm.h2d_Bps + mm.copy_latency_s;
-        const double t_cup = cload ? (double)c.c_bytes / mm.h2d_Bps + mm.copy_latency_s : t_up;
+        const double c_rate_up = c.c_dev ? 1.0e12 : mm.h2d_Bps, c_rate_down = c.c_dev ? 1.0e12 : mm.d2h_Bps;
+        const double t_cup = cload ? (double)c.c_bytes / c_rate_up + mm.copy_latency_s : t_up;
         const double pre = (double)early_uploads(c.h, c.n_sets, c.n_abuf);
         const double drain = std::max(0.0, t_kernel - pre * t_cup);
-        const double refill = std::max(0.0, t_kernel + (double)c.c_bytes / mm.d2h_Bps - std::max(0.0, c.n_sets - pre - 1.0) * t_up);
+        const double refill = std::max(0.0, t_kernel + (double)c.c_bytes / c_rate_down - std::max(0.0, c.n_sets - pre - 1.0) * t_up);
         stall_link = drain + refill;
     }
     const double l_first = link_col(a_first), l_later = link_col(a_later);
@@ -206,6 +210,8 @@ extern "C" int hclooc_plan(int64_t M, int64_t N, int64_t K, int beta_nonzero, in
 extern "C" int hclooc_plan_ex(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zero,
                               size_t device_budget_bytes, int operands_on_device, hclooc_plan_t* out) {
     const MachineModel& mm = machine_model();
+    const bool c_dev = operands_on_device == 2;
+    if (operands_on_device == 2) operands_on_device = 0;
     if (M < 0) return -1;
     if (N < 0) return -2;
     if (K < 0) return -3;
@@ -276,6 +282,7 @@ extern "C" int hclooc_plan_ex(int64_t M, int64_t N, int64_t K, int beta_nonzero,
                     if (force_mb) { nt = 0; if (force_mb <= std::min(M, rows_max)) tried[nt++] = force_mb; }
                     for (int q = 0; q < nt; ++q) {
                         Cand c{};
+                        c.c_dev = c_dev;
                         c.mb = tried[q]; c.nb = nb; c.kb = kb; c.kpanels = kp;
                         c.h = ceil_div(M, c.mb); c.w = weff;
                         c.n_sets = (int)std::min<int64_t>(n_sets, std::max<int64_t>(2, c.h * c.w * kp));
@@ -315,6 +322,7 @@ extern "C" int hclooc_plan_ex(int64_t M, int64_t N, int64_t K, int beta_nonzero,
     out->lda_dev = best.lda_dev; out->ldb_dev = best.ldb_dev; out->ldc_dev = best.ldc_dev;
     out->bytes_a_buf = best.a_bytes; out->bytes_b_buf = best.b_bytes; out->bytes_c_buf = best.c_bytes;
     out->workspace_bytes = best.ws_bytes;
+    out->c_on_device = c_dev ? 1 : 0;
     out->n_scratch = best.n_scratch; out->bytes_scratch = best.n_scratch ? streamk_scratch_bytes() : 0;
     out->bytes_h2d = best.bytes_h2d; out->bytes_d2h = best.bytes_d2h;
     out->n_copies_h2d = best.n_h2d; out->n_copies_d2h = best.n_d2h;

@@ -474,3 +474,44 @@ def test_repeated_identical_call_replays_a_cuda_graph(H):
             check(C.view, ref, None, exact=True)
     finally:
         H.hclooc_ctx_destroy(ctx)
+
+
+@pytest.mark.parametrize("dist", ["int", "uniform"])
+def test_nsteps_mode_keeps_c_on_the_device(H, dist):
+    """hclooc_dgemm_nsteps: C is uploaded at step 0, stays in device memory while a blocked
+    algorithm adds one K panel per call, and comes back at the last step.  Same values as the oracle applied
+    panel by panel; no C traffic over the link in between; host C untouched until the end."""
+    M, N, Kp, nsteps = 520, 392, 160, 4
+    A = [H.HostMatrix(M, Kp) for _ in range(nsteps)]
+    B = [H.HostMatrix(Kp, N) for _ in range(nsteps)]
+    C = H.HostMatrix(M, N)
+    for p in range(nsteps):
+        synthgen.fill(A[p].array, 90 + p, "A", dist)
+        synthgen.fill(B[p].array, 90 + p, "B", dist)
+    synthgen.fill(C.array, 90, "C", dist)
+    C0 = C.view.copy()
+    ref = C0.copy()
+    D = np.zeros((M, N))
+    for p in range(nsteps):                               # the oracle, one panel after the other: beta first, then 1
+        Dp = oracle.dgemm(2.0, A[p].view, B[p].view, 0.5 if p == 0 else 1.0, ref, want_denominator=True)
+        D = Dp if p == 0 else D + Dp                      # a (generous) running denominator for the float gate
+    ctx = H.hclooc_ctx_create(0)
+    try:
+        step = 0
+        for p in range(nsteps):
+            step, st = H.hclooc_dgemm_nsteps(ctx, M, N, Kp, 2.0, A[p], Kp, B[p], N, 0.5 if p == 0 else 1.0, C, N,
+                                             4 * MiB, nsteps, step)
+            assert step == p + 1 and st.plan.c_on_device == 1
+            assert st.bytes_d2h == (M * N * 8 if p == nsteps - 1 else 0)
+            ab = st.bytes_h2d - (M * N * 8 if p == 0 else 0)
+            assert M * Kp * 8 + Kp * N * 8 <= ab <= st.plan.w * M * Kp * 8 + Kp * N * 8      # only A and B cross the link
+            if p < nsteps - 1:
+                assert np.array_equal(C.view, C0)         # host C is written only at the last step
+        check(C.view, ref, D, exact=(dist == "int"))
+        with pytest.raises(H.HclError):                   # a sequence must start at step 0 with its own C
+            H.hclooc_dgemm_nsteps(ctx, M, N, Kp, 1.0, A[0], Kp, B[0], N, 1.0, C, N, 4 * MiB, nsteps, 2)
+        with pytest.raises(H.HclError) as e:              # C larger than the budget: the mode does not apply
+            H.hclooc_dgemm_nsteps(ctx, M, N, Kp, 1.0, A[0], Kp, B[0], N, 1.0, C, N, 1 * MiB, nsteps, 0)
+        assert e.value.status == 1
+    finally:
+        H.hclooc_ctx_destroy(ctx)

@@ -156,6 +156,18 @@ def test_plans_for_random_shapes_and_budgets():
     assert H.hclooc_plan(64, 64, 100000, 1, 0, 600 * 1024).kpanels > 1     # K split only when forced
 
 
+def test_plan_with_c_on_the_device_counts_only_a_and_b_as_link_traffic():
+    M, N, K = 2000, 1500, 700
+    host = H.hclooc_plan_ex(M, N, K, 1, 0, 6 * MiB, 0)
+    cdev = H.hclooc_plan_ex(M, N, K, 1, 0, 6 * MiB, 2)
+    assert host.c_on_device == 0 and cdev.c_on_device == 1
+    assert cdev.bytes_d2h == 0 and host.bytes_d2h == 8 * M * N
+    assert cdev.bytes_h2d <= host.bytes_h2d - 8 * M * N + 8 * (host.w * M * K)      # A and B only
+    assert 8 * (M * K + K * N) <= cdev.bytes_h2d <= 8 * (cdev.w * M * K + K * N)
+    ops = H.hclooc_schedule(cdev, 4)
+    assert int((ops["kind"] == K_H2D_C).sum()) == cdev.h * cdev.w == int((ops["kind"] == K_D2H_C).sum())   # still staged
+
+
 def test_in_core_plan_for_device_resident_operands():
     p = H.hclooc_plan_ex(8192, 8192, 8192, 1, 0, 256 * MiB, 1)
     assert (p.h, p.w, p.kpanels, p.n_steps) == (1, 1, 1, 1) and (p.mb, p.nb, p.kb) == (8192, 8192, 8192)
