@@ -194,7 +194,7 @@ void cost(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool scale_onl
     c.t_model = t_pro + body + OVERLAP_PENALTY * std::min(comp_path, link_path) + t_tail + mm.launch_latency_s;
     // between near-equal plans take the one whose slices are whole tiles: padded tiles burn FP64 issue slots and
     // power for nothing even when the link hides their time
-    c.t_model *= 1.0 + 0.15 * (1.0 - pad_eff);
+    c.t_model *= 1.0 + 0.3 * (1.0 - (double)N / (tile_cols * (double)TILE));     // column padding only: rows pad with mb < 128 by design
 }
 
 }  // namespace
