@@ -222,7 +222,7 @@ def run_ours(args, wl, name):
             t = torch.tensor([ms], device="cuda", dtype=torch.float64)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             ms = float(t.item())
-        return ms / steps, (st, ci95_rel(list(per_call)))
+        return ms / steps, (st, ci95_rel(list(per_call)), 1e3 * float(np.mean(per_call)), 1e3 * float(np.min(per_call)))
 
     def resident():
         return H.hclooc_dgemm_ex(ctx, M, N, K, alpha, dA, K, dB, N, beta, dC, N, budget)
@@ -234,8 +234,8 @@ def run_ours(args, wl, name):
         if args.kernel_only:
             plan = H.hclooc_plan(M, N, K, beta != 0.0, 0, budget)
         else:
-            ms_res, (st_res, ci_res) = timed(resident, args.steps, max(args.warmup, 3))
-            ms_e2e, (st_e2e, ci_e2e) = timed(host, args.steps, max(args.warmup, 3))
+            ms_res, (st_res, ci_res, _, _) = timed(resident, args.steps, max(args.warmup, 3))
+            ms_e2e, (st_e2e, ci_e2e, call_mean_ms, call_min_ms) = timed(host, args.steps, max(args.warmup, 3))
             plan = st_e2e.plan
         # ---- roofline leg: the tile kernel alone, one GPU-filling launch of the plan's B-slice shape
         nb = min(plan.nb, N)
@@ -290,7 +290,8 @@ def run_ours(args, wl, name):
         "e2e": {"value": world * flops / (ms_e2e * 1e-3) / 1e12, "unit": "TFLOP/s", "ms_per_step": ms_e2e,
                 "h2d_bytes_per_step": int(st_e2e.bytes_h2d), "d2h_bytes_per_step": int(st_e2e.bytes_d2h),
                 "roofline_s": t_roof, "t_flop_s": t_flop, "t_link_s": t_link, "bound": "link" if t_link > t_flop else "fp64",
-                "frac_of_roofline": t_roof / (ms_e2e * 1e-3), "link_peaks": LINK, "ci95_rel": ci_e2e},
+                "frac_of_roofline": t_roof / (ms_e2e * 1e-3), "link_peaks": LINK, "ci95_rel": ci_e2e,
+                "call_ms_mean": call_mean_ms, "call_ms_min": call_min_ms},
         "gpu_launches": int((st_res.n_kernels + st_e2e.n_kernels) * args.steps + len(kt) + len(stt)),
         "clocks": clocks,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",

@@ -78,6 +78,13 @@ typedef struct hclooc_plan_t {
     int32_t  c_on_device;         /* C lives in device memory: its block copies are device-to-device and are not
                                      counted in bytes_h2d / bytes_d2h (host-link bytes)                         */
     uint64_t bytes_scratch;       /* one of them (partial-tile slots + counters)                                */
+    int32_t  direct;              /* 1 = DIRECT mode: no device buffer at all -- one launch of the tile kernel whose TMA
+                                     loads read the A and B tiles straight from the (mapped) pinned host matrices and whose
+                                     epilogue reads and writes C in host memory.  Every tile streams over the host link
+                                     (bytes_h2d counts each tile's own reads: A is read ceil(N/128) times, B ceil(M/128)
+                                     times), so it only wins where the staged pipeline is bound by per-copy latency:
+                                     small problems under small budgets (BASELINE config 1).  h = w = n_steps = 1.     */
+    int32_t  reserved1;
 } hclooc_plan_t;
 
 /* Plan only (pure host arithmetic, needs no GPU).  alpha_zero != 0 plans the scale-only pass.
@@ -89,7 +96,10 @@ int hclooc_plan(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zer
  * matrices (h = w = 1, no buffers, no traffic).  hclooc_dgemm_ex picks this from the pointers it is given
  * (device operands that are not 16-byte aligned with even leading dimensions are staged like host ones);
  * 2 = A and B in pinned host memory, C in device memory (the nsteps mode below): C blocks move device to
- * device, so they cost no host-link time and are not counted in bytes_h2d / bytes_d2h.  -8: NULL out. */
+ * device, so they cost no host-link time and are not counted in bytes_h2d / bytes_d2h;
+ * 3 = as 0, and the device can address the host matrices as they are (mapped pinned memory, 16-byte aligned, even
+ * leading dimensions): the cost model may then pick the DIRECT mode (plan.direct) when it beats every staged plan;
+ * 4 = as 3 but direct mode is forced (tests, experiments).  -8: NULL out. */
 int hclooc_plan_ex(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zero,
                    size_t device_budget_bytes, int operands_on_device, hclooc_plan_t* out);
 
@@ -160,6 +170,9 @@ typedef struct hclooc_trace_rec {
     double   t_start_ms, t_end_ms;
 } hclooc_trace_rec;
 int hclooc_ctx_set_trace(hclooc_ctx* ctx, int enable);
+/* Direct mode (plan.direct) policy of this context: -1 = let the cost model choose (default), 0 = never (every call
+ * is staged through device buffers), 1 = always when the operands allow it.  -2: mode outside {-1, 0, 1}.   */
+int hclooc_ctx_set_direct(hclooc_ctx* ctx, int mode);
 int hclooc_ctx_get_trace(hclooc_ctx* ctx, hclooc_trace_rec* recs, size_t max_recs, size_t* n_recs);
 
 /* ------------------------------------------------------------------ the operation

@@ -13,7 +13,7 @@ HCL_H2D, HCL_D2H = 0, 1
 # every symbol include/hclooc.h declares (tests check the .so exports all of them)
 EXPORTS = [
     "hclooc_plan", "hclooc_plan_ex", "hclooc_shard_rows", "hclMatrixPartitioner", "hclooc_schedule", "hclooc_ctx_create", "hclooc_ctx_destroy",
-    "hclooc_ctx_set_trace", "hclooc_ctx_get_trace",
+    "hclooc_ctx_set_trace", "hclooc_ctx_get_trace", "hclooc_ctx_set_direct",
     "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_fig2", "hclooc_dgemm_nsteps", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
     "hclStreamDestroy", "hclEventDestroy", "hclMemcpy", "hclMemcpyAsync", "hclMemcpy2DAsync",
     "hclDgemmAsync", "hclDgemmAsyncEx", "hclWaitEvent", "hclStreamSynchronize", "hclDeviceSynchronize",
@@ -33,7 +33,8 @@ class Plan(ctypes.Structure):
                 ("workspace_bytes", c_uint64), ("bytes_h2d", c_uint64), ("bytes_d2h", c_uint64),
                 ("n_copies_h2d", c_uint64), ("n_copies_d2h", c_uint64),
                 ("flops", c_double), ("t_flop_s", c_double), ("t_link_s", c_double), ("t_model_s", c_double),
-                ("n_scratch", c_int32), ("c_on_device", c_int32), ("bytes_scratch", c_uint64)]
+                ("n_scratch", c_int32), ("c_on_device", c_int32), ("bytes_scratch", c_uint64),
+                ("direct", c_int32), ("reserved1", c_int32)]
 
     def asdict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -80,6 +81,7 @@ def lib():
         L.hclooc_ctx_destroy.argtypes = [vp]
         L.hclooc_ctx_set_trace.argtypes = [vp, c_int]
         L.hclooc_ctx_get_trace.argtypes = [vp, vp, sz, POINTER(sz)]
+        L.hclooc_ctx_set_direct.argtypes = [vp, c_int]
         L.hclooc_dgemm.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz]
         L.hclooc_dgemm_ex.argtypes = [vp, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
         L.hclooc_dgemm_nsteps.argtypes = [vp, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, c_int, POINTER(c_int), POINTER(Stats)]
@@ -239,6 +241,10 @@ TRACE_DTYPE = np.dtype([("kind", "<i4"), ("stream", "<i4"), ("step", "<i8"), ("b
 
 def hclooc_ctx_set_trace(ctx, enable: bool) -> None:
     _check(lib().hclooc_ctx_set_trace(ctx, int(bool(enable))), "hclooc_ctx_set_trace")
+
+
+def hclooc_ctx_set_direct(ctx, mode: int) -> None:
+    _check(lib().hclooc_ctx_set_direct(ctx, int(mode)), "hclooc_ctx_set_direct")
 
 
 def hclooc_ctx_get_trace(ctx) -> np.ndarray:

@@ -224,6 +224,11 @@ struct hclooc_ctx {
     std::vector<cudaEvent_t> events;
     std::vector<hclooc_op_t> ops;
     bool trace = false;
+    int direct_mode = -1;                         // -1 cost model decides, 0 never, 1 whenever the operands allow it
+    // plans of recent calls: the search over candidates costs 0.2 ms (config 1) to 9 ms (config 4) of host time
+    // before the first copy can be issued, and a blocked algorithm repeats the same shapes over and over
+    struct PlanKey { int64_t M, N, K; int beta_nz, alpha_zero, where; size_t budget; };
+    std::vector<std::pair<PlanKey, hclooc_plan_t>> plan_cache;
     std::vector<cudaEvent_t> trace_events;        // 2 per traced op (+1 base), timing enabled
     std::vector<hclooc_trace_rec> trace_recs;     // filled after the final synchronisation
     // the schedule of the last call captured as a CUDA graph (short, latency-bound schedules; same call again
@@ -317,13 +322,15 @@ int default_ctx(hclooc_ctx** out) {
     return HCLOOC_OK;
 }
 
-// 0 = ok, HCLOOC_ERR_NOT_PINNED if pageable host memory; *on_device is cleared unless p is device memory
-int check_resident(const void* p, bool* on_device) {
+// 0 = ok, HCLOOC_ERR_NOT_PINNED if pageable host memory; *on_device is cleared unless p is device memory;
+// *dev_alias (nullable) = the address under which kernels on the device reach p (NULL if they cannot)
+int check_resident(const void* p, bool* on_device, const void** dev_alias = nullptr) {
     cudaPointerAttributes at;
     cudaError_t e = cudaPointerGetAttributes(&at, p);
     if (e != cudaSuccess) { cudaGetLastError(); return HCLOOC_ERR_NOT_PINNED; }
     if (at.type == cudaMemoryTypeUnregistered) return HCLOOC_ERR_NOT_PINNED;
     if (at.type != cudaMemoryTypeDevice) *on_device = false;
+    if (dev_alias) *dev_alias = at.devicePointer;
     return HCLOOC_OK;
 }
 
@@ -369,8 +376,9 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
     std::lock_guard<std::mutex> lk(ctx->mu);
     HCL_CUDA(cudaSetDevice(ctx->device));
     bool on_device = true, c_dev = true, ab_dev = true;
-    if ((rc = check_resident(C, &c_dev))) return rc;
-    if (!scale_only && ((rc = check_resident(A, &ab_dev)) || (rc = check_resident(B, &ab_dev)))) return rc;
+    const void *A_alias = nullptr, *B_alias = nullptr, *C_alias = nullptr;
+    if ((rc = check_resident(C, &c_dev, &C_alias))) return rc;
+    if (!scale_only && ((rc = check_resident(A, &ab_dev, &A_alias)) || (rc = check_resident(B, &ab_dev, &B_alias)))) return rc;
     on_device = c_dev && ab_dev;
 
     // ---------------------------------------------------------------- S1 plan
@@ -389,11 +397,34 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
     const bool aligned = (((uintptr_t)C & 15u) == 0) && (ldc % 2 == 0) &&
                          (scale_only || ((((uintptr_t)A | (uintptr_t)B) & 15u) == 0 && lda % 2 == 0 && ldb % 2 == 0));
     const bool in_core = on_device && aligned && M <= 0x7fffffffLL && N <= 0x7fffffffLL && K <= 0x7fffffffLL;
-    rc = hclooc_plan_ex(M, N, K, beta != 0.0, alpha == 0.0, budget, in_core ? 1 : (c_dev ? 2 : 0), &P);
-    if (rc) return rc;
-    if (in_core) {
+    // direct mode needs host matrices the kernel can address as they are: mapped, TMA-legal, host/device address
+    // arithmetic interchangeable (the alias of the first element is what the tensor maps are built on)
+    static const int direct_env = [] { const char* e = std::getenv("HCLOOC_DIRECT"); return e ? std::atoi(e) : -1; }();
+    const int direct_mode = ctx->direct_mode >= 0 ? ctx->direct_mode : direct_env;
+    const bool direct_ok = !in_core && !c_dev && aligned && direct_mode != 0 && M <= 0x7fffffffLL && N <= 0x7fffffffLL && K <= 0x7fffffffLL &&
+                           C_alias && (((uintptr_t)C_alias & 15u) == 0) &&
+                           (scale_only || (A_alias && B_alias && ((((uintptr_t)A_alias | (uintptr_t)B_alias) & 15u) == 0)));
+    {
+        const hclooc_ctx::PlanKey key{M, N, K, beta != 0.0, alpha == 0.0, in_core ? 1 : (c_dev ? 2 : (direct_ok ? (direct_mode == 1 ? 4 : 3) : 0)), budget};
+        bool hit = false;
+        for (const auto& kv : ctx->plan_cache) {
+            const hclooc_ctx::PlanKey& k = kv.first;
+            if (k.M == key.M && k.N == key.N && k.K == key.K && k.beta_nz == key.beta_nz && k.alpha_zero == key.alpha_zero &&
+                k.where == key.where && k.budget == key.budget) { P = kv.second; hit = true; break; }
+        }
+        if (!hit) {
+            rc = hclooc_plan_ex(M, N, K, key.beta_nz, key.alpha_zero, budget, key.where, &P);
+            if (rc) return rc;
+            if (ctx->plan_cache.size() >= 16) ctx->plan_cache.erase(ctx->plan_cache.begin());
+            ctx->plan_cache.emplace_back(key, P);
+        }
+    }
+    if (in_core || P.direct) {
         const auto t0 = std::chrono::steady_clock::now();
-        rc = launch_dgemm_tiles(M, N, scale_only ? 0 : K, scale_only ? 0.0 : alpha, A, lda, B, ldb, beta, C, ldc, ctx->s_compute[0], -1);
+        if (P.direct) { A = (const double*)A_alias; B = (const double*)B_alias; C = (double*)C_alias; }
+        // direct: one CTA per tile (every tile is bound by its own reads over the link; the persistent kernel's
+        // device scratch would also break the promise that the call uses no device memory)
+        rc = launch_dgemm_tiles(M, N, scale_only ? 0 : K, scale_only ? 0.0 : alpha, A, lda, B, ldb, beta, C, ldc, ctx->s_compute[0], P.direct ? 1 : -1);
         const auto t1 = std::chrono::steady_clock::now();
         cudaError_t e = cudaStreamSynchronize(ctx->s_compute[0]);
         if (rc) return rc;
@@ -402,6 +433,7 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
         if (stats) {
             stats->plan = P;
             stats->n_kernels = 1;
+            stats->bytes_h2d = P.bytes_h2d; stats->bytes_d2h = P.bytes_d2h;      // direct mode: the tiles' own reads and writes
             stats->t_enqueue_s = std::chrono::duration<double>(t1 - t0).count();
             stats->t_total_s = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_begin).count();
         }
@@ -699,6 +731,15 @@ extern "C" int hclooc_ctx_set_trace(hclooc_ctx* ctx, int enable) {
     if (!ctx && (rc = default_ctx(&ctx))) return rc;
     std::lock_guard<std::mutex> lk(ctx->mu);
     ctx->trace = enable != 0;
+    return HCLOOC_OK;
+}
+
+extern "C" int hclooc_ctx_set_direct(hclooc_ctx* ctx, int mode) {
+    int rc;
+    if (mode < -1 || mode > 1) return -2;
+    if (!ctx && (rc = default_ctx(&ctx))) return rc;
+    std::lock_guard<std::mutex> lk(ctx->mu);
+    ctx->direct_mode = mode;
     return HCLOOC_OK;
 }
 

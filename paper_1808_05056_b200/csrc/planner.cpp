@@ -79,15 +79,38 @@ void fill_traffic(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool s
         const int64_t reuse = std::min<int64_t>(c.n_abuf, c.h);                 // slices reused per column switch
         const int64_t rows_top = std::min<int64_t>(M, reuse * c.mb);            // rows of the first `reuse` slices
         const int64_t rows_bottom = M - (c.h - reuse) * c.mb;                   // rows of the last `reuse` slices
-        for (int64_t sl = 0; sl < c.w * c.kpanels; ++sl) {
-            const int64_t p = sl / c.w, j = sl % c.w;
-            const int64_t kk = std::min(c.kb, K - p * c.kb);
-            if (j == 0) { el_h2d += (uint64_t)M * kk; n_h2d += c.h; }           // first column of a panel: every slice
-            else {
-                // column sl-1 ended at the bottom when it ran downwards (even), at the top otherwise
-                const int64_t kept = ((sl - 1) & 1) ? rows_top : rows_bottom;
-                el_h2d += (uint64_t)(M - kept) * kk;
-                n_h2d += c.h - reuse;
+        // per K panel p (depth kk_p): column 0 uploads every slice, column j >= 1 (slab sl = p*w + j) keeps the slices at
+        // the end where column sl-1 stopped: the bottom when sl-1 is even (it ran downwards), the top otherwise.
+        // Closed form over the panels: all but the last are kb deep.
+        const int64_t kk_last = K - (c.kpanels - 1) * c.kb;
+        auto panel_cols = [&](int64_t p, int64_t* n_top, int64_t* n_bottom) {   // columns j = 1..w-1 of panel p by turning end
+            const int64_t first = p * c.w + 1, last = p * c.w + c.w - 1;            // slabs sl; parity of sl-1 decides
+            if (last < first) { *n_top = *n_bottom = 0; return; }
+            const int64_t n = last - first + 1;
+            const int64_t n_odd_prev = ((first - 1) & 1) ? (n + 1) / 2 : n / 2;    // sl-1 odd -> kept = rows_top
+            *n_top = n_odd_prev; *n_bottom = n - n_odd_prev;
+        };
+        for (int pass = 0; pass < 2; ++pass) {
+            // pass 0: the kpanels-1 full panels (their column parities alternate with p*w, so count panel by panel only
+            // when w is odd; for even w every panel looks the same), pass 1: the last panel
+            if (pass == 0) {
+                const int64_t full = c.kpanels - 1;
+                if (full <= 0) continue;
+                int64_t nt = 0, nbm = 0;
+                if (c.w % 2 == 0) { panel_cols(0, &nt, &nbm); nt *= full; nbm *= full; }
+                else {
+                    int64_t t0, b0, t1, b1;
+                    panel_cols(0, &t0, &b0); panel_cols(1, &t1, &b1);
+                    const int64_t even_p = (full + 1) / 2, odd_p = full / 2;
+                    nt = t0 * even_p + t1 * odd_p; nbm = b0 * even_p + b1 * odd_p;
+                }
+                el_h2d += (uint64_t)full * (uint64_t)M * c.kb + (uint64_t)(nt * (M - rows_top) + nbm * (M - rows_bottom)) * c.kb;
+                n_h2d += (uint64_t)full * c.h + (uint64_t)(nt + nbm) * (c.h - reuse);
+            } else {
+                int64_t nt, nbm;
+                panel_cols(c.kpanels - 1, &nt, &nbm);
+                el_h2d += (uint64_t)M * kk_last + (uint64_t)(nt * (M - rows_top) + nbm * (M - rows_bottom)) * kk_last;
+                n_h2d += (uint64_t)c.h + (uint64_t)(nt + nbm) * (c.h - reuse);
             }
         }
         el_h2d += (uint64_t)K * (uint64_t)N;                                    // every B slice once
@@ -95,12 +118,12 @@ void fill_traffic(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool s
         if (c.n_bbuf == 1) n_h2d += slabs;
         else {
             n_h2d += 1;                                                         // first slice in one piece
-            for (uint64_t sl = 1; sl < slabs; ++sl) {
-                const int64_t kk = std::min(c.kb, K - (int64_t)(sl / c.w) * c.kb);
-                int64_t i0, nch;
-                prefetch_layout(c.h, kk, c.n_sets, &i0, &nch);
-                n_h2d += nch;
-            }
+            // prefetched slices sl = 1 .. slabs-1: those of the last panel are kk_last deep, the others kb
+            int64_t i0, nch_full, nch_last;
+            prefetch_layout(c.h, c.kb, c.n_sets, &i0, &nch_full);
+            prefetch_layout(c.h, kk_last, c.n_sets, &i0, &nch_last);
+            const uint64_t in_last = (c.kpanels > 1) ? (uint64_t)c.w : (uint64_t)c.w - 1;   // slabs >= 1 inside the last panel
+            n_h2d += in_last * (uint64_t)nch_last + (slabs - 1 - in_last) * (uint64_t)nch_full;
         }
     }
     const uint64_t MNlink = c.c_dev ? 0 : MN;                                   // copies are still enqueued, bytes are not link bytes
@@ -125,7 +148,7 @@ void cost(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool scale_onl
     const double pad_eff = ((double)M * (double)N) / (tile_rows * tile_cols * (double)(TILE * TILE));
     // too few tiles in flight to fill the SMs: a cluster of 2 or 4 CTAs shares each tile's K range.  When the
     // link is the bound the kernels of successive steps hardly overlap, so one step's tiles are all there is.
-    const int force_ks = (int)env_or("HCLOOC_FORCE_KSPLIT", 0);
+    static const int force_ks = (int)env_or("HCLOOC_FORCE_KSPLIT", 0);
     c.t_flop = flops / mm.fp64_flops;
     const double t_in = c.bytes_h2d / mm.h2d_Bps + c.n_h2d * mm.copy_latency_s;
     const double t_out = c.bytes_d2h / mm.d2h_Bps + c.n_d2h * mm.copy_latency_s;
@@ -211,7 +234,8 @@ extern "C" int hclooc_plan_ex(int64_t M, int64_t N, int64_t K, int beta_nonzero,
                               size_t device_budget_bytes, int operands_on_device, hclooc_plan_t* out) {
     const MachineModel& mm = machine_model();
     const bool c_dev = operands_on_device == 2;
-    if (operands_on_device == 2) operands_on_device = 0;
+    const bool direct_ok = operands_on_device == 3 || operands_on_device == 4, direct_forced = operands_on_device == 4;
+    if (operands_on_device >= 2) operands_on_device = 0;
     if (M < 0) return -1;
     if (N < 0) return -2;
     if (K < 0) return -3;
@@ -312,6 +336,32 @@ extern "C" int hclooc_plan_ex(int64_t M, int64_t N, int64_t K, int beta_nonzero,
                     }
                 }
             }
+        }
+    }
+    // ---- DIRECT mode: no staging, one launch whose tiles read A and B from host memory through TMA and update C in
+    // place over the link.  Measured (profiles/r01_direct_mode.md): SM-initiated reads of pinned host memory run at
+    // ~50 GB/s with no reuse between tiles in L2, so the time is the sum of every tile's own reads over that rate
+    // plus ~30 us fixed -- better than a staged plan only where that one is bound by per-copy latency.
+    if (direct_ok && M <= 0x7fffffffLL && N <= 0x7fffffffLL && K <= 0x7fffffffLL) {
+        const double tm = (double)ceil_div(M, TILE), tn = (double)ceil_div(N, TILE);
+        const double rd = 8.0 * ((scale_only ? 0.0 : tn * (double)M * (double)Keff + tm * (double)Keff * (double)N) +
+                                 (beta_nz ? (double)M * (double)N : 0.0));
+        const double wr = 8.0 * (double)M * (double)N;
+        const double direct_Bps = env_or("HCLOOC_DIRECT_GBPS", 50.0) * 1e9;
+        const double t_link = std::max(std::max(rd / direct_Bps, wr / mm.d2h_Bps), (rd + wr) / mm.duplex_Bps);
+        const double t_flop = (scale_only ? 0.0 : 2.0 * (double)M * (double)N * (double)Keff) / mm.fp64_flops;
+        const double waves = std::ceil(tm * tn / NUM_SMS);
+        const double t_comp = t_flop * (waves * NUM_SMS * (double)(TILE * TILE)) / ((double)M * (double)N);
+        const double t_direct = std::max(t_link, t_comp) + 30e-6;
+        if (direct_forced || !found || t_direct < best.t_model) {
+            out->mb = M; out->nb = N; out->kb = Keff;
+            out->h = out->w = out->kpanels = out->n_steps = 1;
+            out->ksplit = 1;
+            out->direct = 1;
+            out->bytes_h2d = (uint64_t)rd; out->bytes_d2h = (uint64_t)wr;
+            out->flops = scale_only ? 0.0 : 2.0 * (double)M * (double)N * (double)K;
+            out->t_flop_s = t_flop; out->t_link_s = t_link; out->t_model_s = t_direct;
+            return HCLOOC_OK;
         }
     }
     if (!found) return HCLOOC_ERR_BUDGET;

@@ -8,6 +8,12 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 
+# The parity tests written for the staged pipeline (slices streamed through device buffers) keep exercising it on
+# the small shapes they use: without this the cost model would route most of them to the direct mode (plan.direct),
+# which has its own tests (they switch it on per context with hclooc_ctx_set_direct).
+os.environ.setdefault("HCLOOC_DIRECT", "0")
+
+
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run with -m gpu on the B200 box)")
 

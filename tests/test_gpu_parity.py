@@ -515,3 +515,103 @@ def test_nsteps_mode_keeps_c_on_the_device(H, dist):
         assert e.value.status == 1
     finally:
         H.hclooc_ctx_destroy(ctx)
+
+
+# ------------------------------------------------------------------ direct mode (plan.direct): TMA straight from host memory
+@pytest.mark.parametrize("dist,exact", [("uniform", False), ("int", True)])
+def test_config1_direct_mode_uses_no_device_memory(H, dist, exact):
+    """BASELINE.json configs[0] through the direct mode: no device buffer at all (0 <= 1 MiB), one launch, every
+    tile streams its A and B panels from pinned host memory through TMA and updates C in host memory."""
+    M = N = K = 512
+    A, B, C = host_inputs(H, M, N, K, synthgen.BASE_SEED + 1, dist)
+    ref = C.view.copy()
+    D = oracle.dgemm(1.0, A.view, B.view, 0.5, ref, want_denominator=True)
+    staged = C.view.copy()
+    ctx = H.hclooc_ctx_create(0)
+    try:
+        H.hclooc_ctx_set_direct(ctx, 1)
+        st = H.hclooc_dgemm_ex(ctx, M, N, K, 1.0, A, A.ld, B, B.ld, 0.5, C, C.ld, 1 * MiB)
+        assert st.plan.direct == 1 and st.plan.workspace_bytes == 0 and st.n_kernels == 1
+        assert st.n_copies_h2d == 0 and st.n_copies_d2h == 0
+        assert st.bytes_h2d == 8 * (4 * M * K + 4 * K * N + M * N) and st.bytes_d2h == 8 * M * N   # 4 x 4 tiles: 4 reads of A and B
+        check(C.view, ref, D, exact)
+        direct = C.view.copy()
+        # the staged pipeline on the same inputs: same kernel, same summation order -> the same bits
+        H.hclooc_ctx_set_direct(ctx, 0)
+        synthgen.fill(C.array, synthgen.BASE_SEED + 1, "C", dist, cols=N)
+        st = H.hclooc_dgemm_ex(ctx, M, N, K, 1.0, A, A.ld, B, B.ld, 0.5, C, C.ld, 1 * MiB)
+        assert st.plan.direct == 0 and st.plan.n_steps > 4
+        assert np.array_equal(C.view.view(np.uint64), direct.view(np.uint64))
+    finally:
+        H.hclooc_ctx_destroy(ctx)
+    with pytest.raises(H.HclError) as e:
+        H.hclooc_ctx_set_direct(None, 2)
+    assert e.value.status == -2
+
+
+@pytest.mark.parametrize("M,N,K,alpha,beta,dist,pads", [
+    (1, 1, 1, 2.0, 0.5, "uniform", (1, 1, 1)),
+    (300, 260, 200, 1.0, 0.5, "uniform", (0, 0, 0)),          # ragged in m, n and k
+    (129, 257, 33, -1.5, 1.0, "normal", (3, 1, 5)),           # odd sizes made even by the padding
+    (517, 389, 1000, 2.0, -1.0, "int", (2, 3, 1)),
+    (131, 78, 97, 3.0, 0.0, "int", (1, 2, 4)),                # beta == 0: C (NaN) is not read over the link
+    (1500, 1300, 260, 1.0, 0.5, "int", (0, 0, 0)),            # 132 tiles
+    (2200, 1800, 70, 1.0, 1.0, "uniform", (0, 2, 2)),         # 270 tiles: more than one wave
+])
+def test_direct_mode_matches_oracle(H, M, N, K, alpha, beta, dist, pads):
+    A, B, C = host_inputs(H, M, N, K, 43, dist, pads=pads, poison_c=(beta == 0.0))
+    ref = np.zeros((M, N)) if beta == 0.0 else C.view.copy()
+    D = oracle.dgemm(alpha, A.view, B.view, beta, ref, want_denominator=True)
+    ctx = H.hclooc_ctx_create(0)
+    try:
+        H.hclooc_ctx_set_direct(ctx, 1)
+        st = H.hclooc_dgemm_ex(ctx, M, N, K, alpha, A, A.ld, B, B.ld, beta, C, C.ld, 1 * MiB)
+        assert st.plan.direct == 1 and st.plan.workspace_bytes == 0
+        tm, tn = -(-M // 128), -(-N // 128)
+        assert st.bytes_h2d == 8 * (tn * M * K + tm * K * N + (M * N if beta != 0.0 else 0))
+        check(C.view, ref, D, exact=(dist == "int"))
+        assert np.isnan(C.array[:, N:]).all()                                   # host padding of C untouched
+    finally:
+        H.hclooc_ctx_destroy(ctx)
+
+
+def test_direct_mode_falls_back_and_degenerates(H):
+    """Odd leading dimensions are not TMA-legal: the call is staged even when direct mode is forced.  alpha == 0
+    scales C in host memory without touching A and B; registered (not cudaHostAlloc'ed) memory works too."""
+    ctx = H.hclooc_ctx_create(0)
+    try:
+        H.hclooc_ctx_set_direct(ctx, 1)
+        M, N, K = 200, 150, 101
+        A, B, C = host_inputs(H, M, N, K, 44, "int")                            # lda = 101: odd
+        ref = C.view.copy()
+        oracle.dgemm(1.0, A.view, B.view, 0.5, ref)
+        st = H.hclooc_dgemm_ex(ctx, M, N, K, 1.0, A, A.ld, B, B.ld, 0.5, C, C.ld, 1 * MiB)
+        assert st.plan.direct == 0 and st.plan.workspace_bytes > 0
+        assert np.array_equal(C.view, ref)
+        # alpha == 0
+        M, N, K = 300, 200, 64
+        A, B, C = host_inputs(H, M, N, K, 44, "uniform")
+        A.array[...] = np.nan; B.array[...] = np.nan
+        C0 = C.view.copy()
+        st = H.hclooc_dgemm_ex(ctx, M, N, K, 0.0, A, A.ld, B, B.ld, -2.0, C, C.ld, 1 * MiB)
+        assert st.plan.direct == 1 and st.plan.scale_only == 1 and st.bytes_h2d == 8 * M * N
+        assert np.array_equal(C.view, -2.0 * C0)
+        C.view[...] = np.nan
+        H.hclooc_dgemm_ex(ctx, M, N, K, 0.0, A, A.ld, B, B.ld, 0.0, C, C.ld, 1 * MiB)
+        assert np.array_equal(C.view, np.zeros((M, N))) and not np.signbit(C.view).any()
+        # pinned in place with hclooc_host_register
+        M, N, K = 256, 128, 64
+        a = synthgen.fill(np.empty((M, K)), 45, "A", "int"); b = synthgen.fill(np.empty((K, N)), 45, "B", "int")
+        c = synthgen.fill(np.empty((M, N)), 45, "C", "int")
+        ref = c.copy()
+        oracle.dgemm(2.0, a, b, 1.0, ref)
+        for x in (a, b, c):
+            H.hclooc_host_register(x, x.nbytes)
+        try:
+            st = H.hclooc_dgemm_ex(ctx, M, N, K, 2.0, a, K, b, N, 1.0, c, N, 1 * MiB)
+        finally:
+            for x in (a, b, c):
+                H.hclooc_host_unregister(x)
+        assert np.array_equal(c, ref)
+    finally:
+        H.hclooc_ctx_destroy(ctx)

@@ -372,3 +372,24 @@ def test_streamk_steps_use_one_scratch_buffer_per_compute_stream():
     out = subprocess.run([sys.executable, "-c", code], cwd=ROOT, env=dict(os.environ, HCLOOC_STREAMK_STEPS="1"),
                          capture_output=True, text=True, check=True).stdout.strip()
     assert out == "-1 2 1 [2, 3] 1", out
+
+
+def test_direct_mode_is_chosen_only_where_copy_latency_dominates():
+    """plan.direct (operands_on_device = 3: host matrices the device can address): the cost model takes it for
+    BASELINE config 1 (512^3 under 1 MiB: hundreds of <= 64 KiB copies) and leaves configs 2-4 staged; the plan
+    uses no device memory and counts every tile's own reads as host-link traffic."""
+    MiB = 1 << 20
+    p = H.hclooc_plan_ex(512, 512, 512, 1, 0, 1 * MiB, 3)
+    assert p.direct == 1 and p.workspace_bytes == 0 and p.n_steps == 1 and p.h == p.w == p.kpanels == 1
+    assert p.bytes_h2d == 8 * (4 * 512 * 512 * 2 + 512 * 512) and p.bytes_d2h == 8 * 512 * 512
+    assert p.n_copies_h2d == 0 and p.n_copies_d2h == 0
+    staged = H.hclooc_plan_ex(512, 512, 512, 1, 0, 1 * MiB, 0)
+    assert staged.direct == 0 and p.t_model_s < staged.t_model_s
+    for (M, N, K, budget) in ((8192, 8192, 8192, 256 * MiB), (32768, 32768, 32768, 4096 * MiB), (65536, 65536, 16384, 16384 * MiB)):
+        q = H.hclooc_plan_ex(M, N, K, 1, 0, budget, 3)
+        assert q.direct == 0 and q.workspace_bytes > 0
+    forced = H.hclooc_plan_ex(8192, 8192, 8192, 0, 0, 256 * MiB, 4)
+    assert forced.direct == 1 and forced.bytes_h2d == 8 * 2 * 64 * 8192 * 8192
+    # a budget too small for any staged plan is no obstacle: direct mode needs none
+    tiny = H.hclooc_plan_ex(300, 300, 300, 1, 0, 4096, 3)
+    assert tiny.direct == 1
