@@ -85,6 +85,7 @@ typedef struct hclooc_plan_t {
                                      times), so it only wins where the staged pipeline is bound by per-copy latency:
                                      small problems under small budgets (BASELINE config 1).  h = w = n_steps = 1.     */
     int32_t  reserved1;
+    uint64_t bytes_transpose_staging;  /* hclooc_dgemm_t: staging buffers of the transposed operands (part of workspace_bytes) */
 } hclooc_plan_t;
 
 /* Plan only (pure host arithmetic, needs no GPU).  alpha_zero != 0 plans the scale-only pass.
@@ -198,6 +199,22 @@ int hclooc_dgemm(int64_t M, int64_t N, int64_t K, double alpha, const double* A,
 int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
                     int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
                     size_t device_budget_bytes, hclooc_stats* stats_out);
+
+/* Transposed operands (SURVEY 8(f) #3; the paper lists them as future work, :412):
+ *     C = alpha * op(A) * op(B) + beta * C,   op(X) = X (HCL_OP_N) or X^T (HCL_OP_T)
+ * op(A) is M x K and op(B) is K x N: with transa = HCL_OP_T, A is stored K x M (lda >= M); with transb = HCL_OP_T, B is
+ * stored N x K (ldb >= K).  A slice of a transposed operand crosses the link in the layout it is stored in (blocks of 2-D
+ * copies into a staging buffer of budget/16, at most 8 MiB, counted against device_budget_bytes) and a transpose kernel on
+ * the copy stream writes it into the row-major device slice the tile kernel reads -- HBM-bound work, ~2 % of a slice's
+ * transfer time; everything else (plan, schedule, DGEMM kernel, events) is the path of hclooc_dgemm_ex.  Calls with a
+ * transposed operand are always staged (no in-core and no direct mode).
+ * Errors: as hclooc_dgemm_ex with the argument numbers of hclooc_dgemm (-6: lda too small for the STORED shape, ...),
+ * plus -15 / -16: transa / transb is neither HCL_OP_N nor HCL_OP_T.                                                  */
+#define HCL_OP_N 0
+#define HCL_OP_T 1
+int hclooc_dgemm_t(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, int64_t K, double alpha,
+                   const double* A, int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
+                   size_t device_budget_bytes, hclooc_stats* stats_out);
 
 /* nsteps mode (:277-283): MMOOC as a subroutine of a blocked algorithm (SUMMA, HSUMMA) that updates the same C
  * `nsteps` times: C = alpha*A_p*B_p + beta_p*C for p = *step = 0 .. nsteps-1, one call per p.  C is uploaded once

@@ -9,12 +9,13 @@ import numpy as np
 from . import build as _build
 
 HCL_H2D, HCL_D2H = 0, 1
+HCL_OP_N, HCL_OP_T = 0, 1
 
 # every symbol include/hclooc.h declares (tests check the .so exports all of them)
 EXPORTS = [
     "hclooc_plan", "hclooc_plan_ex", "hclooc_shard_rows", "hclMatrixPartitioner", "hclooc_schedule", "hclooc_ctx_create", "hclooc_ctx_destroy",
     "hclooc_ctx_set_trace", "hclooc_ctx_get_trace", "hclooc_ctx_set_direct",
-    "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_fig2", "hclooc_dgemm_nsteps", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
+    "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_t", "hclooc_dgemm_fig2", "hclooc_dgemm_nsteps", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
     "hclStreamDestroy", "hclEventDestroy", "hclMemcpy", "hclMemcpyAsync", "hclMemcpy2DAsync",
     "hclDgemmAsync", "hclDgemmAsyncEx", "hclWaitEvent", "hclStreamSynchronize", "hclDeviceSynchronize",
     "hclooc_host_alloc", "hclooc_host_free", "hclooc_host_register", "hclooc_host_unregister",
@@ -34,7 +35,7 @@ class Plan(ctypes.Structure):
                 ("n_copies_h2d", c_uint64), ("n_copies_d2h", c_uint64),
                 ("flops", c_double), ("t_flop_s", c_double), ("t_link_s", c_double), ("t_model_s", c_double),
                 ("n_scratch", c_int32), ("c_on_device", c_int32), ("bytes_scratch", c_uint64),
-                ("direct", c_int32), ("reserved1", c_int32)]
+                ("direct", c_int32), ("reserved1", c_int32), ("bytes_transpose_staging", c_uint64)]
 
     def asdict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -84,6 +85,7 @@ def lib():
         L.hclooc_ctx_set_direct.argtypes = [vp, c_int]
         L.hclooc_dgemm.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz]
         L.hclooc_dgemm_ex.argtypes = [vp, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
+        L.hclooc_dgemm_t.argtypes = [vp, c_int, c_int, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
         L.hclooc_dgemm_nsteps.argtypes = [vp, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, c_int, POINTER(c_int), POINTER(Stats)]
         L.hclooc_dgemm_fig2.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
         L.hclMalloc.argtypes = [POINTER(vp), sz]
@@ -265,6 +267,14 @@ def hclooc_dgemm_ex(ctx, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_bu
     st = Stats()
     _check(lib().hclooc_dgemm_ex(ctx, M, N, K, alpha, _ptr(A), lda, _ptr(B), ldb, beta, _ptr(C), ldc,
                                  device_budget_bytes, byref(st) if want_stats else None), "hclooc_dgemm_ex")
+    return st if want_stats else None
+
+
+def hclooc_dgemm_t(ctx, transa, transb, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes, want_stats=True):
+    """C = alpha*op(A)*op(B) + beta*C; transa / transb: HCL_OP_N (0) or HCL_OP_T (1)."""
+    st = Stats()
+    _check(lib().hclooc_dgemm_t(ctx, int(transa), int(transb), M, N, K, alpha, _ptr(A), lda, _ptr(B), ldb, beta, _ptr(C), ldc,
+                                device_budget_bytes, byref(st) if want_stats else None), "hclooc_dgemm_t")
     return st if want_stats else None
 
 

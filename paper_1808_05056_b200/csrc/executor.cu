@@ -350,9 +350,36 @@ int copy2d(void* dst, size_t dpitch, const void* src, size_t spitch, size_t widt
 
 }  // namespace
 
-extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
-                               int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
-                               size_t device_budget_bytes, hclooc_stats* stats) {
+namespace {
+
+// Upload of a slice of a TRANSPOSED operand (hclooc_dgemm_t): the region op(X)[r0:r0+nr, c0:c0+nc] is stored as
+// X[c0:c0+nc, r0:r0+nr] (row-major, leading dimension ldx).  It crosses the link in the layout it is stored in, in
+// blocks of at most `stage_bytes` (2-D copies, rows >= 1 KiB wide where the region allows: full link rate), and a
+// transpose kernel on the same stream writes each block into the row-major device slice dst (leading dimension ldd).
+int upload_transposed(double* dst, int64_t ldd, const double* X, int64_t ldx, int64_t r0, int64_t nr, int64_t c0, int64_t nc,
+                      double* stage, size_t stage_bytes, cudaStream_t st, uint64_t* n_copies) {
+    if (nr == 0 || nc == 0) return HCLOOC_OK;
+    // stored region: nc rows x nr columns.  Blocks of sr stored rows x sc stored columns.
+    const int64_t cap = (int64_t)(stage_bytes / 8);
+    const int64_t sc = std::min<int64_t>(nr, std::max<int64_t>(32, std::min<int64_t>(4096, cap / 32)));
+    const int64_t sr = std::max<int64_t>(1, std::min<int64_t>(nc, cap / sc));
+    for (int64_t q0 = 0; q0 < nc; q0 += sr) {
+        const int64_t qn = std::min(sr, nc - q0);
+        for (int64_t p0 = 0; p0 < nr; p0 += sc) {
+            const int64_t pn = std::min(sc, nr - p0);
+            int rc = copy2d(stage, (size_t)pn * 8, X + (c0 + q0) * ldx + (r0 + p0), (size_t)ldx * 8, (size_t)pn * 8, (size_t)qn, st);
+            if (rc) return rc;
+            ++*n_copies;
+            // stage is qn x pn (stored rows x stored cols) -> dst rows p0.., columns q0..
+            if ((rc = launch_transpose(stage, qn, pn, pn, dst + p0 * ldd + q0, ldd, st))) return rc;
+        }
+    }
+    return HCLOOC_OK;
+}
+
+int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
+               int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
+               size_t device_budget_bytes, hclooc_stats* stats) {
     const auto t_begin = std::chrono::steady_clock::now();
     // ---------------------------------------------------------------- S0 validate (argument numbers of hclooc_dgemm)
     if (M < 0) return -1;
@@ -361,16 +388,19 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
     if (stats) std::memset(stats, 0, sizeof(*stats));
     if (M == 0 || N == 0) return HCLOOC_OK;
     const bool scale_only = (alpha == 0.0 || K == 0);
+    // stored shapes: op(A) is M x K, so A is K x M when transposed; op(B) is K x N, so B is N x K when transposed
+    const int64_t a_rows = transa ? K : M, a_cols = transa ? M : K, b_rows = transb ? N : K, b_cols = transb ? K : N;
     if (!scale_only) {
         if (!A) return -5;
-        if (lda < K) return -6;
+        if (lda < a_cols) return -6;
         if (!B) return -7;
-        if (ldb < N) return -8;
+        if (ldb < b_cols) return -8;
     }
     if (!C) return -10;
     if (ldc < N) return -11;
-    if (!scale_only && (overlaps(C, M, N, ldc, A, M, K, lda) || overlaps(C, M, N, ldc, B, K, N, ldb))) return -10;
+    if (!scale_only && (overlaps(C, M, N, ldc, A, a_rows, a_cols, lda) || overlaps(C, M, N, ldc, B, b_rows, b_cols, ldb))) return -10;
     if (scale_only && beta == 1.0) return HCLOOC_OK;            // C = 1*C
+    if (scale_only) transa = transb = 0;                        // A and B are not referenced
     int rc;
     if (!ctx && (rc = default_ctx(&ctx))) return rc;
     std::lock_guard<std::mutex> lk(ctx->mu);
@@ -392,20 +422,29 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
         const size_t margin = (size_t)1 << 30;
         budget = fr > 2 * margin ? fr - margin : fr / 2;
     }
+    // transposed operands are staged in the layout they are stored in: one staging buffer each, inside the budget
+    size_t stage_bytes = 0;
+    if (transa || transb) {
+        stage_bytes = std::min<size_t>((size_t)8 << 20, std::max<size_t>((size_t)32 << 10, budget / 16)) & ~(size_t)1023;
+        const size_t total = stage_bytes * (size_t)((transa ? 1 : 0) + (transb ? 1 : 0));
+        if (budget <= 2 * total) return HCLOOC_ERR_BUDGET;
+        budget -= total;
+    }
     hclooc_plan_t P;
     // in-core case: every operand already in device memory and addressable by the tile kernel as it is
     const bool aligned = (((uintptr_t)C & 15u) == 0) && (ldc % 2 == 0) &&
                          (scale_only || ((((uintptr_t)A | (uintptr_t)B) & 15u) == 0 && lda % 2 == 0 && ldb % 2 == 0));
-    const bool in_core = on_device && aligned && M <= 0x7fffffffLL && N <= 0x7fffffffLL && K <= 0x7fffffffLL;
+    const bool in_core = on_device && aligned && !transa && !transb && M <= 0x7fffffffLL && N <= 0x7fffffffLL && K <= 0x7fffffffLL;
     // direct mode needs host matrices the kernel can address as they are: mapped, TMA-legal, host/device address
     // arithmetic interchangeable (the alias of the first element is what the tensor maps are built on)
     static const int direct_env = [] { const char* e = std::getenv("HCLOOC_DIRECT"); return e ? std::atoi(e) : -1; }();
     const int direct_mode = ctx->direct_mode >= 0 ? ctx->direct_mode : direct_env;
-    const bool direct_ok = !in_core && !c_dev && aligned && direct_mode != 0 && M <= 0x7fffffffLL && N <= 0x7fffffffLL && K <= 0x7fffffffLL &&
+    const bool direct_ok = !in_core && !c_dev && !transa && !transb && aligned && direct_mode != 0 && M <= 0x7fffffffLL && N <= 0x7fffffffLL && K <= 0x7fffffffLL &&
                            C_alias && (((uintptr_t)C_alias & 15u) == 0) &&
                            (scale_only || (A_alias && B_alias && ((((uintptr_t)A_alias | (uintptr_t)B_alias) & 15u) == 0)));
     {
-        const hclooc_ctx::PlanKey key{M, N, K, beta != 0.0, alpha == 0.0, in_core ? 1 : (c_dev ? 2 : (direct_ok ? (direct_mode == 1 ? 4 : 3) : 0)), budget};
+        const int where = in_core ? 1 : (c_dev ? 2 : (direct_ok ? (direct_mode == 1 ? 4 : 3) : 0));
+        const hclooc_ctx::PlanKey key{M, N, K, beta != 0.0, alpha == 0.0, where + (transa ? 8 : 0) + (transb ? 16 : 0), budget};
         bool hit = false;
         for (const auto& kv : ctx->plan_cache) {
             const hclooc_ctx::PlanKey& k = kv.first;
@@ -413,8 +452,10 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
                 k.where == key.where && k.budget == key.budget) { P = kv.second; hit = true; break; }
         }
         if (!hit) {
-            rc = hclooc_plan_ex(M, N, K, key.beta_nz, key.alpha_zero, budget, key.where, &P);
+            rc = hclooc_plan_ex(M, N, K, key.beta_nz, key.alpha_zero, budget, where, &P);
             if (rc) return rc;
+            P.bytes_transpose_staging = stage_bytes * (uint64_t)((transa ? 1 : 0) + (transb ? 1 : 0));
+            P.workspace_bytes += P.bytes_transpose_staging;
             if (ctx->plan_cache.size() >= 16) ctx->plan_cache.erase(ctx->plan_cache.begin());
             ctx->plan_cache.emplace_back(key, P);
         }
@@ -456,6 +497,7 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
     }
     std::vector<double*> bufs(P.n_abuf + P.n_sets + P.n_bbuf);
     uint8_t* scratch[MAX_COMPUTE_STREAMS] = {};
+    double *stage_a = nullptr, *stage_b = nullptr;
     if (P.n_scratch > MAX_COMPUTE_STREAMS) return HCLOOC_ERR_INTERNAL;
     {
         uint8_t* q = base;
@@ -463,6 +505,8 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
         for (int a = 0; a < P.n_abuf; ++a) { bufs[a] = (double*)q; q += P.bytes_a_buf; }
         for (int c = 0; c < P.n_sets; ++c) { bufs[P.n_abuf + c] = (double*)q; q += P.bytes_c_buf; }
         for (int i = 0; i < P.n_scratch; ++i) { scratch[i] = q; q += P.bytes_scratch; }
+        if (transa) { stage_a = (double*)q; q += stage_bytes; }
+        if (transb) { stage_b = (double*)q; q += stage_bytes; }
         if ((size_t)(q - base) != P.workspace_bytes) return HCLOOC_ERR_INTERNAL;
     }
     // ---------------------------------------------------------------- events
@@ -478,6 +522,7 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
         HCL_CUDA(cudaMemsetAsync(scratch[i] + streamk_counter_offset(), 0, streamk_counter_bytes(), ctx->s_compute[i]));
     auto stream_of = [&](int s) { return s == 0 ? ctx->s_h2d : (s == 1 ? ctx->s_d2h : ctx->s_compute[s - 2]); };
     uint64_t bytes_h2d = 0, bytes_d2h = 0, n_h2d = 0, n_d2h = 0, n_kernels = 0;
+    uint64_t n_h2d_blocks = 0, n_trans_ops = 0;   // copies (= transpose kernels) issued for the slices of transposed operands
     const auto t_enq0 = std::chrono::steady_clock::now();
     rc = HCLOOC_OK;
     const bool trace = ctx->trace;
@@ -491,7 +536,7 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
     if (use_graph) {
         union { double d; int64_t i; } ua{alpha}, ub{beta};
         key = {M, N, K, ua.i, ub.i, (int64_t)(uintptr_t)A, lda, (int64_t)(uintptr_t)B, ldb, (int64_t)(uintptr_t)C, ldc,
-               (int64_t)(uintptr_t)base, (int64_t)P.workspace_bytes, P.mb, P.nb, P.kb, P.n_sets, P.n_abuf, P.n_bbuf, P.ksplit};
+               (int64_t)(uintptr_t)base, (int64_t)P.workspace_bytes, P.mb, P.nb, P.kb, P.n_sets, P.n_abuf, P.n_bbuf, P.ksplit, transa, transb};
         if (key != ctx->graph_key) {
             // first time this call is seen: run it the ordinary way, capture it if it comes again
             ctx->graph_key = key;
@@ -548,11 +593,13 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
                 break;
             }
             case HCLOOC_OP_H2D_A:
-                rc = copy2d(bufs[o.buf], (size_t)P.lda_dev * 8, A + o.r0 * lda + o.c0, (size_t)lda * 8, (size_t)o.nc * 8, (size_t)o.nr, st);
+                if (transa) { rc = upload_transposed(bufs[o.buf], P.lda_dev, A, lda, o.r0, o.nr, o.c0, o.nc, stage_a, stage_bytes, st, &n_h2d_blocks); ++n_trans_ops; }
+                else rc = copy2d(bufs[o.buf], (size_t)P.lda_dev * 8, A + o.r0 * lda + o.c0, (size_t)lda * 8, (size_t)o.nc * 8, (size_t)o.nr, st);
                 bytes_h2d += (uint64_t)o.nr * o.nc * 8; ++n_h2d;
                 break;
             case HCLOOC_OP_H2D_B:
-                rc = copy2d(bufs[o.buf] + o.dev_r0 * P.ldb_dev, (size_t)P.ldb_dev * 8, B + o.r0 * ldb + o.c0, (size_t)ldb * 8, (size_t)o.nc * 8, (size_t)o.nr, st);
+                if (transb) { rc = upload_transposed(bufs[o.buf] + o.dev_r0 * P.ldb_dev, P.ldb_dev, B, ldb, o.r0, o.nr, o.c0, o.nc, stage_b, stage_bytes, st, &n_h2d_blocks); ++n_trans_ops; }
+                else rc = copy2d(bufs[o.buf] + o.dev_r0 * P.ldb_dev, (size_t)P.ldb_dev * 8, B + o.r0 * ldb + o.c0, (size_t)ldb * 8, (size_t)o.nc * 8, (size_t)o.nr, st);
                 bytes_h2d += (uint64_t)o.nr * o.nc * 8; ++n_h2d;
                 break;
             case HCLOOC_OP_H2D_C:
@@ -635,11 +682,27 @@ extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K,
     if (stats) {
         stats->plan = P;
         stats->bytes_h2d = bytes_h2d; stats->bytes_d2h = bytes_d2h;
-        stats->n_kernels = n_kernels; stats->n_copies_h2d = n_h2d; stats->n_copies_d2h = n_d2h;
+        stats->n_kernels = n_kernels + n_h2d_blocks; stats->n_copies_h2d = n_h2d - n_trans_ops + n_h2d_blocks; stats->n_copies_d2h = n_d2h;
         stats->t_enqueue_s = std::chrono::duration<double>(t_enq1 - t_enq0).count();
         stats->t_total_s = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_begin).count();
     }
     return HCLOOC_OK;
+}
+
+}  // namespace
+
+extern "C" int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
+                               int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
+                               size_t device_budget_bytes, hclooc_stats* stats) {
+    return dgemm_core(ctx, 0, 0, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes, stats);
+}
+
+extern "C" int hclooc_dgemm_t(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, int64_t K, double alpha,
+                              const double* A, int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
+                              size_t device_budget_bytes, hclooc_stats* stats) {
+    if (transa != HCL_OP_N && transa != HCL_OP_T) return -15;
+    if (transb != HCL_OP_N && transb != HCL_OP_T) return -16;
+    return dgemm_core(ctx, transa, transb, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes, stats);
 }
 
 extern "C" int hclooc_dgemm(int64_t M, int64_t N, int64_t K, double alpha, const double* A, int64_t lda,

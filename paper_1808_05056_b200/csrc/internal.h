@@ -75,6 +75,9 @@ inline int64_t early_uploads(int64_t h, int n_sets, int n_abuf) {
     return pre < 0 ? 0 : pre;
 }
 
+// dst[c*ldd + r] = src[r*lds + c] on device pointers (transpose_sm100.cu): the staging step of hclooc_dgemm_t
+int launch_transpose(const double* src, int64_t rows, int64_t cols, int64_t lds, double* dst, int64_t ldd, cudaStream_t stream);
+
 // number of CTAs the tile kernel uses for an M x N output (for stats / tests)
 int64_t dgemm_tile_count(int64_t M, int64_t N);
 

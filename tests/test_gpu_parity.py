@@ -615,3 +615,79 @@ def test_direct_mode_falls_back_and_degenerates(H):
         assert np.array_equal(c, ref)
     finally:
         H.hclooc_ctx_destroy(ctx)
+
+
+# ------------------------------------------------------------------ transposed operands (hclooc_dgemm_t)
+def stored_inputs(H, transa, transb, M, N, K, seed, dist, pads=(0, 0, 0)):
+    """A, B as the caller stores them (A is K x M when transa, B is N x K when transb), C; NaN padding."""
+    ar, ac = (K, M) if transa else (M, K)
+    br, bc = (N, K) if transb else (K, N)
+    A = H.HostMatrix(ar, ac, ac + pads[0]); B = H.HostMatrix(br, bc, bc + pads[1]); C = H.HostMatrix(M, N, N + pads[2])
+    for X in (A, B, C):
+        X.array[...] = np.nan
+    synthgen.fill(A.array, seed, "A", dist, cols=ac); synthgen.fill(B.array, seed, "B", dist, cols=bc)
+    synthgen.fill(C.array, seed, "C", dist, cols=N)
+    return A, B, C
+
+
+@pytest.mark.parametrize("transa,transb", [(1, 0), (0, 1), (1, 1)])
+@pytest.mark.parametrize("M,N,K,alpha,beta,dist,pads,budget", [
+    (300, 260, 200, 1.0, 0.5, "uniform", (0, 0, 0), 1 * MiB),
+    (129, 257, 33, -1.5, 1.0, "normal", (3, 1, 5), 1 * MiB),
+    (517, 389, 1000, 2.0, -1.0, "int", (2, 3, 1), 2 * MiB),        # many staging blocks per slice
+    (1, 1, 1, 2.0, 0.5, "int", (1, 1, 1), 1 * MiB),
+    (640, 1100, 700, 1.0, 0.0, "int", (0, 0, 0), 64 * MiB),        # beta == 0
+    (96, 112, 20000, 2.0, -1.0, "int", (0, 0, 0), 900 * 1024),     # K panels
+])
+def test_transposed_operands_match_oracle(H, transa, transb, M, N, K, alpha, beta, dist, pads, budget):
+    """C = alpha*op(A)*op(B) + beta*C: the oracle gets op(A), op(B) written out; the library gets the stored matrices."""
+    A, B, C = stored_inputs(H, transa, transb, M, N, K, 46, dist, pads)
+    opA, opB = np.empty((M, K)), np.empty((K, N))
+    opA[...] = A.view.T if transa else A.view
+    opB[...] = B.view.T if transb else B.view
+    if beta == 0.0:
+        C.view[...] = np.nan
+    ref = np.zeros((M, N)) if beta == 0.0 else C.view.copy()
+    D = oracle.dgemm(alpha, opA, opB, beta, ref, want_denominator=True)
+    st = H.hclooc_dgemm_t(None, transa, transb, M, N, K, alpha, A, A.ld, B, B.ld, beta, C, C.ld, budget)
+    assert st.plan.direct == 0 and st.plan.workspace_bytes <= budget
+    assert st.plan.bytes_transpose_staging > 0 and st.plan.bytes_transpose_staging % (transa + transb) == 0
+    assert st.bytes_h2d == st.plan.bytes_h2d and st.bytes_d2h == st.plan.bytes_d2h
+    check(C.view, ref, D, exact=(dist == "int"))
+    assert np.isnan(C.array[:, N:]).all()
+
+
+def test_transposed_call_equals_plain_call_on_written_out_transposes(H):
+    """Same kernel, same order of summation: hclooc_dgemm_t on stored A^T, B^T gives the bits of hclooc_dgemm_ex on
+    op(A), op(B) (K below the cluster split-K threshold, not split into panels)."""
+    M, N, K = 515, 389, 301
+    A, B, C = stored_inputs(H, 1, 1, M, N, K, 47, "uniform", pads=(1, 3, 7))
+    opA, opB = H.HostMatrix(M, K), H.HostMatrix(K, N)
+    opA.view[...] = A.view.T; opB.view[...] = B.view.T
+    C2 = H.HostMatrix(M, N); C2.view[...] = C.view
+    st = H.hclooc_dgemm_t(None, H.HCL_OP_T, H.HCL_OP_T, M, N, K, -0.75, A, A.ld, B, B.ld, 1.25, C, C.ld, 4 * MiB)
+    st2 = H.hclooc_dgemm_ex(None, M, N, K, -0.75, opA, opA.ld, opB, opB.ld, 1.25, C2, C2.ld, 4 * MiB)
+    assert st.plan.kpanels == 1 and st2.plan.kpanels == 1
+    assert np.array_equal(C.view.view(np.uint64), C2.view.view(np.uint64))
+    # HCL_OP_N, HCL_OP_N through the same entry point is hclooc_dgemm_ex
+    C3 = H.HostMatrix(M, N); synthgen.fill(C3.array, 47, "C", "uniform", cols=N)
+    st3 = H.hclooc_dgemm_t(None, 0, 0, M, N, K, -0.75, opA, opA.ld, opB, opB.ld, 1.25, C3, C3.ld, 4 * MiB)
+    assert st3.plan.bytes_transpose_staging == 0
+    assert np.array_equal(C3.view.view(np.uint64), C2.view.view(np.uint64))
+
+
+def test_transposed_argument_errors(H):
+    M, N, K = 64, 48, 32
+    A, B, C = stored_inputs(H, 1, 1, M, N, K, 48, "uniform")
+    before = C.view.copy()
+    for args, want in (((2, 0, M, N, K, 1.0, A, M, B, K, 1.0, C, N), -15), ((0, 3, M, N, K, 1.0, A, M, B, K, 1.0, C, N), -16),
+                       ((1, 1, M, N, K, 1.0, A, M - 1, B, K, 1.0, C, N), -6),       # stored A is K x M: lda >= M
+                       ((1, 1, M, N, K, 1.0, A, M, B, K - 1, 1.0, C, N), -8),       # stored B is N x K: ldb >= K
+                       ((1, 1, M, N, K, 1.0, A, M, B, K, 1.0, C, N - 1), -11)):
+        with pytest.raises(H.HclError) as e:
+            H.hclooc_dgemm_t(None, *args, 1 * MiB)
+        assert e.value.status == want, (args[:2], e.value.status)
+    with pytest.raises(H.HclError) as e:
+        H.hclooc_dgemm_t(None, 1, 1, M, N, K, 1.0, A, M, B, K, 1.0, C, N, 100 * 1024)   # staging alone exceeds the budget
+    assert e.value.status == 1
+    assert np.array_equal(C.view, before)
