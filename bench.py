@@ -227,7 +227,11 @@ def run_ours(args, wl, name):
     def resident():
         return H.hclooc_dgemm_ex(ctx, M, N, K, alpha, dA, K, dB, N, beta, dC, N, budget)
 
+    ta, tb = int(args.trans[0] == "T"), int(args.trans[1] == "T")
+
     def host():
+        if ta or tb:     # the M*K (K*N) doubles of A (B) read as the stored K x M (N x K) matrix
+            return H.hclooc_dgemm_t(ctx, ta, tb, M, N, K, alpha, A, M if ta else K, B, K if tb else N, beta, C, C.ld, budget)
         return H.hclooc_dgemm_ex(ctx, M, N, K, alpha, A, A.ld, B, B.ld, beta, C, C.ld, budget)
 
     with ClockSampler(local) as clk:
@@ -282,7 +286,7 @@ def run_ours(args, wl, name):
         "warmup": max(args.warmup, 3), "ms_per_step": ms_res, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic", "ci95_rel": ci_res,
         "config": {"workload": f"{name}: {wl['desc']}", "M": M, "N": N, "K": K, "alpha": alpha, "beta": beta,
-                   "device_budget_bytes": budget, "dist": wl["dist"], "parallelism": (f"{world} row bands of C of {M} rows each, one per GPU (hclooc_shard_rows), B on every rank, no collective"
+                   "device_budget_bytes": budget, "dist": wl["dist"], "trans": args.trans, "parallelism": (f"{world} row bands of C of {M} rows each, one per GPU (hclooc_shard_rows), B on every rank, no collective"
                                    if world > 1 else "1 GPU"), "M_global": world * M,
                    "plan": {k: getattr(plan, k) for k in ("mb", "nb", "kb", "h", "w", "kpanels", "n_steps", "n_sets", "n_bbuf", "workspace_bytes")},
                    "l2": "inputs (A+B+C = %.2f GB) exceed the 126 MB L2; no flush needed" % ((M * K + K * N + M * N) * 8 / 1e9),
@@ -326,6 +330,8 @@ def main():
     ap.add_argument("--ref-rows", type=int, default=512, help="rows of C per oracle step (reference arm)")
     ap.add_argument("--cpu-rows", type=int, default=0, help="rows of C in the cpu_baseline sample (0 = about 1e12 flop, 10-30 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--trans", default="NN", choices=["NN", "TN", "NT", "TT"],
+                    help="e2e leg through hclooc_dgemm_t with op(A), op(B) transposed (the same buffers read as the stored K x M / N x K matrices)")
     ap.add_argument("--kernel-only", action="store_true", help="only the roofline leg (for ncu captures of the tile kernel)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)

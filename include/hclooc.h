@@ -47,6 +47,9 @@ typedef void* hclEvent;                 /* a cudaEvent_t  (the paper's hclEvent,
 /* copy direction, the paper's enum Direction {H2D, D2H} (:136) */
 #define HCL_H2D 0
 #define HCL_D2H 1
+/* op(X) of hclooc_dgemm_t: X as stored, or its transpose */
+#define HCL_OP_N 0
+#define HCL_OP_T 1
 
 /* ------------------------------------------------------------------ the plan (hclMatrixPartitioner, :186, :289)
  * Loop structure:  for p < kpanels:  for j < w:  for i < h:  one step computes the C block
@@ -84,8 +87,9 @@ typedef struct hclooc_plan_t {
                                      (bytes_h2d counts each tile's own reads: A is read ceil(N/128) times, B ceil(M/128)
                                      times), so it only wins where the staged pipeline is bound by per-copy latency:
                                      small problems under small budgets (BASELINE config 1).  h = w = n_steps = 1.     */
-    int32_t  reserved1;
-    uint64_t bytes_transpose_staging;  /* hclooc_dgemm_t: staging buffers of the transposed operands (part of workspace_bytes) */
+    int32_t  trans;               /* hclooc_dgemm_t: bit 0 = A is stored K x M, bit 1 = B is stored N x K.  The device
+                                     slices keep the stored layout: an A slice is then kb x mb (lda_dev >= mb), a B
+                                     slice nb x kb (ldb_dev >= kb), and the tile kernel reads them transposed       */
 } hclooc_plan_t;
 
 /* Plan only (pure host arithmetic, needs no GPU).  alpha_zero != 0 plans the scale-only pass.
@@ -103,6 +107,13 @@ int hclooc_plan(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zer
  * 4 = as 3 but direct mode is forced (tests, experiments).  -8: NULL out. */
 int hclooc_plan_ex(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zero,
                    size_t device_budget_bytes, int operands_on_device, hclooc_plan_t* out);
+
+/* Same for hclooc_dgemm_t (declared below): transa / transb = HCL_OP_N (0) or HCL_OP_T (1) say which operands are stored
+ * transposed; their device slices keep the stored layout (plan.trans), which changes buffer sizes and leading dimensions
+ * and makes thin row slices of a transposed A expensive to upload (rows of mb doubles).  -8 / -9: transa / transb invalid,
+ * -10: NULL out.                                                                                                       */
+int hclooc_plan_trans(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zero, size_t device_budget_bytes,
+                      int operands_on_device, int transa, int transb, hclooc_plan_t* out);
 
 /* The paper's own rule, kept for reference and tests (:289, worked example :301): EQUAL slices only,
  * working set K*nb + 2*mb*K + 2*mb*nb <= budget_elements, least host-to-device traffic
@@ -203,15 +214,13 @@ int hclooc_dgemm_ex(hclooc_ctx* ctx, int64_t M, int64_t N, int64_t K, double alp
 /* Transposed operands (SURVEY 8(f) #3; the paper lists them as future work, :412):
  *     C = alpha * op(A) * op(B) + beta * C,   op(X) = X (HCL_OP_N) or X^T (HCL_OP_T)
  * op(A) is M x K and op(B) is K x N: with transa = HCL_OP_T, A is stored K x M (lda >= M); with transb = HCL_OP_T, B is
- * stored N x K (ldb >= K).  A slice of a transposed operand crosses the link in the layout it is stored in (blocks of 2-D
- * copies into a staging buffer of budget/16, at most 8 MiB, counted against device_budget_bytes) and a transpose kernel on
- * the copy stream writes it into the row-major device slice the tile kernel reads -- HBM-bound work, ~2 % of a slice's
- * transfer time; everything else (plan, schedule, DGEMM kernel, events) is the path of hclooc_dgemm_ex.  Calls with a
- * transposed operand are always staged (no in-core and no direct mode).
+ * stored N x K (ldb >= K).  Nothing is transposed in memory: slices cross the link and sit in their device buffers in
+ * the layout they are stored in, and the tile kernel reads them through tensor maps and fragment addressing made for
+ * that layout (four variants of the same DMMA loop; the order of summation over k is that of hclooc_dgemm_ex, so the
+ * result has the same bits as a call on written-out transposes).  Plan, schedule, events, direct mode and the in-core
+ * case are those of hclooc_dgemm_ex.
  * Errors: as hclooc_dgemm_ex with the argument numbers of hclooc_dgemm (-6: lda too small for the STORED shape, ...),
  * plus -15 / -16: transa / transb is neither HCL_OP_N nor HCL_OP_T.                                                  */
-#define HCL_OP_N 0
-#define HCL_OP_T 1
 int hclooc_dgemm_t(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, int64_t K, double alpha,
                    const double* A, int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
                    size_t device_budget_bytes, hclooc_stats* stats_out);
@@ -279,6 +288,12 @@ int hclDgemmAsync(int64_t M, int64_t N, int64_t K, double alpha, const double* d
 int hclDgemmAsyncEx(int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda,
                     const double* dB, int64_t ldb, double beta, double* dC, int64_t ldc,
                     hclStream s, hclEvent* ev, int variant);
+/* Same on transposed device operands: dC = alpha*op(dA)*op(dB) + beta*dC with dA stored K x M when transa = HCL_OP_T
+ * (lda >= M) and dB stored N x K when transb = HCL_OP_T (ldb >= K).  variant: HCL_DGEMM_AUTO, 1, 2 or 4 (the persistent
+ * stream-K kernel exists for untransposed operands only).  -15 / -16: transa / transb invalid.                     */
+int hclDgemmAsyncT(int transa, int transb, int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda,
+                   const double* dB, int64_t ldb, double beta, double* dC, int64_t ldc,
+                   hclStream s, hclEvent* ev, int variant);
 int hclWaitEvent(hclStream s, hclEvent e);                        /* :116  stream waits for event   */
 int hclStreamSynchronize(hclStream s);                            /* :115                           */
 int hclDeviceSynchronize(int device);                             /* :114                           */

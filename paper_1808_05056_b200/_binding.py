@@ -13,11 +13,11 @@ HCL_OP_N, HCL_OP_T = 0, 1
 
 # every symbol include/hclooc.h declares (tests check the .so exports all of them)
 EXPORTS = [
-    "hclooc_plan", "hclooc_plan_ex", "hclooc_shard_rows", "hclMatrixPartitioner", "hclooc_schedule", "hclooc_ctx_create", "hclooc_ctx_destroy",
+    "hclooc_plan", "hclooc_plan_ex", "hclooc_plan_trans", "hclooc_shard_rows", "hclMatrixPartitioner", "hclooc_schedule", "hclooc_ctx_create", "hclooc_ctx_destroy",
     "hclooc_ctx_set_trace", "hclooc_ctx_get_trace", "hclooc_ctx_set_direct",
     "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_t", "hclooc_dgemm_fig2", "hclooc_dgemm_nsteps", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
     "hclStreamDestroy", "hclEventDestroy", "hclMemcpy", "hclMemcpyAsync", "hclMemcpy2DAsync",
-    "hclDgemmAsync", "hclDgemmAsyncEx", "hclWaitEvent", "hclStreamSynchronize", "hclDeviceSynchronize",
+    "hclDgemmAsync", "hclDgemmAsyncEx", "hclDgemmAsyncT", "hclWaitEvent", "hclStreamSynchronize", "hclDeviceSynchronize",
     "hclooc_host_alloc", "hclooc_host_free", "hclooc_host_register", "hclooc_host_unregister",
     "hclooc_strerror", "hclooc_last_cuda_error", "hclooc_version",
 ]
@@ -35,7 +35,7 @@ class Plan(ctypes.Structure):
                 ("n_copies_h2d", c_uint64), ("n_copies_d2h", c_uint64),
                 ("flops", c_double), ("t_flop_s", c_double), ("t_link_s", c_double), ("t_model_s", c_double),
                 ("n_scratch", c_int32), ("c_on_device", c_int32), ("bytes_scratch", c_uint64),
-                ("direct", c_int32), ("reserved1", c_int32), ("bytes_transpose_staging", c_uint64)]
+                ("direct", c_int32), ("trans", c_int32)]
 
     def asdict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -76,6 +76,7 @@ def lib():
         L.hclooc_plan.argtypes = [i64, i64, i64, c_int, c_int, sz, POINTER(Plan)]
         L.hclooc_shard_rows.argtypes = [i64, c_int, c_int, i64, POINTER(i64), POINTER(i64)]
         L.hclooc_plan_ex.argtypes = [i64, i64, i64, c_int, c_int, sz, c_int, POINTER(Plan)]
+        L.hclooc_plan_trans.argtypes = [i64, i64, i64, c_int, c_int, sz, c_int, c_int, c_int, POINTER(Plan)]
         L.hclMatrixPartitioner.argtypes = [i64, i64, i64, i64, POINTER(i64), POINTER(i64)]
         L.hclooc_schedule.argtypes = [POINTER(Plan), c_int, vp, sz, POINTER(sz)]
         L.hclooc_ctx_create.argtypes = [POINTER(vp), c_int, vp, sz, vp, vp, POINTER(vp), c_int]
@@ -99,6 +100,7 @@ def lib():
         L.hclMemcpy2DAsync.argtypes = [vp, sz, vp, sz, sz, sz, c_int, vp, POINTER(vp)]
         L.hclDgemmAsync.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, vp, POINTER(vp)]
         L.hclDgemmAsyncEx.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, vp, POINTER(vp), c_int]
+        L.hclDgemmAsyncT.argtypes = [c_int, c_int, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, vp, POINTER(vp), c_int]
         L.hclWaitEvent.argtypes = [vp, vp]
         L.hclStreamSynchronize.argtypes = [vp]
         L.hclDeviceSynchronize.argtypes = [c_int]
@@ -198,6 +200,13 @@ def hclooc_plan_ex(M, N, K, beta_nonzero, alpha_zero, device_budget_bytes, opera
     p = Plan()
     _check(lib().hclooc_plan_ex(M, N, K, int(bool(beta_nonzero)), int(bool(alpha_zero)), device_budget_bytes,
                                 int(operands_on_device), byref(p)), "hclooc_plan_ex")
+    return p
+
+
+def hclooc_plan_trans(M, N, K, beta_nonzero, alpha_zero, device_budget_bytes, operands_on_device, transa, transb) -> Plan:
+    p = Plan()
+    _check(lib().hclooc_plan_trans(M, N, K, int(bool(beta_nonzero)), int(bool(alpha_zero)), device_budget_bytes,
+                                   int(operands_on_device), int(transa), int(transb), byref(p)), "hclooc_plan_trans")
     return p
 
 
@@ -353,6 +362,13 @@ def hclDgemmAsyncEx(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, stream=None
     ev = _ev(want_event, event)
     _check(lib().hclDgemmAsyncEx(M, N, K, alpha, _ptr(dA), lda, _ptr(dB), ldb, beta, _ptr(dC), ldc, _ptr(stream),
                                  byref(ev) if ev is not None else None, variant), "hclDgemmAsyncEx")
+    return ev.value if ev is not None else None
+
+
+def hclDgemmAsyncT(transa, transb, M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, stream=None, want_event=False, event=None, variant=0):
+    ev = _ev(want_event, event)
+    _check(lib().hclDgemmAsyncT(int(transa), int(transb), M, N, K, alpha, _ptr(dA), lda, _ptr(dB), ldb, beta, _ptr(dC), ldc, _ptr(stream),
+                                byref(ev) if ev is not None else None, variant), "hclDgemmAsyncT")
     return ev.value if ev is not None else None
 
 

@@ -103,43 +103,89 @@ __device__ __forceinline__ void tile_coords(int tile, int tiles_m, int tiles_n, 
 // m-tile, the 4 k indices of a k-step and the 8 columns of an n-tile are permuted (row g <-> 4(g&1)+(g>>1),
 // k index t <-> 2t+e, columns interleaved in pairs) so that with the 128-byte swizzle every LDS.128 of a
 // quarter warp hits distinct banks and feeds two DMMAs.
-struct FragLanes {
-    uint32_t a_lane, b_lane[2];
-    int rp, t, wm, wn;
+//
+// Transposed operands (hclooc_dgemm_t) change only how a stage is laid out and read, never the DMMA loop:
+//   operand stored with k contiguous   (A, or B^T = stored N x K): two 16-k halves of 128 rows x 128 B; one LDS.128 of
+//        lane (g, t) at row 8*tile + rp(g), chunk t gives k = 2t and 2t+1 of that row -> the operands of k-steps e = 0, 1;
+//   operand stored with k as the row   (B, or A^T = stored K x M): eight boxes of 32 k-rows x 16 columns; one LDS.128 at
+//        k-row 2t+e, chunk g gives columns 2g and 2g+1 -> the operands of two m- (or n-) tiles of k-step e.
+// Which row (column) of C a DMMA tile's index g stands for follows from that and is undone in the epilogue:
+//   A as stored M x K : row = 8u + rp(g)                      A^T (stored K x M): row = 16(u>>1) + 2g + (u&1)
+//   B as stored K x N : col = 16bx + 2c' + v  (c' = DMMA col)  B^T (stored N x K): col = 8(2bx+v) + rp(c')
+template <bool TA, bool TB>
+struct FragLanesT {
+    uint32_t a_lane, a_lane_t[2], b_lane[2], b_lane_t;
+    int rp, t, g, wm, wn;
     __device__ __forceinline__ void init(int warp, int lane) {
-        const int g = lane >> 2;
+        g = lane >> 2;
         t = lane & 3;
         rp = 4 * (g & 1) + (g >> 1);
         wm = warp & 3;
         wn = warp >> 2;
         a_lane = (uint32_t)((wm * 32 + rp) * 128 + ((t ^ rp) << 4));
+        b_lane_t = (uint32_t)(A_STAGE_BYTES + (wn * 64 + rp) * 128 + ((t ^ rp) << 4));
         #pragma unroll
-        for (int e = 0; e < 2; ++e)
+        for (int e = 0; e < 2; ++e) {
             b_lane[e] = (uint32_t)(A_STAGE_BYTES + wn * 4 * B_BOX_BYTES + (2 * t + e) * 128 + ((g ^ (2 * t + e)) << 4));
+            a_lane_t[e] = (uint32_t)(wm * 2 * B_BOX_BYTES + (2 * t + e) * 128 + ((g ^ (2 * t + e)) << 4));
+        }
+    }
+    // row of C (inside the CTA tile) that accumulator group u of this lane belongs to
+    __device__ __forceinline__ int row_of(int u) const {
+        return TA ? wm * 32 + (u >> 1) * 16 + 2 * g + (u & 1) : wm * 32 + u * 8 + rp;
     }
 };
+using FragLanes = FragLanesT<false, false>;
 
 // One k block (BK deep) of the 32 x 64 warp tile: per group of 8 k, 12 LDS.128 feed 64 DMMA.8x8x4.
-__device__ __forceinline__ void mma_kblock(double (&acc)[4][4][2][2], uint32_t sbase, const FragLanes& f) {
+template <bool TA, bool TB>
+__device__ __forceinline__ void mma_kblock(double (&acc)[4][4][2][2], uint32_t sbase, const FragLanesT<TA, TB>& f) {
     #pragma unroll
     for (int kg = 0; kg < BK / 8; ++kg) {
         double a[4][2];
-        const uint32_t abase = sbase + (kg >> 1) * A_HALF_BYTES + (f.a_lane ^ ((kg & 1) << 6));
-        #pragma unroll
-        for (int u = 0; u < 4; ++u) lds128(a[u][0], a[u][1], abase + u * 1024);
-        #pragma unroll
-        for (int e = 0; e < 2; ++e) {
-            double b[4][2];
+        if (!TA) {
+            const uint32_t abase = sbase + (kg >> 1) * A_HALF_BYTES + (f.a_lane ^ ((kg & 1) << 6));
             #pragma unroll
-            for (int bx = 0; bx < 4; ++bx)
-                lds128(b[bx][0], b[bx][1], sbase + f.b_lane[e] + kg * 1024 + bx * B_BOX_BYTES);
+            for (int u = 0; u < 4; ++u) lds128(a[u][0], a[u][1], abase + u * 1024);
+        } else {
             #pragma unroll
-            for (int u = 0; u < 4; ++u)
+            for (int e = 0; e < 2; ++e)
                 #pragma unroll
-                for (int bx = 0; bx < 4; ++bx) {
-                    dmma(acc[u][bx][0], a[u][e], b[bx][0]);
-                    dmma(acc[u][bx][1], a[u][e], b[bx][1]);
-                }
+                for (int ub = 0; ub < 2; ++ub)
+                    lds128(a[2 * ub][e], a[2 * ub + 1][e], sbase + f.a_lane_t[e] + kg * 1024 + ub * B_BOX_BYTES);
+        }
+        if (!TB) {
+            #pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                double b[4][2];
+                #pragma unroll
+                for (int bx = 0; bx < 4; ++bx)
+                    lds128(b[bx][0], b[bx][1], sbase + f.b_lane[e] + kg * 1024 + bx * B_BOX_BYTES);
+                #pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    #pragma unroll
+                    for (int bx = 0; bx < 4; ++bx) {
+                        dmma(acc[u][bx][0], a[u][e], b[bx][0]);
+                        dmma(acc[u][bx][1], a[u][e], b[bx][1]);
+                    }
+            }
+        } else {
+            const uint32_t bbase = sbase + (kg >> 1) * A_HALF_BYTES + (f.b_lane_t ^ ((kg & 1) << 6));
+            #pragma unroll
+            for (int half = 0; half < 2; ++half) {       // n-tiles j = 2bx + v, four at a time: both k-steps from one LDS.128
+                double b[2][2][2];                        // [bx in half][v][e]
+                #pragma unroll
+                for (int q = 0; q < 4; ++q) lds128(b[q >> 1][q & 1][0], b[q >> 1][q & 1][1], bbase + (half * 4 + q) * 1024);
+                #pragma unroll
+                for (int e = 0; e < 2; ++e)
+                    #pragma unroll
+                    for (int u = 0; u < 4; ++u)
+                        #pragma unroll
+                        for (int bq = 0; bq < 2; ++bq) {
+                            dmma(acc[u][half * 2 + bq][0], a[u][e], b[bq][0][e]);
+                            dmma(acc[u][half * 2 + bq][1], a[u][e], b[bq][1][e]);
+                        }
+            }
         }
     }
 }
@@ -151,35 +197,55 @@ __device__ __forceinline__ int edge_groups(int extent, int origin, int unit) {
     return left <= 0 ? 0 : (left >= 4 * unit ? 4 : (left + unit - 1) / unit);
 }
 
+// alpha*acc + beta*c with the rounding sequence of the definition (oracle: two products and one sum, each
+// rounded): spelled with intrinsics so that no variant of the epilogue is contracted into an FMA differently from another.
+__device__ __forceinline__ double axpby_tail(double alpha_acc, double beta, double c) {
+    return __dadd_rn(alpha_acc, __dmul_rn(beta, c));
+}
+
 // Fused epilogue: C = alpha*acc + beta*C straight from registers; C is not read when beta == 0.
+template <bool TA, bool TB>
 __device__ __forceinline__ void epilogue_store(const double (&acc)[4][4][2][2], double* __restrict__ C, long long ldc,
-                                               int M, int N, int m0, int n0, double alpha, double beta, const FragLanes& f) {
+                                               int M, int N, int m0, int n0, double alpha, double beta, const FragLanesT<TA, TB>& f) {
     const bool read_c = (beta != 0.0);
     const bool vec_ok = ((ldc & 1LL) == 0) && ((reinterpret_cast<uintptr_t>(C) & 15u) == 0);
     #pragma unroll
     for (int u = 0; u < 4; ++u) {
-        const int row = m0 + f.wm * 32 + u * 8 + f.rp;
+        const int row = m0 + f.row_of(u);
         if (row >= M) continue;
         double* crow = C + (long long)row * ldc;
         #pragma unroll
         for (int bx = 0; bx < 4; ++bx) {
-            const int col = n0 + f.wn * 64 + bx * 16 + 4 * f.t;
-            // lane holds 4 consecutive columns: (v=0,c0) (v=1,c0) (v=0,c1) (v=1,c1)
-            double x0 = alpha * acc[u][bx][0][0], x1 = alpha * acc[u][bx][1][0];
-            double x2 = alpha * acc[u][bx][0][1], x3 = alpha * acc[u][bx][1][1];
-            if (col + 3 < N && vec_ok) {
-                double2* p = reinterpret_cast<double2*>(crow + col);
-                if (read_c) {
-                    const double2 c01 = p[0], c23 = p[1];
-                    x0 += beta * c01.x; x1 += beta * c01.y; x2 += beta * c23.x; x3 += beta * c23.y;
+            if (!TB) {
+                const int col = n0 + f.wn * 64 + bx * 16 + 4 * f.t;
+                // lane holds 4 consecutive columns: (v=0,c0) (v=1,c0) (v=0,c1) (v=1,c1)
+                double x0 = __dmul_rn(alpha, acc[u][bx][0][0]), x1 = __dmul_rn(alpha, acc[u][bx][1][0]);
+                double x2 = __dmul_rn(alpha, acc[u][bx][0][1]), x3 = __dmul_rn(alpha, acc[u][bx][1][1]);
+                if (col + 3 < N && vec_ok) {
+                    double2* p = reinterpret_cast<double2*>(crow + col);
+                    if (read_c) {
+                        const double2 c01 = p[0], c23 = p[1];
+                        x0 = axpby_tail(x0, beta, c01.x); x1 = axpby_tail(x1, beta, c01.y);
+                        x2 = axpby_tail(x2, beta, c23.x); x3 = axpby_tail(x3, beta, c23.y);
+                    }
+                    p[0] = make_double2(x0, x1);
+                    p[1] = make_double2(x2, x3);
+                } else {
+                    const double xs[4] = {x0, x1, x2, x3};
+                    #pragma unroll
+                    for (int q = 0; q < 4; ++q)
+                        if (col + q < N) crow[col + q] = read_c ? axpby_tail(xs[q], beta, crow[col + q]) : xs[q];
                 }
-                p[0] = make_double2(x0, x1);
-                p[1] = make_double2(x2, x3);
             } else {
-                const double xs[4] = {x0, x1, x2, x3};
+                // B^T: n-tile j = 2bx + v, DMMA column c' = 2t + c stands for column 8j + rp(c') = 8j + t + 4c
                 #pragma unroll
-                for (int q = 0; q < 4; ++q)
-                    if (col + q < N) crow[col + q] = read_c ? xs[q] + beta * crow[col + q] : xs[q];
+                for (int v = 0; v < 2; ++v)
+                    #pragma unroll
+                    for (int c = 0; c < 2; ++c) {
+                        const int col = n0 + f.wn * 64 + (2 * bx + v) * 8 + f.t + 4 * c;
+                        const double x = __dmul_rn(alpha, acc[u][bx][v][c]);
+                        if (col < N) crow[col] = read_c ? axpby_tail(x, beta, crow[col]) : x;
+                    }
             }
         }
     }

@@ -35,7 +35,9 @@ using namespace dev;
 // CTAs shares the tile: CTA r of the cluster takes the r-th share of the k blocks, the partial
 // accumulators are reduced through distributed shared memory in rank order (deterministic) and CTA 0
 // runs the epilogue.  Used when a pipeline step has too few tiles to fill 148 SMs.
-template <int KSPLIT>
+// TA / TB: the operand is stored transposed (A as K x M, B as N x K; hclooc_dgemm_t): only the TMA boxes and the fragment
+// addressing change (dgemm_device.cuh), the DMMA loop and the order of summation over k do not.
+template <int KSPLIT, bool TA = false, bool TB = false>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 hclooc_dgemm_tile_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                          double* __restrict__ C, long long ldc, int M, int N, int K,
@@ -81,10 +83,20 @@ hclooc_dgemm_tile_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_c
                 const uint32_t sa = smem_base + stage * STAGE_BYTES;
                 const uint32_t sb = sa + A_STAGE_BYTES;
                 const int k0 = (kb_begin + kb) * BK;
-                #pragma unroll
-                for (int hk = 0; hk < BK / 16; ++hk) tma_load_2d(sa + hk * A_HALF_BYTES, &tmA, k0 + 16 * hk, m0, full);
-                #pragma unroll
-                for (int b = 0; b < BN / 16; ++b) tma_load_2d(sb + b * B_BOX_BYTES, &tmB, n0 + 16 * b, k0, full);
+                if (!TA) {
+                    #pragma unroll
+                    for (int hk = 0; hk < BK / 16; ++hk) tma_load_2d(sa + hk * A_HALF_BYTES, &tmA, k0 + 16 * hk, m0, full);
+                } else {        // stored K x M: eight boxes of 32 k-rows x 16 m
+                    #pragma unroll
+                    for (int b = 0; b < BM / 16; ++b) tma_load_2d(sa + b * B_BOX_BYTES, &tmA, m0 + 16 * b, k0, full);
+                }
+                if (!TB) {
+                    #pragma unroll
+                    for (int b = 0; b < BN / 16; ++b) tma_load_2d(sb + b * B_BOX_BYTES, &tmB, n0 + 16 * b, k0, full);
+                } else {        // stored N x K: two 16-k halves of 128 n-rows
+                    #pragma unroll
+                    for (int hk = 0; hk < BK / 16; ++hk) tma_load_2d(sb + hk * A_HALF_BYTES, &tmB, k0 + 16 * hk, n0, full);
+                }
                 if (++stage == STAGES) { stage = 0; phase ^= 1u; }
             }
         }
@@ -97,7 +109,7 @@ hclooc_dgemm_tile_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_c
 
     // ---------------------------------------------------------------- consumer warps: DMMA
     regs_take_consumer();
-    FragLanes f;
+    FragLanesT<TA, TB> f;
     f.init(warp, lane);
 
     double acc[4][4][2][2];
@@ -206,19 +218,28 @@ int make_map(CUtensorMap* map, const double* base, int64_t rows, int64_t cols, i
     return HCLOOC_OK;
 }
 
+template <bool TA, bool TB>
+cudaError_t set_attr_all_splits() {
+    cudaError_t e = cudaFuncSetAttribute(hclooc_dgemm_tile_kernel<1, TA, TB>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(hclooc_dgemm_tile_kernel<2, TA, TB>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(hclooc_dgemm_tile_kernel<4, TA, TB>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    return e;
+}
+
 int ensure_kernel_attr() {
     static int status = -1;
     static std::once_flag once;
     std::call_once(once, [] {
-        cudaError_t e = cudaFuncSetAttribute(hclooc_dgemm_tile_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(hclooc_dgemm_tile_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(hclooc_dgemm_tile_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+        cudaError_t e = set_attr_all_splits<false, false>();
+        if (e == cudaSuccess) e = set_attr_all_splits<true, false>();
+        if (e == cudaSuccess) e = set_attr_all_splits<false, true>();
+        if (e == cudaSuccess) e = set_attr_all_splits<true, true>();
         status = (e == cudaSuccess) ? 0 : cuda_fail(e);
     });
     return status;
 }
 
-template <int KSPLIT>
+template <int KSPLIT, bool TA, bool TB>
 cudaError_t launch_split(unsigned tiles, cudaStream_t stream, const CUtensorMap& tmA, const CUtensorMap& tmB, double* dC,
                          long long ldc, int M, int N, int K, double alpha, double beta, int tm, int tn) {
     cudaLaunchConfig_t cfg = {};
@@ -233,7 +254,16 @@ cudaError_t launch_split(unsigned tiles, cudaStream_t stream, const CUtensorMap&
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, hclooc_dgemm_tile_kernel<KSPLIT>, tmA, tmB, dC, ldc, M, N, K, alpha, beta, tm, tn);
+    return cudaLaunchKernelEx(&cfg, hclooc_dgemm_tile_kernel<KSPLIT, TA, TB>, tmA, tmB, dC, ldc, M, N, K, alpha, beta, tm, tn);
+}
+
+template <bool TA, bool TB>
+cudaError_t launch_any_split(int ksplit, unsigned tiles, cudaStream_t stream, const CUtensorMap& tmA, const CUtensorMap& tmB, double* dC,
+                             long long ldc, int M, int N, int K, double alpha, double beta, int tm, int tn) {
+    if (ksplit >= 4) return launch_split<4, TA, TB>(tiles, stream, tmA, tmB, dC, ldc, M, N, K, alpha, beta, tm, tn);
+    if (ksplit >= 2) return launch_split<2, TA, TB>(tiles, stream, tmA, tmB, dC, ldc, M, N, K, alpha, beta, tm, tn);
+    hclooc_dgemm_tile_kernel<1, TA, TB><<<tiles, NUM_THREADS, SMEM_BYTES, stream>>>(tmA, tmB, dC, ldc, M, N, K, alpha, beta, tm, tn);
+    return cudaGetLastError();
 }
 
 }  // namespace
@@ -249,23 +279,24 @@ int dgemm_auto_ksplit(int64_t tiles_in_flight, int64_t K) {
 
 int launch_dgemm_tiles(int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda,
                        const double* dB, int64_t ldb, double beta, double* dC, int64_t ldc, cudaStream_t stream,
-                       int ksplit, void* streamk_scratch) {
+                       int ksplit, void* streamk_scratch, int transa, int transb) {
     if (M == 0 || N == 0) return HCLOOC_OK;
     if (alpha == 0.0) K = 0;                       // A and B are not referenced (BLAS convention)
     int rc = ensure_kernel_attr();
     if (rc) return rc;
     CUtensorMap tmA, tmB;
     if (K > 0) {
-        if ((rc = make_map(&tmA, dA, M, K, lda, BM))) return rc;
-        if ((rc = make_map(&tmB, dB, K, N, ldb, BK))) return rc;
+        if ((rc = transa ? make_map(&tmA, dA, K, M, lda, BK) : make_map(&tmA, dA, M, K, lda, BM))) return rc;
+        if ((rc = transb ? make_map(&tmB, dB, N, K, ldb, BN) : make_map(&tmB, dB, K, N, ldb, BK))) return rc;
     } else {
         memset(&tmA, 0, sizeof(tmA));
         memset(&tmB, 0, sizeof(tmB));
+        transa = transb = 0;
     }
     const int64_t tm = (M + BM - 1) / BM, tn = (N + BN - 1) / BN;
     if (tm * tn > 0x7fffffffLL || M > 0x7fffffffLL || N > 0x7fffffffLL || K > 0x7fffffffLL) return HCLOOC_ERR_INTERNAL;
     static const bool no_streamk = getenv("HCLOOC_NO_STREAMK") != nullptr;   // experiment knob
-    if (ksplit < 0 && K > 0 && !no_streamk) {
+    if (ksplit < 0 && K > 0 && !no_streamk && !transa && !transb) {
         // A launch that has the GPU to itself.  One CTA per tile runs its main loop ~1 % faster than the persistent
         // kernel (measured 0.981 against 0.969 of peak on whole waves) but leaves the last wave partly empty, so
         // the persistent stream-K kernel is used unless the tiles fill their waves to 98.8 % or better.  A caller
@@ -279,14 +310,12 @@ int launch_dgemm_tiles(int64_t M, int64_t N, int64_t K, double alpha, const doub
     }
     if (ksplit <= 0) ksplit = dgemm_auto_ksplit(tm * tn, K);
     if (K == 0) ksplit = 1;
+    const unsigned tiles = (unsigned)(tm * tn);
     cudaError_t e;
-    if (ksplit >= 4) e = launch_split<4>((unsigned)(tm * tn), stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn);
-    else if (ksplit >= 2) e = launch_split<2>((unsigned)(tm * tn), stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn);
-    else {
-        hclooc_dgemm_tile_kernel<1><<<(unsigned)(tm * tn), NUM_THREADS, SMEM_BYTES, stream>>>(
-            tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn);
-        e = cudaGetLastError();
-    }
+    if (transa && transb) e = launch_any_split<true, true>(ksplit, tiles, stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn);
+    else if (transa) e = launch_any_split<true, false>(ksplit, tiles, stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn);
+    else if (transb) e = launch_any_split<false, true>(ksplit, tiles, stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn);
+    else e = launch_any_split<false, false>(ksplit, tiles, stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn);
     if (e != cudaSuccess) return cuda_fail(e);
     return HCLOOC_OK;
 }

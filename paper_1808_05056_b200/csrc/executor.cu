@@ -352,31 +352,6 @@ int copy2d(void* dst, size_t dpitch, const void* src, size_t spitch, size_t widt
 
 namespace {
 
-// Upload of a slice of a TRANSPOSED operand (hclooc_dgemm_t): the region op(X)[r0:r0+nr, c0:c0+nc] is stored as
-// X[c0:c0+nc, r0:r0+nr] (row-major, leading dimension ldx).  It crosses the link in the layout it is stored in, in
-// blocks of at most `stage_bytes` (2-D copies, rows >= 1 KiB wide where the region allows: full link rate), and a
-// transpose kernel on the same stream writes each block into the row-major device slice dst (leading dimension ldd).
-int upload_transposed(double* dst, int64_t ldd, const double* X, int64_t ldx, int64_t r0, int64_t nr, int64_t c0, int64_t nc,
-                      double* stage, size_t stage_bytes, cudaStream_t st, uint64_t* n_copies) {
-    if (nr == 0 || nc == 0) return HCLOOC_OK;
-    // stored region: nc rows x nr columns.  Blocks of sr stored rows x sc stored columns.
-    const int64_t cap = (int64_t)(stage_bytes / 8);
-    const int64_t sc = std::min<int64_t>(nr, std::max<int64_t>(32, std::min<int64_t>(4096, cap / 32)));
-    const int64_t sr = std::max<int64_t>(1, std::min<int64_t>(nc, cap / sc));
-    for (int64_t q0 = 0; q0 < nc; q0 += sr) {
-        const int64_t qn = std::min(sr, nc - q0);
-        for (int64_t p0 = 0; p0 < nr; p0 += sc) {
-            const int64_t pn = std::min(sc, nr - p0);
-            int rc = copy2d(stage, (size_t)pn * 8, X + (c0 + q0) * ldx + (r0 + p0), (size_t)ldx * 8, (size_t)pn * 8, (size_t)qn, st);
-            if (rc) return rc;
-            ++*n_copies;
-            // stage is qn x pn (stored rows x stored cols) -> dst rows p0.., columns q0..
-            if ((rc = launch_transpose(stage, qn, pn, pn, dst + p0 * ldd + q0, ldd, st))) return rc;
-        }
-    }
-    return HCLOOC_OK;
-}
-
 int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
                int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
                size_t device_budget_bytes, hclooc_stats* stats) {
@@ -422,24 +397,16 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
         const size_t margin = (size_t)1 << 30;
         budget = fr > 2 * margin ? fr - margin : fr / 2;
     }
-    // transposed operands are staged in the layout they are stored in: one staging buffer each, inside the budget
-    size_t stage_bytes = 0;
-    if (transa || transb) {
-        stage_bytes = std::min<size_t>((size_t)8 << 20, std::max<size_t>((size_t)32 << 10, budget / 16)) & ~(size_t)1023;
-        const size_t total = stage_bytes * (size_t)((transa ? 1 : 0) + (transb ? 1 : 0));
-        if (budget <= 2 * total) return HCLOOC_ERR_BUDGET;
-        budget -= total;
-    }
     hclooc_plan_t P;
     // in-core case: every operand already in device memory and addressable by the tile kernel as it is
     const bool aligned = (((uintptr_t)C & 15u) == 0) && (ldc % 2 == 0) &&
                          (scale_only || ((((uintptr_t)A | (uintptr_t)B) & 15u) == 0 && lda % 2 == 0 && ldb % 2 == 0));
-    const bool in_core = on_device && aligned && !transa && !transb && M <= 0x7fffffffLL && N <= 0x7fffffffLL && K <= 0x7fffffffLL;
+    const bool in_core = on_device && aligned && M <= 0x7fffffffLL && N <= 0x7fffffffLL && K <= 0x7fffffffLL;
     // direct mode needs host matrices the kernel can address as they are: mapped, TMA-legal, host/device address
     // arithmetic interchangeable (the alias of the first element is what the tensor maps are built on)
     static const int direct_env = [] { const char* e = std::getenv("HCLOOC_DIRECT"); return e ? std::atoi(e) : -1; }();
     const int direct_mode = ctx->direct_mode >= 0 ? ctx->direct_mode : direct_env;
-    const bool direct_ok = !in_core && !c_dev && !transa && !transb && aligned && direct_mode != 0 && M <= 0x7fffffffLL && N <= 0x7fffffffLL && K <= 0x7fffffffLL &&
+    const bool direct_ok = !in_core && !c_dev && aligned && direct_mode != 0 && M <= 0x7fffffffLL && N <= 0x7fffffffLL && K <= 0x7fffffffLL &&
                            C_alias && (((uintptr_t)C_alias & 15u) == 0) &&
                            (scale_only || (A_alias && B_alias && ((((uintptr_t)A_alias | (uintptr_t)B_alias) & 15u) == 0)));
     {
@@ -452,10 +419,8 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
                 k.where == key.where && k.budget == key.budget) { P = kv.second; hit = true; break; }
         }
         if (!hit) {
-            rc = hclooc_plan_ex(M, N, K, key.beta_nz, key.alpha_zero, budget, where, &P);
+            rc = plan_impl(M, N, K, key.beta_nz, key.alpha_zero, budget, where, transa, transb, &P);
             if (rc) return rc;
-            P.bytes_transpose_staging = stage_bytes * (uint64_t)((transa ? 1 : 0) + (transb ? 1 : 0));
-            P.workspace_bytes += P.bytes_transpose_staging;
             if (ctx->plan_cache.size() >= 16) ctx->plan_cache.erase(ctx->plan_cache.begin());
             ctx->plan_cache.emplace_back(key, P);
         }
@@ -465,7 +430,8 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
         if (P.direct) { A = (const double*)A_alias; B = (const double*)B_alias; C = (double*)C_alias; }
         // direct: one CTA per tile (every tile is bound by its own reads over the link; the persistent kernel's
         // device scratch would also break the promise that the call uses no device memory)
-        rc = launch_dgemm_tiles(M, N, scale_only ? 0 : K, scale_only ? 0.0 : alpha, A, lda, B, ldb, beta, C, ldc, ctx->s_compute[0], P.direct ? 1 : -1);
+        rc = launch_dgemm_tiles(M, N, scale_only ? 0 : K, scale_only ? 0.0 : alpha, A, lda, B, ldb, beta, C, ldc, ctx->s_compute[0], P.direct ? 1 : -1,
+                                nullptr, transa, transb);
         const auto t1 = std::chrono::steady_clock::now();
         cudaError_t e = cudaStreamSynchronize(ctx->s_compute[0]);
         if (rc) return rc;
@@ -497,7 +463,6 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
     }
     std::vector<double*> bufs(P.n_abuf + P.n_sets + P.n_bbuf);
     uint8_t* scratch[MAX_COMPUTE_STREAMS] = {};
-    double *stage_a = nullptr, *stage_b = nullptr;
     if (P.n_scratch > MAX_COMPUTE_STREAMS) return HCLOOC_ERR_INTERNAL;
     {
         uint8_t* q = base;
@@ -505,8 +470,6 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
         for (int a = 0; a < P.n_abuf; ++a) { bufs[a] = (double*)q; q += P.bytes_a_buf; }
         for (int c = 0; c < P.n_sets; ++c) { bufs[P.n_abuf + c] = (double*)q; q += P.bytes_c_buf; }
         for (int i = 0; i < P.n_scratch; ++i) { scratch[i] = q; q += P.bytes_scratch; }
-        if (transa) { stage_a = (double*)q; q += stage_bytes; }
-        if (transb) { stage_b = (double*)q; q += stage_bytes; }
         if ((size_t)(q - base) != P.workspace_bytes) return HCLOOC_ERR_INTERNAL;
     }
     // ---------------------------------------------------------------- events
@@ -522,7 +485,6 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
         HCL_CUDA(cudaMemsetAsync(scratch[i] + streamk_counter_offset(), 0, streamk_counter_bytes(), ctx->s_compute[i]));
     auto stream_of = [&](int s) { return s == 0 ? ctx->s_h2d : (s == 1 ? ctx->s_d2h : ctx->s_compute[s - 2]); };
     uint64_t bytes_h2d = 0, bytes_d2h = 0, n_h2d = 0, n_d2h = 0, n_kernels = 0;
-    uint64_t n_h2d_blocks = 0, n_trans_ops = 0;   // copies (= transpose kernels) issued for the slices of transposed operands
     const auto t_enq0 = std::chrono::steady_clock::now();
     rc = HCLOOC_OK;
     const bool trace = ctx->trace;
@@ -593,13 +555,24 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
                 break;
             }
             case HCLOOC_OP_H2D_A:
-                if (transa) { rc = upload_transposed(bufs[o.buf], P.lda_dev, A, lda, o.r0, o.nr, o.c0, o.nc, stage_a, stage_bytes, st, &n_h2d_blocks); ++n_trans_ops; }
+                // A^T: the slice op(A)[r0.., c0..] is the stored block A[c0.., r0..] (k rows x m columns) and stays that way
+                if (transa) rc = copy2d(bufs[o.buf], (size_t)P.lda_dev * 8, A + o.c0 * lda + o.r0, (size_t)lda * 8, (size_t)o.nr * 8, (size_t)o.nc, st);
                 else rc = copy2d(bufs[o.buf], (size_t)P.lda_dev * 8, A + o.r0 * lda + o.c0, (size_t)lda * 8, (size_t)o.nc * 8, (size_t)o.nr, st);
                 bytes_h2d += (uint64_t)o.nr * o.nc * 8; ++n_h2d;
                 break;
             case HCLOOC_OP_H2D_B:
-                if (transb) { rc = upload_transposed(bufs[o.buf] + o.dev_r0 * P.ldb_dev, P.ldb_dev, B, ldb, o.r0, o.nr, o.c0, o.nc, stage_b, stage_bytes, st, &n_h2d_blocks); ++n_trans_ops; }
-                else rc = copy2d(bufs[o.buf] + o.dev_r0 * P.ldb_dev, (size_t)P.ldb_dev * 8, B + o.r0 * ldb + o.c0, (size_t)ldb * 8, (size_t)o.nc * 8, (size_t)o.nr, st);
+                if (transb) {
+                    // B^T: the slice is the stored block B[c0.., k0..] (n rows x k columns).  The schedule cuts a prefetched
+                    // slice into chunks of k rows [dev_r0, dev_r0 + nr) of kk; for the stored layout those would be narrow
+                    // column strips, so the same chunk takes the matching share of the n rows instead (whole k rows of B^T:
+                    // contiguous runs); the chunks of a slice still tile it exactly, and b_ready follows the last one.
+                    const int64_t k0 = o.r0 - o.dev_r0, kk = std::min(P.kb, K - k0);
+                    const int64_t n_lo = o.nc * o.dev_r0 / kk, n_hi = o.nc * (o.dev_r0 + o.nr) / kk;
+                    rc = copy2d(bufs[o.buf] + n_lo * P.ldb_dev, (size_t)P.ldb_dev * 8, B + (o.c0 + n_lo) * ldb + k0, (size_t)ldb * 8, (size_t)kk * 8, (size_t)(n_hi - n_lo), st);
+                    bytes_h2d += (uint64_t)(n_hi - n_lo) * kk * 8; ++n_h2d;
+                    break;
+                }
+                rc = copy2d(bufs[o.buf] + o.dev_r0 * P.ldb_dev, (size_t)P.ldb_dev * 8, B + o.r0 * ldb + o.c0, (size_t)ldb * 8, (size_t)o.nc * 8, (size_t)o.nr, st);
                 bytes_h2d += (uint64_t)o.nr * o.nc * 8; ++n_h2d;
                 break;
             case HCLOOC_OP_H2D_C:
@@ -616,7 +589,7 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
                 const double b_eff = (o.beta < 0.0) ? beta : o.beta;
                 rc = launch_dgemm_tiles(o.nr, o.nc, o.kk, scale_only ? 0.0 : alpha, o.buf >= 0 ? bufs[o.buf] : nullptr, P.lda_dev,
                                         o.buf2 >= 0 ? bufs[o.buf2] : nullptr, P.ldb_dev, b_eff, bufs[o.buf3], P.ldc_dev, st,
-                                        P.ksplit != 0 ? P.ksplit : 1, P.ksplit < 0 ? scratch[o.stream - 2] : nullptr);
+                                        P.ksplit != 0 ? P.ksplit : 1, P.ksplit < 0 ? scratch[o.stream - 2] : nullptr, transa, transb);
                 ++n_kernels;
                 break;
             }
@@ -682,7 +655,7 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
     if (stats) {
         stats->plan = P;
         stats->bytes_h2d = bytes_h2d; stats->bytes_d2h = bytes_d2h;
-        stats->n_kernels = n_kernels + n_h2d_blocks; stats->n_copies_h2d = n_h2d - n_trans_ops + n_h2d_blocks; stats->n_copies_d2h = n_d2h;
+        stats->n_kernels = n_kernels; stats->n_copies_h2d = n_h2d; stats->n_copies_d2h = n_d2h;
         stats->t_enqueue_s = std::chrono::duration<double>(t_enq1 - t_enq0).count();
         stats->t_total_s = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_begin).count();
     }

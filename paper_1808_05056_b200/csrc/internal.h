@@ -36,8 +36,9 @@ const MachineModel& machine_model();
 int launch_dgemm_tiles(int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda,
                        const double* dB, int64_t ldb, double beta, double* dC, int64_t ldc,
                        cudaStream_t stream, int ksplit,    // ksplit: 1, 2, 4; 0 = choose from the tile count;
-                       void* streamk_scratch = nullptr);   // -1 = the launch has the GPU to itself: persistent stream-K
+                       void* streamk_scratch = nullptr,    // -1 = the launch has the GPU to itself: persistent stream-K
                                                            //      (scratch: streamk_scratch_bytes(), or NULL = library pool)
+                       int transa = 0, int transb = 0);    // dA is stored K x M / dB is stored N x K (hclooc_dgemm_t)
 
 // The persistent stream-K kernel (dgemm_streamk_sm100.cu).  Returns 1 if it does not apply (no scratch buffer
 // free, shape out of range): the caller then launches one CTA per tile.
@@ -75,8 +76,9 @@ inline int64_t early_uploads(int64_t h, int n_sets, int n_abuf) {
     return pre < 0 ? 0 : pre;
 }
 
-// dst[c*ldd + r] = src[r*lds + c] on device pointers (transpose_sm100.cu): the staging step of hclooc_dgemm_t
-int launch_transpose(const double* src, int64_t rows, int64_t cols, int64_t lds, double* dst, int64_t ldd, cudaStream_t stream);
+// hclooc_plan_ex with the operand layouts of hclooc_dgemm_t (planner.cpp)
+int plan_impl(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zero, size_t device_budget_bytes,
+              int operands_on_device, int transa, int transb, hclooc_plan_t* out);
 
 // number of CTAs the tile kernel uses for an M x N output (for stats / tests)
 int64_t dgemm_tile_count(int64_t M, int64_t N);

@@ -54,6 +54,7 @@ namespace {
 struct Cand {
     int64_t mb, nb, kb, h, w, kpanels;
     int n_sets, n_abuf, n_bbuf, ksplit, n_scratch;
+    bool ta;              // A is stored K x M: its slices are uploaded as kb rows of mb doubles (narrow rows when mb is small)
     bool c_dev;           // C lives in device memory: its block copies are device-to-device, not host-link traffic
     int64_t lda_dev, ldb_dev, ldc_dev;
     uint64_t a_bytes, b_bytes, c_bytes, ws_bytes;
@@ -152,7 +153,14 @@ void cost(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool scale_onl
     c.t_flop = flops / mm.fp64_flops;
     const double t_in = c.bytes_h2d / mm.h2d_Bps + c.n_h2d * mm.copy_latency_s;
     const double t_out = c.bytes_d2h / mm.d2h_Bps + c.n_d2h * mm.copy_latency_s;
-    c.t_link = std::max(std::max(t_in, t_out), (double)(c.bytes_h2d + c.bytes_d2h) / mm.duplex_Bps);
+    double t_in_rows = 0.0;
+    if (c.ta && !scale_only && c.mb * 8 < 1024) {
+        // 2-D copies run at full rate only from ~1 KiB per row up (measured: 8.3 GB/s at 128 B, 53 at 1 KiB): the slices
+        // of a transposed A have rows of mb doubles
+        const double a_bytes_all = (double)c.bytes_h2d - 8.0 * (double)K * (double)N - ((beta_nz || c.kpanels > 1) && !c.c_dev ? 8.0 * (double)M * (double)N * (beta_nz ? c.kpanels : c.kpanels - 1) : 0.0);
+        t_in_rows = std::max(0.0, a_bytes_all) / mm.h2d_Bps * (1024.0 / (double)(c.mb * 8) - 1.0);
+    }
+    c.t_link = std::max(std::max(t_in + t_in_rows, t_out), (double)(c.bytes_h2d + c.bytes_d2h) / mm.duplex_Bps + t_in_rows);
     const bool link_bound = c.t_link > c.t_flop / std::max(1e-3, pad_eff);
     const double steps_in_flight = link_bound ? 1.0 : (double)std::max(1, c.n_sets - 2);
     c.ksplit = scale_only ? 1 : (force_ks ? force_ks : dgemm_auto_ksplit((int64_t)(steps_in_flight * tiles_step), c.kb));
@@ -232,6 +240,13 @@ extern "C" int hclooc_plan(int64_t M, int64_t N, int64_t K, int beta_nonzero, in
 
 extern "C" int hclooc_plan_ex(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zero,
                               size_t device_budget_bytes, int operands_on_device, hclooc_plan_t* out) {
+    return plan_impl(M, N, K, beta_nonzero, alpha_zero, device_budget_bytes, operands_on_device, 0, 0, out);
+}
+
+// transa / transb (hclooc_dgemm_t): the device slices keep the layout the operand is stored in -- an A slice is kb x mb
+// (leading dimension lda_dev >= mb), a B slice nb x kb (ldb_dev >= kb) -- which only changes the buffer sizes here.
+int hclooc::plan_impl(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zero, size_t device_budget_bytes,
+                      int operands_on_device, int transa, int transb, hclooc_plan_t* out) {
     const MachineModel& mm = machine_model();
     const bool c_dev = operands_on_device == 2;
     const bool direct_ok = operands_on_device == 3 || operands_on_device == 4, direct_forced = operands_on_device == 4;
@@ -245,6 +260,8 @@ extern "C" int hclooc_plan_ex(int64_t M, int64_t N, int64_t K, int beta_nonzero,
     out->beta_nonzero = beta_nonzero ? 1 : 0;
     const bool scale_only = (alpha_zero != 0) || (K == 0);
     out->scale_only = scale_only ? 1 : 0;
+    if (scale_only) transa = transb = 0;
+    out->trans = (transa ? 1 : 0) | (transb ? 2 : 0);
     if (M == 0 || N == 0) return HCLOOC_OK;                       // nothing to do: zero steps
     if (operands_on_device) {
         // the in-core case (the switch to out-of-core happens only when the matrices do not
@@ -281,9 +298,10 @@ extern "C" int hclooc_plan_ex(int64_t M, int64_t N, int64_t K, int beta_nonzero,
             last_nb = nb;
             if (force_nb && nb != std::min(N, round_up(force_nb, 16))) continue;
             const int64_t weff = ceil_div(N, nb);
-            const int64_t lda_dev = round_up(std::max<int64_t>(kb, 1), LD_ALIGN);
-            const int64_t ldb_dev = round_up(nb, LD_ALIGN), ldc_dev = ldb_dev;
-            const uint64_t b_bytes = scale_only ? 0 : round_up((uint64_t)kb * ldb_dev * 8, BUF_ALIGN);
+            const int64_t lda_dev = round_up(std::max<int64_t>(kb, 1), LD_ALIGN);      // A as stored M x K; A^T: set per candidate
+            const int64_t ldc_dev = round_up(nb, LD_ALIGN);
+            const int64_t ldb_dev = transb ? round_up(std::max<int64_t>(kb, 1), LD_ALIGN) : ldc_dev;
+            const uint64_t b_bytes = scale_only ? 0 : round_up((uint64_t)(transb ? nb : kb) * ldb_dev * 8, BUF_ALIGN);
             for (int n_bbuf = 1; n_bbuf <= (scale_only || weff * kp == 1 ? 1 : 2); ++n_bbuf) {
                 if ((uint64_t)n_bbuf * b_bytes >= S) continue;
                 if (force_bbuf && n_bbuf != force_bbuf && !(scale_only || weff * kp == 1)) continue;
@@ -299,7 +317,7 @@ extern "C" int hclooc_plan_ex(int64_t M, int64_t N, int64_t K, int beta_nonzero,
                     int64_t tried[6];
                     int nt = 0;
                     int64_t top = std::min(M, rows_max);
-                    if (top >= TILE) top = top / TILE * TILE; else if (top >= 8) top = top / 8 * 8;
+                    if (top >= TILE) top = top / TILE * TILE; else if (top >= 16 && transa) top = top / 16 * 16; else if (top >= 8) top = top / 8 * 8;
                     tried[nt++] = top;
                     for (int64_t cand_mb : {(int64_t)1024, (int64_t)512, (int64_t)256, (int64_t)128})
                         if (cand_mb < top) tried[nt++] = cand_mb;
@@ -307,12 +325,14 @@ extern "C" int hclooc_plan_ex(int64_t M, int64_t N, int64_t K, int beta_nonzero,
                     for (int q = 0; q < nt; ++q) {
                         Cand c{};
                         c.c_dev = c_dev;
+                        c.ta = transa != 0;
                         c.mb = tried[q]; c.nb = nb; c.kb = kb; c.kpanels = kp;
                         c.h = ceil_div(M, c.mb); c.w = weff;
                         c.n_sets = (int)std::min<int64_t>(n_sets, std::max<int64_t>(2, c.h * c.w * kp));
                         c.n_bbuf = n_bbuf;
-                        c.lda_dev = scale_only ? 0 : lda_dev; c.ldb_dev = scale_only ? 0 : ldb_dev; c.ldc_dev = ldc_dev;
-                        c.a_bytes = scale_only ? 0 : round_up((uint64_t)c.mb * lda_dev * 8, BUF_ALIGN);
+                        c.lda_dev = scale_only ? 0 : (transa ? round_up(c.mb, LD_ALIGN) : lda_dev);
+                        c.ldb_dev = scale_only ? 0 : ldb_dev; c.ldc_dev = ldc_dev;
+                        c.a_bytes = scale_only ? 0 : round_up((uint64_t)(transa ? kb * c.lda_dev : c.mb * lda_dev) * 8, BUF_ALIGN);
                         c.b_bytes = b_bytes;
                         c.c_bytes = round_up((uint64_t)c.mb * ldc_dev * 8, BUF_ALIGN);
                         c.n_abuf = scale_only ? 0 : c.n_sets;
@@ -379,6 +399,14 @@ extern "C" int hclooc_plan_ex(int64_t M, int64_t N, int64_t K, int beta_nonzero,
     out->flops = scale_only ? 0.0 : 2.0 * (double)M * (double)N * (double)K;
     out->t_flop_s = best.t_flop; out->t_link_s = best.t_link; out->t_model_s = best.t_model;
     return HCLOOC_OK;
+}
+
+extern "C" int hclooc_plan_trans(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zero, size_t device_budget_bytes,
+                                 int operands_on_device, int transa, int transb, hclooc_plan_t* out) {
+    if (transa != HCL_OP_N && transa != HCL_OP_T) return -8;
+    if (transb != HCL_OP_N && transb != HCL_OP_T) return -9;
+    if (!out) return -10;
+    return plan_impl(M, N, K, beta_nonzero, alpha_zero, device_budget_bytes, operands_on_device, transa, transb, out);
 }
 
 // The paper's rule, by divisor enumeration (example :301 -> (h, w) = (4, 2)).

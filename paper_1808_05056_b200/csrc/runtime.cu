@@ -118,6 +118,31 @@ int hclDgemmAsyncEx(int64_t M, int64_t N, int64_t K, double alpha, const double*
     }
     return finish_async((cudaStream_t)s, ev);
 }
+int hclDgemmAsyncT(int transa, int transb, int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda,
+                   const double* dB, int64_t ldb, double beta, double* dC, int64_t ldc, hclStream s, hclEvent* ev, int variant) {
+    if (transa != HCL_OP_N && transa != HCL_OP_T) return -15;
+    if (transb != HCL_OP_N && transb != HCL_OP_T) return -16;
+    if (!transa && !transb) return hclDgemmAsyncEx(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, s, ev, variant);
+    if (M < 0) return -1;
+    if (N < 0) return -2;
+    if (K < 0) return -3;
+    if (variant != HCL_DGEMM_AUTO && variant != 1 && variant != 2 && variant != 4) return -14;
+    const bool noab = (alpha == 0.0 || K == 0);
+    if (M > 0 && N > 0) {
+        if (!noab) {
+            if (!dA) return -5;
+            if (lda < (transa ? M : K)) return -6;
+            if (!dB) return -7;
+            if (ldb < (transb ? K : N)) return -8;
+            if (((uintptr_t)dA & 15u) || ((uintptr_t)dB & 15u) || (lda & 1) || (ldb & 1)) return HCLOOC_ERR_ALIGN;
+        }
+        if (!dC) return -10;
+        if (ldc < N) return -11;
+        int rc = launch_dgemm_tiles(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, (cudaStream_t)s, variant, nullptr, transa, transb);
+        if (rc) return rc;
+    }
+    return finish_async((cudaStream_t)s, ev);
+}
 int hclDgemmAsync(int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda, const double* dB, int64_t ldb,
                   double beta, double* dC, int64_t ldc, hclStream s, hclEvent* ev) {
     return hclDgemmAsyncEx(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, s, ev, HCL_DGEMM_AUTO);

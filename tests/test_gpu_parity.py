@@ -650,8 +650,8 @@ def test_transposed_operands_match_oracle(H, transa, transb, M, N, K, alpha, bet
     ref = np.zeros((M, N)) if beta == 0.0 else C.view.copy()
     D = oracle.dgemm(alpha, opA, opB, beta, ref, want_denominator=True)
     st = H.hclooc_dgemm_t(None, transa, transb, M, N, K, alpha, A, A.ld, B, B.ld, beta, C, C.ld, budget)
-    assert st.plan.direct == 0 and st.plan.workspace_bytes <= budget
-    assert st.plan.bytes_transpose_staging > 0 and st.plan.bytes_transpose_staging % (transa + transb) == 0
+    assert st.plan.direct == 0 and 0 < st.plan.workspace_bytes <= budget
+    assert st.plan.trans == transa + 2 * transb
     assert st.bytes_h2d == st.plan.bytes_h2d and st.bytes_d2h == st.plan.bytes_d2h
     check(C.view, ref, D, exact=(dist == "int"))
     assert np.isnan(C.array[:, N:]).all()
@@ -672,7 +672,7 @@ def test_transposed_call_equals_plain_call_on_written_out_transposes(H):
     # HCL_OP_N, HCL_OP_N through the same entry point is hclooc_dgemm_ex
     C3 = H.HostMatrix(M, N); synthgen.fill(C3.array, 47, "C", "uniform", cols=N)
     st3 = H.hclooc_dgemm_t(None, 0, 0, M, N, K, -0.75, opA, opA.ld, opB, opB.ld, 1.25, C3, C3.ld, 4 * MiB)
-    assert st3.plan.bytes_transpose_staging == 0
+    assert st3.plan.trans == 0
     assert np.array_equal(C3.view.view(np.uint64), C2.view.view(np.uint64))
 
 
@@ -687,7 +687,70 @@ def test_transposed_argument_errors(H):
         with pytest.raises(H.HclError) as e:
             H.hclooc_dgemm_t(None, *args, 1 * MiB)
         assert e.value.status == want, (args[:2], e.value.status)
-    with pytest.raises(H.HclError) as e:
-        H.hclooc_dgemm_t(None, 1, 1, M, N, K, 1.0, A, M, B, K, 1.0, C, N, 100 * 1024)   # staging alone exceeds the budget
-    assert e.value.status == 1
     assert np.array_equal(C.view, before)
+
+
+@pytest.mark.parametrize("transa,transb", [(1, 0), (0, 1), (1, 1)])
+@pytest.mark.parametrize("M,N,K,alpha,beta,dist,variant", [
+    (128, 128, 32, 1.0, 0.0, "uniform", 1),          # one tile, one k block
+    (300, 260, 200, 1.0, 0.5, "uniform", 1),         # ragged in m, n and k
+    (129, 257, 33, -1.5, 1.0, "normal", 1),
+    (131, 77, 97, 3.0, 2.0, "int", 1),
+    (517, 389, 1000, 2.0, -1.0, "int", 0),
+    (128, 256, 4096, 1.0, 0.5, "uniform", 4),        # cluster split-K over the transposed layouts
+    (200, 300, 2061, -1.0, 2.0, "int", 2),
+    (1500, 1400, 300, 1.0, 0.5, "int", 0),           # 132 tiles
+])
+def test_tile_kernel_transposed_layouts(H, transa, transb, M, N, K, alpha, beta, dist, variant):
+    """hclDgemmAsyncT on device pointers: A stored K x M and / or B stored N x K, read by the kernel as they are."""
+    import torch
+    ar, ac = (K, M) if transa else (M, K)
+    br, bc = (N, K) if transb else (K, N)
+    lda, ldb, ldc = ac + (ac % 2) + 4, bc + (bc % 2) + 2, N + (N % 2) + 6
+    A = np.full((ar, lda), np.nan); B = np.full((br, ldb), np.nan); C0 = np.full((M, ldc), np.nan)
+    synthgen.fill(A, 51, "A", dist, cols=ac); synthgen.fill(B, 51, "B", dist, cols=bc); synthgen.fill(C0, 51, "C", dist, cols=N)
+    if beta == 0.0:
+        C0[:, :N] = np.nan
+    dA, dB, dC = (torch.from_numpy(x).cuda() for x in (A, B, C0))
+    H.hclDgemmAsyncT(transa, transb, M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, torch.cuda.current_stream(), variant=variant)
+    torch.cuda.synchronize()
+    got = dC.cpu().numpy()
+    opA, opB = np.empty((M, K)), np.empty((K, N))
+    opA[...] = A[:, :ac].T if transa else A[:, :ac]
+    opB[...] = B[:, :bc].T if transb else B[:, :bc]
+    ref = C0[:, :N].copy()
+    D = oracle.dgemm(alpha, opA, opB, beta, ref, want_denominator=True)
+    check(got[:, :N], ref, D, exact=(dist == "int"))
+    assert np.isnan(got[:, N:]).all()
+    if variant in (0, 1) and K < 1024:
+        # the same bits as the untransposed kernel on written-out transposes (same order of summation)
+        pa, pb = np.zeros((M, K + K % 2)), np.zeros((K, N + N % 2))                  # even leading dimensions
+        pa[:, :K] = opA; pb[:, :N] = opB
+        dA2, dB2, dC2 = torch.from_numpy(pa).cuda(), torch.from_numpy(pb).cuda(), torch.from_numpy(C0).cuda()
+        H.hclDgemmAsyncEx(M, N, K, alpha, dA2, K + K % 2, dB2, N + N % 2, beta, dC2, ldc, torch.cuda.current_stream(), variant=1)
+        torch.cuda.synchronize()
+        assert np.array_equal(dC2.cpu().numpy()[:, :N].view(np.uint64), got[:, :N].view(np.uint64))
+    with pytest.raises(H.HclError) as e:
+        H.hclDgemmAsyncT(transa, 2, M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, torch.cuda.current_stream())
+    assert e.value.status == -16
+
+
+def test_transposed_in_core_and_direct_modes(H):
+    """Device-resident transposed operands run in core (one launch, nothing staged); mapped host operands in direct mode."""
+    import torch
+    M, N, K = 700, 520, 384
+    A, B, C = stored_inputs(H, 1, 1, M, N, K, 52, "int")
+    ref = C.view.copy()
+    oracle.dgemm(1.0, A.view.T.copy(), B.view.T.copy(), 0.5, ref)
+    dA, dB, dC = (torch.from_numpy(X.view.copy()).cuda() for X in (A, B, C))
+    st = H.hclooc_dgemm_t(None, 1, 1, M, N, K, 1.0, dA, M, dB, K, 0.5, dC, N, 0)
+    assert st.plan.n_steps == 1 and st.plan.workspace_bytes == 0 and st.bytes_h2d == 0
+    assert np.array_equal(dC.cpu().numpy(), ref)
+    ctx = H.hclooc_ctx_create(0)
+    try:
+        H.hclooc_ctx_set_direct(ctx, 1)
+        st = H.hclooc_dgemm_t(ctx, 1, 1, M, N, K, 1.0, A, A.ld, B, B.ld, 0.5, C, C.ld, 1 * MiB)
+        assert st.plan.direct == 1 and st.plan.trans == 3 and st.plan.workspace_bytes == 0
+        assert np.array_equal(C.view, ref)
+    finally:
+        H.hclooc_ctx_destroy(ctx)

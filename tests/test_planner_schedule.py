@@ -393,3 +393,29 @@ def test_direct_mode_is_chosen_only_where_copy_latency_dominates():
     # a budget too small for any staged plan is no obstacle: direct mode needs none
     tiny = H.hclooc_plan_ex(300, 300, 300, 1, 0, 4096, 3)
     assert tiny.direct == 1
+
+
+def test_plans_for_transposed_operands_keep_the_stored_layout():
+    """hclooc_plan_trans: an A slice of a transposed A is kb x mb (lda_dev >= mb), a B slice of a transposed B is nb x kb
+    (ldb_dev >= kb); everything still fits the budget and the traffic is that of the untransposed plan."""
+    MiB = 1 << 20
+    for (M, N, K, budget) in ((512, 512, 512, 1 * MiB), (8192, 8192, 8192, 256 * MiB), (3000, 5000, 7000, 64 * MiB), (96, 112, 20000, 900 * 1024)):
+        base = H.hclooc_plan_trans(M, N, K, 1, 0, budget, 0, 0, 0)
+        same = H.hclooc_plan_ex(M, N, K, 1, 0, budget, 0)
+        assert bytes(base) == bytes(same)
+        for ta, tb in ((1, 0), (0, 1), (1, 1)):
+            p = H.hclooc_plan_trans(M, N, K, 1, 0, budget, 0, ta, tb)
+            assert p.trans == ta + 2 * tb and p.workspace_bytes <= budget
+            assert p.workspace_bytes == p.n_bbuf * p.bytes_b_buf + p.n_abuf * p.bytes_a_buf + p.n_sets * p.bytes_c_buf
+            if ta:
+                assert p.lda_dev >= p.mb and p.lda_dev % 16 == 0 and p.bytes_a_buf >= 8 * p.kb * p.lda_dev
+            else:
+                assert p.lda_dev >= p.kb and p.bytes_a_buf >= 8 * p.mb * p.lda_dev
+            if tb:
+                assert p.ldb_dev >= p.kb and p.ldb_dev % 16 == 0 and p.bytes_b_buf >= 8 * p.nb * p.ldb_dev
+            else:
+                assert p.ldb_dev >= p.nb and p.bytes_b_buf >= 8 * p.kb * p.ldb_dev
+            assert p.bytes_d2h == 8 * M * N * p.kpanels and p.n_steps == p.h * p.w * p.kpanels
+    with pytest.raises(H.HclError) as e:
+        H.hclooc_plan_trans(8, 8, 8, 1, 0, 1 * MiB, 0, 2, 0)
+    assert e.value.status == -8
