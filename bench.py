@@ -225,6 +225,8 @@ def run_ours(args, wl, name):
         return ms / steps, (st, ci95_rel(list(per_call)), 1e3 * float(np.mean(per_call)), 1e3 * float(np.min(per_call)))
 
     def resident():
+        if ta or tb:
+            return H.hclooc_dgemm_t(ctx, ta, tb, M, N, K, alpha, dA, M if ta else K, dB, K if tb else N, beta, dC, N, budget)
         return H.hclooc_dgemm_ex(ctx, M, N, K, alpha, dA, K, dB, N, beta, dC, N, budget)
 
     ta, tb = int(args.trans[0] == "T"), int(args.trans[1] == "T")
@@ -248,7 +250,10 @@ def run_ours(args, wl, name):
         for it in range(max(args.warmup, 3) + args.steps):
             k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             k0.record(cur)
-            H.hclDgemmAsync(M, nb, K, alpha, dA, K, dB, N, beta, dC, N, cur)
+            if ta or tb:
+                H.hclDgemmAsyncT(ta, tb, M, nb, K, alpha, dA, M if ta else K, dB, K if tb else N, beta, dC, N, cur)
+            else:
+                H.hclDgemmAsync(M, nb, K, alpha, dA, K, dB, N, beta, dC, N, cur)
             k1.record(cur)
             k1.synchronize()
             if it >= max(args.warmup, 3):
@@ -259,7 +264,7 @@ def run_ours(args, wl, name):
         for it in range(max(args.warmup, 3) + max(args.steps, 10)):
             k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             k0.record(cur)
-            H.hclDgemmAsyncEx(mb, nb, K, alpha, dA, K, dB, N, beta, dC, N, cur, variant=max(1, plan.ksplit))
+            H.hclDgemmAsyncT(ta, tb, mb, nb, K, alpha, dA, M if ta else K, dB, K if tb else N, beta, dC, N, cur, variant=max(1, plan.ksplit))
             k1.record(cur)
             k1.synchronize()
             if it >= max(args.warmup, 3):
@@ -300,7 +305,7 @@ def run_ours(args, wl, name):
         "clocks": clocks,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
                      "frac": achieved / FP64_PEAK_TFLOPS, "traffic": ncu_traffic(f"{M}x{nb}x{K}"),
-                     "kernel": "hclooc_dgemm_streamk_kernel" if -(-M // 128) * -(-nb // 128) >= 148 else "hclooc_dgemm_tile_kernel",
+                     "kernel": "hclooc_dgemm_streamk_kernel" if -(-M // 128) * -(-nb // 128) >= 148 and not (ta or tb) else "hclooc_dgemm_tile_kernel",
                      "launch": f"{M}x{nb}x{K} (one B slice of the plan, all rows)", "ms_per_launch": ms_kernel,
                      "peak_source": "derived 148 SM x 128 FP64 flop/clk x 1.965 GHz; DMMA microbenchmark measured 37.17",
                      "pipeline_step": {"kernel": f"hclooc_dgemm_tile_kernel<{max(1, plan.ksplit)}>", "launch": f"{mb}x{nb}x{K}",

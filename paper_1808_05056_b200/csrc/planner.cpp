@@ -154,11 +154,13 @@ void cost(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool scale_onl
     const double t_in = c.bytes_h2d / mm.h2d_Bps + c.n_h2d * mm.copy_latency_s;
     const double t_out = c.bytes_d2h / mm.d2h_Bps + c.n_d2h * mm.copy_latency_s;
     double t_in_rows = 0.0;
-    if (c.ta && !scale_only && c.mb * 8 < 1024) {
-        // 2-D copies run at full rate only from ~1 KiB per row up (measured: 8.3 GB/s at 128 B, 53 at 1 KiB): the slices
-        // of a transposed A have rows of mb doubles
+    const double a_row_factor = (c.ta && !scale_only && c.mb * 8 < 2048) ? 1.0 + 0.45 * (2048.0 / (double)(c.mb * 8) - 1.0) : 1.0;
+    if (c.ta && !scale_only && c.mb * 8 < 2048) {
+        // 2-D copies run at full rate only from ~2 KiB per row up, and the slices of a transposed A have rows of mb
+        // doubles.  Measured on config 2 with A^T: 1 KiB rows (mb = 128) move at ~35 GB/s inside the pipeline, 2 KiB rows
+        // within 1.3 % of the untransposed call; alone, 128-byte rows reach 8.3 GB/s (profiles/r01_box_probe.md).
         const double a_bytes_all = (double)c.bytes_h2d - 8.0 * (double)K * (double)N - ((beta_nz || c.kpanels > 1) && !c.c_dev ? 8.0 * (double)M * (double)N * (beta_nz ? c.kpanels : c.kpanels - 1) : 0.0);
-        t_in_rows = std::max(0.0, a_bytes_all) / mm.h2d_Bps * (1024.0 / (double)(c.mb * 8) - 1.0);
+        t_in_rows = std::max(0.0, a_bytes_all) / mm.h2d_Bps * 0.45 * (2048.0 / (double)(c.mb * 8) - 1.0);
     }
     c.t_link = std::max(std::max(t_in + t_in_rows, t_out), (double)(c.bytes_h2d + c.bytes_d2h) / mm.duplex_Bps + t_in_rows);
     const bool link_bound = c.t_link > c.t_flop / std::max(1e-3, pad_eff);
@@ -197,7 +199,7 @@ void cost(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool scale_onl
     const double a_later = n_cols > c.kpanels ? std::max(0.0, a_all - a_first * c.kpanels) / (n_cols - c.kpanels) : 0.0;
     const double c_col = c.c_dev ? 0.0 : 8.0 * (double)M * (double)c.nb;
     auto link_col = [&](double a_bytes) {
-        const double up = a_bytes + (scale_only ? 0.0 : (double)c.b_bytes) + (cload ? c_col : 0.0);
+        const double up = a_bytes * a_row_factor + (scale_only ? 0.0 : (double)c.b_bytes) + (cload ? c_col : 0.0);
         const double lat = (double)c.h * 2.0 * mm.copy_latency_s;
         return std::max(std::max(up / mm.h2d_Bps, c_col / mm.d2h_Bps), (up + c_col) / mm.duplex_Bps) + lat;
     };
