@@ -305,7 +305,7 @@ def run_ours(args, wl, name):
         "clocks": clocks,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
                      "frac": achieved / FP64_PEAK_TFLOPS, "traffic": ncu_traffic(f"{M}x{nb}x{K}"),
-                     "kernel": "hclooc_dgemm_streamk_kernel" if -(-M // 128) * -(-nb // 128) >= 148 and not (ta or tb) else "hclooc_dgemm_tile_kernel",
+                     "kernel": "hclooc_dgemm_streamk_kernel" if -(-M // 128) * -(-nb // 128) >= 148 else "hclooc_dgemm_tile_kernel",
                      "launch": f"{M}x{nb}x{K} (one B slice of the plan, all rows)", "ms_per_launch": ms_kernel,
                      "peak_source": "derived 148 SM x 128 FP64 flop/clk x 1.965 GHz; DMMA microbenchmark measured 37.17",
                      "pipeline_step": {"kernel": f"hclooc_dgemm_tile_kernel<{max(1, plan.ksplit)}>", "launch": f"{mb}x{nb}x{K}",

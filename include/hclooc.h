@@ -289,8 +289,8 @@ int hclDgemmAsyncEx(int64_t M, int64_t N, int64_t K, double alpha, const double*
                     const double* dB, int64_t ldb, double beta, double* dC, int64_t ldc,
                     hclStream s, hclEvent* ev, int variant);
 /* Same on transposed device operands: dC = alpha*op(dA)*op(dB) + beta*dC with dA stored K x M when transa = HCL_OP_T
- * (lda >= M) and dB stored N x K when transb = HCL_OP_T (ldb >= K).  variant: HCL_DGEMM_AUTO, 1, 2 or 4 (the persistent
- * stream-K kernel exists for untransposed operands only).  -15 / -16: transa / transb invalid.                     */
+ * (lda >= M) and dB stored N x K when transb = HCL_OP_T (ldb >= K).  variant as hclDgemmAsyncEx.
+ * -15 / -16: transa / transb invalid.                                                                              */
 int hclDgemmAsyncT(int transa, int transb, int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda,
                    const double* dB, int64_t ldb, double beta, double* dC, int64_t ldc,
                    hclStream s, hclEvent* ev, int variant);

@@ -296,7 +296,7 @@ int launch_dgemm_tiles(int64_t M, int64_t N, int64_t K, double alpha, const doub
     const int64_t tm = (M + BM - 1) / BM, tn = (N + BN - 1) / BN;
     if (tm * tn > 0x7fffffffLL || M > 0x7fffffffLL || N > 0x7fffffffLL || K > 0x7fffffffLL) return HCLOOC_ERR_INTERNAL;
     static const bool no_streamk = getenv("HCLOOC_NO_STREAMK") != nullptr;   // experiment knob
-    if (ksplit < 0 && K > 0 && !no_streamk && !transa && !transb) {
+    if (ksplit < 0 && K > 0 && !no_streamk) {
         // A launch that has the GPU to itself.  One CTA per tile runs its main loop ~1 % faster than the persistent
         // kernel (measured 0.981 against 0.969 of peak on whole waves) but leaves the last wave partly empty, so
         // the persistent stream-K kernel is used unless the tiles fill their waves to 98.8 % or better.  A caller
@@ -304,7 +304,7 @@ int launch_dgemm_tiles(int64_t M, int64_t N, int64_t K, double alpha, const doub
         const int64_t T = tm * tn, waves = (T + 147) / 148;
         const bool whole_waves = (double)T >= 0.988 * (double)(waves * 148);
         if (streamk_scratch || !whole_waves) {
-            rc = launch_dgemm_streamk(M, N, K, alpha, tmA, tmB, beta, dC, ldc, stream, streamk_scratch);
+            rc = launch_dgemm_streamk(M, N, K, alpha, tmA, tmB, beta, dC, ldc, stream, streamk_scratch, transa, transb);
             if (rc != 1) return rc;
         }
     }

@@ -79,6 +79,7 @@ __device__ __forceinline__ void ld_partial(const double* p, double& x, double& y
     asm volatile("ld.global.cg.v2.f64 {%0, %1}, [%2];" : "=d"(x), "=d"(y) : "l"(p) : "memory");
 }
 
+template <bool TA, bool TB>       // operand stored transposed (hclooc_dgemm_t): only TMA boxes and fragment addressing change
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 hclooc_dgemm_streamk_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                             double* __restrict__ C, long long ldc, int M, int N, double alpha, double beta,
@@ -121,10 +122,20 @@ hclooc_dgemm_streamk_kernel(const __grid_constant__ CUtensorMap tmA, const __gri
                     const uint32_t sa = smem_base + stage * STAGE_BYTES;
                     const uint32_t sb = sa + A_STAGE_BYTES;
                     const int k0 = kb * BK;
-                    #pragma unroll
-                for (int hk = 0; hk < BK / 16; ++hk) tma_load_2d(sa + hk * A_HALF_BYTES, &tmA, k0 + 16 * hk, m0, full);
-                    #pragma unroll
-                    for (int b = 0; b < BN / 16; ++b) tma_load_2d(sb + b * B_BOX_BYTES, &tmB, n0 + 16 * b, k0, full);
+                    if (!TA) {
+                        #pragma unroll
+                        for (int hk = 0; hk < BK / 16; ++hk) tma_load_2d(sa + hk * A_HALF_BYTES, &tmA, k0 + 16 * hk, m0, full);
+                    } else {
+                        #pragma unroll
+                        for (int b = 0; b < BM / 16; ++b) tma_load_2d(sa + b * B_BOX_BYTES, &tmA, m0 + 16 * b, k0, full);
+                    }
+                    if (!TB) {
+                        #pragma unroll
+                        for (int b = 0; b < BN / 16; ++b) tma_load_2d(sb + b * B_BOX_BYTES, &tmB, n0 + 16 * b, k0, full);
+                    } else {
+                        #pragma unroll
+                        for (int hk = 0; hk < BK / 16; ++hk) tma_load_2d(sb + hk * A_HALF_BYTES, &tmB, k0 + 16 * hk, n0, full);
+                    }
                     if (++stage == STAGES) { stage = 0; phase ^= 1u; }
                 }
             }
@@ -134,7 +145,7 @@ hclooc_dgemm_streamk_kernel(const __grid_constant__ CUtensorMap tmA, const __gri
 
     // ---------------------------------------------------------------- consumer warps: DMMA
     regs_take_consumer();
-    FragLanes f;
+    FragLanesT<TA, TB> f;
     f.init(warp, lane);
     int stage = 0;
     uint32_t phase = 0;
@@ -271,7 +282,10 @@ int ensure_attr() {
     static int status = -1;
     static std::once_flag once;
     std::call_once(once, [] {
-        cudaError_t e = cudaFuncSetAttribute(hclooc_dgemm_streamk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+        cudaError_t e = cudaFuncSetAttribute(hclooc_dgemm_streamk_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(hclooc_dgemm_streamk_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(hclooc_dgemm_streamk_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(hclooc_dgemm_streamk_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
         status = (e == cudaSuccess) ? 0 : cuda_fail(e);
     });
     return status;
@@ -308,7 +322,7 @@ size_t streamk_counter_offset() { return (size_t)2 * SK_MAX_CTAS * SK_SLOT_BYTES
 size_t streamk_counter_bytes() { return SK_MAX_TAIL_TILES * sizeof(unsigned); }
 
 int launch_dgemm_streamk(int64_t M, int64_t N, int64_t K, double alpha, const CUtensorMap& tmA, const CUtensorMap& tmB,
-                         double beta, double* dC, int64_t ldc, cudaStream_t stream, void* scratch) {
+                         double beta, double* dC, int64_t ldc, cudaStream_t stream, void* scratch, int transa, int transb) {
     static int num_sms = 0;
     if (num_sms == 0) {
         int dev = 0, n = 0;
@@ -328,8 +342,10 @@ int launch_dgemm_streamk(int64_t M, int64_t N, int64_t K, double alpha, const CU
     void* mem = scratch ? scratch : sc->mem;
     double* partials = (double*)mem;
     unsigned* counters = (unsigned*)((uint8_t*)mem + (size_t)2 * SK_MAX_CTAS * SK_SLOT_BYTES);
-    hclooc_dgemm_streamk_kernel<<<P.G, NUM_THREADS, SMEM_BYTES, stream>>>(tmA, tmB, dC, (long long)ldc, (int)M, (int)N, alpha, beta,
-                                                                           P, partials, counters);
+    if (transa && transb) hclooc_dgemm_streamk_kernel<true, true><<<P.G, NUM_THREADS, SMEM_BYTES, stream>>>(tmA, tmB, dC, (long long)ldc, (int)M, (int)N, alpha, beta, P, partials, counters);
+    else if (transa) hclooc_dgemm_streamk_kernel<true, false><<<P.G, NUM_THREADS, SMEM_BYTES, stream>>>(tmA, tmB, dC, (long long)ldc, (int)M, (int)N, alpha, beta, P, partials, counters);
+    else if (transb) hclooc_dgemm_streamk_kernel<false, true><<<P.G, NUM_THREADS, SMEM_BYTES, stream>>>(tmA, tmB, dC, (long long)ldc, (int)M, (int)N, alpha, beta, P, partials, counters);
+    else hclooc_dgemm_streamk_kernel<false, false><<<P.G, NUM_THREADS, SMEM_BYTES, stream>>>(tmA, tmB, dC, (long long)ldc, (int)M, (int)N, alpha, beta, P, partials, counters);
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess && sc) e = cudaEventRecord(sc->done, stream);
     if (e != cudaSuccess) return cuda_fail(e);

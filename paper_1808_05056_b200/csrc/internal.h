@@ -43,7 +43,7 @@ int launch_dgemm_tiles(int64_t M, int64_t N, int64_t K, double alpha, const doub
 // The persistent stream-K kernel (dgemm_streamk_sm100.cu).  Returns 1 if it does not apply (no scratch buffer
 // free, shape out of range): the caller then launches one CTA per tile.
 int launch_dgemm_streamk(int64_t M, int64_t N, int64_t K, double alpha, const ::CUtensorMap_st& tmA, const ::CUtensorMap_st& tmB,
-                         double beta, double* dC, int64_t ldc, cudaStream_t stream, void* scratch);
+                         double beta, double* dC, int64_t ldc, cudaStream_t stream, void* scratch, int transa = 0, int transb = 0);
 size_t streamk_scratch_bytes();     // one scratch buffer (partial-tile slots + counters), rounded to 1 KiB
 size_t streamk_counter_offset();    // the counters inside it must be zero before the first launch
 size_t streamk_counter_bytes();

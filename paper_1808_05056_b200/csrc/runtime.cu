@@ -126,7 +126,7 @@ int hclDgemmAsyncT(int transa, int transb, int64_t M, int64_t N, int64_t K, doub
     if (M < 0) return -1;
     if (N < 0) return -2;
     if (K < 0) return -3;
-    if (variant != HCL_DGEMM_AUTO && variant != 1 && variant != 2 && variant != 4) return -14;
+    if (variant != HCL_DGEMM_AUTO && variant != -1 && variant != 1 && variant != 2 && variant != 4) return -14;
     const bool noab = (alpha == 0.0 || K == 0);
     if (M > 0 && N > 0) {
         if (!noab) {
@@ -138,7 +138,8 @@ int hclDgemmAsyncT(int transa, int transb, int64_t M, int64_t N, int64_t K, doub
         }
         if (!dC) return -10;
         if (ldc < N) return -11;
-        int rc = launch_dgemm_tiles(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, (cudaStream_t)s, variant, nullptr, transa, transb);
+        int rc = launch_dgemm_tiles(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, (cudaStream_t)s,
+                                    variant == HCL_DGEMM_AUTO ? (dgemm_tile_count(M, N) >= 148 ? -1 : 0) : variant, nullptr, transa, transb);
         if (rc) return rc;
     }
     return finish_async((cudaStream_t)s, ev);

@@ -754,3 +754,37 @@ def test_transposed_in_core_and_direct_modes(H):
         assert np.array_equal(C.view, ref)
     finally:
         H.hclooc_ctx_destroy(ctx)
+
+
+@pytest.mark.parametrize("transa,transb", [(1, 0), (0, 1), (1, 1)])
+@pytest.mark.parametrize("M,N,K,dist", [
+    (1700, 1500, 1040, "int"),        # 168 tiles: one wave joins the stream-K tail, ragged edges
+    (2048, 2432, 512, "uniform"),     # 2 waves + 8 tiles
+    (384, 640, 4100, "int"),          # 15 tiles cut along K among several CTAs
+])
+def test_streamk_kernel_transposed_layouts(H, transa, transb, M, N, K, dist):
+    """The persistent stream-K kernel on operands stored transposed (variant -1 of hclDgemmAsyncT), and through the
+    in-core path of hclooc_dgemm_t; the same bits as the untransposed stream-K launch on written-out transposes."""
+    import torch
+    ar, ac = (K, M) if transa else (M, K)
+    br, bc = (N, K) if transb else (K, N)
+    A = synthgen.fill(np.empty((ar, ac)), 62, "A", dist); B = synthgen.fill(np.empty((br, bc)), 62, "B", dist)
+    C0 = synthgen.fill(np.empty((M, N)), 62, "C", dist)
+    opA, opB = np.empty((M, K)), np.empty((K, N))
+    opA[...] = A.T if transa else A
+    opB[...] = B.T if transb else B
+    ref = C0.copy()
+    D = oracle.dgemm(1.5, opA, opB, -0.5, ref, want_denominator=True)
+    dA, dB, dC = torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(), torch.from_numpy(C0).cuda()
+    H.hclDgemmAsyncT(transa, transb, M, N, K, 1.5, dA, ac, dB, bc, -0.5, dC, N, torch.cuda.current_stream(), variant=-1)
+    torch.cuda.synchronize()
+    got = dC.cpu().numpy()
+    check(got, ref, D, exact=(dist == "int"))
+    dA2, dB2, dC2 = torch.from_numpy(opA).cuda(), torch.from_numpy(opB).cuda(), torch.from_numpy(C0).cuda()
+    H.hclDgemmAsyncEx(M, N, K, 1.5, dA2, K, dB2, N, -0.5, dC2, N, torch.cuda.current_stream(), variant=-1)
+    torch.cuda.synchronize()
+    assert np.array_equal(dC2.cpu().numpy().view(np.uint64), got.view(np.uint64))
+    dC3 = torch.from_numpy(C0).cuda()
+    st = H.hclooc_dgemm_t(None, transa, transb, M, N, K, 1.5, dA, ac, dB, bc, -0.5, dC3, N, 0)
+    assert st.n_kernels == 1 and st.plan.trans == transa + 2 * transb
+    check(dC3.cpu().numpy(), ref, D, exact=(dist == "int"))
