@@ -84,9 +84,13 @@ typedef struct hclooc_plan_t {
     int32_t  direct;              /* 1 = DIRECT mode: no device buffer at all -- one launch of the tile kernel whose TMA
                                      loads read the A and B tiles straight from the (mapped) pinned host matrices and whose
                                      epilogue reads and writes C in host memory.  Every tile streams over the host link
-                                     (bytes_h2d counts each tile's own reads: A is read ceil(N/128) times, B ceil(M/128)
+                                     (bytes_h2d counts what the tiles read: A ceil(N/128)/direct_cn times, B ceil(M/128)/direct_cm
                                      times), so it only wins where the staged pipeline is bound by per-copy latency:
                                      small problems under small budgets (BASELINE config 1).  h = w = n_steps = 1.     */
+    int32_t  direct_cm, direct_cn; /* direct mode: the launch runs clusters of direct_cm x direct_cn CTAs (neighbouring
+                                     tiles) that share their loads by TMA multicast -- A is read ceil(ceil(N/128)/direct_cn)
+                                     times and B ceil(ceil(M/128)/direct_cm) times; 4 x 4 (one 16-CTA cluster) makes
+                                     config 1's traffic the compulsory minimum                                      */
     int32_t  trans;               /* hclooc_dgemm_t: bit 0 = A is stored K x M, bit 1 = B is stored N x K.  The device
                                      slices keep the stored layout: an A slice is then kb x mb (lda_dev >= mb), a B
                                      slice nb x kb (ldb_dev >= kb), and the tile kernel reads them transposed       */
@@ -283,8 +287,10 @@ int hclDgemmAsync(int64_t M, int64_t N, int64_t K, double alpha, const double* d
 /* Same with the launch variant spelled out: HCL_DGEMM_AUTO (what hclDgemmAsync does: the persistent stream-K
  * kernel when the output has at least 148 tiles of 128 x 128, else one CTA -- or a cluster of 2 or 4 CTAs
  * splitting K -- per tile), 1 / 2 / 4 = that many CTAs per tile (what a pipeline step launches, plan.ksplit),
- * -1 = persistent stream-K.  -14: unknown variant.                                                    */
+ * -1 = persistent stream-K; HCL_DGEMM_CLUSTER(cm, cn), cm, cn in {1, 2, 4} = the direct-mode kernel: clusters of
+ * cm x cn neighbouring tiles sharing their A / B loads by TMA multicast (plan.direct_cm / direct_cn).  -14: unknown.  */
 #define HCL_DGEMM_AUTO 0
+#define HCL_DGEMM_CLUSTER(cm, cn) (100 + 10 * (cm) + (cn))
 int hclDgemmAsyncEx(int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda,
                     const double* dB, int64_t ldb, double beta, double* dC, int64_t ldc,
                     hclStream s, hclEvent* ev, int variant);

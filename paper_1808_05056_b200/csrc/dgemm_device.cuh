@@ -209,6 +209,10 @@ __device__ __forceinline__ void epilogue_store(const double (&acc)[4][4][2][2], 
                                                int M, int N, int m0, int n0, double alpha, double beta, const FragLanesT<TA, TB>& f) {
     const bool read_c = (beta != 0.0);
     const bool vec_ok = ((ldc & 1LL) == 0) && ((reinterpret_cast<uintptr_t>(C) & 15u) == 0);
+    // 256-bit accesses (sm_100: LDG/STG.256): a lane's 4 consecutive columns are one 32-byte sector, a quarter warp's
+    // 16 columns one 128-byte line -- what the host link wants when C lives in host memory (direct mode): 16-byte
+    // stores into lines that were not read first (beta == 0) crossed the link at ~14 GB/s
+    const bool vec4_ok = ((ldc & 3LL) == 0) && ((reinterpret_cast<uintptr_t>(C) & 31u) == 0);
     #pragma unroll
     for (int u = 0; u < 4; ++u) {
         const int row = m0 + f.row_of(u);
@@ -221,7 +225,16 @@ __device__ __forceinline__ void epilogue_store(const double (&acc)[4][4][2][2], 
                 // lane holds 4 consecutive columns: (v=0,c0) (v=1,c0) (v=0,c1) (v=1,c1)
                 double x0 = __dmul_rn(alpha, acc[u][bx][0][0]), x1 = __dmul_rn(alpha, acc[u][bx][1][0]);
                 double x2 = __dmul_rn(alpha, acc[u][bx][0][1]), x3 = __dmul_rn(alpha, acc[u][bx][1][1]);
-                if (col + 3 < N && vec_ok) {
+                if (col + 3 < N && vec4_ok) {
+                    double* p = crow + col;
+                    if (read_c) {
+                        double c0, c1, c2, c3;
+                        asm volatile("ld.global.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(c0), "=d"(c1), "=d"(c2), "=d"(c3) : "l"(p) : "memory");
+                        x0 = axpby_tail(x0, beta, c0); x1 = axpby_tail(x1, beta, c1);
+                        x2 = axpby_tail(x2, beta, c2); x3 = axpby_tail(x3, beta, c3);
+                    }
+                    asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(x0), "d"(x1), "d"(x2), "d"(x3) : "memory");
+                } else if (col + 3 < N && vec_ok) {
                     double2* p = reinterpret_cast<double2*>(crow + col);
                     if (read_c) {
                         const double2 c01 = p[0], c23 = p[1];

@@ -202,9 +202,11 @@ EncodeTiledFn get_encode_fn() {
     return fn;
 }
 
+}  // namespace
+
 // 2-D FP64 tensor map over a row-major matrix (rows x cols, leading dimension ld elements),
 // box = box_rows x 16 columns (128 bytes), 128-byte swizzle, zero fill out of bounds.
-int make_map(CUtensorMap* map, const double* base, int64_t rows, int64_t cols, int64_t ld, int box_rows) {
+int make_tensor_map(CUtensorMap* map, const double* base, int64_t rows, int64_t cols, int64_t ld, int box_rows) {
     EncodeTiledFn enc = get_encode_fn();
     if (!enc) return HCLOOC_ERR_CUDA;
     cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
@@ -216,6 +218,11 @@ int make_map(CUtensorMap* map, const double* base, int64_t rows, int64_t cols, i
                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) { set_last_cuda_error(1000 + (int)r); return HCLOOC_ERR_CUDA; }
     return HCLOOC_OK;
+}
+
+namespace {
+inline int make_map(CUtensorMap* map, const double* base, int64_t rows, int64_t cols, int64_t ld, int box_rows) {
+    return make_tensor_map(map, base, rows, cols, ld, box_rows);
 }
 
 template <bool TA, bool TB>

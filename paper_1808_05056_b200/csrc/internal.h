@@ -76,6 +76,16 @@ inline int64_t early_uploads(int64_t h, int n_sets, int n_abuf) {
     return pre < 0 ? 0 : pre;
 }
 
+// 2-D FP64 tensor map (box_rows x 16 columns, 128-byte swizzle, zero fill out of bounds) over a row-major matrix
+int make_tensor_map(::CUtensorMap_st* map, const double* base, int64_t rows, int64_t cols, int64_t ld, int box_rows);
+
+// Direct mode with thread-block clusters sharing their loads by TMA multicast (dgemm_direct_sm100.cu)
+void direct_cluster_shape(int64_t M, int64_t N, int max_cluster, int* cm, int* cn);   // pure arithmetic
+void set_planner_max_cluster(int n);                                                 // the planner's copy of direct_max_cluster()
+int direct_max_cluster();                                                            // 16 if a 4 x 4 cluster can launch here, else 8
+int launch_dgemm_direct(int64_t M, int64_t N, int64_t K, double alpha, const double* A, int64_t lda, const double* B, int64_t ldb,
+                        double beta, double* C, int64_t ldc, cudaStream_t stream, int cm, int cn);
+
 // hclooc_plan_ex with the operand layouts of hclooc_dgemm_t (planner.cpp)
 int plan_impl(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zero, size_t device_budget_bytes,
               int operands_on_device, int transa, int transb, hclooc_plan_t* out);

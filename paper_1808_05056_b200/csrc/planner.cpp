@@ -49,6 +49,9 @@ const MachineModel& machine_model() {
     return mm;
 }
 
+int g_direct_max_cluster = 16;      // what direct_max_cluster() found on the device (set by the executor); 16 on a B200
+void set_planner_max_cluster(int n) { g_direct_max_cluster = n >= 16 ? 16 : 8; }
+
 namespace {
 
 struct Cand {
@@ -366,13 +369,20 @@ int hclooc::plan_impl(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alp
     // plus ~30 us fixed -- better than a staged plan only where that one is bound by per-copy latency.
     if (direct_ok && M <= 0x7fffffffLL && N <= 0x7fffffffLL && K <= 0x7fffffffLL) {
         const double tm = (double)ceil_div(M, TILE), tn = (double)ceil_div(N, TILE);
-        const double rd = 8.0 * ((scale_only ? 0.0 : tn * (double)M * (double)Keff + tm * (double)Keff * (double)N) +
+        // the tiles of a cluster share their loads by TMA multicast (dgemm_direct_sm100.cu): A crosses the link once per
+        // cluster column, B once per cluster row; transposed operands use the plain tile kernel (no sharing)
+        int cm = 1, cn = 1;
+        if (!transa && !transb && !scale_only) direct_cluster_shape(M, N, g_direct_max_cluster, &cm, &cn);
+        out->direct_cm = cm; out->direct_cn = cn;
+        const double rd = 8.0 * ((scale_only ? 0.0 : std::ceil(tn / cn) * (double)M * (double)Keff + std::ceil(tm / cm) * (double)Keff * (double)N) +
                                  (beta_nz ? (double)M * (double)N : 0.0));
         const double wr = 8.0 * (double)M * (double)N;
-        const double direct_Bps = env_or("HCLOOC_DIRECT_GBPS", 50.0) * 1e9;
+        // measured: 46-50 GB/s when every tile loads for itself, 24-35 GB/s through a multicasting cluster (its CTAs
+        // advance in lockstep, a stage at a time)
+        const double direct_Bps = env_or("HCLOOC_DIRECT_GBPS", cm * cn > 1 ? 33.0 : 50.0) * 1e9;
         const double t_link = std::max(std::max(rd / direct_Bps, wr / mm.d2h_Bps), (rd + wr) / mm.duplex_Bps);
         const double t_flop = (scale_only ? 0.0 : 2.0 * (double)M * (double)N * (double)Keff) / mm.fp64_flops;
-        const double waves = std::ceil(tm * tn / NUM_SMS);
+        const double waves = std::ceil(tm * tn / (cm * cn > 1 ? 128.0 : (double)NUM_SMS));   // whole clusters per GPC
         const double t_comp = t_flop * (waves * NUM_SMS * (double)(TILE * TILE)) / ((double)M * (double)N);
         const double t_direct = std::max(t_link, t_comp) + 30e-6;
         if (direct_forced || !found || t_direct < best.t_model) {

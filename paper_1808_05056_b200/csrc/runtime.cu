@@ -100,7 +100,9 @@ int hclDgemmAsyncEx(int64_t M, int64_t N, int64_t K, double alpha, const double*
     if (M < 0) return -1;
     if (N < 0) return -2;
     if (K < 0) return -3;
-    if (variant != HCL_DGEMM_AUTO && variant != -1 && variant != 1 && variant != 2 && variant != 4) return -14;
+    const int ccm = (variant - 100) / 10, ccn = (variant - 100) % 10;
+    const bool cluster = variant > 100 && (ccm == 1 || ccm == 2 || ccm == 4) && (ccn == 1 || ccn == 2 || ccn == 4);
+    if (variant != HCL_DGEMM_AUTO && variant != -1 && variant != 1 && variant != 2 && variant != 4 && !cluster) return -14;
     const bool noab = (alpha == 0.0 || K == 0);
     if (M > 0 && N > 0) {
         if (!noab) {
@@ -112,8 +114,10 @@ int hclDgemmAsyncEx(int64_t M, int64_t N, int64_t K, double alpha, const double*
         }
         if (!dC) return -10;
         if (ldc < N) return -11;
-        int rc = launch_dgemm_tiles(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, (cudaStream_t)s,
-                                    variant == HCL_DGEMM_AUTO ? (dgemm_tile_count(M, N) >= 148 ? -1 : 0) : variant);
+        int rc = (cluster && !noab)
+                     ? launch_dgemm_direct(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, (cudaStream_t)s, ccm, ccn)
+                     : launch_dgemm_tiles(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, (cudaStream_t)s,
+                                          variant == HCL_DGEMM_AUTO ? (dgemm_tile_count(M, N) >= 148 ? -1 : 0) : (cluster ? 1 : variant));
         if (rc) return rc;
     }
     return finish_async((cudaStream_t)s, ev);

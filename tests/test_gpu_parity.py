@@ -533,7 +533,10 @@ def test_config1_direct_mode_uses_no_device_memory(H, dist, exact):
         st = H.hclooc_dgemm_ex(ctx, M, N, K, 1.0, A, A.ld, B, B.ld, 0.5, C, C.ld, 1 * MiB)
         assert st.plan.direct == 1 and st.plan.workspace_bytes == 0 and st.n_kernels == 1
         assert st.n_copies_h2d == 0 and st.n_copies_d2h == 0
-        assert st.bytes_h2d == 8 * (4 * M * K + 4 * K * N + M * N) and st.bytes_d2h == 8 * M * N   # 4 x 4 tiles: 4 reads of A and B
+        # 4 x 4 tiles in ONE 16-CTA cluster sharing its loads by TMA multicast: A and B cross the link once (compulsory traffic)
+        cm, cn = st.plan.direct_cm, st.plan.direct_cn
+        assert (cm, cn) in ((4, 4), (2, 4))
+        assert st.bytes_h2d == 8 * ((4 // cn) * M * K + (4 // cm) * K * N + M * N) and st.bytes_d2h == 8 * M * N
         check(C.view, ref, D, exact)
         direct = C.view.copy()
         # the staged pipeline on the same inputs: same kernel, same summation order -> the same bits
@@ -568,7 +571,9 @@ def test_direct_mode_matches_oracle(H, M, N, K, alpha, beta, dist, pads):
         st = H.hclooc_dgemm_ex(ctx, M, N, K, alpha, A, A.ld, B, B.ld, beta, C, C.ld, 1 * MiB)
         assert st.plan.direct == 1 and st.plan.workspace_bytes == 0
         tm, tn = -(-M // 128), -(-N // 128)
-        assert st.bytes_h2d == 8 * (tn * M * K + tm * K * N + (M * N if beta != 0.0 else 0))
+        cm, cn = st.plan.direct_cm, st.plan.direct_cn
+        assert cm in (1, 2, 4) and cn in (1, 2, 4) and (cm > 1 or tm == 1) and (cn > 1 or tn == 1)
+        assert st.bytes_h2d == 8 * (-(-tn // cn) * M * K + -(-tm // cm) * K * N + (M * N if beta != 0.0 else 0))
         check(C.view, ref, D, exact=(dist == "int"))
         assert np.isnan(C.array[:, N:]).all()                                   # host padding of C untouched
     finally:

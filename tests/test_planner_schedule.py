@@ -381,7 +381,8 @@ def test_direct_mode_is_chosen_only_where_copy_latency_dominates():
     MiB = 1 << 20
     p = H.hclooc_plan_ex(512, 512, 512, 1, 0, 1 * MiB, 3)
     assert p.direct == 1 and p.workspace_bytes == 0 and p.n_steps == 1 and p.h == p.w == p.kpanels == 1
-    assert p.bytes_h2d == 8 * (4 * 512 * 512 * 2 + 512 * 512) and p.bytes_d2h == 8 * 512 * 512
+    assert (p.direct_cm, p.direct_cn) == (4, 4)              # 4 x 4 tiles in one 16-CTA cluster: A and B cross the link once
+    assert p.bytes_h2d == 8 * 3 * 512 * 512 and p.bytes_d2h == 8 * 512 * 512
     assert p.n_copies_h2d == 0 and p.n_copies_d2h == 0
     staged = H.hclooc_plan_ex(512, 512, 512, 1, 0, 1 * MiB, 0)
     assert staged.direct == 0 and p.t_model_s < staged.t_model_s
@@ -389,7 +390,7 @@ def test_direct_mode_is_chosen_only_where_copy_latency_dominates():
         q = H.hclooc_plan_ex(M, N, K, 1, 0, budget, 3)
         assert q.direct == 0 and q.workspace_bytes > 0
     forced = H.hclooc_plan_ex(8192, 8192, 8192, 0, 0, 256 * MiB, 4)
-    assert forced.direct == 1 and forced.bytes_h2d == 8 * 2 * 64 * 8192 * 8192
+    assert forced.direct == 1 and forced.bytes_h2d == 8 * 2 * 16 * 8192 * 8192      # 64 x 64 tiles in 4 x 4 clusters
     # a budget too small for any staged plan is no obstacle: direct mode needs none
     tiny = H.hclooc_plan_ex(300, 300, 300, 1, 0, 4096, 3)
     assert tiny.direct == 1
