@@ -793,3 +793,31 @@ def test_streamk_kernel_transposed_layouts(H, transa, transb, M, N, K, dist):
     st = H.hclooc_dgemm_t(None, transa, transb, M, N, K, 1.5, dA, ac, dB, bc, -0.5, dC3, N, 0)
     assert st.n_kernels == 1 and st.plan.trans == transa + 2 * transb
     check(dC3.cpu().numpy(), ref, D, exact=(dist == "int"))
+
+
+@pytest.mark.parametrize("cm,cn", [(1, 2), (2, 1), (2, 2), (1, 4), (4, 1), (2, 4), (4, 2), (4, 4)])
+@pytest.mark.parametrize("M,N,K,alpha,beta,dist", [
+    (512, 512, 96, 1.0, 0.5, "int"),              # whole clusters
+    (300, 700, 200, -1.5, 1.0, "uniform"),        # ragged tiles and clusters padded with tiles outside C
+    (129, 130, 33, 2.0, 0.0, "int"),
+    (1300, 900, 70, 1.0, 0.5, "uniform"),         # several clusters
+])
+def test_cluster_multicast_kernel_matches_tile_kernel(H, cm, cn, M, N, K, alpha, beta, dist):
+    """HCL_DGEMM_CLUSTER(cm, cn): the direct-mode kernel (cm x cn CTAs per cluster sharing their loads by TMA multicast)
+    on device pointers -- within the gate of the oracle and the very bits of the one-CTA-per-tile kernel."""
+    import torch
+    lda, ldb, ldc = K + (K % 2) + 4, N + (N % 2) + 2, N + (-N % 4) + 8
+    A = np.full((M, lda), np.nan); B = np.full((K, ldb), np.nan); C0 = np.full((M, ldc), np.nan)
+    synthgen.fill(A, 71, "A", dist, cols=K); synthgen.fill(B, 71, "B", dist, cols=N); synthgen.fill(C0, 71, "C", dist, cols=N)
+    if beta == 0.0:
+        C0[:, :N] = np.nan
+    dA, dB, dC, dC1 = (torch.from_numpy(x).cuda() for x in (A, B, C0, C0))
+    H.hclDgemmAsyncEx(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, torch.cuda.current_stream(), variant=100 + 10 * cm + cn)
+    H.hclDgemmAsyncEx(M, N, K, alpha, dA, lda, dB, ldb, beta, dC1, ldc, torch.cuda.current_stream(), variant=1)
+    torch.cuda.synchronize()
+    got, one = dC.cpu().numpy(), dC1.cpu().numpy()
+    ref = C0[:, :N].copy()
+    D = oracle.dgemm(alpha, A[:, :K], B[:, :N], beta, ref, want_denominator=True)
+    check(got[:, :N], ref, D, exact=(dist == "int"))
+    assert np.isnan(got[:, N:]).all()
+    assert np.array_equal(got[:, :N].view(np.uint64), one[:, :N].view(np.uint64))
