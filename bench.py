@@ -46,7 +46,8 @@ WORKLOADS = {
                  desc="65536x65536x16384 FP64, alpha=2 beta=-1, budget 16 GiB"),
 }
 FP64_PEAK_TFLOPS = 37.2   # 148 SMs x 4 SMSPs x 32 flop/clk (DMMA.8x8x4: 512 flop / 16 clk) x 1.965 GHz; measured 37.17
-LINK = dict(h2d_GBps=55.5, d2h_GBps=51.5, duplex_GBps=88.0)   # measured on the box (profiles/r01_box_probe.md)
+# fallback (the first box probed, profiles/r01_box_probe.md); bench.py measures the link of the box it runs on (measure_link)
+LINK = dict(h2d_GBps=55.5, d2h_GBps=51.5, duplex_GBps=88.0, source="profiles/r01_box_probe.md")
 
 
 class ClockSampler:
@@ -78,6 +79,9 @@ class ClockSampler:
             self.t.join(timeout=2)
 
     def summary(self):
+        t0 = time.time()
+        while self.proc and not self.rows and time.time() - t0 < 3.0:      # a run shorter than the first sample (config 1)
+            time.sleep(0.05)
         sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
         mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
         reasons = set()
@@ -99,6 +103,43 @@ def ncu_traffic(launch):
         return t["dram_bytes"] if t.get("launch") == launch else None
     except (OSError, ValueError, KeyError):
         return None
+
+
+def measure_link(H, total=1 << 30, chunk=256 << 20):
+    """Host-link peaks of THIS box, measured through the library's runtime calls right before the timed legs (boxes of the
+    pool differ: 51.5-57 GB/s D2H, 88-100 GB/s duplex): pinned 256 MiB copies, each direction alone and both at once."""
+    try:
+        host_a, host_b = H.hclooc_host_alloc(total), H.hclooc_host_alloc(total)
+        dev_a, dev_b = H.hclMalloc(total), H.hclMalloc(total)
+        s0, s1 = H.hclStreamCreate(), H.hclStreamCreate()
+    except Exception:
+        return None
+
+    def run(up, down):
+        for off in range(0, total, chunk):
+            if up:
+                H.hclMemcpyAsync(dev_a + off, host_a + off, chunk, H.HCL_H2D, s0)
+            if down:
+                H.hclMemcpyAsync(host_b + off, dev_b + off, chunk, H.HCL_D2H, s1)
+        H.hclStreamSynchronize(s0); H.hclStreamSynchronize(s1)
+
+    out = {}
+    for key, up, down in (("h2d_GBps", True, False), ("d2h_GBps", False, True), ("duplex_GBps", True, True)):
+        run(up, down)
+        best = 0.0
+        for _ in range(2):
+            t0 = time.perf_counter()
+            run(up, down)
+            best = max(best, (int(up) + int(down)) * total / (time.perf_counter() - t0) / 1e9)
+        out[key] = best
+    for p in (dev_a, dev_b):
+        H.hclFree(p)
+    for p in (host_a, host_b):
+        H.hclooc_host_free(p)
+    for s in (s0, s1):
+        H.hclStreamDestroy(s)
+    out["source"] = "measured live on this box (1 GiB in 256 MiB pinned copies per direction, best of 2)"
+    return out
 
 
 def link_roofline_s(flops, bytes_h2d, bytes_d2h):
@@ -236,6 +277,10 @@ def run_ours(args, wl, name):
             return H.hclooc_dgemm_t(ctx, ta, tb, M, N, K, alpha, A, M if ta else K, B, K if tb else N, beta, C, C.ld, budget)
         return H.hclooc_dgemm_ex(ctx, M, N, K, alpha, A, A.ld, B, B.ld, beta, C, C.ld, budget)
 
+    if not args.kernel_only:
+        live = measure_link(H)
+        if live:
+            LINK.update(live)
     with ClockSampler(local) as clk:
         if args.kernel_only:
             plan = H.hclooc_plan(M, N, K, beta != 0.0, 0, budget)

@@ -314,6 +314,11 @@ int   hclooc_host_unregister(void* p);
 const char* hclooc_strerror(int status);
 int         hclooc_last_cuda_error(void);              /* last cudaError_t seen by this thread      */
 const char* hclooc_version(void);
+/* FP64 issue-rate probe of the current device: independent register chains of DMMA.8x8x4 (kind 0: mma.sync.m8n8k4.f64,
+ * what the kernels use) or DFMA (kind 1), no memory traffic, ctas_per_sm x 256 threads per SM, launches repeated for
+ * about `seconds`; writes the best launch in TFLOP/s.  The roofline denominator of DESIGN.md section 6 is this
+ * measurement (python -m paper_1808_05056_b200.box_probe).  -1 kind, -2 ctas_per_sm outside 1..8, -3 seconds, -4 NULL. */
+int hclooc_probe_fp64(int kind, int ctas_per_sm, double seconds, double* tflops);
 
 #ifdef __cplusplus
 }

@@ -13,6 +13,6 @@ from ._binding import (  # noqa: F401
     hclMemcpy, hclMemcpyAsync, hclMemcpy2DAsync, hclDgemmAsync, hclDgemmAsyncEx, hclDgemmAsyncT, hclWaitEvent,
     hclStreamSynchronize, hclDeviceSynchronize,
     hclooc_host_alloc, hclooc_host_free, hclooc_host_register, hclooc_host_unregister,
-    hclooc_strerror, hclooc_last_cuda_error, hclooc_version,
+    hclooc_strerror, hclooc_last_cuda_error, hclooc_version, hclooc_probe_fp64,
     HCL_H2D, HCL_D2H, HCL_OP_N, HCL_OP_T, EXPORTS, OP_DTYPE,
 )

@@ -19,7 +19,7 @@ EXPORTS = [
     "hclStreamDestroy", "hclEventDestroy", "hclMemcpy", "hclMemcpyAsync", "hclMemcpy2DAsync",
     "hclDgemmAsync", "hclDgemmAsyncEx", "hclDgemmAsyncT", "hclWaitEvent", "hclStreamSynchronize", "hclDeviceSynchronize",
     "hclooc_host_alloc", "hclooc_host_free", "hclooc_host_register", "hclooc_host_unregister",
-    "hclooc_strerror", "hclooc_last_cuda_error", "hclooc_version",
+    "hclooc_strerror", "hclooc_last_cuda_error", "hclooc_version", "hclooc_probe_fp64",
 ]
 
 
@@ -113,6 +113,7 @@ def lib():
         L.hclooc_strerror.restype = c_char_p
         L.hclooc_last_cuda_error.argtypes = []
         L.hclooc_version.restype = c_char_p
+        L.hclooc_probe_fp64.argtypes = [c_int, c_int, dbl, POINTER(dbl)]
         for name in EXPORTS:
             if name not in ("hclooc_host_alloc", "hclooc_strerror", "hclooc_version"):
                 getattr(L, name).restype = c_int
@@ -397,6 +398,13 @@ def hclooc_strerror(status: int) -> str:
 
 def hclooc_last_cuda_error() -> int:
     return lib().hclooc_last_cuda_error()
+
+
+def hclooc_probe_fp64(kind: int = 0, ctas_per_sm: int = 4, seconds: float = 1.0) -> float:
+    """Measured FP64 rate (TFLOP/s) of register-resident DMMA (kind 0) or DFMA (kind 1) chains on the current device."""
+    out = c_double(0.0)
+    _check(lib().hclooc_probe_fp64(kind, ctas_per_sm, seconds, byref(out)), "hclooc_probe_fp64")
+    return out.value
 
 
 def hclooc_version() -> str:

@@ -2,6 +2,7 @@
 // as plain C functions: no factory, no virtual dispatch (the paper attributes part of its 4-10 %
 // overhead to the virtual-table lookups, :164).
 #include <cstring>
+#include <algorithm>
 #include "internal.h"
 
 using namespace hclooc;
@@ -18,6 +19,42 @@ int finish_async(cudaStream_t s, hclEvent* ev) {
     return HCLOOC_OK;
 }
 cudaMemcpyKind kind_of(int dir) { return dir == HCL_H2D ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToHost; }
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------
+// FP64 issue-rate probe (hclooc_probe_fp64): independent chains of DMMA.8x8x4 (kind 0) or DFMA (kind 1) in registers,
+// no memory traffic -- the measured denominator of the roofline (148 SMs x 128 flop/clk x clock).
+namespace {
+__global__ void __launch_bounds__(256) probe_dmma_kernel(double* out, int iters) {
+    double c[8][2];
+    #pragma unroll
+    for (int i = 0; i < 8; ++i) { c[i][0] = 0.0; c[i][1] = 0.0; }
+    double a = 1.0 + 1e-9 * threadIdx.x, b = 1.0 - 1e-9 * threadIdx.x;
+    for (int it = 0; it < iters; ++it) {
+        #pragma unroll
+        for (int i = 0; i < 8; ++i)
+            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+                         : "+d"(c[i][0]), "+d"(c[i][1]) : "d"(a), "d"(b));
+    }
+    double s = 0.0;
+    #pragma unroll
+    for (int i = 0; i < 8; ++i) s += c[i][0] + c[i][1];
+    if (s == 123.456) out[0] = s;        // keep the chains alive
+}
+__global__ void __launch_bounds__(256) probe_dfma_kernel(double* out, int iters) {
+    double c[16];
+    #pragma unroll
+    for (int i = 0; i < 16; ++i) c[i] = 1e-3 * i;
+    const double a = 1.0 + 1e-9 * threadIdx.x, b = 1e-9 * threadIdx.x;
+    for (int it = 0; it < iters; ++it) {
+        #pragma unroll
+        for (int i = 0; i < 16; ++i) c[i] = __fma_rn(c[i], a, b);
+    }
+    double s = 0.0;
+    #pragma unroll
+    for (int i = 0; i < 16; ++i) s += c[i];
+    if (s == 123.456) out[0] = s;
+}
 }  // namespace
 
 extern "C" {
@@ -208,6 +245,39 @@ const char* hclooc_strerror(int status) {
         case HCLOOC_ERR_INTERNAL: return "internal invariant violated";
         default: return "unknown status";
     }
+}
+int hclooc_probe_fp64(int kind, int ctas_per_sm, double seconds, double* tflops) {
+    if (kind != 0 && kind != 1) return -1;
+    if (ctas_per_sm < 1 || ctas_per_sm > 8) return -2;
+    if (!(seconds > 0.0) || seconds > 30.0) return -3;
+    if (!tflops) return -4;
+    int dev = 0, sms = 0;
+    HCL_CUDA(cudaGetDevice(&dev));
+    HCL_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    double* d = nullptr;
+    HCL_CUDA(cudaMalloc(&d, 8));
+    cudaEvent_t e0, e1;
+    HCL_CUDA(cudaEventCreate(&e0));
+    HCL_CUDA(cudaEventCreate(&e1));
+    const int grid = sms * ctas_per_sm;
+    // flop per thread per iteration: DMMA: 8 chains x 512 flop per warp-wide instruction / 32 lanes; DFMA: 16 chains x 2
+    const double flop_it = (kind == 0 ? 8.0 * 512.0 / 32.0 : 32.0) * 256.0 * grid;
+    int iters = 1 << 14;
+    double best = 0.0, total = 0.0;
+    for (int rep = 0; rep < 64 && total < seconds; ++rep) {
+        cudaEventRecord(e0, 0);
+        if (kind == 0) probe_dmma_kernel<<<grid, 256>>>(d, iters); else probe_dfma_kernel<<<grid, 256>>>(d, iters);
+        cudaEventRecord(e1, 0);
+        cudaError_t e = cudaEventSynchronize(e1);
+        if (e != cudaSuccess) { cudaFree(d); return cuda_fail(e); }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0) { total += ms * 1e-3; best = std::max(best, flop_it * iters / (ms * 1e-3)); }
+        if (ms < 20.f && iters < (1 << 24)) iters *= 2;         // launches of >= 20 ms
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+    *tflops = best / 1e12;
+    return HCLOOC_OK;
 }
 const char* hclooc_version(void) { return "hclooc-b200 0.1 (sm_100a, DMMA tile kernel)"; }
 

@@ -821,3 +821,14 @@ def test_cluster_multicast_kernel_matches_tile_kernel(H, cm, cn, M, N, K, alpha,
     check(got[:, :N], ref, D, exact=(dist == "int"))
     assert np.isnan(got[:, N:]).all()
     assert np.array_equal(got[:, :N].view(np.uint64), one[:, :N].view(np.uint64))
+
+
+def test_fp64_probe_reports_the_dmma_rate(H):
+    """hclooc_probe_fp64: the measured denominator of the roofline (37.2 TFLOP/s on a B200)."""
+    dmma = H.hclooc_probe_fp64(0, 4, 0.3)
+    dfma = H.hclooc_probe_fp64(1, 4, 0.3)
+    assert 20.0 < dmma < 45.0 and 15.0 < dfma < 45.0, (dmma, dfma)
+    for args, want in (((2, 4, 0.3), -1), ((0, 9, 0.3), -2), ((0, 4, 0.0), -3)):
+        with pytest.raises(H.HclError) as e:
+            H.hclooc_probe_fp64(*args)
+        assert e.value.status == want
