@@ -229,6 +229,23 @@ int hclooc_dgemm_t(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N
                    const double* A, int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
                    size_t device_budget_bytes, hclooc_stats* stats_out);
 
+/* Out-of-core DSYRK on the same path (SURVEY 8(f) #3: "other level-3 BLAS out of core"; the paper's future work, :412):
+ *     C = alpha * A * A^T + beta * C   (trans = HCL_OP_N, A is N x K, lda >= K)
+ *     C = alpha * A^T * A + beta * C   (trans = HCL_OP_T, A is K x N, lda >= N)
+ * C is N x N symmetric and only its `uplo` triangle (HCL_UPLO_LOWER / HCL_UPLO_UPPER, diagonal included) is referenced: the
+ * other triangle is bit-for-bit what it was on return.  The triangle is cut into block columns (lower) or block rows (upper)
+ * of at most 4096 that start on the diagonal, each one call of the hclooc_dgemm_t pipeline with a triangle mask: the kernels
+ * skip tiles that lie wholly in the other triangle and store only the referenced elements of those that cross the diagonal,
+ * so about half the flops and C traffic of the corresponding DGEMM are spent.  C blocks that cross the diagonal are uploaded
+ * even when beta == 0 (their other-triangle part must come back unchanged); a NaN there is carried, never computed with.
+ * alpha == 0 or K == 0: C = beta*C on the triangle, A not referenced.  stats (nullable): sums over the block calls, plan of the
+ * last one.  Errors: -2 uplo, -3 trans, -4 N < 0, -5 K < 0, -7 A NULL, -8 lda too small, -10 C NULL or overlapping A,
+ * -11 ldc < N, and the HCLOOC_ERR_* codes of hclooc_dgemm.                                                              */
+#define HCL_UPLO_LOWER 0
+#define HCL_UPLO_UPPER 1
+int hclooc_dsyrk(hclooc_ctx* ctx, int uplo, int trans, int64_t N, int64_t K, double alpha, const double* A, int64_t lda,
+                 double beta, double* C, int64_t ldc, size_t device_budget_bytes, hclooc_stats* stats_out);
+
 /* nsteps mode (:277-283): MMOOC as a subroutine of a blocked algorithm (SUMMA, HSUMMA) that updates the same C
  * `nsteps` times: C = alpha*A_p*B_p + beta_p*C for p = *step = 0 .. nsteps-1, one call per p.  C is uploaded once
  * at step 0 (if beta != 0), stays in device memory between the calls, and is downloaded once at the last step, so

@@ -6,8 +6,8 @@ with the CUDA path in paper_1808_05056_b200/ and must never be imported by it: o
 __graft_entry__.smoke() and bench.py's cpu_baseline / `--impl reference` legs use it.
 
 Pinned by tests/test_oracle_pins.py (brute force, int64 exactness, closed forms, exact-sum error
-bound, numpy cross-check, the paper's 44-element partition example) -- nothing here is
-"parity unpinned".
+bound, numpy cross-check, the paper's 44-element partition example; dsyrk: brute force on the triangle,
+exact symmetry, int64 exactness, untouched other triangle) -- nothing here is "parity unpinned".
 """
 from __future__ import annotations
 
@@ -112,6 +112,28 @@ def dgemm_sub(alpha, A, B, beta, C0, rows=None, cols=None, want_denominator=True
     bp, ldb = _chk2d(B, "B") if B.size else (0, max(N, 1))
     cp, ldc = _chk2d(C0, "C0") if C0 is not None else (0, N)
     return dgemm_sub_ptr(M, N, K, alpha, ap, lda, bp, ldb, beta, cp, ldc, rows, cols, want_denominator)
+
+
+def dsyrk(uplo, trans, alpha, A, beta, C, want_denominator=False):
+    """The DSYRK definition on one triangle of C, in place (the BLAS operation the paper names as future work):
+        trans = 0: C_ij <- alpha * sum_k A_ik A_jk + beta * C_ij   (A is N x K)
+        trans = 1: C_ij <- alpha * sum_k A_ki A_kj + beta * C_ij   (A is K x N)
+    for j <= i (uplo = 0, lower) or j >= i (uplo = 1, upper); the other triangle is not referenced and keeps its bits.
+    It IS the DGEMM definition with op(B) = op(A)^T restricted to a triangle, so the step is `dgemm` above on a written-out
+    transpose (a copy, no arithmetic), then the triangle is taken.  Returns D on the triangle (0 elsewhere) when asked."""
+    N = C.shape[0]
+    assert C.shape == (N, N)
+    opA = np.empty((N, A.shape[0] if trans else A.shape[1]))
+    opA[...] = A.T if trans else A
+    opAt = np.empty((opA.shape[1], N))
+    opAt[...] = opA.T
+    full = C.copy()
+    D = dgemm(alpha, opA, opAt, beta, full, want_denominator=want_denominator)
+    keep = np.tril(np.ones((N, N), dtype=bool)) if uplo == 0 else np.triu(np.ones((N, N), dtype=bool))
+    C[keep] = full[keep]
+    if D is not None:
+        D[~keep] = 0.0
+    return D
 
 
 def partition(M, N, K, S):

@@ -204,9 +204,16 @@ __device__ __forceinline__ double axpby_tail(double alpha_acc, double beta, doub
 }
 
 // Fused epilogue: C = alpha*acc + beta*C straight from registers; C is not read when beta == 0.
+// tri != 0 (hclooc_dsyrk): only one triangle of C is referenced -- element (row, col) of this launch's C is stored iff
+// col <= row + doff (tri == 1, lower) or col >= row + doff (tri == 2, upper); doff places the launch's block on the diagonal.
+__device__ __forceinline__ bool tri_keep(int tri, int doff, int row, int col) {
+    return tri == 0 || (tri == 1 ? col <= row + doff : col >= row + doff);
+}
+
 template <bool TA, bool TB>
 __device__ __forceinline__ void epilogue_store(const double (&acc)[4][4][2][2], double* __restrict__ C, long long ldc,
-                                               int M, int N, int m0, int n0, double alpha, double beta, const FragLanesT<TA, TB>& f) {
+                                               int M, int N, int m0, int n0, double alpha, double beta, const FragLanesT<TA, TB>& f,
+                                               int tri = 0, int doff = 0) {
     const bool read_c = (beta != 0.0);
     const bool vec_ok = ((ldc & 1LL) == 0) && ((reinterpret_cast<uintptr_t>(C) & 15u) == 0);
     // 256-bit accesses (sm_100: LDG/STG.256): a lane's 4 consecutive columns are one 32-byte sector, a quarter warp's
@@ -225,7 +232,15 @@ __device__ __forceinline__ void epilogue_store(const double (&acc)[4][4][2][2], 
                 // lane holds 4 consecutive columns: (v=0,c0) (v=1,c0) (v=0,c1) (v=1,c1)
                 double x0 = __dmul_rn(alpha, acc[u][bx][0][0]), x1 = __dmul_rn(alpha, acc[u][bx][1][0]);
                 double x2 = __dmul_rn(alpha, acc[u][bx][0][1]), x3 = __dmul_rn(alpha, acc[u][bx][1][1]);
-                if (col + 3 < N && vec4_ok) {
+                const bool keep_lo = tri_keep(tri, doff, row, col), keep_hi = tri_keep(tri, doff, row, col + 3);
+                if (!keep_lo && !keep_hi) continue;                      // the four columns lie in the other triangle
+                const bool keep_all = keep_lo && keep_hi;
+                if (!keep_all) {
+                    const double xs[4] = {x0, x1, x2, x3};
+                    #pragma unroll
+                    for (int q = 0; q < 4; ++q)
+                        if (col + q < N && tri_keep(tri, doff, row, col + q)) crow[col + q] = read_c ? axpby_tail(xs[q], beta, crow[col + q]) : xs[q];
+                } else if (col + 3 < N && vec4_ok) {
                     double* p = crow + col;
                     if (read_c) {
                         double c0, c1, c2, c3;
@@ -257,7 +272,7 @@ __device__ __forceinline__ void epilogue_store(const double (&acc)[4][4][2][2], 
                     for (int c = 0; c < 2; ++c) {
                         const int col = n0 + f.wn * 64 + (2 * bx + v) * 8 + f.t + 4 * c;
                         const double x = __dmul_rn(alpha, acc[u][bx][v][c]);
-                        if (col < N) crow[col] = read_c ? axpby_tail(x, beta, crow[col]) : x;
+                        if (col < N && tri_keep(tri, doff, row, col)) crow[col] = read_c ? axpby_tail(x, beta, crow[col]) : x;
                     }
             }
         }

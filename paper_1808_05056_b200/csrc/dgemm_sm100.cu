@@ -41,7 +41,7 @@ template <int KSPLIT, bool TA = false, bool TB = false>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 hclooc_dgemm_tile_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                          double* __restrict__ C, long long ldc, int M, int N, int K,
-                         double alpha, double beta, int tiles_m, int tiles_n) {
+                         double alpha, double beta, int tiles_m, int tiles_n, int tri, int doff) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;   // 128B swizzle wants 1 KiB alignment
     const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;          // full[s] at +8s, empty[s] at +8(STAGES+s)
@@ -52,6 +52,10 @@ hclooc_dgemm_tile_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_c
     tile_coords((KSPLIT == 1) ? (int)blockIdx.x : (int)(blockIdx.x / KSPLIT), tiles_m, tiles_n, tile_m, tile_n);
     const int m0 = tile_m * BM;
     const int n0 = tile_n * BN;
+    // hclooc_dsyrk: a tile that lies entirely in the triangle of C that is not referenced has nothing to do (every CTA of a
+    // split-K cluster shares the tile, so the whole cluster leaves together, before any barrier exists)
+    if (tri == 1 && n0 > min(m0 + BM, M) - 1 + doff) return;
+    if (tri == 2 && min(n0 + BN, N) - 1 < m0 + doff) return;
     const int num_kb_all = (K + BK - 1) / BK;
     const uint32_t crank = (KSPLIT == 1) ? 0u : cluster_ctarank();
     const int kb_begin = (KSPLIT == 1) ? 0 : (int)(((long long)num_kb_all * crank) / KSPLIT);
@@ -181,7 +185,7 @@ hclooc_dgemm_tile_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_c
     }
 
     // ---------------------------------------------------------------- fused epilogue
-    epilogue_store(acc, C, ldc, M, N, m0, n0, alpha, beta, f);
+    epilogue_store(acc, C, ldc, M, N, m0, n0, alpha, beta, f, tri, doff);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -248,7 +252,7 @@ int ensure_kernel_attr() {
 
 template <int KSPLIT, bool TA, bool TB>
 cudaError_t launch_split(unsigned tiles, cudaStream_t stream, const CUtensorMap& tmA, const CUtensorMap& tmB, double* dC,
-                         long long ldc, int M, int N, int K, double alpha, double beta, int tm, int tn) {
+                         long long ldc, int M, int N, int K, double alpha, double beta, int tm, int tn, int tri, int doff) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(tiles * KSPLIT, 1, 1);
     cfg.blockDim = dim3(NUM_THREADS, 1, 1);
@@ -261,15 +265,15 @@ cudaError_t launch_split(unsigned tiles, cudaStream_t stream, const CUtensorMap&
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, hclooc_dgemm_tile_kernel<KSPLIT, TA, TB>, tmA, tmB, dC, ldc, M, N, K, alpha, beta, tm, tn);
+    return cudaLaunchKernelEx(&cfg, hclooc_dgemm_tile_kernel<KSPLIT, TA, TB>, tmA, tmB, dC, ldc, M, N, K, alpha, beta, tm, tn, tri, doff);
 }
 
 template <bool TA, bool TB>
 cudaError_t launch_any_split(int ksplit, unsigned tiles, cudaStream_t stream, const CUtensorMap& tmA, const CUtensorMap& tmB, double* dC,
-                             long long ldc, int M, int N, int K, double alpha, double beta, int tm, int tn) {
-    if (ksplit >= 4) return launch_split<4, TA, TB>(tiles, stream, tmA, tmB, dC, ldc, M, N, K, alpha, beta, tm, tn);
-    if (ksplit >= 2) return launch_split<2, TA, TB>(tiles, stream, tmA, tmB, dC, ldc, M, N, K, alpha, beta, tm, tn);
-    hclooc_dgemm_tile_kernel<1, TA, TB><<<tiles, NUM_THREADS, SMEM_BYTES, stream>>>(tmA, tmB, dC, ldc, M, N, K, alpha, beta, tm, tn);
+                             long long ldc, int M, int N, int K, double alpha, double beta, int tm, int tn, int tri, int doff) {
+    if (ksplit >= 4) return launch_split<4, TA, TB>(tiles, stream, tmA, tmB, dC, ldc, M, N, K, alpha, beta, tm, tn, tri, doff);
+    if (ksplit >= 2) return launch_split<2, TA, TB>(tiles, stream, tmA, tmB, dC, ldc, M, N, K, alpha, beta, tm, tn, tri, doff);
+    hclooc_dgemm_tile_kernel<1, TA, TB><<<tiles, NUM_THREADS, SMEM_BYTES, stream>>>(tmA, tmB, dC, ldc, M, N, K, alpha, beta, tm, tn, tri, doff);
     return cudaGetLastError();
 }
 
@@ -286,7 +290,7 @@ int dgemm_auto_ksplit(int64_t tiles_in_flight, int64_t K) {
 
 int launch_dgemm_tiles(int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda,
                        const double* dB, int64_t ldb, double beta, double* dC, int64_t ldc, cudaStream_t stream,
-                       int ksplit, void* streamk_scratch, int transa, int transb) {
+                       int ksplit, void* streamk_scratch, int transa, int transb, int tri, int doff) {
     if (M == 0 || N == 0) return HCLOOC_OK;
     if (alpha == 0.0) K = 0;                       // A and B are not referenced (BLAS convention)
     int rc = ensure_kernel_attr();
@@ -303,6 +307,8 @@ int launch_dgemm_tiles(int64_t M, int64_t N, int64_t K, double alpha, const doub
     const int64_t tm = (M + BM - 1) / BM, tn = (N + BN - 1) / BN;
     if (tm * tn > 0x7fffffffLL || M > 0x7fffffffLL || N > 0x7fffffffLL || K > 0x7fffffffLL) return HCLOOC_ERR_INTERNAL;
     static const bool no_streamk = getenv("HCLOOC_NO_STREAMK") != nullptr;   // experiment knob
+    if (tri != 0 && (doff > 0x3fffffff || doff < -0x3fffffff)) return HCLOOC_ERR_INTERNAL;
+    if (ksplit < 0 && tri != 0) ksplit = 0;                    // the persistent kernel has no triangle mask
     if (ksplit < 0 && K > 0 && !no_streamk) {
         // A launch that has the GPU to itself.  One CTA per tile runs its main loop ~1 % faster than the persistent
         // kernel (measured 0.981 against 0.969 of peak on whole waves) but leaves the last wave partly empty, so
@@ -319,10 +325,10 @@ int launch_dgemm_tiles(int64_t M, int64_t N, int64_t K, double alpha, const doub
     if (K == 0) ksplit = 1;
     const unsigned tiles = (unsigned)(tm * tn);
     cudaError_t e;
-    if (transa && transb) e = launch_any_split<true, true>(ksplit, tiles, stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn);
-    else if (transa) e = launch_any_split<true, false>(ksplit, tiles, stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn);
-    else if (transb) e = launch_any_split<false, true>(ksplit, tiles, stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn);
-    else e = launch_any_split<false, false>(ksplit, tiles, stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn);
+    if (transa && transb) e = launch_any_split<true, true>(ksplit, tiles, stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn, tri, doff);
+    else if (transa) e = launch_any_split<true, false>(ksplit, tiles, stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn, tri, doff);
+    else if (transb) e = launch_any_split<false, true>(ksplit, tiles, stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn, tri, doff);
+    else e = launch_any_split<false, false>(ksplit, tiles, stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn, tri, doff);
     if (e != cudaSuccess) return cuda_fail(e);
     return HCLOOC_OK;
 }

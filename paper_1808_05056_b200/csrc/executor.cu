@@ -352,9 +352,12 @@ int copy2d(void* dst, size_t dpitch, const void* src, size_t spitch, size_t widt
 
 namespace {
 
+// tri != 0 (hclooc_dsyrk): only the lower (1) / upper (2) triangle of this call's C, whose element (0, 0) lies on the diagonal,
+// is referenced.  The kernels skip the other triangle; its elements still ride along in the C blocks that cross the
+// diagonal, which is why such a call uploads its C blocks even when beta == 0 (they come back unchanged).
 int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
                int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
-               size_t device_budget_bytes, hclooc_stats* stats) {
+               size_t device_budget_bytes, hclooc_stats* stats, int tri = 0) {
     const auto t_begin = std::chrono::steady_clock::now();
     // ---------------------------------------------------------------- S0 validate (argument numbers of hclooc_dgemm)
     if (M < 0) return -1;
@@ -410,12 +413,12 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
         static std::once_flag once;
         std::call_once(once, [] { set_planner_max_cluster(direct_max_cluster()); });
     }
-    const bool direct_ok = !in_core && !c_dev && aligned && direct_mode != 0 && M <= 0x7fffffffLL && N <= 0x7fffffffLL && K <= 0x7fffffffLL &&
+    const bool direct_ok = !in_core && !c_dev && aligned && direct_mode != 0 && tri == 0 && M <= 0x7fffffffLL && N <= 0x7fffffffLL && K <= 0x7fffffffLL &&
                            C_alias && (((uintptr_t)C_alias & 15u) == 0) &&
                            (scale_only || (A_alias && B_alias && ((((uintptr_t)A_alias | (uintptr_t)B_alias) & 15u) == 0)));
     {
         const int where = in_core ? 1 : (c_dev ? 2 : (direct_ok ? (direct_mode == 1 ? 4 : 3) : 0));
-        const hclooc_ctx::PlanKey key{M, N, K, beta != 0.0, alpha == 0.0, where + (transa ? 8 : 0) + (transb ? 16 : 0), budget};
+        const hclooc_ctx::PlanKey key{M, N, K, beta != 0.0 || tri != 0, alpha == 0.0, where + (transa ? 8 : 0) + (transb ? 16 : 0), budget};
         bool hit = false;
         for (const auto& kv : ctx->plan_cache) {
             const hclooc_ctx::PlanKey& k = kv.first;
@@ -438,7 +441,7 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
             rc = launch_dgemm_direct(M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, ctx->s_compute[0], P.direct_cm, P.direct_cn);
         else
             rc = launch_dgemm_tiles(M, N, scale_only ? 0 : K, scale_only ? 0.0 : alpha, A, lda, B, ldb, beta, C, ldc, ctx->s_compute[0], P.direct ? 1 : -1,
-                                    nullptr, transa, transb);
+                                    nullptr, transa, transb, tri, 0);
         const auto t1 = std::chrono::steady_clock::now();
         cudaError_t e = cudaStreamSynchronize(ctx->s_compute[0]);
         if (rc) return rc;
@@ -505,7 +508,7 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
     if (use_graph) {
         union { double d; int64_t i; } ua{alpha}, ub{beta};
         key = {M, N, K, ua.i, ub.i, (int64_t)(uintptr_t)A, lda, (int64_t)(uintptr_t)B, ldb, (int64_t)(uintptr_t)C, ldc,
-               (int64_t)(uintptr_t)base, (int64_t)P.workspace_bytes, P.mb, P.nb, P.kb, P.n_sets, P.n_abuf, P.n_bbuf, P.ksplit, transa, transb};
+               (int64_t)(uintptr_t)base, (int64_t)P.workspace_bytes, P.mb, P.nb, P.kb, P.n_sets, P.n_abuf, P.n_bbuf, P.ksplit, transa, transb, tri};
         if (key != ctx->graph_key) {
             // first time this call is seen: run it the ordinary way, capture it if it comes again
             ctx->graph_key = key;
@@ -596,7 +599,8 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
                 const double b_eff = (o.beta < 0.0) ? beta : o.beta;
                 rc = launch_dgemm_tiles(o.nr, o.nc, o.kk, scale_only ? 0.0 : alpha, o.buf >= 0 ? bufs[o.buf] : nullptr, P.lda_dev,
                                         o.buf2 >= 0 ? bufs[o.buf2] : nullptr, P.ldb_dev, b_eff, bufs[o.buf3], P.ldc_dev, st,
-                                        P.ksplit != 0 ? P.ksplit : 1, P.ksplit < 0 ? scratch[o.stream - 2] : nullptr, transa, transb);
+                                        P.ksplit != 0 ? P.ksplit : 1, P.ksplit < 0 ? scratch[o.stream - 2] : nullptr, transa, transb,
+                                        tri, (int)(o.r0 - o.c0));
                 ++n_kernels;
                 break;
             }
@@ -683,6 +687,53 @@ extern "C" int hclooc_dgemm_t(hclooc_ctx* ctx, int transa, int transb, int64_t M
     if (transa != HCL_OP_N && transa != HCL_OP_T) return -15;
     if (transb != HCL_OP_N && transb != HCL_OP_T) return -16;
     return dgemm_core(ctx, transa, transb, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes, stats);
+}
+
+// Out-of-core DSYRK on top of the DGEMM path: the referenced triangle is cut into block columns (lower) or block rows
+// (upper) of `nbs` columns / rows that start on the diagonal; each is one call of the pipeline with the triangle mask.
+extern "C" int hclooc_dsyrk(hclooc_ctx* ctx, int uplo, int trans, int64_t N, int64_t K, double alpha, const double* A, int64_t lda,
+                            double beta, double* C, int64_t ldc, size_t device_budget_bytes, hclooc_stats* stats) {
+    const auto t_begin = std::chrono::steady_clock::now();
+    if (uplo != HCL_UPLO_LOWER && uplo != HCL_UPLO_UPPER) return -2;
+    if (trans != HCL_OP_N && trans != HCL_OP_T) return -3;
+    if (N < 0) return -4;
+    if (K < 0) return -5;
+    if (stats) std::memset(stats, 0, sizeof(*stats));
+    if (N == 0) return HCLOOC_OK;
+    const bool scale_only = (alpha == 0.0 || K == 0);
+    if (!scale_only) {
+        if (!A) return -7;
+        if (lda < (trans ? N : K)) return -8;
+    }
+    if (!C) return -10;
+    if (ldc < N) return -11;
+    if (scale_only && beta == 1.0) return HCLOOC_OK;
+    // block width: wide enough that a block column is compute-bound (flops per uploaded byte ~ nbs / 4) and the part of the
+    // diagonal blocks computed for nothing stays small (tiles wholly in the other triangle are skipped by the kernel)
+    const int64_t nbs = std::min<int64_t>(N, 4096);
+    hclooc_stats acc, one;
+    std::memset(&acc, 0, sizeof(acc));
+    for (int64_t j0 = 0; j0 < N; j0 += nbs) {
+        const int64_t nj = std::min(nbs, N - j0), rest = N - j0;
+        // lower: C[j0:N, j0:j0+nj] = alpha*op(A)[j0:N, :] * op(A)[j0:j0+nj, :]^T + beta*C   (M' = rest, N' = nj)
+        // upper: C[j0:j0+nj, j0:N] = alpha*op(A)[j0:j0+nj, :] * op(A)[j0:N, :]^T + beta*C   (M' = nj, N' = rest)
+        const int64_t Mc = uplo == HCL_UPLO_LOWER ? rest : nj, Nc = uplo == HCL_UPLO_LOWER ? nj : rest;
+        const double* Ab = scale_only ? nullptr : (trans ? A + j0 : A + j0 * lda);      // op(A) rows j0.. : both operands start here
+        // trans == N: A is N x K: left operand as stored, right operand = stored rows read transposed (transb)
+        // trans == T: A is K x N: left operand = stored columns read transposed (transa), right operand as stored
+        int rc = dgemm_core(ctx, trans ? 1 : 0, trans ? 0 : 1, Mc, Nc, K, alpha, Ab, lda, Ab, lda, beta, C + j0 * ldc + j0, ldc,
+                            device_budget_bytes, &one, uplo == HCL_UPLO_LOWER ? 1 : 2);
+        if (rc) return rc;
+        acc.plan = one.plan;
+        acc.bytes_h2d += one.bytes_h2d; acc.bytes_d2h += one.bytes_d2h;
+        acc.n_kernels += one.n_kernels; acc.n_copies_h2d += one.n_copies_h2d; acc.n_copies_d2h += one.n_copies_d2h;
+        acc.t_enqueue_s += one.t_enqueue_s;
+    }
+    if (stats) {
+        *stats = acc;
+        stats->t_total_s = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_begin).count();
+    }
+    return HCLOOC_OK;
 }
 
 extern "C" int hclooc_dgemm(int64_t M, int64_t N, int64_t K, double alpha, const double* A, int64_t lda,

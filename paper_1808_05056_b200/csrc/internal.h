@@ -38,7 +38,8 @@ int launch_dgemm_tiles(int64_t M, int64_t N, int64_t K, double alpha, const doub
                        cudaStream_t stream, int ksplit,    // ksplit: 1, 2, 4; 0 = choose from the tile count;
                        void* streamk_scratch = nullptr,    // -1 = the launch has the GPU to itself: persistent stream-K
                                                            //      (scratch: streamk_scratch_bytes(), or NULL = library pool)
-                       int transa = 0, int transb = 0);    // dA is stored K x M / dB is stored N x K (hclooc_dgemm_t)
+                       int transa = 0, int transb = 0,     // dA is stored K x M / dB is stored N x K (hclooc_dgemm_t)
+                       int tri = 0, int doff = 0);         // hclooc_dsyrk: store only col <= row + doff (1) / col >= row + doff (2)
 
 // The persistent stream-K kernel (dgemm_streamk_sm100.cu).  Returns 1 if it does not apply (no scratch buffer
 // free, shape out of range): the caller then launches one CTA per tile.

@@ -832,3 +832,66 @@ def test_fp64_probe_reports_the_dmma_rate(H):
         with pytest.raises(H.HclError) as e:
             H.hclooc_probe_fp64(*args)
         assert e.value.status == want
+
+
+# ------------------------------------------------------------------ out-of-core DSYRK on the same path
+@pytest.mark.parametrize("uplo", [0, 1])
+@pytest.mark.parametrize("trans", [0, 1])
+@pytest.mark.parametrize("N,K,alpha,beta,dist,pad,budget", [
+    (300, 200, 1.0, 0.5, "uniform", 0, 1 * MiB),
+    (517, 389, 2.0, -1.0, "int", 3, 2 * MiB),
+    (129, 33, -1.5, 0.0, "int", 1, 1 * MiB),              # beta == 0: blocks crossing the diagonal are still uploaded
+    (1, 1, 2.0, 0.5, "int", 1, 1 * MiB),
+    (1300, 260, 1.0, 1.0, "normal", 2, 64 * MiB),
+    (96, 20000, 2.0, -1.0, "int", 0, 900 * 1024),          # K panels
+])
+def test_dsyrk_matches_oracle_and_leaves_the_other_triangle(H, uplo, trans, N, K, alpha, beta, dist, pad, budget):
+    ar, ac = (K, N) if trans else (N, K)
+    A = H.HostMatrix(ar, ac, ac + pad); C = H.HostMatrix(N, N, N + pad)
+    A.array[...] = np.nan; C.array[...] = np.nan
+    synthgen.fill(A.array, 81, "A", dist, cols=ac); synthgen.fill(C.array, 81, "C", dist, cols=N)
+    other = np.triu(np.ones((N, N), bool), 1) if uplo == 0 else np.tril(np.ones((N, N), bool), -1)
+    if beta == 0.0:
+        C.view[~other] = np.nan                            # the referenced triangle must not be read
+    marker = C.view.copy()
+    marker[other] = np.arange(int(other.sum())) + 0.25      # recognisable values in the triangle that is not referenced
+    C.view[...] = marker
+    ref = np.where(np.isnan(marker), 0.0, marker) if beta == 0.0 else marker.copy()
+    D = oracle.dsyrk(uplo, trans, alpha, A.view.copy(), beta, ref, want_denominator=True)
+    st = H.hclooc_dsyrk(None, uplo, trans, N, K, alpha, A, A.ld, beta, C, C.ld, budget)
+    assert st.n_kernels >= 1 and st.plan.workspace_bytes <= budget
+    got = C.view.copy()
+    assert np.array_equal(got[other], marker[other])                               # untouched, bit for bit
+    keep = ~other
+    gk, rk = got.copy(), ref.copy()
+    gk[other] = 0.0; rk[other] = 0.0
+    D[other] = 1.0
+    check(gk, rk, D, exact=(dist == "int"))
+    assert np.isnan(C.array[:, N:]).all()
+
+
+def test_dsyrk_large_blocks_symmetry_and_errors(H):
+    """N > 4096: several block columns / rows; lower and upper results are transposes of each other bit for bit; the
+    sampled rows agree with the oracle; argument errors."""
+    N, K = 5000, 300
+    A = H.HostMatrix(N, K); synthgen.fill(A.array, 82, "A", "uniform")
+    lo, up = H.HostMatrix(N, N), H.HostMatrix(N, N)
+    lo.view[...] = 0.0; up.view[...] = 0.0
+    st = H.hclooc_dsyrk(None, H.HCL_UPLO_LOWER, H.HCL_OP_N, N, K, 1.0, A, K, 0.0, lo, N, 256 * MiB)
+    H.hclooc_dsyrk(None, H.HCL_UPLO_UPPER, H.HCL_OP_N, N, K, 1.0, A, K, 0.0, up, N, 256 * MiB)
+    assert st.n_kernels >= 2
+    assert np.array_equal(np.tril(lo.view), np.triu(up.view).T)
+    assert not np.triu(lo.view, 1).any() and not np.tril(up.view, -1).any()
+    rows = np.array([0, 1, 127, 128, 4095, 4096, 4097, N - 1])
+    Bt = np.empty((K, N)); Bt[...] = A.view.T
+    ref, D = oracle.dgemm_sub(1.0, A.view, Bt, 0.0, None, rows=rows)
+    for q, i in enumerate(rows):
+        ok, worst = oracle.within_gate(lo.view[i, : i + 1], ref[q, : i + 1], D[q, : i + 1], RTOL)
+        assert ok, (i, worst)
+    for args, want in (((2, 0, N, K, 1.0, A, K, 0.0, lo, N), -2), ((0, 2, N, K, 1.0, A, K, 0.0, lo, N), -3),
+                       ((0, 0, -1, K, 1.0, A, K, 0.0, lo, N), -4), ((0, 0, N, K, 1.0, None, K, 0.0, lo, N), -7),
+                       ((0, 0, N, K, 1.0, A, K - 1, 0.0, lo, N), -8), ((0, 1, N, K, 1.0, A, N - 1, 0.0, lo, N), -8),
+                       ((0, 0, N, K, 1.0, A, K, 0.0, None, N), -10), ((0, 0, N, K, 1.0, A, K, 0.0, lo, N - 1), -11)):
+        with pytest.raises(H.HclError) as e:
+            H.hclooc_dsyrk(None, *args, 256 * MiB)
+        assert e.value.status == want, (args[:2], e.value.status)

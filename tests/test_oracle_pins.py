@@ -291,3 +291,60 @@ def test_generator_c_and_numpy_twins_agree(dist):
         assert whole.min() >= -1.0 and whole.max() < 1.0 and abs(whole.mean()) < 0.02
     if dist == "normal":
         assert abs(whole.mean()) < 0.03 and abs(whole.std() - 1.0) < 0.03
+
+
+# ------------------------------------------------------------------ dsyrk (the definition restricted to a triangle)
+@pytest.mark.parametrize("uplo", [0, 1])
+@pytest.mark.parametrize("trans", [0, 1])
+def test_dsyrk_brute_force_and_untouched_triangle(uplo, trans):
+    """Pure-Python loops over the referenced triangle in the order of the definition (in-order sum of separately rounded
+    products, then alpha*acc + beta*c): bit-identical; the other triangle keeps its bits (NaN there stays NaN and is never
+    computed with)."""
+    rng = np.random.default_rng(7 + 2 * uplo + trans)
+    for N, K in ((1, 1), (4, 3), (5, 9), (7, 2), (6, 0)):
+        A = rng.uniform(-1, 1, (K, N) if trans else (N, K))
+        C0 = rng.uniform(-1, 1, (N, N))
+        other = np.triu(np.ones((N, N), bool), 1) if uplo == 0 else np.tril(np.ones((N, N), bool), -1)
+        C0[other] = np.nan
+        C = C0.copy()
+        oracle.dsyrk(uplo, trans, 1.5, A, -0.5, C)
+        for i in range(N):
+            for j in range(N):
+                if other[i, j]:
+                    assert np.isnan(C[i, j])
+                    continue
+                acc = 0.0
+                for k in range(K):
+                    acc = acc + ((A[k, i] * A[k, j]) if trans else (A[i, k] * A[j, k]))
+                want = 1.5 * acc + (-0.5) * C0[i, j]
+                assert C[i, j] == want and np.signbit(C[i, j]) == np.signbit(want), (N, K, i, j)
+
+
+def test_dsyrk_symmetry_integers_and_closed_forms():
+    rng = np.random.default_rng(11)
+    N, K = 37, 53
+    A = rng.integers(-4, 5, (N, K)).astype(np.float64)
+    S = rng.integers(-4, 5, (N, N)).astype(np.float64)
+    S = np.tril(S) + np.tril(S, -1).T                                   # symmetric C0
+    lo, up = S.copy(), S.copy()
+    oracle.dsyrk(0, 0, 2.0, A, 0.5, lo)
+    oracle.dsyrk(1, 0, 2.0, A, 0.5, up)
+    # exact in int64 (scaled by 2 for the half-integer beta), and lower == upper^T: a_ik*a_jk commutes, same k order
+    exact2 = 4 * (A.astype(np.int64) @ A.astype(np.int64).T) + S.astype(np.int64)
+    assert np.array_equal(np.tril(lo) * 2, np.tril(exact2).astype(np.float64))
+    assert np.array_equal(np.tril(lo), np.triu(up).T)
+    assert np.array_equal(np.triu(lo, 1), np.triu(S, 1)) and np.array_equal(np.tril(up, -1), np.tril(S, -1))
+    # trans: A^T A of the K x N matrix A^T is the same product
+    lo_t = S.copy()
+    oracle.dsyrk(0, 1, 2.0, np.ascontiguousarray(A.T), 0.5, lo_t)
+    assert np.array_equal(lo_t, lo)
+    # rows of A orthonormal (a permutation of unit vectors): A A^T = I
+    P = np.eye(9)[rng.permutation(9)][:6]
+    C = np.full((6, 6), 3.0)
+    oracle.dsyrk(0, 0, 2.0, P, 1.0, C)
+    assert np.array_equal(np.tril(C), np.tril(2.0 * np.eye(6) + 3.0)) and np.array_equal(np.triu(C, 1), np.triu(np.full((6, 6), 3.0), 1))
+    # rank 1: C_ij = alpha*u_i*u_j with exactly that rounding sequence; float symmetry holds bit for bit
+    u = rng.uniform(-1, 1, (8, 1))
+    lo1, up1 = np.zeros((8, 8)), np.zeros((8, 8))
+    oracle.dsyrk(0, 0, 1.25, u, 0.0, lo1); oracle.dsyrk(1, 0, 1.25, u, 0.0, up1)
+    assert np.array_equal(np.tril(lo1), np.tril(1.25 * (u * u.T))) and np.array_equal(np.tril(lo1), np.triu(up1).T)
