@@ -91,6 +91,10 @@ typedef struct hclooc_plan_t {
                                      tiles) that share their loads by TMA multicast -- A is read ceil(ceil(N/128)/direct_cn)
                                      times and B ceil(ceil(M/128)/direct_cm) times; 4 x 4 (one 16-CTA cluster) makes
                                      config 1's traffic the compulsory minimum                                      */
+    int32_t  tri;                 /* hclooc_dsyrk: 1 / 2 = only the lower / upper triangle of C is referenced; the schedule has no
+                                     step for a block that lies wholly in the other triangle, and bytes_* / n_copies_* are
+                                     those of the schedule (set by the executor; the planner leaves tri = 0)           */
+    int32_t  reserved2;
     int32_t  trans;               /* hclooc_dgemm_t: bit 0 = A is stored K x M, bit 1 = B is stored N x K.  The device
                                      slices keep the stored layout: an A slice is then kb x mb (lda_dev >= mb), a B
                                      slice nb x kb (ldb_dev >= kb), and the tile kernel reads them transposed       */
@@ -233,13 +237,12 @@ int hclooc_dgemm_t(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N
  *     C = alpha * A * A^T + beta * C   (trans = HCL_OP_N, A is N x K, lda >= K)
  *     C = alpha * A^T * A + beta * C   (trans = HCL_OP_T, A is K x N, lda >= N)
  * C is N x N symmetric and only its `uplo` triangle (HCL_UPLO_LOWER / HCL_UPLO_UPPER, diagonal included) is referenced: the
- * other triangle is bit-for-bit what it was on return.  The triangle is cut into block columns (lower) or block rows (upper)
- * of at most 4096 that start on the diagonal, each one call of the hclooc_dgemm_t pipeline with a triangle mask: the kernels
- * skip tiles that lie wholly in the other triangle and store only the referenced elements of those that cross the diagonal,
- * so about half the flops and C traffic of the corresponding DGEMM are spent.  C blocks that cross the diagonal are uploaded
+ * other triangle is bit-for-bit what it was on return.  It is one pass of the hclooc_dgemm_t pipeline with a triangle mask
+ * (plan.tri): the schedule has no step for a block of C that lies wholly in the other triangle, the kernels skip such tiles
+ * inside the blocks that cross the diagonal and store only their referenced elements, so about half the flops and half the
+ * C traffic of the corresponding DGEMM are spent.  C blocks that cross the diagonal are uploaded
  * even when beta == 0 (their other-triangle part must come back unchanged); a NaN there is carried, never computed with.
- * alpha == 0 or K == 0: C = beta*C on the triangle, A not referenced.  stats (nullable): sums over the block calls, plan of the
- * last one.  Errors: -2 uplo, -3 trans, -4 N < 0, -5 K < 0, -7 A NULL, -8 lda too small, -10 C NULL or overlapping A,
+ * alpha == 0 or K == 0: C = beta*C on the triangle, A not referenced.  stats (nullable) as hclooc_dgemm_ex.  Errors: -2 uplo, -3 trans, -4 N < 0, -5 K < 0, -7 A NULL, -8 lda too small, -10 C NULL or overlapping A,
  * -11 ldc < N, and the HCLOOC_ERR_* codes of hclooc_dgemm.                                                              */
 #define HCL_UPLO_LOWER 0
 #define HCL_UPLO_UPPER 1

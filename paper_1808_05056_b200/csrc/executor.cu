@@ -165,18 +165,33 @@ void build_schedule(const hclooc_plan_t& P, int ncs, std::vector<hclooc_op_t>& o
 
     // With one B buffer the uploads of the first steps of a column go out BEFORE the B reload, so the link
     // has work while the kernels of the previous column drain (the paper leaves that reload exposed, :236-242).
-    const int64_t pre = (P.n_bbuf == 1 && !scale_only) ? early_uploads(P.h, n_sets, n_abuf) : 0;
+    // plan.tri (hclooc_dsyrk): blocks that lie wholly in the triangle of C that is not referenced are not steps at all --
+    // no upload, no kernel, no download.  A column's steps are its LIVE blocks, in serpentine order.
+    auto in_triangle = [&](int64_t i, int64_t j) {
+        if (P.tri == 0) return true;
+        const int64_t r0 = i * P.mb, r1 = std::min(P.M, r0 + P.mb), c0 = j * P.nb, c1 = std::min(P.N, c0 + P.nb);
+        return P.tri == 1 ? c0 <= r1 - 1 : c1 - 1 >= r0;
+    };
     std::vector<Step> early;
+    std::vector<int64_t> live;
     int64_t seq = 0;
     for (int64_t sl = 0; sl < slabs; ++sl) {
         const int64_t p = sl / P.w, j = sl % P.w;
         const int64_t kk = scale_only ? 0 : std::min(P.kb, P.K - p * P.kb);
         const int b = (int)(sl % P.n_bbuf);
+        live.clear();
+        for (int64_t t = 0; t < P.h; ++t)
+            if (in_triangle((sl & 1) ? P.h - 1 - t : t, j)) live.push_back(t);
+        if (live.empty()) live.push_back(0);              // keeps the B slice chain intact; the kernel skips its tiles
+        const int64_t hl = (int64_t)live.size();
+        // With one B buffer the uploads of the first steps of a column go out BEFORE the B reload, so the link
+        // has work while the kernels of the previous column drain (the paper leaves that reload exposed, :236-242).
+        const int64_t pre = (P.n_bbuf == 1 && !scale_only) ? early_uploads(hl, n_sets, n_abuf) : 0;
         early.clear();
         if (!scale_only && (P.n_bbuf == 1 || sl == 0)) {
             if (sl > 0) {
-                for (int64_t t = 0; t < pre; ++t) {
-                    early.push_back(make_step(sl, t, seq + t));
+                for (int64_t q = 0; q < pre; ++q) {
+                    early.push_back(make_step(sl, live[q], seq + q));
                     issue_uploads(early.back());
                 }
                 wait_all_kernels(0);             // S(b_j) overwrites the single buffer: every kernel of the previous column is done
@@ -189,19 +204,19 @@ void build_schedule(const hclooc_plan_t& P, int ncs, std::vector<hclooc_op_t>& o
         const int64_t np = (sl + 1) / P.w, nj_idx = (sl + 1) % P.w;
         const int64_t nkk = prefetch ? std::min(P.kb, P.K - np * P.kb) : 0;
         int64_t pf_i0 = 0, nchunks = 0;
-        if (prefetch) prefetch_layout(P.h, nkk, n_sets, &pf_i0, &nchunks);
+        if (prefetch) prefetch_layout(hl, nkk, n_sets, &pf_i0, &nchunks);
         const int nb_buf = (int)((sl + 1) % P.n_bbuf);
-        for (int64_t t = 0; t < P.h; ++t, ++seq) {
-            Step s = (t < (int64_t)early.size()) ? early[t] : make_step(sl, t, seq);
-            const bool any = (t < (int64_t)early.size()) ? s.uploaded : issue_uploads(s);
-            if (prefetch && t >= pf_i0 && t < pf_i0 + nchunks) {
-                const int64_t ci = t - pf_i0;
+        for (int64_t q = 0; q < hl; ++q, ++seq) {
+            Step s = (q < (int64_t)early.size()) ? early[q] : make_step(sl, live[q], seq);
+            const bool any = (q < (int64_t)early.size()) ? s.uploaded : issue_uploads(s);
+            if (prefetch && q >= pf_i0 && q < pf_i0 + nchunks) {
+                const int64_t ci = q - pf_i0;
                 if (ci == 0 && sl >= 1) push(HCLOOC_OP_WAIT, 0, ev.b_free(nb_buf));   // last read by the column before this one
                 const int64_t r_lo = nkk * ci / nchunks, r_hi = nkk * (ci + 1) / nchunks;
                 load_b(np, nj_idx, nb_buf, r_lo, r_hi - r_lo);
                 if (ci == nchunks - 1) push(HCLOOC_OP_RECORD, 0, ev.b_ready(nb_buf));
             }
-            issue_compute(s, any, b, t == P.h - 1);
+            issue_compute(s, any, b, q == hl - 1);
         }
     }
 }
@@ -418,7 +433,7 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
                            (scale_only || (A_alias && B_alias && ((((uintptr_t)A_alias | (uintptr_t)B_alias) & 15u) == 0)));
     {
         const int where = in_core ? 1 : (c_dev ? 2 : (direct_ok ? (direct_mode == 1 ? 4 : 3) : 0));
-        const hclooc_ctx::PlanKey key{M, N, K, beta != 0.0 || tri != 0, alpha == 0.0, where + (transa ? 8 : 0) + (transb ? 16 : 0), budget};
+        const hclooc_ctx::PlanKey key{M, N, K, beta != 0.0 || tri != 0, alpha == 0.0, where + (transa ? 8 : 0) + (transb ? 16 : 0) + 32 * tri, budget};
         bool hit = false;
         for (const auto& kv : ctx->plan_cache) {
             const hclooc_ctx::PlanKey& k = kv.first;
@@ -428,6 +443,7 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
         if (!hit) {
             rc = plan_impl(M, N, K, key.beta_nz, key.alpha_zero, budget, where, transa, transb, &P);
             if (rc) return rc;
+            P.tri = tri;
             if (ctx->plan_cache.size() >= 16) ctx->plan_cache.erase(ctx->plan_cache.begin());
             ctx->plan_cache.emplace_back(key, P);
         }
@@ -491,6 +507,17 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
     }
     // ---------------------------------------------------------------- S2-S7: issue the schedule
     build_schedule(P, ctx->n_compute, ctx->ops);
+    if (P.tri != 0) {
+        // blocks outside the referenced triangle are not steps: the traffic of this plan is what its schedule says
+        uint64_t up = 0, down = 0, nup = 0, ndown = 0;
+        for (const hclooc_op_t& o : ctx->ops) {
+            const uint64_t bytes = (uint64_t)o.nr * (uint64_t)o.nc * 8;
+            if (o.kind == HCLOOC_OP_H2D_A || o.kind == HCLOOC_OP_H2D_B) { up += bytes; ++nup; }
+            else if (o.kind == HCLOOC_OP_H2D_C) { if (!c_dev) up += bytes; ++nup; }
+            else if (o.kind == HCLOOC_OP_D2H_C) { if (!c_dev) down += bytes; ++ndown; }
+        }
+        P.bytes_h2d = up; P.bytes_d2h = down; P.n_copies_h2d = nup; P.n_copies_d2h = ndown;
+    }
     for (int i = 0; i < P.n_scratch && i < ctx->n_compute; ++i)   // stream-K tile counters start at zero
         HCL_CUDA(cudaMemsetAsync(scratch[i] + streamk_counter_offset(), 0, streamk_counter_bytes(), ctx->s_compute[i]));
     auto stream_of = [&](int s) { return s == 0 ? ctx->s_h2d : (s == 1 ? ctx->s_d2h : ctx->s_compute[s - 2]); };
@@ -689,8 +716,7 @@ extern "C" int hclooc_dgemm_t(hclooc_ctx* ctx, int transa, int transb, int64_t M
     return dgemm_core(ctx, transa, transb, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes, stats);
 }
 
-// Out-of-core DSYRK on top of the DGEMM path: the referenced triangle is cut into block columns (lower) or block rows
-// (upper) of `nbs` columns / rows that start on the diagonal; each is one call of the pipeline with the triangle mask.
+// Out-of-core DSYRK on top of the DGEMM path: one pass of the pipeline with the triangle mask (plan.tri).
 extern "C" int hclooc_dsyrk(hclooc_ctx* ctx, int uplo, int trans, int64_t N, int64_t K, double alpha, const double* A, int64_t lda,
                             double beta, double* C, int64_t ldc, size_t device_budget_bytes, hclooc_stats* stats) {
     const auto t_begin = std::chrono::steady_clock::now();
@@ -708,27 +734,15 @@ extern "C" int hclooc_dsyrk(hclooc_ctx* ctx, int uplo, int trans, int64_t N, int
     if (!C) return -10;
     if (ldc < N) return -11;
     if (scale_only && beta == 1.0) return HCLOOC_OK;
-    // block width: wide enough that a block column is compute-bound (flops per uploaded byte ~ nbs / 4) and the part of the
-    // diagonal blocks computed for nothing stays small (tiles wholly in the other triangle are skipped by the kernel)
-    const int64_t nbs = std::min<int64_t>(N, 4096);
-    hclooc_stats acc, one;
+    // One pass of the pipeline over the whole N x N problem with the triangle mask: the schedule leaves out the blocks that lie
+    // wholly in the other triangle (no upload, kernel or download), the kernels skip such tiles inside the blocks that cross the
+    // diagonal and store only referenced elements.  trans == N: A is N x K, the right operand is A read transposed (transb);
+    // trans == T: A is K x N, the left operand is A read transposed (transa).
+    hclooc_stats acc;
     std::memset(&acc, 0, sizeof(acc));
-    for (int64_t j0 = 0; j0 < N; j0 += nbs) {
-        const int64_t nj = std::min(nbs, N - j0), rest = N - j0;
-        // lower: C[j0:N, j0:j0+nj] = alpha*op(A)[j0:N, :] * op(A)[j0:j0+nj, :]^T + beta*C   (M' = rest, N' = nj)
-        // upper: C[j0:j0+nj, j0:N] = alpha*op(A)[j0:j0+nj, :] * op(A)[j0:N, :]^T + beta*C   (M' = nj, N' = rest)
-        const int64_t Mc = uplo == HCL_UPLO_LOWER ? rest : nj, Nc = uplo == HCL_UPLO_LOWER ? nj : rest;
-        const double* Ab = scale_only ? nullptr : (trans ? A + j0 : A + j0 * lda);      // op(A) rows j0.. : both operands start here
-        // trans == N: A is N x K: left operand as stored, right operand = stored rows read transposed (transb)
-        // trans == T: A is K x N: left operand = stored columns read transposed (transa), right operand as stored
-        int rc = dgemm_core(ctx, trans ? 1 : 0, trans ? 0 : 1, Mc, Nc, K, alpha, Ab, lda, Ab, lda, beta, C + j0 * ldc + j0, ldc,
-                            device_budget_bytes, &one, uplo == HCL_UPLO_LOWER ? 1 : 2);
-        if (rc) return rc;
-        acc.plan = one.plan;
-        acc.bytes_h2d += one.bytes_h2d; acc.bytes_d2h += one.bytes_d2h;
-        acc.n_kernels += one.n_kernels; acc.n_copies_h2d += one.n_copies_h2d; acc.n_copies_d2h += one.n_copies_d2h;
-        acc.t_enqueue_s += one.t_enqueue_s;
-    }
+    int rc = dgemm_core(ctx, trans ? 1 : 0, trans ? 0 : 1, N, N, K, alpha, A, lda, A, lda, beta, C, ldc, device_budget_bytes, &acc,
+                        uplo == HCL_UPLO_LOWER ? 1 : 2);
+    if (rc) return rc;
     if (stats) {
         *stats = acc;
         stats->t_total_s = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_begin).count();

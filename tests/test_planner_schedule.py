@@ -420,3 +420,33 @@ def test_plans_for_transposed_operands_keep_the_stored_layout():
     with pytest.raises(H.HclError) as e:
         H.hclooc_plan_trans(8, 8, 8, 1, 0, 1 * MiB, 0, 2, 0)
     assert e.value.status == -8
+
+
+@pytest.mark.parametrize("tri", [1, 2])
+def test_triangle_schedule_has_steps_only_for_blocks_that_touch_the_triangle(tri):
+    """plan.tri (hclooc_dsyrk): a block of C wholly in the triangle that is not referenced is not a step -- no upload, no
+    kernel, no download; every other block is computed exactly once per K panel, in the usual buffers and event order."""
+    MiB = 1 << 20
+    for (N, K, budget) in ((3000, 700, 8 * MiB), (4096, 4096, 64 * MiB), (1000, 30000, 2 * MiB)):
+        p = H.hclooc_plan_ex(N, N, K, 1, 0, budget, 0)
+        full = H.hclooc_schedule(p, 8)
+        p.tri = tri
+        ops = H.hclooc_schedule(p, 8)
+        gemm = ops[ops["kind"] == 3]
+        seen = {}
+        for o in gemm:
+            i, j, pnl = int(o["r0"]) // p.mb, int(o["c0"]) // p.nb, int(o["k0"]) // p.kb
+            seen[(i, j, pnl)] = seen.get((i, j, pnl), 0) + 1
+        for i in range(p.h):
+            for j in range(p.w):
+                r0, r1 = i * p.mb, min(N, (i + 1) * p.mb)
+                c0, c1 = j * p.nb, min(N, (j + 1) * p.nb)
+                touches = (c0 <= r1 - 1) if tri == 1 else (c1 - 1 >= r0)
+                for pnl in range(p.kpanels):
+                    assert seen.get((i, j, pnl), 0) == (1 if touches else 0), (tri, i, j, pnl)
+        up_c, down_c = ops[ops["kind"] == 2], ops[ops["kind"] == 4]
+        assert len(down_c) == len(gemm) and len(up_c) == len(gemm)          # beta != 0: one upload and one download per live block
+        assert len(gemm) < len(full[full["kind"] == 3]) or p.h * p.w == 1
+        # every B slice is still loaded whole, once per K panel
+        b = ops[ops["kind"] == 1]
+        assert int((b["nr"] * b["nc"]).sum()) == K * N
