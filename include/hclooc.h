@@ -173,7 +173,7 @@ typedef struct hclooc_stats {
  * device: CUDA ordinal.  d_workspace/workspace_bytes: caller-owned device memory (e.g. a PyTorch
  * tensor) the context carves all its buffers from, or NULL/0 to let the library cudaMalloc (and grow)
  * its own.  stream_h2d / stream_d2h: caller-owned cudaStream_t or NULL for library-owned.
- * compute_streams[n_compute]: caller-owned compute streams, or NULL/0 for 4 library-owned ones.    */
+ * compute_streams[n_compute]: caller-owned compute streams, or NULL/0 for 8 library-owned ones.    */
 int hclooc_ctx_create(hclooc_ctx** ctx, int device, void* d_workspace, size_t workspace_bytes,
                       hclStream stream_h2d, hclStream stream_d2h, hclStream* compute_streams, int n_compute);
 int hclooc_ctx_destroy(hclooc_ctx* ctx);
