@@ -223,6 +223,7 @@ def run_ours(args, wl, name):
     synthgen.fill(A.array, seed, "A", wl["dist"], row0=rank * M); synthgen.fill(B.array, seed, "B", wl["dist"])
     synthgen.fill(C.array, seed, "C", wl["dist"], row0=rank * M)
     dA, dB, dC = (torch.from_numpy(X.array).cuda() for X in (A, B, C))
+    torch.cuda.synchronize()      # the library's streams do not wait for PyTorch's: device operands must be complete
 
     # ---- PyTorch owns device memory and streams; the library carves its buffers from this workspace
     ws = torch.empty(budget, dtype=torch.uint8, device="cuda")

@@ -200,7 +200,9 @@ int hclooc_ctx_get_trace(hclooc_ctx* ctx, hclooc_trace_rec* recs, size_t max_rec
  *   A: M x K, lda >= K;  B: K x N, ldb >= N;  C: M x N, ldc >= N, updated IN PLACE; A, B read-only.
  *   A, B, C: pinned HOST pointers (the product path).  Device pointers are also accepted: if all three are
  *   device memory the call is in-core (one DGEMM on the caller's matrices, nothing staged) -- bench.py's
- *   HBM-resident `value` leg; a mix is staged through the workspace with device-to-device copies.
+ *   HBM-resident `value` leg; a mix is staged through the workspace with device-to-device copies.  The call runs on the
+ *   context's own non-blocking streams, which do not wait for work the caller has in flight on other streams: device operands
+ *   must be COMPLETE (their producing copies / kernels synchronised) before they are handed over.
  *   device_budget_bytes bounds the sum of all device buffers the call uses (0 = all free HBM minus a
  *   1 GiB margin).  Uses a process-wide default context created on first use.
  *   beta == 0: C is never read (NaN/Inf in C are overwritten).  alpha == 0 or K == 0: A and B are not

@@ -3,6 +3,8 @@
 // overhead to the virtual-table lookups, :164).
 #include <cstring>
 #include <algorithm>
+#include <chrono>
+#include <thread>
 #include "internal.h"
 
 using namespace hclooc;
@@ -212,9 +214,18 @@ int hclDeviceSynchronize(int device) {
 void* hclooc_host_alloc(size_t bytes) {
     void* p = nullptr;
     if (bytes == 0) return nullptr;
-    cudaError_t e = cudaHostAlloc(&p, bytes, cudaHostAllocDefault);
-    if (e != cudaSuccess) { set_last_cuda_error((int)e); cudaGetLastError(); return nullptr; }
-    return p;
+    // Pinning can fail transiently with cudaErrorOperatingSystem (304) although the host has the memory -- seen on the B200
+    // boxes about once in eight fresh processes, succeeding two seconds later -- so a failed attempt is retried a few times.
+    cudaError_t e = cudaSuccess;
+    for (int attempt = 0; attempt < 6; ++attempt) {
+        e = cudaHostAlloc(&p, bytes, cudaHostAllocDefault);
+        if (e == cudaSuccess) return p;
+        cudaGetLastError();
+        if (e != cudaErrorOperatingSystem && e != cudaErrorMemoryAllocation) break;
+        std::this_thread::sleep_for(std::chrono::seconds(2));
+    }
+    set_last_cuda_error((int)e);
+    return nullptr;
 }
 int hclooc_host_free(void* p) {
     if (!p) return HCLOOC_OK;
@@ -224,8 +235,15 @@ int hclooc_host_free(void* p) {
 int hclooc_host_register(void* p, size_t bytes) {
     if (!p) return -1;
     if (bytes == 0) return -2;
-    HCL_CUDA(cudaHostRegister(p, bytes, cudaHostRegisterDefault));
-    return HCLOOC_OK;
+    cudaError_t e = cudaSuccess;
+    for (int attempt = 0; attempt < 6; ++attempt) {          // transient cudaErrorOperatingSystem: see hclooc_host_alloc
+        e = cudaHostRegister(p, bytes, cudaHostRegisterDefault);
+        if (e == cudaSuccess) return HCLOOC_OK;
+        cudaGetLastError();
+        if (e != cudaErrorOperatingSystem && e != cudaErrorMemoryAllocation) break;
+        std::this_thread::sleep_for(std::chrono::seconds(2));
+    }
+    return cuda_fail(e);
 }
 int hclooc_host_unregister(void* p) {
     if (!p) return -1;

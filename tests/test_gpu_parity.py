@@ -40,6 +40,15 @@ def host_inputs(H, M, N, K, seed, dist, pads=(0, 0, 0), poison_c=False):
     return A, B, C
 
 
+def to_dev(x):
+    """numpy -> device tensor, COMPLETE on return: the library launches on its own (non-blocking) streams, which do not wait
+    for PyTorch's stream, so a device operand must be ready before it is handed over (include/hclooc.h, hclooc_dgemm)."""
+    import torch
+    t = torch.from_numpy(x).cuda()
+    torch.cuda.synchronize()
+    return t
+
+
 def check(C_gpu, C_ref, D, exact):
     assert not np.isnan(C_gpu).any()
     if exact:
@@ -72,7 +81,7 @@ def test_tile_kernel_matches_oracle(H, M, N, K, alpha, beta, dist):
     synthgen.fill(A, 21, "A", dist, cols=K); synthgen.fill(B, 21, "B", dist, cols=N); synthgen.fill(C0, 21, "C", dist, cols=N)
     if beta == 0.0:
         C0[:, :N] = np.nan                                                       # must not be read
-    dA, dB, dC = (torch.from_numpy(x).cuda() for x in (A, B, C0))
+    dA, dB, dC = (to_dev(x) for x in (A, B, C0))
     H.hclDgemmAsync(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, torch.cuda.current_stream())
     torch.cuda.synchronize()
     got = dC.cpu().numpy()
@@ -88,11 +97,11 @@ def test_tile_kernel_alpha_zero_and_k_zero(H):
     C0 = synthgen.fill(np.empty((M, N)), 22, "C", "uniform")
     nan = torch.full((M, 64), float("nan"), dtype=torch.float64, device="cuda")
     nanb = torch.full((64, N), float("nan"), dtype=torch.float64, device="cuda")
-    dC = torch.from_numpy(C0).cuda()
+    dC = to_dev(C0)
     H.hclDgemmAsync(M, N, 64, 0.0, nan, 64, nanb, N, -2.0, dC, N, torch.cuda.current_stream())    # alpha == 0: A, B not read
     torch.cuda.synchronize()
     assert np.array_equal(dC.cpu().numpy(), -2.0 * C0)
-    dC = torch.from_numpy(C0).cuda()
+    dC = to_dev(C0)
     H.hclDgemmAsync(M, N, 0, 1.0, None, 2, None, N, 0.5, dC, N, torch.cuda.current_stream())      # K == 0
     torch.cuda.synchronize()
     assert np.array_equal(dC.cpu().numpy(), 0.5 * C0)
@@ -347,20 +356,21 @@ def test_device_resident_operands_run_in_core(H):
     A, B, C = host_inputs(H, M, N, K, 51, "int")
     ref = C.view.copy()
     oracle.dgemm(2.0, A.view, B.view, -1.0, ref)
-    dA, dB = torch.from_numpy(A.view.copy()).cuda(), torch.from_numpy(B.view.copy()).cuda()
-    dC = torch.from_numpy(C.view.copy()).cuda()
+    dA, dB = to_dev(A.view.copy()), to_dev(B.view.copy())
+    dC = to_dev(C.view.copy())
     st = H.hclooc_dgemm_ex(None, M, N, K, 2.0, dA, K, dB, N, -1.0, dC, N, 1 * MiB)
     assert st.n_kernels == 1 and st.bytes_h2d == 0 and st.bytes_d2h == 0 and st.plan.workspace_bytes == 0
     assert st.plan.h == 1 and st.plan.w == 1
     assert np.array_equal(dC.cpu().numpy(), ref)
     # mixed residency: A on the host, B and C on the device -> staged, same values
-    dC2 = torch.from_numpy(C.view.copy()).cuda()
+    dC2 = to_dev(C.view.copy())
     st = H.hclooc_dgemm_ex(None, M, N, K, 2.0, A, A.ld, dB, N, -1.0, dC2, N, 1 * MiB)
     assert st.n_kernels > 1 and st.plan.workspace_bytes <= 1 * MiB
     assert np.array_equal(dC2.cpu().numpy(), ref)
     # odd leading dimension of C on the device: not addressable by the vector epilogue/TMA rules -> staged
     dC3 = torch.zeros(M, N + 1, dtype=torch.float64, device="cuda")
-    dC3[:, :N] = torch.from_numpy(C.view.copy()).cuda()
+    dC3[:, :N] = to_dev(C.view.copy())
+    torch.cuda.synchronize()
     st = H.hclooc_dgemm_ex(None, M, N, K, 2.0, dA, K, dB, N, -1.0, dC3, N + 1, 1 * MiB)
     assert st.n_kernels > 1
     assert np.array_equal(dC3[:, :N].cpu().numpy(), ref) and float(dC3[:, N].abs().max()) == 0.0
@@ -384,10 +394,10 @@ def test_streamk_kernel_matches_oracle(H, M, N, K, dist):
     C0 = synthgen.fill(np.empty((M, N)), 61, "C", dist)
     ref = C0.copy()
     D = oracle.dgemm(1.5, A, B, -0.5, ref, want_denominator=True)
-    dA, dB = torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda()
+    dA, dB = to_dev(A), to_dev(B)
     outs = []
     for rep in range(3):
-        dC = torch.from_numpy(C0).cuda()
+        dC = to_dev(C0)
         st = H.hclooc_dgemm_ex(None, M, N, K, 1.5, dA, K, dB, N, -0.5, dC, N, 0)
         assert st.n_kernels == 1
         outs.append(dC.cpu().numpy())
@@ -404,9 +414,9 @@ def test_streamk_launches_on_two_streams_do_not_share_scratch(H):
     C0 = synthgen.fill(np.empty((M, N)), 62, "C", "int")
     ref = C0.copy()
     oracle.dgemm(1.0, A, B, 1.0, ref)
-    dA, dB = torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda()
+    dA, dB = to_dev(A), to_dev(B)
     streams = [torch.cuda.Stream() for _ in range(3)]
-    dCs = [[torch.from_numpy(C0).cuda() for _ in range(4)] for _ in streams]
+    dCs = [[to_dev(C0) for _ in range(4)] for _ in streams]
     torch.cuda.synchronize()
     for r in range(4):
         for s, row in zip(streams, dCs):
@@ -716,7 +726,7 @@ def test_tile_kernel_transposed_layouts(H, transa, transb, M, N, K, alpha, beta,
     synthgen.fill(A, 51, "A", dist, cols=ac); synthgen.fill(B, 51, "B", dist, cols=bc); synthgen.fill(C0, 51, "C", dist, cols=N)
     if beta == 0.0:
         C0[:, :N] = np.nan
-    dA, dB, dC = (torch.from_numpy(x).cuda() for x in (A, B, C0))
+    dA, dB, dC = (to_dev(x) for x in (A, B, C0))
     H.hclDgemmAsyncT(transa, transb, M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, torch.cuda.current_stream(), variant=variant)
     torch.cuda.synchronize()
     got = dC.cpu().numpy()
@@ -731,7 +741,7 @@ def test_tile_kernel_transposed_layouts(H, transa, transb, M, N, K, alpha, beta,
         # the same bits as the untransposed kernel on written-out transposes (same order of summation)
         pa, pb = np.zeros((M, K + K % 2)), np.zeros((K, N + N % 2))                  # even leading dimensions
         pa[:, :K] = opA; pb[:, :N] = opB
-        dA2, dB2, dC2 = torch.from_numpy(pa).cuda(), torch.from_numpy(pb).cuda(), torch.from_numpy(C0).cuda()
+        dA2, dB2, dC2 = to_dev(pa), to_dev(pb), to_dev(C0)
         H.hclDgemmAsyncEx(M, N, K, alpha, dA2, K + K % 2, dB2, N + N % 2, beta, dC2, ldc, torch.cuda.current_stream(), variant=1)
         torch.cuda.synchronize()
         assert np.array_equal(dC2.cpu().numpy()[:, :N].view(np.uint64), got[:, :N].view(np.uint64))
@@ -747,7 +757,7 @@ def test_transposed_in_core_and_direct_modes(H):
     A, B, C = stored_inputs(H, 1, 1, M, N, K, 52, "int")
     ref = C.view.copy()
     oracle.dgemm(1.0, A.view.T.copy(), B.view.T.copy(), 0.5, ref)
-    dA, dB, dC = (torch.from_numpy(X.view.copy()).cuda() for X in (A, B, C))
+    dA, dB, dC = (to_dev(X.view.copy()) for X in (A, B, C))
     st = H.hclooc_dgemm_t(None, 1, 1, M, N, K, 1.0, dA, M, dB, K, 0.5, dC, N, 0)
     assert st.plan.n_steps == 1 and st.plan.workspace_bytes == 0 and st.bytes_h2d == 0
     assert np.array_equal(dC.cpu().numpy(), ref)
@@ -780,16 +790,16 @@ def test_streamk_kernel_transposed_layouts(H, transa, transb, M, N, K, dist):
     opB[...] = B.T if transb else B
     ref = C0.copy()
     D = oracle.dgemm(1.5, opA, opB, -0.5, ref, want_denominator=True)
-    dA, dB, dC = torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(), torch.from_numpy(C0).cuda()
+    dA, dB, dC = to_dev(A), to_dev(B), to_dev(C0)
     H.hclDgemmAsyncT(transa, transb, M, N, K, 1.5, dA, ac, dB, bc, -0.5, dC, N, torch.cuda.current_stream(), variant=-1)
     torch.cuda.synchronize()
     got = dC.cpu().numpy()
     check(got, ref, D, exact=(dist == "int"))
-    dA2, dB2, dC2 = torch.from_numpy(opA).cuda(), torch.from_numpy(opB).cuda(), torch.from_numpy(C0).cuda()
+    dA2, dB2, dC2 = to_dev(opA), to_dev(opB), to_dev(C0)
     H.hclDgemmAsyncEx(M, N, K, 1.5, dA2, K, dB2, N, -0.5, dC2, N, torch.cuda.current_stream(), variant=-1)
     torch.cuda.synchronize()
     assert np.array_equal(dC2.cpu().numpy().view(np.uint64), got.view(np.uint64))
-    dC3 = torch.from_numpy(C0).cuda()
+    dC3 = to_dev(C0)
     st = H.hclooc_dgemm_t(None, transa, transb, M, N, K, 1.5, dA, ac, dB, bc, -0.5, dC3, N, 0)
     assert st.n_kernels == 1 and st.plan.trans == transa + 2 * transb
     check(dC3.cpu().numpy(), ref, D, exact=(dist == "int"))
@@ -811,7 +821,7 @@ def test_cluster_multicast_kernel_matches_tile_kernel(H, cm, cn, M, N, K, alpha,
     synthgen.fill(A, 71, "A", dist, cols=K); synthgen.fill(B, 71, "B", dist, cols=N); synthgen.fill(C0, 71, "C", dist, cols=N)
     if beta == 0.0:
         C0[:, :N] = np.nan
-    dA, dB, dC, dC1 = (torch.from_numpy(x).cuda() for x in (A, B, C0, C0))
+    dA, dB, dC, dC1 = (to_dev(x) for x in (A, B, C0, C0))
     H.hclDgemmAsyncEx(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, torch.cuda.current_stream(), variant=100 + 10 * cm + cn)
     H.hclDgemmAsyncEx(M, N, K, alpha, dA, lda, dB, ldb, beta, dC1, ldc, torch.cuda.current_stream(), variant=1)
     torch.cuda.synchronize()
@@ -895,3 +905,18 @@ def test_dsyrk_large_blocks_symmetry_and_errors(H):
         with pytest.raises(H.HclError) as e:
             H.hclooc_dsyrk(None, *args, 256 * MiB)
         assert e.value.status == want, (args[:2], e.value.status)
+
+
+@pytest.mark.parametrize("uplo,trans", [(0, 0), (1, 1)])
+def test_dsyrk_on_device_resident_operands_runs_in_core(H, uplo, trans):
+    """A and C in device memory: one masked launch on the caller's matrices, nothing staged; the other triangle untouched."""
+    import torch
+    N, K = 700, 260
+    A = synthgen.fill(np.empty((K, N) if trans else (N, K)), 83, "A", "int")
+    C0 = synthgen.fill(np.empty((N, N)), 83, "C", "int")
+    ref = C0.copy()
+    oracle.dsyrk(uplo, trans, 2.0, A, 0.5, ref)
+    dA, dC = to_dev(A), to_dev(C0)
+    st = H.hclooc_dsyrk(None, uplo, trans, N, K, 2.0, dA, A.shape[1], 0.5, dC, N, 0)
+    assert st.n_kernels == 1 and st.plan.workspace_bytes == 0 and st.bytes_h2d == 0
+    assert np.array_equal(dC.cpu().numpy(), ref)
