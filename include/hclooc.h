@@ -251,6 +251,17 @@ int hclooc_dgemm_t(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N
 int hclooc_dsyrk(hclooc_ctx* ctx, int uplo, int trans, int64_t N, int64_t K, double alpha, const double* A, int64_t lda,
                  double beta, double* C, int64_t ldc, size_t device_budget_bytes, hclooc_stats* stats_out);
 
+/* Out-of-core DSYR2K, two masked passes of the same pipeline (the second accumulates with beta' = 1):
+ *     C = alpha*A*B^T + alpha*B*A^T + beta*C   (trans = HCL_OP_N, A and B are N x K, lda, ldb >= K)
+ *     C = alpha*A^T*B + alpha*B^T*A + beta*C   (trans = HCL_OP_T, A and B are K x N, lda, ldb >= N)
+ * on the `uplo` triangle of the N x N matrix C; the other triangle keeps its bits.  Rounding: the first product is rounded
+ * into C with beta*C, the second is then added (what the oracle's dsyr2k does).  stats: sums over the two passes.
+ * Errors: -2 uplo, -3 trans, -4 N < 0, -5 K < 0, -7 A NULL, -8 lda, -9 B NULL, -10 ldb, -12 C NULL or overlapping A or B,
+ * -13 ldc < N, and the HCLOOC_ERR_* codes.                                                                            */
+int hclooc_dsyr2k(hclooc_ctx* ctx, int uplo, int trans, int64_t N, int64_t K, double alpha, const double* A, int64_t lda,
+                  const double* B, int64_t ldb, double beta, double* C, int64_t ldc, size_t device_budget_bytes,
+                  hclooc_stats* stats_out);
+
 /* nsteps mode (:277-283): MMOOC as a subroutine of a blocked algorithm (SUMMA, HSUMMA) that updates the same C
  * `nsteps` times: C = alpha*A_p*B_p + beta_p*C for p = *step = 0 .. nsteps-1, one call per p.  C is uploaded once
  * at step 0 (if beta != 0), stays in device memory between the calls, and is downloaded once at the last step, so

@@ -136,6 +136,31 @@ def dsyrk(uplo, trans, alpha, A, beta, C, want_denominator=False):
     return D
 
 
+def dsyr2k(uplo, trans, alpha, A, B, beta, C, want_denominator=False):
+    """The DSYR2K definition on one triangle of C, in place, as two DGEMM definitions in sequence:
+        C_ij <- (alpha * sum_k a_ik b_jk + beta * C_ij),  then  C_ij <- alpha * sum_k b_ik a_jk + C_ij      (trans = 0)
+    (A, B are N x K; trans = 1: A, B are K x N and the sums run over a_ki b_kj, b_ki a_kj).  The other triangle keeps its bits.
+    D = |alpha| sum_k (|a_ik||b_jk| + |b_ik||a_jk|) + |beta||C0_ij| on the triangle when asked."""
+    N = C.shape[0]
+    opA, opB = np.empty((N, A.shape[0] if trans else A.shape[1])), np.empty((N, B.shape[0] if trans else B.shape[1]))
+    opA[...] = A.T if trans else A
+    opB[...] = B.T if trans else B
+    opAt, opBt = np.empty(opA.shape[::-1]), np.empty(opB.shape[::-1])
+    opAt[...] = opA.T
+    opBt[...] = opB.T
+    full = C.copy()
+    D1 = dgemm(alpha, opA, opBt, beta, full, want_denominator=want_denominator)
+    mid = full.copy() if want_denominator else None
+    D2 = dgemm(alpha, opB, opAt, 1.0, full, want_denominator=want_denominator)
+    keep = np.tril(np.ones((N, N), dtype=bool)) if uplo == 0 else np.triu(np.ones((N, N), dtype=bool))
+    C[keep] = full[keep]
+    if not want_denominator:
+        return None
+    D = D1 + (D2 - np.abs(mid))          # D2 = |alpha| sum |b||a| + |1||mid|: take the product part, keep D1's |beta||C0|
+    D[~keep] = 0.0
+    return D
+
+
 def partition(M, N, K, S):
     """(h, w) of the paper's hclMatrixPartitioner rule by enumeration, or None if nothing fits."""
     h, w = _i64(), _i64()

@@ -750,6 +750,48 @@ extern "C" int hclooc_dsyrk(hclooc_ctx* ctx, int uplo, int trans, int64_t N, int
     return HCLOOC_OK;
 }
 
+// Out-of-core DSYR2K: two masked passes of the pipeline over the same triangle, the second one accumulating (beta' = 1).
+extern "C" int hclooc_dsyr2k(hclooc_ctx* ctx, int uplo, int trans, int64_t N, int64_t K, double alpha, const double* A, int64_t lda,
+                             const double* B, int64_t ldb, double beta, double* C, int64_t ldc, size_t device_budget_bytes,
+                             hclooc_stats* stats) {
+    const auto t_begin = std::chrono::steady_clock::now();
+    if (uplo != HCL_UPLO_LOWER && uplo != HCL_UPLO_UPPER) return -2;
+    if (trans != HCL_OP_N && trans != HCL_OP_T) return -3;
+    if (N < 0) return -4;
+    if (K < 0) return -5;
+    if (stats) std::memset(stats, 0, sizeof(*stats));
+    if (N == 0) return HCLOOC_OK;
+    const bool scale_only = (alpha == 0.0 || K == 0);
+    if (!scale_only) {
+        if (!A) return -7;
+        if (lda < (trans ? N : K)) return -8;
+        if (!B) return -9;
+        if (ldb < (trans ? N : K)) return -10;
+    }
+    if (!C) return -12;
+    if (ldc < N) return -13;
+    if (scale_only && beta == 1.0) return HCLOOC_OK;
+    const int tri = uplo == HCL_UPLO_LOWER ? 1 : 2, ta = trans ? 1 : 0, tb = trans ? 0 : 1;
+    hclooc_stats one, two;
+    std::memset(&one, 0, sizeof(one));
+    std::memset(&two, 0, sizeof(two));
+    // pass 1: C = alpha * op(A) * op(B)^T + beta * C;  pass 2: C = alpha * op(B) * op(A)^T + C   (each on the triangle only)
+    int rc = dgemm_core(ctx, ta, tb, N, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes, &one, tri);
+    if (rc) return rc == -10 ? -12 : rc;                          // C overlapping A or B: argument 12 of this function
+    if (!scale_only) {
+        rc = dgemm_core(ctx, ta, tb, N, N, K, alpha, B, ldb, A, lda, 1.0, C, ldc, device_budget_bytes, &two, tri);
+        if (rc) return rc == -10 ? -12 : rc;
+    }
+    if (stats) {
+        *stats = one;
+        stats->bytes_h2d += two.bytes_h2d; stats->bytes_d2h += two.bytes_d2h;
+        stats->n_kernels += two.n_kernels; stats->n_copies_h2d += two.n_copies_h2d; stats->n_copies_d2h += two.n_copies_d2h;
+        stats->t_enqueue_s += two.t_enqueue_s;
+        stats->t_total_s = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_begin).count();
+    }
+    return HCLOOC_OK;
+}
+
 extern "C" int hclooc_dgemm(int64_t M, int64_t N, int64_t K, double alpha, const double* A, int64_t lda,
                             const double* B, int64_t ldb, double beta, double* C, int64_t ldc, size_t device_budget_bytes) {
     return hclooc_dgemm_ex(nullptr, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes, nullptr);

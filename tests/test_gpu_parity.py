@@ -920,3 +920,38 @@ def test_dsyrk_on_device_resident_operands_runs_in_core(H, uplo, trans):
     st = H.hclooc_dsyrk(None, uplo, trans, N, K, 2.0, dA, A.shape[1], 0.5, dC, N, 0)
     assert st.n_kernels == 1 and st.plan.workspace_bytes == 0 and st.bytes_h2d == 0
     assert np.array_equal(dC.cpu().numpy(), ref)
+
+
+@pytest.mark.parametrize("uplo", [0, 1])
+@pytest.mark.parametrize("trans", [0, 1])
+@pytest.mark.parametrize("N,K,alpha,beta,dist,budget", [
+    (300, 200, 1.0, 0.5, "uniform", 1 * MiB),
+    (517, 389, 2.0, -1.0, "int", 2 * MiB),
+    (129, 33, -1.5, 0.0, "int", 1 * MiB),
+    (1300, 260, 1.0, 1.0, "normal", 64 * MiB),
+])
+def test_dsyr2k_matches_oracle_and_leaves_the_other_triangle(H, uplo, trans, N, K, alpha, beta, dist, budget):
+    ar, ac = (K, N) if trans else (N, K)
+    A, B, C = H.HostMatrix(ar, ac, ac + 2), H.HostMatrix(ar, ac, ac + 4), H.HostMatrix(N, N, N + 2)
+    for X in (A, B, C):
+        X.array[...] = np.nan
+    synthgen.fill(A.array, 84, "A", dist, cols=ac); synthgen.fill(B.array, 84, "B", dist, cols=ac); synthgen.fill(C.array, 84, "C", dist, cols=N)
+    other = np.triu(np.ones((N, N), bool), 1) if uplo == 0 else np.tril(np.ones((N, N), bool), -1)
+    if beta == 0.0:
+        C.view[~other] = np.nan
+    marker = C.view.copy()
+    marker[other] = np.arange(int(other.sum())) + 0.25
+    C.view[...] = marker
+    ref = np.where(np.isnan(marker), 0.0, marker) if beta == 0.0 else marker.copy()
+    D = oracle.dsyr2k(uplo, trans, alpha, A.view.copy(), B.view.copy(), beta, ref, want_denominator=True)
+    st = H.hclooc_dsyr2k(None, uplo, trans, N, K, alpha, A, A.ld, B, B.ld, beta, C, C.ld, budget)
+    assert st.n_kernels >= 2
+    got = C.view.copy()
+    assert np.array_equal(got[other], marker[other])
+    gk, rk = got.copy(), ref.copy()
+    gk[other] = 0.0; rk[other] = 0.0
+    D[other] = 1.0
+    check(gk, rk, D, exact=(dist == "int"))
+    with pytest.raises(H.HclError) as e:
+        H.hclooc_dsyr2k(None, uplo, trans, N, K, alpha, A, A.ld, None, B.ld, beta, C, C.ld, budget)
+    assert e.value.status == -9

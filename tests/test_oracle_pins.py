@@ -348,3 +348,47 @@ def test_dsyrk_symmetry_integers_and_closed_forms():
     lo1, up1 = np.zeros((8, 8)), np.zeros((8, 8))
     oracle.dsyrk(0, 0, 1.25, u, 0.0, lo1); oracle.dsyrk(1, 0, 1.25, u, 0.0, up1)
     assert np.array_equal(np.tril(lo1), np.tril(1.25 * (u * u.T))) and np.array_equal(np.tril(lo1), np.triu(up1).T)
+
+
+def test_dsyr2k_brute_force_symmetry_and_integers():
+    rng = np.random.default_rng(13)
+    for uplo in (0, 1):
+        for trans in (0, 1):
+            N, K = 6, 5
+            A = rng.uniform(-1, 1, (K, N) if trans else (N, K)); B = rng.uniform(-1, 1, (K, N) if trans else (N, K))
+            C0 = rng.uniform(-1, 1, (N, N))
+            other = np.triu(np.ones((N, N), bool), 1) if uplo == 0 else np.tril(np.ones((N, N), bool), -1)
+            C0[other] = np.nan
+            C = C0.copy()
+            oracle.dsyr2k(uplo, trans, 1.5, A, B, -0.5, C)
+            a = A.T if trans else A
+            b = B.T if trans else B
+            for i in range(N):
+                for j in range(N):
+                    if other[i, j]:
+                        assert np.isnan(C[i, j])
+                        continue
+                    s1 = 0.0
+                    for k in range(K):
+                        s1 = s1 + a[i, k] * b[j, k]
+                    first = 1.5 * s1 + (-0.5) * C0[i, j]
+                    s2 = 0.0
+                    for k in range(K):
+                        s2 = s2 + b[i, k] * a[j, k]
+                    assert C[i, j] == 1.5 * s2 + 1.0 * first, (uplo, trans, i, j)
+    # integers: exact; beta == 0: alpha*S1 + alpha*S2 commutes, so lower == upper^T bit for bit even in floating point
+    N, K = 23, 31
+    A = rng.integers(-4, 5, (N, K)).astype(np.float64); B = rng.integers(-4, 5, (N, K)).astype(np.float64)
+    lo, up = np.zeros((N, N)), np.zeros((N, N))
+    oracle.dsyr2k(0, 0, 2.0, A, B, 0.0, lo); oracle.dsyr2k(1, 0, 2.0, A, B, 0.0, up)
+    Ai, Bi = A.astype(np.int64), B.astype(np.int64)
+    assert np.array_equal(np.tril(lo), np.tril(2 * (Ai @ Bi.T + Bi @ Ai.T)).astype(np.float64))
+    assert np.array_equal(np.tril(lo), np.triu(up).T)
+    Af, Bf = rng.uniform(-1, 1, (N, K)), rng.uniform(-1, 1, (N, K))
+    lo, up = np.zeros((N, N)), np.zeros((N, N))
+    oracle.dsyr2k(0, 0, 1.25, Af, Bf, 0.0, lo); oracle.dsyr2k(1, 0, 1.25, Af, Bf, 0.0, up)
+    assert np.array_equal(np.tril(lo), np.triu(up).T)
+    # B == A: dsyr2k(alpha) == dsyrk(2 alpha) on integers
+    s1, s2 = np.zeros((N, N)), np.zeros((N, N))
+    oracle.dsyr2k(0, 0, 1.0, A, A, 0.0, s1); oracle.dsyrk(0, 0, 2.0, A, 0.0, s2)
+    assert np.array_equal(s1, s2)
