@@ -377,9 +377,10 @@ int hclooc::plan_impl(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alp
         const double rd = 8.0 * ((scale_only ? 0.0 : std::ceil(tn / cn) * (double)M * (double)Keff + std::ceil(tm / cm) * (double)Keff * (double)N) +
                                  (beta_nz ? (double)M * (double)N : 0.0));
         const double wr = 8.0 * (double)M * (double)N;
-        // measured: 46-50 GB/s when every tile loads for itself, 24-35 GB/s through a multicasting cluster (its CTAs
-        // advance in lockstep, a stage at a time)
-        const double direct_Bps = env_or("HCLOOC_DIRECT_GBPS", cm * cn > 1 ? 33.0 : 50.0) * 1e9;
+        // measured: 46-50 GB/s when every tile loads for itself; through multicasting clusters (their CTAs advance in
+        // lockstep, a stage at a time) 24-36 GB/s with one cluster in flight, 35 with four, 44 with 64
+        const double n_clusters = std::ceil(tm / cm) * std::ceil(tn / cn);
+        const double direct_Bps = env_or("HCLOOC_DIRECT_GBPS", cm * cn > 1 ? std::min(45.0, 30.0 + 3.5 * std::sqrt(n_clusters)) : 50.0) * 1e9;
         const double t_link = std::max(std::max(rd / direct_Bps, wr / mm.d2h_Bps), (rd + wr) / mm.duplex_Bps);
         const double t_flop = (scale_only ? 0.0 : 2.0 * (double)M * (double)N * (double)Keff) / mm.fp64_flops;
         const double waves = std::ceil(tm * tn / (cm * cn > 1 ? 128.0 : (double)NUM_SMS));   // whole clusters per GPC
