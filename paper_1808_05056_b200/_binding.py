@@ -175,7 +175,20 @@ class HostMatrix:
         self.rows, self.cols, self.ld = rows, cols, (cols if ld is None else ld)
         assert self.ld >= cols
         self.nbytes = max(1, rows * self.ld) * 8
-        self.ptr = hclooc_host_alloc(self.nbytes)
+        # Pinning large buffers fails now and then with cudaErrorOperatingSystem on the B200 boxes when another CUDA process
+        # has just exited (the driver still tearing its mappings down); the library retries for ~12 s, this convenience class
+        # for about two minutes more before giving up.
+        for attempt in range(9):
+            try:
+                self.ptr = hclooc_host_alloc(self.nbytes)
+                break
+            except HclError:
+                if attempt == 8 or self.nbytes < (64 << 20):
+                    raise
+                import gc
+                import time
+                gc.collect()
+                time.sleep(12)
         buf = (ctypes.c_double * max(1, rows * self.ld)).from_address(self.ptr)
         self.array = np.frombuffer(buf, dtype=np.float64)[: rows * self.ld].reshape(rows, self.ld)
         self.view = self.array[:, :cols]

@@ -1,4 +1,7 @@
-"""bench.py prints ONE JSON line with the keys the driver reads (metric, value, unit, e2e, roofline, cpu_baseline, ...)."""
+"""bench.py prints ONE JSON line with the keys the driver reads (metric, value, unit, e2e, roofline, cpu_baseline, ...).
+
+(Named to run last: it starts bench.py in a subprocess, and pinning tens of GB right after another CUDA process has exited is
+what fails transiently on the boxes -- the full-size tests should not follow it.)"""
 import json
 import os
 import subprocess
