@@ -428,7 +428,7 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
         static std::once_flag once;
         std::call_once(once, [] { set_planner_max_cluster(direct_max_cluster()); });
     }
-    const bool direct_ok = !in_core && !c_dev && aligned && direct_mode != 0 && tri == 0 && M <= 0x7fffffffLL && N <= 0x7fffffffLL && K <= 0x7fffffffLL &&
+    const bool direct_ok = !in_core && !c_dev && aligned && direct_mode != 0 && M <= 0x7fffffffLL && N <= 0x7fffffffLL && K <= 0x7fffffffLL &&
                            C_alias && (((uintptr_t)C_alias & 15u) == 0) &&
                            (scale_only || (A_alias && B_alias && ((((uintptr_t)A_alias | (uintptr_t)B_alias) & 15u) == 0)));
     {
@@ -453,7 +453,7 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
         if (P.direct) { A = (const double*)A_alias; B = (const double*)B_alias; C = (double*)C_alias; }
         // direct: one CTA per tile (every tile is bound by its own reads over the link; the persistent kernel's
         // device scratch would also break the promise that the call uses no device memory)
-        if (P.direct && P.direct_cm * P.direct_cn > 1)
+        if (P.direct && P.direct_cm * P.direct_cn > 1 && tri == 0)     // (a masked call always has a transposed operand: no clusters)
             rc = launch_dgemm_direct(M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, ctx->s_compute[0], P.direct_cm, P.direct_cn);
         else
             rc = launch_dgemm_tiles(M, N, scale_only ? 0 : K, scale_only ? 0.0 : alpha, A, lda, B, ldb, beta, C, ldc, ctx->s_compute[0], P.direct ? 1 : -1,

@@ -955,3 +955,28 @@ def test_dsyr2k_matches_oracle_and_leaves_the_other_triangle(H, uplo, trans, N, 
     with pytest.raises(H.HclError) as e:
         H.hclooc_dsyr2k(None, uplo, trans, N, K, alpha, A, A.ld, None, B.ld, beta, C, C.ld, budget)
     assert e.value.status == -9
+
+
+def test_dsyrk_and_dsyr2k_in_direct_mode(H):
+    """Small symmetric updates under a small budget go through the direct mode too (tile kernel with the triangle mask on the
+    host matrices, no device buffer); the other triangle keeps its bits."""
+    N, K = 500, 300
+    A = H.HostMatrix(N, K); B = H.HostMatrix(N, K); C = H.HostMatrix(N, N)
+    synthgen.fill(A.array, 85, "A", "int"); synthgen.fill(B.array, 85, "B", "int"); synthgen.fill(C.array, 85, "C", "int")
+    c0 = C.view.copy()
+    ctx = H.hclooc_ctx_create(0)
+    try:
+        H.hclooc_ctx_set_direct(ctx, 1)
+        ref = c0.copy()
+        oracle.dsyrk(0, 0, 2.0, A.view, 0.5, ref)
+        st = H.hclooc_dsyrk(ctx, 0, 0, N, K, 2.0, A, K, 0.5, C, N, 1 * MiB)
+        assert st.plan.direct == 1 and st.plan.workspace_bytes == 0 and st.n_kernels == 1
+        assert np.array_equal(C.view, ref)
+        C.view[...] = c0
+        ref = c0.copy()
+        oracle.dsyr2k(1, 0, 1.0, A.view, B.view, -1.0, ref)
+        st = H.hclooc_dsyr2k(ctx, 1, 0, N, K, 1.0, A, K, B, K, -1.0, C, N, 1 * MiB)
+        assert st.plan.direct == 1 and st.n_kernels == 2
+        assert np.array_equal(C.view, ref)
+    finally:
+        H.hclooc_ctx_destroy(ctx)
