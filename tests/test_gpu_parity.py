@@ -980,3 +980,36 @@ def test_dsyrk_and_dsyr2k_in_direct_mode(H):
         assert np.array_equal(C.view, ref)
     finally:
         H.hclooc_ctx_destroy(ctx)
+
+
+@pytest.mark.parametrize("transa,transb,tri", [(0, 0, 0), (1, 1, 0), (0, 1, 0), (0, 1, 1), (1, 0, 2)])
+def test_two_b_buffers_prefetch_in_chunks_with_every_layout(H, monkeypatch, transa, transb, tri):
+    """Plans with two B slice buffers prefetch the next slice in chunks between the steps of a column; for a transposed B the
+    chunks are ranges of its n rows, and with the triangle mask a column has fewer live steps to hang them on.  Forced here
+    (the planner picks two buffers only for large compute-bound problems), integers, bit-exact."""
+    monkeypatch.setenv("HCLOOC_FORCE_BBUF", "2")
+    monkeypatch.setenv("HCLOOC_FORCE_NB", "256")
+    monkeypatch.setenv("HCLOOC_FORCE_MB", "128")
+    N, K = 1100, 300
+    M = N
+    ctx = H.hclooc_ctx_create(0)
+    try:
+        if tri:
+            A = H.HostMatrix(K, N) if transa else H.HostMatrix(N, K)
+            C = H.HostMatrix(N, N)
+            synthgen.fill(A.array, 86, "A", "int"); synthgen.fill(C.array, 86, "C", "int")
+            ref = C.view.copy()
+            oracle.dsyrk(tri - 1, transa, 1.0, A.view, 0.5, ref)
+            st = H.hclooc_dsyrk(ctx, tri - 1, transa, N, K, 1.0, A, A.ld, 0.5, C, N, 64 * MiB)
+        else:
+            A, B, C = stored_inputs(H, transa, transb, M, N, K, 86, "int")
+            opA, opB = np.empty((M, K)), np.empty((K, N))
+            opA[...] = A.view.T if transa else A.view
+            opB[...] = B.view.T if transb else B.view
+            ref = C.view.copy()
+            oracle.dgemm(1.0, opA, opB, 0.5, ref)
+            st = H.hclooc_dgemm_t(ctx, transa, transb, M, N, K, 1.0, A, A.ld, B, B.ld, 0.5, C, C.ld, 64 * MiB)
+        assert st.plan.n_bbuf == 2 and st.plan.w >= 4 and st.plan.h >= 8 and st.plan.direct == 0
+        assert np.array_equal(C.view, ref)
+    finally:
+        H.hclooc_ctx_destroy(ctx)
