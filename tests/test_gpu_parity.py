@@ -1013,3 +1013,34 @@ def test_two_b_buffers_prefetch_in_chunks_with_every_layout(H, monkeypatch, tran
         assert np.array_equal(C.view, ref)
     finally:
         H.hclooc_ctx_destroy(ctx)
+
+
+def test_graph_replay_with_transposed_operands_and_triangle_mask(H):
+    """The CUDA-graph replay of a repeated short call carries the operand layouts and the triangle mask: a transposed DGEMM
+    and a DSYRK, four identical calls each (ordinary, capture + launch, replay, replay), alternating never reuses a graph."""
+    N, K = 512, 384
+    A, B, C = stored_inputs(H, 1, 1, N, N, K, 87, "int")
+    C0 = C.view.copy()
+    opA, opB = np.empty((N, K)), np.empty((K, N))
+    opA[...] = A.view.T; opB[...] = B.view.T
+    ref_t = C0.copy(); oracle.dgemm(1.0, opA, opB, 0.5, ref_t)
+    ref_s = C0.copy(); oracle.dsyrk(0, 1, 1.0, A.view, 0.5, ref_s)                 # A is stored K x N: trans = T
+    ctx = H.hclooc_ctx_create(0)
+    try:
+        for rep in range(4):
+            C.view[...] = C0
+            st = H.hclooc_dgemm_t(ctx, 1, 1, N, N, K, 1.0, A, A.ld, B, B.ld, 0.5, C, C.ld, 1 * MiB)
+            assert st.plan.n_steps > 4 and np.array_equal(C.view, ref_t)
+        for rep in range(4):
+            C.view[...] = C0
+            st = H.hclooc_dsyrk(ctx, 0, 1, N, K, 1.0, A, A.ld, 0.5, C, C.ld, 1 * MiB)
+            assert np.array_equal(C.view, ref_s)
+        for rep in range(3):
+            C.view[...] = C0
+            H.hclooc_dgemm_t(ctx, 1, 1, N, N, K, 1.0, A, A.ld, B, B.ld, 0.5, C, C.ld, 1 * MiB)
+            assert np.array_equal(C.view, ref_t)
+            C.view[...] = C0
+            H.hclooc_dsyrk(ctx, 0, 1, N, K, 1.0, A, A.ld, 0.5, C, C.ld, 1 * MiB)
+            assert np.array_equal(C.view, ref_s)
+    finally:
+        H.hclooc_ctx_destroy(ctx)
