@@ -1044,3 +1044,33 @@ def test_graph_replay_with_transposed_operands_and_triangle_mask(H):
             assert np.array_equal(C.view, ref_s)
     finally:
         H.hclooc_ctx_destroy(ctx)
+
+
+def test_config2_full_size_transposed_sampled_rows_and_columns(H):
+    """BASELINE configs[1] shape with both operands transposed (bench.py --trans TT): 8192^3 under 256 MiB, integer variant:
+    complete rows and columns on both sides of the plan's slab boundaries against the oracle, and exact whole-matrix checksums."""
+    M = N = K = 8192
+    A, B, C = stored_inputs(H, 1, 1, M, N, K, synthgen.BASE_SEED + 2, "int")
+    opA, opB = np.empty((M, K)), np.empty((K, N))
+    opA[...] = A.view.T; opB[...] = B.view.T
+    plan = H.hclooc_plan_trans(M, N, K, 1, 0, 256 * MiB, 0, 1, 1)
+    rng = np.random.default_rng(6)
+    rows = {0, M - 1} | {int(x) for x in rng.integers(0, M, 4)}
+    cols = {0, N - 1} | {int(x) for x in rng.integers(0, N, 4)}
+    for i in (1, plan.h // 2, plan.h - 1):
+        rows |= {i * plan.mb - 1, i * plan.mb}
+    for j in range(1, plan.w):
+        cols |= {j * plan.nb - 1, j * plan.nb}
+    rows, cols = np.array(sorted(rows)), np.array(sorted(cols))
+    C0 = C.view.copy()
+    ref_r, _ = oracle.dgemm_sub(1.0, opA, opB, 1.0, C0, rows=rows)
+    ref_c, _ = oracle.dgemm_sub(1.0, opA, opB, 1.0, C0, cols=cols)
+    st = H.hclooc_dgemm_t(None, 1, 1, M, N, K, 1.0, A, A.ld, B, B.ld, 1.0, C, C.ld, 256 * MiB)
+    assert st.plan.trans == 3 and st.plan.workspace_bytes <= 256 * MiB and st.bytes_h2d == st.plan.bytes_h2d
+    assert (st.plan.mb, st.plan.nb) == (plan.mb, plan.nb)
+    assert np.array_equal(C.view[rows], ref_r) and np.array_equal(C.view[:, cols], ref_c)
+    x = synthgen.fill_numpy(N, 1, 77, "A", "int"); y = synthgen.fill_numpy(1, M, 77, "B", "int")
+    assert np.array_equal(C.view @ x, opA @ (opB @ x) + C0 @ x)
+    assert np.array_equal(y @ C.view, (y @ opA) @ opB + y @ C0)
+    for X in (A, B, C):
+        X.free()
