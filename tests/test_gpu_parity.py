@@ -1074,3 +1074,29 @@ def test_config2_full_size_transposed_sampled_rows_and_columns(H):
     assert np.array_equal(y @ C.view, (y @ opA) @ opB + y @ C0)
     for X in (A, B, C):
         X.free()
+
+
+def test_dsyrk_large_exact_checksums(H):
+    """DSYRK at a size with many blocks and several B slices (12288^2 x 2048 under 512 MiB), integer inputs: the lower triangle
+    mirrored to a full symmetric matrix satisfies S x = alpha*A*(A^T x) + beta*S0 x exactly for an integer x (any wrong element
+    changes a row sum), the strict upper triangle keeps its bits, sampled rows equal the oracle."""
+    N, K = 12288, 2048
+    A, C = H.HostMatrix(N, K), H.HostMatrix(N, N)
+    synthgen.fill(A.array, 88, "A", "int"); synthgen.fill(C.array, 88, "C", "int")
+    upper0 = np.triu(C.view, 1).copy()
+    low0 = np.tril(C.view)
+    S0 = low0 + np.tril(C.view, -1).T
+    x = synthgen.fill_numpy(N, 1, 78, "A", "int")[:, 0]
+    want = 2.0 * (A.view @ (A.view.T @ x)) + 0.5 * (S0 @ x)
+    rows = np.array([0, 127, 128, 4095, 4096, 8191, 8192, N - 1])
+    At = np.empty((K, N)); At[...] = A.view.T
+    ref_rows, _ = oracle.dgemm_sub(2.0, A.view, At, 0.5, C.view.copy(), rows=rows)
+    st = H.hclooc_dsyrk(None, H.HCL_UPLO_LOWER, H.HCL_OP_N, N, K, 2.0, A, K, 0.5, C, N, 512 * MiB)
+    assert st.plan.tri == 1 and st.plan.w >= 2 and st.bytes_d2h < 8 * N * N * 0.8          # blocks above the diagonal never moved
+    assert np.array_equal(np.triu(C.view, 1), upper0)
+    S = np.tril(C.view) + np.tril(C.view, -1).T
+    assert np.array_equal(S @ x, want)
+    for q, i in enumerate(rows):
+        assert np.array_equal(C.view[i, : i + 1], ref_rows[q, : i + 1]), i
+    for X in (A, C):
+        X.free()
