@@ -499,7 +499,7 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
         if ((size_t)(q - base) != P.workspace_bytes) return HCLOOC_ERR_INTERNAL;
     }
     // ---------------------------------------------------------------- events
-    const size_t n_events = 3 * (size_t)P.n_sets + 2 * (size_t)P.n_bbuf + 2 * (size_t)P.n_abuf;
+    const size_t n_events = (size_t)EventIds{P.n_sets, P.n_bbuf, std::max(1, (int)P.n_abuf)}.count();
     while (ctx->events.size() < n_events) {
         cudaEvent_t e;
         HCL_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));

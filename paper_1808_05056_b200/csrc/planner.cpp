@@ -189,7 +189,6 @@ void cost(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool scale_onl
     // one step's kernel running alone: what the link waits for when a column drains, and the tail of the call
     const double sms_step = c.ksplit < 0 ? (double)NUM_SMS : std::min<double>(NUM_SMS, tiles_step * c.ksplit);
     const double t_kernel = (flops / std::max(1.0, steps)) / (mm.fp64_flops * sms_step / NUM_SMS) + mm.launch_latency_s;
-    const double switches = (double)c.w * c.kpanels - 1.0;
     // Column by column: the first column of a K panel uploads every A slice, the later ones only what the cache
     // lost, so the link demand is front-loaded -- a plan with many thin columns is link-bound in its first column
     // even when the whole call is compute-bound (measured: config 4 with 47 columns lost 2 % there).
