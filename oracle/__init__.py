@@ -7,7 +7,8 @@ __graft_entry__.smoke() and bench.py's cpu_baseline / `--impl reference` legs us
 
 Pinned by tests/test_oracle_pins.py (brute force, int64 exactness, closed forms, exact-sum error
 bound, numpy cross-check, the paper's 44-element partition example; dsyrk: brute force on the triangle,
-exact symmetry, int64 exactness, untouched other triangle) -- nothing here is "parity unpinned".
+exact symmetry, int64 exactness, untouched other triangle; dtrsm: scipy's solve_triangular, exact rational
+arithmetic on tiny cases, identity / diagonal / all-ones closed forms, int64 exactness, transposed-storage identity) -- nothing here is "parity unpinned".
 """
 from __future__ import annotations
 
@@ -50,6 +51,11 @@ def _load():
                                          _i64, _ptr, _i64, _ptr, _ptr, _ptr]
         lib.oracle_partition.restype = ctypes.c_int
         lib.oracle_partition.argtypes = [_i64, _i64, _i64, _i64, ctypes.POINTER(_i64), ctypes.POINTER(_i64)]
+        lib.oracle_dtrsm.restype = ctypes.c_int
+        lib.oracle_dtrsm.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, _i64, _i64, _dbl, _ptr, _i64, _ptr, _i64]
+        lib.oracle_dtrsm_residual.restype = ctypes.c_int
+        lib.oracle_dtrsm_residual.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, _i64, _i64, _dbl, _ptr, _i64, _ptr, _i64,
+                                              _ptr, _i64, _i64, _ptr, _i64, _ptr, _ptr, _ptr]
         _lib = lib
     return _lib
 
@@ -159,6 +165,44 @@ def dsyr2k(uplo, trans, alpha, A, B, beta, C, want_denominator=False):
     D = D1 + (D2 - np.abs(mid))          # D2 = |alpha| sum |b||a| + |1||mid|: take the product part, keep D1's |beta||C0|
     D[~keep] = 0.0
     return D
+
+
+def dtrsm(uplo, trans, unit, alpha, A, B):
+    """Solve op(T) X = alpha B by substitution (oracle_dtrsm: the definition, PAPER.md:412 names the routine), X overwrites B.
+    T = the `uplo` (0 lower, 1 upper) triangle of the square row-major A, op = transpose when trans, unit diagonal when unit."""
+    M, N = B.shape
+    assert A.shape == (M, M) or alpha == 0.0
+    ap, lda = _chk2d(A, "A") if A is not None and A.size else (0, max(M, 1))
+    bp, ldb = _chk2d(B, "B") if B.size else (0, max(N, 1))
+    rc = _load().oracle_dtrsm(int(uplo), int(trans), int(unit), M, N, float(alpha), ap, lda, bp, ldb)
+    if rc != 0:
+        raise ValueError("oracle_dtrsm: bad argument")
+
+
+# gate for a triangular solve of order M: substitution in any summation order leaves a residual
+# |alpha b - op(T) x| <= gamma_M |op(T)||x| elementwise, gamma_M = M u / (1 - M u), u = 2^-53 (Higham thm 8.5); the product
+# alpha*b adds one rounding.  DESIGN.md reading G23.
+def dtrsm_gate(M: int) -> float:
+    u = 2.0 ** -53
+    return (M + 2) * u / (1.0 - (M + 2) * u)
+
+
+def dtrsm_residual(uplo, trans, unit, alpha, A, B0, X, rows=None, cols=None):
+    """(res, den) of oracle_dtrsm_residual on the sampled rows x cols (None: all), computed in long double."""
+    M, N = B0.shape
+    ap, lda = _chk2d(A, "A")
+    bp, ldb = _chk2d(B0, "B0")
+    xp, ldx = _chk2d(X, "X")
+    r = None if rows is None else np.ascontiguousarray(rows, dtype=np.int64)
+    c = None if cols is None else np.ascontiguousarray(cols, dtype=np.int64)
+    nr, nc = (M if r is None else r.size), (N if c is None else c.size)
+    res, den = np.empty((nr, nc)), np.empty((nr, nc))
+    rc = _load().oracle_dtrsm_residual(int(uplo), int(trans), int(unit), M, N, float(alpha), ap, lda, bp, ldb, xp, ldx,
+                                       nr, 0 if r is None else r.ctypes.data, nc, 0 if c is None else c.ctypes.data,
+                                       res.ctypes.data, den.ctypes.data)
+    if rc != 0:
+        raise ValueError("oracle_dtrsm_residual: bad argument")
+    return res, den
 
 
 def partition(M, N, K, S):

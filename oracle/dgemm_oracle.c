@@ -176,3 +176,87 @@ int oracle_partition(int64_t M, int64_t N, int64_t K, int64_t S, int64_t* h_out,
     *h_out = best_h; *w_out = best_w;
     return 0;
 }
+
+/* ------------------------------------------------------------------------------------------------------------------
+ * DTRSM, side = Left (the level-3 BLAS routine the paper names as future work):
+ *     solve  op(T) * X = alpha * B  for X,   T = the `uplo` triangle of the M x M matrix A (row-major, lda >= M),
+ *     op(T) = T (trans = 0) or T^T (trans = 1), unit = 1: the diagonal of T is taken as 1 and not read.
+ * B is M x N row-major and is overwritten by X.  Only the `uplo` triangle of A is read.  alpha == 0: X = 0, A not read.
+ * The definition by substitution, written out (Golub & Van Loan alg. 3.1.1 / 3.1.2 applied to each column of B):
+ *     op(T) lower:  x_ij = (alpha*b_ij - sum_{k<i} t_ik x_kj) / t_ii,   i = 0 .. M-1
+ *     op(T) upper:  x_ij = (alpha*b_ij - sum_{k>i} t_ik x_kj) / t_ii,   i = M-1 .. 0
+ * with t_ik = op(T)_ik; the sum runs over k in increasing order (lower) or decreasing order from M-1 (upper), each product
+ * rounded, then subtracted (no FMA: compiled with -ffp-contract=off). */
+static inline double tri_at(const double* A, int64_t lda, int trans, int64_t i, int64_t k) {
+    return trans ? A[k * lda + i] : A[i * lda + k];
+}
+
+int oracle_dtrsm(int uplo, int trans, int unit, int64_t M, int64_t N, double alpha, const double* A, int64_t lda,
+                 double* B, int64_t ldb) {
+    if ((uplo != 0 && uplo != 1) || (trans != 0 && trans != 1) || (unit != 0 && unit != 1)) return -1;
+    if (M < 0 || N < 0) return -1;
+    if (M == 0 || N == 0) return 0;
+    if (!B || ldb < N) return -1;
+    if (alpha == 0.0) {
+        for (int64_t i = 0; i < M; ++i) for (int64_t j = 0; j < N; ++j) B[i * ldb + j] = 0.0;
+        return 0;
+    }
+    if (!A || lda < M) return -1;
+    /* op(T) is lower when (lower, no transpose) or (upper, transpose) */
+    const int lower = (uplo == 0) != (trans != 0);
+    #pragma omp parallel for schedule(static)
+    for (int64_t j = 0; j < N; ++j) {
+        if (lower) {
+            for (int64_t i = 0; i < M; ++i) {
+                double x = alpha * B[i * ldb + j];
+                for (int64_t k = 0; k < i; ++k) { const double p = tri_at(A, lda, trans, i, k) * B[k * ldb + j]; x = x - p; }
+                if (!unit) x = x / tri_at(A, lda, trans, i, i);
+                B[i * ldb + j] = x;
+            }
+        } else {
+            for (int64_t i = M - 1; i >= 0; --i) {
+                double x = alpha * B[i * ldb + j];
+                for (int64_t k = M - 1; k > i; --k) { const double p = tri_at(A, lda, trans, i, k) * B[k * ldb + j]; x = x - p; }
+                if (!unit) x = x / tri_at(A, lda, trans, i, i);
+                B[i * ldb + j] = x;
+            }
+        }
+    }
+    return 0;
+}
+
+/* Residual of a candidate solution X of op(T) X = alpha B on sampled entries, in long double (64-bit significand):
+ *     res[r*nc + c] = | alpha*b_ij - sum_k op(T)_ik x_kj |,   den[r*nc + c] = |alpha||b_ij| + sum_k |op(T)_ik||x_kj|
+ * for i = rows[r] (NULL: r), j = cols[c] (NULL: c), k over the triangle (diagonal term: 1*x_ij when unit).  Substitution in
+ * ANY order of summation satisfies res <= gamma_M * sum_k|t_ik||x_kj| (Higham, Accuracy and Stability, thm 8.5), which is the
+ * gate the parity tests apply to the GPU result at sizes where oracle_dtrsm itself would take too long. */
+int oracle_dtrsm_residual(int uplo, int trans, int unit, int64_t M, int64_t N, double alpha, const double* A, int64_t lda,
+                          const double* B0, int64_t ldb, const double* X, int64_t ldx,
+                          int64_t nr, const int64_t* rows, int64_t nc, const int64_t* cols, double* res, double* den) {
+    if ((uplo != 0 && uplo != 1) || (trans != 0 && trans != 1) || (unit != 0 && unit != 1)) return -1;
+    if (M < 0 || N < 0 || nr < 0 || nc < 0) return -1;
+    if (nr == 0 || nc == 0) return 0;
+    if (!A || !B0 || !X || !res || !den || lda < M || ldb < N || ldx < N) return -1;
+    const int lower = (uplo == 0) != (trans != 0);
+    for (int64_t r = 0; r < nr; ++r) { int64_t i = rows ? rows[r] : r; if (i < 0 || i >= M) return -1; }
+    for (int64_t c = 0; c < nc; ++c) { int64_t j = cols ? cols[c] : c; if (j < 0 || j >= N) return -1; }
+    #pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t r = 0; r < nr; ++r) {
+        const int64_t i = rows ? rows[r] : r;
+        const int64_t k0 = lower ? 0 : i, k1 = lower ? i : M - 1;
+        for (int64_t c = 0; c < nc; ++c) {
+            const int64_t j = cols ? cols[c] : c;
+            long double s = (long double)alpha * (long double)B0[i * ldb + j];
+            long double d = fabsl(s);
+            for (int64_t k = k0; k <= k1; ++k) {
+                const long double t = (k == i && unit) ? 1.0L : (long double)tri_at(A, lda, trans, i, k);
+                const long double x = (long double)X[k * ldx + j];
+                s -= t * x;
+                d += fabsl(t) * fabsl(x);
+            }
+            res[r * nc + c] = (double)fabsl(s);
+            den[r * nc + c] = (double)d;
+        }
+    }
+    return 0;
+}

@@ -392,3 +392,146 @@ def test_dsyr2k_brute_force_symmetry_and_integers():
     s1, s2 = np.zeros((N, N)), np.zeros((N, N))
     oracle.dsyr2k(0, 0, 1.0, A, A, 0.0, s1); oracle.dsyrk(0, 0, 2.0, A, 0.0, s2)
     assert np.array_equal(s1, s2)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# DTRSM (side = Left), the routine PAPER.md:412 names as future work: op(T) X = alpha B by substitution
+ALL_TRSM = list(itertools.product((0, 1), (0, 1), (0, 1)))          # uplo, trans, unit
+
+
+def tri_inputs(rng, M, N, pad=0, ints=False):
+    """A (M x M, NaN in the padding), B (M x N): well conditioned (rows of the off-diagonal part sum to < 1 in magnitude,
+    diagonal in [1, 2)) or small integers with a unit-friendly diagonal of +-1."""
+    abuf = np.full((max(M, 1), M + pad), np.nan); A = abuf[:M, :M]
+    bbuf = np.full((max(M, 1), N + pad), np.nan); B = bbuf[:M, :N]
+    if ints:
+        A[...] = rng.integers(-2, 3, (M, M)).astype(np.float64)
+        A[np.arange(M), np.arange(M)] = rng.choice([-1.0, 1.0], M)
+        B[...] = rng.integers(-4, 5, (M, N)).astype(np.float64)
+    else:
+        A[...] = rng.uniform(-1, 1, (M, M)) / max(M, 1)
+        A[np.arange(M), np.arange(M)] = rng.uniform(1, 2, M) * rng.choice([-1.0, 1.0], M)
+        B[...] = rng.uniform(-1, 1, (M, N))
+    return A, B
+
+
+def op_tri(A, uplo, trans, unit):
+    """op(T) written out densely (zeros outside the triangle, ones on a unit diagonal)."""
+    T = np.tril(A) if uplo == 0 else np.triu(A)
+    if unit:
+        T = T - np.diag(np.diag(T)) + np.eye(A.shape[0])
+    return T.T.copy() if trans else T
+
+
+@pytest.mark.parametrize("uplo,trans,unit", ALL_TRSM)
+def test_dtrsm_exact_rational_arithmetic_on_tiny_cases(uplo, trans, unit):
+    """Brute force: the solution in exact rational arithmetic (fractions), rounded once, against the oracle within the
+    substitution bound gamma_M cond-free residual gate AND to a few ulps on these well conditioned 5 x 5 cases."""
+    from fractions import Fraction
+    rng = np.random.default_rng(7)
+    M, N, alpha = 5, 3, -1.5
+    A, B = tri_inputs(rng, M, N, pad=2)
+    other = np.triu(np.ones((M, M), bool), 1) if uplo == 0 else np.tril(np.ones((M, M), bool), -1)
+    A[other] = np.nan                                              # the other triangle must not be read
+    if unit:
+        A[np.arange(M), np.arange(M)] = np.nan                     # nor a unit diagonal
+    X = B.copy()
+    oracle.dtrsm(uplo, trans, unit, alpha, A, X)
+    T = op_tri(np.nan_to_num(A), uplo, trans, unit)
+    Tf = [[Fraction(float(T[i, k])) for k in range(M)] for i in range(M)]
+    lower = (uplo == 0) != bool(trans)
+    order = range(M) if lower else range(M - 1, -1, -1)
+    for j in range(N):
+        x = [None] * M
+        for i in order:
+            s = Fraction(alpha) * Fraction(float(B[i, j]))
+            for k in (range(i) if lower else range(i + 1, M)):
+                s -= Tf[i][k] * x[k]
+            x[i] = s / Tf[i][i]
+        for i in range(M):
+            assert abs(X[i, j] - float(x[i])) <= 8 * np.spacing(abs(float(x[i]))), (i, j)
+
+
+@pytest.mark.parametrize("uplo,trans,unit", ALL_TRSM)
+def test_dtrsm_against_scipy_and_residual_gate(uplo, trans, unit):
+    import scipy.linalg as sl
+    rng = np.random.default_rng(11)
+    M, N, alpha = 61, 17, 0.75
+    A, B = tri_inputs(rng, M, N, pad=3)
+    X = B.copy()
+    oracle.dtrsm(uplo, trans, unit, alpha, A, X)
+    ref = sl.solve_triangular(A, alpha * B, lower=(uplo == 0), trans=trans, unit_diagonal=bool(unit))
+    assert np.abs(X - ref).max() <= 1e-13 * np.abs(ref).max()
+    res, den = oracle.dtrsm_residual(uplo, trans, unit, alpha, A, B, X)
+    assert (res <= oracle.dtrsm_gate(M) * den).all()
+    # the residual function itself, against the dense product in numpy (longdouble) -- and it does notice a wrong X
+    T = op_tri(A, uplo, trans, unit).astype(np.longdouble)
+    r2 = np.abs(np.longdouble(alpha) * B.astype(np.longdouble) - T @ X.astype(np.longdouble))
+    assert np.allclose(res, r2.astype(np.float64), rtol=0, atol=1e-18)
+    Xbad = X.copy(); Xbad[M // 2, N // 2] *= 1.0 + 1e-9
+    res, den = oracle.dtrsm_residual(uplo, trans, unit, alpha, A, B, Xbad)
+    assert not (res <= oracle.dtrsm_gate(M) * den).all()
+    # sampled rows / columns pick the same numbers
+    rows, cols = np.array([0, 5, M - 1]), np.array([N - 1, 2])
+    rs, ds = oracle.dtrsm_residual(uplo, trans, unit, alpha, A, B, X, rows, cols)
+    rf, df = oracle.dtrsm_residual(uplo, trans, unit, alpha, A, B, X)
+    assert np.array_equal(rs, rf[np.ix_(rows, cols)]) and np.array_equal(ds, df[np.ix_(rows, cols)])
+
+
+def test_dtrsm_closed_forms():
+    rng = np.random.default_rng(3)
+    M, N = 19, 7
+    B = rng.uniform(-1, 1, (M, N))
+    for uplo, trans, unit in ALL_TRSM:
+        # identity: X = alpha*B exactly (one multiplication, a division by 1)
+        X = B.copy(); oracle.dtrsm(uplo, trans, unit, 2.5, np.eye(M), X)
+        assert np.array_equal(X, 2.5 * B)
+        # diagonal: x_ij = (alpha*b_ij)/d_i, or alpha*b_ij when the diagonal is declared unit
+        d = rng.uniform(1, 2, M)
+        X = B.copy(); oracle.dtrsm(uplo, trans, unit, -0.5, np.diag(d), X)
+        assert np.array_equal(X, (-0.5 * B) if unit else (-0.5 * B) / d[:, None])
+        # alpha == 0: zeros, A not read (NaN), NaN in B not propagated (BLAS convention)
+        X = B.copy(); X[3, 2] = np.nan
+        oracle.dtrsm(uplo, trans, unit, 0.0, np.full((M, M), np.nan), X)
+        assert np.array_equal(X, np.zeros((M, N)))
+    # all-ones lower triangle: T X = cumulative sums of X, so X = first differences of B (exact on integers)
+    Bi = rng.integers(-50, 51, (M, N)).astype(np.float64)
+    ones = np.ones((M, M))
+    X = Bi.copy(); oracle.dtrsm(0, 0, 0, 1.0, ones, X)
+    assert np.array_equal(X, np.diff(Bi, axis=0, prepend=0.0))
+    X = Bi.copy(); oracle.dtrsm(1, 0, 1, 1.0, ones, X)                # upper: differences from below
+    assert np.array_equal(X, Bi - np.vstack([Bi[1:], np.zeros((1, N))]))
+    # M == 0, N == 0
+    oracle.dtrsm(0, 0, 0, 1.0, np.zeros((0, 0)), np.zeros((0, 5)))
+    oracle.dtrsm(0, 0, 0, 1.0, np.eye(4), np.zeros((4, 0)))
+
+
+@pytest.mark.parametrize("uplo,trans,unit", ALL_TRSM)
+def test_dtrsm_integers_are_exact(uplo, trans, unit):
+    """B := op(T) X0 in int64, then the solve must return X0 bit for bit (every intermediate is a small integer; the
+    diagonal is +-1, so the divisions are exact too)."""
+    rng = np.random.default_rng(5)
+    M, N = 67, 9
+    A, _ = tri_inputs(rng, M, N, ints=True)
+    X0 = rng.integers(-3, 4, (M, N))
+    T = op_tri(A, uplo, trans, unit).astype(np.int64)
+    B = (T @ X0).astype(np.float64)
+    X = B.copy()
+    oracle.dtrsm(uplo, trans, unit, 1.0, A, X)
+    assert np.array_equal(X, X0.astype(np.float64))
+    X = B.copy()
+    oracle.dtrsm(uplo, trans, unit, 2.0, A, X)
+    assert np.array_equal(X, 2.0 * X0)
+
+
+def test_dtrsm_transposed_storage_identity():
+    """(uplo, trans = 1) on A is the same computation as (other uplo, trans = 0) on the written-out transpose."""
+    rng = np.random.default_rng(9)
+    M, N = 33, 5
+    A, B = tri_inputs(rng, M, N)
+    At = A.T.copy()
+    for uplo in (0, 1):
+        for unit in (0, 1):
+            X1 = B.copy(); oracle.dtrsm(uplo, 1, unit, 1.25, A, X1)
+            X2 = B.copy(); oracle.dtrsm(1 - uplo, 0, unit, 1.25, At, X2)
+            assert np.array_equal(X1, X2)
