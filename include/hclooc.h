@@ -262,6 +262,28 @@ int hclooc_dsyr2k(hclooc_ctx* ctx, int uplo, int trans, int64_t N, int64_t K, do
                   const double* B, int64_t ldb, double beta, double* C, int64_t ldc, size_t device_budget_bytes,
                   hclooc_stats* stats_out);
 
+/* Out-of-core DTRSM, side = Left (the paper's future work, :412):  solve
+ *     op(T) * X = alpha * B,   op(T) = T (trans = HCL_OP_N) or T^T (HCL_OP_T),
+ * where T is the `uplo` triangle of the M x M matrix A (row-major, lda >= M; the other triangle is never read, nor is the
+ * diagonal when diag = HCL_DIAG_UNIT) and B is M x N (ldb >= N); X overwrites B in place.  A and B are pinned host memory
+ * (device memory is accepted too and staged the same way).  Blocked substitution: B is cut into block rows of NB <= 4096
+ * rows (NB*NB*8 <= half the budget); a block row first receives  B_i <- alpha*B_i - op(T)[i, solved]*X[solved]  as ONE
+ * out-of-core DGEMM through the hclooc_dgemm_t pipeline, then its diagonal block is solved in device memory: T_ii is
+ * uploaded once, B_i streams through two column-chunk buffers on two streams, and inside a chunk 128-row triangles are
+ * solved by a substitution kernel (one thread per column of B) with the tile kernel updating the rows still to be solved.
+ * Rounding: substitution with the sums over k taken in blocked order; the result satisfies the elementwise residual bound
+ * |alpha*B - op(T) X| <= gamma_(M+2) (|alpha B| + |op(T)||X|) of substitution in any order (G23), and is exact on
+ * integer data with a +-1 diagonal.  alpha == 0: X = 0, A not referenced.  M == 0 or N == 0: nothing is done.
+ * stats (nullable): byte / copy / kernel counts summed over the DGEMM calls and the diagonal phases; plan.mb = NB,
+ * plan.nb = chunk width, plan.h = block rows, plan.flops = M*M*N, plan.workspace_bytes = the most device memory used.
+ * Errors: -2 uplo, -3 trans, -4 diag, -5 M < 0, -6 N < 0, -8 A NULL, -9 lda < M, -10 B NULL or overlapping A,
+ * -11 ldb < N; HCLOOC_ERR_BUDGET when not even a 32-row block fits; the HCLOOC_ERR_* codes of hclooc_dgemm.  A singular
+ * T gives Inf / NaN as in the BLAS (no check).  Validation errors leave B untouched.                                    */
+#define HCL_DIAG_NONUNIT 0
+#define HCL_DIAG_UNIT    1
+int hclooc_dtrsm(hclooc_ctx* ctx, int uplo, int trans, int diag, int64_t M, int64_t N, double alpha, const double* A, int64_t lda,
+                 double* B, int64_t ldb, size_t device_budget_bytes, hclooc_stats* stats_out);
+
 /* nsteps mode (:277-283): MMOOC as a subroutine of a blocked algorithm (SUMMA, HSUMMA) that updates the same C
  * `nsteps` times: C = alpha*A_p*B_p + beta_p*C for p = *step = 0 .. nsteps-1, one call per p.  C is uploaded once
  * at step 0 (if beta != 0), stays in device memory between the calls, and is downloaded once at the last step, so

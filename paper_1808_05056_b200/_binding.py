@@ -11,12 +11,13 @@ from . import build as _build
 HCL_H2D, HCL_D2H = 0, 1
 HCL_OP_N, HCL_OP_T = 0, 1
 HCL_UPLO_LOWER, HCL_UPLO_UPPER = 0, 1
+HCL_DIAG_NONUNIT, HCL_DIAG_UNIT = 0, 1
 
 # every symbol include/hclooc.h declares (tests check the .so exports all of them)
 EXPORTS = [
     "hclooc_plan", "hclooc_plan_ex", "hclooc_plan_trans", "hclooc_shard_rows", "hclMatrixPartitioner", "hclooc_schedule", "hclooc_ctx_create", "hclooc_ctx_destroy",
     "hclooc_ctx_set_trace", "hclooc_ctx_get_trace", "hclooc_ctx_set_direct",
-    "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_t", "hclooc_dsyrk", "hclooc_dsyr2k", "hclooc_dgemm_fig2", "hclooc_dgemm_nsteps", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
+    "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_t", "hclooc_dsyrk", "hclooc_dsyr2k", "hclooc_dtrsm", "hclooc_dgemm_fig2", "hclooc_dgemm_nsteps", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
     "hclStreamDestroy", "hclEventDestroy", "hclMemcpy", "hclMemcpyAsync", "hclMemcpy2DAsync",
     "hclDgemmAsync", "hclDgemmAsyncEx", "hclDgemmAsyncT", "hclWaitEvent", "hclStreamSynchronize", "hclDeviceSynchronize",
     "hclooc_host_alloc", "hclooc_host_free", "hclooc_host_register", "hclooc_host_unregister",
@@ -89,6 +90,7 @@ def lib():
         L.hclooc_dgemm_ex.argtypes = [vp, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
         L.hclooc_dgemm_t.argtypes = [vp, c_int, c_int, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
         L.hclooc_dsyrk.argtypes = [vp, c_int, c_int, i64, i64, dbl, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
+        L.hclooc_dtrsm.argtypes = [vp, c_int, c_int, c_int, i64, i64, dbl, vp, i64, vp, i64, sz, POINTER(Stats)]
         L.hclooc_dsyr2k.argtypes = [vp, c_int, c_int, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
         L.hclooc_dgemm_nsteps.argtypes = [vp, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, c_int, POINTER(c_int), POINTER(Stats)]
         L.hclooc_dgemm_fig2.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
@@ -317,6 +319,14 @@ def hclooc_dsyr2k(ctx, uplo, trans, N, K, alpha, A, lda, B, ldb, beta, C, ldc, d
     st = Stats()
     _check(lib().hclooc_dsyr2k(ctx, int(uplo), int(trans), N, K, alpha, _ptr(A), lda, _ptr(B), ldb, beta, _ptr(C), ldc,
                                device_budget_bytes, byref(st) if want_stats else None), "hclooc_dsyr2k")
+    return st if want_stats else None
+
+
+def hclooc_dtrsm(ctx, uplo, trans, diag, M, N, alpha, A, lda, B, ldb, device_budget_bytes, want_stats=True):
+    """Solve op(T) X = alpha*B in place (X overwrites B); T = the `uplo` triangle of the M x M matrix A, diag: HCL_DIAG_*."""
+    st = Stats()
+    _check(lib().hclooc_dtrsm(ctx, int(uplo), int(trans), int(diag), M, N, alpha, _ptr(A), lda, _ptr(B), ldb,
+                              device_budget_bytes, byref(st) if want_stats else None), "hclooc_dtrsm")
     return st if want_stats else None
 
 

@@ -798,6 +798,186 @@ extern "C" int hclooc_dgemm(int64_t M, int64_t N, int64_t K, double alpha, const
 }
 
 // ---------------------------------------------------------------------------------------------
+// Out-of-core DTRSM, side = Left (PAPER.md:412 names the routine as future work):
+//     solve op(T) * X = alpha * B,  X overwrites B (M x N, host), T = the `uplo` triangle of the M x M host matrix A.
+// Blocked substitution, left-looking at the out-of-core level: the rows of B are cut into block rows of NB rows; block row i
+// first receives the contribution of the block rows already solved,
+//     B_i <- alpha*B_i - op(T)[i, solved] * X[solved]          one out-of-core DGEMM (dgemm_core: K = rows solved so far)
+// then its diagonal block is solved in device memory:  T_ii (NB x NB) is uploaded once, B_i streams through two column
+// chunks on two streams (upload, solve, download -- each chunk in stream order, the two chunks overlapping), and inside a
+// chunk the solve is right-looking over 128-row blocks: trsm_block_kernel on the 128 x 128 triangle, then one tile-kernel
+// launch that updates the rows of the chunk still to be solved.  Left-looking outside keeps the traffic at one read of
+// X[solved] per block row (2*NB flops per 8 bytes: NB = 4096 is compute bound on this link); right-looking inside gives
+// the tile kernel launches of hundreds of tiles instead of 16.
+namespace {
+
+int ensure_workspace(hclooc_ctx* ctx, size_t bytes) {
+    if (bytes <= ctx->workspace_bytes) return HCLOOC_OK;
+    if (ctx->workspace && !ctx->owns_workspace) return HCLOOC_ERR_BUDGET;
+    if (ctx->workspace) { HCL_CUDA(cudaDeviceSynchronize()); cudaFree(ctx->workspace); ctx->workspace = nullptr; ctx->workspace_bytes = 0; }
+    void* p = nullptr;
+    cudaError_t e = cudaMalloc(&p, bytes);
+    if (e != cudaSuccess) { set_last_cuda_error((int)e); cudaGetLastError(); return HCLOOC_ERR_NOMEM; }
+    ctx->workspace = p; ctx->workspace_bytes = bytes; ctx->owns_workspace = true;
+    return HCLOOC_OK;
+}
+
+struct TrsmShape { int64_t NB, ldt, wc; size_t bytes; };
+
+// Block-row height NB, chunk width wc and the device bytes of the diagonal phase under `budget`: the triangle buffer takes
+// at most half of it (NB <= 4096: beyond that the DGEMM updates gain nothing and the diagonal phase, which no DGEMM
+// overlaps, grows), the two chunk buffers share the rest.
+int trsm_shape(int64_t M, int64_t N, size_t budget, TrsmShape* out) {
+    int64_t NB = 4096;
+    while (NB > 128 && (size_t)NB * NB * 8 > budget / 2) NB -= 128;
+    while (NB > 32 && (size_t)NB * NB * 8 > budget / 2) NB -= 32;
+    if (NB > M) NB = M;
+    const int64_t ldt = (NB + 1) & ~(int64_t)1;
+    const size_t tbytes = ((size_t)NB * ldt * 8 + 1023) & ~(size_t)1023;
+    if (tbytes + 2 * (size_t)NB * 64 * 8 + 4096 > budget) return HCLOOC_ERR_BUDGET;
+    int64_t wc = (int64_t)((budget - tbytes - 4096) / (2 * (size_t)NB * 8)) / 64 * 64;
+    const int64_t npad = (N + 63) / 64 * 64;
+    if (wc > npad) wc = npad;
+    // two chunks in flight overlap copies with kernels: do not take the whole width in one chunk when N is large
+    if (wc == npad && N >= 4096) wc = (npad / 2 + 63) / 64 * 64;
+    out->NB = NB; out->ldt = ldt; out->wc = wc;
+    out->bytes = tbytes + 2 * (((size_t)NB * wc * 8 + 1023) & ~(size_t)1023);
+    return HCLOOC_OK;
+}
+
+}  // namespace
+
+extern "C" int hclooc_dtrsm(hclooc_ctx* ctx, int uplo, int trans, int diag, int64_t M, int64_t N, double alpha,
+                            const double* A, int64_t lda, double* B, int64_t ldb, size_t device_budget_bytes, hclooc_stats* stats) {
+    const auto t_begin = std::chrono::steady_clock::now();
+    if (uplo != HCL_UPLO_LOWER && uplo != HCL_UPLO_UPPER) return -2;
+    if (trans != HCL_OP_N && trans != HCL_OP_T) return -3;
+    if (diag != HCL_DIAG_NONUNIT && diag != HCL_DIAG_UNIT) return -4;
+    if (M < 0) return -5;
+    if (N < 0) return -6;
+    if (stats) std::memset(stats, 0, sizeof(*stats));
+    if (M == 0 || N == 0) return HCLOOC_OK;
+    if (alpha != 0.0) {
+        if (!A) return -8;
+        if (lda < M) return -9;
+    }
+    if (!B) return -10;
+    if (ldb < N) return -11;
+    if (alpha != 0.0 && overlaps(B, M, N, ldb, A, M, M, lda)) return -10;
+    int rc;
+    if (alpha == 0.0) {                                              // X = 0, A not referenced, NaN in B not propagated
+        rc = dgemm_core(ctx, 0, 0, M, N, 0, 0.0, nullptr, 1, nullptr, 1, 0.0, B, ldb, device_budget_bytes, stats);
+        return rc == -10 ? -10 : rc;
+    }
+    if (!ctx && (rc = default_ctx(&ctx))) return rc;
+    size_t budget = device_budget_bytes;
+    {
+        std::lock_guard<std::mutex> lk(ctx->mu);
+        HCL_CUDA(cudaSetDevice(ctx->device));
+        bool dummy = true;
+        if ((rc = check_resident(A, &dummy)) || (rc = check_resident(B, &dummy))) return rc;
+        if (!ctx->owns_workspace && ctx->workspace) {
+            budget = (budget == 0) ? ctx->workspace_bytes : std::min(budget, ctx->workspace_bytes);
+        } else if (budget == 0) {
+            size_t fr = 0, tot = 0;
+            HCL_CUDA(cudaMemGetInfo(&fr, &tot));
+            fr += ctx->workspace_bytes;
+            const size_t margin = (size_t)1 << 30;
+            budget = fr > 2 * margin ? fr - margin : fr / 2;
+        }
+    }
+    TrsmShape S;
+    if ((rc = trsm_shape(M, N, budget, &S))) return rc;
+    const bool lower = (uplo == HCL_UPLO_LOWER) != (trans == HCL_OP_T);       // op(T) is lower triangular
+    const int64_t nblk = (M + S.NB - 1) / S.NB;
+    hclooc_stats acc;
+    std::memset(&acc, 0, sizeof(acc));
+    double t_enq = 0.0;
+    size_t ws_max = S.bytes;
+    for (int64_t bi = 0; bi < nblk; ++bi) {
+        const int64_t i = lower ? bi : nblk - 1 - bi;
+        const int64_t r0 = i * S.NB, nbi = std::min(S.NB, M - r0), r1 = r0 + nbi;
+        // ---- rows already solved: [0, r0) when op(T) is lower, [r1, M) when it is upper
+        const int64_t k0 = lower ? 0 : r1, kk = lower ? r0 : M - r1;
+        double alpha_eff = alpha;
+        if (kk > 0) {
+            const double* Ap = trans ? A + k0 * lda + r0 : A + r0 * lda + k0;       // op(T)[rows of i, solved rows], as stored
+            hclooc_stats one;
+            rc = dgemm_core(ctx, trans ? 1 : 0, 0, nbi, N, kk, -1.0, Ap, lda, B + k0 * ldb, ldb, alpha, B + r0 * ldb, ldb, budget, &one);
+            if (rc) return rc;
+            acc.bytes_h2d += one.bytes_h2d; acc.bytes_d2h += one.bytes_d2h; acc.n_kernels += one.n_kernels;
+            acc.n_copies_h2d += one.n_copies_h2d; acc.n_copies_d2h += one.n_copies_d2h; t_enq += one.t_enqueue_s;
+            ws_max = std::max(ws_max, (size_t)one.plan.workspace_bytes);
+            alpha_eff = 1.0;
+        }
+        // ---- the diagonal block, in device memory
+        std::lock_guard<std::mutex> lk(ctx->mu);
+        HCL_CUDA(cudaSetDevice(ctx->device));
+        const auto te0 = std::chrono::steady_clock::now();
+        if ((rc = ensure_workspace(ctx, S.bytes + 1024))) return rc;
+        uint8_t* base = (uint8_t*)ctx->workspace;
+        const uintptr_t mis = (uintptr_t)base & 1023u;
+        if (mis) base += 1024 - mis;
+        double* dT = (double*)base;
+        const size_t tbytes = ((size_t)S.NB * S.ldt * 8 + 1023) & ~(size_t)1023, cbytes = ((size_t)S.NB * S.wc * 8 + 1023) & ~(size_t)1023;
+        double* dX[2] = {(double*)(base + tbytes), (double*)(base + tbytes + cbytes)};
+        while (ctx->events.size() < 1) {
+            cudaEvent_t e;
+            HCL_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+            ctx->events.push_back(e);
+        }
+        const int ns = ctx->n_compute >= 2 ? 2 : 1;
+        if ((rc = copy2d(dT, (size_t)S.ldt * 8, A + r0 * lda + r0, (size_t)lda * 8, (size_t)nbi * 8, (size_t)nbi, ctx->s_h2d))) return rc;
+        HCL_CUDA(cudaEventRecord(ctx->events[0], ctx->s_h2d));
+        acc.bytes_h2d += (uint64_t)nbi * nbi * 8; ++acc.n_copies_h2d;
+        for (int s = 0; s < ns; ++s) HCL_CUDA(cudaStreamWaitEvent(ctx->s_compute[s], ctx->events[0], 0));
+        int64_t c = 0;
+        for (int64_t c0 = 0; c0 < N; c0 += S.wc, ++c) {
+            const int64_t w = std::min(S.wc, N - c0);
+            cudaStream_t st = ctx->s_compute[c % ns];
+            double* X = dX[c % 2];
+            double* hB = B + r0 * ldb + c0;
+            if ((rc = copy2d(X, (size_t)S.wc * 8, hB, (size_t)ldb * 8, (size_t)w * 8, (size_t)nbi, st))) return rc;
+            const int64_t npb = (nbi + 127) / 128;
+            for (int64_t pb = 0; pb < npb; ++pb) {
+                const int64_t p = lower ? pb : npb - 1 - pb;
+                const int64_t p0 = p * 128, ib = std::min<int64_t>(128, nbi - p0);
+                const double scale = pb == 0 ? alpha_eff : 1.0;
+                if ((rc = launch_trsm_block(dT + p0 * S.ldt + p0, S.ldt, (int)ib, X + p0 * S.wc, S.wc, w, lower ? 1 : 0, trans, diag, scale, st))) return rc;
+                ++acc.n_kernels;
+                const int64_t rest0 = lower ? p0 + ib : 0, nrest = lower ? nbi - rest0 : p0;
+                if (nrest > 0) {
+                    const double* Tp = trans ? dT + p0 * S.ldt + rest0 : dT + rest0 * S.ldt + p0;   // op(T)[rest, block p] as stored
+                    rc = launch_dgemm_tiles(nrest, w, ib, -1.0, Tp, S.ldt, X + p0 * S.wc, S.wc, scale, X + rest0 * S.wc, S.wc, st, 1,
+                                            nullptr, trans ? 1 : 0, 0);
+                    if (rc) return rc;
+                    ++acc.n_kernels;
+                }
+            }
+            if ((rc = copy2d(hB, (size_t)ldb * 8, X, (size_t)S.wc * 8, (size_t)w * 8, (size_t)nbi, st))) return rc;
+            acc.bytes_h2d += (uint64_t)nbi * w * 8; acc.bytes_d2h += (uint64_t)nbi * w * 8; ++acc.n_copies_h2d; ++acc.n_copies_d2h;
+        }
+        t_enq += std::chrono::duration<double>(std::chrono::steady_clock::now() - te0).count();
+        cudaError_t e = cudaSuccess;
+        for (int s = 0; s < ns; ++s) { cudaError_t e2 = cudaStreamSynchronize(ctx->s_compute[s]); if (e == cudaSuccess) e = e2; }
+        if (e != cudaSuccess) return cuda_fail(e);
+    }
+    if (stats) {
+        *stats = acc;
+        stats->plan.M = M; stats->plan.N = N; stats->plan.K = M;
+        stats->plan.mb = S.NB; stats->plan.nb = S.wc; stats->plan.kb = 128;
+        stats->plan.h = nblk; stats->plan.w = (N + S.wc - 1) / S.wc; stats->plan.kpanels = 1; stats->plan.n_steps = nblk;
+        stats->plan.workspace_bytes = ws_max;
+        stats->plan.bytes_h2d = acc.bytes_h2d; stats->plan.bytes_d2h = acc.bytes_d2h;
+        stats->plan.n_copies_h2d = acc.n_copies_h2d; stats->plan.n_copies_d2h = acc.n_copies_d2h;
+        stats->plan.flops = (double)M * (double)M * (double)N;
+        stats->t_enqueue_s = t_enq;
+        stats->t_total_s = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_begin).count();
+    }
+    return HCLOOC_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
 // nsteps mode: MMOOC as a subroutine of a blocked algorithm (SUMMA, HSUMMA) that updates the
 // same C `nsteps` times.  The paper uploads C only at step 0 and downloads it only at the last step; its listing
 // of that logic is garbled (:245, :259-263, G17), so the stated intent is implemented: C lives in device

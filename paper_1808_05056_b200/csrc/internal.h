@@ -91,6 +91,10 @@ int launch_dgemm_direct(int64_t M, int64_t N, int64_t K, double alpha, const dou
 int plan_impl(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zero, size_t device_budget_bytes,
               int operands_on_device, int transa, int transb, hclooc_plan_t* out);
 
+// Diagonal-block solve of hclooc_dtrsm (trsm_sm100.cu): dX (ib x ncols, ib <= 128) <- op(T)^-1 * (scale * dX) in place
+int launch_trsm_block(const double* dT, int64_t ldt, int ib, double* dX, int64_t ldx, int64_t ncols, int lower, int trans,
+                      int unit, double scale, cudaStream_t stream);
+
 // number of CTAs the tile kernel uses for an M x N output (for stats / tests)
 int64_t dgemm_tile_count(int64_t M, int64_t N);
 

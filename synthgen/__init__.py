@@ -103,3 +103,20 @@ def fill_numpy(rows: int, cols: int, seed: int, matrix: str, dist: str, row0: in
         u2 = (_splitmix64(h) >> np.uint64(11)).astype(np.float64) * 2.0 ** -53
         return np.sqrt(-2.0 * np.log(u1)) * np.cos(6.283185307179586476925286766559 * u2)
     raise ValueError(dist)
+
+
+def shape_triangular(A: np.ndarray, dist: str) -> None:
+    """Input recipe for the triangular solves: turn a filled square matrix into a WELL CONDITIONED
+    triangular operand in place -- off-diagonal entries divided by M (absolute row and column sums below 1), diagonal
+    moved to magnitude [1, 2) keeping its sign; for the integer distribution the off-diagonal entries stay as drawn and the
+    diagonal becomes +-1 (divisions exact).  Both triangles are shaped; callers poison the one they do not pass.
+    Input shaping only: none of the solver's arithmetic lives here."""
+    M = A.shape[0]
+    assert A.shape[1] >= M
+    d = A[np.arange(M), np.arange(M)].copy()
+    sign = np.where(d < 0, -1.0, 1.0)
+    if dist == "int":
+        A[np.arange(M), np.arange(M)] = sign
+    else:
+        A[:, :M] /= float(max(M, 1))
+        A[np.arange(M), np.arange(M)] = sign * (1.0 + np.minimum(np.abs(d), 0.999999))

@@ -1,0 +1,136 @@
+"""GPU parity for the out-of-core DTRSM (hclooc_dtrsm, side = Left) against the CPU oracle.
+
+Bar (G23): integer data with a +-1 diagonal -> the solution bit for bit; otherwise the elementwise residual bound of
+substitution in any summation order, |alpha*B - op(T) X| <= gamma_(M+2) * (|alpha B| + |op(T)||X|) (oracle.dtrsm_gate, evaluated
+by the oracle in long double), AND, the operands being well conditioned by construction (synthgen.shape_triangular), agreement
+with the oracle's own solution to 1e-12 of the largest entry.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import synthgen
+
+pytestmark = pytest.mark.gpu
+MiB = 1 << 20
+FWD_RTOL = 1e-12
+
+
+@pytest.fixture(scope="module")
+def H():
+    import paper_1808_05056_b200 as H
+    import torch
+    assert torch.cuda.is_available()
+    torch.cuda.init()
+    return H
+
+
+def trsm_inputs(H, uplo, unit, M, N, seed, dist, pad=0):
+    """A (triangle `uplo` shaped, the other triangle and a unit diagonal NaN), B, and for integers the solution X0 it hides."""
+    A = H.HostMatrix(M, M, M + pad); B = H.HostMatrix(M, N, N + pad)
+    A.array[...] = np.nan; B.array[...] = np.nan
+    synthgen.fill(A.array, seed, "A", dist, cols=M)
+    synthgen.shape_triangular(A.view, dist)
+    synthgen.fill(B.array, seed, "B", dist, cols=N)
+    return A, B
+
+
+def poison(A, uplo, unit):
+    M = A.view.shape[0]
+    other = np.triu(np.ones((M, M), bool), 1) if uplo == 0 else np.tril(np.ones((M, M), bool), -1)
+    A.view[other] = np.nan
+    if unit:
+        A.view[np.arange(M), np.arange(M)] = np.nan
+
+
+def dense_op(Aview, uplo, trans, unit):
+    T = np.tril(Aview) if uplo == 0 else np.triu(Aview)
+    if unit:
+        T = T - np.diag(np.diag(T)) + np.eye(T.shape[0])
+    return T.T if trans else T
+
+
+@pytest.mark.parametrize("uplo", [0, 1])
+@pytest.mark.parametrize("trans", [0, 1])
+@pytest.mark.parametrize("unit", [0, 1])
+@pytest.mark.parametrize("M,N,alpha,dist,pad,budget", [
+    (300, 200, 1.0, "uniform", 3, 1 * MiB),        # NB = 256: two block rows, ragged second, 128-row inner blocks
+    (1000, 517, 2.0, "int", 0, 2 * MiB),           # NB = 256..384: several block rows, ragged chunk, exact
+    (129, 64, -0.5, "uniform", 1, 64 * MiB),       # one block row: no out-of-core update, alpha applied in the diagonal phase
+    (77, 1, 1.0, "int", 0, 512 * 1024),            # a single right-hand side
+    (1500, 333, 1.5, "uniform", 2, 3 * MiB),
+])
+def test_dtrsm_matches_oracle(H, uplo, trans, unit, M, N, alpha, dist, pad, budget):
+    A, B = trsm_inputs(H, uplo, unit, M, N, 91, dist, pad)
+    if dist == "int":
+        # B := op(T) X0 in int64, so that the exact solution is the integer matrix X0 / alpha-scaled copies of it
+        X0 = B.view.copy().astype(np.int64)
+        T = dense_op(np.nan_to_num(A.view), uplo, trans, unit).astype(np.int64)
+        B.view[...] = (T @ X0).astype(np.float64)
+    poison(A, uplo, unit)
+    B0 = B.view.copy()
+    ref = B0.copy()
+    oracle.dtrsm(uplo, trans, unit, alpha, A.view, ref)
+    st = H.hclooc_dtrsm(None, uplo, trans, unit, M, N, alpha, A, A.ld, B, B.ld, budget)
+    got = B.view.copy()
+    assert st.plan.workspace_bytes <= budget and st.n_kernels >= 1
+    assert not np.isnan(got).any()
+    assert np.isnan(B.array[:, N:]).all()                              # padding untouched
+    if dist == "int":
+        assert np.array_equal(ref, alpha * X0)                         # the oracle, against the hidden solution
+        assert np.array_equal(got, alpha * X0), f"{np.count_nonzero(got != alpha * X0)} elements differ"
+    else:
+        Aclean = np.nan_to_num(A.view)
+        res, den = oracle.dtrsm_residual(uplo, trans, unit, alpha, Aclean, B0, got)
+        assert (res <= oracle.dtrsm_gate(M) * den).all(), float((res / den).max())
+        assert np.abs(got - ref).max() <= FWD_RTOL * np.abs(ref).max()
+
+
+def test_dtrsm_alpha_zero_degenerate_and_errors(H):
+    M, N = 200, 100
+    A, B = trsm_inputs(H, 0, 0, M, N, 92, "uniform")
+    B.view[5, 7] = np.nan
+    Anan = H.HostMatrix(M, M, M); Anan.array[...] = np.nan
+    H.hclooc_dtrsm(None, 0, 0, 0, M, N, 0.0, Anan, M, B, B.ld, 1 * MiB)      # alpha == 0: zeros, A not read, NaN not carried
+    assert np.array_equal(B.view, np.zeros((M, N)))
+    synthgen.fill(B.array, 93, "B", "uniform", cols=N)
+    keep = B.view.copy()
+    H.hclooc_dtrsm(None, 0, 0, 0, 0, N, 1.0, A, M, B, B.ld, 1 * MiB)         # M == 0 / N == 0: nothing
+    H.hclooc_dtrsm(None, 0, 0, 0, M, 0, 1.0, A, M, B, B.ld, 1 * MiB)
+    assert np.array_equal(B.view, keep)
+    bad = [((2, 0, 0, M, N, 1.0, A, M, B, N), -2), ((0, 2, 0, M, N, 1.0, A, M, B, N), -3), ((0, 0, 2, M, N, 1.0, A, M, B, N), -4),
+           ((0, 0, 0, -1, N, 1.0, A, M, B, N), -5), ((0, 0, 0, M, -1, 1.0, A, M, B, N), -6), ((0, 0, 0, M, N, 1.0, None, M, B, N), -8),
+           ((0, 0, 0, M, N, 1.0, A, M - 1, B, N), -9), ((0, 0, 0, M, N, 1.0, A, M, None, N), -10), ((0, 0, 0, M, N, 1.0, A, M, B, N - 1), -11)]
+    for args, code in bad:
+        with pytest.raises(H.HclError) as ei:
+            H.hclooc_dtrsm(None, *args, 1 * MiB)
+        assert ei.value.status == code, (args[:6], ei.value.status)
+    with pytest.raises(H.HclError) as ei:                                      # not even a 32-row block fits
+        H.hclooc_dtrsm(None, 0, 0, 0, M, N, 1.0, A, M, B, N, 16 * 1024)
+    assert ei.value.status == 1
+    pageable = np.zeros((M, N))
+    with pytest.raises(H.HclError) as ei:
+        H.hclooc_dtrsm(None, 0, 0, 0, M, N, 1.0, A, M, pageable, N, 1 * MiB)
+    assert ei.value.status == 2
+    assert np.array_equal(B.view, keep)                                        # validation errors leave B untouched
+
+
+@pytest.mark.parametrize("uplo,trans,unit", [(0, 0, 0), (1, 0, 1), (0, 1, 0), (1, 1, 0)])
+def test_dtrsm_large_block_rows_of_4096(H, uplo, trans, unit):
+    """NB = 4096 under 256 MiB: two block rows (one ragged), 32 inner blocks per chunk, two chunks on two streams; the whole
+    result against the oracle, the residual gate on sampled rows and columns."""
+    M, N, alpha = 6000, 4500, 1.25
+    A, B = trsm_inputs(H, uplo, unit, M, N, 94, "uniform")
+    poison(A, uplo, unit)
+    B0 = B.view.copy()
+    st = H.hclooc_dtrsm(None, uplo, trans, unit, M, N, alpha, A, A.ld, B, B.ld, 256 * MiB)
+    got = B.view.copy()
+    assert st.plan.mb == 4096 and st.plan.h == 2 and st.plan.workspace_bytes <= 256 * MiB
+    ref = B0.copy()
+    oracle.dtrsm(uplo, trans, unit, alpha, A.view, ref)
+    assert np.abs(got - ref).max() <= FWD_RTOL * np.abs(ref).max()
+    rng = np.random.default_rng(0)
+    rows = np.unique(np.concatenate([[0, 127, 128, 4095, 4096, M - 1], rng.integers(0, M, 40)]))
+    cols = np.unique(np.concatenate([[0, 63, 64, N - 1], rng.integers(0, N, 40)]))
+    res, den = oracle.dtrsm_residual(uplo, trans, unit, alpha, np.nan_to_num(A.view), B0, got, rows, cols)
+    assert (res <= oracle.dtrsm_gate(M) * den).all()
