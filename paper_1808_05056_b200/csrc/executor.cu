@@ -9,6 +9,7 @@
 // data have completed") can be checked on the list itself without a GPU.
 #include <algorithm>
 #include <chrono>
+#include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <mutex>
@@ -894,73 +895,174 @@ extern "C" int hclooc_dtrsm(hclooc_ctx* ctx, int uplo, int trans, int diag, int6
     std::memset(&acc, 0, sizeof(acc));
     double t_enq = 0.0;
     size_t ws_max = S.bytes;
+    const size_t tbytes = ((size_t)S.NB * S.ldt * 8 + 1023) & ~(size_t)1023, cbytes = ((size_t)S.NB * S.wc * 8 + 1023) & ~(size_t)1023;
+    // ---- RESIDENT mode: a whole block row (NB x N) stays in device memory from its upload to the download of its solution --
+    // the out-of-core DGEMM updates it there (C on the device: its block copies are device-to-device), the diagonal phase solves
+    // it in place, and finished column chunks go down on the D2H stream while the next ones are solved.  With room for two
+    // block rows the next one is uploaded during the diagonal phase.  Needs library-owned device memory and a quarter of the
+    // budget left for the DGEMM pipeline; otherwise the block row is STAGED through two column-chunk buffers after a DGEMM on
+    // host C (one more round trip of B over the link).
+    const int64_t ldx = (N + 1) & ~(int64_t)1;
+    const size_t rbytes = ((size_t)S.NB * ldx * 8 + 1023) & ~(size_t)1023;
+    int nres = 0;
+    {
+        static const int res_env = [] { const char* e = std::getenv("HCLOOC_TRSM_RESIDENT"); return e ? std::atoi(e) : -1; }();
+        std::lock_guard<std::mutex> lk(ctx->mu);
+        const bool own = ctx->owns_workspace || !ctx->workspace;
+        if (own && res_env != 0) {
+            if (nblk > 1 && 2 * rbytes + tbytes + budget / 4 <= budget) nres = 2;
+            else if (rbytes + tbytes + budget / 4 <= budget) nres = 1;
+        }
+    }
+    struct DevMem { void* p = nullptr; ~DevMem() { if (p) cudaFree(p); } } resmem;
+    double* dres[2] = {nullptr, nullptr};
+    double* dTres = nullptr;
+    size_t budget_dgemm = budget;
+    if (nres > 0) {
+        cudaError_t e = cudaMalloc(&resmem.p, nres * rbytes + tbytes);
+        if (e != cudaSuccess) { set_last_cuda_error((int)e); cudaGetLastError(); resmem.p = nullptr; nres = 0; }
+        else {
+            dTres = (double*)resmem.p;
+            for (int b = 0; b < nres; ++b) dres[b] = (double*)((uint8_t*)resmem.p + tbytes + b * rbytes);
+            budget_dgemm = budget - nres * rbytes - tbytes;
+            ws_max = nres * rbytes + tbytes;
+        }
+    }
+    const int ns = ctx->n_compute >= 2 ? 2 : 1;
+    {
+        std::lock_guard<std::mutex> lk(ctx->mu);
+        while (ctx->events.size() < 3) {
+            cudaEvent_t e;
+            HCL_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+            ctx->events.push_back(e);
+        }
+    }
+    // the diagonal phase of one column chunk X (nbi rows, w columns, leading dimension ld) in stream st, by recursive halving
+    // over 128-row blocks: solve the half that comes first in the order of substitution, subtract its contribution from the
+    // other half with ONE tile-kernel launch (K = the half's height: the flops sit in launches with large K, and every row
+    // of the chunk is read and written log2(nbi/128) times instead of nbi/256 times), solve the other half; a 128-row block
+    // goes to trsm_block_kernel.  `scale` (alpha, when no out-of-core update applied it) reaches every row exactly once: as
+    // beta of the first update that touches it, or in the triangle kernel.  One CTA per tile, so that the order of summation
+    // does not depend on the chunk width (resident and staged mode give the same bits).
+    struct Range { int64_t lo, hi; double scale; int stage; };
+    auto solve_chunk = [&](const double* dT, double* X, int64_t ld, int64_t w, int64_t nbi, double alpha_eff, cudaStream_t st) -> int {
+        std::vector<Range> stack;
+        stack.push_back({0, nbi, alpha_eff, 0});
+        while (!stack.empty()) {
+            Range r = stack.back();
+            stack.pop_back();
+            const int64_t rows = r.hi - r.lo;
+            if (rows <= 128) {
+                int e = launch_trsm_block(dT + r.lo * S.ldt + r.lo, S.ldt, (int)rows, X + r.lo * ld, ld, w, lower ? 1 : 0, trans, diag, r.scale, st);
+                if (e) return e;
+                ++acc.n_kernels;
+                continue;
+            }
+            const int64_t mid = r.lo + ((rows + 127) / 128 + 1) / 2 * 128;
+            // first = the half solved first, second = the half that then receives first's contribution
+            const int64_t f0 = lower ? r.lo : mid, f1 = lower ? mid : r.hi, s0 = lower ? mid : r.lo, s1 = lower ? r.hi : mid;
+            if (r.stage == 0) {
+                stack.push_back({r.lo, r.hi, r.scale, 1});            // come back for the update and the second half
+                stack.push_back({f0, f1, r.scale, 0});
+            } else {
+                const double* Tp = trans ? dT + f0 * S.ldt + s0 : dT + s0 * S.ldt + f0;     // op(T)[second, first] as stored
+                int e = launch_dgemm_tiles(s1 - s0, w, f1 - f0, -1.0, Tp, S.ldt, X + f0 * ld, ld, r.scale, X + s0 * ld, ld, st, 1, nullptr, trans ? 1 : 0, 0);
+                if (e) return e;
+                ++acc.n_kernels;
+                stack.push_back({s0, s1, 1.0, 0});
+            }
+        }
+        return HCLOOC_OK;
+    };
     for (int64_t bi = 0; bi < nblk; ++bi) {
         const int64_t i = lower ? bi : nblk - 1 - bi;
         const int64_t r0 = i * S.NB, nbi = std::min(S.NB, M - r0), r1 = r0 + nbi;
         // ---- rows already solved: [0, r0) when op(T) is lower, [r1, M) when it is upper
         const int64_t k0 = lower ? 0 : r1, kk = lower ? r0 : M - r1;
+        const double* Ap = trans ? A + k0 * lda + r0 : A + r0 * lda + k0;           // op(T)[rows of i, solved rows], as stored
         double alpha_eff = alpha;
+        double* dXr = nres ? dres[bi % nres] : nullptr;
+        if (nres) {
+            std::lock_guard<std::mutex> lk(ctx->mu);
+            HCL_CUDA(cudaSetDevice(ctx->device));
+            if (!(nres == 2 && bi > 0)) {                                           // not prefetched during the previous diagonal phase
+                if ((rc = copy2d(dXr, (size_t)ldx * 8, B + r0 * ldb, (size_t)ldb * 8, (size_t)N * 8, (size_t)nbi, ctx->s_h2d))) return rc;
+                acc.bytes_h2d += (uint64_t)nbi * N * 8; ++acc.n_copies_h2d;
+            }
+            HCL_CUDA(cudaStreamSynchronize(ctx->s_h2d));                            // the DGEMM's own streams do not wait for this one
+        }
+        const auto tp0 = std::chrono::steady_clock::now();
         if (kk > 0) {
-            const double* Ap = trans ? A + k0 * lda + r0 : A + r0 * lda + k0;       // op(T)[rows of i, solved rows], as stored
             hclooc_stats one;
-            rc = dgemm_core(ctx, trans ? 1 : 0, 0, nbi, N, kk, -1.0, Ap, lda, B + k0 * ldb, ldb, alpha, B + r0 * ldb, ldb, budget, &one);
+            if (nres) rc = dgemm_core(ctx, trans ? 1 : 0, 0, nbi, N, kk, -1.0, Ap, lda, B + k0 * ldb, ldb, alpha, dXr, ldx, budget_dgemm, &one);
+            else rc = dgemm_core(ctx, trans ? 1 : 0, 0, nbi, N, kk, -1.0, Ap, lda, B + k0 * ldb, ldb, alpha, B + r0 * ldb, ldb, budget, &one);
             if (rc) return rc;
             acc.bytes_h2d += one.bytes_h2d; acc.bytes_d2h += one.bytes_d2h; acc.n_kernels += one.n_kernels;
             acc.n_copies_h2d += one.n_copies_h2d; acc.n_copies_d2h += one.n_copies_d2h; t_enq += one.t_enqueue_s;
-            ws_max = std::max(ws_max, (size_t)one.plan.workspace_bytes);
+            ws_max = std::max(ws_max, (size_t)one.plan.workspace_bytes + (nres ? nres * rbytes + tbytes : 0));
             alpha_eff = 1.0;
         }
         // ---- the diagonal block, in device memory
         std::lock_guard<std::mutex> lk(ctx->mu);
         HCL_CUDA(cudaSetDevice(ctx->device));
         const auto te0 = std::chrono::steady_clock::now();
-        if ((rc = ensure_workspace(ctx, S.bytes + 1024))) return rc;
-        uint8_t* base = (uint8_t*)ctx->workspace;
-        const uintptr_t mis = (uintptr_t)base & 1023u;
-        if (mis) base += 1024 - mis;
-        double* dT = (double*)base;
-        const size_t tbytes = ((size_t)S.NB * S.ldt * 8 + 1023) & ~(size_t)1023, cbytes = ((size_t)S.NB * S.wc * 8 + 1023) & ~(size_t)1023;
-        double* dX[2] = {(double*)(base + tbytes), (double*)(base + tbytes + cbytes)};
-        while (ctx->events.size() < 1) {
-            cudaEvent_t e;
-            HCL_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
-            ctx->events.push_back(e);
+        double* dT = dTres;
+        double* dX[2] = {nullptr, nullptr};
+        if (!nres) {
+            if ((rc = ensure_workspace(ctx, S.bytes + 1024))) return rc;
+            uint8_t* base = (uint8_t*)ctx->workspace;
+            const uintptr_t mis = (uintptr_t)base & 1023u;
+            if (mis) base += 1024 - mis;
+            dT = (double*)base;
+            dX[0] = (double*)(base + tbytes); dX[1] = (double*)(base + tbytes + cbytes);
         }
-        const int ns = ctx->n_compute >= 2 ? 2 : 1;
         if ((rc = copy2d(dT, (size_t)S.ldt * 8, A + r0 * lda + r0, (size_t)lda * 8, (size_t)nbi * 8, (size_t)nbi, ctx->s_h2d))) return rc;
         HCL_CUDA(cudaEventRecord(ctx->events[0], ctx->s_h2d));
         acc.bytes_h2d += (uint64_t)nbi * nbi * 8; ++acc.n_copies_h2d;
         for (int s = 0; s < ns; ++s) HCL_CUDA(cudaStreamWaitEvent(ctx->s_compute[s], ctx->events[0], 0));
-        int64_t c = 0;
-        for (int64_t c0 = 0; c0 < N; c0 += S.wc, ++c) {
-            const int64_t w = std::min(S.wc, N - c0);
-            cudaStream_t st = ctx->s_compute[c % ns];
-            double* X = dX[c % 2];
-            double* hB = B + r0 * ldb + c0;
-            if ((rc = copy2d(X, (size_t)S.wc * 8, hB, (size_t)ldb * 8, (size_t)w * 8, (size_t)nbi, st))) return rc;
-            const int64_t npb = (nbi + 127) / 128;
-            for (int64_t pb = 0; pb < npb; ++pb) {
-                const int64_t p = lower ? pb : npb - 1 - pb;
-                const int64_t p0 = p * 128, ib = std::min<int64_t>(128, nbi - p0);
-                const double scale = pb == 0 ? alpha_eff : 1.0;
-                if ((rc = launch_trsm_block(dT + p0 * S.ldt + p0, S.ldt, (int)ib, X + p0 * S.wc, S.wc, w, lower ? 1 : 0, trans, diag, scale, st))) return rc;
-                ++acc.n_kernels;
-                const int64_t rest0 = lower ? p0 + ib : 0, nrest = lower ? nbi - rest0 : p0;
-                if (nrest > 0) {
-                    const double* Tp = trans ? dT + p0 * S.ldt + rest0 : dT + rest0 * S.ldt + p0;   // op(T)[rest, block p] as stored
-                    rc = launch_dgemm_tiles(nrest, w, ib, -1.0, Tp, S.ldt, X + p0 * S.wc, S.wc, scale, X + rest0 * S.wc, S.wc, st, 1,
-                                            nullptr, trans ? 1 : 0, 0);
-                    if (rc) return rc;
-                    ++acc.n_kernels;
-                }
+        if (nres == 2 && bi + 1 < nblk) {                                           // the next block row comes up meanwhile
+            const int64_t i2 = lower ? bi + 1 : nblk - 2 - bi, q0 = i2 * S.NB, nb2 = std::min(S.NB, M - q0);
+            if ((rc = copy2d(dres[(bi + 1) % 2], (size_t)ldx * 8, B + q0 * ldb, (size_t)ldb * 8, (size_t)N * 8, (size_t)nb2, ctx->s_h2d))) return rc;
+            acc.bytes_h2d += (uint64_t)nb2 * N * 8; ++acc.n_copies_h2d;
+        }
+        if (nres) {
+            int64_t wr = ((N + 7) / 8 + 63) / 64 * 64;                              // about 8 chunks, at least 1024 columns each
+            if (wr < 1024) wr = 1024;
+            int64_t c = 0;
+            for (int64_t c0 = 0; c0 < N; c0 += wr, ++c) {
+                const int64_t w = std::min(wr, N - c0);
+                cudaStream_t st = ctx->s_compute[c % ns];
+                if ((rc = solve_chunk(dT, dXr + c0, ldx, w, nbi, alpha_eff, st))) return rc;
+                HCL_CUDA(cudaEventRecord(ctx->events[1 + c % 2], st));
+                HCL_CUDA(cudaStreamWaitEvent(ctx->s_d2h, ctx->events[1 + c % 2], 0));
+                if ((rc = copy2d(B + r0 * ldb + c0, (size_t)ldb * 8, dXr + c0, (size_t)ldx * 8, (size_t)w * 8, (size_t)nbi, ctx->s_d2h))) return rc;
+                acc.bytes_d2h += (uint64_t)nbi * w * 8; ++acc.n_copies_d2h;
             }
-            if ((rc = copy2d(hB, (size_t)ldb * 8, X, (size_t)S.wc * 8, (size_t)w * 8, (size_t)nbi, st))) return rc;
-            acc.bytes_h2d += (uint64_t)nbi * w * 8; acc.bytes_d2h += (uint64_t)nbi * w * 8; ++acc.n_copies_h2d; ++acc.n_copies_d2h;
+        } else {
+            int64_t c = 0;
+            for (int64_t c0 = 0; c0 < N; c0 += S.wc, ++c) {
+                const int64_t w = std::min(S.wc, N - c0);
+                cudaStream_t st = ctx->s_compute[c % ns];
+                double* X = dX[c % 2];
+                double* hB = B + r0 * ldb + c0;
+                if ((rc = copy2d(X, (size_t)S.wc * 8, hB, (size_t)ldb * 8, (size_t)w * 8, (size_t)nbi, st))) return rc;
+                if ((rc = solve_chunk(dT, X, S.wc, w, nbi, alpha_eff, st))) return rc;
+                if ((rc = copy2d(hB, (size_t)ldb * 8, X, (size_t)S.wc * 8, (size_t)w * 8, (size_t)nbi, st))) return rc;
+                acc.bytes_h2d += (uint64_t)nbi * w * 8; acc.bytes_d2h += (uint64_t)nbi * w * 8; ++acc.n_copies_h2d; ++acc.n_copies_d2h;
+            }
         }
         t_enq += std::chrono::duration<double>(std::chrono::steady_clock::now() - te0).count();
         cudaError_t e = cudaSuccess;
         for (int s = 0; s < ns; ++s) { cudaError_t e2 = cudaStreamSynchronize(ctx->s_compute[s]); if (e == cudaSuccess) e = e2; }
+        { cudaError_t e2 = cudaStreamSynchronize(ctx->s_d2h); if (e == cudaSuccess) e = e2; }
+        if (bi + 1 == nblk) { cudaError_t e2 = cudaStreamSynchronize(ctx->s_h2d); if (e == cudaSuccess) e = e2; }
         if (e != cudaSuccess) return cuda_fail(e);
+        static const bool timing = std::getenv("HCLOOC_TRSM_TIMING") != nullptr;       // experiment knob: phase times per block row
+        if (timing) {
+            const auto tp2 = std::chrono::steady_clock::now();
+            std::fprintf(stderr, "dtrsm block row %lld: K = %lld, update %.2f ms, diagonal phase %.2f ms\n", (long long)i, (long long)kk,
+                         1e3 * std::chrono::duration<double>(te0 - tp0).count(), 1e3 * std::chrono::duration<double>(tp2 - te0).count());
+        }
     }
     if (stats) {
         *stats = acc;
@@ -968,6 +1070,8 @@ extern "C" int hclooc_dtrsm(hclooc_ctx* ctx, int uplo, int trans, int diag, int6
         stats->plan.mb = S.NB; stats->plan.nb = S.wc; stats->plan.kb = 128;
         stats->plan.h = nblk; stats->plan.w = (N + S.wc - 1) / S.wc; stats->plan.kpanels = 1; stats->plan.n_steps = nblk;
         stats->plan.workspace_bytes = ws_max;
+        stats->plan.n_sets = nres;                                  // block rows resident in device memory (0 = staged)
+        stats->plan.ldc_dev = nres ? ldx : S.wc;
         stats->plan.bytes_h2d = acc.bytes_h2d; stats->plan.bytes_d2h = acc.bytes_d2h;
         stats->plan.n_copies_h2d = acc.n_copies_h2d; stats->plan.n_copies_d2h = acc.n_copies_d2h;
         stats->plan.flops = (double)M * (double)M * (double)N;

@@ -74,6 +74,7 @@ def test_dtrsm_matches_oracle(H, uplo, trans, unit, M, N, alpha, dist, pad, budg
     st = H.hclooc_dtrsm(None, uplo, trans, unit, M, N, alpha, A, A.ld, B, B.ld, budget)
     got = B.view.copy()
     assert st.plan.workspace_bytes <= budget and st.n_kernels >= 1
+    assert st.plan.n_sets == (1 if (M, budget) in ((129, 64 * MiB), (77, 512 * 1024), (1500, 3 * MiB)) else 0)   # resident block row?
     assert not np.isnan(got).any()
     assert np.isnan(B.array[:, N:]).all()                              # padding untouched
     if dist == "int":
@@ -115,17 +116,20 @@ def test_dtrsm_alpha_zero_degenerate_and_errors(H):
     assert np.array_equal(B.view, keep)                                        # validation errors leave B untouched
 
 
+@pytest.mark.parametrize("budget,resident", [(256 * MiB, 0), (1024 * MiB, 2)])
 @pytest.mark.parametrize("uplo,trans,unit", [(0, 0, 0), (1, 0, 1), (0, 1, 0), (1, 1, 0)])
-def test_dtrsm_large_block_rows_of_4096(H, uplo, trans, unit):
-    """NB = 4096 under 256 MiB: two block rows (one ragged), 32 inner blocks per chunk, two chunks on two streams; the whole
-    result against the oracle, the residual gate on sampled rows and columns."""
+def test_dtrsm_large_block_rows_of_4096(H, uplo, trans, unit, budget, resident):
+    """NB = 4096: two block rows (one ragged), 32 inner blocks per chunk.  Under 256 MiB the block rows are staged through two
+    column chunks on two streams; under 1 GiB both block rows are resident (the DGEMM updates the second one in device memory
+    while it was uploaded during the first one's diagonal phase).  The whole result against the oracle, the residual gate on
+    sampled rows and columns."""
     M, N, alpha = 6000, 4500, 1.25
     A, B = trsm_inputs(H, uplo, unit, M, N, 94, "uniform")
     poison(A, uplo, unit)
     B0 = B.view.copy()
-    st = H.hclooc_dtrsm(None, uplo, trans, unit, M, N, alpha, A, A.ld, B, B.ld, 256 * MiB)
+    st = H.hclooc_dtrsm(None, uplo, trans, unit, M, N, alpha, A, A.ld, B, B.ld, budget)
     got = B.view.copy()
-    assert st.plan.mb == 4096 and st.plan.h == 2 and st.plan.workspace_bytes <= 256 * MiB
+    assert st.plan.mb == 4096 and st.plan.h == 2 and st.plan.workspace_bytes <= budget and st.plan.n_sets == resident
     ref = B0.copy()
     oracle.dtrsm(uplo, trans, unit, alpha, A.view, ref)
     assert np.abs(got - ref).max() <= FWD_RTOL * np.abs(ref).max()
@@ -134,3 +138,27 @@ def test_dtrsm_large_block_rows_of_4096(H, uplo, trans, unit):
     cols = np.unique(np.concatenate([[0, 63, 64, N - 1], rng.integers(0, N, 40)]))
     res, den = oracle.dtrsm_residual(uplo, trans, unit, alpha, np.nan_to_num(A.view), B0, got, rows, cols)
     assert (res <= oracle.dtrsm_gate(M) * den).all()
+
+
+def test_dtrsm_resident_and_staged_modes_agree_bitwise(H, monkeypatch):
+    """The same solve with the block rows resident in device memory and staged through column chunks: the arithmetic is the
+    same blocked substitution (same NB, same 128-row inner blocks), so the bits agree; and a caller-owned workspace (no
+    library allocation allowed) takes the staged path."""
+    import torch
+    M, N = 3000, 300
+    A, B = trsm_inputs(H, 1, 0, M, N, 95, "uniform", pad=1)
+    poison(A, 1, 0)
+    B0 = B.view.copy()
+    st = H.hclooc_dtrsm(None, 1, 0, 0, M, N, 1.0, A, A.ld, B, B.ld, 48 * MiB)
+    assert st.plan.n_sets == 2 and st.plan.h == 2
+    res = B.view.copy()
+    ws = torch.empty(48 * MiB, dtype=torch.uint8, device="cuda")
+    torch.cuda.synchronize()
+    ctx = H.hclooc_ctx_create(0, ws.data_ptr(), ws.numel())
+    try:
+        B.view[...] = B0
+        st = H.hclooc_dtrsm(ctx, 1, 0, 0, M, N, 1.0, A, A.ld, B, B.ld, 0)
+        assert st.plan.n_sets == 0 and st.plan.workspace_bytes <= 48 * MiB and st.plan.h == 2
+    finally:
+        H.hclooc_ctx_destroy(ctx)
+    assert np.array_equal(B.view, res)
