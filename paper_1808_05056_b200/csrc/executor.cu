@@ -928,7 +928,11 @@ extern "C" int hclooc_dtrsm(hclooc_ctx* ctx, int uplo, int trans, int diag, int6
             ws_max = nres * rbytes + tbytes;
         }
     }
-    const int ns = ctx->n_compute >= 2 ? 2 : 1;
+    const int ns = ctx->n_compute >= 2 ? 2 : 1;                  // staged mode: one stream per chunk buffer
+    // resident mode: the chunks of a block row are independent pieces of one buffer, so more of them can be in flight (the
+    // triangle kernel is latency bound and leaves most SMs to the other chunks' tile launches)
+    static const int ns_env = [] { const char* e = std::getenv("HCLOOC_TRSM_STREAMS"); const int v = e ? std::atoi(e) : 0; return v > 0 ? v : 2; }();
+    const int ns_res = nres ? std::max(1, std::min(ns_env, ctx->n_compute)) : ns;
     {
         std::lock_guard<std::mutex> lk(ctx->mu);
         while (ctx->events.size() < 3) {
@@ -1019,19 +1023,20 @@ extern "C" int hclooc_dtrsm(hclooc_ctx* ctx, int uplo, int trans, int diag, int6
         if ((rc = copy2d(dT, (size_t)S.ldt * 8, A + r0 * lda + r0, (size_t)lda * 8, (size_t)nbi * 8, (size_t)nbi, ctx->s_h2d))) return rc;
         HCL_CUDA(cudaEventRecord(ctx->events[0], ctx->s_h2d));
         acc.bytes_h2d += (uint64_t)nbi * nbi * 8; ++acc.n_copies_h2d;
-        for (int s = 0; s < ns; ++s) HCL_CUDA(cudaStreamWaitEvent(ctx->s_compute[s], ctx->events[0], 0));
+        for (int s = 0; s < ns_res; ++s) HCL_CUDA(cudaStreamWaitEvent(ctx->s_compute[s], ctx->events[0], 0));
         if (nres == 2 && bi + 1 < nblk) {                                           // the next block row comes up meanwhile
             const int64_t i2 = lower ? bi + 1 : nblk - 2 - bi, q0 = i2 * S.NB, nb2 = std::min(S.NB, M - q0);
             if ((rc = copy2d(dres[(bi + 1) % 2], (size_t)ldx * 8, B + q0 * ldb, (size_t)ldb * 8, (size_t)N * 8, (size_t)nb2, ctx->s_h2d))) return rc;
             acc.bytes_h2d += (uint64_t)nb2 * N * 8; ++acc.n_copies_h2d;
         }
         if (nres) {
-            int64_t wr = ((N + 7) / 8 + 63) / 64 * 64;                              // about 8 chunks, at least 1024 columns each
+            static const int nchunk = [] { const char* e = std::getenv("HCLOOC_TRSM_CHUNKS"); const int v = e ? std::atoi(e) : 0; return v > 0 ? v : 8; }();
+            int64_t wr = ((N + nchunk - 1) / nchunk + 63) / 64 * 64;                // about 8 chunks, at least 1024 columns each
             if (wr < 1024) wr = 1024;
             int64_t c = 0;
             for (int64_t c0 = 0; c0 < N; c0 += wr, ++c) {
                 const int64_t w = std::min(wr, N - c0);
-                cudaStream_t st = ctx->s_compute[c % ns];
+                cudaStream_t st = ctx->s_compute[c % ns_res];
                 if ((rc = solve_chunk(dT, dXr + c0, ldx, w, nbi, alpha_eff, st))) return rc;
                 HCL_CUDA(cudaEventRecord(ctx->events[1 + c % 2], st));
                 HCL_CUDA(cudaStreamWaitEvent(ctx->s_d2h, ctx->events[1 + c % 2], 0));
@@ -1053,7 +1058,7 @@ extern "C" int hclooc_dtrsm(hclooc_ctx* ctx, int uplo, int trans, int diag, int6
         }
         t_enq += std::chrono::duration<double>(std::chrono::steady_clock::now() - te0).count();
         cudaError_t e = cudaSuccess;
-        for (int s = 0; s < ns; ++s) { cudaError_t e2 = cudaStreamSynchronize(ctx->s_compute[s]); if (e == cudaSuccess) e = e2; }
+        for (int s = 0; s < ns_res; ++s) { cudaError_t e2 = cudaStreamSynchronize(ctx->s_compute[s]); if (e == cudaSuccess) e = e2; }
         { cudaError_t e2 = cudaStreamSynchronize(ctx->s_d2h); if (e == cudaSuccess) e = e2; }
         if (bi + 1 == nblk) { cudaError_t e2 = cudaStreamSynchronize(ctx->s_h2d); if (e == cudaSuccess) e = e2; }
         if (e != cudaSuccess) return cuda_fail(e);
