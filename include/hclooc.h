@@ -284,6 +284,15 @@ int hclooc_dsyr2k(hclooc_ctx* ctx, int uplo, int trans, int64_t N, int64_t K, do
 int hclooc_dtrsm(hclooc_ctx* ctx, int uplo, int trans, int diag, int64_t M, int64_t N, double alpha, const double* A, int64_t lda,
                  double* B, int64_t ldb, size_t device_budget_bytes, hclooc_stats* stats_out);
 
+/* The shape hclooc_dtrsm works in (pure host arithmetic, needs no GPU): *NB = rows of a block row (<= 4096, NB*NB*8 <= half the
+ * budget, a multiple of 128 -- of 32 below 128 -- or M itself), *chunk = columns of a staged column chunk (multiple of 64),
+ * *resident = block rows kept in device memory (2, 1, or 0 = staged mode; always 0 unless library_owned: a context working in
+ * caller-owned device memory allocates nothing), *device_bytes = what the diagonal phase holds (resident block rows + triangle
+ * buffer, or triangle buffer + two chunk buffers); in resident mode a quarter of the budget at least is left to the DGEMM calls.
+ * Errors: -1 M < 1, -2 N < 1, -5 NULL output, HCLOOC_ERR_BUDGET when not even a 32-row block with 64-column chunks fits.   */
+int hclooc_dtrsm_plan(int64_t M, int64_t N, size_t device_budget_bytes, int library_owned, int64_t* NB, int64_t* chunk,
+                      int* resident, uint64_t* device_bytes);
+
 /* nsteps mode (:277-283): MMOOC as a subroutine of a blocked algorithm (SUMMA, HSUMMA) that updates the same C
  * `nsteps` times: C = alpha*A_p*B_p + beta_p*C for p = *step = 0 .. nsteps-1, one call per p.  C is uploaded once
  * at step 0 (if beta != 0), stays in device memory between the calls, and is downloaded once at the last step, so

@@ -17,7 +17,7 @@ HCL_DIAG_NONUNIT, HCL_DIAG_UNIT = 0, 1
 EXPORTS = [
     "hclooc_plan", "hclooc_plan_ex", "hclooc_plan_trans", "hclooc_shard_rows", "hclMatrixPartitioner", "hclooc_schedule", "hclooc_ctx_create", "hclooc_ctx_destroy",
     "hclooc_ctx_set_trace", "hclooc_ctx_get_trace", "hclooc_ctx_set_direct",
-    "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_t", "hclooc_dsyrk", "hclooc_dsyr2k", "hclooc_dtrsm", "hclooc_dgemm_fig2", "hclooc_dgemm_nsteps", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
+    "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_t", "hclooc_dsyrk", "hclooc_dsyr2k", "hclooc_dtrsm", "hclooc_dtrsm_plan", "hclooc_dgemm_fig2", "hclooc_dgemm_nsteps", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
     "hclStreamDestroy", "hclEventDestroy", "hclMemcpy", "hclMemcpyAsync", "hclMemcpy2DAsync",
     "hclDgemmAsync", "hclDgemmAsyncEx", "hclDgemmAsyncT", "hclWaitEvent", "hclStreamSynchronize", "hclDeviceSynchronize",
     "hclooc_host_alloc", "hclooc_host_free", "hclooc_host_register", "hclooc_host_unregister",
@@ -90,6 +90,7 @@ def lib():
         L.hclooc_dgemm_ex.argtypes = [vp, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
         L.hclooc_dgemm_t.argtypes = [vp, c_int, c_int, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
         L.hclooc_dsyrk.argtypes = [vp, c_int, c_int, i64, i64, dbl, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
+        L.hclooc_dtrsm_plan.argtypes = [i64, i64, sz, c_int, POINTER(i64), POINTER(i64), POINTER(c_int), POINTER(ctypes.c_uint64)]
         L.hclooc_dtrsm.argtypes = [vp, c_int, c_int, c_int, i64, i64, dbl, vp, i64, vp, i64, sz, POINTER(Stats)]
         L.hclooc_dsyr2k.argtypes = [vp, c_int, c_int, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
         L.hclooc_dgemm_nsteps.argtypes = [vp, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, c_int, POINTER(c_int), POINTER(Stats)]
@@ -320,6 +321,14 @@ def hclooc_dsyr2k(ctx, uplo, trans, N, K, alpha, A, lda, B, ldb, beta, C, ldc, d
     _check(lib().hclooc_dsyr2k(ctx, int(uplo), int(trans), N, K, alpha, _ptr(A), lda, _ptr(B), ldb, beta, _ptr(C), ldc,
                                device_budget_bytes, byref(st) if want_stats else None), "hclooc_dsyr2k")
     return st if want_stats else None
+
+
+def hclooc_dtrsm_plan(M, N, device_budget_bytes, library_owned=True):
+    """(NB, chunk, resident, device_bytes) of hclooc_dtrsm under a budget; host arithmetic only."""
+    nb, ch, res, by = c_int64(), c_int64(), c_int(), c_uint64()
+    _check(lib().hclooc_dtrsm_plan(M, N, device_budget_bytes, int(bool(library_owned)), byref(nb), byref(ch), byref(res), byref(by)),
+           "hclooc_dtrsm_plan")
+    return nb.value, ch.value, res.value, by.value
 
 
 def hclooc_dtrsm(ctx, uplo, trans, diag, M, N, alpha, A, lda, B, ldb, device_budget_bytes, want_stats=True):

@@ -833,9 +833,15 @@ int trsm_shape(int64_t M, int64_t N, size_t budget, TrsmShape* out) {
     while (NB > 128 && (size_t)NB * NB * 8 > budget / 2) NB -= 128;
     while (NB > 32 && (size_t)NB * NB * 8 > budget / 2) NB -= 32;
     if (NB > M) NB = M;
-    const int64_t ldt = (NB + 1) & ~(int64_t)1;
-    const size_t tbytes = ((size_t)NB * ldt * 8 + 1023) & ~(size_t)1023;
-    if (tbytes + 2 * (size_t)NB * 64 * 8 + 4096 > budget) return HCLOOC_ERR_BUDGET;
+    int64_t ldt = (NB + 1) & ~(int64_t)1;
+    size_t tbytes = ((size_t)NB * ldt * 8 + 1023) & ~(size_t)1023;
+    while (tbytes + 2 * (size_t)NB * 64 * 8 + 4096 > budget) {       // the two narrowest chunk buffers must fit beside the triangle
+        if (NB <= 32) return HCLOOC_ERR_BUDGET;
+        NB = NB > 128 ? (NB - 1) / 128 * 128 : (NB - 1) / 32 * 32;
+        if (NB < 32) return HCLOOC_ERR_BUDGET;
+        ldt = (NB + 1) & ~(int64_t)1;
+        tbytes = ((size_t)NB * ldt * 8 + 1023) & ~(size_t)1023;
+    }
     int64_t wc = (int64_t)((budget - tbytes - 4096) / (2 * (size_t)NB * 8)) / 64 * 64;
     const int64_t npad = (N + 63) / 64 * 64;
     if (wc > npad) wc = npad;
@@ -846,7 +852,39 @@ int trsm_shape(int64_t M, int64_t N, size_t budget, TrsmShape* out) {
     return HCLOOC_OK;
 }
 
+// Block rows kept resident in device memory (0 = staged mode) and the bytes of one of them: 2 when two fit beside the
+// triangle buffer with a quarter of the budget left for the DGEMM pipeline (and there is more than one block row), else 1
+// under the same condition, else 0.  Needs device memory the library may allocate itself.
+int trsm_resident(int64_t M, int64_t N, size_t budget, const TrsmShape& S, bool library_owned, size_t* rbytes_out) {
+    const int64_t ldx = (N + 1) & ~(int64_t)1;
+    const size_t rbytes = ((size_t)S.NB * ldx * 8 + 1023) & ~(size_t)1023;
+    const size_t tbytes = ((size_t)S.NB * S.ldt * 8 + 1023) & ~(size_t)1023;
+    const int64_t nblk = (M + S.NB - 1) / S.NB;
+    if (rbytes_out) *rbytes_out = rbytes;
+    if (!library_owned) return 0;
+    if (nblk > 1 && 2 * rbytes + tbytes + budget / 4 <= budget) return 2;
+    if (rbytes + tbytes + budget / 4 <= budget) return 1;
+    return 0;
+}
+
 }  // namespace
+
+// The shape hclooc_dtrsm works in under a budget -- pure host arithmetic, needs no GPU (include/hclooc.h).
+extern "C" int hclooc_dtrsm_plan(int64_t M, int64_t N, size_t device_budget_bytes, int library_owned, int64_t* NB, int64_t* chunk,
+                                 int* resident, uint64_t* device_bytes) {
+    if (M < 1) return -1;
+    if (N < 1) return -2;
+    if (!NB || !chunk || !resident || !device_bytes) return -5;
+    TrsmShape S;
+    int rc = trsm_shape(M, N, device_budget_bytes, &S);
+    if (rc) return rc;
+    size_t rbytes = 0;
+    const int nres = trsm_resident(M, N, device_budget_bytes, S, library_owned != 0, &rbytes);
+    const size_t tbytes = ((size_t)S.NB * S.ldt * 8 + 1023) & ~(size_t)1023;
+    *NB = S.NB; *chunk = S.wc; *resident = nres;
+    *device_bytes = nres ? (uint64_t)(nres * rbytes + tbytes) : (uint64_t)(S.bytes + 1024);
+    return HCLOOC_OK;
+}
 
 extern "C" int hclooc_dtrsm(hclooc_ctx* ctx, int uplo, int trans, int diag, int64_t M, int64_t N, double alpha,
                             const double* A, int64_t lda, double* B, int64_t ldb, size_t device_budget_bytes, hclooc_stats* stats) {
@@ -909,10 +947,7 @@ extern "C" int hclooc_dtrsm(hclooc_ctx* ctx, int uplo, int trans, int diag, int6
         static const int res_env = [] { const char* e = std::getenv("HCLOOC_TRSM_RESIDENT"); return e ? std::atoi(e) : -1; }();
         std::lock_guard<std::mutex> lk(ctx->mu);
         const bool own = ctx->owns_workspace || !ctx->workspace;
-        if (own && res_env != 0) {
-            if (nblk > 1 && 2 * rbytes + tbytes + budget / 4 <= budget) nres = 2;
-            else if (rbytes + tbytes + budget / 4 <= budget) nres = 1;
-        }
+        nres = trsm_resident(M, N, budget, S, own && res_env != 0, nullptr);
     }
     struct DevMem { void* p = nullptr; ~DevMem() { if (p) cudaFree(p); } } resmem;
     double* dres[2] = {nullptr, nullptr};

@@ -59,6 +59,7 @@ def dense_op(Aview, uplo, trans, unit):
     (129, 64, -0.5, "uniform", 1, 64 * MiB),       # one block row: no out-of-core update, alpha applied in the diagonal phase
     (77, 1, 1.0, "int", 0, 512 * 1024),            # a single right-hand side
     (1500, 333, 1.5, "uniform", 2, 3 * MiB),
+    (500, 130, 1.0, "int", 1, 192 * 1024),         # NB = 96: six block rows of less than one 128-row inner block, tiny DGEMM budgets
 ])
 def test_dtrsm_matches_oracle(H, uplo, trans, unit, M, N, alpha, dist, pad, budget):
     A, B = trsm_inputs(H, uplo, unit, M, N, 91, dist, pad)
@@ -74,6 +75,7 @@ def test_dtrsm_matches_oracle(H, uplo, trans, unit, M, N, alpha, dist, pad, budg
     st = H.hclooc_dtrsm(None, uplo, trans, unit, M, N, alpha, A, A.ld, B, B.ld, budget)
     got = B.view.copy()
     assert st.plan.workspace_bytes <= budget and st.n_kernels >= 1
+    assert (st.plan.mb, st.plan.n_sets) == H.hclooc_dtrsm_plan(M, N, budget)[::2]
     assert st.plan.n_sets == (1 if (M, budget) in ((129, 64 * MiB), (77, 512 * 1024), (1500, 3 * MiB)) else 0)   # resident block row?
     assert not np.isnan(got).any()
     assert np.isnan(B.array[:, N:]).all()                              # padding untouched

@@ -450,3 +450,38 @@ def test_triangle_schedule_has_steps_only_for_blocks_that_touch_the_triangle(tri
         # every B slice is still loaded whole, once per K panel
         b = ops[ops["kind"] == 1]
         assert int((b["nr"] * b["nc"]).sum()) == K * N
+
+
+def test_dtrsm_plan_respects_the_budget_and_its_own_rules():
+    """hclooc_dtrsm_plan (host arithmetic of hclooc_dtrsm): block-row height, chunk width, resident block rows and the device
+    bytes of the diagonal phase over a grid of shapes and budgets."""
+    import paper_1808_05056_b200 as H
+    MiB = 1 << 20
+    seen = set()
+    for M in (1, 31, 77, 128, 300, 1000, 4096, 6000, 32768, 163840):
+        for N in (1, 64, 333, 4500, 32768):
+            for budget in (64 * 1024, 512 * 1024, 1 * MiB, 3 * MiB, 48 * MiB, 256 * MiB, 1024 * MiB, 4096 * MiB, 170 * 1024 * MiB):
+                for own in (True, False):
+                    NB, chunk, res, dev = H.hclooc_dtrsm_plan(M, N, budget, own)
+                    assert 1 <= NB <= min(M, 4096) and NB * NB * 8 <= max(budget // 2, 32 * 32 * 8)
+                    assert NB == M or NB % 128 == 0 or (NB < 128 and NB % 32 == 0)
+                    assert chunk % 64 == 0 and 64 <= chunk <= (N + 63) // 64 * 64
+                    assert res in (0, 1, 2) and (own or res == 0)
+                    nblk = -(-M // NB)
+                    assert res < 2 or nblk > 1
+                    if res:
+                        assert dev + budget // 4 <= budget                       # the DGEMM pipeline keeps a quarter
+                        assert dev >= res * NB * N * 8 + NB * NB * 8
+                    else:
+                        assert dev <= budget and dev >= NB * NB * 8 + 2 * NB * chunk * 8
+                    seen.add(res)
+    assert seen == {0, 1, 2}
+    # the cases the GPU tests and the profile rely on
+    assert H.hclooc_dtrsm_plan(32768, 32768, 4096 * MiB)[:3] == (4096, 16384, 2)
+    assert H.hclooc_dtrsm_plan(16384, 16384, 256 * MiB)[::2] == (4096, 0)
+    assert H.hclooc_dtrsm_plan(6000, 4500, 1024 * MiB)[::2] == (4096, 2)
+    assert H.hclooc_dtrsm_plan(3000, 300, 48 * MiB, False)[2] == 0
+    for args, code in (((0, 5, MiB), -1), ((5, 0, MiB), -2), ((200, 100, 16 * 1024), 1)):
+        with pytest.raises(H.HclError) as e:
+            H.hclooc_dtrsm_plan(*args)
+        assert e.value.status == code
