@@ -267,7 +267,7 @@ int hclooc_dsyr2k(hclooc_ctx* ctx, int uplo, int trans, int64_t N, int64_t K, do
  * where T is the `uplo` triangle of the M x M matrix A (row-major, lda >= M; the other triangle is never read, nor is the
  * diagonal when diag = HCL_DIAG_UNIT) and B is M x N (ldb >= N); X overwrites B in place.  A and B are pinned host memory
  * (device memory is accepted too and staged the same way).  Blocked substitution: B is cut into block rows of NB <= 4096
- * rows (NB*NB*8 <= half the budget); a block row first receives  B_i <- alpha*B_i - op(T)[i, solved]*X[solved]  as ONE
+ * rows (8192 where two such block rows fit in device memory; NB*NB*8 <= half the budget); a block row first receives  B_i <- alpha*B_i - op(T)[i, solved]*X[solved]  as ONE
  * out-of-core DGEMM through the hclooc_dgemm_t pipeline, then its diagonal block is solved in device memory: T_ii is
  * uploaded once, B_i streams through two column-chunk buffers on two streams, and inside a chunk 128-row triangles are
  * solved by a substitution kernel (one thread per column of B) with the tile kernel updating the rows still to be solved.
@@ -284,7 +284,7 @@ int hclooc_dsyr2k(hclooc_ctx* ctx, int uplo, int trans, int64_t N, int64_t K, do
 int hclooc_dtrsm(hclooc_ctx* ctx, int uplo, int trans, int diag, int64_t M, int64_t N, double alpha, const double* A, int64_t lda,
                  double* B, int64_t ldb, size_t device_budget_bytes, hclooc_stats* stats_out);
 
-/* The shape hclooc_dtrsm works in (pure host arithmetic, needs no GPU): *NB = rows of a block row (<= 4096, NB*NB*8 <= half the
+/* The shape hclooc_dtrsm works in (pure host arithmetic, needs no GPU): *NB = rows of a block row (<= 4096, or <= 8192 in resident mode; NB*NB*8 <= half the
  * budget, a multiple of 128 -- of 32 below 128 -- or M itself), *chunk = columns of a staged column chunk (multiple of 64),
  * *resident = block rows kept in device memory (2, 1, or 0 = staged mode; always 0 unless library_owned: a context working in
  * caller-owned device memory allocates nothing), *device_bytes = what the diagonal phase holds (resident block rows + triangle

@@ -826,10 +826,19 @@ int ensure_workspace(hclooc_ctx* ctx, size_t bytes) {
 struct TrsmShape { int64_t NB, ldt, wc; size_t bytes; };
 
 // Block-row height NB, chunk width wc and the device bytes of the diagonal phase under `budget`: the triangle buffer takes
-// at most half of it (NB <= 4096: beyond that the DGEMM updates gain nothing and the diagonal phase, which no DGEMM
-// overlaps, grows), the two chunk buffers share the rest.
-int trsm_shape(int64_t M, int64_t N, size_t budget, TrsmShape* out) {
+// at most half of it, the two chunk buffers of staged mode share the rest.
+int trsm_shape(int64_t M, int64_t N, size_t budget, bool library_owned, TrsmShape* out) {
+    static const int64_t nb_env = [] { const char* e = std::getenv("HCLOOC_TRSM_NB_MAX"); const long v = e ? std::atol(e) : 0; return v >= 128 ? (int64_t)(v / 128 * 128) : (int64_t)0; }();
+    // Block rows of 4096 rows; of 8192 where two of them (one, if that is the whole problem) can stay resident in device memory
+    // beside their 512 MiB triangle with a quarter of the budget left: half the X[solved] traffic and updates twice as tall
+    // outweigh the longer diagonal phases (32768^2 under 16 GiB: 1.32 s at 4096, 1.20 s at 8192, 1.29 s at 12288, 1.25 s at 16384).
     int64_t NB = 4096;
+    if (library_owned && M > 4096) {
+        const int64_t nb8 = M < 8192 ? (M + 127) / 128 * 128 : 8192, ldx = (N + 1) & ~(int64_t)1;
+        const size_t tb = (size_t)nb8 * nb8 * 8 + 1024, rb = (size_t)nb8 * ldx * 8 + 1024;
+        if (tb <= budget / 2 && (M > nb8 ? 2 : 1) * rb + tb + budget / 4 <= budget) NB = 8192;
+    }
+    if (nb_env) NB = nb_env;                                        // experiment knob
     while (NB > 128 && (size_t)NB * NB * 8 > budget / 2) NB -= 128;
     while (NB > 32 && (size_t)NB * NB * 8 > budget / 2) NB -= 32;
     if (NB > M) NB = M;
@@ -876,7 +885,7 @@ extern "C" int hclooc_dtrsm_plan(int64_t M, int64_t N, size_t device_budget_byte
     if (N < 1) return -2;
     if (!NB || !chunk || !resident || !device_bytes) return -5;
     TrsmShape S;
-    int rc = trsm_shape(M, N, device_budget_bytes, &S);
+    int rc = trsm_shape(M, N, device_budget_bytes, library_owned != 0, &S);
     if (rc) return rc;
     size_t rbytes = 0;
     const int nres = trsm_resident(M, N, device_budget_bytes, S, library_owned != 0, &rbytes);
@@ -910,11 +919,13 @@ extern "C" int hclooc_dtrsm(hclooc_ctx* ctx, int uplo, int trans, int diag, int6
     }
     if (!ctx && (rc = default_ctx(&ctx))) return rc;
     size_t budget = device_budget_bytes;
+    bool own = false;                                            // may the library allocate device memory of its own?
     {
         std::lock_guard<std::mutex> lk(ctx->mu);
         HCL_CUDA(cudaSetDevice(ctx->device));
         bool dummy = true;
         if ((rc = check_resident(A, &dummy)) || (rc = check_resident(B, &dummy))) return rc;
+        own = ctx->owns_workspace || !ctx->workspace;
         if (!ctx->owns_workspace && ctx->workspace) {
             budget = (budget == 0) ? ctx->workspace_bytes : std::min(budget, ctx->workspace_bytes);
         } else if (budget == 0) {
@@ -926,7 +937,9 @@ extern "C" int hclooc_dtrsm(hclooc_ctx* ctx, int uplo, int trans, int diag, int6
         }
     }
     TrsmShape S;
-    if ((rc = trsm_shape(M, N, budget, &S))) return rc;
+    static const int res_env = [] { const char* e = std::getenv("HCLOOC_TRSM_RESIDENT"); return e ? std::atoi(e) : -1; }();
+    if (res_env == 0) own = false;                               // experiment knob: staged mode only
+    if ((rc = trsm_shape(M, N, budget, own, &S))) return rc;
     const bool lower = (uplo == HCL_UPLO_LOWER) != (trans == HCL_OP_T);       // op(T) is lower triangular
     const int64_t nblk = (M + S.NB - 1) / S.NB;
     hclooc_stats acc;
@@ -944,10 +957,7 @@ extern "C" int hclooc_dtrsm(hclooc_ctx* ctx, int uplo, int trans, int diag, int6
     const size_t rbytes = ((size_t)S.NB * ldx * 8 + 1023) & ~(size_t)1023;
     int nres = 0;
     {
-        static const int res_env = [] { const char* e = std::getenv("HCLOOC_TRSM_RESIDENT"); return e ? std::atoi(e) : -1; }();
-        std::lock_guard<std::mutex> lk(ctx->mu);
-        const bool own = ctx->owns_workspace || !ctx->workspace;
-        nres = trsm_resident(M, N, budget, S, own && res_env != 0, nullptr);
+        nres = trsm_resident(M, N, budget, S, own, nullptr);
     }
     struct DevMem { void* p = nullptr; ~DevMem() { if (p) cudaFree(p); } } resmem;
     double* dres[2] = {nullptr, nullptr};

@@ -118,20 +118,20 @@ def test_dtrsm_alpha_zero_degenerate_and_errors(H):
     assert np.array_equal(B.view, keep)                                        # validation errors leave B untouched
 
 
-@pytest.mark.parametrize("budget,resident", [(256 * MiB, 0), (1024 * MiB, 2)])
+@pytest.mark.parametrize("budget,resident", [(256 * MiB, 0), (1024 * MiB, 1)])
 @pytest.mark.parametrize("uplo,trans,unit", [(0, 0, 0), (1, 0, 1), (0, 1, 0), (1, 1, 0)])
 def test_dtrsm_large_block_rows_of_4096(H, uplo, trans, unit, budget, resident):
-    """NB = 4096: two block rows (one ragged), 32 inner blocks per chunk.  Under 256 MiB the block rows are staged through two
-    column chunks on two streams; under 1 GiB both block rows are resident (the DGEMM updates the second one in device memory
-    while it was uploaded during the first one's diagonal phase).  The whole result against the oracle, the residual gate on
-    sampled rows and columns."""
+    """Under 256 MiB: NB = 4096, two block rows (one ragged), staged through two column chunks on two streams, 32 inner blocks
+    per chunk.  Under 1 GiB the whole problem is one resident block row of 6000 rows (no out-of-core update; the recursion of the
+    diagonal phase is 6 levels deep).  The whole result against the oracle, the residual gate on sampled rows and columns."""
     M, N, alpha = 6000, 4500, 1.25
     A, B = trsm_inputs(H, uplo, unit, M, N, 94, "uniform")
     poison(A, uplo, unit)
     B0 = B.view.copy()
     st = H.hclooc_dtrsm(None, uplo, trans, unit, M, N, alpha, A, A.ld, B, B.ld, budget)
     got = B.view.copy()
-    assert st.plan.mb == 4096 and st.plan.h == 2 and st.plan.workspace_bytes <= budget and st.plan.n_sets == resident
+    assert (st.plan.mb, st.plan.h) == ((4096, 2) if resident == 0 else (6000, 1))
+    assert st.plan.workspace_bytes <= budget and st.plan.n_sets == resident
     ref = B0.copy()
     oracle.dtrsm(uplo, trans, unit, alpha, A.view, ref)
     assert np.abs(got - ref).max() <= FWD_RTOL * np.abs(ref).max()
@@ -164,3 +164,24 @@ def test_dtrsm_resident_and_staged_modes_agree_bitwise(H, monkeypatch):
     finally:
         H.hclooc_ctx_destroy(ctx)
     assert np.array_equal(B.view, res)
+
+
+@pytest.mark.parametrize("uplo,trans", [(0, 0), (1, 0)])
+def test_dtrsm_two_resident_block_rows_of_8192(H, uplo, trans):
+    """Block rows of 8192 rows, both resident under 2 GiB: the second one is uploaded during the first one's diagonal phase and
+    updated by the out-of-core DGEMM in device memory.  Forward agreement with the oracle and the residual gate on samples."""
+    M, N, alpha = 10000, 2000, 0.75
+    A, B = trsm_inputs(H, uplo, 0, M, N, 96, "uniform")
+    poison(A, uplo, 0)
+    B0 = B.view.copy()
+    st = H.hclooc_dtrsm(None, uplo, trans, 0, M, N, alpha, A, A.ld, B, B.ld, 2048 * MiB)
+    got = B.view.copy()
+    assert (st.plan.mb, st.plan.h, st.plan.n_sets) == (8192, 2, 2) and st.plan.workspace_bytes <= 2048 * MiB
+    ref = B0.copy()
+    oracle.dtrsm(uplo, trans, 0, alpha, A.view, ref)
+    assert np.abs(got - ref).max() <= FWD_RTOL * np.abs(ref).max()
+    rng = np.random.default_rng(1)
+    rows = np.unique(np.concatenate([[0, 8191, 8192, M - 1], rng.integers(0, M, 40)]))
+    cols = np.unique(np.concatenate([[0, N - 1], rng.integers(0, N, 40)]))
+    res, den = oracle.dtrsm_residual(uplo, trans, 0, alpha, np.nan_to_num(A.view), B0, got, rows, cols)
+    assert (res <= oracle.dtrsm_gate(M) * den).all()

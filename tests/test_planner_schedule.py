@@ -463,7 +463,7 @@ def test_dtrsm_plan_respects_the_budget_and_its_own_rules():
             for budget in (64 * 1024, 512 * 1024, 1 * MiB, 3 * MiB, 48 * MiB, 256 * MiB, 1024 * MiB, 4096 * MiB, 170 * 1024 * MiB):
                 for own in (True, False):
                     NB, chunk, res, dev = H.hclooc_dtrsm_plan(M, N, budget, own)
-                    assert 1 <= NB <= min(M, 4096) and NB * NB * 8 <= max(budget // 2, 32 * 32 * 8)
+                    assert 1 <= NB <= min(M, 8192 if own else 4096) and NB * NB * 8 <= max(budget // 2, 32 * 32 * 8)
                     assert NB == M or NB % 128 == 0 or (NB < 128 and NB % 32 == 0)
                     assert chunk % 64 == 0 and 64 <= chunk <= (N + 63) // 64 * 64
                     assert res in (0, 1, 2) and (own or res == 0)
@@ -479,7 +479,10 @@ def test_dtrsm_plan_respects_the_budget_and_its_own_rules():
     # the cases the GPU tests and the profile rely on
     assert H.hclooc_dtrsm_plan(32768, 32768, 4096 * MiB)[:3] == (4096, 16384, 2)
     assert H.hclooc_dtrsm_plan(16384, 16384, 256 * MiB)[::2] == (4096, 0)
-    assert H.hclooc_dtrsm_plan(6000, 4500, 1024 * MiB)[::2] == (4096, 2)
+    assert H.hclooc_dtrsm_plan(6000, 4500, 1024 * MiB)[::2] == (6000, 1)          # 8192-row block rows allowed: one block row
+    assert H.hclooc_dtrsm_plan(10000, 2000, 2048 * MiB)[::2] == (8192, 2)
+    assert H.hclooc_dtrsm_plan(32768, 32768, 16384 * MiB)[::2] == (8192, 2)
+    assert H.hclooc_dtrsm_plan(32768, 32768, 16384 * MiB, False)[::2] == (4096, 0)
     assert H.hclooc_dtrsm_plan(3000, 300, 48 * MiB, False)[2] == 0
     for args, code in (((0, 5, MiB), -1), ((5, 0, MiB), -2), ((200, 100, 16 * 1024), 1)):
         with pytest.raises(H.HclError) as e:
