@@ -973,6 +973,16 @@ extern "C" int hclooc_dtrsm(hclooc_ctx* ctx, int uplo, int trans, int diag, int6
             ws_max = nres * rbytes + tbytes;
         }
     }
+    // resident mode: T_ii goes up on a stream of its own WHILE the out-of-core update of its block row runs (the update is compute
+    // bound and leaves a third of the link idle; the triangle buffer is free since the previous diagonal phase was drained)
+    struct Prefetch {
+        cudaStream_t s = nullptr; cudaEvent_t e = nullptr;
+        ~Prefetch() { if (e) cudaEventDestroy(e); if (s) cudaStreamDestroy(s); }
+    } pref;
+    if (nres > 0) {
+        HCL_CUDA(cudaStreamCreateWithFlags(&pref.s, cudaStreamNonBlocking));
+        HCL_CUDA(cudaEventCreateWithFlags(&pref.e, cudaEventDisableTiming));
+    }
     const int ns = ctx->n_compute >= 2 ? 2 : 1;                  // staged mode: one stream per chunk buffer
     // resident mode: the chunks of a block row are independent pieces of one buffer, so more of them can be in flight (the
     // triangle kernel is latency bound and leaves most SMs to the other chunks' tile launches)
@@ -1031,6 +1041,7 @@ extern "C" int hclooc_dtrsm(hclooc_ctx* ctx, int uplo, int trans, int diag, int6
         const double* Ap = trans ? A + k0 * lda + r0 : A + r0 * lda + k0;           // op(T)[rows of i, solved rows], as stored
         double alpha_eff = alpha;
         double* dXr = nres ? dres[bi % nres] : nullptr;
+        bool t_prefetched = false;
         if (nres) {
             std::lock_guard<std::mutex> lk(ctx->mu);
             HCL_CUDA(cudaSetDevice(ctx->device));
@@ -1039,6 +1050,12 @@ extern "C" int hclooc_dtrsm(hclooc_ctx* ctx, int uplo, int trans, int diag, int6
                 acc.bytes_h2d += (uint64_t)nbi * N * 8; ++acc.n_copies_h2d;
             }
             HCL_CUDA(cudaStreamSynchronize(ctx->s_h2d));                            // the DGEMM's own streams do not wait for this one
+            if (kk > 0) {
+                if ((rc = copy2d(dTres, (size_t)S.ldt * 8, A + r0 * lda + r0, (size_t)lda * 8, (size_t)nbi * 8, (size_t)nbi, pref.s))) return rc;
+                HCL_CUDA(cudaEventRecord(pref.e, pref.s));
+                acc.bytes_h2d += (uint64_t)nbi * nbi * 8; ++acc.n_copies_h2d;
+                t_prefetched = true;
+            }
         }
         const auto tp0 = std::chrono::steady_clock::now();
         if (kk > 0) {
@@ -1065,10 +1082,12 @@ extern "C" int hclooc_dtrsm(hclooc_ctx* ctx, int uplo, int trans, int diag, int6
             dT = (double*)base;
             dX[0] = (double*)(base + tbytes); dX[1] = (double*)(base + tbytes + cbytes);
         }
-        if ((rc = copy2d(dT, (size_t)S.ldt * 8, A + r0 * lda + r0, (size_t)lda * 8, (size_t)nbi * 8, (size_t)nbi, ctx->s_h2d))) return rc;
-        HCL_CUDA(cudaEventRecord(ctx->events[0], ctx->s_h2d));
-        acc.bytes_h2d += (uint64_t)nbi * nbi * 8; ++acc.n_copies_h2d;
-        for (int s = 0; s < ns_res; ++s) HCL_CUDA(cudaStreamWaitEvent(ctx->s_compute[s], ctx->events[0], 0));
+        if (!t_prefetched) {
+            if ((rc = copy2d(dT, (size_t)S.ldt * 8, A + r0 * lda + r0, (size_t)lda * 8, (size_t)nbi * 8, (size_t)nbi, ctx->s_h2d))) return rc;
+            HCL_CUDA(cudaEventRecord(ctx->events[0], ctx->s_h2d));
+            acc.bytes_h2d += (uint64_t)nbi * nbi * 8; ++acc.n_copies_h2d;
+        }
+        for (int s = 0; s < ns_res; ++s) HCL_CUDA(cudaStreamWaitEvent(ctx->s_compute[s], t_prefetched ? pref.e : ctx->events[0], 0));
         if (nres == 2 && bi + 1 < nblk) {                                           // the next block row comes up meanwhile
             const int64_t i2 = lower ? bi + 1 : nblk - 2 - bi, q0 = i2 * S.NB, nb2 = std::min(S.NB, M - q0);
             if ((rc = copy2d(dres[(bi + 1) % 2], (size_t)ldx * 8, B + q0 * ldb, (size_t)ldb * 8, (size_t)N * 8, (size_t)nb2, ctx->s_h2d))) return rc;
