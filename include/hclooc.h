@@ -278,7 +278,10 @@ int hclooc_dsyr2k(hclooc_ctx* ctx, int uplo, int trans, int64_t N, int64_t K, do
  * plan.nb = chunk width, plan.h = block rows, plan.flops = M*M*N, plan.workspace_bytes = the most device memory used.
  * Errors: -2 uplo, -3 trans, -4 diag, -5 M < 0, -6 N < 0, -8 A NULL, -9 lda < M, -10 B NULL or overlapping A,
  * -11 ldb < N; HCLOOC_ERR_BUDGET when not even a 32-row block fits; the HCLOOC_ERR_* codes of hclooc_dgemm.  A singular
- * T gives Inf / NaN as in the BLAS (no check).  Validation errors leave B untouched.                                    */
+ * T gives Inf / NaN as in the BLAS (no check).  Validation errors leave B untouched.
+ * Experiment knobs (environment, read once): HCLOOC_TRSM_RESIDENT=0 staged mode only; HCLOOC_TRSM_NB_MAX=n block-row height;
+ * HCLOOC_TRSM_CHUNKS / HCLOOC_TRSM_STREAMS column chunks and streams of the resident diagonal phase (default 8 / 2);
+ * HCLOOC_TRSM_TIMING=1 prints the time of each block row's update and diagonal phase to stderr.                          */
 #define HCL_DIAG_NONUNIT 0
 #define HCL_DIAG_UNIT    1
 int hclooc_dtrsm(hclooc_ctx* ctx, int uplo, int trans, int diag, int64_t M, int64_t N, double alpha, const double* A, int64_t lda,
