@@ -54,6 +54,9 @@ void build_schedule(const hclooc_plan_t& P, int ncs, std::vector<hclooc_op_t>& o
     const EventIds ev{n_sets, P.n_bbuf, n_abuf};
     const bool scale_only = P.scale_only != 0;
     std::vector<char> set_used(n_sets, 0), set_stored(n_sets, 0);
+    // K panels p > 0 re-read from the HOST the block that panel p-1 stored there, possibly through another C buffer:
+    // per (i, j) block the C buffer whose R(c_ij) wrote it last (-1: not yet stored in this call)
+    std::vector<int> stored_through(P.kpanels > 1 ? (size_t)(P.h * P.w) : 0, -1);
     // A-slice cache
     struct ABuf { int64_t row = -1, panel = -1; int64_t last_use = -1; int ready_ev = -1; int64_t readers = 0; };
     std::vector<ABuf> acache(n_abuf);
@@ -119,6 +122,13 @@ void build_schedule(const hclooc_plan_t& P, int ncs, std::vector<hclooc_op_t>& o
         }
         if (cload) {
             if (set_stored[c]) push(HCLOOC_OP_WAIT, 0, ev.c_stored(c));                  // Wait(eC): block is back on the host
+            if (s.p > 0) {
+                // the host block itself: S(c_ij) of panel p reads what R(c_ij) of panel p-1 wrote.  That download was issued
+                // earlier (a whole slab of steps ago) on the in-order D2H stream, so the newest record of its buffer's
+                // c_stored event -- that download's own or a later one's -- covers it.
+                const int prev = stored_through[(size_t)(s.i + P.h * s.j)];
+                if (prev >= 0 && prev != c) push(HCLOOC_OP_WAIT, 0, ev.c_stored(prev));
+            }
             hclooc_op_t& o = push(HCLOOC_OP_H2D_C, 0, -1);                                // S(c_ij)
             o.buf = cbuf_id(c); o.r0 = i0; o.nr = mi; o.c0 = j0; o.nc = nj; o.step = idx;
             any = true;
@@ -162,6 +172,7 @@ void build_schedule(const hclooc_plan_t& P, int ncs, std::vector<hclooc_op_t>& o
         }
         push(HCLOOC_OP_RECORD, 1, ev.c_stored(c));                                        // Rec(eC)
         set_stored[c] = 1;
+        if (!stored_through.empty()) stored_through[(size_t)(s.i + P.h * s.j)] = c;
     };
 
     // With one B buffer the uploads of the first steps of a column go out BEFORE the B reload, so the link

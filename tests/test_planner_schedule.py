@@ -215,6 +215,8 @@ def simulate(plan, ops, alpha_zero=False):
             access(int(o["buf"]), s, True, lo, hi, (idx, "h2d", kind))
             h2d += int(o["nr"]) * int(o["nc"]) * 8; n_h2d += 1
             key = (kind, int(o["r0"]), int(o["nr"]), int(o["c0"]), int(o["nc"]))
+            if kind == K_H2D_C:      # reads the HOST block: ordered after the download that wrote it (K panels p > 0)
+                access(("host C", int(o["r0"]), int(o["c0"])), s, False, 0, int(o["nr"]), (idx, "h2d reads host C"))
             if kind == K_H2D_B:
                 held = content.setdefault(int(o["buf"]), {})
                 for old in [r for r in held if not (r[1] <= lo or hi <= r[0])]:
@@ -247,6 +249,7 @@ def simulate(plan, ops, alpha_zero=False):
             access(int(o["buf"]), s, False, 0, int(o["nr"]), (idx, "d2h"))
             c = content[int(o["buf"])]
             assert c[0] == "result" and c[1:5] == (int(o["r0"]), int(o["nr"]), int(o["c0"]), int(o["nc"]))
+            access(("host C", int(o["r0"]), int(o["c0"])), s, True, 0, int(o["nr"]), (idx, "d2h writes host C"))
             d2h += int(o["nr"]) * int(o["nc"]) * 8; n_d2h += 1
     assert h2d == plan.bytes_h2d and d2h == plan.bytes_d2h
     assert n_h2d == plan.n_copies_h2d and n_d2h == plan.n_copies_d2h
@@ -294,6 +297,38 @@ def test_simulator_catches_a_missing_wait():
         assert idx
         with pytest.raises(AssertionError, match="hazard"):
             simulate(p, np.delete(ops, idx))
+
+
+@pytest.mark.parametrize("shape", [(256, 16, 200000, 1 * MiB), (8, 16, 1000000, 1 * MiB), (4096, 16, 2000000, 64 * MiB),
+                                   (96, 112, 20000, 600 * 1024), (64, 1500, 9000, 1 * MiB)])
+def test_k_panels_reread_host_c_only_after_its_download(shape):
+    """K split (kpanels > 1): S(c_ij) of panel p reads the host block R(c_ij) of panel p-1 wrote, possibly through another
+    C buffer (h*w < n_sets, e.g. w == 1 with few rows).  The simulator tracks the host blocks (D2H = write, H2D_C = read);
+    the schedule must order the two, and the check is not vacuous: without the extra waits the first three plans race."""
+    M, N, K, budget = shape
+    p = H.hclooc_plan(M, N, K, 1, 0, budget)
+    assert p.kpanels > 1
+    for ncs in (1, 3, 8):
+        ops = H.hclooc_schedule(p, ncs)
+        simulate(p, ops)
+    if p.h * p.w < p.n_sets or (p.h * p.w) % p.n_sets:
+        ops = H.hclooc_schedule(p, 8)
+        c_stored = range(2 * p.n_sets, 3 * p.n_sets)
+        # the waits of the H2D stream on c_stored that directly precede an H2D_C of a panel p > 0 and are not its own buffer's
+        drop = []
+        for i, o in enumerate(ops):
+            if o["kind"] == K_H2D_C and o["step"] >= p.h * p.w:
+                own = 2 * p.n_sets + (int(o["buf"]) - p.n_abuf)
+                k = i - 1
+                while k >= 0 and ops[k]["kind"] == K_WAIT and ops[k]["stream"] == 0:
+                    if int(ops[k]["event"]) in c_stored and int(ops[k]["event"]) != own:
+                        drop.append(k)
+                    k -= 1
+        if shape[:2] in ((256, 16), (8, 16), (4096, 16)):
+            assert drop
+        if drop:
+            with pytest.raises(AssertionError, match="hazard on buffer \\('host C'"):
+                simulate(p, np.delete(ops, drop))
 
 
 def test_serpentine_order_reuses_resident_a_slices():
