@@ -8,7 +8,9 @@ __graft_entry__.smoke() and bench.py's cpu_baseline / `--impl reference` legs us
 Pinned by tests/test_oracle_pins.py (brute force, int64 exactness, closed forms, exact-sum error
 bound, numpy cross-check, the paper's 44-element partition example; dsyrk: brute force on the triangle,
 exact symmetry, int64 exactness, untouched other triangle; dtrsm: scipy's solve_triangular, exact rational
-arithmetic on tiny cases, identity / diagonal / all-ones closed forms, int64 exactness, transposed-storage identity) -- nothing here is "parity unpinned".
+arithmetic on tiny cases, identity / diagonal / all-ones closed forms, int64 exactness, transposed-storage identity; the D returned
+by dsyrk / dsyr2k against numpy's |A||B|^T products; dtrsm_gate against gamma_(M+2) in exact arithmetic; oracle/checksum.py
+against the full oracle, int64 arithmetic and single-element mutations) -- nothing here is "parity unpinned".
 """
 from __future__ import annotations
 
@@ -179,9 +181,12 @@ def dtrsm(uplo, trans, unit, alpha, A, B):
         raise ValueError("oracle_dtrsm: bad argument")
 
 
-# gate for a triangular solve of order M: substitution in any summation order leaves a residual
-# |alpha b - op(T) x| <= gamma_M |op(T)||x| elementwise, gamma_M = M u / (1 - M u), u = 2^-53 (Higham thm 8.5); the product
-# alpha*b adds one rounding.  DESIGN.md reading G23.
+# gate for a triangular solve of order M (reading G23): substitution in any summation order leaves a residual
+# |b' - op(T) x| <= gamma_M |op(T)||x| elementwise, gamma_n = n u / (1 - n u), u = 2^-53 (Higham thm 8.5); forming b' = alpha*b
+# is one more rounding and the kernel multiplies by a rounded reciprocal of t_ii instead of dividing (one more), so the gate is
+#     |alpha b - op(T) x| <= gamma_(M+2) (|alpha b| + |op(T)||x|)        -- this function returns gamma_(M+2).
+# Pinned by tests/test_oracle_pins.py::test_dtrsm_gate_is_gamma_m_plus_2 (the closed form in exact rational arithmetic, and
+# that oracle.dtrsm's own solutions sit inside it while a one-ulp-per-row perturbation of a long solve does not).
 def dtrsm_gate(M: int) -> float:
     u = 2.0 ** -53
     return (M + 2) * u / (1.0 - (M + 2) * u)

@@ -185,3 +185,29 @@ def test_dtrsm_two_resident_block_rows_of_8192(H, uplo, trans):
     cols = np.unique(np.concatenate([[0, N - 1], rng.integers(0, N, 40)]))
     res, den = oracle.dtrsm_residual(uplo, trans, 0, alpha, np.nan_to_num(A.view), B0, got, rows, cols)
     assert (res <= oracle.dtrsm_gate(M) * den).all()
+
+
+@pytest.mark.parametrize("uplo,trans,budget", [(0, 0, 1 * MiB), (1, 1, 1 * MiB), (1, 0, 64 * MiB)])
+def test_dtrsm_ill_conditioned_only_the_backward_gate_holds(H, uplo, trans, budget):
+    """A triangle whose off-diagonal entries are as large as its diagonal (uniform[-0.8, 0.8) against |t_ii| in [1, 2)): the
+    solution grows by twelve orders of magnitude down the substitution, so agreement with another summation order's solution is
+    not a property of the method -- the elementwise backward bound gamma_(M+2) (G23, Higham thm 8.5) is, and it is the
+    only thing asserted here (the oracle's own solution satisfies it too: tests/test_oracle_pins.py)."""
+    M, N = 600, 40
+    rng = np.random.default_rng(3)
+    T = np.diag(rng.uniform(1, 2, M) * rng.choice([-1, 1], M)) + 0.8 * np.tril(rng.uniform(-1, 1, (M, M)), -1)
+    A = H.HostMatrix(M, M, M); B = H.HostMatrix(M, N, N)
+    lower_stored = (uplo == 0)
+    # op(T) must be the lower-triangular T above: store T or T^T in the triangle `uplo` names
+    stored = T if (lower_stored != bool(trans)) else T.T
+    assert np.array_equal(np.tril(stored) if lower_stored else np.triu(stored), stored)
+    A.view[...] = stored
+    poison(A, uplo, 0)
+    B.view[...] = rng.uniform(-1, 1, (M, N))
+    B0 = B.view.copy()
+    st = H.hclooc_dtrsm(None, uplo, trans, 0, M, N, 1.0, A, A.ld, B, B.ld, budget)
+    got = B.view.copy()
+    assert np.isfinite(got).all() and np.abs(got).max() > 1e9, "the case is meant to be ill conditioned"
+    assert st.plan.h == (1 if budget > 8 * MiB else st.plan.h) and (budget > 8 * MiB or st.plan.h > 1)
+    res, den = oracle.dtrsm_residual(uplo, trans, 0, 1.0, np.nan_to_num(A.view), B0, got)
+    assert (res <= oracle.dtrsm_gate(M) * den).all(), float((res / den).max() / oracle.dtrsm_gate(M))

@@ -394,6 +394,98 @@ def test_dsyr2k_brute_force_symmetry_and_integers():
     assert np.array_equal(s1, s2)
 
 
+def test_dsyrk_and_dsyr2k_denominators_against_the_absolute_value_products():
+    """The D these oracles return is the tolerance denominator of the DSYRK / DSYR2K float parity tests:
+        dsyrk:  D_ij = |alpha| sum_k |a_ik||a_jk| + |beta||C0_ij|
+        dsyr2k: D_ij = |alpha| sum_k (|a_ik||b_jk| + |b_ik||a_jk|) + |beta||C0_ij|
+    on the referenced triangle and 0 elsewhere -- compared here with numpy's |A||B|^T products (an independent routine; the sums
+    of positive terms agree to a few ulps), with a case where the signed result cancels (D must not), and with a wrong formula
+    (a dropped term, |beta| forgotten, the signed instead of the absolute intermediate) shown to fall outside the band."""
+    rng = np.random.default_rng(17)
+    for uplo in (0, 1):
+        for trans in (0, 1):
+            N, K, alpha, beta = 19, 45, -1.75, 2.5
+            A = rng.uniform(-1, 1, (K, N) if trans else (N, K)); B = rng.uniform(-1, 1, (K, N) if trans else (N, K))
+            C0 = rng.uniform(-1, 1, (N, N))
+            a, b = np.abs(A.T if trans else A), np.abs(B.T if trans else B)
+            keep = np.tril(np.ones((N, N), bool)) if uplo == 0 else np.triu(np.ones((N, N), bool))
+            D1 = oracle.dsyrk(uplo, trans, alpha, A, beta, C0.copy(), want_denominator=True)
+            want1 = abs(alpha) * (a @ a.T) + abs(beta) * np.abs(C0)
+            assert np.allclose(D1[keep], want1[keep], rtol=1e-13, atol=0) and (D1[~keep] == 0).all()
+            D2 = oracle.dsyr2k(uplo, trans, alpha, A, B, beta, C0.copy(), want_denominator=True)
+            want2 = abs(alpha) * (a @ b.T + b @ a.T) + abs(beta) * np.abs(C0)
+            assert np.allclose(D2[keep], want2[keep], rtol=1e-13, atol=0) and (D2[~keep] == 0).all()
+            # plausible mistakes are far outside that band
+            for wrong in (abs(alpha) * (a @ b.T) + abs(beta) * np.abs(C0),              # second product dropped
+                          abs(alpha) * (a @ b.T + b @ a.T),                              # |beta||C0| dropped
+                          abs(alpha) * (a @ b.T + b @ a.T) + abs(beta) * np.abs(C0) +
+                          np.abs(alpha * ((A.T if trans else A) @ (B if trans else B.T)) + beta * C0)):  # |mid| not removed
+                assert not np.allclose(D2[keep], wrong[keep], rtol=1e-6, atol=0)
+    # cancellation: B = -A on integers gives C = 0 exactly while D stays the full absolute sum
+    N, K = 9, 14
+    A = rng.integers(-4, 5, (N, K)).astype(np.float64)
+    C = np.zeros((N, N))
+    D = oracle.dsyr2k(0, 0, 1.0, A, -A, 0.0, C, want_denominator=True)
+    assert np.array_equal(np.tril(D), np.tril(2.0 * (np.abs(A) @ np.abs(A).T)))
+    C1 = np.zeros((N, N)); C2 = np.zeros((N, N))
+    oracle.dsyr2k(0, 0, 1.0, A, A, 0.0, C1); oracle.dsyr2k(0, 0, 1.0, A, -A, 0.0, C2)
+    assert np.array_equal(np.tril(C1), -np.tril(C2)) and np.tril(C1).any()
+
+
+# ------------------------------------------------------------------ oracle/checksum.py: the whole-matrix checker of configs 3-5
+def test_checksum_identities_are_exact_on_integers_and_see_one_wrong_element():
+    """oracle.checksum.before / expected against the full oracle on a case small enough to run it (60 x 70 x 50): on integer
+    inputs C x and y^T C are EXACTLY the row / column sums of oracle.dgemm's C (half-integer beta included); the gate
+    denominators Dx, yD equal the oracle's elementwise D summed with |x|, |y|; and a single wrong element of C -- by one unit --
+    flips exactly one row sum and one column sum."""
+    import oracle.checksum as cks
+    M, N, K, alpha, beta = 60, 70, 50, 2.0, -0.5
+    A = synthgen.fill_numpy(M, K, 91, "A", "int"); B = synthgen.fill_numpy(K, N, 91, "B", "int"); C0 = synthgen.fill_numpy(M, N, 91, "C", "int")
+    x = synthgen.fill_numpy(N, 1, 77, "A", "int")[:, 0]; y = synthgen.fill_numpy(1, M, 77, "B", "int")[0]
+    assert x.any() and y.any() and np.abs(x).max() <= 4
+    pre = cks.before(C0, x, y)
+    C = C0.copy()
+    D = oracle.dgemm(alpha, A, B, beta, C, want_denominator=True)
+    Cx, yC, Dx, yD = cks.expected(alpha, A, B, beta, pre, x, y)
+    assert np.array_equal(Cx, C @ x) and np.array_equal(yC, y @ C)
+    # independent exact value: int64 arithmetic, scaled by 2 for the half-integer beta
+    Ci2 = 2 * int(alpha) * (A.astype(np.int64) @ B.astype(np.int64)) + int(2 * beta) * C0.astype(np.int64)
+    assert np.array_equal(2 * Cx, (Ci2 @ x.astype(np.int64)).astype(np.float64))
+    assert np.array_equal(2 * yC, (y.astype(np.int64) @ Ci2).astype(np.float64))
+    assert np.allclose(Dx, D @ np.abs(x), rtol=1e-12, atol=0) and np.allclose(yD, np.abs(y) @ D, rtol=1e-12, atol=0)
+    # one wrong element: exactly its row sum and its column sum move (x_j, y_i nonzero there)
+    i, j = 17, int(np.flatnonzero(x)[3])
+    assert y[i] != 0
+    bad = C.copy(); bad[i, j] += 1.0
+    assert list(np.flatnonzero(bad @ x != Cx)) == [i] and list(np.flatnonzero(y @ bad != yC)) == [j]
+
+
+def test_checksum_gate_on_floats_is_tight_enough_to_see_a_dropped_term():
+    """On float inputs the identities hold within sum_j RTOL*D_ij*|x_j| (and the column form): the oracle's own C passes with
+    three orders of magnitude to spare, a C with one k term dropped in one element fails, and Dx, yD are the elementwise D
+    summed (so the float leg is neither vacuous nor looser than the element gate it stands in for)."""
+    import oracle.checksum as cks
+    rng = np.random.default_rng(19)
+    M, N, K, alpha, beta = 60, 70, 50, 1.0, 0.5
+    A, B, C0 = rng.uniform(-1, 1, (M, K)), rng.uniform(-1, 1, (K, N)), rng.uniform(-1, 1, (M, N))
+    x = synthgen.fill_numpy(N, 1, 77, "A", "int")[:, 0]; y = synthgen.fill_numpy(1, M, 77, "B", "int")[0]
+    pre = cks.before(C0, x, y)
+    C = C0.copy()
+    D = oracle.dgemm(alpha, A, B, beta, C, want_denominator=True)
+    Cx, yC, Dx, yD = cks.expected(alpha, A, B, beta, pre, x, y)
+    assert np.allclose(Dx, D @ np.abs(x), rtol=1e-12, atol=0) and np.allclose(yD, np.abs(y) @ D, rtol=1e-12, atol=0)
+    assert (np.abs(C @ x - Cx) <= 1e-3 * oracle.RTOL * Dx).all() and (np.abs(y @ C - yC) <= 1e-3 * oracle.RTOL * yD).all()
+    i, j = 5, int(np.flatnonzero(x)[0])
+    bad = C.copy(); bad[i, j] -= alpha * A[i, 7] * B[7, j]                       # one k term of one element dropped
+    assert not (np.abs(bad @ x - Cx) <= oracle.RTOL * Dx).all()
+    # exactly-representable closed form: A = I, so C = B + beta*C0 and the sums are plain
+    I = np.eye(M)
+    Bs = rng.integers(-4, 5, (M, N)).astype(np.float64); Cs = rng.integers(-4, 5, (M, N)).astype(np.float64)
+    pre = cks.before(Cs, x, y)
+    Cx, yC, _, _ = cks.expected(1.0, I, Bs, 0.5, pre, x, y)
+    assert np.array_equal(Cx, (Bs + 0.5 * Cs) @ x) and np.array_equal(yC, y @ (Bs + 0.5 * Cs))
+
+
 # ---------------------------------------------------------------------------------------------------------------------
 # DTRSM (side = Left), the routine PAPER.md:412 names as future work: op(T) X = alpha B by substitution
 ALL_TRSM = list(itertools.product((0, 1), (0, 1), (0, 1)))          # uplo, trans, unit
@@ -535,3 +627,29 @@ def test_dtrsm_transposed_storage_identity():
             X1 = B.copy(); oracle.dtrsm(uplo, 1, unit, 1.25, A, X1)
             X2 = B.copy(); oracle.dtrsm(1 - uplo, 0, unit, 1.25, At, X2)
             assert np.array_equal(X1, X2)
+
+
+def test_dtrsm_gate_is_gamma_m_plus_2():
+    """oracle.dtrsm_gate(M) = gamma_(M+2) = (M+2)u / (1 - (M+2)u), u = 2^-53 (Higham, Accuracy and Stability, thm 8.5 plus the
+    two extra roundings of DESIGN.md G23), checked in exact rational arithmetic; it grows with M, and the oracle's own solution of
+    an ILL-CONDITIONED system (forward error large) still sits inside the backward gate -- which is why only that gate is asserted
+    on such systems -- while a solution that is off by a relative 1e-12 in one element does not."""
+    from fractions import Fraction
+    u = Fraction(1, 2 ** 53)
+    for M in (1, 5, 128, 4096, 32768):
+        want = (M + 2) * u / (1 - (M + 2) * u)
+        assert abs(Fraction(oracle.dtrsm_gate(M)) - want) <= want * Fraction(1, 2 ** 50)
+    assert oracle.dtrsm_gate(10) < oracle.dtrsm_gate(11)
+    # ill conditioned: unit lower triangle with -2 below the diagonal everywhere near it (condition number ~ 3^M)
+    rng = np.random.default_rng(23)
+    M, N = 48, 6
+    A = np.eye(M) + np.tril(rng.uniform(-2.0, -1.0, (M, M)), -1)
+    B = rng.uniform(-1, 1, (M, N))
+    X = B.copy()
+    oracle.dtrsm(0, 0, 0, 1.0, A, X)
+    assert np.abs(X).max() > 1e8                                          # the solution blows up: forward error is hopeless
+    res, den = oracle.dtrsm_residual(0, 0, 0, 1.0, A, B, X)
+    assert (res <= oracle.dtrsm_gate(M) * den).all()
+    Xbad = X.copy(); Xbad[M - 1, 0] *= 1.0 + 1e-12
+    res, den = oracle.dtrsm_residual(0, 0, 0, 1.0, A, B, Xbad)
+    assert not (res <= oracle.dtrsm_gate(M) * den).all()
