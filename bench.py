@@ -2,22 +2,32 @@
 """bench.py -- end-to-end out-of-core DGEMM TFLOP/s on one B200 (BASELINE.json metric).
 
 A "step" is one pass of the whole hot path (S0 validate, S1 plan, S2-S4 uploads, S5 DGEMM tile kernel,
-S6 download, S7 events) over one synthetic problem: hclooc_dgemm(M,N,K,alpha,A,lda,B,ldb,beta,C,ldc,budget).
+S6 download, S7 events) over one synthetic problem: hclooc_dgemm(M,N,K,alpha,A,lda,B,ldb,beta,C,ldc,budget)
+with A, B, C in pinned HOST memory.
 
-  value : the same call with A, B, C already resident in HBM (device pointers): the library's in-core case,
-          one DGEMM launch on the caller's matrices with nothing staged, i.e. whole-job
-          throughput with inputs resident when the timed region starts.
-  e2e   : the same call through the C ABI with pinned HOST buffers (the product path): host->device and
-          device->host copies inside the timed region.  Its roofline is max(flops / FP64 peak, link time).
-  roofline : the FP64 DMMA kernel timed alone with CUDA events on its launch stream at a GPU-filling launch of the
-          plan's B-slice shape (M x nb x K; hclDgemmAsync picks the persistent stream-K variant for it);
-          `pipeline_step` inside it is one step of the plan launched exactly as the pipeline launches it
-          (mb x nb x K with plan.ksplit CTAs per tile), against the peak of the SMs that launch occupies.
-  cpu_baseline : the oracle, as it stands, on the host cores, on a bounded row sample of the same workload.
+Workload (`--workload auto`, the default): the LARGEST configuration the host can pin -- BASELINE.json
+configs[4] (beyond-HBM: M = N = 163840, K = 8192, budget = all free HBM) scaled to this host's memory
+("cfg5s": M = N = 147456 on a 196 GiB host, A+B+C = 193 GB > the GPU's memory), else configs[3], [2], [1].
 
-`--impl reference` times the oracle (the reference arm of this tier).  Under torchrun the problem grows to
-world*M rows cut into one row band of C per GPU (independent bands, B on every rank, no collective: weak
-scaling; DESIGN.md "Multi-GPU").
+  value : device-timed (CUDA events around the K calls) throughput of that call.  Nothing of such a problem can
+          be resident in HBM, so the timed region is the host-resident call itself.
+  e2e   : the same K calls timed by the host clock (call entry to return, G16), with the scheduler's actual
+          host<->device bytes; its roofline is max(flops / FP64 peak, link time at the link rates measured
+          on this box right before).
+  in_core : the library's in-core case (all three operands device-resident: one stream-K launch, nothing
+          staged) on a problem that fits -- the kernel-only rate, NOT the metric.
+  per_config : BASELINE configs[0..3] (cfg1-cfg4) end to end in the same run, each with its bytes, bound,
+          fraction of its roofline and plan.
+  roofline : the FP64 DMMA tile kernel AS THE PIPELINE LAUNCHES IT: a traced call brackets every kernel with
+          events on its own compute stream; achieved = flops of all launches / time during which at least one
+          of them was running.  `solo_step` is one step's launch timed alone, `streamk` a GPU-filling launch of
+          the persistent kernel; `peak_measured` is hclooc_probe_fp64 run live.
+  cpu_baseline : the oracle, as it stands, on the host cores, on a bounded sample of the same workload.
+
+`--impl reference` times the oracle (the reference arm of this tier) under the same metric string and
+workload name.  Under torchrun the problem grows to world*M rows cut into one row band of C per GPU
+(independent bands, B on every rank, no collective: weak scaling).
+`--op dsyrk|dtrsm|dpotrf` and `--sweep transition` time the other product paths (one JSON line each).
 """
 import argparse
 import json
@@ -34,10 +44,11 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 MiB, GiB = 1 << 20, 1 << 30
-# BASELINE.json configs (index = position in the list); cfg2 (index 1) is the one the metric is quoted on.
+METRIC = "end-to-end out-of-core DGEMM TFLOP/s (host-resident A,B,C) and % of roofline"
+# BASELINE.json configs (index + 1 = cfg number); budget 0 = all free HBM
 WORKLOADS = {
     "cfg1": dict(M=512, N=512, K=512, alpha=1.0, beta=0.5, budget=1 * MiB, dist="uniform", seed_idx=1,
-                 desc="512^3 FP64, budget 1 MiB"),
+                 desc="512^3 FP64, alpha=1 beta=0.5, budget 1 MiB"),
     "cfg2": dict(M=8192, N=8192, K=8192, alpha=1.0, beta=1.0, budget=256 * MiB, dist="uniform", seed_idx=2,
                  desc="8192^3 FP64, alpha=1 beta=1, budget 256 MiB"),
     "cfg3": dict(M=32768, N=32768, K=32768, alpha=1.0, beta=0.0, budget=4 * GiB, dist="uniform", seed_idx=3,
@@ -45,9 +56,48 @@ WORKLOADS = {
     "cfg4": dict(M=65536, N=65536, K=16384, alpha=2.0, beta=-1.0, budget=16 * GiB, dist="normal", seed_idx=4,
                  desc="65536x65536x16384 FP64, alpha=2 beta=-1, budget 16 GiB"),
 }
-FP64_PEAK_TFLOPS = 37.2   # 148 SMs x 4 SMSPs x 32 flop/clk (DMMA.8x8x4: 512 flop / 16 clk) x 1.965 GHz; measured 37.17
+FP64_PEAK_TFLOPS = 37.2   # 148 SMs x 4 SMSPs x 32 flop/clk (DMMA.8x8x4: 512 flop / 16 clk) x 1.965 GHz
 # fallback (the first box probed, profiles/r01_box_probe.md); bench.py measures the link of the box it runs on (measure_link)
 LINK = dict(h2d_GBps=55.5, d2h_GBps=51.5, duplex_GBps=88.0, source="profiles/r01_box_probe.md")
+
+
+def meminfo(key):
+    with open("/proc/meminfo") as f:
+        for line in f:
+            if line.startswith(key + ":"):
+                return int(line.split()[1]) * 1024
+    return 0
+
+
+def wl_bytes(wl):
+    return 8 * (wl["M"] * wl["K"] + wl["K"] * wl["N"] + wl["M"] * wl["N"])
+
+
+def cfg5_scaled(share=1):
+    """BASELINE configs[4] (M = N = 163840, K = 8192, alpha 1, beta 0.5, budget = all free HBM: 236 GB pinned) scaled to
+    this host: the largest M = N (a multiple of 2048, at most 163840) whose three matrices leave 14 GiB of the host's
+    memory (MemTotal / share, share = ranks on this node) unpinned.  MemTotal, not MemAvailable, so that both arms of a
+    run pick the same size."""
+    room = meminfo("MemTotal") // share - 14 * GiB
+    K, n = 8192, 163840
+    while n > 2048 and 8 * (n * n + 2 * n * K) > room:
+        n -= 2048
+    return dict(M=n, N=n, K=K, alpha=1.0, beta=0.5, budget=0, dist="uniform", seed_idx=5,
+                desc=f"{n}x{n}x{K} FP64, alpha=1 beta=0.5, budget = all free HBM (BASELINE configs[4] scaled to this host's memory)")
+
+
+def pick_workload(name, share=1):
+    """`auto`: the largest configuration whose matrices this host can pin (per rank)."""
+    if name != "auto":
+        return (name, cfg5_scaled(share)) if name == "cfg5s" else (name, WORKLOADS[name])
+    room = meminfo("MemTotal") // share - 14 * GiB
+    s5 = cfg5_scaled(share)
+    if s5["M"] > 65536 and wl_bytes(s5) <= room:
+        return "cfg5s", s5
+    for cand in ("cfg4", "cfg3", "cfg2"):
+        if wl_bytes(WORKLOADS[cand]) <= room:
+            return cand, WORKLOADS[cand]
+    return "cfg1", WORKLOADS["cfg1"]
 
 
 class ClockSampler:
@@ -94,15 +144,17 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def ncu_traffic(launch):
-    """dram__bytes_read.sum + dram__bytes_write.sum of the roofline-leg launch from the committed ncu capture
-    (profiles/r01_traffic.json, written from `ncu --set full`), or None if that capture is of another launch."""
+def ncu_traffic(kernel, launch):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture of that kernel at
+    that launch shape (profiles/traffic.json, one entry per captured launch), or None when no capture matches."""
     try:
-        with open(os.path.join(ROOT, "profiles", "r01_traffic.json")) as f:
-            t = json.load(f)
-        return t["dram_bytes"] if t.get("launch") == launch else None
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            for t in json.load(f)["captures"]:
+                if t.get("launch") == launch and t.get("kernel") == kernel:
+                    return t["dram_bytes"], t.get("source")
     except (OSError, ValueError, KeyError):
-        return None
+        pass
+    return None, None
 
 
 def measure_link(H, total=1 << 30, chunk=256 << 20):
@@ -151,19 +203,37 @@ def link_roofline_s(flops, bytes_h2d, bytes_d2h):
     return max(t_flop, t_link), t_flop, t_link
 
 
-def oracle_sample(wl, rows, seed):
-    """Inputs for the oracle on a bounded sample: the first `rows` rows of C (all N columns, whole K)."""
-    import synthgen
-    M, N, K = rows, wl["N"], wl["K"]
-    A = synthgen.fill(np.empty((M, K)), seed, "A", wl["dist"], logical_cols=K)
-    B = synthgen.fill(np.empty((K, N)), seed, "B", wl["dist"])
-    C = synthgen.fill(np.empty((M, N)), seed, "C", wl["dist"], logical_cols=N)
-    return A, B, C
+def ci95_rel(xs):
+    """Half-width of the 95 % confidence interval of the mean over the mean (Student t; PAPER.md:362 asks for 2.5 %)."""
+    n = len(xs)
+    if n < 2:
+        return None
+    t95 = {2: 12.71, 3: 4.303, 4: 3.182, 5: 2.776, 6: 2.571, 7: 2.447, 8: 2.365, 9: 2.306, 10: 2.262}.get(n, 2.0 if n > 30 else 2.2)
+    return float(t95 * np.std(xs, ddof=1) / np.sqrt(n) / np.mean(xs))
 
 
-def time_oracle(wl, rows, seed, steps, warmup):
+# ---------------------------------------------------------------------------------------------- the oracle legs
+def oracle_sample_shape(wl, flops_target, rows=512):
+    """A bounded sample of the workload for the oracle: the first `rows` rows (32-row blocks x the OpenMP threads) and as many
+    leading columns of C as make about `flops_target` flops, whole K."""
+    rows = min(wl["M"], rows)
+    cols = int(flops_target / (2.0 * rows * wl["K"])) // 128 * 128
+    cols = min(wl["N"], max(128, cols))
+    return rows, cols
+
+
+def time_oracle(wl, rows, cols, seed, steps, warmup, mats=None):
+    """oracle.dgemm on C[:rows, :cols] = alpha * A[:rows] * B[:, :cols] + beta * C[:rows, :cols]; `mats` = (A, B, C) numpy views
+    of the workload's host matrices when the caller has them, else the sample is generated (same seeds, same elements)."""
     import oracle
-    A, B, C = oracle_sample(wl, rows, seed)
+    import synthgen
+    K = wl["K"]
+    if mats is None:
+        A = synthgen.fill(np.empty((rows, K)), seed, "A", wl["dist"], logical_cols=K)
+        B = synthgen.fill(np.empty((K, cols)), seed, "B", wl["dist"], logical_cols=wl["N"])
+        C = synthgen.fill(np.empty((rows, cols)), seed, "C", wl["dist"], logical_cols=wl["N"])
+    else:
+        A, B, C = mats[0][:rows], mats[1][:, :cols], mats[2][:rows, :cols].copy()
     times = []
     for it in range(warmup + steps):
         t0 = time.perf_counter()
@@ -171,23 +241,24 @@ def time_oracle(wl, rows, seed, steps, warmup):
         dt = time.perf_counter() - t0
         if it >= warmup:
             times.append(dt)
-    flops = 2.0 * rows * wl["N"] * wl["K"]
-    return flops, times
+    return 2.0 * rows * cols * K, times
 
 
-def run_reference(args, wl, name):
-    """Reference arm of this tier: the CPU oracle, as it stands, on the host cores."""
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
+def run_reference(args):
+    """Reference arm of this tier: the CPU oracle, as it stands, on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
         return
+    share = int(os.environ.get("LOCAL_WORLD_SIZE", os.environ.get("WORLD_SIZE", "1")))
+    name, wl = pick_workload(args.workload, share)
     cores = os.cpu_count() or 1
-    rows = min(wl["M"], max(32, args.ref_rows))
-    flops, times = time_oracle(wl, rows, 180805056 + wl["seed_idx"], args.steps, max(1, min(args.warmup, 1)))
+    rows, cols = oracle_sample_shape(wl, args.ref_flops, args.ref_rows)
+    steps = args.steps if args.steps else 5
+    flops, times = time_oracle(wl, rows, cols, 180805056 + wl["seed_idx"], steps, args.warmup)
     ms = 1e3 * float(np.mean(times))
     val = flops / (ms * 1e-3) / 1e12
-    sample = f"first {rows} rows of C (all {wl['N']} columns, K={wl['K']}) per step, oracle.dgemm, OpenMP"
-    out = {"impl": "reference", "metric": "end-to-end out-of-core DGEMM TFLOP/s (host-resident A,B,C)", "value": val,
-           "unit": "TFLOP/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+    sample = f"first {rows} rows x first {cols} columns of C (K={wl['K']}) per step, oracle.dgemm, OpenMP"
+    out = {"impl": "reference", "metric": METRIC, "value": val,
+           "unit": "TFLOP/s", "n_gpus": args.gpus, "steps": steps, "warmup": args.warmup, "ms_per_step": ms,
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
            "config": {"workload": f"{name}: {wl['desc']}", "sample": sample},
            "cpu_baseline": {"value": val, "unit": "TFLOP/s", "cores": cores, "kind": "oracle", "sample": sample},
@@ -196,200 +267,366 @@ def run_reference(args, wl, name):
     print(json.dumps(out))
 
 
-def run_ours(args, wl, name):
-    import torch
-    import synthgen
-    import paper_1808_05056_b200 as H
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback for the product path")
-    torch.cuda.set_device(local)
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    M, N, K, alpha, beta, budget = wl["M"], wl["N"], wl["K"], wl["alpha"], wl["beta"], wl["budget"]
-    seed = synthgen.BASE_SEED + wl["seed_idx"]
-    flops = 2.0 * M * N * K
-    # N > 1: ONE problem of world*M rows cut into row bands of C (hclooc_shard_rows): rank r owns rows r*M .. of A
-    # and C, every rank holds all of B; the bands are independent, so no collective is on
-    # the data path and per-GPU work is fixed as N grows (weak scaling).
-    row0, rows = H.hclooc_shard_rows(world * M, world, rank, 128)
-    assert (row0, rows) == (rank * M, M) or M % 128
+# ---------------------------------------------------------------------------------------------- our arm
+class Bench:
+    def __init__(self, args):
+        import torch
+        import synthgen
+        import paper_1808_05056_b200 as H
+        self.torch, self.synthgen, self.H, self.args = torch, synthgen, H, args
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.local = int(os.environ.get("LOCAL_RANK", "0"))
+        self.share = int(os.environ.get("LOCAL_WORLD_SIZE", str(self.world)))
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback for the product path")
+        torch.cuda.set_device(self.local)
+        self.dist = None
+        if self.world > 1:
+            import torch.distributed as dist
+            dist.init_process_group("nccl", device_id=torch.device("cuda", self.local))
+            self.dist = dist
+        self.ta, self.tb = int(args.trans[0] == "T"), int(args.trans[1] == "T")
 
-    # ---- inputs: pinned host matrices (the product path) and HBM-resident copies (the `value` leg)
-    A, B, C = H.HostMatrix(M, K), H.HostMatrix(K, N), H.HostMatrix(M, N)
-    synthgen.fill(A.array, seed, "A", wl["dist"], row0=rank * M); synthgen.fill(B.array, seed, "B", wl["dist"])
-    synthgen.fill(C.array, seed, "C", wl["dist"], row0=rank * M)
-    dA, dB, dC = (torch.from_numpy(X.array).cuda() for X in (A, B, C))
-    torch.cuda.synchronize()      # the library's streams do not wait for PyTorch's: device operands must be complete
+    def barrier(self):
+        if self.dist:
+            self.dist.barrier()
+        self.torch.cuda.synchronize()
 
-    # ---- PyTorch owns device memory and streams; the library carves its buffers from this workspace
-    ws = torch.empty(budget, dtype=torch.uint8, device="cuda")
-    streams = [torch.cuda.Stream() for _ in range(10)]
-    ctx = H.hclooc_ctx_create(local, ws, ws.numel(), streams[0], streams[1], streams[2:])
+    def make_ctx(self, budget):
+        """PyTorch owns device memory and streams; the library carves its buffers from this workspace.  budget 0 = all free
+        HBM (less 2 GiB for the CUDA context and whatever else lives on the device)."""
+        torch = self.torch
+        if budget == 0:
+            torch.cuda.empty_cache()
+            free, _ = torch.cuda.mem_get_info()
+            budget = int(free) - 2 * GiB
+        ws = torch.empty(budget, dtype=torch.uint8, device="cuda")
+        streams = [torch.cuda.Stream() for _ in range(10)]
+        ctx = self.H.hclooc_ctx_create(self.local, ws, ws.numel(), streams[0], streams[1], streams[2:])
+        return ctx, ws, streams, budget
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+    def host_matrices(self, wl, seed):
+        H, sg = self.H, self.synthgen
+        M, N, K = wl["M"], wl["N"], wl["K"]
+        t0 = time.perf_counter()
+        A, B, C = H.HostMatrix(M, K), H.HostMatrix(K, N), H.HostMatrix(M, N)
+        t_pin = time.perf_counter() - t0
+        sg.fill(A.array, seed, "A", wl["dist"], row0=self.rank * M); sg.fill(B.array, seed, "B", wl["dist"])
+        sg.fill(C.array, seed, "C", wl["dist"], row0=self.rank * M)
+        return A, B, C, t_pin
 
-    def ci95_rel(xs):
-        """Half-width of the 95 % confidence interval of the mean over the mean (Student t; PAPER.md:362 asks
-        for 2.5 %)."""
-        n = len(xs)
-        if n < 2:
-            return None
-        t95 = {2: 12.71, 3: 4.303, 4: 3.182, 5: 2.776, 6: 2.571, 7: 2.447, 8: 2.365, 9: 2.306, 10: 2.262}.get(n, 2.0 if n > 30 else 2.2)
-        return float(t95 * np.std(xs, ddof=1) / np.sqrt(n) / np.mean(xs))
+    def call(self, ctx, wl, A, B, C, budget):
+        H, ta, tb = self.H, self.ta, self.tb
+        M, N, K = wl["M"], wl["N"], wl["K"]
+        if ta or tb:     # the M*K (K*N) doubles of A (B) read as the stored K x M (N x K) matrix
+            return H.hclooc_dgemm_t(ctx, ta, tb, M, N, K, wl["alpha"], A, M if ta else K, B, K if tb else N, wl["beta"], C, N, budget)
+        return H.hclooc_dgemm_ex(ctx, M, N, K, wl["alpha"], A, K, B, N, wl["beta"], C, N, budget)
 
-    per_call = []
-
-    def timed(fn, steps, warmup):
+    def timed(self, fn, steps, warmup):
+        """W untimed calls, then exactly K calls between barrier + synchronize: device time from CUDA events (max over
+        ranks), host wall time of the same region, and the per-call wall times the library reports (t_total_s)."""
+        torch = self.torch
         st = None
-        per_call.clear()
         for _ in range(warmup):
             st = fn()
-        barrier()
+        self.barrier()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        per_call = []
         e0.record()
+        t0 = time.perf_counter()
         for _ in range(steps):
             st = fn()
             per_call.append(st.t_total_s)
+        wall = time.perf_counter() - t0
         e1.record()
-        barrier()
+        self.barrier()
         ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        return ms / steps, (st, ci95_rel(list(per_call)), 1e3 * float(np.mean(per_call)), 1e3 * float(np.min(per_call)))
+        if self.dist:
+            t = torch.tensor([ms, wall * 1e3], device="cuda", dtype=torch.float64)
+            self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+            ms, wall = float(t[0].item()), float(t[1].item()) * 1e-3
+        return {"ms_events": ms / steps, "ms_wall": 1e3 * wall / steps, "stats": st, "ci95_rel": ci95_rel(per_call),
+                "call_ms_mean": 1e3 * float(np.mean(per_call)), "call_ms_min": 1e3 * float(np.min(per_call))}
 
-    def resident():
-        if ta or tb:
-            return H.hclooc_dgemm_t(ctx, ta, tb, M, N, K, alpha, dA, M if ta else K, dB, K if tb else N, beta, dC, N, budget)
-        return H.hclooc_dgemm_ex(ctx, M, N, K, alpha, dA, K, dB, N, beta, dC, N, budget)
+    def e2e_record(self, wl, r):
+        st = r["stats"]
+        flops = 2.0 * wl["M"] * wl["N"] * wl["K"]
+        t_roof, t_flop, t_link = link_roofline_s(flops, st.bytes_h2d, st.bytes_d2h)
+        return {"value": self.world * flops / (r["ms_wall"] * 1e-3) / 1e12, "unit": "TFLOP/s", "ms_per_step": r["ms_wall"],
+                "h2d_bytes_per_step": int(st.bytes_h2d), "d2h_bytes_per_step": int(st.bytes_d2h),
+                "roofline_s": t_roof, "t_flop_s": t_flop, "t_link_s": t_link, "bound": "link" if t_link > t_flop else "fp64",
+                "frac_of_roofline": t_roof / (r["ms_wall"] * 1e-3), "ci95_rel": r["ci95_rel"],
+                "call_ms_mean": r["call_ms_mean"], "call_ms_min": r["call_ms_min"],
+                "timer": "host clock around the K calls (each returns with C complete in host memory)"}
 
-    ta, tb = int(args.trans[0] == "T"), int(args.trans[1] == "T")
+    @staticmethod
+    def plan_summary(plan):
+        keys = ("mb", "nb", "kb", "h", "w", "kpanels", "n_steps", "n_sets", "n_abuf", "n_bbuf", "ksplit", "direct", "workspace_bytes")
+        return {k: getattr(plan, k) for k in keys}
 
-    def host():
-        if ta or tb:     # the M*K (K*N) doubles of A (B) read as the stored K x M (N x K) matrix
-            return H.hclooc_dgemm_t(ctx, ta, tb, M, N, K, alpha, A, M if ta else K, B, K if tb else N, beta, C, C.ld, budget)
-        return H.hclooc_dgemm_ex(ctx, M, N, K, alpha, A, A.ld, B, B.ld, beta, C, C.ld, budget)
+    def per_config(self, names):
+        """BASELINE configs cfg1..cfg4 end to end, one after the other (each pins, runs and frees its own matrices)."""
+        out = {}
+        steps_of = {"cfg1": 50, "cfg2": 10, "cfg3": 3, "cfg4": 3}
+        for name in names:
+            wl = WORKLOADS[name]
+            if wl_bytes(wl) + 8 * GiB > meminfo("MemAvailable"):
+                out[name] = {"skipped": "host memory"}
+                continue
+            ctx, ws, streams, budget = self.make_ctx(wl["budget"])
+            A, B, C, _ = self.host_matrices(wl, self.synthgen.BASE_SEED + wl["seed_idx"])
+            try:
+                r = self.timed(lambda: self.call(ctx, wl, A, B, C, budget), steps_of[name], 3)
+                rec = self.e2e_record(wl, r)
+                rec.update({"workload": f"{name}: {wl['desc']}", "steps": steps_of[name], "warmup": 3, "plan": self.plan_summary(r["stats"].plan)})
+                for k in ("roofline_s", "call_ms_mean", "call_ms_min", "timer", "unit"):
+                    rec.pop(k, None)
+                out[name] = rec
+            finally:
+                self.H.hclooc_ctx_destroy(ctx)
+                for X in (A, B, C):
+                    X.free()
+                del ws, streams
+                self.torch.cuda.empty_cache()
+        return out
 
-    if not args.kernel_only:
+    def kernel_legs(self, wl, plan, steps, warmup):
+        """The tile kernel timed alone on device-resident operands of the plan's step shape: one step as the pipeline launches
+        it (mb x nb x K, plan.ksplit CTAs per tile) and a GPU-filling launch (up to 16384 rows x nb x K: hclDgemmAsync picks the
+        persistent stream-K variant).  Operands: seeded uniform[-1,1) generated on the device (values do not matter here)."""
+        torch, H, ta, tb = self.torch, self.H, self.ta, self.tb
+        M, N, K = wl["M"], wl["N"], wl["K"]
+        if plan.direct:
+            mb, nb = M, N
+        else:
+            mb, nb = min(plan.mb, M), min(plan.nb, N)
+        rows = min(M, max(mb, 16384))
+        g = torch.Generator(device="cuda"); g.manual_seed(180805056)
+        dA = torch.rand((K, rows) if ta else (rows, K), generator=g, dtype=torch.float64, device="cuda") * 2 - 1
+        dB = torch.rand((nb, K) if tb else (K, nb), generator=g, dtype=torch.float64, device="cuda") * 2 - 1
+        dC = torch.rand((rows, nb), generator=g, dtype=torch.float64, device="cuda") * 2 - 1
+        torch.cuda.synchronize()
+        cur = torch.cuda.current_stream()
+        lda, ldb = (rows if ta else K), (K if tb else nb)
+
+        def time_launch(m, variant, n_iter):
+            ts = []
+            for it in range(warmup + n_iter):
+                k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                k0.record(cur)
+                H.hclDgemmAsyncT(ta, tb, m, nb, K, wl["alpha"], dA, lda, dB, ldb, wl["beta"], dC, nb, cur, variant=variant)
+                k1.record(cur)
+                k1.synchronize()
+                if it >= warmup:
+                    ts.append(k0.elapsed_time(k1))
+            return float(np.mean(ts))
+
+        ks = max(1, plan.ksplit)
+        clustered = bool(plan.direct and plan.direct_cm * plan.direct_cn > 1)
+        if clustered:      # direct mode: the multicast cluster kernel (here on HBM operands; in the call it reads host memory)
+            ks = 100 + 10 * plan.direct_cm + plan.direct_cn
+        ms_step = time_launch(mb, ks, max(steps, 10))
+        ks = 1 if clustered else ks
+        ms_full = time_launch(rows, 0, max(steps, 5))
+        step_ctas = min(148, -(-mb // 128) * -(-nb // 128) * ks)
+        step_peak = FP64_PEAK_TFLOPS * step_ctas / 148.0
+        tiles_full = -(-rows // 128) * -(-nb // 128)
+        solo = {"kernel": f"hclooc_dgemm_direct_kernel<{plan.direct_cm},{plan.direct_cn}>" if clustered else f"hclooc_dgemm_tile_kernel<{ks}>", "launch": f"{mb}x{nb}x{K}", "ctas": step_ctas, "ms_per_launch": ms_step,
+                "achieved": 2.0 * mb * nb * K / (ms_step * 1e-3) / 1e12, "peak": step_peak,
+                "note": "one step's launch timed ALONE; peak = 37.2 TFLOP/s x min(CTAs, 148)/148 (in the pipeline other steps' kernels run beside it and fill its wave tail)"}
+        solo["frac"] = solo["achieved"] / step_peak
+        full = {"kernel": "hclooc_dgemm_streamk_kernel" if tiles_full >= 148 else "hclooc_dgemm_tile_kernel", "launch": f"{rows}x{nb}x{K}",
+                "ms_per_launch": ms_full, "achieved": 2.0 * rows * nb * K / (ms_full * 1e-3) / 1e12, "peak": FP64_PEAK_TFLOPS}
+        full["frac"] = full["achieved"] / FP64_PEAK_TFLOPS
+        del dA, dB, dC
+        return solo, full, 2 * (warmup + max(steps, 10)) - (max(steps, 10) - max(steps, 5))
+
+    def traced_call(self, ctx, fn):
+        """One more call with the library's tracing on: every kernel bracketed by timing events on ITS compute stream.  Returns
+        (flops of all launches, union of their [start, end] intervals in ms, launches, mean single-launch duration in ms)."""
+        H = self.H
+        H.hclooc_ctx_set_trace(ctx, True)
+        try:
+            fn()
+            recs = H.hclooc_ctx_get_trace(ctx)
+        finally:
+            H.hclooc_ctx_set_trace(ctx, False)
+        g = recs[recs["kind"] == 3]
+        if not len(g):
+            return None
+        order = np.argsort(g["t_start_ms"])
+        s, e = g["t_start_ms"][order], g["t_end_ms"][order]
+        union, cur_s, cur_e = 0.0, s[0], e[0]
+        for a, b in zip(s[1:], e[1:]):
+            if a > cur_e:
+                union += cur_e - cur_s
+                cur_s, cur_e = a, b
+            else:
+                cur_e = max(cur_e, b)
+        union += cur_e - cur_s
+        return float(g["flops"].sum()), float(union), int(len(g)), float(np.mean(e - s))
+
+    def run(self):
+        args, H, torch = self.args, self.H, self.torch
+        name, wl = pick_workload(args.workload, self.share)
+        M, N, K = wl["M"], wl["N"], wl["K"]
+        seed = self.synthgen.BASE_SEED + wl["seed_idx"]
+        flops = 2.0 * M * N * K
+        # N > 1: ONE problem of world*M rows cut into row bands of C (hclooc_shard_rows): rank r owns rows r*M .. of A
+        # and C, every rank holds all of B; the bands are independent (PAPER.md:289, :293), so no collective is on
+        # the data path and per-GPU work is fixed as N grows (weak scaling).
+        row0, rows = H.hclooc_shard_rows(self.world * M, self.world, self.rank, 128)
+        assert (row0, rows) == (self.rank * M, M) or M % 128
+        heavy = flops / 36e12 > 1.0
+        steps = args.steps if args.steps else (3 if heavy else 10)
+        warmup = max(args.warmup, 3)
+
         live = measure_link(H)
         if live:
             LINK.update(live)
-    with ClockSampler(local) as clk:
-        if args.kernel_only:
-            plan = H.hclooc_plan(M, N, K, beta != 0.0, 0, budget)
-        else:
-            ms_res, (st_res, ci_res, _, _) = timed(resident, args.steps, max(args.warmup, 3))
-            ms_e2e, (st_e2e, ci_e2e, call_mean_ms, call_min_ms) = timed(host, args.steps, max(args.warmup, 3))
-            plan = st_e2e.plan
-        # ---- roofline leg: the tile kernel alone, one GPU-filling launch of the plan's B-slice shape
-        nb = min(plan.nb, N)
-        cur = torch.cuda.current_stream()
-        kt = []
-        for it in range(max(args.warmup, 3) + args.steps):
-            k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            k0.record(cur)
-            if ta or tb:
-                H.hclDgemmAsyncT(ta, tb, M, nb, K, alpha, dA, M if ta else K, dB, K if tb else N, beta, dC, N, cur)
-            else:
-                H.hclDgemmAsync(M, nb, K, alpha, dA, K, dB, N, beta, dC, N, cur)
-            k1.record(cur)
-            k1.synchronize()
-            if it >= max(args.warmup, 3):
-                kt.append(k0.elapsed_time(k1))
-        # ---- one pipeline step, launched as the executor launches it (it need not fill the GPU: steps overlap)
-        mb = min(plan.mb, M)
-        stt = []
-        for it in range(max(args.warmup, 3) + max(args.steps, 10)):
-            k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            k0.record(cur)
-            H.hclDgemmAsyncT(ta, tb, mb, nb, K, alpha, dA, M if ta else K, dB, K if tb else N, beta, dC, N, cur, variant=max(1, plan.ksplit))
-            k1.record(cur)
-            k1.synchronize()
-            if it >= max(args.warmup, 3):
-                stt.append(k0.elapsed_time(k1))
-        clocks = clk.summary()
-    ms_step = float(np.mean(stt))
-    step_ctas = min(148, -(-mb // 128) * -(-nb // 128) * max(1, plan.ksplit))
-    step_achieved = 2.0 * mb * nb * K / (ms_step * 1e-3) / 1e12
-    step_peak = FP64_PEAK_TFLOPS * step_ctas / 148.0
-    ms_kernel = float(np.mean(kt))
-    kflops = 2.0 * M * nb * K
-    achieved = kflops / (ms_kernel * 1e-3) / 1e12
-    if args.kernel_only:
-        if rank == 0:
-            print(json.dumps({"kernel_only": True, "launch": f"{M}x{nb}x{K}", "ms_per_launch": ms_kernel, "achieved_tflops": achieved,
-                              "frac": achieved / FP64_PEAK_TFLOPS, "clocks": clocks}))
-        H.hclooc_ctx_destroy(ctx)
-        return
+        peak_measured = H.hclooc_probe_fp64(0, 4, 1.0)
+        per_config = None
+        if self.world == 1 and not args.no_per_config and args.workload == "auto":
+            per_config = self.per_config([c for c in ("cfg1", "cfg2", "cfg3", "cfg4") if c != name])
 
-    t_roof, t_flop, t_link = link_roofline_s(flops, st_e2e.bytes_h2d, st_e2e.bytes_d2h)
-    out = {
-        "metric": "end-to-end out-of-core DGEMM TFLOP/s (host-resident A,B,C) and % of roofline",
-        "value": world * flops / (ms_res * 1e-3) / 1e12, "unit": "TFLOP/s", "n_gpus": world, "steps": args.steps,
-        "warmup": max(args.warmup, 3), "ms_per_step": ms_res, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f64", "data": "synthetic", "ci95_rel": ci_res,
-        "config": {"workload": f"{name}: {wl['desc']}", "M": M, "N": N, "K": K, "alpha": alpha, "beta": beta,
-                   "device_budget_bytes": budget, "dist": wl["dist"], "trans": args.trans, "parallelism": (f"{world} row bands of C of {M} rows each, one per GPU (hclooc_shard_rows), B on every rank, no collective"
-                                   if world > 1 else "1 GPU"), "M_global": world * M,
-                   "plan": {k: getattr(plan, k) for k in ("mb", "nb", "kb", "h", "w", "kpanels", "n_steps", "n_sets", "n_bbuf", "workspace_bytes")},
-                   "l2": "inputs (A+B+C = %.2f GB) exceed the 126 MB L2; no flush needed" % ((M * K + K * N + M * N) * 8 / 1e9),
-                   "value_leg": "A,B,C resident in HBM: in-core case, one tile-kernel launch over the whole problem, nothing staged"},
-        "e2e": {"value": world * flops / (ms_e2e * 1e-3) / 1e12, "unit": "TFLOP/s", "ms_per_step": ms_e2e,
-                "h2d_bytes_per_step": int(st_e2e.bytes_h2d), "d2h_bytes_per_step": int(st_e2e.bytes_d2h),
-                "roofline_s": t_roof, "t_flop_s": t_flop, "t_link_s": t_link, "bound": "link" if t_link > t_flop else "fp64",
-                "frac_of_roofline": t_roof / (ms_e2e * 1e-3), "link_peaks": LINK, "ci95_rel": ci_e2e,
-                "call_ms_mean": call_mean_ms, "call_ms_min": call_min_ms},
-        "gpu_launches": int((st_res.n_kernels + st_e2e.n_kernels) * args.steps + len(kt) + len(stt)),
-        "clocks": clocks,
-        "roofline": {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                     "frac": achieved / FP64_PEAK_TFLOPS, "traffic": ncu_traffic(f"{M}x{nb}x{K}"),
-                     "kernel": "hclooc_dgemm_streamk_kernel" if -(-M // 128) * -(-nb // 128) >= 148 else "hclooc_dgemm_tile_kernel",
-                     "launch": f"{M}x{nb}x{K} (one B slice of the plan, all rows)", "ms_per_launch": ms_kernel,
-                     "peak_source": "derived 148 SM x 128 FP64 flop/clk x 1.965 GHz; DMMA microbenchmark measured 37.17",
-                     "pipeline_step": {"kernel": f"hclooc_dgemm_tile_kernel<{max(1, plan.ksplit)}>", "launch": f"{mb}x{nb}x{K}",
-                                       "ctas": step_ctas, "ms_per_launch": ms_step, "achieved": step_achieved,
-                                       "peak": step_peak, "frac": step_achieved / step_peak,
-                                       "note": "peak = 37.2 TFLOP/s x CTAs/148: a step occupies only its own CTAs, other steps run beside it"}},
-    }
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        rows = min(M, args.cpu_rows if args.cpu_rows > 0 else max(128, int(1.0e12 / (2.0 * N * K)) // 128 * 128))
-        cflops, times = time_oracle(wl, rows, seed, 1, 0)
-        out["cpu_baseline"] = {"value": cflops / times[0] / 1e12, "unit": "TFLOP/s", "cores": os.cpu_count(), "kind": "oracle",
-                               "sample": f"first {rows} rows of C (all {N} columns, K={K}), {times[0]:.1f} s of oracle.dgemm"}
-    H.hclooc_ctx_destroy(ctx)
-    if world > 1:
-        dist.destroy_process_group()
-    if rank == 0:
-        print(json.dumps(out))
+        # ---- the headline workload: pinned host matrices, then the context over (nearly) all that is left of the device
+        in_core = None
+        if not args.no_in_core:
+            in_core = self.in_core_leg(wl, warmup)
+        plan0 = H.hclooc_plan_trans(M, N, K, wl["beta"] != 0.0, 0, wl["budget"] or (int(torch.cuda.mem_get_info()[0]) - 4 * GiB), 0, self.ta, self.tb)
+        solo, full, n_leg_launches = self.kernel_legs(wl, plan0, steps, warmup)
+        torch.cuda.empty_cache()
+        A, B, C, t_pin = self.host_matrices(wl, seed)
+        ctx, ws, streams, budget = self.make_ctx(wl["budget"])
+        fn = lambda: self.call(ctx, wl, A, B, C, budget)
+        with ClockSampler(self.local) as clk:
+            r = self.timed(fn, steps, warmup)
+            clocks = clk.summary()
+        st = r["stats"]
+        plan = st.plan
+        tr = self.traced_call(ctx, fn)
+        ks = max(1, plan.ksplit)
+        kname = (f"hclooc_dgemm_direct_kernel<{plan.direct_cm},{plan.direct_cn}>" if plan.direct and plan.direct_cm * plan.direct_cn > 1
+                 else f"hclooc_dgemm_tile_kernel<{ks}>")
+        launch = f"{min(plan.mb, M)}x{min(plan.nb, N)}x{min(plan.kb, K)}"
+        traffic, traffic_src = ncu_traffic(kname, launch)
+        roof = {"bound": "alu", "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "kernel": kname, "launch": launch,
+                "peak_source": "derived: 148 SM x 128 FP64 flop/clk (DMMA.8x8x4) x 1.965 GHz; peak_measured = hclooc_probe_fp64 (DMMA register chains) run live",
+                "peak_measured": peak_measured, "traffic": traffic, "traffic_source": traffic_src,
+                "solo_step": solo, "streamk": full}
+        if tr:
+            fl, union_ms, n_launch, mean_ms = tr
+            roof.update({"achieved": fl / (union_ms * 1e-3) / 1e12, "launches_per_step": n_launch, "ms_kernels_busy": union_ms,
+                         "ms_per_launch": union_ms / n_launch, "ms_per_launch_solo_span": mean_ms,
+                         "how": "one traced call (timing events around every kernel on its own compute stream): flops of all launches / time during "
+                                "which at least one was running; several steps' kernels overlap on up to 8 streams, so the per-launch figure is that time / launches"})
+        else:   # direct mode: one launch, the call IS the kernel
+            roof.update({"achieved": solo["achieved"], "ms_per_launch": solo["ms_per_launch"], "how": "the call is one launch; see solo_step"})
+        roof["frac"] = roof["achieved"] / FP64_PEAK_TFLOPS
+        e2e = self.e2e_record(wl, r)
+        e2e["link_peaks"] = LINK
+        out = {
+            "metric": METRIC,
+            "value": self.world * flops / (r["ms_events"] * 1e-3) / 1e12, "unit": "TFLOP/s", "n_gpus": self.world, "steps": steps,
+            "warmup": warmup, "ms_per_step": r["ms_events"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "ci95_rel": r["ci95_rel"],
+            "config": {"workload": f"{name}: {wl['desc']}", "M": M, "N": N, "K": K, "alpha": wl["alpha"], "beta": wl["beta"],
+                       "device_budget_bytes": budget, "dist": wl["dist"], "trans": args.trans,
+                       "parallelism": (f"{self.world} row bands of C of {M} rows each, one per GPU (hclooc_shard_rows), B on every rank, no collective"
+                                       if self.world > 1 else "1 GPU"), "M_global": self.world * M,
+                       "matrices_bytes": wl_bytes(wl), "hbm_total_bytes": int(torch.cuda.get_device_properties(self.local).total_memory),
+                       "exceeds_hbm": wl_bytes(wl) > int(torch.cuda.get_device_properties(self.local).total_memory),
+                       "host_mem_total_bytes": meminfo("MemTotal"), "t_pin_s": t_pin,
+                       "plan": self.plan_summary(plan),
+                       "l2": "inputs (A+B+C = %.2f GB) are host-resident and exceed the 126 MB L2; no flush needed" % (wl_bytes(wl) / 1e9),
+                       "value_leg": "CUDA events around the K host-resident calls (the pipeline: uploads, kernels, downloads); the in-core kernel rate is under in_core"},
+            "e2e": e2e,
+            "gpu_launches": int(st.n_kernels * steps),
+            "gpu_launches_outside_timed_region": {"traced_call": int(st.n_kernels), "kernel_legs": n_leg_launches},
+            "clocks": clocks,
+            "roofline": roof,
+        }
+        if in_core:
+            out["in_core"] = in_core
+        if per_config is not None:
+            out["per_config"] = per_config
+        if self.rank == 0 and self.world == 1 and not args.no_cpu_baseline:
+            crows, ccols = oracle_sample_shape(wl, args.cpu_flops, 512)
+            cflops, times = time_oracle(wl, crows, ccols, seed, 1, 0, mats=(A.view, B.view, C.view))
+            out["cpu_baseline"] = {"value": cflops / times[0] / 1e12, "unit": "TFLOP/s", "cores": os.cpu_count(), "kind": "oracle",
+                                   "sample": f"first {crows} rows x first {ccols} columns of C (K={K}), {times[0]:.1f} s of oracle.dgemm"}
+        H.hclooc_ctx_destroy(ctx)
+        for X in (A, B, C):
+            X.free()
+        if self.dist:
+            self.dist.destroy_process_group()
+        if self.rank == 0:
+            print(json.dumps(out))
+
+    def in_core_leg(self, wl, warmup):
+        """The in-core case of the library: all three operands device-resident, one launch, nothing staged
+        -- on the workload itself when it fits a quarter of the device, else on its first 16384 rows and columns."""
+        torch, H = self.torch, self.H
+        free = int(torch.cuda.mem_get_info()[0])
+        m, n, k = wl["M"], wl["N"], wl["K"]
+        if wl_bytes(wl) > free // 4:
+            m, n = min(m, 16384), min(n, 16384)
+        g = torch.Generator(device="cuda"); g.manual_seed(180805057)
+        ta, tb = self.ta, self.tb
+        dA = torch.rand((k, m) if ta else (m, k), generator=g, dtype=torch.float64, device="cuda") * 2 - 1
+        dB = torch.rand((n, k) if tb else (k, n), generator=g, dtype=torch.float64, device="cuda") * 2 - 1
+        dC = torch.rand((m, n), generator=g, dtype=torch.float64, device="cuda") * 2 - 1
+        torch.cuda.synchronize()
+        ctx = H.hclooc_ctx_create(self.local)
+        sub = dict(wl, M=m, N=n, K=k)
+        try:
+            r = self.timed(lambda: self.call(ctx, sub, dA, dB, dC, 256 * MiB), 10, warmup)
+        finally:
+            H.hclooc_ctx_destroy(ctx)
+        fl = 2.0 * m * n * k
+        val = fl / (r["ms_events"] * 1e-3) / 1e12
+        del dA, dB, dC
+        torch.cuda.empty_cache()
+        return {"value": val, "unit": "TFLOP/s", "ms_per_step": r["ms_events"], "shape": f"{m}x{n}x{k}", "frac_of_fp64_peak": val / FP64_PEAK_TFLOPS,
+                "note": "A, B, C resident in HBM: one stream-K launch on the caller's matrices, nothing staged (kernel-only rate; not the metric)"}
+
+    def kernel_only(self):
+        """Only the kernel legs (for ncu captures of the tile kernel at the workload's step shape)."""
+        name, wl = pick_workload(self.args.workload, self.share)
+        budget = wl["budget"] or (int(self.torch.cuda.mem_get_info()[0]) - 4 * GiB)
+        plan = self.H.hclooc_plan_trans(wl["M"], wl["N"], wl["K"], wl["beta"] != 0.0, 0, budget, 0, self.ta, self.tb)
+        with ClockSampler(self.local) as clk:
+            solo, full, _ = self.kernel_legs(wl, plan, self.args.steps or 3, max(self.args.warmup, 1))
+            clocks = clk.summary()
+        if self.rank == 0:
+            print(json.dumps({"kernel_only": True, "workload": name, "solo_step": solo, "streamk": full, "clocks": clocks}))
 
 
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=0, help="timed calls (0 = 3 for workloads of more than a second per call, else 10)")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=sorted(WORKLOADS))
+    ap.add_argument("--workload", default="auto", choices=["auto", "cfg5s"] + sorted(WORKLOADS))
     ap.add_argument("--ref-rows", type=int, default=512, help="rows of C per oracle step (reference arm)")
-    ap.add_argument("--cpu-rows", type=int, default=0, help="rows of C in the cpu_baseline sample (0 = about 1e12 flop, 10-30 s)")
+    ap.add_argument("--ref-flops", type=float, default=1.5e11, help="flops per oracle step (reference arm): about 2 s on 16 cores")
+    ap.add_argument("--cpu-flops", type=float, default=1.0e12, help="flops of the cpu_baseline sample: 10-30 s of the oracle")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the cfg1-cfg4 block of the default (auto) run")
+    ap.add_argument("--no-in-core", action="store_true")
     ap.add_argument("--trans", default="NN", choices=["NN", "TN", "NT", "TT"],
                     help="e2e leg through hclooc_dgemm_t with op(A), op(B) transposed (the same buffers read as the stored K x M / N x K matrices)")
-    ap.add_argument("--kernel-only", action="store_true", help="only the roofline leg (for ncu captures of the tile kernel)")
+    ap.add_argument("--kernel-only", action="store_true", help="only the kernel legs (for ncu captures of the tile kernel)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
-    wl, name = WORKLOADS[args.workload], args.workload
     if args.impl == "reference":
-        return run_reference(args, wl, name)
-    run_ours(args, wl, name)
+        return run_reference(args)
+    b = Bench(args)
+    if args.kernel_only:
+        return b.kernel_only()
+    b.run()
 
 
 if __name__ == "__main__":

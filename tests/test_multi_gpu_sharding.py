@@ -97,3 +97,41 @@ def test_two_ranks_over_gloo_reproduce_the_whole_problem():
         assert p.exitcode == 0
     assert res[0] == "ok", res
     assert res[1] is True and res[2] == (M, N) and sum(res[3]) == M and res[3] == [160, 141]
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("M,world,dist", [(1000, 3, "uniform"), (1000, 3, "int"), (777, 2, "uniform"), (130, 4, "int")])
+def test_bands_through_the_cuda_path_equal_the_single_call_bitwise(M, world, dist):
+    """What bench.py's ranks do, on one GPU: the M rows (ragged, align 128) are cut into `world` bands with hclooc_shard_rows and
+    hclooc_dgemm runs on each band's POINTERS into the same host matrices (rows row0.. of A and C, all of B).  The stacked
+    bands must equal the single call bit for bit (K is not split, so every element sums in the same order whatever the banding)
+    and the oracle within the gate (exactly on integers).  Trailing ranks with no rows do nothing."""
+    import oracle
+    import synthgen
+    N, K, alpha, beta, budget = 390, 300, 1.5, -0.5, 2 << 20
+    A, B, C = H.HostMatrix(M, K, K + 2), H.HostMatrix(K, N, N + 4), H.HostMatrix(M, N, N + 6)
+    for X in (A, B, C):
+        X.array[...] = np.nan
+    synthgen.fill(A.array, 51, "A", dist, cols=K); synthgen.fill(B.array, 51, "B", dist, cols=N); synthgen.fill(C.array, 51, "C", dist, cols=N)
+    C0 = C.view.copy()
+    ref = C0.copy()
+    D = oracle.dgemm(alpha, A.view, B.view, beta, ref, want_denominator=True)
+    st = H.hclooc_dgemm_ex(None, M, N, K, alpha, A, A.ld, B, B.ld, beta, C, C.ld, budget)
+    assert st.plan.kpanels == 1
+    whole = C.view.copy()
+    C.view[...] = C0
+    covered = 0
+    for rank in range(world):
+        row0, rows = H.hclooc_shard_rows(M, world, rank, 128)
+        assert row0 == covered
+        covered += rows
+        st = H.hclooc_dgemm_ex(None, rows, N, K, alpha, A.ptr + 8 * row0 * A.ld, A.ld, B, B.ld, beta, C.ptr + 8 * row0 * C.ld, C.ld, budget)
+        assert st.bytes_d2h == rows * N * 8
+    assert covered == M
+    assert np.array_equal(C.view.view(np.uint64), whole.view(np.uint64))
+    assert np.isnan(C.array[:, N:]).all()
+    if dist == "int":
+        assert np.array_equal(C.view, ref)
+    else:
+        ok, worst = oracle.within_gate(C.view, ref, D, 1e-13)
+        assert ok, worst

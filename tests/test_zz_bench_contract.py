@@ -22,6 +22,26 @@ def run_bench(*args):
     return json.loads(lines[0])
 
 
+def test_both_arms_print_the_same_metric_and_pick_the_same_workload():
+    """The driver divides the two arms' values only when metric and workload agree: one METRIC string serves both, and the
+    default (`auto`) workload is a function of the host's MemTotal alone -- the largest configuration it can pin."""
+    sys.path.insert(0, ROOT)
+    import bench
+    name, wl = bench.pick_workload("auto")
+    assert (name, wl) == bench.pick_workload("auto")
+    total = bench.wl_bytes(wl)
+    assert total <= bench.meminfo("MemTotal") - 14 * (1 << 30) or name == "cfg1"
+    if name == "cfg5s":
+        assert wl["M"] == wl["N"] and wl["M"] % 2048 == 0 and 65536 < wl["M"] <= 163840 and wl["K"] == 8192 and wl["budget"] == 0
+    # per rank under torchrun: a smaller share of the host
+    n8, w8 = bench.pick_workload("auto", 8)
+    assert bench.wl_bytes(w8) <= bench.meminfo("MemTotal") // 8 or n8 == "cfg1"
+    d = run_bench("--impl", "reference", "--workload", "cfg1", "--steps", "1", "--warmup", "0")
+    assert d["metric"] == bench.METRIC and d["config"]["workload"].startswith("cfg1: ")
+    rows, cols = bench.oracle_sample_shape(bench.cfg5_scaled(), 1.5e11)
+    assert rows == 512 and cols % 128 == 0 and 1.0e11 < 2.0 * rows * cols * 8192 <= 1.5e11
+
+
 def test_reference_arm_times_the_oracle_on_the_host_cores():
     """`--impl reference`: the oracle, as it stands, on a bounded sample of the same workload (no GPU needed)."""
     d = run_bench("--impl", "reference", "--workload", "cfg1", "--steps", "2", "--warmup", "1", "--ref-rows", "256")
@@ -34,7 +54,7 @@ def test_reference_arm_times_the_oracle_on_the_host_cores():
 
 @pytest.mark.gpu
 def test_our_arm_carries_roofline_e2e_clocks_and_launch_count():
-    d = run_bench("--workload", "cfg1", "--steps", "5", "--warmup", "3", "--cpu-rows", "256")
+    d = run_bench("--workload", "cfg1", "--steps", "5", "--warmup", "3", "--cpu-flops", "1e8")
     assert BASE_KEYS | {"roofline", "cpu_baseline", "clocks"} <= set(d) and "impl" not in d
     assert d["n_gpus"] == 1 and d["steps"] == 5 and d["warmup"] >= 3 and d["higher_is_better"] is True and d["scaling"] == "weak"
     assert d["dtype"] == "f64" and d["data"] == "synthetic" and d["vs_baseline"] is None and d["gpu_launches"] > 0
@@ -43,7 +63,8 @@ def test_our_arm_carries_roofline_e2e_clocks_and_launch_count():
     assert 0 < e["frac_of_roofline"] <= 1.0 and e["bound"] in ("link", "fp64") and e["link_peaks"]["h2d_GBps"] > 10
     r = d["roofline"]
     assert r["bound"] == "alu" and r["unit"] == "TFLOP/s" and r["peak"] == 37.2 and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
-    assert "traffic" in r and 0 < r["frac"] <= 1.0
+    assert "traffic" in r and 0 < r["frac"] <= 1.0 and 30.0 < r["peak_measured"] < 40.0 and "solo_step" in r and "streamk" in r
+    assert abs(d["value"] - e["value"]) < 0.05 * e["value"] and d["in_core"]["value"] > 0
     c = d["cpu_baseline"]
     assert c["kind"] == "oracle" and c["value"] > 0 and c["cores"] >= 1 and "sample" in c
     assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"} and not set(d["clocks"]["reasons"]) & {"hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"}
