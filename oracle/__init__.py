@@ -10,7 +10,8 @@ bound, numpy cross-check, the paper's 44-element partition example; dsyrk: brute
 exact symmetry, int64 exactness, untouched other triangle; dtrsm: scipy's solve_triangular, exact rational
 arithmetic on tiny cases, identity / diagonal / all-ones closed forms, int64 exactness, transposed-storage identity; the D returned
 by dsyrk / dsyr2k against numpy's |A||B|^T products; dtrsm_gate against gamma_(M+2) in exact arithmetic; oracle/checksum.py
-against the full oracle, int64 arithmetic and single-element mutations) -- nothing here is "parity unpinned".
+against the full oracle, int64 arithmetic and single-element mutations; dtrsm_right / dtrmm / dsymm / dpotrf (level3_oracle.c) in
+tests/test_oracle_level3.py) -- nothing here is "parity unpinned".
 """
 from __future__ import annotations
 
@@ -22,6 +23,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "dgemm_oracle.c")
+_SRC3 = os.path.join(_HERE, "level3_oracle.c")          # DTRSM (right), DTRMM, DPOTRF: the routines PAPER.md:412 names
 _LIB = os.path.join(_HERE, "liboracle.so")
 
 # the gate of BASELINE.json north_star as read in DESIGN.md (G14): |C - C_ref| <= RTOL * D
@@ -30,9 +32,9 @@ RTOL = 1e-13
 
 def build(force: bool = False) -> str:
     """Compile liboracle.so if missing or stale.  Never -ffast-math, never contraction."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC3)):
         subprocess.check_call(["gcc", "-O2", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
-                               "-o", _LIB, _SRC, "-lm"])
+                               "-o", _LIB, _SRC, _SRC3, "-lm"])
     return _LIB
 
 
@@ -58,6 +60,14 @@ def _load():
         lib.oracle_dtrsm_residual.restype = ctypes.c_int
         lib.oracle_dtrsm_residual.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, _i64, _i64, _dbl, _ptr, _i64, _ptr, _i64,
                                               _ptr, _i64, _i64, _ptr, _i64, _ptr, _ptr, _ptr]
+        lib.oracle_dtrsm_right.restype = ctypes.c_int
+        lib.oracle_dtrsm_right.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, _i64, _i64, _dbl, _ptr, _i64, _ptr, _i64]
+        lib.oracle_dtrmm.restype = ctypes.c_int
+        lib.oracle_dtrmm.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, _i64, _i64, _dbl, _ptr, _i64, _ptr, _i64]
+        lib.oracle_dpotrf.restype = ctypes.c_int
+        lib.oracle_dpotrf.argtypes = [ctypes.c_int, _i64, _ptr, _i64, ctypes.POINTER(_i64)]
+        lib.oracle_dpotrf_residual.restype = ctypes.c_int
+        lib.oracle_dpotrf_residual.argtypes = [ctypes.c_int, _i64, _ptr, _i64, _ptr, _i64, _i64, _ptr, _i64, _ptr, _ptr, _ptr]
         _lib = lib
     return _lib
 
@@ -207,6 +217,84 @@ def dtrsm_residual(uplo, trans, unit, alpha, A, B0, X, rows=None, cols=None):
                                        res.ctypes.data, den.ctypes.data)
     if rc != 0:
         raise ValueError("oracle_dtrsm_residual: bad argument")
+    return res, den
+
+
+def dtrsm_right(uplo, trans, unit, alpha, A, B):
+    """Solve X op(T) = alpha B by substitution along each row (oracle_dtrsm_right: the definition), X overwrites B (M x N);
+    T = the `uplo` (0 lower, 1 upper) triangle of the N x N row-major A."""
+    M, N = B.shape
+    assert A.shape == (N, N) or alpha == 0.0
+    ap, lda = _chk2d(A, "A") if A is not None and A.size else (0, max(N, 1))
+    bp, ldb = _chk2d(B, "B") if B.size else (0, max(N, 1))
+    rc = _load().oracle_dtrsm_right(int(uplo), int(trans), int(unit), M, N, float(alpha), ap, lda, bp, ldb)
+    if rc != 0:
+        raise ValueError("oracle_dtrsm_right: bad argument")
+
+
+def dtrmm(side, uplo, trans, unit, alpha, A, B):
+    """B <- alpha op(T) B (side = 0) or alpha B op(T) (side = 1), in place (oracle_dtrmm: the definition from the original B)."""
+    M, N = B.shape
+    n = M if side == 0 else N
+    assert A.shape == (n, n) or alpha == 0.0
+    ap, lda = _chk2d(A, "A") if A is not None and A.size else (0, max(n, 1))
+    bp, ldb = _chk2d(B, "B") if B.size else (0, max(N, 1))
+    rc = _load().oracle_dtrmm(int(side), int(uplo), int(trans), int(unit), M, N, float(alpha), ap, lda, bp, ldb)
+    if rc != 0:
+        raise ValueError(f"oracle_dtrmm failed: {rc}")
+
+
+def dsymm(side, uplo, alpha, A, B, beta, C, want_denominator=False):
+    """The DSYMM definition, in place:  C <- alpha*S*B + beta*C (side = 0, S is M x M) or alpha*B*S + beta*C (side = 1, S is
+    N x N), where S is the symmetric matrix whose `uplo` triangle is stored in A (the other triangle of A is never read).
+    It IS the DGEMM definition on the written-out symmetric matrix (mirroring the triangle is a copy, no arithmetic), so the step
+    is `dgemm` above: sums over k in increasing order, s_ik taken from the triangle at (max, min) or (min, max)."""
+    n = A.shape[0]
+    tri = np.tril(A) if uplo == 0 else np.triu(A)
+    other = np.tril(A, -1).T if uplo == 0 else np.triu(A, 1).T
+    S = np.empty((n, n))
+    S[...] = tri
+    mask = np.triu(np.ones((n, n), dtype=bool), 1) if uplo == 0 else np.tril(np.ones((n, n), dtype=bool), -1)
+    S[mask] = other[mask]
+    Bc = np.ascontiguousarray(B)
+    return dgemm(alpha, S, Bc, beta, C, want_denominator) if side == 0 else dgemm(alpha, Bc, S, beta, C, want_denominator)
+
+
+def dpotrf(uplo, A):
+    """Cholesky-Banachiewicz on the `uplo` triangle of the square row-major A, in place (oracle_dpotrf: the definition).
+    Returns LAPACK's info: 0, or i+1 when the leading minor of order i+1 is not positive definite (the routine stops there)."""
+    N = A.shape[0]
+    assert A.shape == (N, N)
+    ap, lda = _chk2d(A, "A") if A.size else (0, 1)
+    info = _i64(0)
+    rc = _load().oracle_dpotrf(int(uplo), N, ap, lda, ctypes.byref(info))
+    if rc != 0:
+        raise ValueError("oracle_dpotrf: bad argument")
+    return int(info.value)
+
+
+# gate for a Cholesky factorization of order N (DESIGN.md reading G24): the computed factor of ANY summation order satisfies
+# |A - L L^T| <= gamma_(N+1) |L||L^T| elementwise (Higham thm 10.3); the CUDA path multiplies by a rounded reciprocal of l_jj
+# instead of dividing (one more rounding per element), so the gate is gamma_(N+2) -- this function returns gamma_(N+2).
+def dpotrf_gate(N: int) -> float:
+    u = 2.0 ** -53
+    return (N + 2) * u / (1.0 - (N + 2) * u)
+
+
+def dpotrf_residual(uplo, A0, F, rows=None, cols=None):
+    """(res, den) of oracle_dpotrf_residual on the sampled rows x cols (None: all): |a_ij - sum_k f_ik f_jk| and
+    sum_k |f_ik||f_jk| in long double, A0 = the original matrix (its `uplo` triangle), F = the candidate factor."""
+    N = A0.shape[0]
+    ap, lda = _chk2d(A0, "A0")
+    fp, ldf = _chk2d(F, "F")
+    r = None if rows is None else np.ascontiguousarray(rows, dtype=np.int64)
+    c = None if cols is None else np.ascontiguousarray(cols, dtype=np.int64)
+    nr, nc = (N if r is None else r.size), (N if c is None else c.size)
+    res, den = np.empty((nr, nc)), np.empty((nr, nc))
+    rc = _load().oracle_dpotrf_residual(int(uplo), N, ap, lda, fp, ldf, nr, 0 if r is None else r.ctypes.data,
+                                        nc, 0 if c is None else c.ctypes.data, res.ctypes.data, den.ctypes.data)
+    if rc != 0:
+        raise ValueError("oracle_dpotrf_residual: bad argument")
     return res, den
 
 
