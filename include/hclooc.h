@@ -11,7 +11,9 @@
  * and runs a hand-written sm_100a FP64 tile kernel per step (the "in-core DGEMM" of :308).
  *
  * Conventions for every function
- *   - Storage is ROW-MAJOR, no transposes; leading dimensions are in ELEMENTS (doubles).
+ *   - Storage is ROW-MAJOR; leading dimensions are in ELEMENTS (doubles).  hclooc_dgemm is the paper's untransposed
+ *     operation (:180); transposed operands and the other level-3 routines the paper names as future work (:412) have their
+ *     own entry points below (hclooc_dgemm_t, hclooc_dsyrk, hclooc_dsyr2k, hclooc_dtrsm[_side], hclooc_dpotrf).
  *   - All functions return an int status: 0 = success; a NEGATIVE value -k means the k-th argument
  *     (1-based, in the order of the C prototype) is invalid (LAPACK "info" convention); POSITIVE
  *     values are the HCLOOC_ERR_* codes below.  Nothing aborts and nothing throws across this ABI.
@@ -295,6 +297,44 @@ int hclooc_dtrsm(hclooc_ctx* ctx, int uplo, int trans, int diag, int64_t M, int6
  * Errors: -1 M < 1, -2 N < 1, -5 NULL output, HCLOOC_ERR_BUDGET when not even a 32-row block with 64-column chunks fits.   */
 int hclooc_dtrsm_plan(int64_t M, int64_t N, size_t device_budget_bytes, int library_owned, int64_t* NB, int64_t* chunk,
                       int* resident, uint64_t* device_bytes);
+
+/* DTRSM with a side argument (BLAS order of arguments).  side = HCL_SIDE_LEFT is hclooc_dtrsm above (error codes then count
+ * the arguments of THIS prototype).  side = HCL_SIDE_RIGHT solves
+ *     X * op(T) = alpha * B,    T = the `uplo` triangle of the N x N matrix A (lda >= N),  B is M x N (ldb >= N), X overwrites B.
+ * Every row of B is an independent system: the rows are cut into bands whose block columns (NB <= 4096 columns; the NB x NB
+ * triangle and a band of one block column each take at most a quarter of the budget) sit in device memory one at a time; a
+ * block column first receives  B_j <- alpha*B_j - X[:, solved] * op(T)[solved, j]  as one out-of-core DGEMM (C in device
+ * memory), then its diagonal block is solved there by recursive halving down to 128-column blocks (one thread per row of B in
+ * the block kernel).  Rounding and gate as hclooc_dtrsm (G23) with N in place of M; exact on integer data with a
+ * power-of-two diagonal.  alpha == 0: X = 0, A not referenced.  stats: plan.mb = band height, plan.nb = NB, plan.flops = M*N*N.
+ * Errors: -2 side, -3 uplo, -4 trans, -5 diag, -6 M < 0, -7 N < 0, -9 A NULL, -10 lda too small, -11 B NULL or overlapping A,
+ * -12 ldb < N; HCLOOC_ERR_BUDGET when not even a 32-column block fits; the HCLOOC_ERR_* codes of hclooc_dgemm.             */
+#define HCL_SIDE_LEFT  0
+#define HCL_SIDE_RIGHT 1
+int hclooc_dtrsm_side(hclooc_ctx* ctx, int side, int uplo, int trans, int diag, int64_t M, int64_t N, double alpha,
+                      const double* A, int64_t lda, double* B, int64_t ldb, size_t device_budget_bytes, hclooc_stats* stats_out);
+
+/* Out-of-core Cholesky factorization (DPOTRF; the paper's future work, :412: "out-of-core factorizations (LU, QR, Cholesky) that
+ * use the out-of-core matrix-matrix multiplication (DGEMM) as a fundamental building block"):
+ *     uplo = HCL_UPLO_LOWER:  A = L * L^T,  L overwrites the lower triangle of A;    HCL_UPLO_UPPER:  A = U^T * U,  U the upper one.
+ * A is N x N, symmetric positive definite, row-major in pinned host memory (lda >= N); only its `uplo` triangle is read and
+ * written, the other triangle keeps its bits.  Left-looking by panels of NB <= 4096 columns (rows, for the upper factor): the
+ * panel sits in device memory (at most half the budget: N * NB * 8 bytes), receives the contribution of the panels before it as
+ * ONE out-of-core DGEMM with the triangle mask (hclooc_dsyrk's), then its diagonal block is factored in device memory -- recursive
+ * halving whose flops sit in tile-kernel launches, 128 x 128 blocks by a one-CTA kernel -- the rest of the panel is solved
+ * against it (X L_jj^T = P, the right-side DTRSM above), and the panel goes back to the host.
+ * *info (LAPACK): 0, or k > 0 when the leading minor of order k is not positive definite -- the factorization stops; the
+ * panels before the one holding column k-1 are complete, the rest of A is unchanged.  The function still returns 0 then.
+ * Rounding: the factor satisfies |A - L L^T| <= gamma_(N+2) |L||L^T| elementwise (any order of summation does, Higham thm 10.3;
+ * DESIGN.md G24); exact on integer data whose factor is integer with a power-of-two diagonal.
+ * stats (nullable): sums over the DGEMM calls and the panel copies; plan.nb (lower) / plan.mb (upper) = NB, plan.flops = N^3/3.
+ * Errors: -2 uplo, -3 N < 0, -4 A NULL, -5 lda < N, -7 info NULL; HCLOOC_ERR_BUDGET when not even a 32-column panel fits half
+ * the budget (N * 512 bytes); the HCLOOC_ERR_* codes of hclooc_dgemm.  Experiment knob: HCLOOC_POTRF_NB=n panel width.      */
+int hclooc_dpotrf(hclooc_ctx* ctx, int uplo, int64_t N, double* A, int64_t lda, size_t device_budget_bytes,
+                  int64_t* info, hclooc_stats* stats_out);
+/* The panel width hclooc_dpotrf works with (pure host arithmetic) and the device bytes of its resident panel.
+ * Errors: -1 N < 1, -3 NULL output, HCLOOC_ERR_BUDGET.                                                                      */
+int hclooc_dpotrf_plan(int64_t N, size_t device_budget_bytes, int64_t* NB, uint64_t* panel_bytes);
 
 /* nsteps mode (:277-283): MMOOC as a subroutine of a blocked algorithm (SUMMA, HSUMMA) that updates the same C
  * `nsteps` times: C = alpha*A_p*B_p + beta_p*C for p = *step = 0 .. nsteps-1, one call per p.  C is uploaded once

@@ -15,21 +15,40 @@ from __future__ import annotations
 import numpy as np
 
 
-def _abs_mv(X: np.ndarray, v: np.ndarray, chunk: int = 2048) -> np.ndarray:
-    """|X| @ |v| in row chunks (bounded temporaries for multi-GB X)."""
+def _chunks(n: int, chunk: int):
+    return [(r, min(n, r + chunk)) for r in range(0, n, chunk)]
+
+
+def _pool():
+    from concurrent.futures import ThreadPoolExecutor
+    import os
+    return ThreadPoolExecutor(max_workers=min(16, os.cpu_count() or 1))
+
+
+def _abs_mv(X: np.ndarray, v: np.ndarray, chunk: int = 256) -> np.ndarray:
+    """|X| @ |v| in row chunks (bounded temporaries for multi-GB X; the chunks run on a thread pool -- every output element
+    is still one dot product of its own row, so the values do not depend on the chunking)."""
     av = np.abs(v)
     out = np.empty(X.shape[0])
-    for r in range(0, X.shape[0], chunk):
-        out[r:r + chunk] = np.abs(X[r:r + chunk]) @ av
+
+    def one(rr):
+        out[rr[0]:rr[1]] = np.abs(X[rr[0]:rr[1]]) @ av
+
+    with _pool() as ex:
+        list(ex.map(one, _chunks(X.shape[0], chunk)))
     return out
 
 
-def _abs_vm(v: np.ndarray, X: np.ndarray, chunk: int = 2048) -> np.ndarray:
-    """|v| @ |X| in row chunks."""
+def _abs_vm(v: np.ndarray, X: np.ndarray, chunk: int = 256) -> np.ndarray:
+    """|v| @ |X| in row chunks: the chunk partials are computed on a thread pool and added up in chunk order."""
     av = np.abs(v)
     out = np.zeros(X.shape[1])
-    for r in range(0, X.shape[0], chunk):
-        out += av[r:r + chunk] @ np.abs(X[r:r + chunk])
+    rows = _chunks(X.shape[0], chunk)
+    with _pool() as ex:
+        for base in range(0, len(rows), 64):          # bounded number of partials alive
+            parts = list(ex.map(lambda rr: av[rr[0]:rr[1]] @ np.abs(X[rr[0]:rr[1]]), rows[base:base + 64]))
+            for p in parts:
+                out += p
     return out
 
 

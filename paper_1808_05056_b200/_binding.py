@@ -12,12 +12,13 @@ HCL_H2D, HCL_D2H = 0, 1
 HCL_OP_N, HCL_OP_T = 0, 1
 HCL_UPLO_LOWER, HCL_UPLO_UPPER = 0, 1
 HCL_DIAG_NONUNIT, HCL_DIAG_UNIT = 0, 1
+HCL_SIDE_LEFT, HCL_SIDE_RIGHT = 0, 1
 
 # every symbol include/hclooc.h declares (tests check the .so exports all of them)
 EXPORTS = [
     "hclooc_plan", "hclooc_plan_ex", "hclooc_plan_trans", "hclooc_shard_rows", "hclMatrixPartitioner", "hclooc_schedule", "hclooc_ctx_create", "hclooc_ctx_destroy",
     "hclooc_ctx_set_trace", "hclooc_ctx_get_trace", "hclooc_ctx_set_direct",
-    "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_t", "hclooc_dsyrk", "hclooc_dsyr2k", "hclooc_dtrsm", "hclooc_dtrsm_plan", "hclooc_dgemm_fig2", "hclooc_dgemm_nsteps", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
+    "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_t", "hclooc_dsyrk", "hclooc_dsyr2k", "hclooc_dtrsm", "hclooc_dtrsm_plan", "hclooc_dtrsm_side", "hclooc_dpotrf", "hclooc_dpotrf_plan", "hclooc_dgemm_fig2", "hclooc_dgemm_nsteps", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
     "hclStreamDestroy", "hclEventDestroy", "hclMemcpy", "hclMemcpyAsync", "hclMemcpy2DAsync",
     "hclDgemmAsync", "hclDgemmAsyncEx", "hclDgemmAsyncT", "hclWaitEvent", "hclStreamSynchronize", "hclDeviceSynchronize",
     "hclooc_host_alloc", "hclooc_host_free", "hclooc_host_register", "hclooc_host_unregister",
@@ -92,6 +93,9 @@ def lib():
         L.hclooc_dsyrk.argtypes = [vp, c_int, c_int, i64, i64, dbl, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
         L.hclooc_dtrsm_plan.argtypes = [i64, i64, sz, c_int, POINTER(i64), POINTER(i64), POINTER(c_int), POINTER(ctypes.c_uint64)]
         L.hclooc_dtrsm.argtypes = [vp, c_int, c_int, c_int, i64, i64, dbl, vp, i64, vp, i64, sz, POINTER(Stats)]
+        L.hclooc_dtrsm_side.argtypes = [vp, c_int, c_int, c_int, c_int, i64, i64, dbl, vp, i64, vp, i64, sz, POINTER(Stats)]
+        L.hclooc_dpotrf.argtypes = [vp, c_int, i64, vp, i64, sz, POINTER(i64), POINTER(Stats)]
+        L.hclooc_dpotrf_plan.argtypes = [i64, sz, POINTER(i64), POINTER(ctypes.c_uint64)]
         L.hclooc_dsyr2k.argtypes = [vp, c_int, c_int, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
         L.hclooc_dgemm_nsteps.argtypes = [vp, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, c_int, POINTER(c_int), POINTER(Stats)]
         L.hclooc_dgemm_fig2.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
@@ -337,6 +341,27 @@ def hclooc_dtrsm(ctx, uplo, trans, diag, M, N, alpha, A, lda, B, ldb, device_bud
     _check(lib().hclooc_dtrsm(ctx, int(uplo), int(trans), int(diag), M, N, alpha, _ptr(A), lda, _ptr(B), ldb,
                               device_budget_bytes, byref(st) if want_stats else None), "hclooc_dtrsm")
     return st if want_stats else None
+
+
+def hclooc_dtrsm_side(ctx, side, uplo, trans, diag, M, N, alpha, A, lda, B, ldb, device_budget_bytes, want_stats=True):
+    st = Stats()
+    _check(lib().hclooc_dtrsm_side(ctx, side, uplo, trans, diag, M, N, alpha, _ptr(A), lda, _ptr(B), ldb, device_budget_bytes,
+                                   byref(st) if want_stats else None), "hclooc_dtrsm_side")
+    return st if want_stats else None
+
+
+def hclooc_dpotrf(ctx, uplo, N, A, lda, device_budget_bytes):
+    """Returns (info, stats)."""
+    st, info = Stats(), c_int64(0)
+    _check(lib().hclooc_dpotrf(ctx, uplo, N, _ptr(A), lda, device_budget_bytes, byref(info), byref(st)), "hclooc_dpotrf")
+    return int(info.value), st
+
+
+def hclooc_dpotrf_plan(N, device_budget_bytes):
+    """(NB, panel_bytes)."""
+    nb, pb = c_int64(), ctypes.c_uint64()
+    _check(lib().hclooc_dpotrf_plan(N, device_budget_bytes, byref(nb), byref(pb)), "hclooc_dpotrf_plan")
+    return int(nb.value), int(pb.value)
 
 
 def hclooc_dgemm_nsteps(ctx, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes, nsteps, step):

@@ -15,6 +15,7 @@
 #include <mutex>
 #include <vector>
 #include "internal.h"
+#include "executor.h"
 
 namespace hclooc {
 
@@ -24,7 +25,6 @@ void set_last_cuda_error(int e) { g_last_cuda_error = e; }
 namespace {
 
 constexpr int DEFAULT_COMPUTE_STREAMS = 8;
-constexpr int MAX_COMPUTE_STREAMS = 16;
 
 // event ids inside a schedule
 struct EventIds {
@@ -238,39 +238,6 @@ void build_schedule(const hclooc_plan_t& P, int ncs, std::vector<hclooc_op_t>& o
 
 using namespace hclooc;
 
-struct hclooc_ctx {
-    int device = 0;
-    void* workspace = nullptr;
-    size_t workspace_bytes = 0;
-    bool owns_workspace = false;
-    cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
-    bool owns_h2d = false, owns_d2h = false;
-    cudaStream_t s_compute[MAX_COMPUTE_STREAMS] = {};
-    int n_compute = 0;
-    bool owns_compute = false;
-    std::vector<cudaEvent_t> events;
-    std::vector<hclooc_op_t> ops;
-    bool trace = false;
-    int direct_mode = -1;                         // -1 cost model decides, 0 never, 1 whenever the operands allow it
-    // plans of recent calls: the search over candidates costs 0.2 ms (config 1) to 9 ms (config 4) of host time
-    // before the first copy can be issued, and a blocked algorithm repeats the same shapes over and over
-    struct PlanKey { int64_t M, N, K; int beta_nz, alpha_zero, where; size_t budget; };
-    std::vector<std::pair<PlanKey, hclooc_plan_t>> plan_cache;
-    std::vector<cudaEvent_t> trace_events;        // 2 per traced op (+1 base), timing enabled
-    std::vector<hclooc_trace_rec> trace_recs;     // filled after the final synchronisation
-    // the schedule of the last call captured as a CUDA graph (short, latency-bound schedules; same call again
-    // -> one graph launch instead of hundreds of enqueues)
-    cudaGraphExec_t graph_exec = nullptr;
-    bool graph_valid = false;                     // graph_exec is the schedule of graph_key
-    std::vector<int64_t> graph_key;               // the previous call
-    std::vector<cudaEvent_t> join_events;
-    // nsteps mode (hclooc_dgemm_nsteps): C kept in device memory between the calls of one sequence
-    double* res_c = nullptr;
-    int64_t res_ld = 0, res_M = 0, res_N = 0, res_ldc = 0;
-    const double* res_host = nullptr;
-    size_t res_bytes = 0;
-    std::mutex mu;
-};
 
 extern "C" int hclooc_schedule(const hclooc_plan_t* plan, int n_compute, hclooc_op_t* ops, size_t max_ops, size_t* n_ops) {
     if (!plan) return -1;
@@ -333,9 +300,11 @@ extern "C" int hclooc_ctx_destroy(hclooc_ctx* c) {
 }
 
 namespace {
-
 hclooc_ctx* g_default_ctx = nullptr;
 std::mutex g_default_mu;
+}  // namespace
+
+namespace hclooc {
 
 int default_ctx(hclooc_ctx** out) {
     std::lock_guard<std::mutex> lk(g_default_mu);
@@ -351,7 +320,7 @@ int default_ctx(hclooc_ctx** out) {
 
 // 0 = ok, HCLOOC_ERR_NOT_PINNED if pageable host memory; *on_device is cleared unless p is device memory;
 // *dev_alias (nullable) = the address under which kernels on the device reach p (NULL if they cannot)
-int check_resident(const void* p, bool* on_device, const void** dev_alias = nullptr) {
+int check_resident(const void* p, bool* on_device, const void** dev_alias) {
     cudaPointerAttributes at;
     cudaError_t e = cudaPointerGetAttributes(&at, p);
     if (e != cudaSuccess) { cudaGetLastError(); return HCLOOC_ERR_NOT_PINNED; }
@@ -375,16 +344,25 @@ int copy2d(void* dst, size_t dpitch, const void* src, size_t spitch, size_t widt
     return HCLOOC_OK;
 }
 
-}  // namespace
-
-namespace {
-
 // tri != 0 (hclooc_dsyrk): only the lower (1) / upper (2) triangle of this call's C, whose element (0, 0) lies on the diagonal,
 // is referenced.  The kernels skip the other triangle; its elements still ride along in the C blocks that cross the
 // diagonal, which is why such a call uploads its C blocks even when beta == 0 (they come back unchanged).
 int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
                int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
-               size_t device_budget_bytes, hclooc_stats* stats, int tri = 0) {
+               size_t device_budget_bytes, hclooc_stats* stats, int tri) {
+    // argument errors and the quick returns need no context (and must not create one: validation touches no device)
+    int rc = dgemm_core_locked(nullptr, transa, transb, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes, stats, tri);
+    if (rc != HCLOOC_ERR_INTERNAL + 1000) return rc;
+    if (!ctx && (rc = default_ctx(&ctx))) return rc;
+    std::lock_guard<std::mutex> lk(ctx->mu);
+    return dgemm_core_locked(ctx, transa, transb, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes, stats, tri);
+}
+
+// the same with ctx->mu already held by the caller (a routine that keeps one lock over all its DGEMM calls and its own
+// device work between them: hclooc_dtrsm, hclooc_dpotrf); ctx must not be NULL
+int dgemm_core_locked(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
+                      int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
+                      size_t device_budget_bytes, hclooc_stats* stats, int tri) {
     const auto t_begin = std::chrono::steady_clock::now();
     // ---------------------------------------------------------------- S0 validate (argument numbers of hclooc_dgemm)
     if (M < 0) return -1;
@@ -406,9 +384,8 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
     if (!scale_only && (overlaps(C, M, N, ldc, A, a_rows, a_cols, lda) || overlaps(C, M, N, ldc, B, b_rows, b_cols, ldb))) return -10;
     if (scale_only && beta == 1.0) return HCLOOC_OK;            // C = 1*C
     if (scale_only) transa = transb = 0;                        // A and B are not referenced
+    if (!ctx) return HCLOOC_ERR_INTERNAL + 1000;                // validation-only pass of dgemm_core: the arguments are fine
     int rc;
-    if (!ctx && (rc = default_ctx(&ctx))) return rc;
-    std::lock_guard<std::mutex> lk(ctx->mu);
     HCL_CUDA(cudaSetDevice(ctx->device));
     bool on_device = true, c_dev = true, ab_dev = true;
     const void *A_alias = nullptr, *B_alias = nullptr, *C_alias = nullptr;
@@ -426,6 +403,11 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
         fr += ctx->workspace_bytes;                                // what we already hold counts as free
         const size_t margin = (size_t)1 << 30;
         budget = fr > 2 * margin ? fr - margin : fr / 2;
+    }
+    const size_t reserved = ctx->reserved_bytes;
+    if (reserved) {
+        if (budget <= reserved) return HCLOOC_ERR_BUDGET;
+        budget -= reserved;
     }
     hclooc_plan_t P;
     // in-core case: every operand already in device memory and addressable by the tile kernel as it is
@@ -484,7 +466,8 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
         }
         return HCLOOC_OK;
     }
-    if (P.workspace_bytes > ctx->workspace_bytes) {
+    if (reserved && P.workspace_bytes + reserved > ctx->workspace_bytes) return HCLOOC_ERR_BUDGET;   // the caller sized the workspace
+    if (!reserved && P.workspace_bytes > ctx->workspace_bytes) {
         if (ctx->workspace && !ctx->owns_workspace) return HCLOOC_ERR_BUDGET;
         if (ctx->workspace) { HCL_CUDA(cudaDeviceSynchronize()); cudaFree(ctx->workspace); ctx->workspace = nullptr; ctx->workspace_bytes = 0; }
         void* p = nullptr;
@@ -493,11 +476,11 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
         ctx->workspace = p; ctx->workspace_bytes = P.workspace_bytes; ctx->owns_workspace = true;
     }
     // ---------------------------------------------------------------- buffers carved from the workspace
-    uint8_t* base = (uint8_t*)ctx->workspace;
+    uint8_t* base = (uint8_t*)ctx->workspace + reserved;
     const uintptr_t mis = (uintptr_t)base & 1023u;
     if (mis) {   // caller workspace not 1 KiB aligned: shift (costs < 1 KiB, checked against the size)
         base += 1024 - mis;
-        if (P.workspace_bytes + 1024 - mis > ctx->workspace_bytes) return HCLOOC_ERR_BUDGET;
+        if (P.workspace_bytes + reserved + 1024 - mis > ctx->workspace_bytes) return HCLOOC_ERR_BUDGET;
     }
     std::vector<double*> bufs(P.n_abuf + P.n_sets + P.n_bbuf);
     uint8_t* scratch[MAX_COMPUTE_STREAMS] = {};
@@ -821,7 +804,23 @@ extern "C" int hclooc_dgemm(int64_t M, int64_t N, int64_t K, double alpha, const
 // launch that updates the rows of the chunk still to be solved.  Left-looking outside keeps the traffic at one read of
 // X[solved] per block row (2*NB flops per 8 bytes: NB = 4096 is compute bound on this link); right-looking inside gives
 // the tile kernel launches of hundreds of tiles instead of 16.
-namespace {
+namespace hclooc {
+
+int resolve_budget(hclooc_ctx* ctx, size_t device_budget_bytes, size_t* budget_out, bool* library_owned) {
+    size_t budget = device_budget_bytes;
+    if (library_owned) *library_owned = ctx->owns_workspace || !ctx->workspace;
+    if (!ctx->owns_workspace && ctx->workspace) {
+        budget = (budget == 0) ? ctx->workspace_bytes : std::min(budget, ctx->workspace_bytes);
+    } else if (budget == 0) {
+        size_t fr = 0, tot = 0;
+        HCL_CUDA(cudaMemGetInfo(&fr, &tot));
+        fr += ctx->workspace_bytes;                                // what we already hold counts as free
+        const size_t margin = (size_t)1 << 30;
+        budget = fr > 2 * margin ? fr - margin : fr / 2;
+    }
+    *budget_out = budget;
+    return HCLOOC_OK;
+}
 
 int ensure_workspace(hclooc_ctx* ctx, size_t bytes) {
     if (bytes <= ctx->workspace_bytes) return HCLOOC_OK;
@@ -833,6 +832,10 @@ int ensure_workspace(hclooc_ctx* ctx, size_t bytes) {
     ctx->workspace = p; ctx->workspace_bytes = bytes; ctx->owns_workspace = true;
     return HCLOOC_OK;
 }
+
+}  // namespace hclooc
+
+namespace {
 
 struct TrsmShape { int64_t NB, ldt, wc; size_t bytes; };
 

@@ -1,0 +1,69 @@
+// executor.h -- the context and the entry points of executor.cu that the other out-of-core routines (factor.cu) build on.
+#pragma once
+#include <mutex>
+#include <utility>
+#include <vector>
+#include "internal.h"
+
+constexpr int MAX_COMPUTE_STREAMS = 16;
+
+struct hclooc_ctx {
+    int device = 0;
+    void* workspace = nullptr;
+    size_t workspace_bytes = 0;
+    bool owns_workspace = false;
+    cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
+    bool owns_h2d = false, owns_d2h = false;
+    cudaStream_t s_compute[MAX_COMPUTE_STREAMS] = {};
+    int n_compute = 0;
+    bool owns_compute = false;
+    std::vector<cudaEvent_t> events;
+    std::vector<hclooc_op_t> ops;
+    bool trace = false;
+    int direct_mode = -1;                         // -1 cost model decides, 0 never, 1 whenever the operands allow it
+    // plans of recent calls: the search over candidates costs 0.2 ms (config 1) to 9 ms (config 4) of host time
+    // before the first copy can be issued, and a blocked algorithm repeats the same shapes over and over
+    struct PlanKey { int64_t M, N, K; int beta_nz, alpha_zero, where; size_t budget; };
+    std::vector<std::pair<PlanKey, hclooc_plan_t>> plan_cache;
+    std::vector<cudaEvent_t> trace_events;        // 2 per traced op (+1 base), timing enabled
+    std::vector<hclooc_trace_rec> trace_recs;     // filled after the final synchronisation
+    // the schedule of the last call captured as a CUDA graph (short, latency-bound schedules; same call again
+    // -> one graph launch instead of hundreds of enqueues)
+    cudaGraphExec_t graph_exec = nullptr;
+    bool graph_valid = false;                     // graph_exec is the schedule of graph_key
+    std::vector<int64_t> graph_key;               // the previous call
+    std::vector<cudaEvent_t> join_events;
+    // nsteps mode (hclooc_dgemm_nsteps): C kept in device memory between the calls of one sequence
+    double* res_c = nullptr;
+    int64_t res_ld = 0, res_M = 0, res_N = 0, res_ldc = 0;
+    const double* res_host = nullptr;
+    size_t res_bytes = 0;
+    // bytes at the front of the workspace that a routine running several DGEMM calls keeps for itself (a resident panel of
+    // hclooc_dpotrf / hclooc_dtrsm_side): dgemm_core_locked carves its buffers behind them and plans with the rest of the budget
+    size_t reserved_bytes = 0;
+    std::mutex mu;
+};
+
+namespace hclooc {
+
+int default_ctx(hclooc_ctx** out);
+// 0 = ok, HCLOOC_ERR_NOT_PINNED if pageable host memory; *on_device is cleared unless p is device memory;
+// *dev_alias (nullable) = the address under which kernels on the device reach p (NULL if they cannot)
+int check_resident(const void* p, bool* on_device, const void** dev_alias = nullptr);
+bool overlaps(const double* a, int64_t rows_a, int64_t cols_a, int64_t lda, const double* b, int64_t rows_b, int64_t cols_b, int64_t ldb);
+int copy2d(void* dst, size_t dpitch, const void* src, size_t spitch, size_t width, size_t rows, cudaStream_t s);
+// the budget a call works under: the caller's figure, clipped to a caller-owned workspace, or all free device memory less 1 GiB
+int resolve_budget(hclooc_ctx* ctx, size_t device_budget_bytes, size_t* budget, bool* library_owned);
+int ensure_workspace(hclooc_ctx* ctx, size_t bytes);
+
+// C = alpha*op(A)*op(B) + beta*C through the pipeline (executor.cu).  tri != 0: only the lower (1) / upper (2) triangle of this
+// call's C -- element (0, 0) on the diagonal -- is referenced (hclooc_dsyrk, the Cholesky panel).  Takes ctx->mu itself.
+int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
+               int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
+               size_t device_budget_bytes, hclooc_stats* stats, int tri = 0);
+// the same with ctx->mu already held by the caller (ctx not NULL)
+int dgemm_core_locked(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
+                      int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
+                      size_t device_budget_bytes, hclooc_stats* stats, int tri = 0);
+
+}  // namespace hclooc

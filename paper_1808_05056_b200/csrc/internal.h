@@ -92,8 +92,14 @@ int plan_impl(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zero,
               int operands_on_device, int transa, int transb, hclooc_plan_t* out);
 
 // Diagonal-block solve of hclooc_dtrsm (trsm_sm100.cu): dX (ib x ncols, ib <= 128) <- op(T)^-1 * (scale * dX) in place
+// right != 0: dX is ncols x ib and dX <- (scale * dX) * op(T)^-1 (one thread per row)
 int launch_trsm_block(const double* dT, int64_t ldt, int ib, double* dX, int64_t ldx, int64_t ncols, int lower, int trans,
-                      int unit, double scale, cudaStream_t stream);
+                      int unit, double scale, cudaStream_t stream, int right = 0);
+
+// Cholesky factorization of one diagonal block of at most 128 x 128 in device memory (potrf_sm100.cu): the `lower` (1) or upper
+// (0) triangle of dA is overwritten by its factor; *d_info (device, int64) receives info_base + j + 1 if the pivot of column j is
+// not positive and *d_info was 0 (the block is then left partly factored).
+int launch_potrf_block(double* dA, int64_t lda, int n, int lower, long long* d_info, long long info_base, cudaStream_t stream);
 
 // number of CTAs the tile kernel uses for an M x N output (for stats / tests)
 int64_t dgemm_tile_count(int64_t M, int64_t N);

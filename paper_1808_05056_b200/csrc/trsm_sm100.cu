@@ -22,7 +22,7 @@ constexpr int TSTAGE = 256;      // threads per CTA: all of them stage the trian
 constexpr size_t TRSM_SMEM = (size_t)TB * TS * 8 + (size_t)TB * TCOLS * 8;   // 130 KiB triangle + 64 KiB solved rows
 
 __global__ void __launch_bounds__(TSTAGE, 1)
-trsm_block_kernel(const double* __restrict__ T, long long ldt, int ib, double* __restrict__ X, long long ldx, int ncols,
+trsm_block_kernel(const double* __restrict__ T, long long ldt, int ib, double* __restrict__ X, long long sq, long long si, int ncols,
                   int lower, int trans, int unit, double scale) {
     extern __shared__ __align__(16) double smem[];
     double* sTt = smem;                       // sTt[p * TS + q] = T'[q][p], T' = op(T) in logical (lower) order, 0 above, 1 on
@@ -64,7 +64,7 @@ trsm_block_kernel(const double* __restrict__ T, long long ldt, int ib, double* _
         for (int t = 0; t < SUB; ++t) {
             const int q = q0 + t;
             const int r = lower ? q : ib - 1 - q;
-            b[t] = (live && q < ib) ? scale * X[(long long)r * ldx + col] : 0.0;
+            b[t] = (live && q < ib) ? scale * X[(long long)r * sq + (long long)col * si] : 0.0;
         }
         // left-looking: subtract the contribution of the rows solved so far (xs is private to this thread's column)
 #pragma unroll 2
@@ -93,7 +93,7 @@ trsm_block_kernel(const double* __restrict__ T, long long ldt, int ib, double* _
             xs[q * TCOLS + tid] = b[t];
             if (live && q < ib) {
                 const int r = lower ? q : ib - 1 - q;
-                X[(long long)r * ldx + col] = b[t];
+                X[(long long)r * sq + (long long)col * si] = b[t];
             }
         }
     }
@@ -103,14 +103,20 @@ trsm_block_kernel(const double* __restrict__ T, long long ldt, int ib, double* _
 
 // X (ib x ncols, row-major, ldx) <- op(T)^-1 * (scale * X) for the ib x ib diagonal block T (row-major as stored, ldt);
 // lower = op(T) is lower triangular, trans = op(T)[r][c] is stored at T[c][r], unit = the diagonal is 1 and not read.
+// right != 0 (DTRSM side = Right, and the Cholesky panel): X is ncols x ib and X <- (scale * X) * op(T)^-1.  Every ROW of X is
+// then an independent system op(T)^T x^T = b^T: the same substitution with the triangle read transposed and one thread per row
+// of X instead of one per column (only the addressing of X changes: element (q, item) sits at X[item*ldx + q]).
 int launch_trsm_block(const double* dT, int64_t ldt, int ib, double* dX, int64_t ldx, int64_t ncols, int lower, int trans,
-                      int unit, double scale, cudaStream_t stream) {
+                      int unit, double scale, cudaStream_t stream, int right) {
     if (ib <= 0 || ncols <= 0) return HCLOOC_OK;
     if (ib > TB || ncols > 0x7fffffffLL) return HCLOOC_ERR_INTERNAL;
     static cudaError_t attr = cudaFuncSetAttribute(trsm_block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TRSM_SMEM);
     if (attr != cudaSuccess) return cuda_fail(attr);
     const unsigned grid = (unsigned)((ncols + TCOLS - 1) / TCOLS);
-    trsm_block_kernel<<<grid, TSTAGE, TRSM_SMEM, stream>>>(dT, (long long)ldt, ib, dX, (long long)ldx, (int)ncols, lower, trans, unit, scale);
+    if (right)      // the operator of the row systems is op(T)^T: lower where op(T) is upper, and read with `trans` flipped
+        trsm_block_kernel<<<grid, TSTAGE, TRSM_SMEM, stream>>>(dT, (long long)ldt, ib, dX, 1LL, (long long)ldx, (int)ncols, !lower, !trans, unit, scale);
+    else
+        trsm_block_kernel<<<grid, TSTAGE, TRSM_SMEM, stream>>>(dT, (long long)ldt, ib, dX, (long long)ldx, 1LL, (int)ncols, lower, trans, unit, scale);
     HCL_CUDA(cudaGetLastError());
     return HCLOOC_OK;
 }
