@@ -57,7 +57,7 @@ def spd_host(H, N, seed, dist, pad=0):
     (1000, "int", 0, 32 * MiB),              # one panel of 1000: three levels of recursion, exact
     (1000, "uniform", 3, 2 * MiB),           # panels of 128 columns: 8 out-of-core updates
     (1500, "int", 1, 4 * MiB),               # panels of 128..160, K up to 1400 in the updates, exact
-    (2049, "uniform", 0, 16 * MiB),          # odd size: the last panel is one column
+    (2049, "uniform", 0, 16 * MiB),          # odd size: panels of 384, a ragged last one of 129
 ])
 def test_dpotrf_matches_oracle(H, uplo, N, dist, pad, budget):
     A, L0 = spd_host(H, N, 71, dist, pad)
