@@ -603,6 +603,148 @@ class Bench:
             print(json.dumps({"kernel_only": True, "workload": name, "solo_step": solo, "streamk": full, "clocks": clocks}))
 
 
+# ---------------------------------------------------------------------------------------------- the other product paths
+def run_op(args):
+    """`--op dsyrk|dsyr2k|dtrsm|dtrsm_right|dpotrf`: the routines built on the out-of-core DGEMM, timed like the
+    DGEMM -- pinned host operands, a context created beforehand, wall time inside the call -- against the roofline of the call
+    (the slower of its flops at the FP64 peak and its own bytes at the link rates measured here).  One JSON line."""
+    import torch
+    import synthgen
+    import paper_1808_05056_b200 as H
+    torch.cuda.set_device(0)
+    live = measure_link(H)
+    if live:
+        LINK.update(live)
+    op, M, N, K, budget = args.op, args.m, args.n, args.k, args.budget
+    seed = synthgen.BASE_SEED + 9
+    ctx = H.hclooc_ctx_create(0)
+    mats = []
+
+    def host(rows, cols, name, dist="uniform"):
+        X = H.HostMatrix(rows, cols)
+        synthgen.fill(X.array, seed, name, dist)
+        mats.append(X)
+        return X
+
+    extra = {}
+    if op in ("dsyrk", "dsyr2k"):
+        A, C = host(N, K, "A"), host(N, N, "C")
+        Bm = host(N, K, "B") if op == "dsyr2k" else None
+        flops = float(N) * (N + 1) * K * (2 if op == "dsyr2k" else 1)
+        if op == "dsyrk":
+            call = lambda: H.hclooc_dsyrk(ctx, args.uplo, args.trans, N, K, 1.0, A, A.ld, args.beta, C, N, budget)
+        else:
+            call = lambda: H.hclooc_dsyr2k(ctx, args.uplo, args.trans, N, K, 1.0, A, A.ld, Bm, Bm.ld, args.beta, C, N, budget)
+        shape = {"N": N, "K": K}
+    elif op in ("dtrsm", "dtrsm_right"):
+        n_tri = M if op == "dtrsm" else N
+        A, Bm = host(n_tri, n_tri, "A"), host(M, N, "B")
+        synthgen.shape_triangular(A.view, "uniform")
+        flops = float(M) * N * n_tri
+        B0 = None
+        if op == "dtrsm":
+            call = lambda: H.hclooc_dtrsm(ctx, args.uplo, args.trans, 0, M, N, 1.0, A, A.ld, Bm, Bm.ld, budget)
+        else:
+            call = lambda: H.hclooc_dtrsm_side(ctx, H.HCL_SIDE_RIGHT, args.uplo, args.trans, 0, M, N, 1.0, A, A.ld, Bm, Bm.ld, budget)
+        shape = {"M": M, "N": N}
+    elif op == "dpotrf":
+        # symmetric positive definite by construction: uniform[-1,1) entries / N off the diagonal (row sums < 1), diagonal in [1, 2)
+        A = host(N, N, "A")
+        synthgen.shape_triangular(A.view, "uniform")
+        d = np.abs(A.view[np.arange(N), np.arange(N)]).copy()
+        A0 = H.HostMatrix(N, N)
+        mats.append(A0)
+        half = np.tril(A.view, -1)
+        A0.view[...] = half
+        A0.view[...] += half.T
+        A0.view[np.arange(N), np.arange(N)] = d
+        del half
+        flops = float(N) ** 3 / 3.0
+        infos = []
+
+        def call():
+            A.view[...] = A0.view                      # the factorization overwrites its input: restore it (outside the timed span:
+            info, st = H.hclooc_dpotrf(ctx, args.uplo, N, A, A.ld, budget)      # t_total_s is the wall time inside the call)
+            infos.append(info)
+            return st
+        shape = {"N": N}
+        extra["info"] = infos
+    else:
+        raise SystemExit(f"unknown --op {op}")
+    try:
+        with ClockSampler(0) as clk:
+            ts, st = [], None
+            for _ in range(max(2, args.steps or 3)):
+                st = call()
+                ts.append(st.t_total_s)
+            clocks = clk.summary()
+    finally:
+        H.hclooc_ctx_destroy(ctx)
+        for X in mats:
+            X.free()
+    t = float(np.mean(ts[1:]))
+    t_roof, t_flop, t_link = link_roofline_s(flops, st.bytes_h2d, st.bytes_d2h)
+    out = {"op": f"hclooc_{op}", **shape, "uplo": args.uplo, "trans": args.trans, "budget_bytes": budget, "t_s": t, "t_all_s": ts,
+           "tflops": flops / t / 1e12, "flops": flops, "h2d_GB": st.bytes_h2d / 1e9, "d2h_GB": st.bytes_d2h / 1e9,
+           "kernels": int(st.n_kernels), "plan": Bench.plan_summary(st.plan), "t_flop_s": t_flop, "t_link_s": t_link,
+           "bound": "fp64" if t_flop >= t_link else "link", "frac_of_roofline": t_roof / t, "link_peaks": LINK, "clocks": clocks, **extra}
+    print(json.dumps(out))
+
+
+TRANSITION_SIZES = [4096, 8192, 12288, 16384, 20480, 22528, 23552, 24576, 28672, 32768, 36864, 40960, 46080]
+
+
+def run_transition_sweep(args):
+    """`--sweep transition`: the paper's own experiment shape: square FP64 DGEMM, N
+    swept across the point where A, B and C stop fitting the device budget (default 12.2e9 bytes: the paper's 12 GB cards
+    switched to out-of-core above N = 22528), end to end, for the tuned scheduler (hclooc_dgemm_ex) and the paper's Figure-2
+    pipeline (hclooc_dgemm_fig2), each with its fraction of max(T_flop, T_link).  One JSON line per size, then a Markdown table."""
+    import ctypes
+    import torch
+    import synthgen
+    import paper_1808_05056_b200 as H
+    torch.cuda.set_device(0)
+    live = measure_link(H)
+    if live:
+        LINK.update(live)
+    budget = args.budget if args.budget else 12_200_000_000
+    sizes = sorted(int(x) for x in args.sizes.split(",")) if args.sizes else TRANSITION_SIZES
+    nmax = sizes[-1]
+    bufs = [H.HostMatrix(nmax, nmax) for _ in range(3)]        # one pinned allocation per matrix, reused as a dense N x N matrix
+    ctx = H.hclooc_ctx_create(0)
+    rows = []
+    try:
+        for n in sizes:
+            A, B, C = (np.frombuffer((ctypes.c_double * (n * n)).from_address(X.ptr), dtype=np.float64).reshape(n, n) for X in bufs)
+            for arr, nm in ((A, "A"), (B, "B"), (C, "C")):
+                synthgen.fill(arr, synthgen.BASE_SEED + 9, nm, "uniform")
+            rec = {"N": n, "fits_budget": 24 * n * n <= budget, "budget_bytes": budget, "flops": 2.0 * n ** 3}
+            for label, call in (("tuned", lambda: H.hclooc_dgemm_ex(ctx, n, n, n, 1.0, A, n, B, n, args.beta, C, n, budget)),
+                                ("fig2", lambda: H.hclooc_dgemm_fig2(n, n, n, 1.0, A, n, B, n, args.beta, C, n, budget))):
+                ts, st = [], None
+                for _ in range(max(2, args.steps or 3)):
+                    st = call()
+                    ts.append(st.t_total_s)
+                t = float(np.mean(ts[1:]))
+                t_roof, t_flop, t_link = link_roofline_s(2.0 * n ** 3, st.bytes_h2d, st.bytes_d2h)
+                rec[label] = {"t_s": t, "tflops": 2.0 * n ** 3 / t / 1e12, "h": st.plan.h, "w": st.plan.w, "kpanels": st.plan.kpanels, "steps": st.plan.n_steps,
+                              "h2d_GB": st.bytes_h2d / 1e9, "d2h_GB": st.bytes_d2h / 1e9, "frac_of_roofline": t_roof / t,
+                              "bound": "fp64" if t_flop >= t_link else "link"}
+            rec["fig2_over_tuned"] = rec["fig2"]["tflops"] / rec["tuned"]["tflops"]
+            rows.append(rec)
+            print(json.dumps(rec), flush=True)
+    finally:
+        H.hclooc_ctx_destroy(ctx)
+        for X in bufs:
+            X.free()
+    print("| N | fits budget | tuned TFLOP/s (h x w x kpanels) | tuned / roofline | Figure-2 TFLOP/s (h x w) | Figure-2 / roofline | Figure-2 / tuned |")
+    print("|---|---|---|---|---|---|---|")
+    for r in rows:
+        print(f"| {r['N']} | {'yes' if r['fits_budget'] else 'no'} | {r['tuned']['tflops']:.2f} ({r['tuned']['h']} x {r['tuned']['w']} x {r['tuned']['kpanels']}) | "
+              f"{r['tuned']['frac_of_roofline']:.3f} ({r['tuned']['bound']}) | {r['fig2']['tflops']:.2f} ({r['fig2']['h']} x {r['fig2']['w']}) | "
+              f"{r['fig2']['frac_of_roofline']:.3f} | {r['fig2_over_tuned']:.3f} |")
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -619,8 +761,24 @@ def main():
     ap.add_argument("--trans", default="NN", choices=["NN", "TN", "NT", "TT"],
                     help="e2e leg through hclooc_dgemm_t with op(A), op(B) transposed (the same buffers read as the stored K x M / N x K matrices)")
     ap.add_argument("--kernel-only", action="store_true", help="only the kernel legs (for ncu captures of the tile kernel)")
+    ap.add_argument("--op", default="dgemm", choices=["dgemm", "dsyrk", "dsyr2k", "dtrsm", "dtrsm_right", "dpotrf"],
+                    help="time another routine of the library instead (sizes from --m/--n/--k/--budget; --steps calls, the first discarded)")
+    ap.add_argument("--sweep", default="", choices=["", "transition"], help="transition: the paper's N sweep across the in-core / out-of-core point")
+    ap.add_argument("--m", type=int, default=32768)
+    ap.add_argument("--n", type=int, default=32768)
+    ap.add_argument("--k", type=int, default=8192)
+    ap.add_argument("--budget", type=int, default=0, help="--op / --sweep: device budget in bytes (0: 4 GiB for --op, 12.2e9 for the sweep)")
+    ap.add_argument("--uplo", type=int, default=0)
+    ap.add_argument("--beta", type=float, default=1.0)
+    ap.add_argument("--sizes", default="", help="--sweep transition: comma-separated N")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
+    if args.sweep == "transition":
+        return run_transition_sweep(args)
+    if args.op != "dgemm":
+        args.trans = int(args.trans[0] == "T") if isinstance(args.trans, str) else args.trans
+        args.budget = args.budget or (4 << 30)
+        return run_op(args)
     if args.impl == "reference":
         return run_reference(args)
     b = Bench(args)
