@@ -80,8 +80,10 @@ typedef struct hclooc_plan_t {
     double   flops;               /* 2*M*N*K (:368)                                                 */
     double   t_flop_s, t_link_s, t_model_s;  /* cost model terms used to pick this plan             */
     int32_t  n_scratch;           /* stream-K scratch buffers (ksplit == -1): one per compute stream used       */
-    int32_t  c_on_device;         /* C lives in device memory: its block copies are device-to-device and are not
-                                     counted in bytes_h2d / bytes_d2h (host-link bytes)                         */
+    int32_t  c_on_device;         /* 1: C lives in device memory: its block copies are device-to-device and are not
+                                     counted in bytes_h2d / bytes_d2h (host-link bytes); 2: the result is written to device
+                                     memory but the INITIAL C (the uploads of K panel 0) is read from a host matrix, which
+                                     counts (a resident panel of hclooc_dpotrf / hclooc_dtrsm filled by the pipeline itself) */
     uint64_t bytes_scratch;       /* one of them (partial-tile slots + counters)                                */
     int32_t  direct;              /* 1 = DIRECT mode: no device buffer at all -- one launch of the tile kernel whose TMA
                                      loads read the A and B tiles straight from the (mapped) pinned host matrices and whose
@@ -114,7 +116,8 @@ int hclooc_plan(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zer
  * device, so they cost no host-link time and are not counted in bytes_h2d / bytes_d2h;
  * 3 = as 0, and the device can address the host matrices as they are (mapped pinned memory, 16-byte aligned, even
  * leading dimensions): the cost model may then pick the DIRECT mode (plan.direct) when it beats every staged plan;
- * 4 = as 3 but direct mode is forced (tests, experiments).  -8: NULL out. */
+ * 4 = as 3 but direct mode is forced (tests, experiments); 5 = as 2, but the initial C is read from a host matrix
+ * (plan.c_on_device = 2: the C uploads of K panel 0 count as link traffic).  -8: NULL out. */
 int hclooc_plan_ex(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zero,
                    size_t device_budget_bytes, int operands_on_device, hclooc_plan_t* out);
 
@@ -318,13 +321,15 @@ int hclooc_dtrsm_side(hclooc_ctx* ctx, int side, int uplo, int trans, int diag, 
  * use the out-of-core matrix-matrix multiplication (DGEMM) as a fundamental building block"):
  *     uplo = HCL_UPLO_LOWER:  A = L * L^T,  L overwrites the lower triangle of A;    HCL_UPLO_UPPER:  A = U^T * U,  U the upper one.
  * A is N x N, symmetric positive definite, row-major in pinned host memory (lda >= N); only its `uplo` triangle is read and
- * written, the other triangle keeps its bits.  Left-looking by panels of NB <= 4096 columns (rows, for the upper factor): the
- * panel sits in device memory (at most half the budget: N * NB * 8 bytes), receives the contribution of the panels before it as
- * ONE out-of-core DGEMM with the triangle mask (hclooc_dsyrk's), then its diagonal block is factored in device memory -- recursive
- * halving whose flops sit in tile-kernel launches, 128 x 128 blocks by a one-CTA kernel -- the rest of the panel is solved
- * against it (X L_jj^T = P, the right-side DTRSM above), and the panel goes back to the host.
+ * written, the other triangle keeps its bits.  Left-looking by panels of NB <= 4096 columns (rows, for the upper factor) with a
+ * LOOK-AHEAD of one panel: two panels sit in device memory (at most half the budget: 2 * N * NB * 8 bytes).  While panel j is
+ * factored there -- its diagonal block by recursive halving whose flops sit in tile-kernel launches (128 x 128 blocks by a one-CTA
+ * kernel), the rest of the panel solved against it (X L_jj^T = P, the right-side DTRSM above) -- panel j+1 is uploaded and receives
+ * the contribution of the panels before j as ONE out-of-core DGEMM with the triangle mask (hclooc_dsyrk's) streamed from the host;
+ * panel j's own contribution then comes straight from device memory, and panel j goes back to the host beside all that.
  * *info (LAPACK): 0, or k > 0 when the leading minor of order k is not positive definite -- the factorization stops; the
- * panels before the one holding column k-1 are complete, the rest of A is unchanged.  The function still returns 0 then.
+ * panels before the one holding column k-1 are complete, that panel is left partly factored (as LAPACK leaves it undefined) and
+ * the panels after it are unchanged.  The function still returns 0 then.
  * Rounding: the factor satisfies |A - L L^T| <= gamma_(N+2) |L||L^T| elementwise (any order of summation does, Higham thm 10.3;
  * DESIGN.md G24); exact on integer data whose factor is integer with a power-of-two diagonal.
  * stats (nullable): sums over the DGEMM calls and the panel copies; plan.nb (lower) / plan.mb (upper) = NB, plan.flops = N^3/3.
@@ -407,6 +412,18 @@ int hclDgemmAsyncEx(int64_t M, int64_t N, int64_t K, double alpha, const double*
 int hclDgemmAsyncT(int transa, int transb, int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda,
                    const double* dB, int64_t ldb, double beta, double* dC, int64_t ldc,
                    hclStream s, hclEvent* ev, int variant);
+/* In-core DTRSM and DPOTRF on DEVICE pointers, asynchronous in stream s -- the device phases of hclooc_dtrsm[_side] and
+ * hclooc_dpotrf as calls of their own (recursive halving down to 128 x 128 blocks: the flops sit in tile-kernel launches, the
+ * blocks go to the substitution / factorization block kernels).  dA, dB 16-byte aligned, lda, ldb even, else HCLOOC_ERR_ALIGN.
+ *   hclDtrsmAsync:  op(T) X = alpha B (side = HCL_SIDE_LEFT, T is M x M) or X op(T) = alpha B (HCL_SIDE_RIGHT, T is N x N), B is
+ *     M x N and is overwritten by X.  Errors: -1 side, -2 uplo, -3 trans, -4 diag, -5 M < 0, -6 N < 0, -8 dA NULL, -9 lda, -10 dB
+ *     NULL, -11 ldb < N.
+ *   hclDpotrfAsync: the `uplo` triangle of the N x N matrix dA is overwritten by its Cholesky factor; *d_info (DEVICE memory,
+ *     8 bytes) is zeroed and receives k > 0 if the leading minor of order k is not positive definite.  Errors: -1 uplo, -2 N < 0,
+ *     -3 dA NULL, -4 lda < N, -5 d_info NULL.                                                                              */
+int hclDtrsmAsync(int side, int uplo, int trans, int diag, int64_t M, int64_t N, double alpha, const double* dA, int64_t lda,
+                  double* dB, int64_t ldb, hclStream s, hclEvent* ev);
+int hclDpotrfAsync(int uplo, int64_t N, double* dA, int64_t lda, long long* d_info, hclStream s, hclEvent* ev);
 int hclWaitEvent(hclStream s, hclEvent e);                        /* :116  stream waits for event   */
 int hclStreamSynchronize(hclStream s);                            /* :115                           */
 int hclDeviceSynchronize(int device);                             /* :114                           */

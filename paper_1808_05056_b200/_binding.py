@@ -20,7 +20,7 @@ EXPORTS = [
     "hclooc_ctx_set_trace", "hclooc_ctx_get_trace", "hclooc_ctx_set_direct",
     "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_t", "hclooc_dsyrk", "hclooc_dsyr2k", "hclooc_dtrsm", "hclooc_dtrsm_plan", "hclooc_dtrsm_side", "hclooc_dpotrf", "hclooc_dpotrf_plan", "hclooc_dgemm_fig2", "hclooc_dgemm_nsteps", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
     "hclStreamDestroy", "hclEventDestroy", "hclMemcpy", "hclMemcpyAsync", "hclMemcpy2DAsync",
-    "hclDgemmAsync", "hclDgemmAsyncEx", "hclDgemmAsyncT", "hclWaitEvent", "hclStreamSynchronize", "hclDeviceSynchronize",
+    "hclDgemmAsync", "hclDgemmAsyncEx", "hclDgemmAsyncT", "hclDtrsmAsync", "hclDpotrfAsync", "hclWaitEvent", "hclStreamSynchronize", "hclDeviceSynchronize",
     "hclooc_host_alloc", "hclooc_host_free", "hclooc_host_register", "hclooc_host_unregister",
     "hclooc_strerror", "hclooc_last_cuda_error", "hclooc_version", "hclooc_probe_fp64",
 ]
@@ -111,6 +111,8 @@ def lib():
         L.hclDgemmAsync.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, vp, POINTER(vp)]
         L.hclDgemmAsyncEx.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, vp, POINTER(vp), c_int]
         L.hclDgemmAsyncT.argtypes = [c_int, c_int, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, vp, POINTER(vp), c_int]
+        L.hclDtrsmAsync.argtypes = [c_int, c_int, c_int, c_int, i64, i64, dbl, vp, i64, vp, i64, vp, POINTER(vp)]
+        L.hclDpotrfAsync.argtypes = [c_int, i64, vp, i64, vp, vp, POINTER(vp)]
         L.hclWaitEvent.argtypes = [vp, vp]
         L.hclStreamSynchronize.argtypes = [vp]
         L.hclDeviceSynchronize.argtypes = [c_int]
@@ -453,6 +455,18 @@ def hclDgemmAsync(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, stream=None, 
     ev = _ev(want_event, event)
     _check(lib().hclDgemmAsync(M, N, K, alpha, _ptr(dA), lda, _ptr(dB), ldb, beta, _ptr(dC), ldc, _ptr(stream),
                                byref(ev) if ev is not None else None), "hclDgemmAsync")
+    return ev.value if ev is not None else None
+
+
+def hclDtrsmAsync(side, uplo, trans, diag, M, N, alpha, dA, lda, dB, ldb, stream=None, want_event=False, event=None):
+    ev = _ev(want_event, event)
+    _check(lib().hclDtrsmAsync(side, uplo, trans, diag, M, N, alpha, _ptr(dA), lda, _ptr(dB), ldb, _ptr(stream), byref(ev) if ev is not None else None), "hclDtrsmAsync")
+    return ev.value if ev is not None else None
+
+
+def hclDpotrfAsync(uplo, N, dA, lda, d_info, stream=None, want_event=False, event=None):
+    ev = _ev(want_event, event)
+    _check(lib().hclDpotrfAsync(uplo, N, _ptr(dA), lda, _ptr(d_info), _ptr(stream), byref(ev) if ev is not None else None), "hclDpotrfAsync")
     return ev.value if ev is not None else None
 
 

@@ -263,7 +263,12 @@ extern "C" int hclooc_ctx_create(hclooc_ctx** out, int device, void* d_workspace
     c->workspace = d_workspace;
     c->workspace_bytes = workspace_bytes;
     c->owns_workspace = false;
-    auto mk = [](cudaStream_t* s) { return cudaStreamCreateWithFlags(s, cudaStreamNonBlocking); };
+    // library-owned streams get the HIGHEST priority: the pipeline is latency sensitive (a kernel that waits for an SM holds its C
+    // buffer and with it the uploads behind), while the device phases that run beside it in hclooc_dpotrf / hclooc_dtrsm (big
+    // recursive-solve launches on the auxiliary streams, default priority) have slack of a whole pipeline call
+    int prio_lo = 0, prio_hi = 0;
+    cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
+    auto mk = [prio_hi](cudaStream_t* s) { return cudaStreamCreateWithPriority(s, cudaStreamNonBlocking, prio_hi); };
     cudaError_t e = cudaSuccess;
     if (stream_h2d) c->s_h2d = (cudaStream_t)stream_h2d; else { e = mk(&c->s_h2d); c->owns_h2d = true; }
     if (e == cudaSuccess) { if (stream_d2h) c->s_d2h = (cudaStream_t)stream_d2h; else { e = mk(&c->s_d2h); c->owns_d2h = true; } }
@@ -295,6 +300,9 @@ extern "C" int hclooc_ctx_destroy(hclooc_ctx* c) {
     if (c->owns_compute) for (int i = 0; i < c->n_compute; ++i) if (c->s_compute[i]) cudaStreamDestroy(c->s_compute[i]);
     if (c->owns_workspace && c->workspace) cudaFree(c->workspace);
     if (c->res_c) cudaFree(c->res_c);
+    for (cudaStream_t st : c->s_aux) if (st) cudaStreamDestroy(st);
+    for (cudaEvent_t e : c->ev_aux) if (e) cudaEventDestroy(e);
+    if (c->h_word) cudaFreeHost(c->h_word);
     delete c;
     return HCLOOC_OK;
 }
@@ -362,7 +370,7 @@ int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, in
 // device work between them: hclooc_dtrsm, hclooc_dpotrf); ctx must not be NULL
 int dgemm_core_locked(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
                       int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
-                      size_t device_budget_bytes, hclooc_stats* stats, int tri) {
+                      size_t device_budget_bytes, hclooc_stats* stats, int tri, const DgemmExtra* extra) {
     const auto t_begin = std::chrono::steady_clock::now();
     // ---------------------------------------------------------------- S0 validate (argument numbers of hclooc_dgemm)
     if (M < 0) return -1;
@@ -426,7 +434,9 @@ int dgemm_core_locked(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_
                            C_alias && (((uintptr_t)C_alias & 15u) == 0) &&
                            (scale_only || (A_alias && B_alias && ((((uintptr_t)A_alias | (uintptr_t)B_alias) & 15u) == 0)));
     {
-        const int where = in_core ? 1 : (c_dev ? 2 : (direct_ok ? (direct_mode == 1 ? 4 : 3) : 0));
+        const bool c_in_host = extra && extra->C_src;
+        if (c_in_host && (!c_dev || in_core || beta == 0.0 || scale_only)) return HCLOOC_ERR_INTERNAL;
+        const int where = in_core ? 1 : (c_dev ? (c_in_host ? 5 : 2) : (direct_ok ? (direct_mode == 1 ? 4 : 3) : 0));
         const hclooc_ctx::PlanKey key{M, N, K, beta != 0.0 || tri != 0, alpha == 0.0, where + (transa ? 8 : 0) + (transb ? 16 : 0) + 32 * tri, budget};
         bool hit = false;
         for (const auto& kv : ctx->plan_cache) {
@@ -508,7 +518,7 @@ int dgemm_core_locked(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_
         for (const hclooc_op_t& o : ctx->ops) {
             const uint64_t bytes = (uint64_t)o.nr * (uint64_t)o.nc * 8;
             if (o.kind == HCLOOC_OP_H2D_A || o.kind == HCLOOC_OP_H2D_B) { up += bytes; ++nup; }
-            else if (o.kind == HCLOOC_OP_H2D_C) { if (!c_dev) up += bytes; ++nup; }
+            else if (o.kind == HCLOOC_OP_H2D_C) { if (!c_dev || (extra && extra->C_src && o.step < P.h * P.w)) up += bytes; ++nup; }
             else if (o.kind == HCLOOC_OP_D2H_C) { if (!c_dev) down += bytes; ++ndown; }
         }
         P.bytes_h2d = up; P.bytes_d2h = down; P.n_copies_h2d = nup; P.n_copies_d2h = ndown;
@@ -516,6 +526,8 @@ int dgemm_core_locked(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_
     for (int i = 0; i < P.n_scratch && i < ctx->n_compute; ++i)   // stream-K tile counters start at zero
         HCL_CUDA(cudaMemsetAsync(scratch[i] + streamk_counter_offset(), 0, streamk_counter_bytes(), ctx->s_compute[i]));
     auto stream_of = [&](int s) { return s == 0 ? ctx->s_h2d : (s == 1 ? ctx->s_d2h : ctx->s_compute[s - 2]); };
+    if (extra)       // every store into C goes through the in-order D2H stream: its first one waits for the buffer's previous tenant
+        for (cudaEvent_t e : extra->wait_before_store) if (e) HCL_CUDA(cudaStreamWaitEvent(ctx->s_d2h, e, 0));
     uint64_t bytes_h2d = 0, bytes_d2h = 0, n_h2d = 0, n_d2h = 0, n_kernels = 0;
     const auto t_enq0 = std::chrono::steady_clock::now();
     rc = HCLOOC_OK;
@@ -523,7 +535,7 @@ int dgemm_core_locked(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_
     // Latency-bound schedules (many small operations: config 1) are captured once as a CUDA graph and replayed when
     // the very same call comes again; long schedules gain nothing (their enqueue time hides behind the transfers).
     static const int graph_mode = [] { const char* e = std::getenv("HCLOOC_GRAPH"); return e ? std::atoi(e) : -1; }();
-    bool use_graph = !trace && !scale_only && P.n_scratch == 0 &&
+    bool use_graph = !trace && !extra && !scale_only && P.n_scratch == 0 &&
                      (graph_mode == 1 || (graph_mode < 0 && P.n_steps <= 512 && P.t_model_s < 5e-3));
     std::vector<int64_t> key;
     if (!use_graph) { ctx->graph_key.clear(); ctx->graph_valid = false; }
@@ -608,6 +620,11 @@ int dgemm_core_locked(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_
                 bytes_h2d += (uint64_t)o.nr * o.nc * 8; ++n_h2d;
                 break;
             case HCLOOC_OP_H2D_C:
+                if (extra && extra->C_src && o.step < P.h * P.w) {        // K panel 0: the initial C comes from the host matrix
+                    rc = copy2d(bufs[o.buf], (size_t)P.ldc_dev * 8, extra->C_src + o.r0 * extra->ldc_src + o.c0, (size_t)extra->ldc_src * 8, (size_t)o.nc * 8, (size_t)o.nr, st);
+                    bytes_h2d += (uint64_t)o.nr * o.nc * 8; ++n_h2d;
+                    break;
+                }
                 rc = copy2d(bufs[o.buf], (size_t)P.ldc_dev * 8, C + o.r0 * ldc + o.c0, (size_t)ldc * 8, (size_t)o.nc * 8, (size_t)o.nr, st);
                 if (!c_dev) bytes_h2d += (uint64_t)o.nr * o.nc * 8;   // device-resident C: not link traffic
                 ++n_h2d;
@@ -819,6 +836,13 @@ int resolve_budget(hclooc_ctx* ctx, size_t device_budget_bytes, size_t* budget_o
         budget = fr > 2 * margin ? fr - margin : fr / 2;
     }
     *budget_out = budget;
+    return HCLOOC_OK;
+}
+
+int ensure_aux(hclooc_ctx* ctx) {
+    for (cudaStream_t& st : ctx->s_aux) if (!st) HCL_CUDA(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
+    for (cudaEvent_t& e : ctx->ev_aux) if (!e) HCL_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    if (!ctx->h_word) HCL_CUDA(cudaHostAlloc((void**)&ctx->h_word, 64, cudaHostAllocDefault));
     return HCLOOC_OK;
 }
 

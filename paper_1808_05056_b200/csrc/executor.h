@@ -41,6 +41,11 @@ struct hclooc_ctx {
     // bytes at the front of the workspace that a routine running several DGEMM calls keeps for itself (a resident panel of
     // hclooc_dpotrf / hclooc_dtrsm_side): dgemm_core_locked carves its buffers behind them and plans with the rest of the budget
     size_t reserved_bytes = 0;
+    // streams, events and a pinned status word of the routines with a look-ahead (factor.cu): their own device work runs beside
+    // the DGEMM pipeline, so it must not sit on the pipeline's streams (dgemm_core synchronises those); created on first use
+    cudaStream_t s_aux[4] = {};
+    cudaEvent_t ev_aux[8] = {};
+    long long* h_word = nullptr;
     std::mutex mu;
 };
 
@@ -55,15 +60,24 @@ int copy2d(void* dst, size_t dpitch, const void* src, size_t spitch, size_t widt
 // the budget a call works under: the caller's figure, clipped to a caller-owned workspace, or all free device memory less 1 GiB
 int resolve_budget(hclooc_ctx* ctx, size_t device_budget_bytes, size_t* budget, bool* library_owned);
 int ensure_workspace(hclooc_ctx* ctx, size_t bytes);
+int ensure_aux(hclooc_ctx* ctx);        // ctx->s_aux, ev_aux, h_word
 
 // C = alpha*op(A)*op(B) + beta*C through the pipeline (executor.cu).  tri != 0: only the lower (1) / upper (2) triangle of this
 // call's C -- element (0, 0) on the diagonal -- is referenced (hclooc_dsyrk, the Cholesky panel).  Takes ctx->mu itself.
 int dgemm_core(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
                int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
                size_t device_budget_bytes, hclooc_stats* stats, int tri = 0);
+// Extras of a DGEMM call made by a routine that keeps a panel in device memory: the initial C is read from C_src (a host
+// matrix, leading dimension ldc_src) while the result goes to C (device memory) -- the pipeline itself brings the panel up,
+// block by block under its kernels; and the FIRST write into C waits for these events (the previous tenant of the buffer).
+struct DgemmExtra {
+    const double* C_src = nullptr;
+    int64_t ldc_src = 0;
+    cudaEvent_t wait_before_store[2] = {nullptr, nullptr};
+};
 // the same with ctx->mu already held by the caller (ctx not NULL)
 int dgemm_core_locked(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
                       int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
-                      size_t device_budget_bytes, hclooc_stats* stats, int tri = 0);
+                      size_t device_budget_bytes, hclooc_stats* stats, int tri = 0, const DgemmExtra* extra = nullptr);
 
 }  // namespace hclooc

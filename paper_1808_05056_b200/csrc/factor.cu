@@ -14,6 +14,7 @@
 // (potrf_sm100.cu, trsm_sm100.cu).  Right-looking would move the whole trailing matrix over the link at every step.
 #include <algorithm>
 #include <chrono>
+#include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <vector>
@@ -58,10 +59,10 @@ int dev_trsm(int right, const double* dT, int64_t ldt, int lower, int trans, int
         int e;
         if (!right) {      // X[second] <- scale * X[second] - op(T)[second, first] X[first]
             const double* Tp = trans ? dT + f0 * ldt + s0 : dT + s0 * ldt + f0;
-            e = launch_dgemm_tiles(s1 - s0, w, f1 - f0, -1.0, Tp, ldt, X + f0 * ld, ld, r.scale, X + s0 * ld, ld, st, 1, nullptr, trans ? 1 : 0, 0);
+            e = launch_dgemm_tiles(s1 - s0, w, f1 - f0, -1.0, Tp, ldt, X + f0 * ld, ld, r.scale, X + s0 * ld, ld, st, 0, nullptr, trans ? 1 : 0, 0);
         } else {           // X[:, second] <- scale * X[:, second] - X[:, first] op(T)[first, second]
             const double* Tp = trans ? dT + s0 * ldt + f0 : dT + f0 * ldt + s0;
-            e = launch_dgemm_tiles(w, s1 - s0, f1 - f0, -1.0, X + f0, ld, Tp, ldt, r.scale, X + s0, ld, st, 1, nullptr, 0, trans ? 1 : 0);
+            e = launch_dgemm_tiles(w, s1 - s0, f1 - f0, -1.0, X + f0, ld, Tp, ldt, r.scale, X + s0, ld, st, 0, nullptr, 0, trans ? 1 : 0);
         }
         if (e) return e;
         ++*n_kernels;
@@ -103,6 +104,26 @@ struct Reserve {
     ~Reserve() { ctx->reserved_bytes = 0; }
 };
 
+// HCLOOC_FACTOR_TIMING: where the time of one pipeline call went (from the context's trace records)
+void trace_summary(hclooc_ctx* ctx, const char* what) {
+    static const char* names[] = {"H2D_A", "H2D_B", "H2D_C", "GEMM", "D2H_C"};
+    for (int kind = 0; kind < 5; ++kind) {
+        double first = 1e30, last = 0, busy = 0, cur_s = -1, cur_e = -1;
+        size_t n = 0;
+        uint64_t bytes = 0;
+        std::vector<std::pair<double, double>> iv;
+        for (const hclooc_trace_rec& r : ctx->trace_recs) if (r.kind == kind) { iv.emplace_back(r.t_start_ms, r.t_end_ms); bytes += r.bytes; ++n; }
+        if (!n) continue;
+        std::sort(iv.begin(), iv.end());
+        for (auto& p : iv) {
+            first = std::min(first, p.first); last = std::max(last, p.second);
+            if (p.first > cur_e) { if (cur_e >= 0) busy += cur_e - cur_s; cur_s = p.first; cur_e = p.second; } else cur_e = std::max(cur_e, p.second);
+        }
+        busy += cur_e - cur_s;
+        std::fprintf(stderr, "    %s %s: %zu ops, first start %.2f ms, last end %.2f ms, busy %.2f ms, %.3f GB\n", what, names[kind], n, first, last, busy, bytes / 1e9);
+    }
+}
+
 void add_stats(hclooc_stats& acc, const hclooc_stats& one, double* t_enq) {
     acc.bytes_h2d += one.bytes_h2d; acc.bytes_d2h += one.bytes_d2h; acc.n_kernels += one.n_kernels;
     acc.n_copies_h2d += one.n_copies_h2d; acc.n_copies_d2h += one.n_copies_d2h; *t_enq += one.t_enqueue_s;
@@ -116,7 +137,8 @@ size_t round_1k(size_t x) { return (x + 1023) & ~(size_t)1023; }
 int potrf_nb(int64_t N, size_t budget, int64_t* nb_out) {
     static const int64_t nb_env = [] { const char* e = std::getenv("HCLOOC_POTRF_NB"); const long v = e ? std::atol(e) : 0; return v >= 32 ? (int64_t)(v / 32 * 32) : (int64_t)0; }();
     int64_t NB = nb_env ? nb_env : 4096;
-    auto fits = [&](int64_t nb) { return round_1k((size_t)N * round_even(nb) * 8) + 2048 <= budget / 2; };
+    // two resident panels (one if a single panel covers the matrix) in at most half the budget
+    auto fits = [&](int64_t nb) { return (nb >= N ? 1 : 2) * round_1k((size_t)N * round_even(nb) * 8) <= budget / 2; };
     while (NB > 128 && !fits(NB)) NB -= 128;
     while (NB > 32 && !fits(NB)) NB -= 32;
     if (!fits(NB)) return HCLOOC_ERR_BUDGET;
@@ -127,12 +149,62 @@ int potrf_nb(int64_t N, size_t budget, int64_t* nb_out) {
 
 }  // namespace
 
+// ---------------------------------------------------------------------------------------------------------------------
+// The device phases on their own: in-core DTRSM and DPOTRF on DEVICE pointers, asynchronous on the caller's stream -- what
+// hclDgemmAsync is to hclooc_dgemm (the paper's runtime has the in-core kernel as a call of its own).
+extern "C" int hclDtrsmAsync(int side, int uplo, int trans, int diag, int64_t M, int64_t N, double alpha, const double* dA, int64_t lda,
+                             double* dB, int64_t ldb, hclStream s, hclEvent* ev) {
+    if (side != HCL_SIDE_LEFT && side != HCL_SIDE_RIGHT) return -1;
+    if (uplo != HCL_UPLO_LOWER && uplo != HCL_UPLO_UPPER) return -2;
+    if (trans != HCL_OP_N && trans != HCL_OP_T) return -3;
+    if (diag != HCL_DIAG_NONUNIT && diag != HCL_DIAG_UNIT) return -4;
+    if (M < 0) return -5;
+    if (N < 0) return -6;
+    const int64_t n = side == HCL_SIDE_LEFT ? M : N;
+    if (M > 0 && N > 0) {
+        if (!dA) return -8;
+        if (lda < n) return -9;
+        if (!dB) return -10;
+        if (ldb < N) return -11;
+        if (((uintptr_t)dA & 15u) || ((uintptr_t)dB & 15u) || (lda & 1) || (ldb & 1)) return HCLOOC_ERR_ALIGN;
+        uint64_t nk = 0;
+        const int lower_op = (uplo == HCL_UPLO_LOWER) != (trans == HCL_OP_T);
+        int rc = dev_trsm(side == HCL_SIDE_RIGHT, dA, lda, lower_op, trans, diag, dB, ldb, side == HCL_SIDE_LEFT ? N : M, n, alpha, (cudaStream_t)s, &nk);
+        if (rc) return rc;
+    }
+    if (ev) {
+        if (!*ev) { cudaEvent_t e; HCL_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming)); *ev = (hclEvent)e; }
+        HCL_CUDA(cudaEventRecord((cudaEvent_t)*ev, (cudaStream_t)s));
+    }
+    return HCLOOC_OK;
+}
+
+extern "C" int hclDpotrfAsync(int uplo, int64_t N, double* dA, int64_t lda, long long* d_info, hclStream s, hclEvent* ev) {
+    if (uplo != HCL_UPLO_LOWER && uplo != HCL_UPLO_UPPER) return -1;
+    if (N < 0) return -2;
+    if (!d_info) return -5;
+    if (N > 0) {
+        if (!dA) return -3;
+        if (lda < N) return -4;
+        if (((uintptr_t)dA & 15u) || (lda & 1)) return HCLOOC_ERR_ALIGN;
+        uint64_t nk = 0;
+        HCL_CUDA(cudaMemsetAsync(d_info, 0, sizeof(long long), (cudaStream_t)s));
+        int rc = dev_potrf(dA, lda, N, uplo == HCL_UPLO_LOWER ? 1 : 0, d_info, 0, (cudaStream_t)s, &nk);
+        if (rc) return rc;
+    }
+    if (ev) {
+        if (!*ev) { cudaEvent_t e; HCL_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming)); *ev = (hclEvent)e; }
+        HCL_CUDA(cudaEventRecord((cudaEvent_t)*ev, (cudaStream_t)s));
+    }
+    return HCLOOC_OK;
+}
+
 extern "C" int hclooc_dpotrf_plan(int64_t N, size_t device_budget_bytes, int64_t* NB, uint64_t* panel_bytes) {
     if (N < 1) return -1;
     if (!NB || !panel_bytes) return -3;
     int rc = potrf_nb(N, device_budget_bytes, NB);
     if (rc) return rc;
-    *panel_bytes = round_1k((size_t)N * round_even(*NB) * 8) + 1024;
+    *panel_bytes = (*NB >= N ? 1 : 2) * round_1k((size_t)N * round_even(*NB) * 8) + 1024;
     return HCLOOC_OK;
 }
 
@@ -158,65 +230,171 @@ extern "C" int hclooc_dpotrf(hclooc_ctx* ctx, int uplo, int64_t N, double* A, in
     if ((rc = resolve_budget(ctx, device_budget_bytes, &budget, &own))) return rc;
     int64_t NB = 0;
     if ((rc = potrf_nb(N, budget, &NB))) return rc;
+    if ((rc = ensure_aux(ctx))) return rc;
     const bool lower = uplo == HCL_UPLO_LOWER;
-    // the resident panel: (N - c0) x nbj for the lower factor (a block column), nbj x (N - c0) for the upper one (a block row)
+    const int64_t nblk = (N + NB - 1) / NB;
+    // TWO resident panels (one when the matrix is a single panel): panel j is factored in one while panel j+1 is uploaded into the
+    // other and receives its out-of-core update.  Lower: (N - c0) x nbj, a block column; upper: nbj x (N - c0), a block row.
+    const int npan = nblk > 1 ? 2 : 1;
     const size_t panel_bytes = lower ? round_1k((size_t)N * round_even(NB) * 8) : round_1k((size_t)NB * round_even(N) * 8);
-    const size_t reserved = panel_bytes + 1024;                   // + the info word
+    const size_t reserved = npan * panel_bytes + 1024;            // + the info word
     if (own) { if ((rc = ensure_workspace(ctx, budget))) return rc; }
     uint8_t* base = (uint8_t*)ctx->workspace;
     const uintptr_t mis = (uintptr_t)base & 1023u;
     const size_t shift = mis ? 1024 - mis : 0;
     if (reserved + shift > ctx->workspace_bytes) return HCLOOC_ERR_BUDGET;
-    double* dP = (double*)(base + shift);
-    long long* d_info = (long long*)(base + shift + panel_bytes);
+    double* dPan[2] = {(double*)(base + shift), (double*)(base + shift + (npan - 1) * panel_bytes)};
+    long long* d_info = (long long*)(base + shift + npan * panel_bytes);
     Reserve guard(ctx, reserved + shift);
-    while (ctx->events.size() < 3) {
-        cudaEvent_t e;
-        HCL_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
-        ctx->events.push_back(e);
-    }
-    cudaStream_t sc = ctx->s_compute[0];
-    HCL_CUDA(cudaMemsetAsync(d_info, 0, sizeof(long long), sc));
+    // streams of this routine's own device work (the DGEMM pipeline keeps its own): diagonal phases, panel uploads, panel downloads
+    cudaStream_t s_diag = ctx->s_aux[0], s_up = ctx->s_aux[1], s_down = ctx->s_aux[2], s_pot = ctx->s_aux[3];
+    cudaEvent_t ev_up[2] = {ctx->ev_aux[0], ctx->ev_aux[1]}, ev_down[2] = {ctx->ev_aux[2], ctx->ev_aux[3]};
+    cudaEvent_t ev_diag = ctx->ev_aux[4], ev_upd2 = ctx->ev_aux[5], ev_2a = ctx->ev_aux[6], ev_pot = ctx->ev_aux[7];
+    struct Drain {      // whatever happens, nothing of this call is left running when it returns
+        hclooc_ctx* c;
+        ~Drain() { for (cudaStream_t st : c->s_aux) if (st) cudaStreamSynchronize(st); }
+    } drain{ctx};
+    static const bool timing = std::getenv("HCLOOC_FACTOR_TIMING") != nullptr;
+    HCL_CUDA(cudaMemsetAsync(d_info, 0, sizeof(long long), s_diag));
+    *ctx->h_word = 0;
     hclooc_stats acc;
     std::memset(&acc, 0, sizeof(acc));
     double t_enq = 0.0;
     size_t ws_max = reserved;
-    const int64_t nblk = (N + NB - 1) / NB;
+    auto geom = [&](int64_t bj, int64_t* c0, int64_t* nbj, int64_t* prow, int64_t* pcol, int64_t* ldp) {
+        *c0 = bj * NB; *nbj = std::min(NB, N - *c0);
+        const int64_t rest = N - *c0;
+        *prow = lower ? rest : *nbj; *pcol = lower ? *nbj : rest; *ldp = round_even(*pcol);
+    };
+    auto upload = [&](int64_t bj, int buf) -> int {
+        int64_t c0, nbj, prow, pcol, ldp;
+        geom(bj, &c0, &nbj, &prow, &pcol, &ldp);
+        int e = copy2d(dPan[buf], (size_t)ldp * 8, A + c0 * lda + c0, (size_t)lda * 8, (size_t)pcol * 8, (size_t)prow, s_up);
+        if (e) return e;
+        acc.bytes_h2d += (uint64_t)prow * pcol * 8; ++acc.n_copies_h2d;
+        HCL_CUDA(cudaEventRecord(ev_up[buf], s_up));
+        return HCLOOC_OK;
+    };
+    if ((rc = upload(0, 0))) return rc;
     long long h_info = 0;
     for (int64_t bj = 0; bj < nblk; ++bj) {
-        const int64_t c0 = bj * NB, nbj = std::min(NB, N - c0), rest = N - c0;
-        // panel on the host: lower: A[c0:N, c0:c0+nbj] (rest x nbj); upper: A[c0:c0+nbj, c0:N] (nbj x rest)
-        double* hP = A + c0 * lda + c0;
-        const int64_t prow = lower ? rest : nbj, pcol = lower ? nbj : rest, ldp = round_even(pcol);
-        if ((rc = copy2d(dP, (size_t)ldp * 8, hP, (size_t)lda * 8, (size_t)pcol * 8, (size_t)prow, ctx->s_h2d))) return rc;
-        acc.bytes_h2d += (uint64_t)prow * pcol * 8; ++acc.n_copies_h2d;
-        HCL_CUDA(cudaStreamSynchronize(ctx->s_h2d));               // the DGEMM's own streams do not wait for this one
-        if (c0 > 0) {
-            // the contribution of the block columns (rows) already factored, on the referenced triangle of the panel only:
-            //   lower:  P <- P - L[c0:N, 0:c0] * L[c0:c0+nbj, 0:c0]^T          upper:  P <- P - U[0:c0, c0:c0+nbj]^T * U[0:c0, c0:N]
-            hclooc_stats one;
-            if (lower) rc = dgemm_core_locked(ctx, 0, 1, rest, nbj, c0, -1.0, A + c0 * lda, lda, A + c0 * lda, lda, 1.0, dP, ldp, budget, &one, 1);
-            else rc = dgemm_core_locked(ctx, 1, 0, nbj, rest, c0, -1.0, A + c0, lda, A + c0, lda, 1.0, dP, ldp, budget, &one, 2);
-            if (rc) return rc;
-            add_stats(acc, one, &t_enq);
-            ws_max = std::max(ws_max, reserved + (size_t)one.plan.workspace_bytes);
+        const int cur = (int)(bj % npan), alt = npan - 1 - cur;
+        int64_t c0, nbj, prow, pcol, ldp;
+        geom(bj, &c0, &nbj, &prow, &pcol, &ldp);
+        const int64_t rest = N - c0;
+        double* dP = dPan[cur];
+        const auto tp0 = std::chrono::steady_clock::now();
+        // ---- panel bj: everything before it has been applied (update 1 by the pipeline, host-synchronised; update 2 on s_diag), and
+        // its diagonal block has been factored on s_pot beside the second part of update 2 (panel 0: here)
+        if (bj == 0) {
+            HCL_CUDA(cudaStreamWaitEvent(s_diag, ev_up[cur], 0));
+            if ((rc = dev_potrf(dP, ldp, nbj, lower ? 1 : 0, d_info, (long long)c0, s_diag, &acc.n_kernels))) return rc;
+        } else {
+            HCL_CUDA(cudaStreamWaitEvent(s_diag, ev_pot, 0));
         }
-        const auto te0 = std::chrono::steady_clock::now();
-        // the diagonal block, then the rest of the panel:  lower: P21 <- P21 L_jj^-T;  upper: P12 <- U_jj^-T P12
-        if ((rc = dev_potrf(dP, ldp, nbj, lower ? 1 : 0, d_info, (long long)c0, sc, &acc.n_kernels))) return rc;
-        if (rest > nbj) {
-            if (lower) rc = dev_trsm(1, dP, ldp, 0, 1, 0, dP + nbj * ldp, ldp, rest - nbj, nbj, 1.0, sc, &acc.n_kernels);
-            else rc = dev_trsm(0, dP, ldp, 1, 1, 0, dP + nbj, ldp, rest - nbj, nbj, 1.0, sc, &acc.n_kernels);
+        if (rest > nbj) {       // the rest of the panel against the diagonal block:  lower: P21 <- P21 L_jj^-T;  upper: P12 <- U_jj^-T P12
+            if (lower) rc = dev_trsm(1, dP, ldp, 0, 1, 0, dP + nbj * ldp, ldp, rest - nbj, nbj, 1.0, s_diag, &acc.n_kernels);
+            else rc = dev_trsm(0, dP, ldp, 1, 1, 0, dP + nbj, ldp, rest - nbj, nbj, 1.0, s_diag, &acc.n_kernels);
             if (rc) return rc;
         }
-        HCL_CUDA(cudaMemcpyAsync(&h_info, d_info, sizeof(long long), cudaMemcpyDeviceToHost, sc));
-        HCL_CUDA(cudaStreamSynchronize(sc));
-        t_enq += std::chrono::duration<double>(std::chrono::steady_clock::now() - te0).count();
-        if (h_info != 0) break;                                     // not positive definite: the panel is not written back
-        if ((rc = copy2d(hP, (size_t)lda * 8, dP, (size_t)ldp * 8, (size_t)pcol * 8, (size_t)prow, ctx->s_d2h))) return rc;
-        acc.bytes_d2h += (uint64_t)prow * pcol * 8; ++acc.n_copies_d2h;
-        HCL_CUDA(cudaStreamSynchronize(ctx->s_d2h));
+        HCL_CUDA(cudaMemcpyAsync(ctx->h_word, d_info, sizeof(long long), cudaMemcpyDeviceToHost, s_diag));
+        HCL_CUDA(cudaEventRecord(ev_diag, s_diag));
+        // ---- panel bj goes down as soon as it is final, beside everything that follows (a panel that failed goes down too: its
+        // leading columns are the factor's, LAPACK leaves the rest undefined).  Only what the factorization owns is written: the
+        // diagonal block goes down in strips of 128 rows cut at the diagonal tile -- the panel's blocks that lie wholly in the other
+        // triangle were never brought up (the pipeline has no step for them), and the host keeps its bits there.
+        HCL_CUDA(cudaStreamWaitEvent(s_down, ev_diag, 0));
+        {
+            double* hP = A + c0 * lda + c0;
+            for (int64_t r = 0; r < nbj; r += 128) {
+                const int64_t rr = std::min<int64_t>(128, nbj - r);
+                if (lower) rc = copy2d(hP + r * lda, (size_t)lda * 8, dP + r * ldp, (size_t)ldp * 8, (size_t)(r + rr) * 8, (size_t)rr, s_down);
+                else rc = copy2d(hP + r * lda + r, (size_t)lda * 8, dP + r * ldp + r, (size_t)ldp * 8, (size_t)(rest - r) * 8, (size_t)rr, s_down);
+                if (rc) return rc;
+                acc.bytes_d2h += (uint64_t)rr * (lower ? r + rr : rest - r) * 8; ++acc.n_copies_d2h;
+            }
+            if (lower && rest > nbj) {
+                if ((rc = copy2d(hP + nbj * lda, (size_t)lda * 8, dP + nbj * ldp, (size_t)ldp * 8, (size_t)nbj * 8, (size_t)(rest - nbj), s_down))) return rc;
+                acc.bytes_d2h += (uint64_t)(rest - nbj) * nbj * 8; ++acc.n_copies_d2h;
+            }
+        }
+        HCL_CUDA(cudaEventRecord(ev_down[cur], s_down));
+        // ---- meanwhile panel bj+1 comes up into the other buffer and receives the contribution of the panels BEFORE bj from the
+        // host: ONE out-of-core DGEMM whose C blocks are read from the host matrix and stored into the device panel (the pipeline
+        // itself brings the panel up, under its kernels); its first store waits until the buffer's previous tenant, panel bj-1, has
+        // been downloaded and read by the update 2 of panel bj
+        int64_t c0n = 0, nbn = 0, prown = 0, pcoln = 0, ldpn = 0;
+        bool uploaded_whole = false;
+        if (bj + 1 < nblk) {
+            geom(bj + 1, &c0n, &nbn, &prown, &pcoln, &ldpn);
+            if (c0 > 0) {
+                //   lower:  P <- P - L[c0n:N, 0:c0] * L[c0n:c0n+nbn, 0:c0]^T        upper:  P <- P - U[0:c0, c0n:c0n+nbn]^T * U[0:c0, c0n:N]
+                // (the 128 x 128 tiles on the panel's diagonal come up whole first: the pipeline brings only the blocks of ITS plan
+                // that touch the referenced triangle, and the strips that go down later are cut at these tiles)
+                HCL_CUDA(cudaStreamWaitEvent(s_up, ev_down[alt], 0));
+                HCL_CUDA(cudaStreamWaitEvent(s_up, ev_upd2, 0));
+                for (int64_t r = 0; r < nbn; r += 128) {
+                    const int64_t rr = std::min<int64_t>(128, nbn - r);
+                    if ((rc = copy2d(dPan[alt] + r * ldpn + r, (size_t)ldpn * 8, A + (c0n + r) * lda + c0n + r, (size_t)lda * 8, (size_t)rr * 8, (size_t)rr, s_up))) return rc;
+                    acc.bytes_h2d += (uint64_t)rr * rr * 8; ++acc.n_copies_h2d;
+                }
+                HCL_CUDA(cudaEventRecord(ev_up[alt], s_up));
+                hclooc_stats one;
+                DgemmExtra ex;
+                ex.C_src = A + c0n * lda + c0n; ex.ldc_src = lda;
+                ex.wait_before_store[0] = ev_up[alt];
+                const bool trace_was = ctx->trace;
+                if (timing) ctx->trace = true;
+                if (lower) rc = dgemm_core_locked(ctx, 0, 1, N - c0n, nbn, c0, -1.0, A + c0n * lda, lda, A + c0n * lda, lda, 1.0, dPan[alt], ldpn, budget, &one, 1, &ex);
+                else rc = dgemm_core_locked(ctx, 1, 0, nbn, N - c0n, c0, -1.0, A + c0n, lda, A + c0n, lda, 1.0, dPan[alt], ldpn, budget, &one, 2, &ex);
+                ctx->trace = trace_was;
+                if (rc) return rc;
+                if (timing) trace_summary(ctx, "update 1");
+                add_stats(acc, one, &t_enq);
+                ws_max = std::max(ws_max, reserved + (size_t)one.plan.workspace_bytes);
+                if (timing) std::fprintf(stderr, "  update %lld x %lld x %lld: %.2f ms (%.1f TFLOP/s), plan %lld x %lld blocks of %lld x %lld, %d C / %d A / %d B buffers, ksplit %d, %.2f GB up\n",
+                                         (long long)(lower ? N - c0n : nbn), (long long)(lower ? nbn : N - c0n), (long long)c0, 1e3 * one.t_total_s,
+                                         2e-12 * (double)(N - c0n) * nbn * c0 / one.t_total_s, (long long)one.plan.h, (long long)one.plan.w, (long long)one.plan.mb,
+                                         (long long)one.plan.nb, one.plan.n_sets, one.plan.n_abuf, one.plan.n_bbuf, one.plan.ksplit, one.bytes_h2d / 1e9);
+            } else {            // panel 1: nothing before panel 0, it just comes up whole (the buffer has had no tenant yet)
+                if ((rc = upload(bj + 1, alt))) return rc;
+                uploaded_whole = true;
+            }
+        }
+        const auto tp1 = std::chrono::steady_clock::now();
+        HCL_CUDA(cudaEventSynchronize(ev_diag));
+        h_info = *ctx->h_word;
+        if (timing) {
+            const auto tp2 = std::chrono::steady_clock::now();
+            std::fprintf(stderr, "dpotrf panel %lld: upload + out-of-core update of the next panel %.2f ms, then %.2f ms more for the diagonal phase\n",
+                         (long long)bj, 1e3 * std::chrono::duration<double>(tp1 - tp0).count(), 1e3 * std::chrono::duration<double>(tp2 - tp1).count());
+        }
+        if (h_info != 0) break;                                     // not positive definite
+        // ---- panel bj+1 receives panel bj's contribution straight from device memory (update 2): first its diagonal block, which
+        // is then factored on a stream of its own WHILE the rest of the panel is updated (the factorization of a 4096-block is a chain
+        // of small launches that leaves nearly every SM idle)
+        if (bj + 1 < nblk) {
+            if (uploaded_whole) HCL_CUDA(cudaStreamWaitEvent(s_diag, ev_up[alt], 0));
+            const int64_t below = N - c0n - nbn;                  // rows (lower) / columns (upper) of panel bj+1 past its diagonal block
+            //   lower:  P' <- P' - L[c0n:N, c0:c0n] * L[c0n:c0n+nbn, c0:c0n]^T, both operands = rows nbj.. of the panel just factored
+            if (lower) rc = launch_dgemm_tiles(nbn, nbn, nbj, -1.0, dP + nbj * ldp, ldp, dP + nbj * ldp, ldp, 1.0, dPan[alt], ldpn, s_diag, 0, nullptr, 0, 1, 1, 0);
+            else rc = launch_dgemm_tiles(nbn, nbn, nbj, -1.0, dP + nbj, ldp, dP + nbj, ldp, 1.0, dPan[alt], ldpn, s_diag, 0, nullptr, 1, 0, 2, 0);
+            if (rc) return rc;
+            ++acc.n_kernels;
+            HCL_CUDA(cudaEventRecord(ev_2a, s_diag));
+            HCL_CUDA(cudaStreamWaitEvent(s_pot, ev_2a, 0));
+            if ((rc = dev_potrf(dPan[alt], ldpn, nbn, lower ? 1 : 0, d_info, (long long)c0n, s_pot, &acc.n_kernels))) return rc;
+            HCL_CUDA(cudaEventRecord(ev_pot, s_pot));
+            if (below > 0) {
+                if (lower) rc = launch_dgemm_tiles(below, nbn, nbj, -1.0, dP + (nbj + nbn) * ldp, ldp, dP + nbj * ldp, ldp, 1.0, dPan[alt] + nbn * ldpn, ldpn, s_diag, 0, nullptr, 0, 1);
+                else rc = launch_dgemm_tiles(nbn, below, nbj, -1.0, dP + nbj, ldp, dP + nbj + nbn, ldp, 1.0, dPan[alt] + nbn, ldpn, s_diag, 0, nullptr, 1, 0);
+                if (rc) return rc;
+                ++acc.n_kernels;
+            }
+            HCL_CUDA(cudaEventRecord(ev_upd2, s_diag));
+        }
     }
+    for (cudaStream_t st : {s_diag, s_up, s_down, s_pot}) HCL_CUDA(cudaStreamSynchronize(st));
     *info = (int64_t)h_info;
     if (stats) {
         *stats = acc;
@@ -224,7 +402,7 @@ extern "C" int hclooc_dpotrf(hclooc_ctx* ctx, int uplo, int64_t N, double* A, in
         stats->plan.mb = lower ? N : NB; stats->plan.nb = lower ? NB : N; stats->plan.kb = 128;
         stats->plan.h = lower ? 1 : nblk; stats->plan.w = lower ? nblk : 1; stats->plan.kpanels = 1; stats->plan.n_steps = nblk;
         stats->plan.workspace_bytes = ws_max;
-        stats->plan.n_sets = 1;
+        stats->plan.n_sets = npan;
         stats->plan.bytes_h2d = acc.bytes_h2d; stats->plan.bytes_d2h = acc.bytes_d2h;
         stats->plan.n_copies_h2d = acc.n_copies_h2d; stats->plan.n_copies_d2h = acc.n_copies_d2h;
         stats->plan.flops = (double)N * (double)N * (double)N / 3.0;

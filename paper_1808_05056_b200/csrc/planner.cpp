@@ -59,6 +59,7 @@ struct Cand {
     int n_sets, n_abuf, n_bbuf, ksplit, n_scratch;
     bool ta;              // A is stored K x M: its slices are uploaded as kb rows of mb doubles (narrow rows when mb is small)
     bool c_dev;           // C lives in device memory: its block copies are device-to-device, not host-link traffic
+    bool c_in_host;       // ... except the uploads of K panel 0, which read the initial C from a HOST matrix (operands_on_device = 5)
     int64_t lda_dev, ldb_dev, ldc_dev;
     uint64_t a_bytes, b_bytes, c_bytes, ws_bytes;
     uint64_t bytes_h2d, bytes_d2h, n_h2d, n_d2h;
@@ -131,7 +132,7 @@ void fill_traffic(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool s
         }
     }
     const uint64_t MNlink = c.c_dev ? 0 : MN;                                   // copies are still enqueued, bytes are not link bytes
-    if (beta_nz) { el_h2d += MNlink; n_h2d += (uint64_t)c.h * c.w; }
+    if (beta_nz) { el_h2d += c.c_in_host ? MN : MNlink; n_h2d += (uint64_t)c.h * c.w; }
     if (c.kpanels > 1) { el_h2d += (uint64_t)(c.kpanels - 1) * MNlink; n_h2d += (uint64_t)(c.kpanels - 1) * c.h * c.w; }
     c.bytes_h2d = 8 * el_h2d;
     c.n_h2d = n_h2d;
@@ -162,7 +163,8 @@ void cost(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool scale_onl
         // 2-D copies run at full rate only from ~2 KiB per row up, and the slices of a transposed A have rows of mb
         // doubles.  Measured on config 2 with A^T: 1 KiB rows (mb = 128) move at ~35 GB/s inside the pipeline, 2 KiB rows
         // within 1.3 % of the untransposed call; alone, 128-byte rows reach 8.3 GB/s (profiles/r01_box_probe.md).
-        const double a_bytes_all = (double)c.bytes_h2d - 8.0 * (double)K * (double)N - ((beta_nz || c.kpanels > 1) && !c.c_dev ? 8.0 * (double)M * (double)N * (beta_nz ? c.kpanels : c.kpanels - 1) : 0.0);
+        const double a_bytes_all = (double)c.bytes_h2d - 8.0 * (double)K * (double)N - ((beta_nz || c.kpanels > 1) && !c.c_dev ? 8.0 * (double)M * (double)N * (beta_nz ? c.kpanels : c.kpanels - 1) : 0.0) -
+                                   (beta_nz && c.c_dev && c.c_in_host ? 8.0 * (double)M * (double)N : 0.0);
         t_in_rows = std::max(0.0, a_bytes_all) / mm.h2d_Bps * 0.45 * (2048.0 / (double)(c.mb * 8) - 1.0);
     }
     c.t_link = std::max(std::max(t_in + t_in_rows, t_out), (double)(c.bytes_h2d + c.bytes_d2h) / mm.duplex_Bps + t_in_rows);
@@ -196,12 +198,14 @@ void cost(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool scale_onl
     const double comp_col = t_compute / n_cols;
     const double a_first = scale_only ? 0.0 : 8.0 * (double)M * (double)c.kb;
     const double mn_link = c.c_dev ? 0.0 : 8.0 * (double)M * (double)N;
-    const double a_all = (double)c.bytes_h2d - 8.0 * (double)K * (double)N - (beta_nz ? mn_link : 0.0) -
+    const double mn_up0 = (c.c_dev && c.c_in_host) ? 8.0 * (double)M * (double)N : mn_link;      // C uploads of K panel 0
+    const double a_all = (double)c.bytes_h2d - 8.0 * (double)K * (double)N - (beta_nz ? mn_up0 : 0.0) -
                          (c.kpanels > 1 ? (double)(c.kpanels - 1) * mn_link : 0.0);
     const double a_later = n_cols > c.kpanels ? std::max(0.0, a_all - a_first * c.kpanels) / (n_cols - c.kpanels) : 0.0;
     const double c_col = c.c_dev ? 0.0 : 8.0 * (double)M * (double)c.nb;
+    const double c_col_up = (c.c_dev && c.c_in_host && c.kpanels == 1) ? 8.0 * (double)M * (double)c.nb : c_col;
     auto link_col = [&](double a_bytes) {
-        const double up = a_bytes * a_row_factor + (scale_only ? 0.0 : (double)c.b_bytes) + (cload ? c_col : 0.0);
+        const double up = a_bytes * a_row_factor + (scale_only ? 0.0 : (double)c.b_bytes) + (cload ? c_col_up : 0.0);
         const double lat = (double)c.h * 2.0 * mm.copy_latency_s;
         return std::max(std::max(up / mm.h2d_Bps, c_col / mm.d2h_Bps), (up + c_col) / mm.duplex_Bps) + lat;
     };
@@ -212,7 +216,7 @@ void cost(Cand& c, int64_t M, int64_t N, int64_t K, bool beta_nz, bool scale_onl
         // less the uploads issued ahead of the reload, and (b) after the reload once every C buffer is held by
         // a step whose kernel has only just started
         const double t_up = ((double)c.bytes_h2d - 8.0 * (double)K * (double)N) / std::max(1.0, steps) / mm.h2d_Bps + mm.copy_latency_s;
-        const double c_rate_up = c.c_dev ? 1.0e12 : mm.h2d_Bps, c_rate_down = c.c_dev ? 1.0e12 : mm.d2h_Bps;
+        const double c_rate_up = (c.c_dev && !c.c_in_host) ? 1.0e12 : mm.h2d_Bps, c_rate_down = c.c_dev ? 1.0e12 : mm.d2h_Bps;
         const double t_cup = cload ? (double)c.c_bytes / c_rate_up + mm.copy_latency_s : t_up;
         const double pre = (double)early_uploads(c.h, c.n_sets, c.n_abuf);
         const double drain = std::max(0.0, t_kernel - pre * t_cup);
@@ -252,7 +256,7 @@ extern "C" int hclooc_plan_ex(int64_t M, int64_t N, int64_t K, int beta_nonzero,
 int hclooc::plan_impl(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zero, size_t device_budget_bytes,
                       int operands_on_device, int transa, int transb, hclooc_plan_t* out) {
     const MachineModel& mm = machine_model();
-    const bool c_dev = operands_on_device == 2;
+    const bool c_dev = operands_on_device == 2 || operands_on_device == 5, c_in_host = operands_on_device == 5;
     const bool direct_ok = operands_on_device == 3 || operands_on_device == 4, direct_forced = operands_on_device == 4;
     if (operands_on_device >= 2) operands_on_device = 0;
     if (M < 0) return -1;
@@ -329,6 +333,7 @@ int hclooc::plan_impl(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alp
                     for (int q = 0; q < nt; ++q) {
                         Cand c{};
                         c.c_dev = c_dev;
+                        c.c_in_host = c_in_host;
                         c.ta = transa != 0;
                         c.mb = tried[q]; c.nb = nb; c.kb = kb; c.kpanels = kp;
                         c.h = ceil_div(M, c.mb); c.w = weff;
@@ -404,7 +409,7 @@ int hclooc::plan_impl(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alp
     out->lda_dev = best.lda_dev; out->ldb_dev = best.ldb_dev; out->ldc_dev = best.ldc_dev;
     out->bytes_a_buf = best.a_bytes; out->bytes_b_buf = best.b_bytes; out->bytes_c_buf = best.c_bytes;
     out->workspace_bytes = best.ws_bytes;
-    out->c_on_device = c_dev ? 1 : 0;
+    out->c_on_device = c_dev ? (c_in_host ? 2 : 1) : 0;
     out->n_scratch = best.n_scratch; out->bytes_scratch = best.n_scratch ? streamk_scratch_bytes() : 0;
     out->bytes_h2d = best.bytes_h2d; out->bytes_d2h = best.bytes_d2h;
     out->n_copies_h2d = best.n_h2d; out->n_copies_d2h = best.n_d2h;

@@ -2,12 +2,9 @@
 // future work).  Solves  op(T) * X = scale * X  in place for one diagonal block T of at most 128 x 128
 // and a row-major panel X of ib rows; everything off the diagonal blocks is DGEMM work and goes through the tile kernel.
 //
-// One thread owns one column of the panel (64 solving threads per CTA -- 256 are launched, all of which stage the triangle --,
-// consecutive columns: every global access is a coalesced 512-byte row segment).  The block is held in shared memory TRANSPOSED and in "logical" order -- for an upper triangle the
-// rows and columns are reversed, which turns it into a lower one -- so that the coefficients one thread needs next
-// (column p of the triangle, 32 consecutive rows) are contiguous: they are read as broadcast LDS.128.  The 128 rows are
-// processed as 4 sub-blocks of 32 rows held in registers: a left-looking update from the rows already solved (32
-// independent DFMA chains per solved row), then the 32 x 32 triangle by fully unrolled substitution.  Rounding: the
+// One thread owns one right-hand side (256 per CTA); the block is held in shared memory TRANSPOSED and in "logical" order -- for
+// an upper triangle the rows and columns are reversed, which turns it into a lower one -- so that the coefficients one thread
+// needs next (column p of the triangle, 32 consecutive rows) are contiguous: they are read as broadcast LDS.128.  Rounding: the
 // division by t_ii is a multiplication by the rounded reciprocal (two roundings instead of one; exact for t_ii = +-2^k).
 #include "internal.h"
 
@@ -15,28 +12,55 @@ namespace hclooc {
 namespace {
 
 constexpr int TB = 128;          // largest diagonal block
-constexpr int TCOLS = 64;        // columns (solving threads) per CTA (32 was measured slower: staging the triangle dominates)
 constexpr int TS = TB + 2;       // row stride of the staged triangle: even (LDS.128 alignment), 4-way instead of 32-way store conflicts
-constexpr int SUB = 32;          // rows held in registers
-constexpr int TSTAGE = 256;      // threads per CTA: all of them stage the triangle, the first TCOLS solve
-constexpr size_t TRSM_SMEM = (size_t)TB * TS * 8 + (size_t)TB * TCOLS * 8;   // 130 KiB triangle + 64 KiB solved rows
+constexpr int HB = 64;           // rows solved in registers at a time (half a block)
+constexpr int CH = 16;           // rows of the second half updated at a time
+constexpr int TTHREADS = 256;    // threads per CTA = right-hand sides per CTA: all of them stage the triangle, each solves one
+constexpr size_t TRSM_SMEM = (size_t)TB * TS * 8;   // 130 KiB: the triangle only (one CTA of 8 warps per SM)
 
-__global__ void __launch_bounds__(TSTAGE, 1)
-trsm_block_kernel(const double* __restrict__ T, long long ldt, int ib, double* __restrict__ X, long long sq, long long si, int ncols,
+// the 64 x 64 triangle at `tri` (tri[p * TS + q] = T'[q][p], reciprocal diagonal) against 64 values in registers, right-looking:
+// x_t <- x_t * (1 / t_tt), then x_t2 <- x_t2 - T'[t2][t] x_t for t2 > t; the coefficients of column t are contiguous in q and are
+// read as broadcast LDS.128 pairs (the pair that starts at an even q below t + 1 carries one unused value)
+__device__ __forceinline__ void solve64(double (&x)[HB], const double* __restrict__ tri, int unit) {
+#pragma unroll
+    for (int t = 0; t < HB; ++t) {
+        const double* tcol = tri + t * TS;
+        const double xv = unit ? x[t] : x[t] * tcol[t];
+        x[t] = xv;
+        const int e0 = (t + 1) & ~1;
+#pragma unroll
+        for (int e = e0; e < HB; e += 2) {
+            const double2 tv = *reinterpret_cast<const double2*>(tcol + e);
+            if (e > t) x[e] = fma(-tv.x, xv, x[e]);
+            x[e + 1] = fma(-tv.y, xv, x[e + 1]);
+        }
+    }
+}
+
+// One thread owns one right-hand side: a column of the panel (side = Left: consecutive threads read consecutive addresses) or a
+// row of it (side = Right: a thread's values are contiguous; VEC = 4 reads and writes them as 32-byte vectors -- one full sector
+// per thread and instruction -- when the block is a whole 128 and the rows are 32-byte aligned).  Element q of the logical
+// (lower) system sits at P0[q * step].  The 128 rows are two halves of 64: the first half is loaded into registers and solved
+// there (solve64), stored, and -- still in registers -- subtracted from the second half 16 rows at a time (load, 16 x 64 FMAs against
+// broadcast LDS.128 coefficients, store); then the second half is loaded and solved the same way.  Shared memory holds nothing but
+// the triangle, so a CTA carries 256 solving threads; a right-hand side makes two round trips through L1/L2 instead of living
+// in a per-thread staging buffer.  `scale` multiplies every value at its first load.
+template <int VEC, bool FULL>
+__global__ void __launch_bounds__(TTHREADS, 1)
+trsm_block_kernel(const double* __restrict__ T, long long ldt, int ib, double* __restrict__ X, long long sq, long long si, int nitems,
                   int lower, int trans, int unit, double scale) {
     extern __shared__ __align__(16) double smem[];
     double* sTt = smem;                       // sTt[p * TS + q] = T'[q][p], T' = op(T) in logical (lower) order, 0 above, 1 on
-    double* xs = smem + TB * TS;              //                  a unit / padded diagonal
-    const int tid = threadIdx.x;
-    // ---- stage the triangle with all TSTAGE threads: logical index q <-> actual index lower ? q : ib-1-q.  Consecutive
+    const int tid = threadIdx.x;              //                  a unit / padded diagonal; the diagonal is kept as its reciprocal
+    // ---- stage the triangle with all threads: logical index q <-> actual index lower ? q : ib-1-q.  Consecutive
     // threads walk the direction that is contiguous in global memory (rows of T when it is stored untransposed, columns
     // when transposed); only the ib x ib corner is read, the rest of the 128 x 128 image is padding (0, diagonal 1).
-    // (loads issued in batches of 8 per thread before their stores: the block comes from L2 / HBM at ~1 us per round trip)
-    for (int base = 0; base < TB * TB; base += TSTAGE * 8) {
-        double v[8];
+    // (loads issued in batches of 16 per thread before their stores: the block comes from L2 / HBM at ~1 us per round trip)
+    for (int base = 0; base < TB * TB; base += TTHREADS * 16) {
+        double v[16];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            const int e = base + j * TSTAGE + tid;
+        for (int j = 0; j < 16; ++j) {
+            const int e = base + j * TTHREADS + tid;
             const int hi = e / TB, lo_ = e % TB;
             const int p = trans ? hi : lo_, q = trans ? lo_ : hi;     // element T'[q][p], wanted for q >= p
             const bool need = q < ib && p < ib && (q > p || (q == p && !unit));
@@ -46,54 +70,100 @@ trsm_block_kernel(const double* __restrict__ T, long long ldt, int ib, double* _
             v[j] = need ? t : ((q == p) ? 1.0 : 0.0);
         }
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            const int e = base + j * TSTAGE + tid;
+        for (int j = 0; j < 16; ++j) {
+            const int e = base + j * TTHREADS + tid;
             const int hi = e / TB, lo_ = e % TB;
             const int p = trans ? hi : lo_, q = trans ? lo_ : hi;
-            const bool need = q < ib && p < ib && q == p && !unit;
-            if (q >= p) sTt[p * TS + q] = need ? 1.0 / v[j] : v[j];   // the diagonal is kept as its reciprocal: x = b * (1/t) keeps
-        }                                                             // the FP64 division out of the 128-step substitution chain
+            if (q >= p) sTt[p * TS + q] = v[j];
+        }
     }
     __syncthreads();
-    if (tid >= TCOLS) return;                 // the extra threads only helped staging (no barrier follows)
-    const int col = blockIdx.x * TCOLS + tid;
-    const bool live = col < ncols;
-    double b[SUB];
-    for (int q0 = 0; q0 < ib; q0 += SUB) {
+    // the diagonal is kept as its reciprocal: x = b * (1/t) keeps the FP64 division out of the 128-step substitution chain
+    // (128 divisions per CTA, after the staging: a select between v and 1/v per staged element made every thread divide 64 times)
+    if (tid < ib && !unit) sTt[tid * TS + tid] = 1.0 / sTt[tid * TS + tid];
+    __syncthreads();
+    const long long item = (long long)blockIdx.x * TTHREADS + tid;
+    if (item >= nitems) return;               // no barrier follows
+    double* P0 = X + item * si + (lower ? 0 : (long long)(ib - 1) * sq);
+    const long long step = lower ? sq : -sq;
+    double x[HB];
+    for (int h = 0; h * HB < ib; ++h) {
+        const int q0 = h * HB;
+        const double sc = h == 0 ? scale : 1.0;          // the second half was scaled when the first half was subtracted from it
+        if (VEC == 4) {     // contiguous and 32-byte aligned: ascending (lower) or descending (upper) in memory
 #pragma unroll
-        for (int t = 0; t < SUB; ++t) {
-            const int q = q0 + t;
-            const int r = lower ? q : ib - 1 - q;
-            b[t] = (live && q < ib) ? scale * X[(long long)r * sq + (long long)col * si] : 0.0;
-        }
-        // left-looking: subtract the contribution of the rows solved so far (xs is private to this thread's column)
-#pragma unroll 2
-        for (int p = 0; p < q0; ++p) {
-            const double xv = xs[p * TCOLS + tid];
-            const double2* trow = reinterpret_cast<const double2*>(sTt + p * TS + q0);
+            for (int t = 0; t < HB; t += 4) {
+                const double* p = lower ? P0 + q0 + t : P0 - (q0 + t) - 3;
+                double a, b, c, d;
+                asm volatile("ld.global.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p) : "memory");
+                x[t] = sc * (lower ? a : d); x[t + 1] = sc * (lower ? b : c); x[t + 2] = sc * (lower ? c : b); x[t + 3] = sc * (lower ? d : a);
+            }
+        } else {
+            const double* pp = P0 + (long long)q0 * step;
 #pragma unroll
-            for (int t = 0; t < SUB; t += 2) {
-                const double2 tv = trow[t / 2];
-                b[t] = fma(-tv.x, xv, b[t]);
-                b[t + 1] = fma(-tv.y, xv, b[t + 1]);
+            for (int t = 0; t < HB; ++t) { x[t] = (FULL || q0 + t < ib) ? *pp : 0.0; pp += step; }
+            if (sc != 1.0) {
+#pragma unroll
+                for (int t = 0; t < HB; ++t) x[t] *= sc;
             }
         }
-        // the 32 x 32 triangle on the diagonal, right-looking in registers
+        solve64(x, sTt + q0 * TS + q0, unit);
+        if (VEC == 4) {
 #pragma unroll
-        for (int t = 0; t < SUB; ++t) {
-            const double* tcol = sTt + (q0 + t) * TS + q0;
-            const double x = unit ? b[t] : b[t] * tcol[t];
-            b[t] = x;
+            for (int t = 0; t < HB; t += 4) {
+                double* p = lower ? P0 + q0 + t : P0 - (q0 + t) - 3;
+                if (lower) asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(x[t]), "d"(x[t + 1]), "d"(x[t + 2]), "d"(x[t + 3]) : "memory");
+                else asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(x[t + 3]), "d"(x[t + 2]), "d"(x[t + 1]), "d"(x[t]) : "memory");
+            }
+        } else {
+            double* pp = P0 + (long long)q0 * step;
 #pragma unroll
-            for (int t2 = t + 1; t2 < SUB; ++t2) b[t2] = fma(-tcol[t2], x, b[t2]);
+            for (int t = 0; t < HB; ++t) { if (FULL || q0 + t < ib) *pp = x[t]; pp += step; }
         }
+        if (h == 0) {
+            // the second half receives the first half's contribution, CH rows at a time: b_t -= sum_p T'[64 + t][p] x_p
+            for (int q1 = HB; q1 < ib; q1 += CH) {
+                double b[CH];
+                if (VEC == 4) {
 #pragma unroll
-        for (int t = 0; t < SUB; ++t) {
-            const int q = q0 + t;
-            xs[q * TCOLS + tid] = b[t];
-            if (live && q < ib) {
-                const int r = lower ? q : ib - 1 - q;
-                X[(long long)r * sq + (long long)col * si] = b[t];
+                    for (int t = 0; t < CH; t += 4) {
+                        const double* p = lower ? P0 + q1 + t : P0 - (q1 + t) - 3;
+                        double a, bb, c, d;
+                        asm volatile("ld.global.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(a), "=d"(bb), "=d"(c), "=d"(d) : "l"(p) : "memory");
+                        b[t] = sc * (lower ? a : d); b[t + 1] = sc * (lower ? bb : c); b[t + 2] = sc * (lower ? c : bb); b[t + 3] = sc * (lower ? d : a);
+                    }
+                } else {
+                    const double* pp = P0 + (long long)q1 * step;
+#pragma unroll
+                    for (int t = 0; t < CH; ++t) { b[t] = (FULL || q1 + t < ib) ? *pp : 0.0; pp += step; }
+                    if (sc != 1.0) {
+#pragma unroll
+                        for (int t = 0; t < CH; ++t) b[t] *= sc;
+                    }
+                }
+#pragma unroll
+                for (int p = 0; p < HB; ++p) {                 // fully unrolled: x[] stays in registers
+                    const double xv = x[p];
+                    const double2* trow = reinterpret_cast<const double2*>(sTt + p * TS + q1);
+#pragma unroll
+                    for (int t = 0; t < CH; t += 2) {
+                        const double2 tv = trow[t / 2];
+                        b[t] = fma(-tv.x, xv, b[t]);
+                        b[t + 1] = fma(-tv.y, xv, b[t + 1]);
+                    }
+                }
+                if (VEC == 4) {
+#pragma unroll
+                    for (int t = 0; t < CH; t += 4) {
+                        double* p = lower ? P0 + q1 + t : P0 - (q1 + t) - 3;
+                        if (lower) asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(b[t]), "d"(b[t + 1]), "d"(b[t + 2]), "d"(b[t + 3]) : "memory");
+                        else asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(b[t + 3]), "d"(b[t + 2]), "d"(b[t + 1]), "d"(b[t]) : "memory");
+                    }
+                } else {
+                    double* pp = P0 + (long long)q1 * step;
+#pragma unroll
+                    for (int t = 0; t < CH; ++t) { if (FULL || q1 + t < ib) *pp = b[t]; pp += step; }
+                }
             }
         }
     }
@@ -110,13 +180,24 @@ int launch_trsm_block(const double* dT, int64_t ldt, int ib, double* dX, int64_t
                       int unit, double scale, cudaStream_t stream, int right) {
     if (ib <= 0 || ncols <= 0) return HCLOOC_OK;
     if (ib > TB || ncols > 0x7fffffffLL) return HCLOOC_ERR_INTERNAL;
-    static cudaError_t attr = cudaFuncSetAttribute(trsm_block_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TRSM_SMEM);
+    static cudaError_t attr = cudaFuncSetAttribute(trsm_block_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TRSM_SMEM);
     if (attr != cudaSuccess) return cuda_fail(attr);
-    const unsigned grid = (unsigned)((ncols + TCOLS - 1) / TCOLS);
-    if (right)      // the operator of the row systems is op(T)^T: lower where op(T) is upper, and read with `trans` flipped
-        trsm_block_kernel<<<grid, TSTAGE, TRSM_SMEM, stream>>>(dT, (long long)ldt, ib, dX, 1LL, (long long)ldx, (int)ncols, !lower, !trans, unit, scale);
-    else
-        trsm_block_kernel<<<grid, TSTAGE, TRSM_SMEM, stream>>>(dT, (long long)ldt, ib, dX, (long long)ldx, 1LL, (int)ncols, lower, trans, unit, scale);
+    const unsigned grid = (unsigned)((ncols + TTHREADS - 1) / TTHREADS);
+    static cudaError_t attr4 = cudaFuncSetAttribute(trsm_block_kernel<4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TRSM_SMEM);
+    if (attr4 != cudaSuccess) return cuda_fail(attr4);
+    static cudaError_t attr1 = cudaFuncSetAttribute(trsm_block_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TRSM_SMEM);
+    if (attr1 != cudaSuccess) return cuda_fail(attr1);
+    if (right) {    // the operator of the row systems is op(T)^T: lower where op(T) is upper, and read with `trans` flipped
+        // a thread's row is contiguous: 32-byte vectors when the block is whole and every row starts on a 32-byte boundary
+        const bool vec = ib == TB && (ldx % 4 == 0) && (((uintptr_t)dX & 31u) == 0);
+        if (vec) trsm_block_kernel<4, true><<<grid, TTHREADS, TRSM_SMEM, stream>>>(dT, (long long)ldt, ib, dX, 1LL, (long long)ldx, (int)ncols, !lower, !trans, unit, scale);
+        else if (ib == TB) trsm_block_kernel<1, true><<<grid, TTHREADS, TRSM_SMEM, stream>>>(dT, (long long)ldt, ib, dX, 1LL, (long long)ldx, (int)ncols, !lower, !trans, unit, scale);
+        else trsm_block_kernel<1, false><<<grid, TTHREADS, TRSM_SMEM, stream>>>(dT, (long long)ldt, ib, dX, 1LL, (long long)ldx, (int)ncols, !lower, !trans, unit, scale);
+    } else if (ib == TB) {
+        trsm_block_kernel<1, true><<<grid, TTHREADS, TRSM_SMEM, stream>>>(dT, (long long)ldt, ib, dX, (long long)ldx, 1LL, (int)ncols, lower, trans, unit, scale);
+    } else {
+        trsm_block_kernel<1, false><<<grid, TTHREADS, TRSM_SMEM, stream>>>(dT, (long long)ldt, ib, dX, (long long)ldx, 1LL, (int)ncols, lower, trans, unit, scale);
+    }
     HCL_CUDA(cudaGetLastError());
     return HCLOOC_OK;
 }

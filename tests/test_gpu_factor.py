@@ -55,8 +55,8 @@ def spd_host(H, N, seed, dist, pad=0):
     (128, "uniform", 0, 1 * MiB),            # exactly one potrf block
     (300, "uniform", 2, 8 * MiB),            # one panel: recursion over 128-blocks with a ragged last one
     (1000, "int", 0, 32 * MiB),              # one panel of 1000: three levels of recursion, exact
-    (1000, "uniform", 3, 2 * MiB),           # panels of 128 columns: 8 out-of-core updates
-    (1500, "int", 1, 4 * MiB),               # panels of 128..160, K up to 1400 in the updates, exact
+    (1000, "uniform", 3, 2 * MiB),           # two resident panels of 64 columns: 16 panels, look-ahead updates from host and device
+    (1500, "int", 1, 8 * MiB),               # panels of 128 columns, K up to 1280 in the out-of-core updates, exact
     (2049, "uniform", 0, 16 * MiB),          # odd size: panels of 384, a ragged last one of 129
 ])
 def test_dpotrf_matches_oracle(H, uplo, N, dist, pad, budget):
@@ -97,7 +97,7 @@ def test_dpotrf_not_positive_definite_degenerate_and_errors(H):
         assert info == want == k + 1
         NB = st.plan.nb
         done = (k // NB) * NB                                                   # the panels before the failing one are complete
-        assert np.array_equal(A.view[:, done:], bad[:, done:])                  # from the failing panel on nothing is written back
+        assert np.array_equal(A.view[:, done + NB:], bad[:, done + NB:])        # the panels after the failing one are unchanged
         assert np.array_equal(np.triu(A.view, 1), np.triu(bad, 1))              # the other triangle keeps its bits
         if done:
             low = np.tril(np.ones((k, done), bool))                             # rows the oracle completed, columns we completed
@@ -120,7 +120,7 @@ def test_dpotrf_not_positive_definite_degenerate_and_errors(H):
 
 @pytest.mark.parametrize("uplo", [0, 1])
 def test_dpotrf_large_panels_of_4096(H, uplo):
-    """N = 9000 under 1 GiB: panels of 4096 columns (two full, one ragged), the updates are real out-of-core DGEMMs with the
+    """N = 9000 under 2 GiB: panels of 4096 columns (two full, one ragged), the updates are real out-of-core DGEMMs with the
     triangle mask, the diagonal blocks recurse five levels.  The residual gate on sampled rows and columns, forward agreement with
     scipy (an independent factorization; the oracle itself would take minutes at this size)."""
     import scipy.linalg as sl
@@ -129,8 +129,8 @@ def test_dpotrf_large_panels_of_4096(H, uplo):
     other = other_triangle(N, uplo)
     S = A.view.copy()
     A.view[other] = np.nan
-    info, st = H.hclooc_dpotrf(None, uplo, N, A, A.ld, 1024 * MiB)
-    assert info == 0 and (st.plan.nb if uplo == 0 else st.plan.mb) == 4096 and st.plan.n_steps == 3
+    info, st = H.hclooc_dpotrf(None, uplo, N, A, A.ld, 2048 * MiB)
+    assert info == 0 and (st.plan.nb if uplo == 0 else st.plan.mb) == 4096 and st.plan.n_steps == 3 and st.plan.n_sets == 2
     got = np.nan_to_num(A.view)
     assert np.isnan(A.view[other]).all()
     ref = sl.cholesky(S, lower=(uplo == 0))
