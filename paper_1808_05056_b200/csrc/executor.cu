@@ -997,6 +997,14 @@ extern "C" int hclooc_dtrsm(hclooc_ctx* ctx, int uplo, int trans, int diag, int6
     {
         nres = trsm_resident(M, N, budget, S, own, nullptr);
     }
+    // two block rows AND two NB x NB blocks of T beside a quarter of the budget for the pipeline: the look-ahead form (factor.cu)
+    static const bool no_lookahead = [] { const char* e = std::getenv("HCLOOC_TRSM_LOOKAHEAD"); return e && std::atoi(e) == 0; }();
+    if (nres == 2 && !no_lookahead && 2 * rbytes + 2 * tbytes + budget / 4 <= budget) {
+        std::lock_guard<std::mutex> lk(ctx->mu);
+        rc = dtrsm_left_lookahead(ctx, uplo, trans, diag, M, N, alpha, A, lda, B, ldb, budget, own, S.NB, stats);
+        if (!rc && stats) stats->t_total_s = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_begin).count();
+        return rc;
+    }
     struct DevMem { void* p = nullptr; ~DevMem() { if (p) cudaFree(p); } } resmem;
     double* dres[2] = {nullptr, nullptr};
     double* dTres = nullptr;

@@ -80,4 +80,8 @@ int dgemm_core_locked(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_
                       int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
                       size_t device_budget_bytes, hclooc_stats* stats, int tri = 0, const DgemmExtra* extra = nullptr);
 
+// hclooc_dtrsm (side = Left) with two resident block rows and a look-ahead of one (factor.cu); ctx->mu held by the caller
+int dtrsm_left_lookahead(hclooc_ctx* ctx, int uplo, int trans, int diag, int64_t M, int64_t N, double alpha, const double* A, int64_t lda,
+                         double* B, int64_t ldb, size_t budget, bool own, int64_t NB, hclooc_stats* stats);
+
 }  // namespace hclooc

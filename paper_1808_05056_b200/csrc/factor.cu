@@ -526,3 +526,149 @@ extern "C" int hclooc_dtrsm_side(hclooc_ctx* ctx, int side, int uplo, int trans,
     }
     return HCLOOC_OK;
 }
+
+// ---------------------------------------------------------------------------------------------------------------------
+// hclooc_dtrsm (side = Left) with a LOOK-AHEAD of one block row, the resident mode of executor.cu's hclooc_dtrsm when two block
+// rows and two NB x NB blocks of T fit beside the pipeline.  Block row i (NB x N) is solved in device memory -- T_ii uploaded,
+// column chunks on two streams, each chunk downloaded as soon as it is solved -- WHILE block row i+1 is brought up and receives
+//     B_{i+1} <- alpha*B_{i+1} - op(T)[i+1, solved before i] X[solved before i]
+// as one out-of-core DGEMM whose C blocks are read from the host matrix and stored into the other resident buffer (the pipeline
+// itself brings the block row up).  The contribution of block row i, -op(T)[i+1, i] X_i, then comes straight from device memory
+// (one GPU-filling launch; only the NB x NB block of T crosses the link).  ctx->mu is held by the caller for the whole solve.
+namespace hclooc {
+
+int dtrsm_left_lookahead(hclooc_ctx* ctx, int uplo, int trans, int diag, int64_t M, int64_t N, double alpha, const double* A, int64_t lda,
+                         double* B, int64_t ldb, size_t budget, bool own, int64_t NB, hclooc_stats* stats) {
+    const auto t_begin = std::chrono::steady_clock::now();
+    int rc;
+    HCL_CUDA(cudaSetDevice(ctx->device));
+    if ((rc = ensure_aux(ctx))) return rc;
+    const bool lower = (uplo == HCL_UPLO_LOWER) != (trans == HCL_OP_T);       // op(T) is lower triangular
+    const int64_t nblk = (M + NB - 1) / NB, ldx = round_even(N), ldt = round_even(NB);
+    const size_t rbytes = round_1k((size_t)NB * ldx * 8), tbytes = round_1k((size_t)NB * ldt * 8);
+    const size_t reserved0 = 2 * rbytes + 2 * tbytes;
+    if (own) { if ((rc = ensure_workspace(ctx, budget))) return rc; }
+    uint8_t* base = (uint8_t*)ctx->workspace;
+    const uintptr_t mis = (uintptr_t)base & 1023u;
+    const size_t shift = mis ? 1024 - mis : 0;
+    if (reserved0 + shift > ctx->workspace_bytes) return HCLOOC_ERR_BUDGET;
+    double* dR[2] = {(double*)(base + shift), (double*)(base + shift + rbytes)};
+    double* dT = (double*)(base + shift + 2 * rbytes);              // T_ii of the block row being solved
+    double* dT2 = (double*)(base + shift + 2 * rbytes + tbytes);    // op(T)[next, current] as stored
+    Reserve guard(ctx, reserved0 + shift);
+    cudaStream_t s_sol[2] = {ctx->s_aux[0], ctx->s_aux[3]}, s_up = ctx->s_aux[1], s_down = ctx->s_aux[2];
+    cudaEvent_t ev_T = ctx->ev_aux[0], ev_T2 = ctx->ev_aux[1], ev_down[2] = {ctx->ev_aux[2], ctx->ev_aux[3]};
+    cudaEvent_t ev_sol[2] = {ctx->ev_aux[4], ctx->ev_aux[5]}, ev_ready = ctx->ev_aux[6], ev_chunk = ctx->ev_aux[7];
+    struct Drain {
+        hclooc_ctx* c;
+        ~Drain() { for (cudaStream_t st : c->s_aux) if (st) cudaStreamSynchronize(st); }
+    } drain{ctx};
+    static const bool timing = std::getenv("HCLOOC_FACTOR_TIMING") != nullptr;
+    static const int nchunk = [] { const char* e = std::getenv("HCLOOC_TRSM_CHUNKS"); const int v = e ? std::atoi(e) : 0; return v > 0 ? v : 4; }();
+    hclooc_stats acc;
+    std::memset(&acc, 0, sizeof(acc));
+    double t_enq = 0.0;
+    size_t ws_max = reserved0;
+    auto rows_of = [&](int64_t bi, int64_t* r0, int64_t* nbi) {
+        const int64_t i = lower ? bi : nblk - 1 - bi;
+        *r0 = i * NB; *nbi = std::min(NB, M - *r0);
+    };
+    // block row 0 comes up whole
+    {
+        int64_t r0, nb0;
+        rows_of(0, &r0, &nb0);
+        if ((rc = copy2d(dR[0], (size_t)ldx * 8, B + r0 * ldb, (size_t)ldb * 8, (size_t)N * 8, (size_t)nb0, s_up))) return rc;
+        acc.bytes_h2d += (uint64_t)nb0 * N * 8; ++acc.n_copies_h2d;
+        HCL_CUDA(cudaEventRecord(ev_ready, s_up));
+    }
+    bool scaled = false;                                                        // has alpha reached the block row in dR[cur]?
+    for (int64_t bi = 0; bi < nblk; ++bi) {
+        const int cur = (int)(bi & 1), alt = 1 - cur;
+        int64_t r0, nbi;
+        rows_of(bi, &r0, &nbi);
+        const auto tp0 = std::chrono::steady_clock::now();
+        // ---- T_ii up, then the column chunks of block row bi on two streams; every chunk goes down as soon as it is solved
+        if ((rc = copy2d(dT, (size_t)ldt * 8, A + r0 * lda + r0, (size_t)lda * 8, (size_t)nbi * 8, (size_t)nbi, s_up))) return rc;
+        acc.bytes_h2d += (uint64_t)nbi * nbi * 8; ++acc.n_copies_h2d;
+        HCL_CUDA(cudaEventRecord(ev_T, s_up));
+        int64_t wr = ((N + nchunk - 1) / nchunk + 63) / 64 * 64;
+        if (wr < 1024) wr = 1024;
+        int64_t c = 0;
+        for (int64_t c0 = 0; c0 < N; c0 += wr, ++c) {
+            const int64_t w = std::min(wr, N - c0);
+            cudaStream_t st = s_sol[c & 1];
+            if (c < 2) { HCL_CUDA(cudaStreamWaitEvent(st, ev_T, 0)); HCL_CUDA(cudaStreamWaitEvent(st, ev_ready, 0)); }
+            if ((rc = dev_trsm(0, dT, ldt, lower ? 1 : 0, trans, diag, dR[cur] + c0, ldx, w, nbi, scaled ? 1.0 : alpha, st, &acc.n_kernels))) return rc;
+            HCL_CUDA(cudaEventRecord(ev_chunk, st));
+            HCL_CUDA(cudaStreamWaitEvent(s_down, ev_chunk, 0));
+            if ((rc = copy2d(B + r0 * ldb + c0, (size_t)ldb * 8, dR[cur] + c0, (size_t)ldx * 8, (size_t)w * 8, (size_t)nbi, s_down))) return rc;
+            acc.bytes_d2h += (uint64_t)nbi * w * 8; ++acc.n_copies_d2h;
+        }
+        HCL_CUDA(cudaEventRecord(ev_down[cur], s_down));
+        for (int s = 0; s < 2; ++s) HCL_CUDA(cudaEventRecord(ev_sol[s], s_sol[s]));
+        if (bi + 1 == nblk) break;
+        // ---- meanwhile: block row bi+1
+        int64_t q0, nb2;
+        rows_of(bi + 1, &q0, &nb2);
+        // op(T)[next, current] as stored: T[q0.., r0..] (nb2 x nbi), or, transposed, T[r0.., q0..] (nbi x nb2); dT2's previous
+        // reader is the update 2 of this block row, issued at the end of the last round and possibly still running
+        HCL_CUDA(cudaStreamWaitEvent(s_up, ev_ready, 0));                      // ... on the device: after that update 2
+        if (trans) rc = copy2d(dT2, (size_t)ldt * 8, A + r0 * lda + q0, (size_t)lda * 8, (size_t)nb2 * 8, (size_t)nbi, s_up);
+        else rc = copy2d(dT2, (size_t)ldt * 8, A + q0 * lda + r0, (size_t)lda * 8, (size_t)nbi * 8, (size_t)nb2, s_up);
+        if (rc) return rc;
+        acc.bytes_h2d += (uint64_t)nbi * nb2 * 8; ++acc.n_copies_h2d;
+        HCL_CUDA(cudaEventRecord(ev_T2, s_up));
+        // rows solved BEFORE the current block row: [0, r0) when op(T) is lower, [r0 + nbi, M) when it is upper
+        const int64_t k0 = lower ? 0 : r0 + nbi, kk = lower ? r0 : M - (r0 + nbi);
+        bool next_scaled = false;
+        if (kk > 0) {
+            HCL_CUDA(cudaEventSynchronize(ev_down[alt]));                       // X of block row bi-1 is on the host (the pipeline reads it)
+            const double* Ap = trans ? A + k0 * lda + q0 : A + q0 * lda + k0;   // op(T)[next, solved], as stored
+            hclooc_stats one;
+            DgemmExtra ex;
+            ex.C_src = B + q0 * ldb; ex.ldc_src = ldb;
+            ex.wait_before_store[0] = ev_ready;                                 // update 2 of block row bi read X_{bi-1} from dR[alt]
+            rc = dgemm_core_locked(ctx, trans ? 1 : 0, 0, nb2, N, kk, -1.0, Ap, lda, B + k0 * ldb, ldb, alpha, dR[alt], ldx, budget, &one, 0, &ex);
+            if (rc) return rc;
+            add_stats(acc, one, &t_enq);
+            ws_max = std::max(ws_max, reserved0 + (size_t)one.plan.workspace_bytes);
+            next_scaled = true;
+            if (timing) std::fprintf(stderr, "  dtrsm update %lld x %lld x %lld: %.2f ms (%.1f TFLOP/s), %lld x %lld blocks of %lld x %lld, %.2f GB up\n", (long long)nb2, (long long)N,
+                                     (long long)kk, 1e3 * one.t_total_s, 2e-12 * (double)nb2 * N * kk / one.t_total_s, (long long)one.plan.h, (long long)one.plan.w,
+                                     (long long)one.plan.mb, (long long)one.plan.nb, one.bytes_h2d / 1e9);
+        } else {                                                                // the second block row: nothing before the first one
+            if ((rc = copy2d(dR[alt], (size_t)ldx * 8, B + q0 * ldb, (size_t)ldb * 8, (size_t)N * 8, (size_t)nb2, s_up))) return rc;
+            acc.bytes_h2d += (uint64_t)nb2 * N * 8; ++acc.n_copies_h2d;
+            HCL_CUDA(cudaEventRecord(ev_T2, s_up));                             // (covers the block of T and the block row)
+        }
+        const auto tp1 = std::chrono::steady_clock::now();
+        for (int s = 0; s < 2; ++s) HCL_CUDA(cudaEventSynchronize(ev_sol[s]));  // block row bi is solved
+        if (timing) std::fprintf(stderr, "dtrsm block row %lld: next block row's upload + out-of-core update %.2f ms, then %.2f ms more for the solve\n", (long long)bi,
+                                 1e3 * std::chrono::duration<double>(tp1 - tp0).count(), 1e3 * std::chrono::duration<double>(std::chrono::steady_clock::now() - tp1).count());
+        // ---- update 2: B_next <- beta' * B_next - op(T)[next, current] X_current, all in device memory
+        HCL_CUDA(cudaStreamWaitEvent(s_sol[0], ev_T2, 0));
+        rc = launch_dgemm_tiles(nb2, N, nbi, -1.0, dT2, ldt, dR[cur], ldx, next_scaled ? 1.0 : alpha, dR[alt], ldx, s_sol[0], -1, nullptr, trans ? 1 : 0, 0);
+        if (rc) return rc;
+        ++acc.n_kernels;
+        HCL_CUDA(cudaEventRecord(ev_ready, s_sol[0]));
+        scaled = true;
+    }
+    for (cudaStream_t st : ctx->s_aux) if (st) HCL_CUDA(cudaStreamSynchronize(st));
+    if (stats) {
+        *stats = acc;
+        stats->plan.M = M; stats->plan.N = N; stats->plan.K = M;
+        stats->plan.mb = NB; stats->plan.nb = std::min<int64_t>(N, std::max<int64_t>(1024, ((N + nchunk - 1) / nchunk + 63) / 64 * 64)); stats->plan.kb = 128;
+        stats->plan.h = nblk; stats->plan.w = (N + stats->plan.nb - 1) / stats->plan.nb; stats->plan.kpanels = 1; stats->plan.n_steps = nblk;
+        stats->plan.workspace_bytes = ws_max;
+        stats->plan.n_sets = 2;
+        stats->plan.ldc_dev = ldx;
+        stats->plan.bytes_h2d = acc.bytes_h2d; stats->plan.bytes_d2h = acc.bytes_d2h;
+        stats->plan.n_copies_h2d = acc.n_copies_h2d; stats->plan.n_copies_d2h = acc.n_copies_d2h;
+        stats->plan.flops = (double)M * (double)M * (double)N;
+        stats->t_enqueue_s = t_enq;
+        stats->t_total_s = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_begin).count();
+    }
+    return HCLOOC_OK;
+}
+
+}  // namespace hclooc
