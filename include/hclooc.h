@@ -199,6 +199,18 @@ int hclooc_ctx_set_trace(hclooc_ctx* ctx, int enable);
  * is staged through device buffers), 1 = always when the operands allow it.  -2: mode outside {-1, 0, 1}.   */
 int hclooc_ctx_set_direct(hclooc_ctx* ctx, int mode);
 int hclooc_ctx_get_trace(hclooc_ctx* ctx, hclooc_trace_rec* recs, size_t max_recs, size_t* n_recs);
+/* Debug shaker (the rule it exercises is PAPER.md:311: "data stored in device buffers is not overwritten until
+ * kernel executions that operate on the data have completed").  jitter_seed != 0: every copy and kernel the library enqueues on this
+ * context -- the DGEMM pipeline, the device phases of hclooc_dtrsm[_side] and hclooc_dpotrf -- is preceded, with probability 1/2,
+ * by a spin kernel of random length (up to ~150 us) in its stream, so that the streams drift against each other differently in
+ * every call.  poison != 0: a device buffer region is filled with NaN at the moment the schedule declares it free -- in front of
+ * the upload that overwrites it (behind that upload's waits) and behind the download of a C block -- so that a reader the event
+ * waits failed to order sees NaN instead of stale but plausible data.  A schedule that is race free gives the same results with
+ * the shaker on (the parity tests run under it); CUDA-graph replay is off while it is on.  HCLOOC_DEBUG_JITTER=<seed> in the
+ * environment switches both on for every context created afterwards.  poison == 2 additionally SABOTAGES the pipeline (its
+ * upload stream skips every event wait): the tests use it to show that the shaker does turn a missing wait into wrong results.
+ * Returns 0.                                                                                                                */
+int hclooc_ctx_set_debug(hclooc_ctx* ctx, uint64_t jitter_seed, int poison);
 
 /* ------------------------------------------------------------------ the operation
  * hclooc_dgemm: C = alpha*A*B + beta*C, synchronous: C is complete in host memory on return.

@@ -283,6 +283,7 @@ extern "C" int hclooc_ctx_create(hclooc_ctx** out, int device, void* d_workspace
         }
     }
     if (e != cudaSuccess) { hclooc_ctx_destroy(c); return cuda_fail(e); }
+    if (const char* j = std::getenv("HCLOOC_DEBUG_JITTER")) { c->dbg_rng = (uint64_t)std::strtoull(j, nullptr, 10); c->dbg_poison = c->dbg_rng != 0; }
     *out = c;
     return HCLOOC_OK;
 }
@@ -535,7 +536,7 @@ int dgemm_core_locked(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_
     // Latency-bound schedules (many small operations: config 1) are captured once as a CUDA graph and replayed when
     // the very same call comes again; long schedules gain nothing (their enqueue time hides behind the transfers).
     static const int graph_mode = [] { const char* e = std::getenv("HCLOOC_GRAPH"); return e ? std::atoi(e) : -1; }();
-    bool use_graph = !trace && !extra && !scale_only && P.n_scratch == 0 &&
+    bool use_graph = !trace && !extra && !scale_only && P.n_scratch == 0 && !ctx->dbg_rng && !ctx->dbg_poison &&
                      (graph_mode == 1 || (graph_mode < 0 && P.n_steps <= 512 && P.t_model_s < 5e-3));
     std::vector<int64_t> key;
     if (!use_graph) { ctx->graph_key.clear(); ctx->graph_valid = false; }
@@ -587,8 +588,15 @@ int dgemm_core_locked(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_
             else r.bytes = (uint64_t)o.nr * (uint64_t)o.nc * 8;
             ctx->trace_recs.push_back(r);
         }
+        if (ctx->dbg_rng && o.kind != HCLOOC_OP_WAIT && o.kind != HCLOOC_OP_RECORD && !use_graph) debug_jitter(ctx, st);
+        if (ctx->dbg_poison && !use_graph) {       // the op list has put every wait this overwrite needs in front of it
+            if (o.kind == HCLOOC_OP_H2D_A) debug_poison(ctx, bufs[o.buf], P.lda_dev, transa ? o.nc : o.nr, transa ? o.nr : o.nc, st);
+            else if (o.kind == HCLOOC_OP_H2D_B && !transb) debug_poison(ctx, bufs[o.buf] + o.dev_r0 * P.ldb_dev, P.ldb_dev, o.nr, o.nc, st);
+            else if (o.kind == HCLOOC_OP_H2D_C) debug_poison(ctx, bufs[o.buf], P.ldc_dev, o.nr, o.nc, st);
+        }
         switch (o.kind) {
             case HCLOOC_OP_WAIT: {
+                if (ctx->dbg_poison == 2 && o.stream == 0) break;     // sabotage (tests): the upload stream ignores its waits
                 cudaError_t e = cudaStreamWaitEvent(st, ctx->events[o.event], 0);
                 if (e != cudaSuccess) rc = cuda_fail(e);
                 break;
@@ -633,6 +641,7 @@ int dgemm_core_locked(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_
                 rc = copy2d(C + o.r0 * ldc + o.c0, (size_t)ldc * 8, bufs[o.buf], (size_t)P.ldc_dev * 8, (size_t)o.nc * 8, (size_t)o.nr, st);
                 if (!c_dev) bytes_d2h += (uint64_t)o.nr * o.nc * 8;
                 ++n_d2h;
+                if (ctx->dbg_poison && !use_graph) debug_poison(ctx, bufs[o.buf], P.ldc_dev, o.nr, o.nc, st);   // stored: nobody may still want it
                 break;
             case HCLOOC_OP_GEMM: {
                 const double b_eff = (o.beta < 0.0) ? beta : o.beta;
@@ -1280,6 +1289,16 @@ extern "C" int hclooc_ctx_set_trace(hclooc_ctx* ctx, int enable) {
     if (!ctx && (rc = default_ctx(&ctx))) return rc;
     std::lock_guard<std::mutex> lk(ctx->mu);
     ctx->trace = enable != 0;
+    return HCLOOC_OK;
+}
+
+extern "C" int hclooc_ctx_set_debug(hclooc_ctx* ctx, uint64_t jitter_seed, int poison) {
+    int rc;
+    if (!ctx && (rc = default_ctx(&ctx))) return rc;
+    std::lock_guard<std::mutex> lk(ctx->mu);
+    ctx->dbg_rng = jitter_seed;
+    ctx->dbg_poison = poison == 2 ? 2 : (poison != 0);
+    ctx->graph_key.clear(); ctx->graph_valid = false;       // a captured schedule carries no shaker
     return HCLOOC_OK;
 }
 

@@ -46,6 +46,10 @@ struct hclooc_ctx {
     cudaStream_t s_aux[4] = {};
     cudaEvent_t ev_aux[8] = {};
     long long* h_word = nullptr;
+    // debug shaker (hclooc_ctx_set_debug / HCLOOC_DEBUG_JITTER): random spin kernels in front of copies and kernels, NaN in every
+    // device buffer region the moment the schedule declares it free to overwrite
+    uint64_t dbg_rng = 0;                         // 0 = off, else the xorshift state
+    int dbg_poison = 0;
     std::mutex mu;
 };
 
@@ -61,6 +65,11 @@ int copy2d(void* dst, size_t dpitch, const void* src, size_t spitch, size_t widt
 int resolve_budget(hclooc_ctx* ctx, size_t device_budget_bytes, size_t* budget, bool* library_owned);
 int ensure_workspace(hclooc_ctx* ctx, size_t bytes);
 int ensure_aux(hclooc_ctx* ctx);        // ctx->s_aux, ev_aux, h_word
+// debug shaker (runtime.cu): a spin kernel of random length in `s` (with probability 1/2) when ctx->dbg_rng != 0 ...
+void debug_jitter(hclooc_ctx* ctx, cudaStream_t s);
+// ... and NaN over a rows x cols region (leading dimension ld) in `s` when ctx->dbg_poison != 0: called where a buffer is about
+// to be overwritten -- after the schedule's waits -- so that a reader the waits failed to cover sees NaN instead of stale data
+void debug_poison(hclooc_ctx* ctx, double* p, int64_t ld, int64_t rows, int64_t cols, cudaStream_t s);
 
 // C = alpha*op(A)*op(B) + beta*C through the pipeline (executor.cu).  tri != 0: only the lower (1) / upper (2) triangle of this
 // call's C -- element (0, 0) on the diagonal -- is referenced (hclooc_dsyrk, the Cholesky panel).  Takes ctx->mu itself.

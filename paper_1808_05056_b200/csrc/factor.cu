@@ -24,6 +24,14 @@ using namespace hclooc;
 
 namespace {
 
+// the context whose debug shaker (executor.h) applies to the device recursions below: set by the routine that runs them
+thread_local hclooc_ctx* t_dbg = nullptr;
+struct DbgScope {
+    hclooc_ctx* prev;
+    explicit DbgScope(hclooc_ctx* c) : prev(t_dbg) { t_dbg = c; }
+    ~DbgScope() { t_dbg = prev; }
+};
+
 int64_t split_point(int64_t lo, int64_t hi) { return lo + ((hi - lo + 127) / 128 + 1) / 2 * 128; }
 
 // X <- op(T)^-1 (scale X) (right = 0: X is n x w) or X <- (scale X) op(T)^-1 (right = 1: X is w x n) in device memory, T the
@@ -43,6 +51,7 @@ int dev_trsm(int right, const double* dT, int64_t ldt, int lower, int trans, int
         const Range r = stack.back();
         stack.pop_back();
         const int64_t len = r.hi - r.lo;
+        debug_jitter(t_dbg, st);
         if (len <= 128) {
             int e = launch_trsm_block(dT + r.lo * ldt + r.lo, ldt, (int)len, right ? X + r.lo : X + r.lo * ld, ld, w, lower, trans, unit, r.scale, st, right);
             if (e) return e;
@@ -75,6 +84,7 @@ int dev_trsm(int right, const double* dT, int64_t ldt, int lower, int trans, int
 // triangle, by recursive halving:  factor A11;  A21 <- A21 L11^-T (a right-side solve; upper: A12 <- U11^-T A12, a left-side one);
 // A22 <- A22 - A21 A21^T on its triangle (the tile kernel with the triangle mask);  factor A22.
 int dev_potrf(double* dA, int64_t ld, int64_t n, int lower, long long* d_info, long long info_base, cudaStream_t st, uint64_t* n_kernels) {
+    debug_jitter(t_dbg, st);
     if (n <= 128) {
         ++*n_kernels;
         return launch_potrf_block(dA, ld, (int)n, lower, d_info, info_base, st);
@@ -246,6 +256,7 @@ extern "C" int hclooc_dpotrf(hclooc_ctx* ctx, int uplo, int64_t N, double* A, in
     double* dPan[2] = {(double*)(base + shift), (double*)(base + shift + (npan - 1) * panel_bytes)};
     long long* d_info = (long long*)(base + shift + npan * panel_bytes);
     Reserve guard(ctx, reserved + shift);
+    DbgScope dbg(ctx);
     // streams of this routine's own device work (the DGEMM pipeline keeps its own): diagonal phases, panel uploads, panel downloads
     cudaStream_t s_diag = ctx->s_aux[0], s_up = ctx->s_aux[1], s_down = ctx->s_aux[2], s_pot = ctx->s_aux[3];
     cudaEvent_t ev_up[2] = {ctx->ev_aux[0], ctx->ev_aux[1]}, ev_down[2] = {ctx->ev_aux[2], ctx->ev_aux[3]};
@@ -304,6 +315,7 @@ extern "C" int hclooc_dpotrf(hclooc_ctx* ctx, int uplo, int64_t N, double* A, in
         // diagonal block goes down in strips of 128 rows cut at the diagonal tile -- the panel's blocks that lie wholly in the other
         // triangle were never brought up (the pipeline has no step for them), and the host keeps its bits there.
         HCL_CUDA(cudaStreamWaitEvent(s_down, ev_diag, 0));
+        debug_jitter(ctx, s_down);
         {
             double* hP = A + c0 * lda + c0;
             for (int64_t r = 0; r < nbj; r += 128) {
@@ -331,8 +343,10 @@ extern "C" int hclooc_dpotrf(hclooc_ctx* ctx, int uplo, int64_t N, double* A, in
                 //   lower:  P <- P - L[c0n:N, 0:c0] * L[c0n:c0n+nbn, 0:c0]^T        upper:  P <- P - U[0:c0, c0n:c0n+nbn]^T * U[0:c0, c0n:N]
                 // (the 128 x 128 tiles on the panel's diagonal come up whole first: the pipeline brings only the blocks of ITS plan
                 // that touch the referenced triangle, and the strips that go down later are cut at these tiles)
-                HCL_CUDA(cudaStreamWaitEvent(s_up, ev_down[alt], 0));
-                HCL_CUDA(cudaStreamWaitEvent(s_up, ev_upd2, 0));
+                HCL_CUDA(cudaEventSynchronize(ev_down[alt]));   // panel bj-1 is on the HOST: the pipeline is about to read it as an operand
+                HCL_CUDA(cudaStreamWaitEvent(s_up, ev_upd2, 0));  // (found by the debug shaker: nothing else orders that download before the uploads)
+                debug_jitter(ctx, s_up);
+                debug_poison(ctx, dPan[alt], ldpn, prown, pcoln, s_up);         // the buffer is free now: nobody may still read panel bj-1
                 for (int64_t r = 0; r < nbn; r += 128) {
                     const int64_t rr = std::min<int64_t>(128, nbn - r);
                     if ((rc = copy2d(dPan[alt] + r * ldpn + r, (size_t)ldpn * 8, A + (c0n + r) * lda + c0n + r, (size_t)lda * 8, (size_t)rr * 8, (size_t)rr, s_up))) return rc;
@@ -375,6 +389,7 @@ extern "C" int hclooc_dpotrf(hclooc_ctx* ctx, int uplo, int64_t N, double* A, in
         // of small launches that leaves nearly every SM idle)
         if (bj + 1 < nblk) {
             if (uploaded_whole) HCL_CUDA(cudaStreamWaitEvent(s_diag, ev_up[alt], 0));
+            debug_jitter(ctx, s_diag);
             const int64_t below = N - c0n - nbn;                  // rows (lower) / columns (upper) of panel bj+1 past its diagonal block
             //   lower:  P' <- P' - L[c0n:N, c0:c0n] * L[c0n:c0n+nbn, c0:c0n]^T, both operands = rows nbj.. of the panel just factored
             if (lower) rc = launch_dgemm_tiles(nbn, nbn, nbj, -1.0, dP + nbj * ldp, ldp, dP + nbj * ldp, ldp, 1.0, dPan[alt], ldpn, s_diag, 0, nullptr, 0, 1, 1, 0);
@@ -383,6 +398,7 @@ extern "C" int hclooc_dpotrf(hclooc_ctx* ctx, int uplo, int64_t N, double* A, in
             ++acc.n_kernels;
             HCL_CUDA(cudaEventRecord(ev_2a, s_diag));
             HCL_CUDA(cudaStreamWaitEvent(s_pot, ev_2a, 0));
+            debug_jitter(ctx, s_pot);
             if ((rc = dev_potrf(dPan[alt], ldpn, nbn, lower ? 1 : 0, d_info, (long long)c0n, s_pot, &acc.n_kernels))) return rc;
             HCL_CUDA(cudaEventRecord(ev_pot, s_pot));
             if (below > 0) {
@@ -475,6 +491,7 @@ extern "C" int hclooc_dtrsm_side(hclooc_ctx* ctx, int side, int uplo, int trans,
     double* dT = (double*)(base + shift);
     double* dP = (double*)(base + shift + tbytes);
     Reserve guard(ctx, reserved + shift);
+    DbgScope dbg(ctx);
     const bool lower_op = (uplo == HCL_UPLO_LOWER) != (trans == HCL_OP_T);     // op(T) is lower triangular
     const int64_t nblk = (N + NB - 1) / NB;
     cudaStream_t sc = ctx->s_compute[0];
@@ -556,6 +573,7 @@ int dtrsm_left_lookahead(hclooc_ctx* ctx, int uplo, int trans, int diag, int64_t
     double* dT = (double*)(base + shift + 2 * rbytes);              // T_ii of the block row being solved
     double* dT2 = (double*)(base + shift + 2 * rbytes + tbytes);    // op(T)[next, current] as stored
     Reserve guard(ctx, reserved0 + shift);
+    DbgScope dbg(ctx);
     cudaStream_t s_sol[2] = {ctx->s_aux[0], ctx->s_aux[3]}, s_up = ctx->s_aux[1], s_down = ctx->s_aux[2];
     cudaEvent_t ev_T = ctx->ev_aux[0], ev_T2 = ctx->ev_aux[1], ev_down[2] = {ctx->ev_aux[2], ctx->ev_aux[3]};
     cudaEvent_t ev_sol[2] = {ctx->ev_aux[4], ctx->ev_aux[5]}, ev_ready = ctx->ev_aux[6], ev_chunk = ctx->ev_aux[7];
@@ -601,6 +619,7 @@ int dtrsm_left_lookahead(hclooc_ctx* ctx, int uplo, int trans, int diag, int64_t
             if ((rc = dev_trsm(0, dT, ldt, lower ? 1 : 0, trans, diag, dR[cur] + c0, ldx, w, nbi, scaled ? 1.0 : alpha, st, &acc.n_kernels))) return rc;
             HCL_CUDA(cudaEventRecord(ev_chunk, st));
             HCL_CUDA(cudaStreamWaitEvent(s_down, ev_chunk, 0));
+            debug_jitter(ctx, s_down);
             if ((rc = copy2d(B + r0 * ldb + c0, (size_t)ldb * 8, dR[cur] + c0, (size_t)ldx * 8, (size_t)w * 8, (size_t)nbi, s_down))) return rc;
             acc.bytes_d2h += (uint64_t)nbi * w * 8; ++acc.n_copies_d2h;
         }
@@ -628,6 +647,11 @@ int dtrsm_left_lookahead(hclooc_ctx* ctx, int uplo, int trans, int diag, int64_t
             DgemmExtra ex;
             ex.C_src = B + q0 * ldb; ex.ldc_src = ldb;
             ex.wait_before_store[0] = ev_ready;                                 // update 2 of block row bi read X_{bi-1} from dR[alt]
+            if (ctx->dbg_poison) {                                              // debug: the buffer is free now, nobody may still read X_{bi-1}
+                debug_poison(ctx, dR[alt], ldx, nb2, N, s_up);                  // (s_up has waited for ev_ready above; the download was host-synchronised)
+                HCL_CUDA(cudaEventRecord(ev_T2, s_up));
+                ex.wait_before_store[1] = ev_T2;
+            }
             rc = dgemm_core_locked(ctx, trans ? 1 : 0, 0, nb2, N, kk, -1.0, Ap, lda, B + k0 * ldb, ldb, alpha, dR[alt], ldx, budget, &one, 0, &ex);
             if (rc) return rc;
             add_stats(acc, one, &t_enq);
@@ -647,6 +671,7 @@ int dtrsm_left_lookahead(hclooc_ctx* ctx, int uplo, int trans, int diag, int64_t
                                  1e3 * std::chrono::duration<double>(tp1 - tp0).count(), 1e3 * std::chrono::duration<double>(std::chrono::steady_clock::now() - tp1).count());
         // ---- update 2: B_next <- beta' * B_next - op(T)[next, current] X_current, all in device memory
         HCL_CUDA(cudaStreamWaitEvent(s_sol[0], ev_T2, 0));
+        debug_jitter(ctx, s_sol[0]);
         rc = launch_dgemm_tiles(nb2, N, nbi, -1.0, dT2, ldt, dR[cur], ldx, next_scaled ? 1.0 : alpha, dR[alt], ldx, s_sol[0], -1, nullptr, trans ? 1 : 0, 0);
         if (rc) return rc;
         ++acc.n_kernels;

@@ -6,6 +6,8 @@
 #include <chrono>
 #include <thread>
 #include "internal.h"
+#include "executor.h"
+#include <algorithm>
 
 using namespace hclooc;
 
@@ -58,6 +60,37 @@ __global__ void __launch_bounds__(256) probe_dfma_kernel(double* out, int iters)
     if (s == 123.456) out[0] = s;
 }
 }  // namespace
+
+namespace {
+__global__ void debug_spin_kernel(long long cycles) {
+    const long long t0 = clock64();
+    while (clock64() - t0 < cycles) { }
+}
+__global__ void debug_fill_kernel(double* p, long long ld, long long rows, long long cols, double v) {
+    const long long n = rows * cols;
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (long long)gridDim.x * blockDim.x)
+        p[(e / cols) * ld + e % cols] = v;
+}
+}  // namespace
+
+namespace hclooc {
+void debug_jitter(hclooc_ctx* ctx, cudaStream_t s) {
+    if (!ctx || !ctx->dbg_rng) return;
+    uint64_t x = ctx->dbg_rng;
+    x ^= x << 13; x ^= x >> 7; x ^= x << 17;
+    ctx->dbg_rng = x ? x : 0x9E3779B97F4A7C15ull;
+    if (x & 1) debug_spin_kernel<<<1, 1, 0, s>>>((long long)((x >> 8) % 300000));       // up to ~150 us at 1.965 GHz
+}
+void debug_poison(hclooc_ctx* ctx, double* p, int64_t ld, int64_t rows, int64_t cols, cudaStream_t s) {
+    if (!ctx || !ctx->dbg_poison || !p || rows <= 0 || cols <= 0) return;
+    const long long n = (long long)rows * cols;
+    const unsigned grid = (unsigned)std::min<long long>(1184, (n + 255) / 256);
+    const unsigned long long bits = 0x7ff8000000000badull;              // a quiet NaN with a recognisable payload
+    double nan_v;
+    memcpy(&nan_v, &bits, sizeof(nan_v));
+    debug_fill_kernel<<<grid, 256, 0, s>>>(p, (long long)ld, (long long)rows, (long long)cols, nan_v);
+}
+}  // namespace hclooc
 
 extern "C" {
 
