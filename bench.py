@@ -485,6 +485,10 @@ class Bench:
         live = measure_link(H)
         if live:
             LINK.update(live)
+        cal = None
+        if not args.no_calibrate:      # the planner's cost model takes THIS box's link rates (hclooc_calibrate_link) instead of its defaults
+            cal = dict(zip(("h2d_GBps", "d2h_GBps", "duplex_GBps"), H.hclooc_calibrate_link(None)))
+        self.calibration = cal
         peak_measured = H.hclooc_probe_fp64(0, 4, 1.0)
         per_config = None
         if self.world == 1 and not args.no_per_config and args.workload == "auto":
@@ -538,6 +542,7 @@ class Bench:
                        "matrices_bytes": wl_bytes(wl), "hbm_total_bytes": int(torch.cuda.get_device_properties(self.local).total_memory),
                        "exceeds_hbm": wl_bytes(wl) > int(torch.cuda.get_device_properties(self.local).total_memory),
                        "host_mem_total_bytes": meminfo("MemTotal"), "t_pin_s": t_pin,
+                       "cost_model_link": self.calibration or "library defaults (55.5 / 51.5 / 88 GB/s)",
                        "plan": self.plan_summary(plan),
                        "l2": "inputs (A+B+C = %.2f GB) are host-resident and exceed the 126 MB L2; no flush needed" % (wl_bytes(wl) / 1e9),
                        "value_leg": "CUDA events around the K host-resident calls (the pipeline: uploads, kernels, downloads); the in-core kernel rate is under in_core"},
@@ -590,6 +595,52 @@ class Bench:
         torch.cuda.empty_cache()
         return {"value": val, "unit": "TFLOP/s", "ms_per_step": r["ms_events"], "shape": f"{m}x{n}x{k}", "frac_of_fp64_peak": val / FP64_PEAK_TFLOPS,
                 "note": "A, B, C resident in HBM: one stream-K launch on the caller's matrices, nothing staged (kernel-only rate; not the metric)"}
+
+    def phases(self):
+        """Where the time of a small, latency-bound call goes (BASELINE config 1 in direct mode: ONE kernel launch whose TMA loads
+        read A and B from pinned host memory and whose epilogue reads and writes C there): the same call timed with parts of its
+        work removed -- a 128 x 128 x 16 call (launch + synchronisation floor), beta = 0 (no C read), alpha = 0 (no A / B stream:
+        C read and written only) -- and the plain copies of the same bytes (what a staged path would at least pay)."""
+        H, torch = self.H, self.torch
+        name, wl = pick_workload(self.args.workload, self.share)
+        M, N, K = wl["M"], wl["N"], wl["K"]
+        live = measure_link(H)
+        if live:
+            LINK.update(live)
+        ctx, ws, streams, budget = self.make_ctx(wl["budget"])
+        A, B, C, _ = self.host_matrices(wl, self.synthgen.BASE_SEED + wl["seed_idx"])
+        steps = self.args.steps or 200
+
+        def t_us(fn):
+            return 1e3 * self.timed(fn, steps, 10)["ms_wall"]
+
+        out = {"phases": True, "workload": f"{name}: {wl['desc']}", "steps": steps, "unit": "us per call (host clock around the calls)"}
+        st = H.hclooc_dgemm_ex(ctx, M, N, K, wl["alpha"], A, K, B, N, wl["beta"], C, N, budget)
+        out["plan"] = self.plan_summary(st.plan)
+        out["call"] = t_us(lambda: H.hclooc_dgemm_ex(ctx, M, N, K, wl["alpha"], A, K, B, N, wl["beta"], C, N, budget))
+        out["call_beta0_no_C_read"] = t_us(lambda: H.hclooc_dgemm_ex(ctx, M, N, K, wl["alpha"], A, K, B, N, 0.0, C, N, budget))
+        out["call_alpha0_C_read_and_write_only"] = t_us(lambda: H.hclooc_dgemm_ex(ctx, M, N, K, 0.0, A, K, B, N, wl["beta"], C, N, budget))
+        out["call_128x128x16_launch_and_sync_floor"] = t_us(lambda: H.hclooc_dgemm_ex(ctx, 128, 128, 16, wl["alpha"], A, K, B, N, 0.0, C, N, budget))
+        nb_in, nb_out = 8 * (M * K + K * N + M * N), 8 * M * N
+        d = H.hclMalloc(nb_in)
+        s0 = H.hclStreamCreate()
+
+        def copies():
+            H.hclMemcpyAsync(d, A, 8 * M * K, H.HCL_H2D, s0); H.hclMemcpyAsync(d + 8 * M * K, B, 8 * K * N, H.HCL_H2D, s0)
+            H.hclMemcpyAsync(d + 8 * (M * K + K * N), C, 8 * M * N, H.HCL_H2D, s0); H.hclMemcpyAsync(C, d, nb_out, H.HCL_D2H, s0)
+            H.hclStreamSynchronize(s0)
+            return st
+        out["four_plain_copies_of_the_same_bytes"] = t_us(copies)
+        t_roof, t_flop, t_link = link_roofline_s(2.0 * M * N * K, st.bytes_h2d, st.bytes_d2h)
+        out["roofline_us"] = 1e6 * t_roof
+        out["frac_of_roofline"] = 1e6 * t_roof / out["call"]
+        floor = out["call_128x128x16_launch_and_sync_floor"]
+        out["cap_on_frac_from_the_floor"] = 1e6 * t_roof / (1e6 * t_roof + floor)
+        out["link_peaks"] = LINK
+        H.hclFree(d); H.hclStreamDestroy(s0)
+        H.hclooc_ctx_destroy(ctx)
+        if self.rank == 0:
+            print(json.dumps(out))
 
     def kernel_only(self):
         """Only the kernel legs (for ncu captures of the tile kernel at the workload's step shape)."""
@@ -758,6 +809,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-per-config", action="store_true", help="skip the cfg1-cfg4 block of the default (auto) run")
     ap.add_argument("--no-in-core", action="store_true")
+    ap.add_argument("--no-calibrate", action="store_true", help="leave the planner's cost model on its default link rates")
+    ap.add_argument("--phases", action="store_true", help="--workload cfg1: where the time of the call goes (launch + synchronisation floor, "
+                                                          "C read, C write, operand stream), one JSON line")
     ap.add_argument("--trans", default="NN", choices=["NN", "TN", "NT", "TT"],
                     help="e2e leg through hclooc_dgemm_t with op(A), op(B) transposed (the same buffers read as the stored K x M / N x K matrices)")
     ap.add_argument("--kernel-only", action="store_true", help="only the kernel legs (for ncu captures of the tile kernel)")
@@ -782,6 +836,8 @@ def main():
     if args.impl == "reference":
         return run_reference(args)
     b = Bench(args)
+    if args.phases:
+        return b.phases()
     if args.kernel_only:
         return b.kernel_only()
     b.run()

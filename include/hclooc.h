@@ -199,6 +199,12 @@ int hclooc_ctx_set_trace(hclooc_ctx* ctx, int enable);
  * is staged through device buffers), 1 = always when the operands allow it.  -2: mode outside {-1, 0, 1}.   */
 int hclooc_ctx_set_direct(hclooc_ctx* ctx, int mode);
 int hclooc_ctx_get_trace(hclooc_ctx* ctx, hclooc_trace_rec* recs, size_t max_recs, size_t* n_recs);
+/* Calibrates the planner's cost model to THIS box: measures the host link of the context's device (256 MiB of pinned 64 MiB copies:
+ * host->device alone, device->host alone, both at once; about 60 ms) and replaces the model's default rates -- those of the first
+ * box probed, 55.5 / 51.5 / 88 GB/s; the boxes of a pool differ by 10 % -- for every later plan of the process (rates pinned by
+ * the HCLOOC_*_GBPS environment variables stay).  The three outputs (nullable) receive the rates in GB/s.  ctx == NULL: default
+ * context.  Errors: HCLOOC_ERR_CUDA (allocation or copy failed; the model is left as it was).                               */
+int hclooc_calibrate_link(hclooc_ctx* ctx, double* h2d_GBps, double* d2h_GBps, double* duplex_GBps);
 /* Debug shaker (the rule it exercises is PAPER.md:311: "data stored in device buffers is not overwritten until
  * kernel executions that operate on the data have completed").  jitter_seed != 0: every copy and kernel the library enqueues on this
  * context -- the DGEMM pipeline, the device phases of hclooc_dtrsm[_side] and hclooc_dpotrf -- is preceded, with probability 1/2,

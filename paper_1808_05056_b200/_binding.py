@@ -17,7 +17,7 @@ HCL_SIDE_LEFT, HCL_SIDE_RIGHT = 0, 1
 # every symbol include/hclooc.h declares (tests check the .so exports all of them)
 EXPORTS = [
     "hclooc_plan", "hclooc_plan_ex", "hclooc_plan_trans", "hclooc_shard_rows", "hclMatrixPartitioner", "hclooc_schedule", "hclooc_ctx_create", "hclooc_ctx_destroy",
-    "hclooc_ctx_set_trace", "hclooc_ctx_get_trace", "hclooc_ctx_set_direct", "hclooc_ctx_set_debug",
+    "hclooc_ctx_set_trace", "hclooc_ctx_get_trace", "hclooc_ctx_set_direct", "hclooc_ctx_set_debug", "hclooc_calibrate_link",
     "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_t", "hclooc_dsyrk", "hclooc_dsyr2k", "hclooc_dtrsm", "hclooc_dtrsm_plan", "hclooc_dtrsm_side", "hclooc_dpotrf", "hclooc_dpotrf_plan", "hclooc_dgemm_fig2", "hclooc_dgemm_nsteps", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
     "hclStreamDestroy", "hclEventDestroy", "hclMemcpy", "hclMemcpyAsync", "hclMemcpy2DAsync",
     "hclDgemmAsync", "hclDgemmAsyncEx", "hclDgemmAsyncT", "hclDtrsmAsync", "hclDpotrfAsync", "hclWaitEvent", "hclStreamSynchronize", "hclDeviceSynchronize",
@@ -88,6 +88,7 @@ def lib():
         L.hclooc_ctx_get_trace.argtypes = [vp, vp, sz, POINTER(sz)]
         L.hclooc_ctx_set_direct.argtypes = [vp, c_int]
         L.hclooc_ctx_set_debug.argtypes = [vp, c_uint64, c_int]
+        L.hclooc_calibrate_link.argtypes = [vp, POINTER(c_double), POINTER(c_double), POINTER(c_double)]
         L.hclooc_dgemm.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz]
         L.hclooc_dgemm_ex.argtypes = [vp, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
         L.hclooc_dgemm_t.argtypes = [vp, c_int, c_int, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
@@ -283,6 +284,13 @@ def hclooc_ctx_set_trace(ctx, enable: bool) -> None:
 
 def hclooc_ctx_set_direct(ctx, mode: int) -> None:
     _check(lib().hclooc_ctx_set_direct(ctx, int(mode)), "hclooc_ctx_set_direct")
+
+
+def hclooc_calibrate_link(ctx=None):
+    """(h2d, d2h, duplex) in GB/s as measured on this box; the planner's cost model uses them from now on."""
+    a, b, c = c_double(), c_double(), c_double()
+    _check(lib().hclooc_calibrate_link(ctx, byref(a), byref(b), byref(c)), "hclooc_calibrate_link")
+    return a.value, b.value, c.value
 
 
 def hclooc_ctx_set_debug(ctx, jitter_seed: int, poison) -> None:

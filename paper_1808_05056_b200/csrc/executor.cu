@@ -1292,6 +1292,56 @@ extern "C" int hclooc_ctx_set_trace(hclooc_ctx* ctx, int enable) {
     return HCLOOC_OK;
 }
 
+// Measures the host link of the current device -- 256 MiB pinned, 4 copies of 64 MiB per direction alone, then both at once -- and
+// hands the rates to the planner's cost model (they stay in force for the process; plans cached by contexts are dropped lazily:
+// a context re-plans when its cache misses).  About 60 ms.
+extern "C" int hclooc_calibrate_link(hclooc_ctx* ctx, double* h2d_GBps, double* d2h_GBps, double* duplex_GBps) {
+    int rc;
+    if (!ctx && (rc = default_ctx(&ctx))) return rc;
+    std::lock_guard<std::mutex> lk(ctx->mu);
+    HCL_CUDA(cudaSetDevice(ctx->device));
+    const size_t chunk = (size_t)64 << 20, total = 4 * chunk;
+    void *ha = nullptr, *hb = nullptr, *da = nullptr, *db = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    double rate[3] = {0, 0, 0};
+    cudaError_t e = cudaHostAlloc(&ha, total, cudaHostAllocDefault);
+    if (e == cudaSuccess) e = cudaHostAlloc(&hb, total, cudaHostAllocDefault);
+    if (e == cudaSuccess) e = cudaMalloc(&da, total);
+    if (e == cudaSuccess) e = cudaMalloc(&db, total);
+    if (e == cudaSuccess) e = cudaEventCreate(&e0);
+    if (e == cudaSuccess) e = cudaEventCreate(&e1);
+    if (e == cudaSuccess) {
+        std::memset(ha, 0, total);
+        for (int mode = 0; mode < 3 && e == cudaSuccess; ++mode) {          // 0: up, 1: down, 2: both
+            for (int rep = 0; rep < 2 && e == cudaSuccess; ++rep) {          // the first round warms up
+                cudaStreamSynchronize(ctx->s_h2d); cudaStreamSynchronize(ctx->s_d2h);
+                const auto t0 = std::chrono::steady_clock::now();
+                for (size_t off = 0; off < total; off += chunk) {
+                    if (mode != 1) cudaMemcpyAsync((char*)da + off, (char*)ha + off, chunk, cudaMemcpyHostToDevice, ctx->s_h2d);
+                    if (mode != 0) cudaMemcpyAsync((char*)hb + off, (char*)db + off, chunk, cudaMemcpyDeviceToHost, ctx->s_d2h);
+                }
+                e = cudaStreamSynchronize(ctx->s_h2d);
+                if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->s_d2h);
+                const double t = std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+                if (rep == 1) rate[mode] = (mode == 2 ? 2.0 : 1.0) * (double)total / t;
+            }
+        }
+    }
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (da) cudaFree(da);
+    if (db) cudaFree(db);
+    if (ha) cudaFreeHost(ha);
+    if (hb) cudaFreeHost(hb);
+    if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(e); }
+    set_machine_link(rate[0], rate[1], rate[2]);
+    ctx->plan_cache.clear();
+    if (h2d_GBps) *h2d_GBps = rate[0] / 1e9;
+    if (d2h_GBps) *d2h_GBps = rate[1] / 1e9;
+    if (duplex_GBps) *duplex_GBps = rate[2] / 1e9;
+    return HCLOOC_OK;
+}
+
 extern "C" int hclooc_ctx_set_debug(hclooc_ctx* ctx, uint64_t jitter_seed, int poison) {
     int rc;
     if (!ctx && (rc = default_ctx(&ctx))) return rc;

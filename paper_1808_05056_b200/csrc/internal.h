@@ -30,6 +30,7 @@ struct MachineModel {
     double launch_latency_s;
 };
 const MachineModel& machine_model();
+void set_machine_link(double h2d_Bps, double d2h_Bps, double duplex_Bps);   // hclooc_calibrate_link
 
 // Launch the tile kernel: dC = alpha*dA*dB + beta*dC on device pointers (row-major).
 // Preconditions (checked by callers): pointers 16-byte aligned, leading dimensions even.

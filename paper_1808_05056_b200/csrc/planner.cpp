@@ -37,16 +37,28 @@ constexpr double OVERLAP_PENALTY = 0.02;   // measured: with the link 70 % busy 
 constexpr double STREAMK_MIN_TILES = 32;
 }  // namespace
 
-const MachineModel& machine_model() {
-    static const MachineModel mm = {
+namespace {
+MachineModel& model_storage() {
+    static MachineModel mm = {
         env_or("HCLOOC_FP64_TFLOPS", 37.17) * 1e12,   // DMMA loop, 148 SMs, sustained (profiles/r01_box_probe.md)
-        env_or("HCLOOC_H2D_GBPS", 55.5) * 1e9,
-        env_or("HCLOOC_D2H_GBPS", 51.5) * 1e9,
+        env_or("HCLOOC_H2D_GBPS", 55.5) * 1e9,        // link rates of the first box probed; hclooc_calibrate_link() replaces them with
+        env_or("HCLOOC_D2H_GBPS", 51.5) * 1e9,        // what THIS box measures (the boxes of the pool differ: 51.5-57 D2H, 88-100 duplex)
         env_or("HCLOOC_DUPLEX_GBPS", 88.0) * 1e9,
         env_or("HCLOOC_COPY_LATENCY_US", 8.0) * 1e-6, // per copy inside the pipeline (event waits between copies); 4-5 us back to back
         env_or("HCLOOC_LAUNCH_LATENCY_US", 5.0) * 1e-6,
     };
     return mm;
+}
+}  // namespace
+
+const MachineModel& machine_model() { return model_storage(); }
+
+// measured link rates replace the defaults (not a rate the environment pins)
+void set_machine_link(double h2d_Bps, double d2h_Bps, double duplex_Bps) {
+    MachineModel& mm = model_storage();
+    if (!std::getenv("HCLOOC_H2D_GBPS") && h2d_Bps > 1e9) mm.h2d_Bps = h2d_Bps;
+    if (!std::getenv("HCLOOC_D2H_GBPS") && d2h_Bps > 1e9) mm.d2h_Bps = d2h_Bps;
+    if (!std::getenv("HCLOOC_DUPLEX_GBPS") && duplex_Bps > 1e9) mm.duplex_Bps = duplex_Bps;
 }
 
 int g_direct_max_cluster = 16;      // what direct_max_cluster() found on the device (set by the executor); 16 on a B200
