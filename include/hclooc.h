@@ -359,6 +359,30 @@ int hclooc_dpotrf(hclooc_ctx* ctx, int uplo, int64_t N, double* A, int64_t lda, 
  * Errors: -1 N < 1, -3 NULL output, HCLOOC_ERR_BUDGET.                                                                      */
 int hclooc_dpotrf_plan(int64_t N, size_t device_budget_bytes, int64_t* NB, uint64_t* panel_bytes);
 
+/* Out-of-core DTRMM and DSYMM (the paper's future work, :412: "full support for level-3 BLAS kernels"): the routines whose operand
+ * is a TRIANGLE of a stored matrix.  The pipeline streams the stored matrix as it is and the tile kernel is told which part of
+ * op(A) / op(B) counts: a tile runs only over the k blocks that can hold counted elements, and in the blocks that cross the
+ * diagonal the rest is zeroed by a select -- the other triangle (and a unit diagonal) is never multiplied, NaN there is harmless.
+ *   hclooc_dtrmm:  B := alpha * op(T) * B (side = HCL_SIDE_LEFT, T = the `uplo` triangle of the M x M matrix A) or
+ *     B := alpha * B * op(T) (HCL_SIDE_RIGHT, A is N x N), B is M x N (ldb >= N), IN PLACE.  Left: one pass of the pipeline with C = B
+ *     (a step reads device copies of its operands made before the first block of its column is stored; needs a budget that holds a
+ *     16-column slice of B without K panels, else HCLOOC_ERR_BUDGET).  Right: B goes through the device in row bands (a band is copied
+ *     up once, at most a quarter of the budget, and is the left operand of its own pass).  diag = HCL_DIAG_UNIT: the strict triangle
+ *     multiplies and B itself enters as beta * C with beta = alpha.  alpha == 0: B = 0, A not referenced.
+ *     Errors: -2 side, -3 uplo, -4 trans, -5 diag, -6 M < 0, -7 N < 0, -9 A NULL, -10 lda too small, -11 B NULL or overlapping A,
+ *     -12 ldb < N, and the HCLOOC_ERR_* codes.  stats: plan of the (last) pass, byte / copy / kernel counts summed, plan.flops = M*N*n.
+ *   hclooc_dsymm:  C := alpha * S * B + beta * C (HCL_SIDE_LEFT, S is M x M) or alpha * B * S + beta * C (HCL_SIDE_RIGHT, S is N x N), S the
+ *     symmetric matrix whose `uplo` triangle is stored in A (the other triangle is never read), B and C M x N.  Two passes of the
+ *     pipeline: the stored triangle, then its strict part read transposed with beta' = 1 (rounding: the first partial sum is rounded
+ *     into C with beta*C, the second is added; within the gate of hclooc_dgemm, exact on integers).  alpha == 0: C = beta*C.
+ *     Errors: -2 side, -3 uplo, -4 M < 0, -5 N < 0, -7 A NULL, -8 lda, -9 B NULL, -10 ldb < N, -12 C NULL or overlapping A or B,
+ *     -13 ldc < N, and the HCLOOC_ERR_* codes.  stats: sums over the two passes, plan.flops = 2*M*N*n.                          */
+int hclooc_dtrmm(hclooc_ctx* ctx, int side, int uplo, int trans, int diag, int64_t M, int64_t N, double alpha,
+                 const double* A, int64_t lda, double* B, int64_t ldb, size_t device_budget_bytes, hclooc_stats* stats_out);
+int hclooc_dsymm(hclooc_ctx* ctx, int side, int uplo, int64_t M, int64_t N, double alpha, const double* A, int64_t lda,
+                 const double* B, int64_t ldb, double beta, double* C, int64_t ldc, size_t device_budget_bytes,
+                 hclooc_stats* stats_out);
+
 /* nsteps mode (:277-283): MMOOC as a subroutine of a blocked algorithm (SUMMA, HSUMMA) that updates the same C
  * `nsteps` times: C = alpha*A_p*B_p + beta_p*C for p = *step = 0 .. nsteps-1, one call per p.  C is uploaded once
  * at step 0 (if beta != 0), stays in device memory between the calls, and is downloaded once at the last step, so

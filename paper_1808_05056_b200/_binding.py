@@ -18,7 +18,7 @@ HCL_SIDE_LEFT, HCL_SIDE_RIGHT = 0, 1
 EXPORTS = [
     "hclooc_plan", "hclooc_plan_ex", "hclooc_plan_trans", "hclooc_shard_rows", "hclMatrixPartitioner", "hclooc_schedule", "hclooc_ctx_create", "hclooc_ctx_destroy",
     "hclooc_ctx_set_trace", "hclooc_ctx_get_trace", "hclooc_ctx_set_direct", "hclooc_ctx_set_debug", "hclooc_calibrate_link",
-    "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_t", "hclooc_dsyrk", "hclooc_dsyr2k", "hclooc_dtrsm", "hclooc_dtrsm_plan", "hclooc_dtrsm_side", "hclooc_dpotrf", "hclooc_dpotrf_plan", "hclooc_dgemm_fig2", "hclooc_dgemm_nsteps", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
+    "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_t", "hclooc_dsyrk", "hclooc_dsyr2k", "hclooc_dtrsm", "hclooc_dtrsm_plan", "hclooc_dtrsm_side", "hclooc_dpotrf", "hclooc_dpotrf_plan", "hclooc_dtrmm", "hclooc_dsymm", "hclooc_dgemm_fig2", "hclooc_dgemm_nsteps", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
     "hclStreamDestroy", "hclEventDestroy", "hclMemcpy", "hclMemcpyAsync", "hclMemcpy2DAsync",
     "hclDgemmAsync", "hclDgemmAsyncEx", "hclDgemmAsyncT", "hclDtrsmAsync", "hclDpotrfAsync", "hclWaitEvent", "hclStreamSynchronize", "hclDeviceSynchronize",
     "hclooc_host_alloc", "hclooc_host_free", "hclooc_host_register", "hclooc_host_unregister",
@@ -96,6 +96,8 @@ def lib():
         L.hclooc_dtrsm_plan.argtypes = [i64, i64, sz, c_int, POINTER(i64), POINTER(i64), POINTER(c_int), POINTER(ctypes.c_uint64)]
         L.hclooc_dtrsm.argtypes = [vp, c_int, c_int, c_int, i64, i64, dbl, vp, i64, vp, i64, sz, POINTER(Stats)]
         L.hclooc_dtrsm_side.argtypes = [vp, c_int, c_int, c_int, c_int, i64, i64, dbl, vp, i64, vp, i64, sz, POINTER(Stats)]
+        L.hclooc_dtrmm.argtypes = [vp, c_int, c_int, c_int, c_int, i64, i64, dbl, vp, i64, vp, i64, sz, POINTER(Stats)]
+        L.hclooc_dsymm.argtypes = [vp, c_int, c_int, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
         L.hclooc_dpotrf.argtypes = [vp, c_int, i64, vp, i64, sz, POINTER(i64), POINTER(Stats)]
         L.hclooc_dpotrf_plan.argtypes = [i64, sz, POINTER(i64), POINTER(ctypes.c_uint64)]
         L.hclooc_dsyr2k.argtypes = [vp, c_int, c_int, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
@@ -363,6 +365,18 @@ def hclooc_dtrsm_side(ctx, side, uplo, trans, diag, M, N, alpha, A, lda, B, ldb,
     _check(lib().hclooc_dtrsm_side(ctx, side, uplo, trans, diag, M, N, alpha, _ptr(A), lda, _ptr(B), ldb, device_budget_bytes,
                                    byref(st) if want_stats else None), "hclooc_dtrsm_side")
     return st if want_stats else None
+
+
+def hclooc_dtrmm(ctx, side, uplo, trans, diag, M, N, alpha, A, lda, B, ldb, device_budget_bytes):
+    st = Stats()
+    _check(lib().hclooc_dtrmm(ctx, side, uplo, trans, diag, M, N, alpha, _ptr(A), lda, _ptr(B), ldb, device_budget_bytes, byref(st)), "hclooc_dtrmm")
+    return st
+
+
+def hclooc_dsymm(ctx, side, uplo, M, N, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes):
+    st = Stats()
+    _check(lib().hclooc_dsymm(ctx, side, uplo, M, N, alpha, _ptr(A), lda, _ptr(B), ldb, beta, _ptr(C), ldc, device_budget_bytes, byref(st)), "hclooc_dsymm")
+    return st
 
 
 def hclooc_dpotrf(ctx, uplo, N, A, lda, device_budget_bytes):

@@ -138,8 +138,18 @@ struct FragLanesT {
 using FragLanes = FragLanesT<false, false>;
 
 // One k block (BK deep) of the 32 x 64 warp tile: per group of 8 k, 12 LDS.128 feed 64 DMMA.8x8x4.
-template <bool TA, bool TB>
-__device__ __forceinline__ void mma_kblock(double (&acc)[4][4][2][2], uint32_t sbase, const FragLanesT<TA, TB>& f) {
+// MASK (hclooc_dtrmm, hclooc_dsymm: an operand that is a triangle of a stored matrix whose other triangle must not count): the
+// fragments of the k blocks that cross the diagonal are zeroed where they fall outside the triangle --
+//   am = 1: op(A)[r][k] counts iff k <= r + da,   am = 2: iff k >= r + da          (r, k: indices inside the tile / k block)
+//   bm = 1: op(B)[k][c] counts iff c <= k + db,   bm = 2: iff c >= k + db
+// -- by a select, never by a product (the other triangle may hold NaN).  Index maps: a[u][e] is row f.row_of(u), k = 8kg + 2t + e;
+// b[bx][v] (k-step e) is column 16bx + 2g + v (B as stored) or 8(2bx + v) + rp (B^T) of the warp's 64, same k.
+__device__ __forceinline__ bool mask_keep(int m, int major, int minor, int d) {      // m = 1: minor <= major + d, m = 2: minor >= major + d
+    return m == 1 ? minor <= major + d : minor >= major + d;
+}
+template <bool TA, bool TB, bool MASK = false>
+__device__ __forceinline__ void mma_kblock(double (&acc)[4][4][2][2], uint32_t sbase, const FragLanesT<TA, TB>& f,
+                                           int am = 0, int da = 0, int bm = 0, int db = 0) {
     #pragma unroll
     for (int kg = 0; kg < BK / 8; ++kg) {
         double a[4][2];
@@ -154,6 +164,13 @@ __device__ __forceinline__ void mma_kblock(double (&acc)[4][4][2][2], uint32_t s
                 for (int ub = 0; ub < 2; ++ub)
                     lds128(a[2 * ub][e], a[2 * ub + 1][e], sbase + f.a_lane_t[e] + kg * 1024 + ub * B_BOX_BYTES);
         }
+        if (MASK && am) {
+            #pragma unroll
+            for (int u = 0; u < 4; ++u)
+                #pragma unroll
+                for (int e = 0; e < 2; ++e)
+                    if (!mask_keep(am, f.row_of(u), kg * 8 + 2 * f.t + e, da)) a[u][e] = 0.0;
+        }
         if (!TB) {
             #pragma unroll
             for (int e = 0; e < 2; ++e) {
@@ -161,6 +178,13 @@ __device__ __forceinline__ void mma_kblock(double (&acc)[4][4][2][2], uint32_t s
                 #pragma unroll
                 for (int bx = 0; bx < 4; ++bx)
                     lds128(b[bx][0], b[bx][1], sbase + f.b_lane[e] + kg * 1024 + bx * B_BOX_BYTES);
+                if (MASK && bm) {
+                    #pragma unroll
+                    for (int bx = 0; bx < 4; ++bx)
+                        #pragma unroll
+                        for (int v = 0; v < 2; ++v)
+                            if (!mask_keep(bm, kg * 8 + 2 * f.t + e, f.wn * 64 + 16 * bx + 2 * f.g + v, db)) b[bx][v] = 0.0;
+                }
                 #pragma unroll
                 for (int u = 0; u < 4; ++u)
                     #pragma unroll
@@ -176,6 +200,13 @@ __device__ __forceinline__ void mma_kblock(double (&acc)[4][4][2][2], uint32_t s
                 double b[2][2][2];                        // [bx in half][v][e]
                 #pragma unroll
                 for (int q = 0; q < 4; ++q) lds128(b[q >> 1][q & 1][0], b[q >> 1][q & 1][1], bbase + (half * 4 + q) * 1024);
+                if (MASK && bm) {
+                    #pragma unroll
+                    for (int q = 0; q < 4; ++q)
+                        #pragma unroll
+                        for (int e = 0; e < 2; ++e)
+                            if (!mask_keep(bm, kg * 8 + 2 * f.t + e, f.wn * 64 + 8 * (half * 4 + q) + f.rp, db)) b[q >> 1][q & 1][e] = 0.0;
+                }
                 #pragma unroll
                 for (int e = 0; e < 2; ++e)
                     #pragma unroll

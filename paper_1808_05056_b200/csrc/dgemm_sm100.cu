@@ -37,11 +37,16 @@ using namespace dev;
 // runs the epilogue.  Used when a pipeline step has too few tiles to fill 148 SMs.
 // TA / TB: the operand is stored transposed (A as K x M, B as N x K; hclooc_dgemm_t): only the TMA boxes and the fragment
 // addressing change (dgemm_device.cuh), the DMMA loop and the order of summation over k do not.
-template <int KSPLIT, bool TA = false, bool TB = false>
+// MASK (KSPLIT == 1 only; hclooc_dtrmm / hclooc_dsymm): op(A) and / or op(B) is a TRIANGLE of the stored operand -- opmask = am | bm << 2,
+// am / bm = 0 none, 1: op(A)[r][k] counts iff k <= r + adoff resp. op(B)[k][c] iff c <= k + bdoff, 2: iff >= (indices of this launch).
+// A tile runs only over the k blocks that can hold counted elements, and the blocks that cross a diagonal zero the rest by a
+// select in registers (mma_kblock<.., MASK>): what lies outside the triangle is never multiplied, NaN there is harmless.
+template <int KSPLIT, bool TA = false, bool TB = false, bool MASK = false>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 hclooc_dgemm_tile_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                          double* __restrict__ C, long long ldc, int M, int N, int K,
-                         double alpha, double beta, int tiles_m, int tiles_n, int tri, int doff) {
+                         double alpha, double beta, int tiles_m, int tiles_n, int tri, int doff,
+                         int opmask = 0, int adoff = 0, int bdoff = 0) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;   // 128B swizzle wants 1 KiB alignment
     const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;          // full[s] at +8s, empty[s] at +8(STAGES+s)
@@ -58,8 +63,21 @@ hclooc_dgemm_tile_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_c
     if (tri == 2 && min(n0 + BN, N) - 1 < m0 + doff) return;
     const int num_kb_all = (K + BK - 1) / BK;
     const uint32_t crank = (KSPLIT == 1) ? 0u : cluster_ctarank();
-    const int kb_begin = (KSPLIT == 1) ? 0 : (int)(((long long)num_kb_all * crank) / KSPLIT);
-    const int kb_end = (KSPLIT == 1) ? num_kb_all : (int)(((long long)num_kb_all * (crank + 1)) / KSPLIT);
+    int kb_begin = (KSPLIT == 1) ? 0 : (int)(((long long)num_kb_all * crank) / KSPLIT);
+    int kb_end = (KSPLIT == 1) ? num_kb_all : (int)(((long long)num_kb_all * (crank + 1)) / KSPLIT);
+    const int am = MASK ? (opmask & 3) : 0, bm = MASK ? ((opmask >> 2) & 3) : 0;
+    if (MASK) {
+        // the k range in which this tile's rows of op(A) / columns of op(B) can hold counted elements
+        long long klo = 0, khi = K;
+        const int m1 = min(m0 + BM, M) - 1, n1 = min(n0 + BN, N) - 1;
+        if (am == 1) khi = min(khi, (long long)m1 + adoff + 1);
+        if (am == 2) klo = max(klo, (long long)m0 + adoff);
+        if (bm == 1) klo = max(klo, (long long)n0 - bdoff);          // c <= k + bdoff  <=>  k >= c - bdoff
+        if (bm == 2) khi = min(khi, (long long)n1 - bdoff + 1);
+        kb_begin = (int)(max(klo, 0LL) / BK);
+        kb_end = khi <= 0 ? 0 : (int)((khi + BK - 1) / BK);
+        if (kb_end < kb_begin) kb_end = kb_begin;
+    }
     const int num_kb = kb_end - kb_begin;
 
     if (threadIdx.x == 0) {
@@ -131,7 +149,16 @@ hclooc_dgemm_tile_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_c
         if (nu != 0 && nbx != 0) {
             for (int kb = 0; kb < num_kb; ++kb) {
                 mbar_wait(bar_base + 8 * stage, phase);
-                mma_kblock(acc, smem_base + stage * STAGE_BYTES, f);
+                if (MASK) {
+                    // tile-local offsets of the diagonals in this k block; the block needs the select only if it crosses one
+                    const int k0 = (kb_begin + kb) * BK;
+                    const int da = m0 + adoff - k0, db = k0 + bdoff - n0;
+                    const bool cross = (am == 1 && BK - 1 > da) || (am == 2 && 0 < BM - 1 + da) || (bm == 1 && BN - 1 > db) || (bm == 2 && 0 < BK - 1 + db);
+                    if (cross) mma_kblock<TA, TB, true>(acc, smem_base + stage * STAGE_BYTES, f, am, da, bm, db);
+                    else mma_kblock(acc, smem_base + stage * STAGE_BYTES, f);
+                } else {
+                    mma_kblock(acc, smem_base + stage * STAGE_BYTES, f);
+                }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(bar_base + 8 * (STAGES + stage));
                 if (++stage == STAGES) { stage = 0; phase ^= 1u; }
@@ -234,6 +261,7 @@ cudaError_t set_attr_all_splits() {
     cudaError_t e = cudaFuncSetAttribute(hclooc_dgemm_tile_kernel<1, TA, TB>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(hclooc_dgemm_tile_kernel<2, TA, TB>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(hclooc_dgemm_tile_kernel<4, TA, TB>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(hclooc_dgemm_tile_kernel<1, TA, TB, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
     return e;
 }
 
@@ -265,12 +293,17 @@ cudaError_t launch_split(unsigned tiles, cudaStream_t stream, const CUtensorMap&
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, hclooc_dgemm_tile_kernel<KSPLIT, TA, TB>, tmA, tmB, dC, ldc, M, N, K, alpha, beta, tm, tn, tri, doff);
+    return cudaLaunchKernelEx(&cfg, hclooc_dgemm_tile_kernel<KSPLIT, TA, TB>, tmA, tmB, dC, ldc, M, N, K, alpha, beta, tm, tn, tri, doff, 0, 0, 0);
 }
 
 template <bool TA, bool TB>
 cudaError_t launch_any_split(int ksplit, unsigned tiles, cudaStream_t stream, const CUtensorMap& tmA, const CUtensorMap& tmB, double* dC,
-                             long long ldc, int M, int N, int K, double alpha, double beta, int tm, int tn, int tri, int doff) {
+                             long long ldc, int M, int N, int K, double alpha, double beta, int tm, int tn, int tri, int doff,
+                             int opmask = 0, int adoff = 0, int bdoff = 0) {
+    if (opmask) {      // a triangular operand: one CTA per tile, each over its own k range
+        hclooc_dgemm_tile_kernel<1, TA, TB, true><<<tiles, NUM_THREADS, SMEM_BYTES, stream>>>(tmA, tmB, dC, ldc, M, N, K, alpha, beta, tm, tn, tri, doff, opmask, adoff, bdoff);
+        return cudaGetLastError();
+    }
     if (ksplit >= 4) return launch_split<4, TA, TB>(tiles, stream, tmA, tmB, dC, ldc, M, N, K, alpha, beta, tm, tn, tri, doff);
     if (ksplit >= 2) return launch_split<2, TA, TB>(tiles, stream, tmA, tmB, dC, ldc, M, N, K, alpha, beta, tm, tn, tri, doff);
     hclooc_dgemm_tile_kernel<1, TA, TB><<<tiles, NUM_THREADS, SMEM_BYTES, stream>>>(tmA, tmB, dC, ldc, M, N, K, alpha, beta, tm, tn, tri, doff);
@@ -290,7 +323,7 @@ int dgemm_auto_ksplit(int64_t tiles_in_flight, int64_t K) {
 
 int launch_dgemm_tiles(int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda,
                        const double* dB, int64_t ldb, double beta, double* dC, int64_t ldc, cudaStream_t stream,
-                       int ksplit, void* streamk_scratch, int transa, int transb, int tri, int doff) {
+                       int ksplit, void* streamk_scratch, int transa, int transb, int tri, int doff, int opmask, int adoff, int bdoff) {
     if (M == 0 || N == 0) return HCLOOC_OK;
     if (alpha == 0.0) K = 0;                       // A and B are not referenced (BLAS convention)
     int rc = ensure_kernel_attr();
@@ -309,6 +342,11 @@ int launch_dgemm_tiles(int64_t M, int64_t N, int64_t K, double alpha, const doub
     static const bool no_streamk = getenv("HCLOOC_NO_STREAMK") != nullptr;   // experiment knob
     if (tri != 0 && (doff > 0x3fffffff || doff < -0x3fffffff)) return HCLOOC_ERR_INTERNAL;
     if (ksplit < 0 && tri != 0) ksplit = 0;                    // the persistent kernel has no triangle mask
+    if (K == 0) opmask = 0;
+    if (opmask) {
+        ksplit = 1;
+        if (adoff > 0x3fffffff || adoff < -0x3fffffff || bdoff > 0x3fffffff || bdoff < -0x3fffffff) return HCLOOC_ERR_INTERNAL;
+    }
     if (ksplit < 0 && K > 0 && !no_streamk) {
         // A launch that has the GPU to itself.  One CTA per tile runs its main loop ~1 % faster than the persistent
         // kernel (measured 0.981 against 0.969 of peak on whole waves) but leaves the last wave partly empty, so
@@ -325,10 +363,10 @@ int launch_dgemm_tiles(int64_t M, int64_t N, int64_t K, double alpha, const doub
     if (K == 0) ksplit = 1;
     const unsigned tiles = (unsigned)(tm * tn);
     cudaError_t e;
-    if (transa && transb) e = launch_any_split<true, true>(ksplit, tiles, stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn, tri, doff);
-    else if (transa) e = launch_any_split<true, false>(ksplit, tiles, stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn, tri, doff);
-    else if (transb) e = launch_any_split<false, true>(ksplit, tiles, stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn, tri, doff);
-    else e = launch_any_split<false, false>(ksplit, tiles, stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn, tri, doff);
+    if (transa && transb) e = launch_any_split<true, true>(ksplit, tiles, stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn, tri, doff, opmask, adoff, bdoff);
+    else if (transa) e = launch_any_split<true, false>(ksplit, tiles, stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn, tri, doff, opmask, adoff, bdoff);
+    else if (transb) e = launch_any_split<false, true>(ksplit, tiles, stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn, tri, doff, opmask, adoff, bdoff);
+    else e = launch_any_split<false, false>(ksplit, tiles, stream, tmA, tmB, dC, (long long)ldc, (int)M, (int)N, (int)K, alpha, beta, (int)tm, (int)tn, tri, doff, opmask, adoff, bdoff);
     if (e != cudaSuccess) return cuda_fail(e);
     return HCLOOC_OK;
 }

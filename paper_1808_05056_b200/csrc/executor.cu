@@ -390,7 +390,8 @@ int dgemm_core_locked(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_
     }
     if (!C) return -10;
     if (ldc < N) return -11;
-    if (!scale_only && (overlaps(C, M, N, ldc, A, a_rows, a_cols, lda) || overlaps(C, M, N, ldc, B, b_rows, b_cols, ldb))) return -10;
+    if (!scale_only && !(extra && extra->in_place) &&
+        (overlaps(C, M, N, ldc, A, a_rows, a_cols, lda) || overlaps(C, M, N, ldc, B, b_rows, b_cols, ldb))) return -10;
     if (scale_only && beta == 1.0) return HCLOOC_OK;            // C = 1*C
     if (scale_only) transa = transb = 0;                        // A and B are not referenced
     if (!ctx) return HCLOOC_ERR_INTERNAL + 1000;                // validation-only pass of dgemm_core: the arguments are fine
@@ -422,7 +423,8 @@ int dgemm_core_locked(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_
     // in-core case: every operand already in device memory and addressable by the tile kernel as it is
     const bool aligned = (((uintptr_t)C & 15u) == 0) && (ldc % 2 == 0) &&
                          (scale_only || ((((uintptr_t)A | (uintptr_t)B) & 15u) == 0 && lda % 2 == 0 && ldb % 2 == 0));
-    const bool in_core = on_device && aligned && M <= 0x7fffffffLL && N <= 0x7fffffffLL && K <= 0x7fffffffLL;
+    const bool masked = extra && (extra->amask || extra->bmask || extra->in_place);     // triangular operands: the staged pipeline only
+    const bool in_core = on_device && aligned && !masked && M <= 0x7fffffffLL && N <= 0x7fffffffLL && K <= 0x7fffffffLL;
     // direct mode needs host matrices the kernel can address as they are: mapped, TMA-legal, host/device address
     // arithmetic interchangeable (the alias of the first element is what the tensor maps are built on)
     static const int direct_env = [] { const char* e = std::getenv("HCLOOC_DIRECT"); return e ? std::atoi(e) : -1; }();
@@ -431,7 +433,7 @@ int dgemm_core_locked(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_
         static std::once_flag once;
         std::call_once(once, [] { set_planner_max_cluster(direct_max_cluster()); });
     }
-    const bool direct_ok = !in_core && !c_dev && aligned && direct_mode != 0 && M <= 0x7fffffffLL && N <= 0x7fffffffLL && K <= 0x7fffffffLL &&
+    const bool direct_ok = !in_core && !c_dev && aligned && !masked && direct_mode != 0 && M <= 0x7fffffffLL && N <= 0x7fffffffLL && K <= 0x7fffffffLL &&
                            C_alias && (((uintptr_t)C_alias & 15u) == 0) &&
                            (scale_only || (A_alias && B_alias && ((((uintptr_t)A_alias | (uintptr_t)B_alias) & 15u) == 0)));
     {
@@ -453,6 +455,7 @@ int dgemm_core_locked(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_
             ctx->plan_cache.emplace_back(key, P);
         }
     }
+    if (extra && extra->in_place && P.kpanels > 1) return HCLOOC_ERR_BUDGET;
     if (in_core || P.direct) {
         const auto t0 = std::chrono::steady_clock::now();
         if (P.direct) { A = (const double*)A_alias; B = (const double*)B_alias; C = (double*)C_alias; }
@@ -648,7 +651,8 @@ int dgemm_core_locked(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_
                 rc = launch_dgemm_tiles(o.nr, o.nc, o.kk, scale_only ? 0.0 : alpha, o.buf >= 0 ? bufs[o.buf] : nullptr, P.lda_dev,
                                         o.buf2 >= 0 ? bufs[o.buf2] : nullptr, P.ldb_dev, b_eff, bufs[o.buf3], P.ldc_dev, st,
                                         P.ksplit != 0 ? P.ksplit : 1, P.ksplit < 0 ? scratch[o.stream - 2] : nullptr, transa, transb,
-                                        tri, (int)(o.r0 - o.c0));
+                                        tri, (int)(o.r0 - o.c0), extra ? (extra->amask | (extra->bmask << 2)) : 0,
+                                        extra ? (int)(o.r0 - o.k0) + extra->adiag : 0, extra ? (int)(o.k0 - o.c0) + extra->bdiag : 0);
                 ++n_kernels;
                 break;
             }

@@ -83,6 +83,12 @@ struct DgemmExtra {
     const double* C_src = nullptr;
     int64_t ldc_src = 0;
     cudaEvent_t wait_before_store[2] = {nullptr, nullptr};
+    // a triangular operand (hclooc_dtrmm, hclooc_dsymm): op(A)[r][k] counts iff k <= r + adiag (amask = 1) / k >= r + adiag (2);
+    // op(B)[k][c] counts iff c <= k + bdiag (bmask = 1) / c >= k + bdiag (2); what lies outside is never read into a product
+    int amask = 0, adiag = 0, bmask = 0, bdiag = 0;
+    // C may overlap an operand (hclooc_dtrmm works in place): legal only with one K panel -- every step then reads device
+    // copies made before the first block of its column is stored -- so a plan with K panels is refused (HCLOOC_ERR_BUDGET)
+    bool in_place = false;
 };
 // the same with ctx->mu already held by the caller (ctx not NULL)
 int dgemm_core_locked(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,

@@ -40,7 +40,10 @@ int launch_dgemm_tiles(int64_t M, int64_t N, int64_t K, double alpha, const doub
                        void* streamk_scratch = nullptr,    // -1 = the launch has the GPU to itself: persistent stream-K
                                                            //      (scratch: streamk_scratch_bytes(), or NULL = library pool)
                        int transa = 0, int transb = 0,     // dA is stored K x M / dB is stored N x K (hclooc_dgemm_t)
-                       int tri = 0, int doff = 0);         // hclooc_dsyrk: store only col <= row + doff (1) / col >= row + doff (2)
+                       int tri = 0, int doff = 0,          // hclooc_dsyrk: store only col <= row + doff (1) / col >= row + doff (2)
+                       int opmask = 0, int adoff = 0, int bdoff = 0);   // hclooc_dtrmm / dsymm: op(A) / op(B) is a triangle of the stored
+                                                           // operand: opmask = am | bm << 2; am = 1: op(A)[r][k] counts iff k <= r + adoff,
+                                                           // 2: iff k >= r + adoff; bm = 1: op(B)[k][c] counts iff c <= k + bdoff, 2: iff >=
 
 // The persistent stream-K kernel (dgemm_streamk_sm100.cu).  Returns 1 if it does not apply (no scratch buffer
 // free, shape out of range): the caller then launches one CTA per tile.
