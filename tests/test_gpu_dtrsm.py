@@ -133,7 +133,10 @@ def test_dtrsm_large_block_rows_of_4096(H, uplo, trans, unit, budget, resident):
     assert (st.plan.mb, st.plan.h) == ((4096, 2) if resident == 0 else (6000, 1))
     assert st.plan.workspace_bytes <= budget and st.plan.n_sets == resident
     ref = B0.copy()
-    oracle.dtrsm(uplo, trans, unit, alpha, A.view, ref)
+    if trans:   # the oracle walks a transposed triangle column-wise (slow); (uplo, T) on A is (other uplo, N) on the written-out transpose, bit for bit (pinned)
+        oracle.dtrsm(1 - uplo, 0, unit, alpha, np.ascontiguousarray(np.nan_to_num(A.view).T), ref)
+    else:
+        oracle.dtrsm(uplo, trans, unit, alpha, A.view, ref)
     assert np.abs(got - ref).max() <= FWD_RTOL * np.abs(ref).max()
     rng = np.random.default_rng(0)
     rows = np.unique(np.concatenate([[0, 127, 128, 4095, 4096, M - 1], rng.integers(0, M, 40)]))

@@ -300,12 +300,24 @@ def test_config2_full_size_every_element(H):
         A, B, C = host_inputs(H, M, N, K, synthgen.BASE_SEED + 2, dist)
         x = synthgen.fill_numpy(N, 1, 77, "A", "int")[:, 0]; y = synthgen.fill_numpy(1, M, 77, "B", "int")[0]
         pre = cks.before(C.view, x, y)
-        ref = C.view.copy()
-        D = oracle.dgemm(1.0, A.view, B.view, 1.0, ref, want_denominator=True)
+        C0 = C.view.copy()
         st = H.hclooc_dgemm_ex(None, M, N, K, 1.0, A, A.ld, B, B.ld, 1.0, C, C.ld, 256 * MiB)
         assert st.plan.workspace_bytes <= 256 * MiB and st.bytes_h2d == st.plan.bytes_h2d and st.plan.n_steps > 16
-        check(C.view, ref, D, exact)
-        Cx, yC, Dx, yD = cks.expected(1.0, A.view, B.view, 1.0, pre, x, y)
+        if not exact:        # the float variant: the full oracle, every element
+            ref = C0
+            D = oracle.dgemm(1.0, A.view, B.view, 1.0, ref, want_denominator=True)
+            check(C.view, ref, D, exact)
+        else:                # the integer variant: oracle rows and columns on both sides of every slab boundary, bit for bit ...
+            plan = st.plan
+            rng = np.random.default_rng(5)
+            rows = {0, M - 1} | {int(v) for v in rng.integers(0, M, 6)} | {i * plan.mb - d for i in (1, plan.h // 2, plan.h - 1) for d in (0, 1)}
+            cols = {0, N - 1} | {int(v) for v in rng.integers(0, N, 6)} | {j * plan.nb - d for j in range(1, plan.w) for d in (0, 1)}
+            rows, cols = np.array(sorted(rows)), np.array(sorted(cols))
+            ref_r, _ = oracle.dgemm_sub(1.0, A.view, B.view, 1.0, C0, rows=rows)
+            ref_c, _ = oracle.dgemm_sub(1.0, A.view, B.view, 1.0, C0, cols=cols)
+            check(C.view[rows], ref_r, None, True)
+            check(C.view[:, cols], ref_c, None, True)
+        Cx, yC, Dx, yD = cks.expected(1.0, A.view, B.view, 1.0, pre, x, y)       # ... and the exact checksums over the whole matrix
         gx, gy = C.view @ x, y @ C.view
         if exact:
             assert np.array_equal(gx, Cx) and np.array_equal(gy, yC)
@@ -321,7 +333,7 @@ def test_k_panels_reread_the_host_block_after_its_download(H, M, N, K, budget):
     block panel p-1's R(c_ij) wrote through ANOTHER C buffer, so the upload must wait for that download (the schedule's
     host-block rule, tests/test_planner_schedule.py).  Integers: every panel's contribution and beta*C0 arrive exactly."""
     plan = H.hclooc_plan(M, N, K, 1, 0, budget)
-    assert plan.kpanels > 1 and (plan.h * plan.w < plan.n_sets or (plan.h * plan.w) % plan.n_sets)
+    assert plan.kpanels > 1 and plan.w == 1          # serpentine order: the last row block of panel p is the first of panel p+1
     for rep in range(3):                                     # a race shows up only sometimes: a few rounds
         A, B, C = host_inputs(H, M, N, K, 340 + rep, "int")
         ref = C.view.copy()
