@@ -669,6 +669,8 @@ def run_op(args):
         LINK.update(live)
     op, M, N, K, budget = args.op, args.m, args.n, args.k, args.budget
     seed = synthgen.BASE_SEED + 9
+    if op in ("dtrsm_dev", "dtrsm_right_dev", "dpotrf_dev"):
+        return run_dev_op(args, H, torch)
     ctx = H.hclooc_ctx_create(0)
     mats = []
 
@@ -741,6 +743,41 @@ def run_op(args):
            "kernels": int(st.n_kernels), "plan": Bench.plan_summary(st.plan), "t_flop_s": t_flop, "t_link_s": t_link,
            "bound": "fp64" if t_flop >= t_link else "link", "frac_of_roofline": t_roof / t, "link_peaks": LINK, "clocks": clocks, **extra}
     print(json.dumps(out))
+
+
+def run_dev_op(args, H, torch):
+    """`--op dtrsm_dev|dtrsm_right_dev|dpotrf_dev`: the DEVICE phases alone (hclDtrsmAsync / hclDpotrfAsync on device-resident operands:
+    recursive halving down to the 128 x 128 block kernels), CUDA events on the launching stream, median of --steps launches.  With
+    --m 128 (dtrsm_dev) / --n 128 (the others) the call is ONE launch of the block kernel."""
+    op, M, N = args.op, args.m, args.n
+    cur = torch.cuda.current_stream()
+    g = torch.Generator(device="cuda"); g.manual_seed(180805056)
+    n = M if op == "dtrsm_dev" else N
+    T = torch.rand((n, n), generator=g, dtype=torch.float64, device="cuda") / n + torch.eye(n, dtype=torch.float64, device="cuda") * 1.5
+    if op == "dpotrf_dev":
+        S = (T + T.T) / 2 + torch.eye(n, dtype=torch.float64, device="cuda")
+        W = S.clone()
+        info = torch.zeros(1, dtype=torch.int64, device="cuda")
+        fn = lambda: H.hclDpotrfAsync(args.uplo, n, W, n, info, cur)
+        pre = lambda: W.copy_(S)
+        flops, shape = n ** 3 / 3.0, {"N": n}
+    else:
+        Bm = torch.rand((M, N), generator=g, dtype=torch.float64, device="cuda")
+        side = 0 if op == "dtrsm_dev" else 1
+        fn = lambda: H.hclDtrsmAsync(side, args.uplo, args.trans, 0, M, N, 1.0, T, n, Bm, N, cur)
+        pre = lambda: None
+        flops, shape = float(M) * N * n, {"M": M, "N": N}
+    torch.cuda.synchronize()
+    ts = []
+    for it in range(3 + max(5, args.steps or 20)):
+        pre()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(cur); fn(); e1.record(cur); e1.synchronize()
+        if it >= 3:
+            ts.append(e0.elapsed_time(e1))
+    ms = float(np.median(ts))
+    print(json.dumps({"op": "hcl" + {"dtrsm_dev": "DtrsmAsync (Left)", "dtrsm_right_dev": "DtrsmAsync (Right)", "dpotrf_dev": "DpotrfAsync"}[op], **shape,
+                      "uplo": args.uplo, "trans": args.trans, "ms": ms, "tflops": flops / ms / 1e9, "frac_of_fp64_peak": flops / ms / 1e9 / FP64_PEAK_TFLOPS}))
 
 
 TRANSITION_SIZES = [4096, 8192, 12288, 16384, 20480, 22528, 23552, 24576, 28672, 32768, 36864, 40960, 46080]
@@ -816,7 +853,7 @@ def main():
     ap.add_argument("--trans", default="NN", choices=["NN", "TN", "NT", "TT"],
                     help="e2e leg through hclooc_dgemm_t with op(A), op(B) transposed (the same buffers read as the stored K x M / N x K matrices)")
     ap.add_argument("--kernel-only", action="store_true", help="only the kernel legs (for ncu captures of the tile kernel)")
-    ap.add_argument("--op", default="dgemm", choices=["dgemm", "dsyrk", "dsyr2k", "dtrsm", "dtrsm_right", "dpotrf"],
+    ap.add_argument("--op", default="dgemm", choices=["dgemm", "dsyrk", "dsyr2k", "dtrsm", "dtrsm_right", "dpotrf", "dtrsm_dev", "dtrsm_right_dev", "dpotrf_dev"],
                     help="time another routine of the library instead (sizes from --m/--n/--k/--budget; --steps calls, the first discarded)")
     ap.add_argument("--sweep", default="", choices=["", "transition"], help="transition: the paper's N sweep across the in-core / out-of-core point")
     ap.add_argument("--m", type=int, default=32768)
