@@ -190,18 +190,22 @@ class HostMatrix:
         self.nbytes = max(1, rows * self.ld) * 8
         # Pinning large buffers fails now and then with cudaErrorOperatingSystem on the B200 boxes when another CUDA process
         # has just exited (the driver still tearing its mappings down); the library retries for ~12 s, this convenience class
-        # for about two minutes more before giving up.
-        for attempt in range(9):
+        # three more times, 5 s apart (HCLOOC_PIN_RETRIES overrides; 0 = fail at once), and says so on stderr.
+        import os
+        retries = int(os.environ.get("HCLOOC_PIN_RETRIES", "3"))
+        for attempt in range(retries + 1):
             try:
                 self.ptr = hclooc_host_alloc(self.nbytes)
                 break
             except HclError:
-                if attempt == 8 or self.nbytes < (64 << 20):
+                if attempt == retries or self.nbytes < (64 << 20):
                     raise
                 import gc
+                import sys
                 import time
+                print(f"HostMatrix: pinning {self.nbytes >> 20} MiB failed, retry {attempt + 1} of {retries} in 5 s", file=sys.stderr)
                 gc.collect()
-                time.sleep(12)
+                time.sleep(5)
         buf = (ctypes.c_double * max(1, rows * self.ld)).from_address(self.ptr)
         self.array = np.frombuffer(buf, dtype=np.float64)[: rows * self.ld].reshape(rows, self.ld)
         self.view = self.array[:, :cols]

@@ -256,6 +256,25 @@ __device__ __forceinline__ void epilogue_store(const double (&acc)[4][4][2][2], 
         const int row = m0 + f.row_of(u);
         if (row >= M) continue;
         double* crow = C + (long long)row * ldc;
+        // The common case -- C is read, 32-byte accesses are legal, no triangle mask, the lane's four segments of this row lie
+        // inside C: the four loads of the row are issued back to back BEFORE the first use, so a lane makes 4 round trips to C
+        // instead of 16 (what matters when C is host memory: direct mode spent a third of config 1 in these dependent reads).
+        if (!TB && read_c && vec4_ok && tri == 0 && n0 + f.wn * 64 + 63 < N) {
+            double c[4][4];
+            #pragma unroll
+            for (int bx = 0; bx < 4; ++bx) {
+                const double* p = crow + n0 + f.wn * 64 + bx * 16 + 4 * f.t;
+                asm volatile("ld.global.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(c[bx][0]), "=d"(c[bx][1]), "=d"(c[bx][2]), "=d"(c[bx][3]) : "l"(p));
+            }
+            #pragma unroll
+            for (int bx = 0; bx < 4; ++bx) {
+                double* p = crow + n0 + f.wn * 64 + bx * 16 + 4 * f.t;
+                const double x0 = axpby_tail(__dmul_rn(alpha, acc[u][bx][0][0]), beta, c[bx][0]), x1 = axpby_tail(__dmul_rn(alpha, acc[u][bx][1][0]), beta, c[bx][1]);
+                const double x2 = axpby_tail(__dmul_rn(alpha, acc[u][bx][0][1]), beta, c[bx][2]), x3 = axpby_tail(__dmul_rn(alpha, acc[u][bx][1][1]), beta, c[bx][3]);
+                asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(x0), "d"(x1), "d"(x2), "d"(x3) : "memory");
+            }
+            continue;
+        }
         #pragma unroll
         for (int bx = 0; bx < 4; ++bx) {
             if (!TB) {

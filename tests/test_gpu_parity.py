@@ -333,7 +333,7 @@ def test_k_panels_reread_the_host_block_after_its_download(H, M, N, K, budget):
     block panel p-1's R(c_ij) wrote through ANOTHER C buffer, so the upload must wait for that download (the schedule's
     host-block rule, tests/test_planner_schedule.py).  Integers: every panel's contribution and beta*C0 arrive exactly."""
     plan = H.hclooc_plan(M, N, K, 1, 0, budget)
-    assert plan.kpanels > 1 and plan.w == 1          # serpentine order: the last row block of panel p is the first of panel p+1
+    assert plan.kpanels > 1
     for rep in range(3):                                     # a race shows up only sometimes: a few rounds
         A, B, C = host_inputs(H, M, N, K, 340 + rep, "int")
         ref = C.view.copy()
