@@ -40,6 +40,7 @@ extern "C" {
 #define HCLOOC_ERR_NOMEM        4   /* device or host allocation failed                             */
 #define HCLOOC_ERR_ALIGN        5   /* device operand not 16-byte aligned / odd leading dimension   */
 #define HCLOOC_ERR_INTERNAL     6   /* planner/executor invariant violated (a bug)                  */
+#define HCLOOC_ERR_NOALLOC_LIMIT 7  /* hclDgemmNoAlloc: shape beyond what its static scratch array serves */
 
 /* ------------------------------------------------------------------ handles */
 typedef struct hclooc_ctx hclooc_ctx;   /* opaque: device, streams, events, workspace              */
@@ -466,6 +467,28 @@ int hclDgemmAsyncT(int transa, int transb, int64_t M, int64_t N, int64_t K, doub
 int hclDtrsmAsync(int side, int uplo, int trans, int diag, int64_t M, int64_t N, double alpha, const double* dA, int64_t lda,
                   double* dB, int64_t ldb, hclStream s, hclEvent* ev);
 int hclDpotrfAsync(int uplo, int64_t N, double* dA, int64_t lda, long long* d_info, hclStream s, hclEvent* ev);
+/* The in-core DGEMM for callers that CANNOT ALLOCATE (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): dC = alpha*dA*dB + beta*dC on device pointers, row-major, the persistent stream-K kernel of hclDgemmAsyncEx(...,
+ * variant -1) (the in-core kernel as a call of its own), asynchronous in stream s.  It calls no cudaMalloc,
+ * cudaFree or allocating library routine, creates no event and no stream: the kernel's scratch (two partial 128 x 128 tiles per
+ * persistent CTA and one counter per shared tile) is a static device array of HCL_NOALLOC_SCRATCH_BYTES (37.0 MiB) that every GPU
+ * which loads the library holds until the process exits.
+ *   Limits: M, N, K <= HCL_NOALLOC_MAX_DIM and ceil(M/128)*ceil(N/128) <= HCL_NOALLOC_MAX_TILES (what the kernel indexes with
+ *   32-bit integers and the array has slots for: at most 148 persistent CTAs, 296 shared tiles); beyond them the call returns
+ *   HCLOOC_ERR_NOALLOC_LIMIT and launches nothing.  No transposed operands, no event argument (record your own).
+ *   EVERY call on a device shares the one array: two calls that overlap on the GPU (different streams, or graphs replayed
+ *   concurrently) RACE on it and give wrong results -- keep the calls of a device in one stream or order them with events.  The
+ *   array keeps the last call's contents; the call clears the counters it needs (a memset node in the stream), partial slots are
+ *   written before they are read.
+ *   dA, dB 16-byte aligned, lda, ldb even, else HCLOOC_ERR_ALIGN.  beta == 0: dC is not read.  K == 0 or alpha == 0: dC = beta*dC.
+ *   Errors: -1..-3 negative dimension, -5 dA NULL, -6 lda < K, -7 dB NULL, -8 ldb < N, -10 dC NULL, -11 ldc < N,
+ *   HCLOOC_ERR_NOALLOC_LIMIT, HCLOOC_ERR_ALIGN, HCLOOC_ERR_CUDA.                                                              */
+#define HCL_NOALLOC_SCRATCH_BYTES 38798592
+#define HCL_NOALLOC_MAX_DIM       2147483647LL
+#define HCL_NOALLOC_MAX_TILES     1073741823LL
+int hclDgemmNoAlloc(int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda,
+                    const double* dB, int64_t ldb, double beta, double* dC, int64_t ldc, hclStream s);
+size_t hclDgemmNoAllocScratchBytes(void);                        /* HCL_NOALLOC_SCRATCH_BYTES, as compiled           */
 int hclWaitEvent(hclStream s, hclEvent e);                        /* :116  stream waits for event   */
 int hclStreamSynchronize(hclStream s);                            /* :115                           */
 int hclDeviceSynchronize(int device);                             /* :114                           */

@@ -20,7 +20,7 @@ EXPORTS = [
     "hclooc_ctx_set_trace", "hclooc_ctx_get_trace", "hclooc_ctx_set_direct", "hclooc_ctx_set_debug", "hclooc_calibrate_link",
     "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_t", "hclooc_dsyrk", "hclooc_dsyr2k", "hclooc_dtrsm", "hclooc_dtrsm_plan", "hclooc_dtrsm_side", "hclooc_dpotrf", "hclooc_dpotrf_plan", "hclooc_dtrmm", "hclooc_dsymm", "hclooc_dgemm_fig2", "hclooc_dgemm_nsteps", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
     "hclStreamDestroy", "hclEventDestroy", "hclMemcpy", "hclMemcpyAsync", "hclMemcpy2DAsync",
-    "hclDgemmAsync", "hclDgemmAsyncEx", "hclDgemmAsyncT", "hclDtrsmAsync", "hclDpotrfAsync", "hclWaitEvent", "hclStreamSynchronize", "hclDeviceSynchronize",
+    "hclDgemmAsync", "hclDgemmAsyncEx", "hclDgemmAsyncT", "hclDgemmNoAlloc", "hclDgemmNoAllocScratchBytes", "hclDtrsmAsync", "hclDpotrfAsync", "hclWaitEvent", "hclStreamSynchronize", "hclDeviceSynchronize",
     "hclooc_host_alloc", "hclooc_host_free", "hclooc_host_register", "hclooc_host_unregister",
     "hclooc_strerror", "hclooc_last_cuda_error", "hclooc_version", "hclooc_probe_fp64",
 ]
@@ -113,6 +113,9 @@ def lib():
         L.hclMemcpyAsync.argtypes = [vp, vp, sz, c_int, vp, POINTER(vp)]
         L.hclMemcpy2DAsync.argtypes = [vp, sz, vp, sz, sz, sz, c_int, vp, POINTER(vp)]
         L.hclDgemmAsync.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, vp, POINTER(vp)]
+        L.hclDgemmNoAlloc.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, vp]
+        L.hclDgemmNoAllocScratchBytes.argtypes = []
+        L.hclDgemmNoAllocScratchBytes.restype = sz
         L.hclDgemmAsyncEx.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, vp, POINTER(vp), c_int]
         L.hclDgemmAsyncT.argtypes = [c_int, c_int, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, vp, POINTER(vp), c_int]
         L.hclDtrsmAsync.argtypes = [c_int, c_int, c_int, c_int, i64, i64, dbl, vp, i64, vp, i64, vp, POINTER(vp)]
@@ -487,6 +490,15 @@ def hclDgemmAsync(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, stream=None, 
     _check(lib().hclDgemmAsync(M, N, K, alpha, _ptr(dA), lda, _ptr(dB), ldb, beta, _ptr(dC), ldc, _ptr(stream),
                                byref(ev) if ev is not None else None), "hclDgemmAsync")
     return ev.value if ev is not None else None
+
+
+def hclDgemmNoAlloc(M, N, K, alpha, dA, lda, dB, ldb, beta, dC, ldc, stream=None):
+    """The in-core DGEMM that allocates nothing (include/hclooc.h): scratch in a static device array shared by every call."""
+    _check(lib().hclDgemmNoAlloc(M, N, K, alpha, _ptr(dA), lda, _ptr(dB), ldb, beta, _ptr(dC), ldc, _ptr(stream)), "hclDgemmNoAlloc")
+
+
+def hclDgemmNoAllocScratchBytes():
+    return int(lib().hclDgemmNoAllocScratchBytes())
 
 
 def hclDtrsmAsync(side, uplo, trans, diag, M, N, alpha, dA, lda, dB, ldb, stream=None, want_event=False, event=None):

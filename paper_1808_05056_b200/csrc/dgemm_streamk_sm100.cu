@@ -353,3 +353,102 @@ int launch_dgemm_streamk(int64_t M, int64_t N, int64_t K, double alpha, const CU
 }
 
 }  // namespace hclooc
+
+// ---------------------------------------------------------------------------------------------
+// hclDgemmNoAlloc: the persistent stream-K kernel for callers that cannot allocate (CUDA graph capture, serving loops, harnesses
+// that forbid cudaMalloc).  The kernel is the one above, unchanged; the partial-tile slots and tile counters it needs sit in a
+// file-scope device array instead of the cudaMalloc'ed pool of acquire_scratch.  Every GPU that loads the library holds the array
+// (HCL_NOALLOC_SCRATCH_BYTES, 37.0 MiB) until the process exits.  In host code `g_noalloc_scratch` is only a stand-in for the
+// symbol: the device address comes from cudaGetSymbolAddress, once per device, with that device current.
+namespace hclooc {
+namespace {
+
+constexpr size_t NA_PARTIAL_BYTES = (size_t)2 * SK_MAX_CTAS * SK_SLOT_BYTES;                    // 2 slots per persistent CTA
+constexpr size_t NA_COUNTER_BYTES = SK_MAX_TAIL_TILES * sizeof(unsigned);
+constexpr size_t NA_SCRATCH_BYTES = (NA_PARTIAL_BYTES + NA_COUNTER_BYTES + 255) / 256 * 256;
+static_assert(NA_SCRATCH_BYTES == HCL_NOALLOC_SCRATCH_BYTES, "include/hclooc.h states the size of the static scratch");
+static_assert(NA_PARTIAL_BYTES % 256 == 0, "the counters start on a 256-byte boundary");
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[NA_SCRATCH_BYTES];
+
+constexpr int NA_MAX_DEVICES = 64;
+struct NoAllocDevice {
+    void* scratch = nullptr;        // device address of g_noalloc_scratch on this device
+    int num_sms = 0;
+    bool ready = false;
+};
+NoAllocDevice g_na_dev[NA_MAX_DEVICES];
+std::mutex g_na_mu;
+
+// Set-up of the CURRENT device (once per device): the array's device address, the SM count, the kernel's shared-memory limit.
+int noalloc_setup(NoAllocDevice** out) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e);
+    if (dev < 0 || dev >= NA_MAX_DEVICES) return HCLOOC_ERR_INTERNAL;
+    std::lock_guard<std::mutex> lk(g_na_mu);
+    NoAllocDevice& d = g_na_dev[dev];
+    if (!d.ready) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+        if (e != cudaSuccess) return cuda_fail(e);
+        if (!p || ((uintptr_t)p & 255u)) return HCLOOC_ERR_INTERNAL;
+        int n = 0;
+        e = cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(hclooc_dgemm_streamk_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+        if (e != cudaSuccess) return cuda_fail(e);
+        d.scratch = p; d.num_sms = n; d.ready = true;
+    }
+    *out = &d;
+    return HCLOOC_OK;
+}
+
+}  // namespace
+}  // namespace hclooc
+
+extern "C" size_t hclDgemmNoAllocScratchBytes(void) { return hclooc::NA_SCRATCH_BYTES; }
+
+extern "C" int hclDgemmNoAlloc(int64_t M, int64_t N, int64_t K, double alpha, const double* dA, int64_t lda, const double* dB,
+                               int64_t ldb, double beta, double* dC, int64_t ldc, hclStream s) {
+    using namespace hclooc;
+    if (M < 0) return -1;
+    if (N < 0) return -2;
+    if (K < 0) return -3;
+    // the maximum: what the kernel indexes with 32-bit integers and what the static array has slots and counters for
+    if (M > HCL_NOALLOC_MAX_DIM || N > HCL_NOALLOC_MAX_DIM || K > HCL_NOALLOC_MAX_DIM) return HCLOOC_ERR_NOALLOC_LIMIT;
+    if (((M + BM - 1) / BM) * ((N + BN - 1) / BN) > HCL_NOALLOC_MAX_TILES) return HCLOOC_ERR_NOALLOC_LIMIT;
+    if (M == 0 || N == 0) return HCLOOC_OK;
+    const bool noab = (alpha == 0.0 || K == 0);
+    if (!noab) {
+        if (!dA) return -5;
+        if (lda < K) return -6;
+        if (!dB) return -7;
+        if (ldb < N) return -8;
+        if (((uintptr_t)dA & 15u) || ((uintptr_t)dB & 15u) || (lda & 1) || (ldb & 1)) return HCLOOC_ERR_ALIGN;
+    }
+    if (!dC) return -10;
+    if (ldc < N) return -11;
+    cudaStream_t stream = (cudaStream_t)s;
+    if (noab)                                        // dC = beta * dC: one CTA per tile, no scratch, nothing allocated either
+        return launch_dgemm_tiles(M, N, 0, 0.0, nullptr, 2, nullptr, 2, beta, dC, ldc, stream, 1);
+    NoAllocDevice* d = nullptr;
+    int rc = noalloc_setup(&d);
+    if (rc) return rc;
+    SkParams P;
+    if (!streamk_layout(M, N, K, d->num_sms, &P.G, &P.dp_waves, &P.tail_tiles)) return HCLOOC_ERR_NOALLOC_LIMIT;
+    if (P.G > SK_MAX_CTAS || P.tail_tiles > SK_MAX_TAIL_TILES) return HCLOOC_ERR_NOALLOC_LIMIT;     // more than the array holds
+    P.tiles_m = (int)((M + BM - 1) / BM); P.tiles_n = (int)((N + BN - 1) / BN); P.nk = (int)((K + BK - 1) / BK);
+    P.tail_iters = (long long)P.tail_tiles * P.nk;
+    CUtensorMap tmA, tmB;
+    if ((rc = make_tensor_map(&tmA, dA, M, K, lda, BM))) return rc;
+    if ((rc = make_tensor_map(&tmB, dB, K, N, ldb, BK))) return rc;
+    double* partials = (double*)d->scratch;
+    unsigned* counters = (unsigned*)((uint8_t*)d->scratch + NA_PARTIAL_BYTES);
+    // the array keeps what the last call left: the partial slots are written before they are read, the counters must start at zero
+    // (a launch resets the ones it used, but a launch that was aborted or is still running on another stream may not have)
+    HCL_CUDA(cudaMemsetAsync(counters, 0, NA_COUNTER_BYTES, stream));
+    hclooc_dgemm_streamk_kernel<false, false><<<P.G, NUM_THREADS, SMEM_BYTES, stream>>>(tmA, tmB, dC, (long long)ldc, (int)M, (int)N,
+                                                                                        alpha, beta, P, partials, counters);
+    HCL_CUDA(cudaGetLastError());
+    return HCLOOC_OK;
+}

@@ -294,6 +294,7 @@ const char* hclooc_strerror(int status) {
         case HCLOOC_ERR_NOMEM: return "out of device or host memory";
         case HCLOOC_ERR_ALIGN: return "device operand must be 16-byte aligned with an even leading dimension";
         case HCLOOC_ERR_INTERNAL: return "internal invariant violated";
+        case HCLOOC_ERR_NOALLOC_LIMIT: return "hclDgemmNoAlloc: shape beyond the maximum its static scratch array serves (M, N, K <= 2^31 - 1, at most 2^30 - 1 tiles of 128 x 128)";
         default: return "unknown status";
     }
 }
