@@ -362,7 +362,7 @@ class Bench:
 
     @staticmethod
     def plan_summary(plan):
-        keys = ("mb", "nb", "kb", "h", "w", "kpanels", "n_steps", "n_sets", "n_abuf", "n_bbuf", "ksplit", "direct", "workspace_bytes")
+        keys = ("mb", "nb", "kb", "h", "w", "kpanels", "n_steps", "n_sets", "n_abuf", "n_bbuf", "ksplit", "direct", "resident", "workspace_bytes")
         return {k: getattr(plan, k) for k in keys}
 
     def per_config(self, names):
@@ -797,6 +797,8 @@ def run_transition_sweep(args):
     if live:
         LINK.update(live)
     budget = args.budget if args.budget else 12_200_000_000
+    if not args.no_calibrate:          # the choice between the resident schedule and the slice pipeline rests on the link rates
+        print(json.dumps({"cost_model_link": dict(zip(("h2d_GBps", "d2h_GBps", "duplex_GBps"), H.hclooc_calibrate_link(None)))}), flush=True)
     sizes = sorted(int(x) for x in args.sizes.split(",")) if args.sizes else TRANSITION_SIZES
     nmax = sizes[-1]
     bufs = [H.HostMatrix(nmax, nmax) for _ in range(3)]        # one pinned allocation per matrix, reused as a dense N x N matrix
@@ -818,7 +820,28 @@ def run_transition_sweep(args):
                 t_roof, t_flop, t_link = link_roofline_s(2.0 * n ** 3, st.bytes_h2d, st.bytes_d2h)
                 rec[label] = {"t_s": t, "tflops": 2.0 * n ** 3 / t / 1e12, "h": st.plan.h, "w": st.plan.w, "kpanels": st.plan.kpanels, "steps": st.plan.n_steps,
                               "h2d_GB": st.bytes_h2d / 1e9, "d2h_GB": st.bytes_d2h / 1e9, "frac_of_roofline": t_roof / t,
-                              "bound": "fp64" if t_flop >= t_link else "link"}
+                              "bound": "fp64" if t_flop >= t_link else "link", "t_model_s": st.plan.t_model_s}
+                if label == "tuned":
+                    st_tuned = st
+            rec["tuned"]["resident"] = st_tuned.plan.resident
+            if st_tuned.plan.resident:
+                # the resident schedule was picked (the matrices fit the budget): the slice pipeline on the same call, for comparison
+                prev = os.environ.get("HCLOOC_RESIDENT")
+                os.environ["HCLOOC_RESIDENT"] = "0"
+                try:
+                    ts = []
+                    for _ in range(max(2, args.steps or 3)):
+                        st = H.hclooc_dgemm_ex(ctx, n, n, n, 1.0, A, n, B, n, args.beta, C, n, budget)
+                        ts.append(st.t_total_s)
+                finally:
+                    if prev is None:
+                        del os.environ["HCLOOC_RESIDENT"]
+                    else:
+                        os.environ["HCLOOC_RESIDENT"] = prev
+                t = float(np.mean(ts[1:]))
+                t_roof, t_flop, t_link = link_roofline_s(2.0 * n ** 3, st.bytes_h2d, st.bytes_d2h)
+                rec["slices"] = {"t_s": t, "tflops": 2.0 * n ** 3 / t / 1e12, "h": st.plan.h, "w": st.plan.w, "kpanels": st.plan.kpanels,
+                                 "frac_of_roofline": t_roof / t, "t_model_s": st.plan.t_model_s}
             rec["fig2_over_tuned"] = rec["fig2"]["tflops"] / rec["tuned"]["tflops"]
             rows.append(rec)
             print(json.dumps(rec), flush=True)
@@ -826,11 +849,13 @@ def run_transition_sweep(args):
         H.hclooc_ctx_destroy(ctx)
         for X in bufs:
             X.free()
-    print("| N | fits budget | tuned TFLOP/s (h x w x kpanels) | tuned / roofline | Figure-2 TFLOP/s (h x w) | Figure-2 / roofline | Figure-2 / tuned |")
-    print("|---|---|---|---|---|---|---|")
+    print("| N | fits budget | tuned TFLOP/s (h x w x kpanels) | schedule | tuned / roofline | slice pipeline on the same call / roofline | Figure-2 TFLOP/s (h x w) | Figure-2 / roofline | Figure-2 / tuned |")
+    print("|---|---|---|---|---|---|---|---|---|")
     for r in rows:
-        print(f"| {r['N']} | {'yes' if r['fits_budget'] else 'no'} | {r['tuned']['tflops']:.2f} ({r['tuned']['h']} x {r['tuned']['w']} x {r['tuned']['kpanels']}) | "
-              f"{r['tuned']['frac_of_roofline']:.3f} ({r['tuned']['bound']}) | {r['fig2']['tflops']:.2f} ({r['fig2']['h']} x {r['fig2']['w']}) | "
+        sl = f"{r['slices']['frac_of_roofline']:.3f} ({r['slices']['h']} x {r['slices']['w']} x {r['slices']['kpanels']})" if "slices" in r else "-"
+        sched = f"resident, switch at panel {r['tuned']['resident'] - 1}" if r["tuned"]["resident"] else "slices"
+        print(f"| {r['N']} | {'yes' if r['fits_budget'] else 'no'} | {r['tuned']['tflops']:.2f} ({r['tuned']['h']} x {r['tuned']['w']} x {r['tuned']['kpanels']}) | {sched} | "
+              f"{r['tuned']['frac_of_roofline']:.3f} ({r['tuned']['bound']}) | {sl} | {r['fig2']['tflops']:.2f} ({r['fig2']['h']} x {r['fig2']['w']}) | "
               f"{r['fig2']['frac_of_roofline']:.3f} | {r['fig2_over_tuned']:.3f} |")
 
 

@@ -99,7 +99,12 @@ typedef struct hclooc_plan_t {
     int32_t  tri;                 /* hclooc_dsyrk: 1 / 2 = only the lower / upper triangle of C is referenced; the schedule has no
                                      step for a block that lies wholly in the other triangle, and bytes_* / n_copies_* are
                                      those of the schedule (set by the executor; the planner leaves tri = 0)           */
-    int32_t  reserved2;
+    int32_t  resident;            /* != 0: the RESIDENT schedule ran (host matrices that fit the budget; resident.cu): A, B and C have
+                                     device copies (lda_dev / ldb_dev / ldc_dev; bytes_a_buf / bytes_b_buf are the whole matrices and
+                                     workspace_bytes also counts the M x ldc_dev copy of C), A and B go up in `kpanels` K panels of kb
+                                     with whole-C kernels behind them, and from panel resident - 1 on C is finished in h row blocks
+                                     of mb (w = 1): one launch over the remaining panels, dC += beta * C0 from a ring of n_sets
+                                     staging buffers of bytes_c_buf, download.  n_steps = (resident - 1) + h DGEMM launches        */
     int32_t  trans;               /* hclooc_dgemm_t: bit 0 = A is stored K x M, bit 1 = B is stored N x K.  The device
                                      slices keep the stored layout: an A slice is then kb x mb (lda_dev >= mb), a B
                                      slice nb x kb (ldb_dev >= kb), and the tile kernel reads them transposed       */

@@ -38,7 +38,7 @@ class Plan(ctypes.Structure):
                 ("n_copies_h2d", c_uint64), ("n_copies_d2h", c_uint64),
                 ("flops", c_double), ("t_flop_s", c_double), ("t_link_s", c_double), ("t_model_s", c_double),
                 ("n_scratch", c_int32), ("c_on_device", c_int32), ("bytes_scratch", c_uint64),
-                ("direct", c_int32), ("direct_cm", c_int32), ("direct_cn", c_int32), ("tri", c_int32), ("reserved2", c_int32), ("trans", c_int32)]
+                ("direct", c_int32), ("direct_cm", c_int32), ("direct_cn", c_int32), ("tri", c_int32), ("resident", c_int32), ("trans", c_int32)]
 
     def asdict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

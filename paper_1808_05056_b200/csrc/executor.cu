@@ -397,10 +397,11 @@ int dgemm_core_locked(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_
     if (!ctx) return HCLOOC_ERR_INTERNAL + 1000;                // validation-only pass of dgemm_core: the arguments are fine
     int rc;
     HCL_CUDA(cudaSetDevice(ctx->device));
-    bool on_device = true, c_dev = true, ab_dev = true;
+    bool on_device = true, c_dev = true, a_dev = true, b_dev = true;
     const void *A_alias = nullptr, *B_alias = nullptr, *C_alias = nullptr;
     if ((rc = check_resident(C, &c_dev, &C_alias))) return rc;
-    if (!scale_only && ((rc = check_resident(A, &ab_dev, &A_alias)) || (rc = check_resident(B, &ab_dev, &B_alias)))) return rc;
+    if (!scale_only && ((rc = check_resident(A, &a_dev, &A_alias)) || (rc = check_resident(B, &b_dev, &B_alias)))) return rc;
+    const bool ab_dev = a_dev && b_dev;
     on_device = c_dev && ab_dev;
 
     // ---------------------------------------------------------------- S1 plan
@@ -456,6 +457,14 @@ int dgemm_core_locked(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_
         }
     }
     if (extra && extra->in_place && P.kpanels > 1) return HCLOOC_ERR_BUDGET;
+    // host matrices that fit the budget: the resident schedule (resident.cu) where its model beats the slice plan's
+    if (!in_core && !P.direct && !scale_only && !c_dev && !a_dev && !b_dev && !transa && !transb && tri == 0 && !extra && !reserved) {
+        ResidentShape RS;
+        if (resident_applies(M, N, K, beta != 0.0, budget, P.t_model_s, &RS)) {
+            ctx->graph_key.clear(); ctx->graph_valid = false;
+            return dgemm_resident(ctx, RS, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, stats, t_begin);
+        }
+    }
     if (in_core || P.direct) {
         const auto t0 = std::chrono::steady_clock::now();
         if (P.direct) { A = (const double*)A_alias; B = (const double*)B_alias; C = (double*)C_alias; }

@@ -1,5 +1,6 @@
 // executor.h -- the context and the entry points of executor.cu that the other out-of-core routines (factor.cu) build on.
 #pragma once
+#include <chrono>
 #include <mutex>
 #include <utility>
 #include <vector>
@@ -94,6 +95,23 @@ struct DgemmExtra {
 int dgemm_core_locked(hclooc_ctx* ctx, int transa, int transb, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
                       int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc,
                       size_t device_budget_bytes, hclooc_stats* stats, int tri = 0, const DgemmExtra* extra = nullptr);
+
+// The resident schedule of hclooc_dgemm (resident.cu): A, B and C fit the budget, K is streamed in panels, C finished row block
+// by row block.  resident_applies says whether the call takes it (shape, memory, cost model against the slice plan's t_model_s;
+// HCLOOC_RESIDENT=0 / 1 forces the answer) and fills the shape; dgemm_resident runs it (ctx->mu held by the caller).
+constexpr int RESIDENT_MAX_PANELS = 128;
+struct ResidentShape {
+    int64_t mb, h, kb, npanels, p_switch;          // row blocks of mb rows, K panels of at most kb, phase 2 starts with panel p_switch
+    int64_t pk0[RESIDENT_MAX_PANELS], pkk[RESIDENT_MAX_PANELS];   // panel p = columns [pk0, pk0 + pkk) of A, the same rows of B
+    int64_t ldA, ldB, ldC;                         // leading dimensions of the device copies
+    size_t bytesA, bytesB, bytesC, bytes_stage, bytes_scratch, total;
+    int ring;                                      // staging buffers for the initial C (0 when beta == 0)
+    double t_flop_s, t_link_s, t_model_s;
+};
+bool resident_applies(int64_t M, int64_t N, int64_t K, bool beta_nonzero, size_t budget, double t_slice_model_s, ResidentShape* out);
+int dgemm_resident(hclooc_ctx* ctx, const ResidentShape& S, int64_t M, int64_t N, int64_t K, double alpha, const double* A, int64_t lda,
+                   const double* B, int64_t ldb, double beta, double* C, int64_t ldc, hclooc_stats* stats,
+                   std::chrono::steady_clock::time_point t_begin);
 
 // hclooc_dtrsm (side = Left) with two resident block rows and a look-ahead of one (factor.cu); ctx->mu held by the caller
 int dtrsm_left_lookahead(hclooc_ctx* ctx, int uplo, int trans, int diag, int64_t M, int64_t N, double alpha, const double* A, int64_t lda,
