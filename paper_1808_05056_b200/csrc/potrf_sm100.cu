@@ -60,10 +60,23 @@ potrf_block_kernel(double* __restrict__ A, long long lda, int n, int lower, long
     if (tid == 0) bad = -1;
     // stage: consecutive threads walk the direction that is contiguous in global memory (rows of A); rows and columns beyond n are
     // padded with the identity so that the last step of a ragged block factors a full 32 x 32 block
-    for (int e = tid; e < PB * PB; e += PT) {
-        const int r = e / PB, c = e % PB;                // global element A[r][c] = logical (r, c) of a lower, (c, r) of an upper block
-        const int i = lower ? r : c, k = lower ? c : r;  // logical element (i, k), wanted for k <= i
-        if (k <= i) S[i * PS + k] = (i < n) ? A[(long long)r * lda + c] : (i == k ? 1.0 : 0.0);
+    // (loads issued in batches of 16 per thread before their stores: one round trip to L2 / HBM per batch instead of one per element)
+    for (int base = 0; base < PB * PB; base += PT * 16) {
+        double v[16];
+#pragma unroll
+        for (int u = 0; u < 16; ++u) {
+            const int e = base + u * PT + tid;
+            const int r = e / PB, c = e % PB;                // global element A[r][c] = logical (r, c) of a lower, (c, r) of an upper block
+            const int i = lower ? r : c, k = lower ? c : r;  // logical element (i, k), wanted for k <= i
+            v[u] = (k <= i && i < n) ? A[(long long)r * lda + c] : (i == k ? 1.0 : 0.0);
+        }
+#pragma unroll
+        for (int u = 0; u < 16; ++u) {
+            const int e = base + u * PT + tid;
+            const int r = e / PB, c = e % PB;
+            const int i = lower ? r : c, k = lower ? c : r;
+            if (k <= i) S[i * PS + k] = v[u];
+        }
     }
     __syncthreads();
     for (int c0 = 0; c0 < n; c0 += PW) {

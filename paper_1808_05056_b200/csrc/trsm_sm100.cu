@@ -6,6 +6,7 @@
 // an upper triangle the rows and columns are reversed, which turns it into a lower one -- so that the coefficients one thread
 // needs next (column p of the triangle, 32 consecutive rows) are contiguous: they are read as broadcast LDS.128.  Rounding: the
 // division by t_ii is a multiplication by the rounded reciprocal (two roundings instead of one; exact for t_ii = +-2^k).
+#include <cstdlib>
 #include "internal.h"
 
 namespace hclooc {
@@ -37,21 +38,10 @@ __device__ __forceinline__ void solve64(double (&x)[HB], const double* __restric
     }
 }
 
-// One thread owns one right-hand side: a column of the panel (side = Left: consecutive threads read consecutive addresses) or a
-// row of it (side = Right: a thread's values are contiguous; VEC = 4 reads and writes them as 32-byte vectors -- one full sector
-// per thread and instruction -- when the block is a whole 128 and the rows are 32-byte aligned).  Element q of the logical
-// (lower) system sits at P0[q * step].  The 128 rows are two halves of 64: the first half is loaded into registers and solved
-// there (solve64), stored, and -- still in registers -- subtracted from the second half 16 rows at a time (load, 16 x 64 FMAs against
-// broadcast LDS.128 coefficients, store); then the second half is loaded and solved the same way.  Shared memory holds nothing but
-// the triangle, so a CTA carries 256 solving threads; a right-hand side makes two round trips through L1/L2 instead of living
-// in a per-thread staging buffer.  `scale` multiplies every value at its first load.
-template <int VEC, bool FULL>
-__global__ void __launch_bounds__(TTHREADS, 1)
-trsm_block_kernel(const double* __restrict__ T, long long ldt, int ib, double* __restrict__ X, long long sq, long long si, int nitems,
-                  int lower, int trans, int unit, double scale) {
-    extern __shared__ __align__(16) double smem[];
-    double* sTt = smem;                       // sTt[p * TS + q] = T'[q][p], T' = op(T) in logical (lower) order, 0 above, 1 on
-    const int tid = threadIdx.x;              //                  a unit / padded diagonal; the diagonal is kept as its reciprocal
+// Stage the triangle with all threads of the CTA: sTt[p * TS + q] = T'[q][p] for q >= p, T' = op(T) in logical (lower) order, 1 on a
+// unit / padded diagonal, the diagonal kept as its reciprocal.  Ends with a barrier.
+__device__ __forceinline__ void stage_triangle(double* __restrict__ sTt, const double* __restrict__ T, long long ldt, int ib, int lower, int trans,
+                                               int unit, int tid) {
     // ---- stage the triangle with all threads: logical index q <-> actual index lower ? q : ib-1-q.  Consecutive
     // threads walk the direction that is contiguous in global memory (rows of T when it is stored untransposed, columns
     // when transposed); only the ib x ib corner is read, the rest of the 128 x 128 image is padding (0, diagonal 1).
@@ -82,6 +72,24 @@ trsm_block_kernel(const double* __restrict__ T, long long ldt, int ib, double* _
     // (128 divisions per CTA, after the staging: a select between v and 1/v per staged element made every thread divide 64 times)
     if (tid < ib && !unit) sTt[tid * TS + tid] = 1.0 / sTt[tid * TS + tid];
     __syncthreads();
+}
+
+// One thread owns one right-hand side: a column of the panel (side = Left: consecutive threads read consecutive addresses) or a
+// row of it (side = Right: a thread's values are contiguous; VEC = 4 reads and writes them as 32-byte vectors -- one full sector
+// per thread and instruction -- when the block is a whole 128 and the rows are 32-byte aligned).  Element q of the logical
+// (lower) system sits at P0[q * step].  The 128 rows are two halves of 64: the first half is loaded into registers and solved
+// there (solve64), stored, and -- still in registers -- subtracted from the second half 16 rows at a time (load, 16 x 64 FMAs against
+// broadcast LDS.128 coefficients, store); then the second half is loaded and solved the same way.  Shared memory holds nothing but
+// the triangle, so a CTA carries 256 solving threads; a right-hand side makes two round trips through L1/L2 instead of living
+// in a per-thread staging buffer.  `scale` multiplies every value at its first load.
+template <int VEC, bool FULL>
+__global__ void __launch_bounds__(TTHREADS, 1)
+trsm_block_kernel(const double* __restrict__ T, long long ldt, int ib, double* __restrict__ X, long long sq, long long si, int nitems,
+                  int lower, int trans, int unit, double scale) {
+    extern __shared__ __align__(16) double smem[];
+    double* sTt = smem;                       // sTt[p * TS + q] = T'[q][p], T' = op(T) in logical (lower) order, 0 above, 1 on
+    const int tid = threadIdx.x;              //                  a unit / padded diagonal; the diagonal is kept as its reciprocal
+    stage_triangle(sTt, T, ldt, ib, lower, trans, unit, tid);
     const long long item = (long long)blockIdx.x * TTHREADS + tid;
     if (item >= nitems) return;               // no barrier follows
     double* P0 = X + item * si + (lower ? 0 : (long long)(ib - 1) * sq);
@@ -169,6 +177,88 @@ trsm_block_kernel(const double* __restrict__ T, long long ldt, int ib, double* _
     }
 }
 
+// The same substitution for SMALL panels (fewer right-hand sides than 64 per SM): a right-hand side is shared by SPLIT = 4
+// neighbouring lanes, so a CTA of 256 threads solves 64 of them and the 128-step chain costs a quarter of the FMAs per lane -- the
+// launch is latency bound (a panel of the Cholesky / DTRSM recursion: 96 us with one thread per right-hand side, whatever the
+// panel's size).  Lane j of a group owns the logical elements 16 i + 4 j + c (i < 8, c < 4): 32 values in registers, read and
+// written as 32-byte vectors when the panel allows it.  Step t: the owner of x_t scales it by 1 / t_tt, a width-4 shuffle hands
+// it to the group, every lane updates its own elements below t.  The operations on an element and their order are those of
+// trsm_block_kernel, so the two kernels give the same bits.
+constexpr int SPLIT = 4;
+constexpr int SITEMS = TTHREADS / SPLIT;
+
+template <int VEC, bool FULL>
+__global__ void __launch_bounds__(TTHREADS, 1)
+trsm_block_split_kernel(const double* __restrict__ T, long long ldt, int ib, double* __restrict__ X, long long sq, long long si, int nitems,
+                        int lower, int trans, int unit, double scale) {
+    extern __shared__ __align__(16) double smem[];
+    double* sTt = smem;
+    const int tid = threadIdx.x;
+    stage_triangle(sTt, T, ldt, ib, lower, trans, unit, tid);
+    const int j = tid & (SPLIT - 1);
+    long long item = (long long)blockIdx.x * SITEMS + (tid >> 2);
+    const bool live = item < nitems;          // a group past the end solves the last right-hand side again and stores nothing
+    if (!live) item = nitems - 1;             // (the shuffles below name every lane of the warp)
+    double* P0 = X + item * si + (lower ? 0 : (long long)(ib - 1) * sq);
+    const long long step = lower ? sq : -sq;
+    double x[32];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const int q = 16 * i + 4 * j;
+        if (VEC == 4) {
+            const double* p = lower ? P0 + q : P0 - q - 3;
+            double a, b, c, d;
+            asm volatile("ld.global.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p) : "memory");
+            x[4 * i] = scale * (lower ? a : d); x[4 * i + 1] = scale * (lower ? b : c); x[4 * i + 2] = scale * (lower ? c : b); x[4 * i + 3] = scale * (lower ? d : a);
+        } else {
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const double v = (FULL || q + c < ib) ? P0[(long long)(q + c) * step] : 0.0;
+                x[4 * i + c] = scale != 1.0 ? scale * v : v;
+            }
+        }
+    }
+#pragma unroll
+    for (int t = 0; t < TB; ++t) {
+        const int li = (t / 16) * 4 + (t % 4), owner = (t / 4) % 4;
+        const double* tcol = sTt + t * TS;
+        const double cand = unit ? x[li] : x[li] * tcol[t];
+        const double xv = __shfl_sync(0xffffffffu, cand, owner, SPLIT);
+        if (j == owner) x[li] = xv;
+#pragma unroll
+        for (int i = t / 16; i < 8; ++i) {
+            const double2 t01 = *reinterpret_cast<const double2*>(tcol + 16 * i + 4 * j);
+            const double2 t23 = *reinterpret_cast<const double2*>(tcol + 16 * i + 4 * j + 2);
+            if (i > t / 16) {
+                x[4 * i] = fma(-t01.x, xv, x[4 * i]);
+                x[4 * i + 1] = fma(-t01.y, xv, x[4 * i + 1]);
+                x[4 * i + 2] = fma(-t23.x, xv, x[4 * i + 2]);
+                x[4 * i + 3] = fma(-t23.y, xv, x[4 * i + 3]);
+            } else {                              // the block that holds t: only the elements below it (what lies above is not staged)
+                const int e = 4 * j - (t % 16);   // element c is below t iff e + c > 0
+                if (e > 0) x[4 * i] = fma(-t01.x, xv, x[4 * i]);
+                if (e + 1 > 0) x[4 * i + 1] = fma(-t01.y, xv, x[4 * i + 1]);
+                if (e + 2 > 0) x[4 * i + 2] = fma(-t23.x, xv, x[4 * i + 2]);
+                if (e + 3 > 0) x[4 * i + 3] = fma(-t23.y, xv, x[4 * i + 3]);
+            }
+        }
+    }
+    if (!live) return;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const int q = 16 * i + 4 * j;
+        if (VEC == 4) {
+            double* p = lower ? P0 + q : P0 - q - 3;
+            if (lower) asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(x[4 * i]), "d"(x[4 * i + 1]), "d"(x[4 * i + 2]), "d"(x[4 * i + 3]) : "memory");
+            else asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(x[4 * i + 3]), "d"(x[4 * i + 2]), "d"(x[4 * i + 1]), "d"(x[4 * i]) : "memory");
+        } else {
+#pragma unroll
+            for (int c = 0; c < 4; ++c)
+                if (FULL || q + c < ib) P0[(long long)(q + c) * step] = x[4 * i + c];
+        }
+    }
+}
+
 }  // namespace
 
 // X (ib x ncols, row-major, ldx) <- op(T)^-1 * (scale * X) for the ib x ib diagonal block T (row-major as stored, ldt);
@@ -183,6 +273,37 @@ int launch_trsm_block(const double* dT, int64_t ldt, int ib, double* dX, int64_t
     static cudaError_t attr = cudaFuncSetAttribute(trsm_block_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TRSM_SMEM);
     if (attr != cudaSuccess) return cuda_fail(attr);
     const unsigned grid = (unsigned)((ncols + TTHREADS - 1) / TTHREADS);
+    // small panels: four lanes per right-hand side (same bits, a quarter of the chain per lane) while that still fits one wave
+    const char* split_e = getenv("HCLOOC_TRSM_SPLIT");       // 0: never, 1: always (tests: the two kernels must give the same bits)
+    const int split_env = split_e ? atoi(split_e) : -1;
+    static int split_items = 0;
+    if (split_items == 0) {
+        int dev = 0, sms = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) sms = 148;
+        split_items = SITEMS * sms;
+    }
+    if (split_env != 0 && (split_env == 1 || ncols <= split_items)) {
+        static cudaError_t sa = [] {
+            cudaError_t e = cudaFuncSetAttribute(trsm_block_split_kernel<4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TRSM_SMEM);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(trsm_block_split_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TRSM_SMEM);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(trsm_block_split_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TRSM_SMEM);
+            return e;
+        }();
+        if (sa != cudaSuccess) return cuda_fail(sa);
+        const unsigned sgrid = (unsigned)((ncols + SITEMS - 1) / SITEMS);
+        if (right) {
+            const bool vec = ib == TB && (ldx % 4 == 0) && (((uintptr_t)dX & 31u) == 0);
+            if (vec) trsm_block_split_kernel<4, true><<<sgrid, TTHREADS, TRSM_SMEM, stream>>>(dT, (long long)ldt, ib, dX, 1LL, (long long)ldx, (int)ncols, !lower, !trans, unit, scale);
+            else if (ib == TB) trsm_block_split_kernel<1, true><<<sgrid, TTHREADS, TRSM_SMEM, stream>>>(dT, (long long)ldt, ib, dX, 1LL, (long long)ldx, (int)ncols, !lower, !trans, unit, scale);
+            else trsm_block_split_kernel<1, false><<<sgrid, TTHREADS, TRSM_SMEM, stream>>>(dT, (long long)ldt, ib, dX, 1LL, (long long)ldx, (int)ncols, !lower, !trans, unit, scale);
+        } else if (ib == TB) {
+            trsm_block_split_kernel<1, true><<<sgrid, TTHREADS, TRSM_SMEM, stream>>>(dT, (long long)ldt, ib, dX, (long long)ldx, 1LL, (int)ncols, lower, trans, unit, scale);
+        } else {
+            trsm_block_split_kernel<1, false><<<sgrid, TTHREADS, TRSM_SMEM, stream>>>(dT, (long long)ldt, ib, dX, (long long)ldx, 1LL, (int)ncols, lower, trans, unit, scale);
+        }
+        HCL_CUDA(cudaGetLastError());
+        return HCLOOC_OK;
+    }
     static cudaError_t attr4 = cudaFuncSetAttribute(trsm_block_kernel<4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TRSM_SMEM);
     if (attr4 != cudaSuccess) return cuda_fail(attr4);
     static cudaError_t attr1 = cudaFuncSetAttribute(trsm_block_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TRSM_SMEM);
