@@ -437,7 +437,10 @@ class Bench:
                 "achieved": 2.0 * mb * nb * K / (ms_step * 1e-3) / 1e12, "peak": step_peak,
                 "note": "one step's launch timed ALONE; peak = 37.2 TFLOP/s x min(CTAs, 148)/148 (in the pipeline other steps' kernels run beside it and fill its wave tail)"}
         solo["frac"] = solo["achieved"] / step_peak
-        full = {"kernel": "hclooc_dgemm_streamk_kernel" if tiles_full >= 148 else "hclooc_dgemm_tile_kernel", "launch": f"{rows}x{nb}x{K}",
+        # the library's own rule (launch_dgemm_tiles): persistent stream-K unless the tiles fill their waves of 148 to 98.8 % or better
+        waves_full = -(-tiles_full // 148)
+        full_is_streamk = tiles_full >= 148 and tiles_full < 0.988 * waves_full * 148
+        full = {"kernel": "hclooc_dgemm_streamk_kernel" if full_is_streamk else "hclooc_dgemm_tile_kernel<1> (whole waves: one CTA per tile)", "launch": f"{rows}x{nb}x{K}",
                 "ms_per_launch": ms_full, "achieved": 2.0 * rows * nb * K / (ms_full * 1e-3) / 1e12, "peak": FP64_PEAK_TFLOPS}
         full["frac"] = full["achieved"] / FP64_PEAK_TFLOPS
         del dA, dB, dC

@@ -429,6 +429,146 @@ extern "C" int hclooc_dpotrf(hclooc_ctx* ctx, int uplo, int64_t N, double* A, in
 }
 
 // ---------------------------------------------------------------------------------------------------------------------
+// DTRSM, side = Right, with a LOOK-AHEAD of one block column: the mirror image of dtrsm_left_lookahead below.  Block column j
+// (M x NB) is solved in device memory -- T_jj uploaded, row chunks on two streams, each chunk downloaded as soon as it is solved --
+// WHILE block column j+1 is brought up by the DGEMM pipeline and receives
+//     B_{j+1} <- alpha*B_{j+1} - X[:, solved before j] op(T)[solved before j, j+1]
+// (C blocks read from the host matrix, stored into the other resident buffer); the contribution of block column j,
+// -X_j op(T)[j, j+1], then comes straight from device memory.  ctx->mu is held by the caller.
+static int dtrsm_right_lookahead(hclooc_ctx* ctx, int uplo, int trans, int diag, int64_t M, int64_t N, double alpha, const double* A, int64_t lda,
+                                 double* B, int64_t ldb, size_t budget, bool own, int64_t NB, hclooc_stats* stats) {
+    const auto t_begin = std::chrono::steady_clock::now();
+    int rc;
+    if ((rc = ensure_aux(ctx))) return rc;
+    const bool lower_op = (uplo == HCL_UPLO_LOWER) != (trans == HCL_OP_T);    // op(T) is lower triangular
+    const int64_t nblk = (N + NB - 1) / NB, ldp = round_even(NB), ldt = round_even(NB);
+    const size_t pbytes = round_1k((size_t)M * ldp * 8), tbytes = round_1k((size_t)NB * ldt * 8);
+    const size_t reserved0 = 2 * pbytes + 2 * tbytes;
+    if (own) { if ((rc = ensure_workspace(ctx, budget))) return rc; }
+    uint8_t* base = (uint8_t*)ctx->workspace;
+    const uintptr_t mis = (uintptr_t)base & 1023u;
+    const size_t shift = mis ? 1024 - mis : 0;
+    if (reserved0 + shift > ctx->workspace_bytes) return HCLOOC_ERR_BUDGET;
+    double* dP[2] = {(double*)(base + shift), (double*)(base + shift + pbytes)};
+    double* dT = (double*)(base + shift + 2 * pbytes);               // T_jj of the block column being solved
+    double* dT2 = (double*)(base + shift + 2 * pbytes + tbytes);     // op(T)[current, next] as stored
+    Reserve guard(ctx, reserved0 + shift);
+    DbgScope dbg(ctx);
+    cudaStream_t s_sol[2] = {ctx->s_aux[0], ctx->s_aux[3]}, s_up = ctx->s_aux[1], s_down = ctx->s_aux[2];
+    cudaEvent_t ev_T = ctx->ev_aux[0], ev_T2 = ctx->ev_aux[1], ev_down[2] = {ctx->ev_aux[2], ctx->ev_aux[3]};
+    cudaEvent_t ev_sol[2] = {ctx->ev_aux[4], ctx->ev_aux[5]}, ev_ready = ctx->ev_aux[6], ev_chunk = ctx->ev_aux[7];
+    struct Drain {
+        hclooc_ctx* c;
+        ~Drain() { for (cudaStream_t st : c->s_aux) if (st) cudaStreamSynchronize(st); }
+    } drain{ctx};
+    static const int nchunk = [] { const char* e = std::getenv("HCLOOC_TRSM_CHUNKS"); const int v = e ? std::atoi(e) : 0; return v > 0 ? v : 4; }();
+    hclooc_stats acc;
+    std::memset(&acc, 0, sizeof(acc));
+    double t_enq = 0.0;
+    size_t ws_max = reserved0;
+    // x_j depends on the block columns BEFORE j when op(T) is upper, on the ones after it when op(T) is lower
+    auto cols_of = [&](int64_t bj, int64_t* c0, int64_t* nbj) {
+        const int64_t j = lower_op ? nblk - 1 - bj : bj;
+        *c0 = j * NB; *nbj = std::min(NB, N - *c0);
+    };
+    {   // block column 0 comes up whole
+        int64_t c0, nb0;
+        cols_of(0, &c0, &nb0);
+        if ((rc = copy2d(dP[0], (size_t)ldp * 8, B + c0, (size_t)ldb * 8, (size_t)nb0 * 8, (size_t)M, s_up))) return rc;
+        acc.bytes_h2d += (uint64_t)M * nb0 * 8; ++acc.n_copies_h2d;
+        HCL_CUDA(cudaEventRecord(ev_ready, s_up));
+    }
+    int64_t hr = ((M + nchunk - 1) / nchunk + 63) / 64 * 64;        // rows per chunk
+    if (hr < 1024) hr = 1024;
+    bool scaled = false;                                            // has alpha reached the block column in dP[cur]?
+    for (int64_t bj = 0; bj < nblk; ++bj) {
+        const int cur = (int)(bj & 1), alt = 1 - cur;
+        int64_t c0, nbj;
+        cols_of(bj, &c0, &nbj);
+        // ---- T_jj up, then the row chunks of block column bj on two streams; every chunk goes down as soon as it is solved
+        if ((rc = copy2d(dT, (size_t)ldt * 8, A + c0 * lda + c0, (size_t)lda * 8, (size_t)nbj * 8, (size_t)nbj, s_up))) return rc;
+        acc.bytes_h2d += (uint64_t)nbj * nbj * 8; ++acc.n_copies_h2d;
+        HCL_CUDA(cudaEventRecord(ev_T, s_up));
+        int64_t c = 0;
+        for (int64_t r0 = 0; r0 < M; r0 += hr, ++c) {
+            const int64_t hrows = std::min(hr, M - r0);
+            cudaStream_t st = s_sol[c & 1];
+            if (c < 2) { HCL_CUDA(cudaStreamWaitEvent(st, ev_T, 0)); HCL_CUDA(cudaStreamWaitEvent(st, ev_ready, 0)); }
+            if ((rc = dev_trsm(1, dT, ldt, lower_op ? 1 : 0, trans, diag, dP[cur] + r0 * ldp, ldp, hrows, nbj, scaled ? 1.0 : alpha, st, &acc.n_kernels))) return rc;
+            HCL_CUDA(cudaEventRecord(ev_chunk, st));
+            HCL_CUDA(cudaStreamWaitEvent(s_down, ev_chunk, 0));
+            debug_jitter(ctx, s_down);
+            if ((rc = copy2d(B + r0 * ldb + c0, (size_t)ldb * 8, dP[cur] + r0 * ldp, (size_t)ldp * 8, (size_t)nbj * 8, (size_t)hrows, s_down))) return rc;
+            acc.bytes_d2h += (uint64_t)hrows * nbj * 8; ++acc.n_copies_d2h;
+        }
+        HCL_CUDA(cudaEventRecord(ev_down[cur], s_down));
+        for (int s = 0; s < 2; ++s) HCL_CUDA(cudaEventRecord(ev_sol[s], s_sol[s]));
+        if (bj + 1 == nblk) break;
+        // ---- meanwhile: block column bj+1
+        int64_t q0, nb2;
+        cols_of(bj + 1, &q0, &nb2);
+        // op(T)[current, next] as stored: T[c0.., q0..] (nbj x nb2), or, transposed, T[q0.., c0..] (nb2 x nbj); dT2's previous reader
+        // is the update 2 of this block column, issued at the end of the last round and possibly still running
+        HCL_CUDA(cudaStreamWaitEvent(s_up, ev_ready, 0));
+        if (trans) rc = copy2d(dT2, (size_t)ldt * 8, A + q0 * lda + c0, (size_t)lda * 8, (size_t)nbj * 8, (size_t)nb2, s_up);
+        else rc = copy2d(dT2, (size_t)ldt * 8, A + c0 * lda + q0, (size_t)lda * 8, (size_t)nb2 * 8, (size_t)nbj, s_up);
+        if (rc) return rc;
+        acc.bytes_h2d += (uint64_t)nbj * nb2 * 8; ++acc.n_copies_h2d;
+        HCL_CUDA(cudaEventRecord(ev_T2, s_up));
+        // columns solved BEFORE the current block column: [0, c0) when op(T) is upper, [c0 + nbj, N) when it is lower
+        const int64_t k0 = lower_op ? c0 + nbj : 0, kk = lower_op ? N - (c0 + nbj) : c0;
+        bool next_scaled = false;
+        if (kk > 0) {
+            HCL_CUDA(cudaEventSynchronize(ev_down[alt]));                       // X of block column bj-1 is on the host (the pipeline reads it)
+            const double* Tp = trans ? A + q0 * lda + k0 : A + k0 * lda + q0;   // op(T)[solved, next], as stored
+            hclooc_stats one;
+            DgemmExtra ex;
+            ex.C_src = B + q0; ex.ldc_src = ldb;
+            ex.wait_before_store[0] = ev_ready;                                 // update 2 of block column bj read X_{bj-1} from dP[alt]
+            if (ctx->dbg_poison) {                                              // debug: the buffer is free now, nobody may still read X_{bj-1}
+                debug_poison(ctx, dP[alt], ldp, M, nb2, s_up);
+                HCL_CUDA(cudaEventRecord(ev_T2, s_up));
+                ex.wait_before_store[1] = ev_T2;
+            }
+            rc = dgemm_core_locked(ctx, 0, trans ? 1 : 0, M, nb2, kk, -1.0, B + k0, ldb, Tp, lda, alpha, dP[alt], ldp, budget, &one, 0, &ex);
+            if (rc) return rc;
+            add_stats(acc, one, &t_enq);
+            ws_max = std::max(ws_max, reserved0 + (size_t)one.plan.workspace_bytes);
+            next_scaled = true;
+        } else {                                                                // the second block column: nothing before the first one
+            if ((rc = copy2d(dP[alt], (size_t)ldp * 8, B + q0, (size_t)ldb * 8, (size_t)nb2 * 8, (size_t)M, s_up))) return rc;
+            acc.bytes_h2d += (uint64_t)M * nb2 * 8; ++acc.n_copies_h2d;
+            HCL_CUDA(cudaEventRecord(ev_T2, s_up));                             // (covers the block of T and the block column)
+        }
+        for (int s = 0; s < 2; ++s) HCL_CUDA(cudaEventSynchronize(ev_sol[s]));  // block column bj is solved
+        // ---- update 2: B_next <- beta' * B_next - X_current op(T)[current, next], all in device memory
+        HCL_CUDA(cudaStreamWaitEvent(s_sol[0], ev_T2, 0));
+        debug_jitter(ctx, s_sol[0]);
+        rc = launch_dgemm_tiles(M, nb2, nbj, -1.0, dP[cur], ldp, dT2, ldt, next_scaled ? 1.0 : alpha, dP[alt], ldp, s_sol[0], -1, nullptr, 0, trans ? 1 : 0);
+        if (rc) return rc;
+        ++acc.n_kernels;
+        HCL_CUDA(cudaEventRecord(ev_ready, s_sol[0]));
+        scaled = true;
+    }
+    for (cudaStream_t st : ctx->s_aux) if (st) HCL_CUDA(cudaStreamSynchronize(st));
+    if (stats) {
+        *stats = acc;
+        stats->plan.M = M; stats->plan.N = N; stats->plan.K = N;
+        stats->plan.mb = std::min(M, hr); stats->plan.nb = NB; stats->plan.kb = 128;
+        stats->plan.h = (M + hr - 1) / hr; stats->plan.w = nblk; stats->plan.kpanels = 1; stats->plan.n_steps = nblk;
+        stats->plan.workspace_bytes = ws_max;
+        stats->plan.n_sets = 2;
+        stats->plan.ldc_dev = ldp;
+        stats->plan.bytes_h2d = acc.bytes_h2d; stats->plan.bytes_d2h = acc.bytes_d2h;
+        stats->plan.n_copies_h2d = acc.n_copies_h2d; stats->plan.n_copies_d2h = acc.n_copies_d2h;
+        stats->plan.flops = (double)M * (double)N * (double)N;
+        stats->t_enqueue_s = t_enq;
+        stats->t_total_s = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_begin).count();
+    }
+    return HCLOOC_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
 // DTRSM with a side argument.  side = Right:  X op(T) = alpha B,  B is M x N (host), T the `uplo` triangle of the N x N host
 // matrix A.  Every row of B is an independent system, so (a) the rows are cut into bands small enough for a band of one block
 // column to sit in device memory, and (b) inside a band the block columns are solved in the order of substitution (ascending
@@ -468,7 +608,23 @@ extern "C" int hclooc_dtrsm_side(hclooc_ctx* ctx, int side, int uplo, int trans,
     size_t budget = 0;
     bool own = false;
     if ((rc = resolve_budget(ctx, device_budget_bytes, &budget, &own))) return rc;
-    // block-column width NB: the triangle buffer (NB x NB) takes at most a quarter of the budget; band height Mb: a band of one
+    // two whole block columns (M x NB) and two NB x NB blocks of T beside a quarter of the budget for the pipeline: the look-ahead
+    // form above (HCLOOC_TRSM_LOOKAHEAD=0: never); the widest NB of 4096, 2048, 1024 that fits
+    {
+        const char* e = std::getenv("HCLOOC_TRSM_LOOKAHEAD");
+        if (!(e && std::atoi(e) == 0) && N > 1024) {
+            for (int64_t nb = 4096; nb >= 1024; nb /= 2) {
+                const int64_t nbe = std::min(nb, N);
+                const size_t pb = round_1k((size_t)M * round_even(nbe) * 8), tb = round_1k((size_t)nbe * round_even(nbe) * 8);
+                if (2 * pb + 2 * tb + budget / 4 <= budget) {
+                    rc = dtrsm_right_lookahead(ctx, uplo, trans, diag, M, N, alpha, A, lda, B, ldb, budget, own, nbe, stats);
+                    if (!rc && stats) stats->t_total_s = std::chrono::duration<double>(std::chrono::steady_clock::now() - t_begin).count();
+                    return rc;
+                }
+            }
+        }
+    }
+    // staged form.  Block-column width NB: the triangle buffer (NB x NB) takes at most a quarter of the budget; band height Mb: a band of one
     // block column (Mb x NB) takes at most a quarter as well; the out-of-core DGEMM keeps the other half
     int64_t NB = 4096;
     while (NB > 128 && (size_t)NB * NB * 8 + 1024 > budget / 4) NB -= 128;

@@ -170,6 +170,8 @@ def dense_op(Aview, uplo, trans, unit):
     (64, 129, -0.5, "uniform", 1, 64 * MiB),       # one block column: no out-of-core update
     (1, 77, 1.0, "int", 0, 512 * 1024),            # a single row
     (700, 1500, 1.5, "uniform", 2, 6 * MiB),
+    (700, 2500, 1.5, "uniform", 2, 64 * MiB),      # two resident block columns of 1024 with the look-ahead, ragged third one
+    (517, 2100, 2.0, "int", 1, 48 * MiB),          # the same, exact
 ])
 def test_dtrsm_right_matches_oracle(H, uplo, trans, unit, M, N, alpha, dist, pad, budget):
     A = tri_host(H, N, 81, dist, pad)
@@ -190,6 +192,7 @@ def test_dtrsm_right_matches_oracle(H, uplo, trans, unit, M, N, alpha, dist, pad
     st = H.hclooc_dtrsm_side(None, H.HCL_SIDE_RIGHT, uplo, trans, unit, M, N, alpha, A, A.ld, B, B.ld, budget)
     got = B.view.copy()
     assert st.plan.workspace_bytes <= budget and st.n_kernels >= 1
+    assert st.plan.n_sets == (2 if budget >= 48 * MiB and N > 1024 else 1)       # look-ahead over two resident block columns / staged
     assert not np.isnan(got).any() and np.isnan(B.array[:, N:]).all()
     if dist == "int":
         assert np.array_equal(ref, alpha * X0)

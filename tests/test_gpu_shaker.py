@@ -97,17 +97,18 @@ def test_dtrsm_lookahead_staged_and_right_side_under_the_shaker(H, uplo, trans):
                 st = H.hclooc_dtrsm(None, uplo, trans, 0, M, N, 1.0, T, T.ld, B, B.ld, budget)
                 assert np.array_equal(B.view, X0.astype(np.float64)), (budget, seed)
             assert st.plan.n_sets == (2 if budget > 8 * MiB else 0)
-        # side = Right: row bands x block columns
-        Mr, Nr = 517, 1000
-        T = tri_host(H, Nr, 64, "int")
-        X0 = synthgen.fill_numpy(Mr, Nr, 64, "B", "int").astype(np.int64)
-        B = H.HostMatrix(Mr, Nr)
-        rhs = (X0 @ dense_op(T.view, uplo, trans, 0).astype(np.int64)).astype(np.float64)
-        for seed in SEEDS[:2]:
-            B.view[...] = rhs
-            H.hclooc_ctx_set_debug(None, seed, 1)
-            H.hclooc_dtrsm_side(None, 1, uplo, trans, 0, Mr, Nr, 1.0, T, T.ld, B, B.ld, 2 * MiB)
-            assert np.array_equal(B.view, X0.astype(np.float64)), seed
+        # side = Right: row bands x block columns (staged, 2 MiB), and two resident block columns of 1024 with the look-ahead (48 MiB)
+        for Mr, Nr, budget in ((517, 1000, 2 * MiB), (600, 2600, 48 * MiB)):
+            T = tri_host(H, Nr, 64, "int")
+            X0 = synthgen.fill_numpy(Mr, Nr, 64, "B", "int").astype(np.int64)
+            B = H.HostMatrix(Mr, Nr)
+            rhs = (X0 @ dense_op(T.view, uplo, trans, 0).astype(np.int64)).astype(np.float64)
+            for seed in SEEDS[:2]:
+                B.view[...] = rhs
+                H.hclooc_ctx_set_debug(None, seed, 1)
+                st = H.hclooc_dtrsm_side(None, 1, uplo, trans, 0, Mr, Nr, 1.0, T, T.ld, B, B.ld, budget)
+                assert np.array_equal(B.view, X0.astype(np.float64)), (budget, seed)
+            assert st.plan.n_sets == (2 if budget > 8 * MiB else 1) and st.plan.workspace_bytes <= budget
     finally:
         H.hclooc_ctx_set_debug(None, 0, 0)
 
