@@ -68,14 +68,14 @@ potrf_block_kernel(double* __restrict__ A, long long lda, int n, int lower, long
             const int e = base + u * PT + tid;
             const int r = e / PB, c = e % PB;                // global element A[r][c] = logical (r, c) of a lower, (c, r) of an upper block
             const int i = lower ? r : c, k = lower ? c : r;  // logical element (i, k), wanted for k <= i
-            v[u] = (k <= i && i < n) ? A[(long long)r * lda + c] : (i == k ? 1.0 : 0.0);
+            v[u] = A[(k <= i && i < n) ? (long long)r * lda + c : 0];    // unconditional (element 0 when not wanted): the loads of a batch must not wait for each other
         }
 #pragma unroll
         for (int u = 0; u < 16; ++u) {
             const int e = base + u * PT + tid;
             const int r = e / PB, c = e % PB;
             const int i = lower ? r : c, k = lower ? c : r;
-            if (k <= i) S[i * PS + k] = v[u];
+            if (k <= i) S[i * PS + k] = (i < n) ? v[u] : (i == k ? 1.0 : 0.0);
         }
     }
     __syncthreads();

@@ -56,15 +56,15 @@ __device__ __forceinline__ void stage_triangle(double* __restrict__ sTt, const d
             const bool need = q < ib && p < ib && (q > p || (q == p && !unit));
             const int r = lower ? q : ib - 1 - q, c = lower ? p : ib - 1 - p;         // op(T)[r][c]
             const long long at = need ? (trans ? (long long)c * ldt + r : (long long)r * ldt + c) : 0;
-            const double t = need ? T[at] : 0.0;
-            v[j] = need ? t : ((q == p) ? 1.0 : 0.0);
-        }
+            v[j] = __ldg(T + at);             // UNCONDITIONAL (element 0 when not needed): a predicated load followed by its select
+        }                                     // made ptxas wait for every load before issuing the next -- 64 round trips, 30 us
 #pragma unroll
         for (int j = 0; j < 16; ++j) {
             const int e = base + j * TTHREADS + tid;
             const int hi = e / TB, lo_ = e % TB;
             const int p = trans ? hi : lo_, q = trans ? lo_ : hi;
-            if (q >= p) sTt[p * TS + q] = v[j];
+            const bool need = q < ib && p < ib && (q > p || (q == p && !unit));
+            if (q >= p) sTt[p * TS + q] = need ? v[j] : ((q == p) ? 1.0 : 0.0);
         }
     }
     __syncthreads();
@@ -218,44 +218,55 @@ trsm_block_split_kernel(const double* __restrict__ T, long long ldt, int ib, dou
             }
         }
     }
+    // Eight groups of 16 steps, ONE copy of the code (a fully unrolled chain is 96 KB of straight-line code: every instruction
+    // a cache miss): after a group its 16 elements are final -- each lane stores its four and shifts the rest down, so the pivot
+    // block is always x[0..3] and the live blocks are i < 8 - tb (a uniform branch per block).
+#pragma unroll 1
+    for (int tb = 0; tb < 8; ++tb) {
+        const int nact = 8 - tb;
+        const double* tbase = sTt + (16 * tb) * TS + 16 * tb;      // tbase[tt * TS + e] = T'[16 tb + e][16 tb + tt]
 #pragma unroll
-    for (int t = 0; t < TB; ++t) {
-        const int li = (t / 16) * 4 + (t % 4), owner = (t / 4) % 4;
-        const double* tcol = sTt + t * TS;
-        const double cand = unit ? x[li] : x[li] * tcol[t];
-        const double xv = __shfl_sync(0xffffffffu, cand, owner, SPLIT);
-        if (j == owner) x[li] = xv;
+        for (int tt = 0; tt < 16; ++tt) {
+            const int li = tt % 4, owner = tt / 4;
+            const double* tcol = tbase + tt * TS;
+            const double cand = unit ? x[li] : x[li] * tcol[tt];
+            const double xv = __shfl_sync(0xffffffffu, cand, owner, SPLIT);
+            if (j == owner) x[li] = xv;
+            {                                     // the block that holds the pivot: only the elements below it (what lies above is not staged)
+                const double2 t01 = *reinterpret_cast<const double2*>(tcol + 4 * j);
+                const double2 t23 = *reinterpret_cast<const double2*>(tcol + 4 * j + 2);
+                const int e = 4 * j - tt;         // element c is below the pivot iff e + c > 0
+                if (e > 0) x[0] = fma(-t01.x, xv, x[0]);
+                if (e + 1 > 0) x[1] = fma(-t01.y, xv, x[1]);
+                if (e + 2 > 0) x[2] = fma(-t23.x, xv, x[2]);
+                if (e + 3 > 0) x[3] = fma(-t23.y, xv, x[3]);
+            }
 #pragma unroll
-        for (int i = t / 16; i < 8; ++i) {
-            const double2 t01 = *reinterpret_cast<const double2*>(tcol + 16 * i + 4 * j);
-            const double2 t23 = *reinterpret_cast<const double2*>(tcol + 16 * i + 4 * j + 2);
-            if (i > t / 16) {
-                x[4 * i] = fma(-t01.x, xv, x[4 * i]);
-                x[4 * i + 1] = fma(-t01.y, xv, x[4 * i + 1]);
-                x[4 * i + 2] = fma(-t23.x, xv, x[4 * i + 2]);
-                x[4 * i + 3] = fma(-t23.y, xv, x[4 * i + 3]);
-            } else {                              // the block that holds t: only the elements below it (what lies above is not staged)
-                const int e = 4 * j - (t % 16);   // element c is below t iff e + c > 0
-                if (e > 0) x[4 * i] = fma(-t01.x, xv, x[4 * i]);
-                if (e + 1 > 0) x[4 * i + 1] = fma(-t01.y, xv, x[4 * i + 1]);
-                if (e + 2 > 0) x[4 * i + 2] = fma(-t23.x, xv, x[4 * i + 2]);
-                if (e + 3 > 0) x[4 * i + 3] = fma(-t23.y, xv, x[4 * i + 3]);
+            for (int i = 1; i < 8; ++i) {
+                if (i < nact) {                   // uniform
+                    const double2 t01 = *reinterpret_cast<const double2*>(tcol + 16 * i + 4 * j);
+                    const double2 t23 = *reinterpret_cast<const double2*>(tcol + 16 * i + 4 * j + 2);
+                    x[4 * i] = fma(-t01.x, xv, x[4 * i]);
+                    x[4 * i + 1] = fma(-t01.y, xv, x[4 * i + 1]);
+                    x[4 * i + 2] = fma(-t23.x, xv, x[4 * i + 2]);
+                    x[4 * i + 3] = fma(-t23.y, xv, x[4 * i + 3]);
+                }
             }
         }
-    }
-    if (!live) return;
+        if (live) {
+            const int q = 16 * tb + 4 * j;
+            if (VEC == 4) {
+                double* p = lower ? P0 + q : P0 - q - 3;
+                if (lower) asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(x[0]), "d"(x[1]), "d"(x[2]), "d"(x[3]) : "memory");
+                else asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(x[3]), "d"(x[2]), "d"(x[1]), "d"(x[0]) : "memory");
+            } else {
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        const int q = 16 * i + 4 * j;
-        if (VEC == 4) {
-            double* p = lower ? P0 + q : P0 - q - 3;
-            if (lower) asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(x[4 * i]), "d"(x[4 * i + 1]), "d"(x[4 * i + 2]), "d"(x[4 * i + 3]) : "memory");
-            else asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(x[4 * i + 3]), "d"(x[4 * i + 2]), "d"(x[4 * i + 1]), "d"(x[4 * i]) : "memory");
-        } else {
-#pragma unroll
-            for (int c = 0; c < 4; ++c)
-                if (FULL || q + c < ib) P0[(long long)(q + c) * step] = x[4 * i + c];
+                for (int c = 0; c < 4; ++c)
+                    if (FULL || q + c < ib) P0[(long long)(q + c) * step] = x[c];
+            }
         }
+#pragma unroll
+        for (int k = 0; k < 28; ++k) x[k] = x[k + 4];
     }
 }
 
