@@ -134,6 +134,26 @@ int hclooc_plan_ex(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_
 int hclooc_plan_trans(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alpha_zero, size_t device_budget_bytes,
                       int operands_on_device, int transa, int transb, hclooc_plan_t* out);
 
+/* The RESIDENT schedule's shape for a call whose A, B and C fit the budget (pure host arithmetic; what hclooc_dgemm consults after
+ * planning the slices): applies = 1 if hclooc_dgemm would run it -- M, N, K >= 1024 and M*N*K >= 8e9 (small calls are latency bound:
+ * direct mode and graph replay own them), the device copies + stream-K scratch + staging ring within the budget, at least two K
+ * panels, and the schedule's estimate t_model_s below 0.985 * t_slice_model_s (pass the slice plan's plan.t_model_s; <= 0 skips the
+ * comparison); HCLOOC_RESIDENT=0 / 1 in the environment forces the answer where the schedule fits at all.  The shape is filled
+ * whenever it fits: h row blocks of mb rows, `npanels` K panels [panel_k0[p], panel_k0[p] + panel_kk[p]) graded from 256 or 512
+ * columns up to kb, phase 2 from panel p_switch on, `ring` staging buffers for the initial C (0 when beta == 0), workspace_bytes.
+ * Errors: -1..-3 non-positive dimension, -7 NULL out.                                                                         */
+#define HCLOOC_RESIDENT_MAX_PANELS 128
+typedef struct hclooc_resident_plan_t {
+    int32_t  applies, ring;
+    int64_t  mb, h, kb, npanels, p_switch;
+    int64_t  lda_dev, ldb_dev, ldc_dev;
+    uint64_t workspace_bytes;
+    double   t_flop_s, t_link_s, t_model_s;
+    int64_t  panel_k0[HCLOOC_RESIDENT_MAX_PANELS], panel_kk[HCLOOC_RESIDENT_MAX_PANELS];
+} hclooc_resident_plan_t;
+int hclooc_plan_resident(int64_t M, int64_t N, int64_t K, int beta_nonzero, size_t device_budget_bytes, double t_slice_model_s,
+                         hclooc_resident_plan_t* out);
+
 /* The paper's own rule, kept for reference and tests (:289, worked example :301): EQUAL slices only,
  * working set K*nb + 2*mb*K + 2*mb*nb <= budget_elements, least host-to-device traffic
  * w*M*K + K*N + M*N; ties: fewest steps, then smallest h.  Returns HCLOOC_ERR_BUDGET if nothing fits. */
@@ -236,6 +256,11 @@ int hclooc_ctx_set_debug(hclooc_ctx* ctx, uint64_t jitter_seed, int poison);
  *   1 GiB margin).  Uses a process-wide default context created on first use.
  *   beta == 0: C is never read (NaN/Inf in C are overwritten).  alpha == 0 or K == 0: A and B are not
  *   referenced, C = beta*C streamed through the device.  M == 0 or N == 0: returns 0, touches nothing.
+ *   Schedules: slices of A, B and C through the buffers of a plan (hclooc_plan; the paper's pipeline, :182-271); DIRECT mode for
+ *   small latency-bound calls (plan.direct); and, when A, B and C all FIT the budget and the cost model prefers it, the RESIDENT
+ *   schedule (plan.resident: K streamed in panels behind the uploads, C finished row block by row block under its own downloads;
+ *   HCLOOC_RESIDENT=0 / 1 in the environment forces the choice).  Floating-point results of different schedules agree within the
+ *   1e-13 * D gate, not bit for bit (the order of summation over K differs); integer-valued data is exact under all of them.
  * Errors: -1/-2/-3 negative M/N/K; -5 A NULL; -6 lda < K; -7 B NULL; -8 ldb < N; -10 C NULL or C
  *   overlaps A or B; -11 ldc < N; HCLOOC_ERR_BUDGET; HCLOOC_ERR_NOT_PINNED; HCLOOC_ERR_NOMEM;
  *   HCLOOC_ERR_CUDA.  Validation errors leave C untouched; after HCLOOC_ERR_CUDA C is unspecified.  */
@@ -332,8 +357,12 @@ int hclooc_dtrsm_plan(int64_t M, int64_t N, size_t device_budget_bytes, int libr
  * triangle and a band of one block column each take at most a quarter of the budget) sit in device memory one at a time; a
  * block column first receives  B_j <- alpha*B_j - X[:, solved] * op(T)[solved, j]  as one out-of-core DGEMM (C in device
  * memory), then its diagonal block is solved there by recursive halving down to 128-column blocks (one thread per row of B in
- * the block kernel).  Rounding and gate as hclooc_dtrsm (G23) with N in place of M; exact on integer data with a
- * power-of-two diagonal.  alpha == 0: X = 0, A not referenced.  stats: plan.mb = band height, plan.nb = NB, plan.flops = M*N*N.
+ * the block kernel).  When two whole block columns (M x NB, NB = 4096, 2048 or 1024) and two NB x NB blocks of T leave a quarter
+ * of the budget to the DGEMM pipeline, the LOOK-AHEAD form runs instead (plan.n_sets = 2): block column j is solved in device
+ * memory and downloaded in row chunks while the pipeline brings block column j+1 up with the update from the columns solved
+ * before j; HCLOOC_TRSM_LOOKAHEAD=0 in the environment keeps the staged form.  Rounding and gate as hclooc_dtrsm (DESIGN.md
+ * G23) with N in place of M; exact on integer data with a power-of-two diagonal.  alpha == 0: X = 0, A not referenced.
+ * stats: plan.mb = band height (staged) / rows per chunk (look-ahead), plan.nb = NB, plan.flops = M*N*N.
  * Errors: -2 side, -3 uplo, -4 trans, -5 diag, -6 M < 0, -7 N < 0, -9 A NULL, -10 lda too small, -11 B NULL or overlapping A,
  * -12 ldb < N; HCLOOC_ERR_BUDGET when not even a 32-column block fits; the HCLOOC_ERR_* codes of hclooc_dgemm.             */
 #define HCL_SIDE_LEFT  0

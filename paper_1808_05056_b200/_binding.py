@@ -16,7 +16,7 @@ HCL_SIDE_LEFT, HCL_SIDE_RIGHT = 0, 1
 
 # every symbol include/hclooc.h declares (tests check the .so exports all of them)
 EXPORTS = [
-    "hclooc_plan", "hclooc_plan_ex", "hclooc_plan_trans", "hclooc_shard_rows", "hclMatrixPartitioner", "hclooc_schedule", "hclooc_ctx_create", "hclooc_ctx_destroy",
+    "hclooc_plan", "hclooc_plan_ex", "hclooc_plan_trans", "hclooc_plan_resident", "hclooc_shard_rows", "hclMatrixPartitioner", "hclooc_schedule", "hclooc_ctx_create", "hclooc_ctx_destroy",
     "hclooc_ctx_set_trace", "hclooc_ctx_get_trace", "hclooc_ctx_set_direct", "hclooc_ctx_set_debug", "hclooc_calibrate_link",
     "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_t", "hclooc_dsyrk", "hclooc_dsyr2k", "hclooc_dtrsm", "hclooc_dtrsm_plan", "hclooc_dtrsm_side", "hclooc_dpotrf", "hclooc_dpotrf_plan", "hclooc_dtrmm", "hclooc_dsymm", "hclooc_dgemm_fig2", "hclooc_dgemm_nsteps", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
     "hclStreamDestroy", "hclEventDestroy", "hclMemcpy", "hclMemcpyAsync", "hclMemcpy2DAsync",
@@ -24,6 +24,13 @@ EXPORTS = [
     "hclooc_host_alloc", "hclooc_host_free", "hclooc_host_register", "hclooc_host_unregister",
     "hclooc_strerror", "hclooc_last_cuda_error", "hclooc_version", "hclooc_probe_fp64",
 ]
+
+
+class ResidentPlan(ctypes.Structure):
+    _fields_ = [("applies", c_int32), ("ring", c_int32), ("mb", c_int64), ("h", c_int64), ("kb", c_int64), ("npanels", c_int64),
+                ("p_switch", c_int64), ("lda_dev", c_int64), ("ldb_dev", c_int64), ("ldc_dev", c_int64), ("workspace_bytes", c_uint64),
+                ("t_flop_s", c_double), ("t_link_s", c_double), ("t_model_s", c_double),
+                ("panel_k0", c_int64 * 128), ("panel_kk", c_int64 * 128)]
 
 
 class Plan(ctypes.Structure):
@@ -77,6 +84,7 @@ def lib():
         L = ctypes.CDLL(_build.build())
         i64, dbl, vp, sz = c_int64, c_double, c_void_p, c_size_t
         L.hclooc_plan.argtypes = [i64, i64, i64, c_int, c_int, sz, POINTER(Plan)]
+        L.hclooc_plan_resident.argtypes = [i64, i64, i64, c_int, sz, dbl, POINTER(ResidentPlan)]
         L.hclooc_shard_rows.argtypes = [i64, c_int, c_int, i64, POINTER(i64), POINTER(i64)]
         L.hclooc_plan_ex.argtypes = [i64, i64, i64, c_int, c_int, sz, c_int, POINTER(Plan)]
         L.hclooc_plan_trans.argtypes = [i64, i64, i64, c_int, c_int, sz, c_int, c_int, c_int, POINTER(Plan)]
@@ -314,6 +322,13 @@ def hclooc_ctx_get_trace(ctx) -> np.ndarray:
     if n.value:
         _check(lib().hclooc_ctx_get_trace(ctx, recs.ctypes.data, n.value, byref(n)), "hclooc_ctx_get_trace")
     return recs
+
+
+def hclooc_plan_resident(M, N, K, beta_nonzero, device_budget_bytes, t_slice_model_s=0.0) -> ResidentPlan:
+    """The resident schedule's shape for a call whose matrices fit the budget (include/hclooc.h); .applies says whether hclooc_dgemm takes it."""
+    out = ResidentPlan()
+    _check(lib().hclooc_plan_resident(M, N, K, int(bool(beta_nonzero)), device_budget_bytes, float(t_slice_model_s), byref(out)), "hclooc_plan_resident")
+    return out
 
 
 def hclooc_dgemm(M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes) -> None:

@@ -51,8 +51,8 @@ bool resident_applies(int64_t M, int64_t N, int64_t K, bool beta_nonzero, size_t
     if (mode == 0) return false;
     if (M < 256 || N < 256 || K < 512) return false;
     if (M > 0x7fffffffLL || N > 0x7fffffffLL || K > 0x7fffffffLL) return false;
-    // small problems are latency bound: the pipeline's graph replay and direct mode own them
-    if (mode < 0 && ((double)M * (double)N * (double)K < 8e9 || M < 1024 || N < 1024 || K < 1024)) return false;
+    // small problems are latency bound: the pipeline's graph replay and direct mode own them (decided below, after the shape)
+    const bool small = (double)M * (double)N * (double)K < 8e9 || M < 1024 || N < 1024 || K < 1024;
     const MachineModel& mm = machine_model();
     ResidentShape S;
     std::memset(&S, 0, sizeof(S));
@@ -120,6 +120,8 @@ bool resident_applies(int64_t M, int64_t N, int64_t K, bool beta_nonzero, size_t
     S.t_model_s = std::max(t_compute_path, t_link_path) + t_tail;
     *out = S;
     if (mode > 0) return true;
+    if (small) return false;
+    if (!(t_slice_model_s > 0.0)) return true;
     // measured against the slice pipeline on the same calls (profiles/r02_transition_sweep.md): both models are within 2 % of the
     // clock, the resident schedule wins by 25 % at N = 8192, 4 % at 12288, 1.3 % at 16384 and ties at 20480
     return S.t_model_s < 0.985 * t_slice_model_s;
@@ -323,3 +325,25 @@ int dgemm_resident(hclooc_ctx* ctx, const ResidentShape& S, int64_t M, int64_t N
 }
 
 }  // namespace hclooc
+
+extern "C" int hclooc_plan_resident(int64_t M, int64_t N, int64_t K, int beta_nonzero, size_t device_budget_bytes, double t_slice_model_s,
+                                    hclooc_resident_plan_t* out) {
+    if (M < 1) return -1;
+    if (N < 1) return -2;
+    if (K < 1) return -3;
+    if (!out) return -7;
+    std::memset(out, 0, sizeof(*out));
+    hclooc::ResidentShape S;
+    std::memset(&S, 0, sizeof(S));
+    S.total = 0;
+    out->applies = hclooc::resident_applies(M, N, K, beta_nonzero != 0, device_budget_bytes, t_slice_model_s, &S) ? 1 : 0;
+    if (S.total == 0) return HCLOOC_OK;                 // it does not fit at all: nothing to describe
+    out->ring = S.ring;
+    out->mb = S.mb; out->h = S.h; out->kb = S.kb; out->npanels = S.npanels; out->p_switch = S.p_switch;
+    out->lda_dev = S.ldA; out->ldb_dev = S.ldB; out->ldc_dev = S.ldC;
+    out->workspace_bytes = S.total;
+    out->t_flop_s = S.t_flop_s; out->t_link_s = S.t_link_s; out->t_model_s = S.t_model_s;
+    for (int64_t p = 0; p < S.npanels; ++p) { out->panel_k0[p] = S.pk0[p]; out->panel_kk[p] = S.pkk[p]; }
+    return HCLOOC_OK;
+}
+
