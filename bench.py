@@ -748,6 +748,84 @@ def run_op(args):
     print(json.dumps(out))
 
 
+def run_cublasxt(args):
+    """`--op cublasxt`: SIDE REFERENCE ONLY (north_star: "cuBLAS-XT may be timed as a side reference only"; it is the library the paper
+    compares with, PAPER.md:372 / :396).  NVIDIA's out-of-core DGEMM, cublasXtDgemm, on the same pinned host matrices as `bench.py
+    --workload ...` / `--m --n --k`, one GPU, block dimension --xt-block (its tile size; the library streams tiles itself), wall time of
+    the call, beside hclooc_dgemm_ex on the very same buffers in the same process.  Loaded with ctypes from the CUDA toolkit's libcublas;
+    nothing of the product path links or calls it.  Row-major C = A B is the column-major product C^T = B^T A^T, so the operands swap."""
+    import ctypes
+    import glob
+    import torch
+    import synthgen
+    import paper_1808_05056_b200 as H
+    torch.cuda.set_device(0)
+    cands = sorted(glob.glob("/usr/local/cuda/lib64/libcublas.so.*")) or ["libcublas.so.12"]
+    try:
+        L = ctypes.CDLL(cands[0])
+    except OSError as e:
+        print(json.dumps({"op": "cublasXtDgemm", "unavailable": str(e)}))
+        return
+    M, N, K, budget = args.m, args.n, args.k, args.budget or 4 * GiB
+    live = measure_link(H)
+    if live:
+        LINK.update(live)
+    A, B, C = H.HostMatrix(M, K), H.HostMatrix(K, N), H.HostMatrix(M, N)
+    seed = synthgen.BASE_SEED + 9
+    for X, nm in ((A, "A"), (B, "B"), (C, "C")):
+        synthgen.fill(X.array, seed, nm, "uniform")
+    C0 = C.view[:64].copy()
+    handle = ctypes.c_void_p()
+    vp, i32, sz, dbl = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t, ctypes.c_double
+    L.cublasXtCreate.argtypes = [ctypes.POINTER(vp)]
+    L.cublasXtDestroy.argtypes = [vp]
+    L.cublasXtDeviceSelect.argtypes = [vp, i32, ctypes.POINTER(i32)]
+    L.cublasXtSetBlockDim.argtypes = [vp, i32]
+    L.cublasXtSetPinningMemMode.argtypes = [vp, i32]
+    L.cublasXtDgemm.argtypes = [vp, i32, i32, sz, sz, sz, ctypes.POINTER(dbl), vp, sz, vp, sz, ctypes.POINTER(dbl), vp, sz]
+
+    def chk(rc, what):
+        if rc != 0:
+            raise SystemExit(f"{what}: cublasStatus {rc}")
+    chk(L.cublasXtCreate(ctypes.byref(handle)), "cublasXtCreate")
+    dev = (i32 * 1)(0)
+    chk(L.cublasXtDeviceSelect(handle, 1, dev), "cublasXtDeviceSelect")
+    chk(L.cublasXtSetBlockDim(handle, args.xt_block), "cublasXtSetBlockDim")
+    alpha, beta = dbl(1.0), dbl(args.beta)
+    flops = 2.0 * M * N * K
+    rec = {"op": "cublasXtDgemm (side reference, not the product path)", "M": M, "N": N, "K": K, "beta": args.beta, "xt_block_dim": args.xt_block, "lib": cands[0]}
+    try:
+        ts = []
+        for _ in range(max(2, args.steps or 3)):
+            t0 = time.perf_counter()
+            # column-major: C^T (N x M, ld N) = B^T (N x K, ld N) * A^T (K x M, ld K);  CUBLAS_OP_N = 0
+            chk(L.cublasXtDgemm(handle, 0, 0, N, M, K, ctypes.byref(alpha), B.ptr, N, A.ptr, K, ctypes.byref(beta), C.ptr, N), "cublasXtDgemm")
+            torch.cuda.synchronize()
+            ts.append(time.perf_counter() - t0)
+        t = float(np.mean(ts[1:]))
+        t_roof, t_flop, t_link = link_roofline_s(flops, 8 * (M * K + K * N + (M * N if args.beta else 0)), 8 * M * N)
+        rec["cublasxt"] = {"t_s": t, "t_all_s": ts, "tflops": flops / t / 1e12, "frac_of_roofline_on_compulsory_bytes": t_roof / t}
+        # the product path on the very same buffers
+        ctx = H.hclooc_ctx_create(0)
+        try:
+            ts2, st = [], None
+            for _ in range(max(2, args.steps or 3)):
+                st = H.hclooc_dgemm_ex(ctx, M, N, K, 1.0, A, K, B, N, args.beta, C, N, budget)
+                ts2.append(st.t_total_s)
+        finally:
+            H.hclooc_ctx_destroy(ctx)
+        t2 = float(np.mean(ts2[1:]))
+        t_roof2, _, _ = link_roofline_s(flops, st.bytes_h2d, st.bytes_d2h)
+        rec["hclooc_dgemm"] = {"t_s": t2, "tflops": flops / t2 / 1e12, "budget_bytes": budget, "frac_of_roofline": t_roof2 / t2, "plan": Bench.plan_summary(st.plan)}
+        rec["hclooc_over_cublasxt"] = t / t2
+        rec["link_peaks"] = LINK
+    finally:
+        L.cublasXtDestroy(handle)
+        for X in (A, B, C):
+            X.free()
+    print(json.dumps(rec))
+
+
 def run_dev_op(args, H, torch):
     """`--op dtrsm_dev|dtrsm_right_dev|dpotrf_dev`: the DEVICE phases alone (hclDtrsmAsync / hclDpotrfAsync on device-resident operands:
     recursive halving down to the 128 x 128 block kernels), CUDA events on the launching stream, median of --steps launches.  With
@@ -881,8 +959,9 @@ def main():
     ap.add_argument("--trans", default="NN", choices=["NN", "TN", "NT", "TT"],
                     help="e2e leg through hclooc_dgemm_t with op(A), op(B) transposed (the same buffers read as the stored K x M / N x K matrices)")
     ap.add_argument("--kernel-only", action="store_true", help="only the kernel legs (for ncu captures of the tile kernel)")
-    ap.add_argument("--op", default="dgemm", choices=["dgemm", "dsyrk", "dsyr2k", "dtrsm", "dtrsm_right", "dpotrf", "dtrsm_dev", "dtrsm_right_dev", "dpotrf_dev"],
+    ap.add_argument("--op", default="dgemm", choices=["dgemm", "dsyrk", "dsyr2k", "dtrsm", "dtrsm_right", "dpotrf", "dtrsm_dev", "dtrsm_right_dev", "dpotrf_dev", "cublasxt"],
                     help="time another routine of the library instead (sizes from --m/--n/--k/--budget; --steps calls, the first discarded)")
+    ap.add_argument("--xt-block", type=int, default=8192, help="--op cublasxt: cublasXtSetBlockDim (the side reference's tile size)")
     ap.add_argument("--sweep", default="", choices=["", "transition"], help="transition: the paper's N sweep across the in-core / out-of-core point")
     ap.add_argument("--m", type=int, default=32768)
     ap.add_argument("--n", type=int, default=32768)
@@ -898,7 +977,7 @@ def main():
     if args.op != "dgemm":
         args.trans = int(args.trans[0] == "T") if isinstance(args.trans, str) else args.trans
         args.budget = args.budget or (4 << 30)
-        return run_op(args)
+        return run_cublasxt(args) if args.op == "cublasxt" else run_op(args)
     if args.impl == "reference":
         return run_reference(args)
     b = Bench(args)
