@@ -760,11 +760,19 @@ def run_cublasxt(args):
     import synthgen
     import paper_1808_05056_b200 as H
     torch.cuda.set_device(0)
-    cands = sorted(glob.glob("/usr/local/cuda/lib64/libcublas.so.*")) or ["libcublas.so.12"]
-    try:
-        L = ctypes.CDLL(cands[0])
-    except OSError as e:
-        print(json.dumps({"op": "cublasXtDgemm", "unavailable": str(e)}))
+    # the copy torch itself loaded its cublasLt from comes first (the toolkit's libcublas wants the toolkit's libcublasLt)
+    cands = sorted(glob.glob(os.path.join(os.path.dirname(os.path.dirname(torch.__file__)), "nvidia", "cublas", "lib", "libcublas.so.*"))) + \
+        sorted(glob.glob("/usr/local/cuda/lib64/libcublas.so.*")) + ["libcublas.so.12"]
+    L, errs = None, []
+    for cand in cands:
+        try:
+            L = ctypes.CDLL(cand)
+            cands = [cand]
+            break
+        except OSError as e:
+            errs.append(str(e))
+    if L is None:
+        print(json.dumps({"op": "cublasXtDgemm", "unavailable": errs}))
         return
     M, N, K, budget = args.m, args.n, args.k, args.budget or 4 * GiB
     live = measure_link(H)

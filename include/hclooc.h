@@ -153,6 +153,17 @@ typedef struct hclooc_resident_plan_t {
 } hclooc_resident_plan_t;
 int hclooc_plan_resident(int64_t M, int64_t N, int64_t K, int beta_nonzero, size_t device_budget_bytes, double t_slice_model_s,
                          hclooc_resident_plan_t* out);
+/* The resident schedule as the exact list of operations hclooc_dgemm enqueues for it, in host issue order (hclooc_op_t, declared
+ * below with the pipeline's schedule).  Streams: 0 = uploads, 1 = downloads, 2.. = compute (phase 2 alternates between 2 and 3 when
+ * n_compute >= 2).  Device buffers: 0 = the copy of A, 1 = of B, 2 = of C, 3 + s = staging slot s of the initial C.  Per kind:
+ * H2D_A / H2D_B: K panel [k0, k0 + kk) (all rows of A / those rows of B); GEMM: dC[r0 : r0 + nr, :] = alpha * dA[r0.., k0 : k0 + kk] *
+ * dB[k0.., :] + beta * dC[...]; H2D_C: host C rows [r0, r0 + nr) -> staging slot `buf`; AXPY: dC[r0.., :] += beta_call * slot `buf`;
+ * D2H_C: dC rows -> host C rows.  Events: panel p uploaded = p; C0 block r uploaded = npanels + r; slot of block r free again =
+ * npanels + h + r; row block r finished = npanels + 2h + r; phase 1 finished = npanels + 3h.  The tests run a vector-clock hazard
+ * check over this list without a GPU.  Errors: -1 plan NULL or inconsistent with M, -2..-4 dimensions, -6 n_compute < 1, -9 NULL.  */
+struct hclooc_op_t;
+int hclooc_resident_schedule(const hclooc_resident_plan_t* plan, int64_t M, int64_t N, int64_t K, int beta_nonzero, int n_compute,
+                             struct hclooc_op_t* ops, size_t max_ops, size_t* n_ops);
 
 /* The paper's own rule, kept for reference and tests (:289, worked example :301): EQUAL slices only,
  * working set K*nb + 2*mb*K + 2*mb*nb <= budget_elements, least host-to-device traffic
@@ -171,6 +182,7 @@ int hclMatrixPartitioner(int64_t M, int64_t N, int64_t K, int64_t budget_element
 #define HCLOOC_OP_D2H_C   4   /* R(c_ij) :309  device buffer `buf` -> host C[r0.., c0..]                    */
 #define HCLOOC_OP_WAIT    5   /* stream waits for event (hclWaitEvent, :116)                              */
 #define HCLOOC_OP_RECORD  6   /* event recorded in stream (Rec(x), :311)                                  */
+#define HCLOOC_OP_AXPY    7   /* resident schedule only: dC[r0.., :] += beta * staging buffer `buf`       */
 /* streams: 0 = H2D copy stream, 1 = D2H copy stream, 2 + c = compute stream c.
  * buffers: A slice buffer a = a; C block buffer c = n_abuf + c; B slice buffer b = n_abuf + n_sets + b.
  * events:  c = uploads of the step using C buffer c arrived (rA/rC); n_sets + c = its kernel finished (eA);

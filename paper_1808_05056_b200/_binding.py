@@ -16,7 +16,7 @@ HCL_SIDE_LEFT, HCL_SIDE_RIGHT = 0, 1
 
 # every symbol include/hclooc.h declares (tests check the .so exports all of them)
 EXPORTS = [
-    "hclooc_plan", "hclooc_plan_ex", "hclooc_plan_trans", "hclooc_plan_resident", "hclooc_shard_rows", "hclMatrixPartitioner", "hclooc_schedule", "hclooc_ctx_create", "hclooc_ctx_destroy",
+    "hclooc_plan", "hclooc_plan_ex", "hclooc_plan_trans", "hclooc_plan_resident", "hclooc_resident_schedule", "hclooc_shard_rows", "hclMatrixPartitioner", "hclooc_schedule", "hclooc_ctx_create", "hclooc_ctx_destroy",
     "hclooc_ctx_set_trace", "hclooc_ctx_get_trace", "hclooc_ctx_set_direct", "hclooc_ctx_set_debug", "hclooc_calibrate_link",
     "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_t", "hclooc_dsyrk", "hclooc_dsyr2k", "hclooc_dtrsm", "hclooc_dtrsm_plan", "hclooc_dtrsm_side", "hclooc_dpotrf", "hclooc_dpotrf_plan", "hclooc_dtrmm", "hclooc_dsymm", "hclooc_dgemm_fig2", "hclooc_dgemm_nsteps", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
     "hclStreamDestroy", "hclEventDestroy", "hclMemcpy", "hclMemcpyAsync", "hclMemcpy2DAsync",
@@ -85,6 +85,7 @@ def lib():
         i64, dbl, vp, sz = c_int64, c_double, c_void_p, c_size_t
         L.hclooc_plan.argtypes = [i64, i64, i64, c_int, c_int, sz, POINTER(Plan)]
         L.hclooc_plan_resident.argtypes = [i64, i64, i64, c_int, sz, dbl, POINTER(ResidentPlan)]
+        L.hclooc_resident_schedule.argtypes = [POINTER(ResidentPlan), i64, i64, i64, c_int, c_int, vp, sz, POINTER(sz)]
         L.hclooc_shard_rows.argtypes = [i64, c_int, c_int, i64, POINTER(i64), POINTER(i64)]
         L.hclooc_plan_ex.argtypes = [i64, i64, i64, c_int, c_int, sz, c_int, POINTER(Plan)]
         L.hclooc_plan_trans.argtypes = [i64, i64, i64, c_int, c_int, sz, c_int, c_int, c_int, POINTER(Plan)]
@@ -329,6 +330,16 @@ def hclooc_plan_resident(M, N, K, beta_nonzero, device_budget_bytes, t_slice_mod
     out = ResidentPlan()
     _check(lib().hclooc_plan_resident(M, N, K, int(bool(beta_nonzero)), device_budget_bytes, float(t_slice_model_s), byref(out)), "hclooc_plan_resident")
     return out
+
+
+def hclooc_resident_schedule(plan: ResidentPlan, M, N, K, beta_nonzero, n_compute=8) -> np.ndarray:
+    """The operations hclooc_dgemm enqueues for the resident schedule, in host issue order (OP_DTYPE records)."""
+    n = c_size_t()
+    _check(lib().hclooc_resident_schedule(byref(plan), M, N, K, int(bool(beta_nonzero)), n_compute, None, 0, byref(n)), "hclooc_resident_schedule")
+    ops = np.zeros(n.value, dtype=OP_DTYPE)
+    _check(lib().hclooc_resident_schedule(byref(plan), M, N, K, int(bool(beta_nonzero)), n_compute, ops.ctypes.data if n.value else None, n.value, byref(n)),
+           "hclooc_resident_schedule")
+    return ops
 
 
 def hclooc_dgemm(M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes) -> None:

@@ -342,7 +342,15 @@ int hclooc::plan_impl(int64_t M, int64_t N, int64_t K, int beta_nonzero, int alp
                     for (int64_t cand_mb : {(int64_t)1024, (int64_t)512, (int64_t)256, (int64_t)128})
                         if (cand_mb < top) tried[nt++] = cand_mb;
                     if (force_mb) { nt = 0; if (force_mb <= std::min(M, rows_max)) tried[nt++] = force_mb; }
+                    // a call that fills a resident panel of a look-ahead routine (C read from the host, stored on the device:
+                    // hclooc_dpotrf, hclooc_dtrsm[_side]) shares the SMs with that routine's device phase on other streams; the model
+                    // sees a link-bound call and would cut it into 128-row steps of split-K clusters.  Measured (32768^2, 4 GiB): blocks
+                    // of 1024 rows make the Cholesky (tall panels: M = 4096..28672) 4.7 % and the right-side DTRSM (M = 32768) 2 % faster;
+                    // the left-side DTRSM fills block ROWS (M = NB = 4096, N wide), where 1024-row blocks leave 4 steps per column and
+                    // cost 4 %: the floor is a sixteenth of M, at most 1024.
+                    const int64_t mb_floor = (c_in_host && !force_mb) ? std::min<int64_t>(top, std::min<int64_t>(1024, std::max<int64_t>(128, M / 16 / 128 * 128))) : 0;
                     for (int q = 0; q < nt; ++q) {
+                        if (tried[q] < mb_floor) continue;
                         Cand c{};
                         c.c_dev = c_dev;
                         c.c_in_host = c_in_host;

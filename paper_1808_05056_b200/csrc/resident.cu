@@ -127,6 +127,79 @@ bool resident_applies(int64_t M, int64_t N, int64_t K, bool beta_nonzero, size_t
     return S.t_model_s < 0.985 * t_slice_model_s;
 }
 
+// The resident schedule as a list of stream operations in host issue order -- the ONE source of what dgemm_resident enqueues
+// (hclooc_resident_schedule exports it; tests/test_resident_plan.py runs a vector-clock hazard check over it without a GPU).
+// Streams: 0 = uploads, 1 = downloads, 2.. = compute.  Device buffers: 0 = dA, 1 = dB, 2 = dC, 3 + s = staging slot s.
+// Events: panel p uploaded [0, np), C0 block r uploaded [np, np + h), staging slot of block r free again [np + h, np + 2h),
+// row block r finished [np + 2h, np + 3h), phase 1 finished np + 3h.
+void build_resident_schedule(const ResidentShape& S, int64_t M, int64_t N, int64_t K, bool c0, int n_compute, std::vector<hclooc_op_t>& ops) {
+    ops.clear();
+    const int64_t h = S.h, np = S.npanels, p_sw = S.p_switch;
+    auto blank = [](int kind, int stream) {
+        hclooc_op_t o;
+        std::memset(&o, 0, sizeof(o));
+        o.kind = kind; o.stream = stream; o.event = -1; o.buf = o.buf2 = o.buf3 = -1;
+        return o;
+    };
+    auto wait = [&](int stream, int64_t ev) { hclooc_op_t o = blank(HCLOOC_OP_WAIT, stream); o.event = (int32_t)ev; ops.push_back(o); };
+    auto record = [&](int stream, int64_t ev) { hclooc_op_t o = blank(HCLOOC_OP_RECORD, stream); o.event = (int32_t)ev; ops.push_back(o); };
+    auto upload_c0 = [&](int64_t r) {
+        const int64_t r0 = r * S.mb, mr = std::min(S.mb, M - r0);
+        if (r >= S.ring) wait(0, np + h + (r - S.ring));            // the slot's previous tenant has been added to its row block
+        hclooc_op_t o = blank(HCLOOC_OP_H2D_C, 0);
+        o.buf = 3 + (int32_t)(r % S.ring); o.r0 = r0; o.nr = mr; o.c0 = 0; o.nc = N; o.step = r;
+        ops.push_back(o);
+        record(0, np + r);
+    };
+    // ---- phase 1: panels up, whole-C kernels behind them
+    for (int64_t p = 0; p < np; ++p) {
+        hclooc_op_t a = blank(HCLOOC_OP_H2D_A, 0);
+        a.buf = 0; a.r0 = 0; a.nr = M; a.c0 = S.pk0[p]; a.nc = S.pkk[p]; a.k0 = S.pk0[p]; a.kk = S.pkk[p]; a.step = p;
+        ops.push_back(a);
+        hclooc_op_t b = blank(HCLOOC_OP_H2D_B, 0);
+        b.buf = 1; b.r0 = S.pk0[p]; b.nr = S.pkk[p]; b.c0 = 0; b.nc = N; b.k0 = S.pk0[p]; b.kk = S.pkk[p]; b.step = p;
+        ops.push_back(b);
+        record(0, p);
+        if (p < p_sw) {
+            wait(2, p);
+            hclooc_op_t g = blank(HCLOOC_OP_GEMM, 2);
+            g.buf = 0; g.buf2 = 1; g.buf3 = 2; g.r0 = 0; g.nr = M; g.c0 = 0; g.nc = N; g.k0 = S.pk0[p]; g.kk = S.pkk[p];
+            g.beta = p == 0 ? 0.0 : 1.0; g.step = p;
+            ops.push_back(g);
+        }
+    }
+    // ---- phase 2: row blocks finished, joined with C0, downloaded
+    if (c0) for (int64_t r = 0; r < std::min<int64_t>(h, S.ring); ++r) upload_c0(r);
+    const int n_k2 = n_compute >= 2 ? 2 : 1;
+    const int64_t k_sw = S.pk0[p_sw], k_rest = K - k_sw;
+    record(2, np + 3 * h);
+    for (int i = 0; i < n_k2; ++i) {
+        wait(2 + i, np - 1);                                         // the upload stream is in order: every panel is there
+        if (i > 0) wait(2 + i, np + 3 * h);                          // and phase 1 has finished on stream 2
+    }
+    for (int64_t r = 0; r < h; ++r) {
+        const int64_t r0 = r * S.mb, mr = std::min(S.mb, M - r0);
+        const int st = 2 + (int)(r % n_k2);
+        hclooc_op_t g = blank(HCLOOC_OP_GEMM, st);
+        g.buf = 0; g.buf2 = 1; g.buf3 = 2; g.r0 = r0; g.nr = mr; g.c0 = 0; g.nc = N; g.k0 = k_sw; g.kk = k_rest;
+        g.beta = p_sw == 0 ? 0.0 : 1.0; g.step = np + r;
+        ops.push_back(g);
+        if (c0) {
+            wait(st, np + r);
+            hclooc_op_t x = blank(HCLOOC_OP_AXPY, st);
+            x.buf = 3 + (int32_t)(r % S.ring); x.buf3 = 2; x.r0 = r0; x.nr = mr; x.c0 = 0; x.nc = N; x.beta = -1.0; x.step = np + h + r;
+            ops.push_back(x);
+            record(st, np + h + r);
+        }
+        record(st, np + 2 * h + r);
+        wait(1, np + 2 * h + r);
+        hclooc_op_t d = blank(HCLOOC_OP_D2H_C, 1);
+        d.buf = 2; d.r0 = r0; d.nr = mr; d.c0 = 0; d.nc = N; d.step = r;
+        ops.push_back(d);
+        if (c0 && r + S.ring < h) upload_c0(r + S.ring);
+    }
+}
+
 int dgemm_resident(hclooc_ctx* ctx, const ResidentShape& S, int64_t M, int64_t N, int64_t K, double alpha, const double* A, int64_t lda,
                    const double* B, int64_t ldb, double beta, double* C, int64_t ldc, hclooc_stats* stats,
                    std::chrono::steady_clock::time_point t_begin) {
@@ -141,151 +214,113 @@ int dgemm_resident(hclooc_ctx* ctx, const ResidentShape& S, int64_t M, int64_t N
     double* dC = (double*)(base + S.bytesA + S.bytesB);
     uint8_t* scratch = base + S.bytesA + S.bytesB + S.bytesC;
     uint8_t* stage0 = scratch + S.bytes_scratch;
-    auto stage = [&](int64_t r) { return (double*)(stage0 + (size_t)(r % S.ring) * S.bytes_stage); };
     const bool c0 = beta != 0.0;
     const int64_t h = S.h, np = S.npanels, p_sw = S.p_switch;
-    // events: panel p uploaded [0, np), C0 block r uploaded [np, np + h), staging slot free again [np + h, np + 2h),
-    // row block r finished [np + 2h, np + 3h)
-    const size_t n_events = (size_t)(np + 3 * h + 1);            // + phase 1 finished
+    const size_t n_events = (size_t)(np + 3 * h + 1);
     while (ctx->events.size() < n_events) {
         cudaEvent_t e;
         HCL_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
         ctx->events.push_back(e);
     }
-    auto ev_panel = [&](int64_t p) { return ctx->events[(size_t)p]; };
-    auto ev_c0 = [&](int64_t r) { return ctx->events[(size_t)(np + r)]; };
-    auto ev_free = [&](int64_t r) { return ctx->events[(size_t)(np + h + r)]; };
-    auto ev_done = [&](int64_t r) { return ctx->events[(size_t)(np + 2 * h + r)]; };
-    cudaEvent_t ev_phase1 = ctx->events[(size_t)(np + 3 * h)];
-    cudaStream_t s_up = ctx->s_h2d, s_down = ctx->s_d2h, s_k = ctx->s_compute[0];
     // phase 2 alternates between two compute streams when the context has them: the launch of row block r + 1 fills the partly
     // empty last wave of row block r (what the slice pipeline's kernels do for each other)
     const int n_k2 = ctx->n_compute >= 2 ? 2 : 1;
-    cudaStream_t s_k2[2] = {ctx->s_compute[0], ctx->n_compute >= 2 ? ctx->s_compute[1] : ctx->s_compute[0]};
+    build_resident_schedule(S, M, N, K, c0, ctx->n_compute, ctx->ops);
+    auto stream_of = [&](int s) { return s == 0 ? ctx->s_h2d : (s == 1 ? ctx->s_d2h : ctx->s_compute[s - 2]); };
     // tracing: timing events around every copy and kernel, as the pipeline's executor records them
     const bool trace = ctx->trace;
     size_t n_traced = 0;
     if (trace) {
-        const size_t need = 1 + 2 * (size_t)(2 * np + (c0 ? 2 * h : 0) + p_sw + 2 * h);
+        size_t need = 1;
+        for (const hclooc_op_t& o : ctx->ops) if (o.kind != HCLOOC_OP_WAIT && o.kind != HCLOOC_OP_RECORD) need += 2;
         while (ctx->trace_events.size() < need) {
             cudaEvent_t e;
             HCL_CUDA(cudaEventCreate(&e));
             ctx->trace_events.push_back(e);
         }
         ctx->trace_recs.clear();
-        HCL_CUDA(cudaEventRecord(ctx->trace_events[0], s_up));
+        HCL_CUDA(cudaEventRecord(ctx->trace_events[0], ctx->s_h2d));
     }
-    auto trace_begin = [&](int kind, int stream, int64_t step, double flops, uint64_t bytes, cudaStream_t st) {
-        if (!trace) return;
-        cudaEventRecord(ctx->trace_events[1 + 2 * n_traced], st);
-        hclooc_trace_rec r;
-        std::memset(&r, 0, sizeof(r));
-        r.kind = kind; r.stream = stream; r.step = step; r.flops = flops; r.bytes = bytes;
-        ctx->trace_recs.push_back(r);
-    };
-    auto trace_end = [&](cudaStream_t st) {
-        if (!trace) return;
-        cudaEventRecord(ctx->trace_events[2 + 2 * n_traced], st);
-        ++n_traced;
-    };
     uint64_t bytes_h2d = 0, bytes_d2h = 0, n_h2d = 0, n_d2h = 0, n_kernels = 0;
     const auto t_enq0 = std::chrono::steady_clock::now();
     if (ctx->dbg_poison) {           // nothing of a previous call may stand in for an upload that never came
-        debug_poison(ctx, dA, S.ldA, M, S.ldA, s_up);
-        debug_poison(ctx, dB, S.ldB, K, S.ldB, s_up);
-        debug_poison(ctx, dC, S.ldC, M, S.ldC, s_up);
+        debug_poison(ctx, dA, S.ldA, M, S.ldA, ctx->s_h2d);
+        debug_poison(ctx, dB, S.ldB, K, S.ldB, ctx->s_h2d);
+        debug_poison(ctx, dC, S.ldC, M, S.ldC, ctx->s_h2d);
     }
-    HCL_CUDA(cudaMemsetAsync(scratch + streamk_counter_offset(), 0, streamk_counter_bytes(), s_k));
-    // a launch fills whole waves of 148 tiles well enough by itself, or runs as the persistent stream-K kernel
-    auto launch = [&](int64_t m, int64_t k, const double* a, const double* b, double bt, double* c, cudaStream_t st, bool alone) {
-        const int64_t T = ((m + 127) / 128) * ((N + 127) / 128), waves = (T + 147) / 148;
-        const bool whole = !alone || (double)T >= 0.988 * (double)(waves * 148);
-        return launch_dgemm_tiles(m, N, k, alpha, a, S.ldA, b, S.ldB, bt, c, S.ldC, st, whole ? 1 : -1, whole ? nullptr : scratch);
-    };
-    // ---------------------------------------------------------------- phase 1: panels up, whole-C kernels behind them
-    for (int64_t p = 0; p < np && !rc; ++p) {
-        const int64_t k0 = S.pk0[p], kk = S.pkk[p];
-        debug_jitter(ctx, s_up);
-        trace_begin(HCLOOC_OP_H2D_A, 0, p, 0.0, (uint64_t)M * kk * 8, s_up);
-        rc = copy2d(dA + k0, (size_t)S.ldA * 8, A + k0, (size_t)lda * 8, (size_t)kk * 8, (size_t)M, s_up);
-        trace_end(s_up);
-        if (rc) break;
-        debug_jitter(ctx, s_up);
-        trace_begin(HCLOOC_OP_H2D_B, 0, p, 0.0, (uint64_t)kk * N * 8, s_up);
-        rc = copy2d(dB + k0 * S.ldB, (size_t)S.ldB * 8, B + k0 * ldb, (size_t)ldb * 8, (size_t)N * 8, (size_t)kk, s_up);
-        trace_end(s_up);
-        if (rc) break;
-        bytes_h2d += (uint64_t)(M + N) * kk * 8; n_h2d += 2;
-        HCL_CUDA(cudaEventRecord(ev_panel(p), s_up));
-        if (p < p_sw) {
-            HCL_CUDA(cudaStreamWaitEvent(s_k, ev_panel(p), 0));
-            debug_jitter(ctx, s_k);
-            trace_begin(HCLOOC_OP_GEMM, 2, p, 2.0 * (double)M * (double)N * (double)kk, 0, s_k);
-            rc = launch(M, kk, dA + k0, dB + k0 * S.ldB, p == 0 ? 0.0 : 1.0, dC, s_k, true);
-            trace_end(s_k);
-            ++n_kernels;
+    HCL_CUDA(cudaMemsetAsync(scratch + streamk_counter_offset(), 0, streamk_counter_bytes(), ctx->s_compute[0]));
+    rc = HCLOOC_OK;
+    for (const hclooc_op_t& o : ctx->ops) {
+        cudaStream_t st = stream_of(o.stream);
+        if (o.kind == HCLOOC_OP_WAIT) {
+            // sabotage mode of the shaker: the staging ring's waits are dropped on both sides (slots refilled before their tenant
+            // was used: event range [np + h, np + 2h) on the upload stream; blocks used before they arrived: [np, np + h))
+            if (ctx->dbg_poison == 2 && o.event >= np && o.event < np + 2 * h) continue;
+            HCL_CUDA(cudaStreamWaitEvent(st, ctx->events[(size_t)o.event], 0));
+            continue;
         }
-    }
-    // ---------------------------------------------------------------- phase 2: row blocks finished, joined with C0, downloaded
-    auto upload_c0 = [&](int64_t r) -> int {
-        const int64_t r0 = r * S.mb, mr = std::min(S.mb, M - r0);
-        // the slot's previous tenant must have been added to its row block (sabotage mode 2 of the shaker: the wait is skipped)
-        if (r >= S.ring && ctx->dbg_poison != 2) HCL_CUDA(cudaStreamWaitEvent(s_up, ev_free(r - S.ring), 0));
-        debug_jitter(ctx, s_up);
-        if (ctx->dbg_poison) debug_poison(ctx, stage(r), S.ldC, mr, N, s_up);
-        trace_begin(HCLOOC_OP_H2D_C, 0, r, 0.0, (uint64_t)mr * N * 8, s_up);
-        int rc2 = copy2d(stage(r), (size_t)S.ldC * 8, C + r0 * ldc, (size_t)ldc * 8, (size_t)N * 8, (size_t)mr, s_up);
-        trace_end(s_up);
-        if (rc2) return rc2;
-        bytes_h2d += (uint64_t)mr * N * 8; ++n_h2d;
-        HCL_CUDA(cudaEventRecord(ev_c0(r), s_up));
-        return HCLOOC_OK;
-    };
-    if (c0) for (int64_t r = 0; r < std::min<int64_t>(h, S.ring) && !rc; ++r) rc = upload_c0(r);
-    const int64_t k_sw = S.pk0[p_sw], k_rest = K - k_sw;
-    if (!rc) {
-        HCL_CUDA(cudaEventRecord(ev_phase1, s_k));
-        for (int i = 0; i < n_k2; ++i) {
-            HCL_CUDA(cudaStreamWaitEvent(s_k2[i], ev_panel(np - 1), 0));   // the upload stream is in order: every panel is there
-            if (s_k2[i] != s_k) HCL_CUDA(cudaStreamWaitEvent(s_k2[i], ev_phase1, 0));
+        if (o.kind == HCLOOC_OP_RECORD) {
+            HCL_CUDA(cudaEventRecord(ctx->events[(size_t)o.event], st));
+            continue;
         }
-    }
-    for (int64_t r = 0; r < h && !rc; ++r) {
-        const int64_t r0 = r * S.mb, mr = std::min(S.mb, M - r0);
-        double* dCr = dC + r0 * S.ldC;
-        cudaStream_t s_r = s_k2[r % n_k2];
-        const int sid = 2 + (int)(r % n_k2);
-        debug_jitter(ctx, s_r);
-        trace_begin(HCLOOC_OP_GEMM, sid, np + r, 2.0 * (double)mr * (double)N * (double)k_rest, 0, s_r);
-        rc = launch(mr, k_rest, dA + r0 * S.ldA + k_sw, dB + k_sw * S.ldB, p_sw == 0 ? 0.0 : 1.0, dCr, s_r, n_k2 == 1);
-        trace_end(s_r);
-        ++n_kernels;
-        if (rc) break;
-        if (c0) {
-            if (ctx->dbg_poison != 2) HCL_CUDA(cudaStreamWaitEvent(s_r, ev_c0(r), 0));     // (sabotage mode of the shaker: not waited for)
-            debug_jitter(ctx, s_r);
-            trace_begin(HCLOOC_OP_GEMM, sid, np + h + r, 2.0 * (double)mr * (double)N, 0, s_r);
-            const int cols2 = (int)((N + 1) / 2);
-            dim3 grid((unsigned)std::min<int64_t>((cols2 + 255) / 256, 32), (unsigned)std::min<int64_t>(mr, 1024));
-            resident_axpy_kernel<<<grid, 256, 0, s_r>>>(dCr, (long long)S.ldC, stage(r), (long long)S.ldC, (int)mr, cols2, beta);
-            trace_end(s_r);
-            HCL_CUDA(cudaGetLastError());
-            ++n_kernels;
-            HCL_CUDA(cudaEventRecord(ev_free(r), s_r));
+        debug_jitter(ctx, st);
+        double* stage = o.buf >= 3 ? (double*)(stage0 + (size_t)(o.buf - 3) * S.bytes_stage) : nullptr;
+        if (o.kind == HCLOOC_OP_H2D_C && ctx->dbg_poison) debug_poison(ctx, stage, S.ldC, o.nr, N, st);
+        if (trace) {
+            cudaEventRecord(ctx->trace_events[1 + 2 * n_traced], st);
+            hclooc_trace_rec r;
+            std::memset(&r, 0, sizeof(r));
+            r.kind = o.kind == HCLOOC_OP_AXPY ? HCLOOC_OP_GEMM : o.kind; r.stream = o.stream; r.step = o.step;
+            if (o.kind == HCLOOC_OP_GEMM) r.flops = 2.0 * (double)o.nr * (double)o.nc * (double)o.kk;
+            else if (o.kind == HCLOOC_OP_AXPY) r.flops = 2.0 * (double)o.nr * (double)o.nc;
+            else r.bytes = (uint64_t)o.nr * (uint64_t)o.nc * 8;
+            ctx->trace_recs.push_back(r);
         }
-        HCL_CUDA(cudaEventRecord(ev_done(r), s_r));
-        HCL_CUDA(cudaStreamWaitEvent(s_down, ev_done(r), 0));
-        debug_jitter(ctx, s_down);
-        trace_begin(HCLOOC_OP_D2H_C, 1, r, 0.0, (uint64_t)mr * N * 8, s_down);
-        rc = copy2d(C + r0 * ldc, (size_t)ldc * 8, dCr, (size_t)S.ldC * 8, (size_t)N * 8, (size_t)mr, s_down);
-        trace_end(s_down);
-        bytes_d2h += (uint64_t)mr * N * 8; ++n_d2h;
+        switch (o.kind) {
+            case HCLOOC_OP_H2D_A:
+                rc = copy2d(dA + o.k0, (size_t)S.ldA * 8, A + o.k0, (size_t)lda * 8, (size_t)o.kk * 8, (size_t)M, st);
+                bytes_h2d += (uint64_t)M * o.kk * 8; ++n_h2d;
+                break;
+            case HCLOOC_OP_H2D_B:
+                rc = copy2d(dB + o.k0 * S.ldB, (size_t)S.ldB * 8, B + o.k0 * ldb, (size_t)ldb * 8, (size_t)N * 8, (size_t)o.kk, st);
+                bytes_h2d += (uint64_t)o.kk * N * 8; ++n_h2d;
+                break;
+            case HCLOOC_OP_H2D_C:
+                rc = copy2d(stage, (size_t)S.ldC * 8, C + o.r0 * ldc, (size_t)ldc * 8, (size_t)N * 8, (size_t)o.nr, st);
+                bytes_h2d += (uint64_t)o.nr * N * 8; ++n_h2d;
+                break;
+            case HCLOOC_OP_D2H_C:
+                rc = copy2d(C + o.r0 * ldc, (size_t)ldc * 8, dC + o.r0 * S.ldC, (size_t)S.ldC * 8, (size_t)N * 8, (size_t)o.nr, st);
+                bytes_d2h += (uint64_t)o.nr * N * 8; ++n_d2h;
+                break;
+            case HCLOOC_OP_GEMM: {
+                // a launch that runs alone fills whole waves of 148 tiles well enough by itself or goes out as the persistent
+                // stream-K kernel; the phase-2 launches on two streams fill each other's last wave
+                const bool alone = o.step < np || n_k2 == 1;
+                const int64_t T = ((o.nr + 127) / 128) * ((N + 127) / 128), waves = (T + 147) / 148;
+                const bool whole = !alone || (double)T >= 0.988 * (double)(waves * 148);
+                rc = launch_dgemm_tiles(o.nr, N, o.kk, alpha, dA + o.r0 * S.ldA + o.k0, S.ldA, dB + o.k0 * S.ldB, S.ldB, o.beta,
+                                        dC + o.r0 * S.ldC, S.ldC, st, whole ? 1 : -1, whole ? nullptr : scratch);
+                ++n_kernels;
+                break;
+            }
+            case HCLOOC_OP_AXPY: {
+                const int cols2 = (int)((N + 1) / 2);
+                dim3 grid((unsigned)std::min<int64_t>((cols2 + 255) / 256, 32), (unsigned)std::min<int64_t>(o.nr, 1024));
+                resident_axpy_kernel<<<grid, 256, 0, st>>>(dC + o.r0 * S.ldC, (long long)S.ldC, stage, (long long)S.ldC, (int)o.nr, cols2, beta);
+                cudaError_t e = cudaGetLastError();
+                if (e != cudaSuccess) rc = cuda_fail(e);
+                ++n_kernels;
+                break;
+            }
+            default: rc = HCLOOC_ERR_INTERNAL;
+        }
+        if (trace) { cudaEventRecord(ctx->trace_events[2 + 2 * n_traced], st); ++n_traced; }
         if (rc) break;
-        if (c0 && r + S.ring < h) rc = upload_c0(r + S.ring);
     }
     const auto t_enq1 = std::chrono::steady_clock::now();
-    cudaError_t e1 = cudaStreamSynchronize(s_down), e2 = cudaStreamSynchronize(s_up), e3 = cudaStreamSynchronize(s_k);
-    if (e3 == cudaSuccess) e3 = cudaStreamSynchronize(s_k2[1]);
+    cudaError_t e1 = cudaStreamSynchronize(ctx->s_d2h), e2 = cudaStreamSynchronize(ctx->s_h2d), e3 = cudaStreamSynchronize(ctx->s_compute[0]);
+    if (e3 == cudaSuccess && n_k2 == 2) e3 = cudaStreamSynchronize(ctx->s_compute[1]);
     if (rc) return rc;
     if (e1 != cudaSuccess) return cuda_fail(e1);
     if (e2 != cudaSuccess) return cuda_fail(e2);
@@ -344,6 +379,27 @@ extern "C" int hclooc_plan_resident(int64_t M, int64_t N, int64_t K, int beta_no
     out->workspace_bytes = S.total;
     out->t_flop_s = S.t_flop_s; out->t_link_s = S.t_link_s; out->t_model_s = S.t_model_s;
     for (int64_t p = 0; p < S.npanels; ++p) { out->panel_k0[p] = S.pk0[p]; out->panel_kk[p] = S.pkk[p]; }
+    return HCLOOC_OK;
+}
+
+extern "C" int hclooc_resident_schedule(const hclooc_resident_plan_t* plan, int64_t M, int64_t N, int64_t K, int beta_nonzero, int n_compute,
+                                        hclooc_op_t* ops, size_t max_ops, size_t* n_ops) {
+    if (!plan) return -1;
+    if (M < 1) return -2;
+    if (N < 1) return -3;
+    if (K < 1) return -4;
+    if (n_compute < 1) return -6;
+    if (!n_ops) return -9;
+    if (plan->npanels < 1 || plan->npanels > HCLOOC_RESIDENT_MAX_PANELS || plan->mb < 1 || plan->h != (M + plan->mb - 1) / plan->mb ||
+        plan->p_switch < 0 || plan->p_switch >= plan->npanels || (beta_nonzero && plan->ring < 1)) return -1;
+    hclooc::ResidentShape S;
+    std::memset(&S, 0, sizeof(S));
+    S.mb = plan->mb; S.h = plan->h; S.kb = plan->kb; S.npanels = plan->npanels; S.p_switch = plan->p_switch; S.ring = plan->ring;
+    for (int64_t p = 0; p < plan->npanels; ++p) { S.pk0[p] = plan->panel_k0[p]; S.pkk[p] = plan->panel_kk[p]; }
+    std::vector<hclooc_op_t> v;
+    hclooc::build_resident_schedule(S, M, N, K, beta_nonzero != 0, n_compute, v);
+    *n_ops = v.size();
+    if (ops) std::memcpy(ops, v.data(), std::min(max_ops, v.size()) * sizeof(hclooc_op_t));
     return HCLOOC_OK;
 }
 
