@@ -11,7 +11,7 @@ exact symmetry, int64 exactness, untouched other triangle; dtrsm: scipy's solve_
 arithmetic on tiny cases, identity / diagonal / all-ones closed forms, int64 exactness, transposed-storage identity; the D returned
 by dsyrk / dsyr2k against numpy's |A||B|^T products; dtrsm_gate against gamma_(M+2) in exact arithmetic; oracle/checksum.py
 against the full oracle, int64 arithmetic and single-element mutations; dtrsm_right / dtrmm / dsymm / dpotrf (level3_oracle.c) in
-tests/test_oracle_level3.py) -- nothing here is "parity unpinned".
+tests/test_oracle_level3.py; dgetrf and its residual in tests/test_oracle_lu.py) -- nothing here is "parity unpinned".
 """
 from __future__ import annotations
 
@@ -68,6 +68,10 @@ def _load():
         lib.oracle_dpotrf.argtypes = [ctypes.c_int, _i64, _ptr, _i64, ctypes.POINTER(_i64)]
         lib.oracle_dpotrf_residual.restype = ctypes.c_int
         lib.oracle_dpotrf_residual.argtypes = [ctypes.c_int, _i64, _ptr, _i64, _ptr, _i64, _i64, _ptr, _i64, _ptr, _ptr, _ptr]
+        lib.oracle_dgetrf.restype = ctypes.c_int
+        lib.oracle_dgetrf.argtypes = [_i64, _i64, _ptr, _i64, _ptr, ctypes.POINTER(_i64)]
+        lib.oracle_dgetrf_residual.restype = ctypes.c_int
+        lib.oracle_dgetrf_residual.argtypes = [_i64, _i64, _ptr, _i64, _ptr, _i64, _ptr, _i64, _ptr, _i64, _ptr, _ptr, _ptr]
         _lib = lib
     return _lib
 
@@ -295,6 +299,48 @@ def dpotrf_residual(uplo, A0, F, rows=None, cols=None):
                                         nc, 0 if c is None else c.ctypes.data, res.ctypes.data, den.ctypes.data)
     if rc != 0:
         raise ValueError("oracle_dpotrf_residual: bad argument")
+    return res, den
+
+
+def dgetrf(A):
+    """LU factorization with partial pivoting of the row-major M x N matrix A, in place (oracle_dgetrf: Gaussian elimination
+    column by column, first maximum as the pivot).  Returns (ipiv, info): ipiv[j] = the row (0-based) exchanged with row j,
+    j < min(M, N); info = 0, or j+1 for the first exactly-zero pivot."""
+    M, N = A.shape
+    ap, lda = _chk2d(A, "A") if A.size else (0, 1)
+    ipiv = np.zeros(min(M, N), dtype=np.int64)
+    info = _i64(0)
+    rc = _load().oracle_dgetrf(M, N, ap, lda, ipiv.ctypes.data if ipiv.size else 0, ctypes.byref(info))
+    if rc != 0:
+        raise ValueError("oracle_dgetrf: bad argument")
+    return ipiv, int(info.value)
+
+
+# gate for an LU factorization with n = min(M, N) pivots (DESIGN.md reading G27): the computed factors of Gaussian elimination in
+# ANY order of its operations satisfy |P A - L U| <= gamma_n |L||U| elementwise (Higham thm 9.3; partitioned LU with conventional
+# matrix products keeps the bound, Higham section 13.2).
+def dgetrf_gate(n: int) -> float:
+    u = 2.0 ** -53
+    return n * u / (1.0 - n * u)
+
+
+def dgetrf_residual(A0, F, ipiv, rows=None, cols=None):
+    """(res, den) of oracle_dgetrf_residual on the sampled rows x cols (None: all): |(P A0)_ij - sum_k l_ik u_kj| and
+    sum_k |l_ik||u_kj| in long double; A0 = the original matrix, F = the candidate factors (L below the diagonal, unit diagonal
+    not stored, U on and above it), ipiv = the candidate interchanges (0-based)."""
+    M, N = A0.shape
+    ap, lda = _chk2d(A0, "A0")
+    fp, ldf = _chk2d(F, "F")
+    ip = np.ascontiguousarray(ipiv, dtype=np.int64)
+    assert ip.size == min(M, N)
+    r = None if rows is None else np.ascontiguousarray(rows, dtype=np.int64)
+    c = None if cols is None else np.ascontiguousarray(cols, dtype=np.int64)
+    nr, nc = (M if r is None else r.size), (N if c is None else c.size)
+    res, den = np.empty((nr, nc)), np.empty((nr, nc))
+    rc = _load().oracle_dgetrf_residual(M, N, ap, lda, fp, ldf, ip.ctypes.data, nr, 0 if r is None else r.ctypes.data,
+                                        nc, 0 if c is None else c.ctypes.data, res.ctypes.data, den.ctypes.data)
+    if rc != 0:
+        raise ValueError("oracle_dgetrf_residual: bad argument (an interchange out of range?)")
     return res, den
 
 

@@ -6,6 +6,8 @@
  *     oracle_dtrmm         B := alpha * op(T) * B   or   B := alpha * B * op(T)    (DTRMM, both sides)
  *     oracle_dpotrf        A = L * L^T  or  A = U^T * U                            (Cholesky factorization, DPOTRF)
  *     oracle_dpotrf_residual   |A - L L^T| and |L||L^T| on sampled entries, in long double
+ *     oracle_dgetrf        P * A = L * U                                           (LU factorization with partial pivoting, DGETRF)
+ *     oracle_dgetrf_residual   |P A - L U| and |L||U| on sampled entries, in long double
  *
  * The paper gives no algorithm for any of them, so each oracle is the plain textbook DEFINITION written out element by element
  * (row-major storage, leading dimensions in elements, FP64, every product rounded and then added or subtracted: compiled with
@@ -184,5 +186,90 @@ int oracle_dpotrf_residual(int uplo, int64_t N, const double* A0, int64_t lda, c
             den[r * nc + c] = (double)d;
         }
     }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------------------------------------------------
+ * DGETRF: the LU factorization with partial pivoting (row interchanges) of a general M x N matrix (PAPER.md:412 names
+ * "LU" first among the out-of-core factorizations to be built on the DGEMM; reading G27 in DESIGN.md):
+ *     P * A = L * U,    L  M x min(M,N) unit lower trapezoidal (|l_ij| <= 1),   U  min(M,N) x N upper trapezoidal,
+ * L (without its unit diagonal) and U overwrite A.  The textbook definition, Gaussian elimination column by column
+ * (Golub & Van Loan, Matrix Computations, alg. 3.4.1; LAPACK's unblocked DGETF2 is the same recurrences):
+ *     for j = 0 .. min(M,N)-1:
+ *         p = the SMALLEST i >= j with |a_ij| = max_{i >= j} |a_ij|                 (the first maximum, as IDAMAX)
+ *         ipiv[j] = p  (0-based; LAPACK's is 1-based);  exchange rows j and p of the whole matrix (all N columns)
+ *         if a_jj == 0:  *info = j+1 unless it is set already; next j   (the column is zero from row j down: nothing to eliminate)
+ *         for i > j:   a_ij = a_ij / a_jj;    for k > j:  a_ik = a_ik - a_ij * a_jk     (product rounded, then subtracted)
+ * *info = 0, or j+1 for the first exactly-zero pivot u_jj (the factorization is completed all the same, as in LAPACK; U is
+ * then singular).  NaN entries: unspecified.  Returns 0 (also when *info > 0), -1 on a bad argument. */
+int oracle_dgetrf(int64_t M, int64_t N, double* A, int64_t lda, int64_t* ipiv, int64_t* info) {
+    if (M < 0 || N < 0 || !info) return -1;
+    *info = 0;
+    if (M == 0 || N == 0) return 0;
+    if (!A || lda < N || !ipiv) return -1;
+    const int64_t n = M < N ? M : N;
+    for (int64_t j = 0; j < n; ++j) {
+        int64_t p = j;
+        double best = fabs(A[j * lda + j]);
+        for (int64_t i = j + 1; i < M; ++i) {
+            const double v = fabs(A[i * lda + j]);
+            if (v > best) { best = v; p = i; }
+        }
+        ipiv[j] = p;
+        if (p != j)
+            for (int64_t k = 0; k < N; ++k) { const double t = A[j * lda + k]; A[j * lda + k] = A[p * lda + k]; A[p * lda + k] = t; }
+        const double piv = A[j * lda + j];
+        if (piv == 0.0) { if (*info == 0) *info = j + 1; continue; }
+        for (int64_t i = j + 1; i < M; ++i) {
+            const double l = A[i * lda + j] / piv;
+            A[i * lda + j] = l;
+            for (int64_t k = j + 1; k < N; ++k) { const double prod = l * A[j * lda + k]; A[i * lda + k] = A[i * lda + k] - prod; }
+        }
+    }
+    return 0;
+}
+
+/* Backward residual of a candidate LU factorization on sampled entries, in long double:
+ *     res[r*nc + c] = | (P A0)_ij - sum_k l_ik u_kj |,    den[r*nc + c] = sum_k |l_ik||u_kj|,    k = 0 .. min(i, j, min(M,N)-1)
+ * for i = rows[r] (NULL: r), j = cols[c] (NULL: c); l_ik = F[i][k] for k < i, l_ii = 1, u_kj = F[k][j] for k <= j; P A0 is A0 with
+ * the interchanges ipiv[0], ipiv[1], ... applied in that order (row j <-> row ipiv[j]).  Gaussian elimination in ANY order of
+ * the operations satisfies |P A - L U| <= gamma_n |L||U| elementwise, n = min(M,N) (Higham, Accuracy and Stability of Numerical
+ * Algorithms, thm 9.3), which is the gate of the parity tests (G27).  Returns -1 on a bad argument (also an
+ * interchange out of range: ipiv[j] < j or >= M). */
+int oracle_dgetrf_residual(int64_t M, int64_t N, const double* A0, int64_t lda, const double* F, int64_t ldf, const int64_t* ipiv,
+                           int64_t nr, const int64_t* rows, int64_t nc, const int64_t* cols, double* res, double* den) {
+    if (M < 0 || N < 0 || nr < 0 || nc < 0) return -1;
+    if (nr == 0 || nc == 0) return 0;
+    if (!A0 || !F || !ipiv || !res || !den || lda < N || ldf < N) return -1;
+    const int64_t n = M < N ? M : N;
+    for (int64_t r = 0; r < nr; ++r) { int64_t i = rows ? rows[r] : r; if (i < 0 || i >= M) return -1; }
+    for (int64_t c = 0; c < nc; ++c) { int64_t j = cols ? cols[c] : c; if (j < 0 || j >= N) return -1; }
+    int64_t* perm = (int64_t*)malloc((size_t)M * sizeof(int64_t));      /* row i of P A0 is row perm[i] of A0 */
+    if (!perm) return -1;
+    for (int64_t i = 0; i < M; ++i) perm[i] = i;
+    for (int64_t j = 0; j < n; ++j) {
+        const int64_t p = ipiv[j];
+        if (p < j || p >= M) { free(perm); return -1; }
+        const int64_t t = perm[j]; perm[j] = perm[p]; perm[p] = t;
+    }
+    #pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t r = 0; r < nr; ++r) {
+        const int64_t i = rows ? rows[r] : r;
+        for (int64_t c = 0; c < nc; ++c) {
+            const int64_t j = cols ? cols[c] : c;
+            int64_t top = i < j ? i : j;
+            if (top > n - 1) top = n - 1;
+            long double s = (long double)A0[perm[i] * lda + j], d = 0.0L;
+            for (int64_t k = 0; k <= top; ++k) {
+                const long double l = k == i ? 1.0L : (long double)F[i * ldf + k];
+                const long double u = (long double)F[k * ldf + j];
+                s -= l * u;
+                d += fabsl(l) * fabsl(u);
+            }
+            res[r * nc + c] = (double)fabsl(s);
+            den[r * nc + c] = (double)d;
+        }
+    }
+    free(perm);
     return 0;
 }
