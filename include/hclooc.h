@@ -406,6 +406,38 @@ int hclooc_dpotrf(hclooc_ctx* ctx, int uplo, int64_t N, double* A, int64_t lda, 
  * Errors: -1 N < 1, -3 NULL output, HCLOOC_ERR_BUDGET.                                                                      */
 int hclooc_dpotrf_plan(int64_t N, size_t device_budget_bytes, int64_t* NB, uint64_t* panel_bytes);
 
+/* Out-of-core LU factorization with partial pivoting (the paper's future work: "out-of-core factorizations (LU, QR,
+ * Cholesky) that use the out-of-core matrix-matrix multiplication (DGEMM) as a fundamental building block", G27):
+ *     P * A = L * U
+ * A is M x N, row-major in PINNED HOST memory (lda >= N, in elements), overwritten in place by L (below the diagonal, unit diagonal
+ * not stored, |l_ij| <= 1) and U (on and above it) -- LAPACK DGETRF's result for the row-major matrix, L in the FINAL row order.
+ * ipiv: min(M, N) entries of HOST memory (pageable is fine), written: ipiv[j] = the row, 0-BASED (LAPACK: 1-based), exchanged with
+ * row j at step j; the pivot of a column is its entry of largest magnitude from the diagonal down, the FIRST one on ties.
+ * Left-looking over block columns of NB columns (hclooc_dgetrf_plan): a panel of all M rows stays in device memory while, for every
+ * block column before it, it takes that block's interchanges, a device DTRSM against the block's unit lower triangle and one
+ * out-of-core DGEMM (L streamed from the host, the panel in device memory); then its rows from the diagonal down are factored in
+ * device memory (recursive halving: tile-kernel DGEMMs and DTRSMs; at the bottom a cooperative multi-CTA kernel that keeps a
+ * 32-column panel in shared memory and pays one grid barrier per column).  The host matrix sees no row interchange until a final
+ * pass brings every block column of L into the final order.  Synchronous: returns with A and ipiv complete.
+ * *info (LAPACK): 0, or j+1 > 0 for the first pivot u_jj that is exactly zero (the factorization is completed all the same; U is
+ * singular).  The function still returns 0 then.  NaN in A: unspecified pivots.
+ * Rounding: |P A - L U| <= gamma_n |L||U| elementwise, n = min(M, N) (Gaussian elimination in any order of operations, Higham
+ * thm 9.3 / section 13.2); on data whose elimination is exact in FP64 the result is bit-identical to the unblocked definition.
+ * stats (nullable): sums over the DGEMM calls and the panel copies; plan.nb = NB, plan.flops = M N^2 - N^3/3 (M >= N).
+ * Errors: -2 M < 0 (or >= 2^31), -3 N, -4 A NULL, -5 lda < N, -6 ipiv NULL, -8 info NULL; HCLOOC_ERR_BUDGET when two 32-column
+ * panels and their scratch do not fit 5/8 of the budget; the HCLOOC_ERR_* codes of hclooc_dgemm.  Knob: HCLOOC_GETRF_NB=n.     */
+int hclooc_dgetrf(hclooc_ctx* ctx, int64_t M, int64_t N, double* A, int64_t lda, int64_t* ipiv, size_t device_budget_bytes,
+                  int64_t* info, hclooc_stats* stats_out);
+/* The panel width hclooc_dgetrf works with (pure host arithmetic) and the device bytes it keeps for itself (two panels, two
+ * diagonal blocks, scratch).  Errors: -1 M < 1, -2 N < 1, -4 NULL output, HCLOOC_ERR_BUDGET.                                 */
+int hclooc_dgetrf_plan(int64_t M, int64_t N, size_t device_budget_bytes, int64_t* NB, uint64_t* reserved_bytes);
+/* The device phase on its own: P A = L U of an M x N row-major matrix in DEVICE memory (16-byte aligned, lda even), in place, on
+ * stream s.  ipiv (min(M, N) entries) and info are HOST memory.  NOT asynchronous: the host folds each panel's interchanges into
+ * a permutation before the kernels that apply them are enqueued, so the call returns with the factorization complete; it
+ * allocates (and frees) its scratch -- at most 64 MiB + 2 MiB of device memory, 1 MiB + 8 min(M, N) bytes of pinned host memory.
+ * Errors: -1 M, -2 N, -3 dA NULL, -4 lda, -5 ipiv NULL, -6 info NULL; HCLOOC_ERR_ALIGN, HCLOOC_ERR_NOMEM, HCLOOC_ERR_CUDA.      */
+int hclDgetrf(int64_t M, int64_t N, double* dA, int64_t lda, int64_t* ipiv, int64_t* info, hclStream s);
+
 /* Out-of-core DTRMM and DSYMM (the paper's future work, :412: "full support for level-3 BLAS kernels"): the routines whose operand
  * is a TRIANGLE of a stored matrix.  The pipeline streams the stored matrix as it is and the tile kernel is told which part of
  * op(A) / op(B) counts: a tile runs only over the k blocks that can hold counted elements, and in the blocks that cross the

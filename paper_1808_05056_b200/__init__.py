@@ -8,7 +8,7 @@ the binding's functions raises.
 from ._binding import (  # noqa: F401
     HclError, lib, HostMatrix, Plan, ResidentPlan, Stats,
     hclooc_plan, hclooc_plan_ex, hclooc_plan_trans, hclooc_plan_resident, hclooc_resident_schedule, hclooc_shard_rows, hclooc_schedule, hclMatrixPartitioner,
-    hclooc_ctx_create, hclooc_ctx_destroy, hclooc_ctx_set_trace, hclooc_ctx_get_trace, hclooc_ctx_set_direct, hclooc_ctx_set_debug, hclooc_calibrate_link, TRACE_DTYPE, hclooc_dgemm, hclooc_dgemm_ex, hclooc_dgemm_t, hclooc_dsyrk, hclooc_dsyr2k, hclooc_dtrsm, hclooc_dtrsm_plan, hclooc_dtrsm_side, hclooc_dpotrf, hclooc_dpotrf_plan, hclooc_dtrmm, hclooc_dsymm, hclooc_dgemm_fig2, hclooc_dgemm_nsteps,
+    hclooc_ctx_create, hclooc_ctx_destroy, hclooc_ctx_set_trace, hclooc_ctx_get_trace, hclooc_ctx_set_direct, hclooc_ctx_set_debug, hclooc_calibrate_link, TRACE_DTYPE, hclooc_dgemm, hclooc_dgemm_ex, hclooc_dgemm_t, hclooc_dsyrk, hclooc_dsyr2k, hclooc_dtrsm, hclooc_dtrsm_plan, hclooc_dtrsm_side, hclooc_dpotrf, hclooc_dpotrf_plan, hclooc_dgetrf, hclooc_dgetrf_plan, hclDgetrf, hclooc_dtrmm, hclooc_dsymm, hclooc_dgemm_fig2, hclooc_dgemm_nsteps,
     hclMalloc, hclFree, hclGetMemSize, hclStreamCreate, hclStreamDestroy, hclEventDestroy,
     hclMemcpy, hclMemcpyAsync, hclMemcpy2DAsync, hclDgemmAsync, hclDgemmAsyncEx, hclDgemmAsyncT, hclDgemmNoAlloc, hclDgemmNoAllocScratchBytes, hclDtrsmAsync, hclDpotrfAsync, hclWaitEvent,
     hclStreamSynchronize, hclDeviceSynchronize,

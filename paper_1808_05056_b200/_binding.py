@@ -18,7 +18,7 @@ HCL_SIDE_LEFT, HCL_SIDE_RIGHT = 0, 1
 EXPORTS = [
     "hclooc_plan", "hclooc_plan_ex", "hclooc_plan_trans", "hclooc_plan_resident", "hclooc_resident_schedule", "hclooc_shard_rows", "hclMatrixPartitioner", "hclooc_schedule", "hclooc_ctx_create", "hclooc_ctx_destroy",
     "hclooc_ctx_set_trace", "hclooc_ctx_get_trace", "hclooc_ctx_set_direct", "hclooc_ctx_set_debug", "hclooc_calibrate_link",
-    "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_t", "hclooc_dsyrk", "hclooc_dsyr2k", "hclooc_dtrsm", "hclooc_dtrsm_plan", "hclooc_dtrsm_side", "hclooc_dpotrf", "hclooc_dpotrf_plan", "hclooc_dtrmm", "hclooc_dsymm", "hclooc_dgemm_fig2", "hclooc_dgemm_nsteps", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
+    "hclooc_dgemm", "hclooc_dgemm_ex", "hclooc_dgemm_t", "hclooc_dsyrk", "hclooc_dsyr2k", "hclooc_dtrsm", "hclooc_dtrsm_plan", "hclooc_dtrsm_side", "hclooc_dpotrf", "hclooc_dpotrf_plan", "hclooc_dgetrf", "hclooc_dgetrf_plan", "hclDgetrf", "hclooc_dtrmm", "hclooc_dsymm", "hclooc_dgemm_fig2", "hclooc_dgemm_nsteps", "hclMalloc", "hclFree", "hclGetMemSize", "hclStreamCreate",
     "hclStreamDestroy", "hclEventDestroy", "hclMemcpy", "hclMemcpyAsync", "hclMemcpy2DAsync",
     "hclDgemmAsync", "hclDgemmAsyncEx", "hclDgemmAsyncT", "hclDgemmNoAlloc", "hclDgemmNoAllocScratchBytes", "hclDtrsmAsync", "hclDpotrfAsync", "hclWaitEvent", "hclStreamSynchronize", "hclDeviceSynchronize",
     "hclooc_host_alloc", "hclooc_host_free", "hclooc_host_register", "hclooc_host_unregister",
@@ -109,6 +109,9 @@ def lib():
         L.hclooc_dsymm.argtypes = [vp, c_int, c_int, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
         L.hclooc_dpotrf.argtypes = [vp, c_int, i64, vp, i64, sz, POINTER(i64), POINTER(Stats)]
         L.hclooc_dpotrf_plan.argtypes = [i64, sz, POINTER(i64), POINTER(ctypes.c_uint64)]
+        L.hclooc_dgetrf.argtypes = [vp, i64, i64, vp, i64, vp, sz, POINTER(i64), POINTER(Stats)]
+        L.hclooc_dgetrf_plan.argtypes = [i64, i64, sz, POINTER(i64), POINTER(ctypes.c_uint64)]
+        L.hclDgetrf.argtypes = [i64, i64, vp, i64, vp, POINTER(i64), vp]
         L.hclooc_dsyr2k.argtypes = [vp, c_int, c_int, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
         L.hclooc_dgemm_nsteps.argtypes = [vp, i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, c_int, POINTER(c_int), POINTER(Stats)]
         L.hclooc_dgemm_fig2.argtypes = [i64, i64, i64, dbl, vp, i64, vp, i64, dbl, vp, i64, sz, POINTER(Stats)]
@@ -424,6 +427,31 @@ def hclooc_dpotrf_plan(N, device_budget_bytes):
     nb, pb = c_int64(), ctypes.c_uint64()
     _check(lib().hclooc_dpotrf_plan(N, device_budget_bytes, byref(nb), byref(pb)), "hclooc_dpotrf_plan")
     return int(nb.value), int(pb.value)
+
+
+def hclooc_dgetrf(ctx, M, N, A, lda, device_budget_bytes):
+    """Returns (ipiv, info, stats): ipiv = numpy int64 array of min(M, N) 0-based rows."""
+    import numpy as np
+    st, info = Stats(), c_int64(0)
+    ipiv = np.zeros(max(min(M, N), 1), dtype=np.int64)
+    _check(lib().hclooc_dgetrf(ctx, M, N, _ptr(A), lda, ipiv.ctypes.data, device_budget_bytes, byref(info), byref(st)), "hclooc_dgetrf")
+    return ipiv[:min(M, N)], int(info.value), st
+
+
+def hclooc_dgetrf_plan(M, N, device_budget_bytes):
+    """(NB, reserved_bytes)."""
+    nb, rb = c_int64(), ctypes.c_uint64()
+    _check(lib().hclooc_dgetrf_plan(M, N, device_budget_bytes, byref(nb), byref(rb)), "hclooc_dgetrf_plan")
+    return int(nb.value), int(rb.value)
+
+
+def hclDgetrf(M, N, dA, lda, stream=None):
+    """In-core LU of a device matrix; returns (ipiv, info).  Synchronous."""
+    import numpy as np
+    info = c_int64(0)
+    ipiv = np.zeros(max(min(M, N), 1), dtype=np.int64)
+    _check(lib().hclDgetrf(M, N, _ptr(dA), lda, ipiv.ctypes.data, byref(info), _ptr(stream)), "hclDgetrf")
+    return ipiv[:min(M, N)], int(info.value)
 
 
 def hclooc_dgemm_nsteps(ctx, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc, device_budget_bytes, nsteps, step):

@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhclooc_b200.so")
-SOURCES = ["dgemm_sm100.cu", "dgemm_streamk_sm100.cu", "dgemm_direct_sm100.cu", "trsm_sm100.cu", "potrf_sm100.cu", "factor.cu", "blas3_ooc.cu", "resident.cu", "executor.cu", "fig2_pipeline.cu", "runtime.cu", "planner.cpp"]
+SOURCES = ["dgemm_sm100.cu", "dgemm_streamk_sm100.cu", "dgemm_direct_sm100.cu", "trsm_sm100.cu", "potrf_sm100.cu", "getrf_sm100.cu", "factor.cu", "lu.cu", "blas3_ooc.cu", "resident.cu", "executor.cu", "fig2_pipeline.cu", "runtime.cu", "planner.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "-cudart", "static", "-diag-suppress", "177"]
 

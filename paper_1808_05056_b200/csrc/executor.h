@@ -117,4 +117,18 @@ int dgemm_resident(hclooc_ctx* ctx, const ResidentShape& S, int64_t M, int64_t N
 int dtrsm_left_lookahead(hclooc_ctx* ctx, int uplo, int trans, int diag, int64_t M, int64_t N, double alpha, const double* A, int64_t lda,
                          double* B, int64_t ldb, size_t budget, bool own, int64_t NB, hclooc_stats* stats);
 
+// X <- op(T)^-1 (scale X) (right = 0: X is n x w) / X <- (scale X) op(T)^-1 (right = 1: X is w x n) in device memory by recursive
+// halving (factor.cu dev_trsm); lower: op(T) is lower triangular; trans: op(T)[r][c] is stored at T[c][r]
+int dev_trsm_ctx(hclooc_ctx* dbg, int right, const double* dT, int64_t ldt, int lower, int trans, int unit, double* X, int64_t ld, int64_t w,
+                 int64_t n, double scale, cudaStream_t st, uint64_t* n_kernels);
+
+// the block kernels of the LU factorization (getrf_sm100.cu)
+size_t getrf_slot_bytes(int gcap);            // scratch of the panel kernel for launches of at most gcap CTAs; its first 8 bytes: the barrier counter
+int getrf_panel_shape(long long m, int* G_out, int* rpc_out);
+int launch_getrf_panel(double* dA, int64_t lda, int64_t m, int w, long long* ipiv_out, long long row_base, long long* d_info,
+                       long long info_base, void* slots, int gcap, unsigned long long* bar_base, cudaStream_t stream);
+int launch_row_permute(double* X, int64_t ld, int64_t ncols, int nt, const int* src, const int* dst, double* tmp, size_t tmp_elems,
+                       cudaStream_t stream, uint64_t* n_kernels);
+int launch_row_gather_all(const double* X, int64_t ldx, int64_t ncols, int64_t nrows, const int* perm, double* Y, int64_t ldy, cudaStream_t stream);
+
 }  // namespace hclooc

@@ -710,6 +710,13 @@ extern "C" int hclooc_dtrsm_side(hclooc_ctx* ctx, int side, int uplo, int trans,
 // (one GPU-filling launch; only the NB x NB block of T crosses the link).  ctx->mu is held by the caller for the whole solve.
 namespace hclooc {
 
+// the device triangular solve for the other routines built on it (lu.cu); dbg: the context whose debug shaker applies (nullable)
+int dev_trsm_ctx(hclooc_ctx* dbg, int right, const double* dT, int64_t ldt, int lower, int trans, int unit, double* X, int64_t ld, int64_t w,
+                 int64_t n, double scale, cudaStream_t st, uint64_t* n_kernels) {
+    DbgScope scope(dbg);
+    return dev_trsm(right, dT, ldt, lower, trans, unit, X, ld, w, n, scale, st, n_kernels);
+}
+
 int dtrsm_left_lookahead(hclooc_ctx* ctx, int uplo, int trans, int diag, int64_t M, int64_t N, double alpha, const double* A, int64_t lda,
                          double* B, int64_t ldb, size_t budget, bool own, int64_t NB, hclooc_stats* stats) {
     const auto t_begin = std::chrono::steady_clock::now();

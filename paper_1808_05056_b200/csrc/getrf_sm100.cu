@@ -1,0 +1,285 @@
+// getrf_sm100.cu -- the block kernels of the LU factorization with partial pivoting (hclooc_dgetrf / hclDgetrf; PAPER.md:412
+// names LU first among the out-of-core factorizations to be built on the DGEMM):
+//
+//   getrf_panel_kernel   factors ONE tall panel of m rows and w <= 32 columns that sits in device memory.  The flops of an LU
+//                        factorization are DGEMM / DTRSM work on the tile kernel; what is left at the bottom of the recursion is
+//                        this: per column a pivot search over ALL remaining rows, one row interchange, a division per row and a
+//                        rank-1 update of at most 31 columns -- latency, not arithmetic.  So the panel is spread over up to one
+//                        CTA per SM (cooperative launch): every CTA keeps its slab of rows in SHARED MEMORY for the whole panel
+//                        (one read and one write of the panel in HBM), and a column costs ONE grid-wide barrier: before it every
+//                        CTA publishes its best candidate (|value|, row, and the row's contents) and CTA 0 publishes row j; after
+//                        it every CTA picks the same winner (largest |value|, smallest row on ties: the FIRST maximum, as IDAMAX
+//                        and the oracle), the two CTAs that own row j and the pivot row exchange them from the published copies,
+//                        and everybody eliminates in its own slab.
+//   row_gather_kernel /  a sequence of row interchanges applied to OTHER columns as one permutation: the host folds the sequence
+//   row_scatter_kernel   into (destination <- source) pairs; the rows are gathered into a scratch buffer and scattered back --
+//                        two fully parallel passes instead of thousands of dependent row swaps.
+#include <cooperative_groups.h>
+#include "internal.h"
+
+namespace hclooc {
+namespace {
+
+constexpr int LU_T = 256;           // threads per CTA
+constexpr int LU_W = 32;            // widest panel
+constexpr int LU_MAXG = 192;        // most CTAs of a panel launch (>= SMs of the device, checked at launch)
+
+__device__ __forceinline__ double lu_shfl_down(double v, int off) {
+    int lo = __double2loint(v), hi = __double2hiint(v);
+    lo = __shfl_down_sync(0xffffffffu, lo, off);
+    hi = __shfl_down_sync(0xffffffffu, hi, off);
+    return __hiloint2double(hi, lo);
+}
+
+__device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// candidate order: larger |value| first, smaller row on ties
+__device__ __forceinline__ bool lu_better(double v, int r, double bv, int br) { return v > bv || (v == bv && r < br); }
+
+struct PanelSlots {                 // global scratch of one panel launch, one set per column (no reuse inside a launch)
+    double* cval;                   // [LU_W][G]          best |a_ij| of CTA g in column j (-1: no row of it is still in play)
+    int* crow;                      // [LU_W][G]          its row (panel-local)
+    double* ccont;                  // [LU_W][G][LU_W]    that row's contents
+    double* top;                    // [LU_W][LU_W]       row j before the interchange of column j
+    unsigned long long* counter;    // arrivals at the grid barrier, monotone across launches (bar_base = its value at launch)
+};
+
+__global__ void __launch_bounds__(LU_T, 1)
+getrf_panel_kernel(double* __restrict__ A, long long lda, long long m, int w, int rpc, int G, long long* __restrict__ ipiv_out,
+                   long long row_base, long long* __restrict__ info, long long info_base, PanelSlots sl, unsigned long long bar_base) {
+    extern __shared__ __align__(16) double S[];     // S[r * SW + c]: this CTA's rows, odd stride (column access hits 32 banks)
+    __shared__ double red_v[LU_T / 32];
+    __shared__ int red_r[LU_T / 32];
+    __shared__ double P_s[LU_W], T_s[LU_W];         // the pivot row / row j as published
+    __shared__ int win_cta, win_row;
+    const int g = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const long long r0 = (long long)g * rpc;
+    const int nloc = (int)(m - r0 < (long long)rpc ? m - r0 : (long long)rpc);
+    const int SW = w | 1;
+    for (int r = warp; r < nloc; r += LU_T / 32)
+        if (lane < w) S[r * SW + lane] = A[(r0 + r) * lda + lane];
+    __syncthreads();
+    const int nsteps = (int)(m < (long long)w ? m : (long long)w);
+    for (int j = 0; j < nsteps; ++j) {
+        // ---- this CTA's candidate for the pivot of column j
+        double best = -1.0;
+        int brow = 0x7fffffff;
+        for (int r = tid; r < nloc; r += LU_T) {
+            if (r0 + r >= j) {
+                const double v = fabs(S[r * SW + j]);
+                if (v > best) { best = v; brow = (int)(r0 + r); }
+            }
+        }
+#pragma unroll
+        for (int off = 16; off; off >>= 1) {
+            const double ov = lu_shfl_down(best, off);
+            const int orow = __shfl_down_sync(0xffffffffu, brow, off);
+            if (lu_better(ov, orow, best, brow)) { best = ov; brow = orow; }
+        }
+        if (lane == 0) { red_v[warp] = best; red_r[warp] = brow; }
+        __syncthreads();
+        if (tid == 0) {
+            for (int k = 1; k < LU_T / 32; ++k)
+                if (lu_better(red_v[k], red_r[k], best, brow)) { best = red_v[k]; brow = red_r[k]; }
+            red_v[0] = best; red_r[0] = brow;
+        }
+        __syncthreads();
+        best = red_v[0]; brow = red_r[0];
+        const size_t slot = (size_t)j * G + g;
+        if (tid == 0) { sl.cval[slot] = best; sl.crow[slot] = brow; }
+        if (tid < w && best >= 0.0) sl.ccont[slot * LU_W + tid] = S[(size_t)(brow - r0) * SW + tid];
+        if (g == 0 && tid >= 32 && tid < 32 + w) sl.top[j * LU_W + tid - 32] = S[j * SW + tid - 32];
+        // ---- the grid barrier of column j
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) {
+            atomicAdd(sl.counter, 1ULL);
+            const unsigned long long target = bar_base + (unsigned long long)G * (unsigned long long)(j + 1);
+            while (ld_acquire_u64(sl.counter) < target) { }
+        }
+        __syncthreads();
+        // ---- the same winner in every CTA
+        if (warp == 0) {
+            double bv = -2.0;
+            int br = 0x7fffffff, bc = -1;
+            for (int c = lane; c < G; c += 32) {
+                const double v = __ldcg(&sl.cval[(size_t)j * G + c]);
+                const int r = __ldcg(&sl.crow[(size_t)j * G + c]);
+                if (lu_better(v, r, bv, br)) { bv = v; br = r; bc = c; }
+            }
+#pragma unroll
+            for (int off = 16; off; off >>= 1) {
+                const double ov = lu_shfl_down(bv, off);
+                const int orow = __shfl_down_sync(0xffffffffu, br, off);
+                const int oc = __shfl_down_sync(0xffffffffu, bc, off);
+                if (lu_better(ov, orow, bv, br)) { bv = ov; br = orow; bc = oc; }
+            }
+            if (lane == 0) {
+                if (!(bv >= 0.0)) { br = j; bc = -1; }      // nothing comparable in the column (NaN): no interchange
+                win_cta = bc; win_row = br;
+            }
+        }
+        __syncthreads();
+        const int wc = win_cta, pr = win_row;
+        if (tid < w) P_s[tid] = wc < 0 ? __ldcg(&sl.top[j * LU_W + tid]) : __ldcg(&sl.ccont[((size_t)j * G + wc) * LU_W + tid]);
+        else if (tid >= 32 && tid < 32 + w) T_s[tid - 32] = __ldcg(&sl.top[j * LU_W + tid - 32]);
+        __syncthreads();
+        const double pivot = P_s[j];
+        if (pr != j) {                               // rows j and pr change places, each owner taking the other's published copy
+            if (g == wc && tid < w) S[(size_t)(pr - r0) * SW + tid] = T_s[tid];
+            if (g == 0 && tid >= 32 && tid < 32 + w) S[j * SW + tid - 32] = P_s[tid - 32];
+        }
+        if (g == 0 && tid == 0) {
+            ipiv_out[j] = row_base + pr;
+            if (pivot == 0.0) atomicCAS((unsigned long long*)info, 0ULL, (unsigned long long)(info_base + j + 1));
+        }
+        __syncthreads();
+        if (pivot != 0.0) {                          // a zero pivot: the column is zero from row j down, nothing to eliminate
+            for (int r = tid; r < nloc; r += LU_T)
+                if (r0 + r > j) S[r * SW + j] = S[r * SW + j] / pivot;            // IEEE division, as the definition
+            __syncthreads();
+            if (lane > j && lane < w) {
+                const double pc = P_s[lane];
+                for (int r = warp; r < nloc; r += LU_T / 32)
+                    if (r0 + r > j) S[r * SW + lane] = __dsub_rn(S[r * SW + lane], __dmul_rn(S[r * SW + j], pc));
+            }
+        }
+        __syncthreads();
+    }
+    for (int r = warp; r < nloc; r += LU_T / 32)
+        if (lane < w) A[(r0 + r) * lda + lane] = S[r * SW + lane];
+}
+
+// rows on grid.x (as many as a permutation touches), 256 columns per CTA on grid.y
+__global__ void __launch_bounds__(256)
+row_gather_kernel(const double* __restrict__ X, long long ld, int ncols, const int* __restrict__ src, double* __restrict__ tmp, long long ldt) {
+    __shared__ int s;
+    if (threadIdx.x == 0) s = src[blockIdx.x];
+    __syncthreads();
+    const int c = blockIdx.y * 256 + threadIdx.x;
+    if (c < ncols) tmp[(long long)blockIdx.x * ldt + c] = X[(long long)s * ld + c];
+}
+
+__global__ void __launch_bounds__(256)
+row_scatter_kernel(double* __restrict__ X, long long ld, int ncols, const int* __restrict__ dst, const double* __restrict__ tmp, long long ldt) {
+    __shared__ int d;
+    if (threadIdx.x == 0) d = dst[blockIdx.x];
+    __syncthreads();
+    const int c = blockIdx.y * 256 + threadIdx.x;
+    if (c < ncols) X[(long long)d * ld + c] = tmp[(long long)blockIdx.x * ldt + c];
+}
+
+}  // namespace
+
+// device scratch of the panel kernel for launches of at most gcap CTAs: [counter 64 B][top][cval][ccont][crow]
+size_t getrf_slot_bytes(int gcap) {
+    return 64 + (size_t)LU_W * LU_W * 8 + (size_t)LU_W * gcap * 8 + (size_t)LU_W * gcap * LU_W * 8 + (size_t)LU_W * gcap * 4 + 64;
+}
+
+// Panel width the kernel can take for m rows on this device (32, or less when a CTA's slab of a very tall panel would not fit
+// its shared memory), the CTAs it will use and their rows; 0 if even 8 columns do not fit.
+int getrf_panel_shape(long long m, int* G_out, int* rpc_out) {
+    static int sms = 0, smem_max = 0, coop = 0;
+    if (!sms) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    }
+    const int maxg = sms < LU_MAXG ? sms : LU_MAXG;
+    const size_t avail = (size_t)smem_max - 4096;                 // static shared memory and the runtime's share
+    for (int w = LU_W; w >= 8; w >>= 1) {
+        long long G = (m + 127) / 128;
+        if (G > maxg) G = maxg;
+        if (G < 1) G = 1;
+        if (!coop) G = 1;
+        long long rpc = (m + G - 1) / G;
+        if (rpc < w) rpc = w;                                      // CTA 0 owns every row that can become row j
+        G = (m + rpc - 1) / rpc;
+        if ((size_t)rpc * (w | 1) * 8 <= avail) { *G_out = (int)G; *rpc_out = (int)rpc; return w; }
+    }
+    return 0;
+}
+
+// Factor the m x w panel at dA (device, row-major, leading dimension lda) in place; pivot rows (panel-local + row_base) go to
+// ipiv_out[0 .. min(m, w)) -- memory the device can write, e.g. pinned host memory; *d_info (device) receives
+// info_base + j + 1 for the first exactly-zero pivot if it was 0.  `slots`: getrf_slot_bytes(gcap) of device scratch whose barrier
+// counter (its first 8 bytes) holds *bar_base on entry; *bar_base is advanced by the arrivals of this launch.
+int launch_getrf_panel(double* dA, int64_t lda, int64_t m, int w, long long* ipiv_out, long long row_base, long long* d_info,
+                       long long info_base, void* slots, int gcap, unsigned long long* bar_base, cudaStream_t stream) {
+    if (m <= 0 || w <= 0) return HCLOOC_OK;
+    int G = 0, rpc = 0;
+    const int wmax = getrf_panel_shape(m, &G, &rpc);
+    if (w > wmax || G > gcap) return HCLOOC_ERR_INTERNAL;
+    static bool attr_set = false;
+    static int smem_max = 0;
+    if (!attr_set) {
+        int dev = 0;
+        HCL_CUDA(cudaGetDevice(&dev));
+        HCL_CUDA(cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+        HCL_CUDA(cudaFuncSetAttribute(getrf_panel_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max - 4096));
+        attr_set = true;
+    }
+    // with fewer columns than the shape was made for, the rows per CTA stay (they fit a fortiori); rpc >= w holds
+    PanelSlots sl;
+    uint8_t* p = (uint8_t*)slots;
+    sl.counter = (unsigned long long*)p;  p += 64;
+    sl.top = (double*)p;                  p += (size_t)LU_W * LU_W * 8;
+    sl.cval = (double*)p;                 p += (size_t)LU_W * gcap * 8;
+    sl.ccont = (double*)p;                p += (size_t)LU_W * gcap * LU_W * 8;
+    sl.crow = (int*)p;
+    long long lda_ll = lda, m_ll = m;
+    unsigned long long base = *bar_base;
+    const size_t smem = (size_t)rpc * (w | 1) * 8;
+    void* args[] = {&dA, &lda_ll, &m_ll, &w, &rpc, &G, &ipiv_out, &row_base, &d_info, &info_base, &sl, &base};
+    if (G > 1) HCL_CUDA(cudaLaunchCooperativeKernel((const void*)getrf_panel_kernel, dim3(G), dim3(LU_T), args, smem, stream));
+    else HCL_CUDA(cudaLaunchKernel((const void*)getrf_panel_kernel, dim3(1), dim3(LU_T), args, smem, stream));
+    *bar_base = base + (unsigned long long)G * (unsigned long long)(m < w ? m : w);
+    return HCLOOC_OK;
+}
+
+// X[dst[i]][c] <- X[src[i]][c] for i < nt, c < ncols, all sources read before any destination is written: gathered into tmp
+// (at least nt * min(ncols, tmp_elems / nt) doubles, in column chunks), then scattered.  src / dst: memory the device can read.
+int launch_row_permute(double* X, int64_t ld, int64_t ncols, int nt, const int* src, const int* dst, double* tmp, size_t tmp_elems,
+                       cudaStream_t stream, uint64_t* n_kernels) {
+    if (nt <= 0 || ncols <= 0) return HCLOOC_OK;
+    int64_t chunk = (int64_t)(tmp_elems / (size_t)nt) / 32 * 32;
+    if (chunk < 32) return HCLOOC_ERR_BUDGET;
+    if (chunk > ncols) chunk = ncols;
+    for (int64_t c0 = 0; c0 < ncols; c0 += chunk) {
+        const int nc = (int)(ncols - c0 < chunk ? ncols - c0 : chunk);
+        const dim3 grid((unsigned)nt, (unsigned)((nc + 255) / 256));
+        row_gather_kernel<<<grid, 256, 0, stream>>>(X + c0, ld, nc, src, tmp, chunk);
+        row_scatter_kernel<<<grid, 256, 0, stream>>>(X + c0, ld, nc, dst, tmp, chunk);
+        *n_kernels += 2;
+    }
+    HCL_CUDA(cudaGetLastError());
+    return HCLOOC_OK;
+}
+
+// Y[i][c] <- X[perm[i]][c] for i < nrows (out of place; the final pass of hclooc_dgetrf)
+namespace {
+__global__ void __launch_bounds__(256)
+row_gather_all_kernel(const double* __restrict__ X, long long ldx, int ncols, const int* __restrict__ perm, double* __restrict__ Y, long long ldy) {
+    __shared__ int s;
+    if (threadIdx.x == 0) s = perm[blockIdx.x];
+    __syncthreads();
+    const int c = blockIdx.y * 256 + threadIdx.x;
+    if (c < ncols) Y[(long long)blockIdx.x * ldy + c] = X[(long long)s * ldx + c];
+}
+}  // namespace
+
+int launch_row_gather_all(const double* X, int64_t ldx, int64_t ncols, int64_t nrows, const int* perm, double* Y, int64_t ldy, cudaStream_t stream) {
+    if (nrows <= 0 || ncols <= 0) return HCLOOC_OK;
+    const dim3 grid((unsigned)nrows, (unsigned)((ncols + 255) / 256));
+    row_gather_all_kernel<<<grid, 256, 0, stream>>>(X, ldx, (int)ncols, perm, Y, ldy);
+    HCL_CUDA(cudaGetLastError());
+    return HCLOOC_OK;
+}
+
+}  // namespace hclooc
