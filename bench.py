@@ -672,7 +672,7 @@ def run_op(args):
         LINK.update(live)
     op, M, N, K, budget = args.op, args.m, args.n, args.k, args.budget
     seed = synthgen.BASE_SEED + 9
-    if op in ("dtrsm_dev", "dtrsm_right_dev", "dpotrf_dev"):
+    if op in ("dtrsm_dev", "dtrsm_right_dev", "dpotrf_dev", "dgetrf_dev"):
         return run_dev_op(args, H, torch)
     ctx = H.hclooc_ctx_create(0)
     mats = []
@@ -725,6 +725,23 @@ def run_op(args):
             infos.append(info)
             return st
         shape = {"N": N}
+        extra["info"] = infos
+    elif op == "dgetrf":
+        # a general matrix: uniform[-1,1) entries (partial pivoting does the rest); the factorization overwrites its input, which is
+        # restored from a copy before every call (outside the timed span: t_total_s is the wall time inside the call)
+        A = host(M, N, "A")
+        A0 = H.HostMatrix(M, N)
+        mats.append(A0)
+        A0.view[...] = A.view
+        flops = float(M) * N * N - float(N) ** 3 / 3.0 if M >= N else float(N) * M * M - float(M) ** 3 / 3.0
+        infos = []
+
+        def call():
+            A.view[...] = A0.view
+            ipiv, info, st = H.hclooc_dgetrf(ctx, M, N, A, A.ld, budget)
+            infos.append(info)
+            return st
+        shape = {"M": M, "N": N}
         extra["info"] = infos
     else:
         raise SystemExit(f"unknown --op {op}")
@@ -842,7 +859,7 @@ def run_dev_op(args, H, torch):
     cur = torch.cuda.current_stream()
     g = torch.Generator(device="cuda"); g.manual_seed(180805056)
     n = M if op == "dtrsm_dev" else N
-    T = torch.rand((n, n), generator=g, dtype=torch.float64, device="cuda") / n + torch.eye(n, dtype=torch.float64, device="cuda") * 1.5
+    T = None if op == "dgetrf_dev" else torch.rand((n, n), generator=g, dtype=torch.float64, device="cuda") / n + torch.eye(n, dtype=torch.float64, device="cuda") * 1.5
     if op == "dpotrf_dev":
         S = (T + T.T) / 2 + torch.eye(n, dtype=torch.float64, device="cuda")
         W = S.clone()
@@ -850,6 +867,13 @@ def run_dev_op(args, H, torch):
         fn = lambda: H.hclDpotrfAsync(args.uplo, n, W, n, info, cur)
         pre = lambda: W.copy_(S)
         flops, shape = n ** 3 / 3.0, {"N": n}
+    elif op == "dgetrf_dev":
+        S = torch.rand((M, N), generator=g, dtype=torch.float64, device="cuda") * 2 - 1
+        W = S.clone()
+        fn = lambda: H.hclDgetrf(M, N, W, N, cur)           # synchronous: the host folds the interchanges (include/hclooc.h)
+        pre = lambda: W.copy_(S)
+        flops = float(M) * N * N - float(N) ** 3 / 3.0 if M >= N else float(N) * M * M - float(M) ** 3 / 3.0
+        shape = {"M": M, "N": N}
     else:
         Bm = torch.rand((M, N), generator=g, dtype=torch.float64, device="cuda")
         side = 0 if op == "dtrsm_dev" else 1
@@ -865,7 +889,7 @@ def run_dev_op(args, H, torch):
         if it >= 3:
             ts.append(e0.elapsed_time(e1))
     ms = float(np.median(ts))
-    print(json.dumps({"op": "hcl" + {"dtrsm_dev": "DtrsmAsync (Left)", "dtrsm_right_dev": "DtrsmAsync (Right)", "dpotrf_dev": "DpotrfAsync"}[op], **shape,
+    print(json.dumps({"op": "hcl" + {"dtrsm_dev": "DtrsmAsync (Left)", "dtrsm_right_dev": "DtrsmAsync (Right)", "dpotrf_dev": "DpotrfAsync", "dgetrf_dev": "Dgetrf"}[op], **shape,
                       "uplo": args.uplo, "trans": args.trans, "ms": ms, "tflops": flops / ms / 1e9, "frac_of_fp64_peak": flops / ms / 1e9 / FP64_PEAK_TFLOPS}))
 
 
@@ -967,7 +991,7 @@ def main():
     ap.add_argument("--trans", default="NN", choices=["NN", "TN", "NT", "TT"],
                     help="e2e leg through hclooc_dgemm_t with op(A), op(B) transposed (the same buffers read as the stored K x M / N x K matrices)")
     ap.add_argument("--kernel-only", action="store_true", help="only the kernel legs (for ncu captures of the tile kernel)")
-    ap.add_argument("--op", default="dgemm", choices=["dgemm", "dsyrk", "dsyr2k", "dtrsm", "dtrsm_right", "dpotrf", "dtrsm_dev", "dtrsm_right_dev", "dpotrf_dev", "cublasxt"],
+    ap.add_argument("--op", default="dgemm", choices=["dgemm", "dsyrk", "dsyr2k", "dtrsm", "dtrsm_right", "dpotrf", "dgetrf", "dtrsm_dev", "dtrsm_right_dev", "dpotrf_dev", "dgetrf_dev", "cublasxt"],
                     help="time another routine of the library instead (sizes from --m/--n/--k/--budget; --steps calls, the first discarded)")
     ap.add_argument("--xt-block", type=int, default=8192, help="--op cublasxt: cublasXtSetBlockDim (the side reference's tile size)")
     ap.add_argument("--sweep", default="", choices=["", "transition"], help="transition: the paper's N sweep across the in-core / out-of-core point")

@@ -22,6 +22,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <thread>
 #include <unordered_map>
 #include <vector>
 #include "executor.h"
@@ -158,7 +159,7 @@ int lu_shape(int64_t M, int64_t N, size_t budget, LuShape* out) {
         s->t_bytes = s->npan == 1 ? 0 : round_1k((size_t)s->NB * s->ldt * 8);
         s->tmp_bytes = round_1k(std::min(LU_TMP_MAX, (size_t)2 * s->NB * std::max<int64_t>(s->NB, 32) * 8));
         s->slot_bytes = round_1k(getrf_slot_bytes(gcap));
-        s->reserved = s->npan * s->panel_bytes + 2 * s->t_bytes + s->tmp_bytes + s->slot_bytes + 1024;
+        s->reserved = s->npan * s->panel_bytes + 2 * s->t_bytes + 2 * s->tmp_bytes + s->slot_bytes + 1024;
         return s->reserved <= budget / 8 * 5;
     };
     int64_t NB = nb_env ? nb_env : 4096;
@@ -277,41 +278,55 @@ extern "C" int hclooc_dgetrf(hclooc_ctx* ctx, int64_t M, int64_t N, double* A, i
     double* dT[2];
     dT[0] = (double*)q; q += S.t_bytes;
     dT[1] = (double*)q; q += S.t_bytes;
-    LuState L;
+    // L: the state of this thread's stream (interchanges, DTRSMs, the update from the freshest block); W: the worker's, which
+    // factors a panel on a stream of its own while this thread drives the next panel's out-of-core updates through the pipeline
+    LuState L, W;
     L.ctx = ctx;
     L.tmp = (double*)q; L.tmp_elems = S.tmp_bytes / 8; q += S.tmp_bytes;
-    L.slots = q; q += S.slot_bytes;
-    L.d_info = (long long*)q;
+    W.tmp = (double*)q; W.tmp_elems = S.tmp_bytes / 8; q += S.tmp_bytes;
+    W.slots = q; q += S.slot_bytes;
+    L.d_info = W.d_info = (long long*)q;
     struct Reserve {
         hclooc_ctx* c;
         Reserve(hclooc_ctx* cc, size_t bytes) : c(cc) { c->reserved_bytes = bytes; }
         ~Reserve() { c->reserved_bytes = 0; }
     } guard(ctx, S.reserved + shift);
     int G, rpc;
-    L.bw = getrf_panel_shape(M, &G, &rpc);
+    W.bw = L.bw = getrf_panel_shape(M, &G, &rpc);
     if (L.bw < 8) return HCLOOC_ERR_BUDGET;
-    L.gcap = (int)std::min<int64_t>((M + 127) / 128, 192);
-    if (G > L.gcap) return HCLOOC_ERR_INTERNAL;
+    W.gcap = (int)std::min<int64_t>((M + 127) / 128, 192);
+    if (G > W.gcap) return HCLOOC_ERR_INTERNAL;
     PinnedBuf hp, ha, hperm;
-    if ((rc = hp.alloc((size_t)n * 8 + 64)) || (rc = ha.alloc(LU_ARENA_INTS * 4)) || (rc = hperm.alloc((size_t)M * 4 * 2))) return rc;
-    L.h_ipiv = (long long*)hp.p;
+    if ((rc = hp.alloc((size_t)n * 8 + 64)) || (rc = ha.alloc(2 * LU_ARENA_INTS * 4)) || (rc = hperm.alloc((size_t)M * 4 * 2))) return rc;
+    L.h_ipiv = W.h_ipiv = (long long*)hp.p;
     L.arena = (int*)ha.p; L.arena_ints = LU_ARENA_INTS;
+    W.arena = (int*)ha.p + LU_ARENA_INTS; W.arena_ints = LU_ARENA_INTS;
     cudaStream_t st = ctx->s_aux[0], s_up = ctx->s_aux[1], s_down = ctx->s_aux[2], s_T = ctx->s_aux[3];
     L.st = st;
+    struct OwnStream {
+        cudaStream_t s = nullptr;
+        ~OwnStream() { if (s) { cudaStreamSynchronize(s); cudaStreamDestroy(s); } }
+    } fact_stream;
+    HCL_CUDA(cudaStreamCreateWithFlags(&fact_stream.s, cudaStreamNonBlocking));
+    cudaStream_t s_fact = fact_stream.s;
+    W.st = s_fact;
+    // the worker's share of the debug shaker: a context of its own for the random delays (the generator is not thread-safe)
+    hclooc_ctx shadow;
+    shadow.dbg_rng = ctx->dbg_rng ? ctx->dbg_rng * 0x9E3779B97F4A7C15ull + 1 : 0;
+    shadow.dbg_poison = ctx->dbg_poison;
+    W.ctx = &shadow;
     cudaEvent_t ev_up[2] = {ctx->ev_aux[0], ctx->ev_aux[1]}, ev_down[2] = {ctx->ev_aux[2], ctx->ev_aux[3]};
     cudaEvent_t ev_T[2] = {ctx->ev_aux[4], ctx->ev_aux[5]}, ev_Tfree[2] = {ctx->ev_aux[6], ctx->ev_aux[7]};
     EventSet extra;
-    if ((rc = extra.make(4))) return rc;
-    cudaEvent_t ev_fact = extra.ev[0], ev_g = extra.ev[1], ev_u = extra.ev[2], ev_d = extra.ev[3];
-    struct Drain {      // whatever happens, nothing of this call is left running when it returns
-        hclooc_ctx* c;
-        ~Drain() { for (cudaStream_t s : c->s_aux) if (s) cudaStreamSynchronize(s); }
-    } drain{ctx};
+    if ((rc = extra.make(5))) return rc;
+    cudaEvent_t ev_fresh = extra.ev[0], ev_g = extra.ev[1], ev_u = extra.ev[2], ev_d = extra.ev[3], ev_fact = extra.ev[4];
     static const bool timing = std::getenv("HCLOOC_FACTOR_TIMING") != nullptr;
-    HCL_CUDA(cudaMemsetAsync(L.slots, 0, 64, st));
+    static const bool lookahead = [] { const char* e = std::getenv("HCLOOC_GETRF_LOOKAHEAD"); return !e || std::atoi(e) != 0; }();
+    HCL_CUDA(cudaMemsetAsync(W.slots, 0, 64, st));
     HCL_CUDA(cudaMemsetAsync(L.d_info, 0, 8, st));
-    hclooc_stats acc;
+    hclooc_stats acc, wacc;                                   // wacc: what the worker counts (merged after it has been joined)
     std::memset(&acc, 0, sizeof(acc));
+    std::memset(&wacc, 0, sizeof(wacc));
     double t_enq = 0.0;
     size_t ws_max = S.reserved;
     bool down_pending[2] = {false, false}, tfree_recorded[2] = {false, false};
@@ -327,12 +342,10 @@ extern "C" int hclooc_dgetrf(hclooc_ctx* ctx, int64_t M, int64_t N, double* A, i
         HCL_CUDA(cudaEventRecord(ev_up[buf], s_up));
         return HCLOOC_OK;
     };
-    // L_kk (pk x pk, unit lower) of pivot block k comes up into dT[k & 1]; `freshest`: block k was factored as the previous panel
-    // and must have reached the host first
-    auto upload_T = [&](int64_t k, int64_t bj) -> int {
+    // L_kk (pk x pk, unit lower) of pivot block k comes up from the host into dT[k & 1]
+    auto upload_T = [&](int64_t k) -> int {
         const int64_t c0k = k * NB, pk = std::min(NB, n - c0k);
         const int b = (int)(k & 1);
-        if (k == bj - 1 && down_pending[(int)(k % S.npan)]) HCL_CUDA(cudaEventSynchronize(ev_down[(int)(k % S.npan)]));
         if (tfree_recorded[b]) HCL_CUDA(cudaStreamWaitEvent(s_T, ev_Tfree[b], 0));
         debug_jitter(ctx, s_T);
         int e = copy2d(dT[b], (size_t)ldt * 8, A + c0k * lda + c0k, (size_t)lda * 8, (size_t)pk * 8, (size_t)pk, s_T);
@@ -341,61 +354,118 @@ extern "C" int hclooc_dgetrf(hclooc_ctx* ctx, int64_t M, int64_t N, double* A, i
         HCL_CUDA(cudaEventRecord(ev_T[b], s_T));
         return HCLOOC_OK;
     };
+    // the worker's job: the rows of panel bj from its diagonal down are factored on s_fact (which has been told to wait for the
+    // panel's last update), and the finished panel goes down at once
+    std::chrono::steady_clock::time_point w_t0, w_t1;
+    auto factor_panel = [&](int64_t bj, int buf) -> int {
+        w_t0 = std::chrono::steady_clock::now();
+        if (cudaSetDevice(ctx->device) != cudaSuccess) return HCLOOC_ERR_CUDA;
+        const int64_t c0 = bj * NB, nbj = width(bj);
+        int e = HCLOOC_OK;
+        if (c0 < n) e = dev_getrf(W, dPan[buf] + c0 * ldp, ldp, M - c0, nbj, c0, c0);
+        if (e) return e;
+        HCL_CUDA(cudaEventRecord(ev_fact, s_fact));
+        HCL_CUDA(cudaStreamWaitEvent(s_down, ev_fact, 0));
+        debug_jitter(W.ctx, s_down);
+        if ((e = copy2d(A + c0, (size_t)lda * 8, dPan[buf], (size_t)ldp * 8, (size_t)nbj * 8, (size_t)M, s_down))) return e;
+        wacc.bytes_d2h += (uint64_t)M * nbj * 8; ++wacc.n_copies_d2h;
+        HCL_CUDA(cudaEventRecord(ev_down[buf], s_down));
+        e = lu_sync(W);                                          // the interchanges of the panel are on the host
+        w_t1 = std::chrono::steady_clock::now();
+        return e;
+    };
+    struct Worker {
+        std::thread th;
+        int rc = HCLOOC_OK;
+        bool active = false;
+        int join() { if (active) { th.join(); active = false; } return rc; }
+        ~Worker() { join(); }
+    } worker;
+    struct Drain {      // whatever happens, nothing of this call is left running when it returns (declared after the worker: runs first... the
+        hclooc_ctx* c;  // worker's destructor joins before the streams are drained because it is destroyed later -- so join explicitly)
+        Worker* w;
+        ~Drain() { w->join(); for (cudaStream_t s : c->s_aux) if (s) cudaStreamSynchronize(s); }
+    } drain{ctx, &worker};
     if ((rc = upload(0, 0))) return rc;
     for (int64_t bj = 0; bj < npanels; ++bj) {
         const int cur = (int)(bj % S.npan), alt = S.npan - 1 - cur;
-        const int64_t c0 = bj * NB, nbj = width(bj);
+        const int64_t nbj = width(bj);
         double* dP = dPan[cur];
         const auto tp0 = std::chrono::steady_clock::now();
-        if (bj + 1 < npanels && (rc = upload(bj + 1, alt))) return rc;          // the next panel comes up beside everything below
+        // ---- panel bj-1 is factored, its interchanges are known and its download has been enqueued
+        if ((rc = worker.join())) return rc;
+        if (bj >= 1) down_pending[alt] = true;
+        if (timing && bj >= 1) std::fprintf(stderr, "dgetrf panel %lld: factorization %.2f ms (worker)\n", (long long)(bj - 1), 1e3 * std::chrono::duration<double>(w_t1 - w_t0).count());
         HCL_CUDA(cudaStreamWaitEvent(st, ev_up[cur], 0));
-        const int64_t nk = std::min(bj, npiv);
-        if (nk > 0 && (rc = upload_T(0, bj))) return rc;
-        for (int64_t k = 0; k < nk; ++k) {
-            const int64_t c0k = k * NB, pk = std::min(NB, n - c0k), r1 = c0k + pk;
-            const int b = (int)(k & 1);
-            // (1) the interchanges of block k, over all rows from c0k down
+        // ---- the update from the FRESHEST block (k = bj-1) comes straight from device memory: panel bj-1 still sits in the other
+        // buffer, so neither its download nor the link is waited for
+        if (bj >= 1 && bj - 1 < npiv) {
+            const int64_t k = bj - 1, c0k = k * NB, pk = std::min(NB, n - c0k), r1 = c0k + pk;
+            const double* Lk = dPan[alt] + c0k * ldp;                                // rows c0k.. of panel k: L_kk, then L[r1:M, block k]
             if ((rc = lu_permute(L, dP, ldp, nbj, c0k, c0k + pk, 0))) return rc;
-            // (2) block row k of the panel:  U_kj <- L_kk^-1 P_k
-            HCL_CUDA(cudaStreamWaitEvent(st, ev_T[b], 0));
-            if ((rc = dev_trsm_ctx(ctx, 0, dT[b], ldt, 1, 0, 1, dP + c0k * ldp, ldp, nbj, pk, 1.0, st, &L.n_kernels))) return rc;
-            HCL_CUDA(cudaEventRecord(ev_Tfree[b], st));
-            tfree_recorded[b] = true;
-            if (k + 1 < nk && (rc = upload_T(k + 1, bj))) return rc;
-            // (3) the rows below:  P[r1:M] <- P[r1:M] - L[r1:M, block k] U_kj, L streamed from the host by the pipeline
+            if ((rc = dev_trsm_ctx(ctx, 0, Lk, ldp, 1, 0, 1, dP + c0k * ldp, ldp, nbj, pk, 1.0, st, &L.n_kernels))) return rc;
             if (M > r1) {
-                if ((rc = lu_sync(L))) return rc;
-                hclooc_stats one;
-                rc = dgemm_core_locked(ctx, 0, 0, M - r1, nbj, pk, -1.0, A + r1 * lda + c0k, lda, dP + c0k * ldp, ldp, 1.0, dP + r1 * ldp, ldp, budget, &one);
-                if (rc) return rc;
-                acc.bytes_h2d += one.bytes_h2d; acc.bytes_d2h += one.bytes_d2h; acc.n_kernels += one.n_kernels;
-                acc.n_copies_h2d += one.n_copies_h2d; acc.n_copies_d2h += one.n_copies_d2h; t_enq += one.t_enqueue_s;
-                ws_max = std::max(ws_max, S.reserved + (size_t)one.plan.workspace_bytes);
-                if (timing) std::fprintf(stderr, "  dgetrf panel %lld, block %lld: update %lld x %lld x %lld %.2f ms (%.1f TFLOP/s), %lld x %lld blocks of %lld x %lld\n",
-                                         (long long)bj, (long long)k, (long long)(M - r1), (long long)nbj, (long long)pk, 1e3 * one.t_total_s,
-                                         2e-12 * (double)(M - r1) * nbj * pk / one.t_total_s, (long long)one.plan.h, (long long)one.plan.w, (long long)one.plan.mb, (long long)one.plan.nb);
+                debug_jitter(ctx, st);
+                if ((rc = launch_dgemm_tiles(M - r1, nbj, pk, -1.0, Lk + pk * ldp, ldp, dP + c0k * ldp, ldp, 1.0, dP + r1 * ldp, ldp, st, -1))) return rc;            // (the GPU is this launch's: the worker has been joined, the pipeline is idle)
+                ++L.n_kernels;
             }
         }
+        HCL_CUDA(cudaEventRecord(ev_fresh, st));
         const auto tp1 = std::chrono::steady_clock::now();
-        // ---- the panel's own rows: factored in device memory
-        if (c0 < n && (rc = dev_getrf(L, dP + c0 * ldp, ldp, M - c0, nbj, c0, c0))) return rc;
-        HCL_CUDA(cudaEventRecord(ev_fact, st));
-        HCL_CUDA(cudaStreamWaitEvent(s_down, ev_fact, 0));
-        debug_jitter(ctx, s_down);
-        if ((rc = copy2d(A + c0, (size_t)lda * 8, dP, (size_t)ldp * 8, (size_t)nbj * 8, (size_t)M, s_down))) return rc;
-        acc.bytes_d2h += (uint64_t)M * nbj * 8; ++acc.n_copies_d2h;
-        HCL_CUDA(cudaEventRecord(ev_down[cur], s_down));
-        down_pending[cur] = true;
-        if (timing) {
-            if ((rc = lu_sync(L))) return rc;
-            const auto tp2 = std::chrono::steady_clock::now();
-            std::fprintf(stderr, "dgetrf panel %lld (%lld columns): %lld updates %.2f ms, factorization of %lld rows %.2f ms\n", (long long)bj, (long long)nbj,
-                         (long long)nk, 1e3 * std::chrono::duration<double>(tp1 - tp0).count(), (long long)std::max<int64_t>(M - c0, 0),
-                         1e3 * std::chrono::duration<double>(tp2 - tp1).count());
+        // ---- panel bj is factored by the worker ...
+        HCL_CUDA(cudaStreamWaitEvent(s_fact, ev_fresh, 0));
+        worker.rc = HCLOOC_OK;
+        if (lookahead) {
+            worker.active = true;
+            worker.th = std::thread([&worker, &factor_panel, bj, cur] { worker.rc = factor_panel(bj, cur); });
+        } else if ((rc = factor_panel(bj, cur))) return rc;
+        // ---- ... while panel bj+1 comes up and receives the updates of the blocks BEFORE bj through the pipeline (L from the host)
+        if (bj + 1 < npanels) {
+            HCL_CUDA(cudaStreamWaitEvent(s_up, ev_fresh, 0));                        // the freshest update has read the buffer's previous tenant
+            if ((rc = upload(bj + 1, alt))) return rc;
+            HCL_CUDA(cudaStreamWaitEvent(st, ev_up[alt], 0));
+            double* dQ = dPan[alt];
+            const int64_t nbn = width(bj + 1);
+            const int64_t nk = std::min(bj, npiv);
+            if (nk > 0) {
+                if (down_pending[alt]) HCL_CUDA(cudaEventSynchronize(ev_down[alt]));  // block bj-1 is on the host: the pipeline reads L there
+                if ((rc = upload_T(0))) return rc;
+            }
+            for (int64_t k = 0; k < nk; ++k) {
+                const int64_t c0k = k * NB, pk = std::min(NB, n - c0k), r1 = c0k + pk;
+                const int b = (int)(k & 1);
+                // (1) the interchanges of block k, over all rows from c0k down
+                if ((rc = lu_permute(L, dQ, ldp, nbn, c0k, c0k + pk, 0))) return rc;
+                // (2) block row k of the panel:  U_kj <- L_kk^-1 P_k
+                HCL_CUDA(cudaStreamWaitEvent(st, ev_T[b], 0));
+                if ((rc = dev_trsm_ctx(ctx, 0, dT[b], ldt, 1, 0, 1, dQ + c0k * ldp, ldp, nbn, pk, 1.0, st, &L.n_kernels))) return rc;
+                HCL_CUDA(cudaEventRecord(ev_Tfree[b], st));
+                tfree_recorded[b] = true;
+                if (k + 1 < nk && (rc = upload_T(k + 1))) return rc;
+                // (3) the rows below:  P[r1:M] <- P[r1:M] - L[r1:M, block k] U_kj, L streamed from the host by the pipeline
+                if (M > r1) {
+                    if ((rc = lu_sync(L))) return rc;
+                    hclooc_stats one;
+                    rc = dgemm_core_locked(ctx, 0, 0, M - r1, nbn, pk, -1.0, A + r1 * lda + c0k, lda, dQ + c0k * ldp, ldp, 1.0, dQ + r1 * ldp, ldp, budget, &one);
+                    if (rc) return rc;
+                    acc.bytes_h2d += one.bytes_h2d; acc.bytes_d2h += one.bytes_d2h; acc.n_kernels += one.n_kernels;
+                    acc.n_copies_h2d += one.n_copies_h2d; acc.n_copies_d2h += one.n_copies_d2h; t_enq += one.t_enqueue_s;
+                    ws_max = std::max(ws_max, S.reserved + (size_t)one.plan.workspace_bytes);
+                    if (timing) std::fprintf(stderr, "  dgetrf panel %lld, block %lld: update %lld x %lld x %lld %.2f ms (%.1f TFLOP/s), %lld x %lld blocks of %lld x %lld\n",
+                                             (long long)(bj + 1), (long long)k, (long long)(M - r1), (long long)nbn, (long long)pk, 1e3 * one.t_total_s,
+                                             2e-12 * (double)(M - r1) * nbn * pk / one.t_total_s, (long long)one.plan.h, (long long)one.plan.w, (long long)one.plan.mb, (long long)one.plan.nb);
+                }
+            }
         }
+        if (timing) std::fprintf(stderr, "dgetrf iteration %lld: freshest update enqueued in %.2f ms, look-ahead updates of panel %lld %.2f ms\n", (long long)bj,
+                                 1e3 * std::chrono::duration<double>(tp1 - tp0).count(), (long long)(bj + 1),
+                                 1e3 * std::chrono::duration<double>(std::chrono::steady_clock::now() - tp1).count());
     }
+    if ((rc = worker.join())) return rc;
     if ((rc = lu_sync(L))) return rc;
     HCL_CUDA(cudaStreamSynchronize(s_down));
+    acc.bytes_d2h += wacc.bytes_d2h; acc.n_copies_d2h += wacc.n_copies_d2h;
+    L.n_kernels += W.n_kernels;
     // ---- final pass: block column k of L, rows below its diagonal block, into the final row order (the interchanges of the
     // blocks after it); X = dPan[0], Y = dPan[1]; upload k+1 runs beside download k
     const auto tf0 = std::chrono::steady_clock::now();
