@@ -14,7 +14,8 @@
 //   row_gather_kernel /  a sequence of row interchanges applied to OTHER columns as one permutation: the host folds the sequence
 //   row_scatter_kernel   into (destination <- source) pairs; the rows are gathered into a scratch buffer and scattered back --
 //                        two fully parallel passes instead of thousands of dependent row swaps.
-#include <cooperative_groups.h>
+#include <algorithm>
+#include <cstdlib>
 #include "internal.h"
 
 namespace hclooc {
@@ -191,7 +192,8 @@ int getrf_panel_shape(long long m, int* G_out, int* rpc_out) {
         cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     }
-    const int maxg = sms < LU_MAXG ? sms : LU_MAXG;
+    static const int g_env = [] { const char* e = getenv("HCLOOC_GETRF_MAXG"); const int v = e ? atoi(e) : 0; return v > 0 ? v : LU_MAXG; }();   // experiment knob
+    const int maxg = std::min(sms < LU_MAXG ? sms : LU_MAXG, g_env);
     const size_t avail = (size_t)smem_max - 4096;                 // static shared memory and the runtime's share
     for (int w = LU_W; w >= 8; w >>= 1) {
         long long G = (m + 127) / 128;

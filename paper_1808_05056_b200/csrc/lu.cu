@@ -151,16 +151,25 @@ struct LuShape { int64_t NB, ldp, ldt; int npan; size_t panel_bytes, t_bytes, tm
 int lu_shape(int64_t M, int64_t N, size_t budget, LuShape* out) {
     const int gcap = (int)std::min<int64_t>((M + 127) / 128, 192);            // at most one CTA per 128 rows (getrf_panel_shape)
     static const int64_t nb_env = [] { const char* e = std::getenv("HCLOOC_GETRF_NB"); const long v = e ? std::atol(e) : 0; return v >= 32 ? (int64_t)(v / 32 * 32) : (int64_t)0; }();
+    const int npan_env = [] { const char* e = std::getenv("HCLOOC_GETRF_PANELS"); const int v = e ? std::atoi(e) : 0; return v == 2 || v == 3 ? v : 0; }();   // knob, read at every call
+    // three resident panels where they fit 7/8 of the budget (the pipeline works in what is left: its buffers for K = NB are a few
+    // hundred MiB at most): the panel after next is then uploaded a whole iteration ahead; else two in 5/8 (its upload follows the
+    // freshest update range by range); one if a single panel covers the matrix
     auto shape = [&](int64_t nb, LuShape* s) {
         s->NB = std::min(nb, N);
-        s->npan = s->NB >= N ? 1 : 2;
         s->ldp = round_even(s->NB); s->ldt = s->ldp;
         s->panel_bytes = round_1k((size_t)M * s->ldp * 8);
-        s->t_bytes = s->npan == 1 ? 0 : round_1k((size_t)s->NB * s->ldt * 8);
         s->tmp_bytes = round_1k(std::min(LU_TMP_MAX, (size_t)2 * s->NB * std::max<int64_t>(s->NB, 32) * 8));
         s->slot_bytes = round_1k(getrf_slot_bytes(gcap));
-        s->reserved = s->npan * s->panel_bytes + 2 * s->t_bytes + 2 * s->tmp_bytes + s->slot_bytes + 1024;
-        return s->reserved <= budget / 8 * 5;
+        const int64_t npanels = (N + s->NB - 1) / s->NB;
+        for (int np = npanels >= 3 ? 3 : (int)npanels; np >= (npanels >= 2 ? 2 : 1); --np) {
+            if (npan_env && np > npan_env) continue;
+            s->npan = np;
+            s->t_bytes = np == 1 ? 0 : round_1k((size_t)s->NB * s->ldt * 8);
+            s->reserved = np * s->panel_bytes + 2 * s->t_bytes + 2 * s->tmp_bytes + s->slot_bytes + 1024;
+            if (s->reserved <= budget / 8 * (np == 3 ? 7 : 5)) return true;
+        }
+        return false;
     };
     int64_t NB = nb_env ? nb_env : 4096;
     LuShape s;
@@ -272,9 +281,8 @@ extern "C" int hclooc_dgetrf(hclooc_ctx* ctx, int64_t M, int64_t N, double* A, i
     const size_t shift = mis ? 1024 - mis : 0;
     if (S.reserved + shift > ctx->workspace_bytes) return HCLOOC_ERR_BUDGET;
     uint8_t* q = base + shift;
-    double* dPan[2];
-    dPan[0] = (double*)q; q += S.panel_bytes;
-    dPan[1] = S.npan == 2 ? (double*)q : dPan[0]; q += (S.npan - 1) * S.panel_bytes;
+    double* dPan[3];
+    for (int i = 0; i < 3; ++i) { dPan[i] = i < S.npan ? (double*)q : dPan[0]; if (i < S.npan) q += S.panel_bytes; }
     double* dT[2];
     dT[0] = (double*)q; q += S.t_bytes;
     dT[1] = (double*)q; q += S.t_bytes;
@@ -301,25 +309,37 @@ extern "C" int hclooc_dgetrf(hclooc_ctx* ctx, int64_t M, int64_t N, double* A, i
     L.h_ipiv = W.h_ipiv = (long long*)hp.p;
     L.arena = (int*)ha.p; L.arena_ints = LU_ARENA_INTS;
     W.arena = (int*)ha.p + LU_ARENA_INTS; W.arena_ints = LU_ARENA_INTS;
-    cudaStream_t st = ctx->s_aux[0], s_up = ctx->s_aux[1], s_down = ctx->s_aux[2], s_T = ctx->s_aux[3];
+    // streams of this call: four for this thread's device work (interchanges, DTRSMs in column chunks, the freshest update) at a
+    // priority between the pipeline's (highest) and the worker's factorization (lowest), so that the latency-bound solves on the
+    // critical path are scheduled ahead of the factorization that runs beside them; copies go on the context's streams
+    cudaStream_t s_up = ctx->s_aux[1], s_down = ctx->s_aux[2], s_T = ctx->s_aux[3];
+    struct OwnStreams {
+        cudaStream_t s[5] = {};
+        ~OwnStreams() { for (cudaStream_t x : s) if (x) { cudaStreamSynchronize(x); cudaStreamDestroy(x); } }
+    } streams;
+    {
+        int prio_lo = 0, prio_hi = 0;
+        HCL_CUDA(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));
+        static const int wp = [] { const char* e = std::getenv("HCLOOC_GETRF_WORKER_PRIO"); return e ? std::atoi(e) : 2; }();   // experiment knob: 0 lowest, 1 middle, 2 highest (measured best: 1.24 s against 1.27-1.28 s)
+        static const int mp = [] { const char* e = std::getenv("HCLOOC_GETRF_MAIN_PRIO"); return e ? std::atoi(e) : 1; }();
+        const int pr[3] = {prio_lo, (prio_lo + prio_hi) / 2, prio_hi};
+        for (int i = 0; i < 5; ++i) HCL_CUDA(cudaStreamCreateWithPriority(&streams.s[i], cudaStreamNonBlocking, i < 4 ? pr[mp] : pr[wp]));
+    }
+    cudaStream_t st = streams.s[0], s_fact = streams.s[4];
     L.st = st;
-    struct OwnStream {
-        cudaStream_t s = nullptr;
-        ~OwnStream() { if (s) { cudaStreamSynchronize(s); cudaStreamDestroy(s); } }
-    } fact_stream;
-    HCL_CUDA(cudaStreamCreateWithFlags(&fact_stream.s, cudaStreamNonBlocking));
-    cudaStream_t s_fact = fact_stream.s;
     W.st = s_fact;
     // the worker's share of the debug shaker: a context of its own for the random delays (the generator is not thread-safe)
     hclooc_ctx shadow;
     shadow.dbg_rng = ctx->dbg_rng ? ctx->dbg_rng * 0x9E3779B97F4A7C15ull + 1 : 0;
     shadow.dbg_poison = ctx->dbg_poison;
     W.ctx = &shadow;
-    cudaEvent_t ev_up[2] = {ctx->ev_aux[0], ctx->ev_aux[1]}, ev_down[2] = {ctx->ev_aux[2], ctx->ev_aux[3]};
     cudaEvent_t ev_T[2] = {ctx->ev_aux[4], ctx->ev_aux[5]}, ev_Tfree[2] = {ctx->ev_aux[6], ctx->ev_aux[7]};
     EventSet extra;
-    if ((rc = extra.make(5))) return rc;
+    if ((rc = extra.make(22))) return rc;
+    cudaEvent_t ev_up[3] = {extra.ev[16], extra.ev[17], extra.ev[18]}, ev_down[3] = {extra.ev[19], extra.ev[20], extra.ev[21]};
     cudaEvent_t ev_fresh = extra.ev[0], ev_g = extra.ev[1], ev_u = extra.ev[2], ev_d = extra.ev[3], ev_fact = extra.ev[4];
+    cudaEvent_t ev_s0 = extra.ev[5], ev_sol[3] = {extra.ev[6], extra.ev[7], extra.ev[8]}, ev_ftrsm = extra.ev[9];
+    cudaEvent_t ev_fchunk[6] = {extra.ev[10], extra.ev[11], extra.ev[12], extra.ev[13], extra.ev[14], extra.ev[15]};
     static const bool timing = std::getenv("HCLOOC_FACTOR_TIMING") != nullptr;
     static const bool lookahead = [] { const char* e = std::getenv("HCLOOC_GETRF_LOOKAHEAD"); return !e || std::atoi(e) != 0; }();
     HCL_CUDA(cudaMemsetAsync(W.slots, 0, 64, st));
@@ -329,17 +349,43 @@ extern "C" int hclooc_dgetrf(hclooc_ctx* ctx, int64_t M, int64_t N, double* A, i
     std::memset(&wacc, 0, sizeof(wacc));
     double t_enq = 0.0;
     size_t ws_max = S.reserved;
-    bool down_pending[2] = {false, false}, tfree_recorded[2] = {false, false};
+    bool down_pending[3] = {false, false, false}, tfree_recorded[2] = {false, false};
     auto width = [&](int64_t bj) { return std::min(NB, N - bj * NB); };
-    auto upload = [&](int64_t bj, int buf) -> int {
+    // rows [r_lo, r_hi) of panel bj come up into dPan[buf] on s_up, after `after` (nullable: nothing more to wait for)
+    auto upload_rows = [&](int64_t bj, int buf, int64_t r_lo, int64_t r_hi, cudaEvent_t after) -> int {
+        if (r_hi <= r_lo) return HCLOOC_OK;
         const int64_t c0 = bj * NB, nbj = width(bj);
-        if (down_pending[buf]) HCL_CUDA(cudaStreamWaitEvent(s_up, ev_down[buf], 0));      // the buffer's previous tenant has gone down
+        if (after) HCL_CUDA(cudaStreamWaitEvent(s_up, after, 0));
         debug_jitter(ctx, s_up);
-        debug_poison(ctx, dPan[buf], ldp, M, nbj, s_up);
-        int e = copy2d(dPan[buf], (size_t)ldp * 8, A + c0, (size_t)lda * 8, (size_t)nbj * 8, (size_t)M, s_up);
+        debug_poison(ctx, dPan[buf] + r_lo * ldp, ldp, r_hi - r_lo, nbj, s_up);
+        int e = copy2d(dPan[buf] + r_lo * ldp, (size_t)ldp * 8, A + r_lo * lda + c0, (size_t)lda * 8, (size_t)nbj * 8, (size_t)(r_hi - r_lo), s_up);
         if (e) return e;
-        acc.bytes_h2d += (uint64_t)M * nbj * 8; ++acc.n_copies_h2d;
+        acc.bytes_h2d += (uint64_t)(r_hi - r_lo) * nbj * 8; ++acc.n_copies_h2d;
+        return HCLOOC_OK;
+    };
+    auto upload = [&](int64_t bj, int buf) -> int {
+        if (down_pending[buf]) HCL_CUDA(cudaStreamWaitEvent(s_up, ev_down[buf], 0));      // the buffer's previous tenant has gone down
+        int e = upload_rows(bj, buf, 0, M, nullptr);
+        if (e) return e;
         HCL_CUDA(cudaEventRecord(ev_up[buf], s_up));
+        return HCLOOC_OK;
+    };
+    // X (pk x ncols, leading dimension ldp) <- T^-1 X, T unit lower: the columns in up to four chunks on as many streams (one
+    // chunk's recursion is a chain of small launches that leaves most SMs idle); everything is ordered after and before `st`
+    auto solve_chunks = [&](const double* T, int64_t ldT, double* X, int64_t ncols, int64_t pk) -> int {
+        const int nch = ncols >= 2048 ? 4 : (ncols >= 1024 ? 2 : 1);
+        if (nch == 1) return dev_trsm_ctx(ctx, 0, T, ldT, 1, 0, 1, X, ldp, ncols, pk, 1.0, st, &L.n_kernels);
+        const int64_t wc = ((ncols + nch - 1) / nch + 127) / 128 * 128;
+        HCL_CUDA(cudaEventRecord(ev_s0, st));
+        int c = 0;
+        for (int64_t x0 = 0; x0 < ncols; x0 += wc, ++c) {
+            cudaStream_t sc = streams.s[c];
+            if (c) HCL_CUDA(cudaStreamWaitEvent(sc, ev_s0, 0));
+            int e = dev_trsm_ctx(ctx, 0, T, ldT, 1, 0, 1, X + x0, ldp, std::min(wc, ncols - x0), pk, 1.0, sc, &L.n_kernels);
+            if (e) return e;
+            if (c) HCL_CUDA(cudaEventRecord(ev_sol[c - 1], sc));
+        }
+        for (int i = 1; i < c; ++i) HCL_CUDA(cudaStreamWaitEvent(st, ev_sol[i - 1], 0));
         return HCLOOC_OK;
     };
     // L_kk (pk x pk, unit lower) of pivot block k comes up from the host into dT[k & 1]
@@ -386,9 +432,12 @@ extern "C" int hclooc_dgetrf(hclooc_ctx* ctx, int64_t M, int64_t N, double* A, i
         Worker* w;
         ~Drain() { w->join(); for (cudaStream_t s : c->s_aux) if (s) cudaStreamSynchronize(s); }
     } drain{ctx, &worker};
-    if ((rc = upload(0, 0))) return rc;
+    for (int64_t b0 = 0; b0 < std::min<int64_t>(std::max(S.npan - 1, 1), npanels); ++b0)
+        if ((rc = upload(b0, (int)b0))) return rc;
     for (int64_t bj = 0; bj < npanels; ++bj) {
-        const int cur = (int)(bj % S.npan), alt = S.npan - 1 - cur;
+        // panel bj sits in buffer cur, panel bj-1 in alt, panel bj+1 goes to (or is in) nxt; `take` is the panel that takes over alt
+        const int cur = (int)(bj % S.npan), alt = (int)((bj + S.npan - 1) % S.npan), nxt = (int)((bj + 1) % S.npan);
+        const int64_t take = bj + std::max(S.npan - 1, 1);
         const int64_t nbj = width(bj);
         double* dP = dPan[cur];
         const auto tp0 = std::chrono::steady_clock::now();
@@ -399,16 +448,39 @@ extern "C" int hclooc_dgetrf(hclooc_ctx* ctx, int64_t M, int64_t N, double* A, i
         HCL_CUDA(cudaStreamWaitEvent(st, ev_up[cur], 0));
         // ---- the update from the FRESHEST block (k = bj-1) comes straight from device memory: panel bj-1 still sits in the other
         // buffer, so neither its download nor the link is waited for
+        // (the next panel comes up into that buffer range by range, each as soon as this update has read it: its top rows -- the U
+        // part of panel bj-1 -- at once, the diagonal block after the DTRSM, the rest behind the row chunks of the product)
+        const bool next = S.npan >= 2 && take < npanels;
+        bool next_up = false;
         if (bj >= 1 && bj - 1 < npiv) {
             const int64_t k = bj - 1, c0k = k * NB, pk = std::min(NB, n - c0k), r1 = c0k + pk;
             const double* Lk = dPan[alt] + c0k * ldp;                                // rows c0k.. of panel k: L_kk, then L[r1:M, block k]
-            if ((rc = lu_permute(L, dP, ldp, nbj, c0k, c0k + pk, 0))) return rc;
-            if ((rc = dev_trsm_ctx(ctx, 0, Lk, ldp, 1, 0, 1, dP + c0k * ldp, ldp, nbj, pk, 1.0, st, &L.n_kernels))) return rc;
-            if (M > r1) {
-                debug_jitter(ctx, st);
-                if ((rc = launch_dgemm_tiles(M - r1, nbj, pk, -1.0, Lk + pk * ldp, ldp, dP + c0k * ldp, ldp, 1.0, dP + r1 * ldp, ldp, st, -1))) return rc;            // (the GPU is this launch's: the worker has been joined, the pipeline is idle)
-                ++L.n_kernels;
+            if (next) {
+                if (down_pending[alt]) HCL_CUDA(cudaStreamWaitEvent(s_up, ev_down[alt], 0));
+                if ((rc = upload_rows(take, alt, 0, c0k, nullptr))) return rc;
             }
+            if ((rc = lu_permute(L, dP, ldp, nbj, c0k, c0k + pk, 0))) return rc;
+            if ((rc = solve_chunks(Lk, ldp, dP + c0k * ldp, nbj, pk))) return rc;
+            HCL_CUDA(cudaEventRecord(ev_ftrsm, st));
+            if (next && (rc = upload_rows(take, alt, c0k, r1, ev_ftrsm))) return rc;
+            if (M > r1) {
+                // (the GPU is these launches': the worker has been joined, the pipeline is idle)
+                const int64_t rows = M - r1;
+                const int nch = rows >= 16384 ? 6 : (rows >= 4096 ? 4 : 1);
+                const int64_t hc = ((rows + nch - 1) / nch + 127) / 128 * 128;
+                int c = 0;
+                for (int64_t x0 = 0; x0 < rows; x0 += hc, ++c) {
+                    const int64_t hh = std::min(hc, rows - x0);
+                    debug_jitter(ctx, st);
+                    if ((rc = launch_dgemm_tiles(hh, nbj, pk, -1.0, Lk + (pk + x0) * ldp, ldp, dP + c0k * ldp, ldp, 1.0, dP + (r1 + x0) * ldp, ldp, st, -1))) return rc;
+                    ++L.n_kernels;
+                    if (next) {
+                        HCL_CUDA(cudaEventRecord(ev_fchunk[c], st));
+                        if ((rc = upload_rows(take, alt, r1 + x0, r1 + x0 + hh, ev_fchunk[c]))) return rc;
+                    }
+                }
+            }
+            if (next) { HCL_CUDA(cudaEventRecord(ev_up[alt], s_up)); next_up = true; }
         }
         HCL_CUDA(cudaEventRecord(ev_fresh, st));
         const auto tp1 = std::chrono::steady_clock::now();
@@ -420,31 +492,44 @@ extern "C" int hclooc_dgetrf(hclooc_ctx* ctx, int64_t M, int64_t N, double* A, i
             worker.th = std::thread([&worker, &factor_panel, bj, cur] { worker.rc = factor_panel(bj, cur); });
         } else if ((rc = factor_panel(bj, cur))) return rc;
         // ---- ... while panel bj+1 comes up and receives the updates of the blocks BEFORE bj through the pipeline (L from the host)
+        if (next && !next_up) {
+            HCL_CUDA(cudaStreamWaitEvent(s_up, ev_fresh, 0));                        // nothing of this call still reads the buffer's previous tenant
+            if ((rc = upload(take, alt))) return rc;
+        }
         if (bj + 1 < npanels) {
-            HCL_CUDA(cudaStreamWaitEvent(s_up, ev_fresh, 0));                        // the freshest update has read the buffer's previous tenant
-            if ((rc = upload(bj + 1, alt))) return rc;
-            HCL_CUDA(cudaStreamWaitEvent(st, ev_up[alt], 0));
-            double* dQ = dPan[alt];
+            HCL_CUDA(cudaStreamWaitEvent(st, ev_up[nxt], 0));
+            if (timing) {
+                HCL_CUDA(cudaEventSynchronize(ev_up[nxt]));
+                std::fprintf(stderr, "  dgetrf panel %lld is up %.2f ms after the freshest update of panel %lld was enqueued\n", (long long)(bj + 1),
+                             1e3 * std::chrono::duration<double>(std::chrono::steady_clock::now() - tp1).count(), (long long)bj);
+            }
+            double* dQ = dPan[nxt];
             const int64_t nbn = width(bj + 1);
             const int64_t nk = std::min(bj, npiv);
-            if (nk > 0) {
-                if (down_pending[alt]) HCL_CUDA(cudaEventSynchronize(ev_down[alt]));  // block bj-1 is on the host: the pipeline reads L there
-                if ((rc = upload_T(0))) return rc;
-            }
+            // block bj-1 must be on the HOST before the pipeline (and the upload of its diagonal block) reads L there: its download
+            // was enqueued when its factorization ended, moments ago -- waited for as late as possible
+            auto host_has = [&](int64_t k) -> int {
+                if (k == bj - 1 && down_pending[alt]) HCL_CUDA(cudaEventSynchronize(ev_down[alt]));
+                return HCLOOC_OK;
+            };
+            if (nk > 0 && ((rc = host_has(0)) || (rc = upload_T(0)))) return rc;
             for (int64_t k = 0; k < nk; ++k) {
                 const int64_t c0k = k * NB, pk = std::min(NB, n - c0k), r1 = c0k + pk;
                 const int b = (int)(k & 1);
+                const auto ts0 = std::chrono::steady_clock::now();
                 // (1) the interchanges of block k, over all rows from c0k down
                 if ((rc = lu_permute(L, dQ, ldp, nbn, c0k, c0k + pk, 0))) return rc;
                 // (2) block row k of the panel:  U_kj <- L_kk^-1 P_k
                 HCL_CUDA(cudaStreamWaitEvent(st, ev_T[b], 0));
-                if ((rc = dev_trsm_ctx(ctx, 0, dT[b], ldt, 1, 0, 1, dQ + c0k * ldp, ldp, nbn, pk, 1.0, st, &L.n_kernels))) return rc;
+                if ((rc = solve_chunks(dT[b], ldt, dQ + c0k * ldp, nbn, pk))) return rc;
                 HCL_CUDA(cudaEventRecord(ev_Tfree[b], st));
                 tfree_recorded[b] = true;
-                if (k + 1 < nk && (rc = upload_T(k + 1))) return rc;
+                if (k + 1 < nk && ((rc = host_has(k + 1)) || (rc = upload_T(k + 1)))) return rc;
                 // (3) the rows below:  P[r1:M] <- P[r1:M] - L[r1:M, block k] U_kj, L streamed from the host by the pipeline
                 if (M > r1) {
                     if ((rc = lu_sync(L))) return rc;
+                    if (timing) std::fprintf(stderr, "  dgetrf panel %lld, block %lld: interchanges + DTRSM %.2f ms\n", (long long)(bj + 1), (long long)k,
+                                             1e3 * std::chrono::duration<double>(std::chrono::steady_clock::now() - ts0).count());
                     hclooc_stats one;
                     rc = dgemm_core_locked(ctx, 0, 0, M - r1, nbn, pk, -1.0, A + r1 * lda + c0k, lda, dQ + c0k * ldp, ldp, 1.0, dQ + r1 * ldp, ldp, budget, &one);
                     if (rc) return rc;
@@ -469,7 +554,7 @@ extern "C" int hclooc_dgetrf(hclooc_ctx* ctx, int64_t M, int64_t N, double* A, i
     // ---- final pass: block column k of L, rows below its diagonal block, into the final row order (the interchanges of the
     // blocks after it); X = dPan[0], Y = dPan[1]; upload k+1 runs beside download k
     const auto tf0 = std::chrono::steady_clock::now();
-    if (S.npan == 2) {
+    if (S.npan >= 2) {
         int* perm[2] = {(int*)hperm.p, (int*)hperm.p + M};
         bool first = true;
         int which = 0;

@@ -183,6 +183,26 @@ def test_dgetrf_large(H, dist):
         check_float(M, N, A0, got, ipiv, info, full_oracle=False)
 
 
+@pytest.mark.parametrize("panels", [2, 3])
+def test_dgetrf_two_and_three_resident_panels(H, panels, monkeypatch):
+    """HCLOOC_GETRF_PANELS caps the resident panels: with two, the next panel's upload follows the freshest update range by range
+    into the buffer that update is still reading; with three it goes a whole iteration ahead.  Same bits either way."""
+    monkeypatch.setenv("HCLOOC_GETRF_PANELS", str(panels))
+    M, N = 2300, 2100
+    vals, F_want, ipiv_want = exact_lu_case(M, N, 4242)
+    ctx = H.hclooc_ctx_create()
+    try:
+        for seed in (0, 5):
+            A = host_matrix(H, vals, 2)
+            H.hclooc_ctx_set_debug(ctx, seed, 1 if seed else 0)
+            ipiv, info, st = H.hclooc_dgetrf(ctx, M, N, A, A.ld, 24 * MiB)
+            assert st.plan.n_sets == panels and st.plan.n_steps >= 4
+            assert info == 0 and np.array_equal(ipiv, ipiv_want) and np.array_equal(A.view, F_want)
+    finally:
+        H.hclooc_ctx_set_debug(ctx, 0, 0)
+        H.hclooc_ctx_destroy(ctx)
+
+
 def test_dgetrf_under_the_debug_shaker(H):
     """Random delays in front of every copy and kernel, NaN in buffers the schedule declares free: an exact case must stay exact."""
     M, N = 1300, 1200
