@@ -13,7 +13,7 @@
  * Conventions for every function
  *   - Storage is ROW-MAJOR; leading dimensions are in ELEMENTS (doubles).  hclooc_dgemm is the paper's untransposed
  *     operation (:180); transposed operands and the other level-3 routines the paper names as future work (:412) have their
- *     own entry points below (hclooc_dgemm_t, hclooc_dsyrk, hclooc_dsyr2k, hclooc_dtrsm[_side], hclooc_dpotrf).
+ *     own entry points below (hclooc_dgemm_t, hclooc_dsyrk, hclooc_dsyr2k, hclooc_dtrsm[_side], hclooc_dpotrf, hclooc_dgetrf).
  *   - All functions return an int status: 0 = success; a NEGATIVE value -k means the k-th argument
  *     (1-based, in the order of the C prototype) is invalid (LAPACK "info" convention); POSITIVE
  *     values are the HCLOOC_ERR_* codes below.  Nothing aborts and nothing throws across this ABI.
@@ -418,14 +418,17 @@ int hclooc_dpotrf_plan(int64_t N, size_t device_budget_bytes, int64_t* NB, uint6
  * out-of-core DGEMM (L streamed from the host, the panel in device memory); then its rows from the diagonal down are factored in
  * device memory (recursive halving: tile-kernel DGEMMs and DTRSMs; at the bottom a cooperative multi-CTA kernel that keeps a
  * 32-column panel in shared memory and pays one grid barrier per column).  The host matrix sees no row interchange until a final
- * pass brings every block column of L into the final order.  Synchronous: returns with A and ipiv complete.
+ * pass brings every block column of L into the final order.  Look-ahead of one panel: the call starts ONE worker thread per panel
+ * (joined before it returns) that drives the device factorization of panel j on a stream of its own while the calling thread drives the
+ * out-of-core updates of panel j+1; three panels stay resident where they fit 7/8 of the budget, else two in 5/8 (knobs:
+ * HCLOOC_GETRF_PANELS=2|3, HCLOOC_GETRF_LOOKAHEAD=0 factors in line).  Synchronous: returns with A and ipiv complete.
  * *info (LAPACK): 0, or j+1 > 0 for the first pivot u_jj that is exactly zero (the factorization is completed all the same; U is
  * singular).  The function still returns 0 then.  NaN in A: unspecified pivots.
  * Rounding: |P A - L U| <= gamma_n |L||U| elementwise, n = min(M, N) (Gaussian elimination in any order of operations, Higham
  * thm 9.3 / section 13.2); on data whose elimination is exact in FP64 the result is bit-identical to the unblocked definition.
  * stats (nullable): sums over the DGEMM calls and the panel copies; plan.nb = NB, plan.flops = M N^2 - N^3/3 (M >= N).
  * Errors: -2 M < 0 (or >= 2^31), -3 N, -4 A NULL, -5 lda < N, -6 ipiv NULL, -8 info NULL; HCLOOC_ERR_BUDGET when two 32-column
- * panels and their scratch do not fit 5/8 of the budget; the HCLOOC_ERR_* codes of hclooc_dgemm.  Knob: HCLOOC_GETRF_NB=n.     */
+ * panels and their scratch do not fit 5/8 of the budget (about 2 * M * 256 bytes + 1/4 MiB); the HCLOOC_ERR_* codes of hclooc_dgemm.  Knob: HCLOOC_GETRF_NB=n.     */
 int hclooc_dgetrf(hclooc_ctx* ctx, int64_t M, int64_t N, double* A, int64_t lda, int64_t* ipiv, size_t device_budget_bytes,
                   int64_t* info, hclooc_stats* stats_out);
 /* The panel width hclooc_dgetrf works with (pure host arithmetic) and the device bytes it keeps for itself (two panels, two
