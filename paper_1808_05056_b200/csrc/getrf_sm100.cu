@@ -1,10 +1,10 @@
 // getrf_sm100.cu -- the block kernels of the LU factorization with partial pivoting (hclooc_dgetrf / hclDgetrf; PAPER.md:412
 // names LU first among the out-of-core factorizations to be built on the DGEMM):
 //
-//   getrf_panel_kernel   factors ONE tall panel of m rows and w <= 32 columns that sits in device memory.  The flops of an LU
+//   getrf_panel_kernel   factors ONE tall panel of m rows and w <= 128 columns that sits in device memory.  The flops of an LU
 //                        factorization are DGEMM / DTRSM work on the tile kernel; what is left at the bottom of the recursion is
 //                        this: per column a pivot search over ALL remaining rows, one row interchange, a division per row and a
-//                        rank-1 update of at most 31 columns -- latency, not arithmetic.  So the panel is spread over up to one
+//                        rank-1 update of at most 127 columns -- latency, not arithmetic.  So the panel is spread over up to one
 //                        CTA per SM (cooperative launch): every CTA keeps its slab of rows in SHARED MEMORY for the whole panel
 //                        (one read and one write of the panel in HBM), and a column costs ONE grid-wide barrier: before it every
 //                        CTA publishes its best candidate (|value|, row, and the row's contents) and CTA 0 publishes row j; after
@@ -22,7 +22,7 @@ namespace hclooc {
 namespace {
 
 constexpr int LU_T = 256;           // threads per CTA
-constexpr int LU_W = 32;            // widest panel
+constexpr int LU_W = 128;           // widest panel
 constexpr int LU_MAXG = 192;        // most CTAs of a panel launch (>= SMs of the device, checked at launch)
 
 __device__ __forceinline__ double lu_shfl_down(double v, int off) {
@@ -41,11 +41,14 @@ __device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long
 // candidate order: larger |value| first, smaller row on ties
 __device__ __forceinline__ bool lu_better(double v, int r, double bv, int br) { return v > bv || (v == bv && r < br); }
 
-struct PanelSlots {                 // global scratch of one panel launch, one set per column (no reuse inside a launch)
-    double* cval;                   // [LU_W][G]          best |a_ij| of CTA g in column j (-1: no row of it is still in play)
-    int* crow;                      // [LU_W][G]          its row (panel-local)
-    double* ccont;                  // [LU_W][G][LU_W]    that row's contents
-    double* top;                    // [LU_W][LU_W]       row j before the interchange of column j
+// Global scratch of the panel launches.  TWO sets, used by the columns of even and of odd index: set j & 1 is written before the
+// barrier of column j and read right after it; a CTA writes it again only after the barrier of column j+1, at which every CTA has
+// arrived -- i.e. has finished those reads.
+struct PanelSlots {
+    double* cval;                   // [2][G]          best |a_ij| of CTA g in the column (-1: no row of it is still in play)
+    int* crow;                      // [2][G]          its row (panel-local)
+    double* ccont;                  // [2][G][LU_W]    that row's contents
+    double* top;                    // [2][LU_W]       row j before the interchange of column j
     unsigned long long* counter;    // arrivals at the grid barrier, monotone across launches (bar_base = its value at launch)
 };
 
@@ -62,10 +65,11 @@ getrf_panel_kernel(double* __restrict__ A, long long lda, long long m, int w, in
     const int nloc = (int)(m - r0 < (long long)rpc ? m - r0 : (long long)rpc);
     const int SW = w | 1;
     for (int r = warp; r < nloc; r += LU_T / 32)
-        if (lane < w) S[r * SW + lane] = A[(r0 + r) * lda + lane];
+        for (int c = lane; c < w; c += 32) S[r * SW + c] = A[(r0 + r) * lda + c];
     __syncthreads();
     const int nsteps = (int)(m < (long long)w ? m : (long long)w);
     for (int j = 0; j < nsteps; ++j) {
+        const int set = j & 1;
         // ---- this CTA's candidate for the pivot of column j
         double best = -1.0;
         int brow = 0x7fffffff;
@@ -90,10 +94,10 @@ getrf_panel_kernel(double* __restrict__ A, long long lda, long long m, int w, in
         }
         __syncthreads();
         best = red_v[0]; brow = red_r[0];
-        const size_t slot = (size_t)j * G + g;
+        const size_t slot = (size_t)set * G + g;
         if (tid == 0) { sl.cval[slot] = best; sl.crow[slot] = brow; }
         if (tid < w && best >= 0.0) sl.ccont[slot * LU_W + tid] = S[(size_t)(brow - r0) * SW + tid];
-        if (g == 0 && tid >= 32 && tid < 32 + w) sl.top[j * LU_W + tid - 32] = S[j * SW + tid - 32];
+        if (g == 0 && tid >= LU_W && tid < LU_W + w) sl.top[set * LU_W + tid - LU_W] = S[j * SW + tid - LU_W];
         // ---- the grid barrier of column j
         __threadfence();
         __syncthreads();
@@ -108,8 +112,8 @@ getrf_panel_kernel(double* __restrict__ A, long long lda, long long m, int w, in
             double bv = -2.0;
             int br = 0x7fffffff, bc = -1;
             for (int c = lane; c < G; c += 32) {
-                const double v = __ldcg(&sl.cval[(size_t)j * G + c]);
-                const int r = __ldcg(&sl.crow[(size_t)j * G + c]);
+                const double v = __ldcg(&sl.cval[(size_t)set * G + c]);
+                const int r = __ldcg(&sl.crow[(size_t)set * G + c]);
                 if (lu_better(v, r, bv, br)) { bv = v; br = r; bc = c; }
             }
 #pragma unroll
@@ -126,13 +130,13 @@ getrf_panel_kernel(double* __restrict__ A, long long lda, long long m, int w, in
         }
         __syncthreads();
         const int wc = win_cta, pr = win_row;
-        if (tid < w) P_s[tid] = wc < 0 ? __ldcg(&sl.top[j * LU_W + tid]) : __ldcg(&sl.ccont[((size_t)j * G + wc) * LU_W + tid]);
-        else if (tid >= 32 && tid < 32 + w) T_s[tid - 32] = __ldcg(&sl.top[j * LU_W + tid - 32]);
+        if (tid < w) P_s[tid] = wc < 0 ? __ldcg(&sl.top[set * LU_W + tid]) : __ldcg(&sl.ccont[((size_t)set * G + wc) * LU_W + tid]);
+        else if (tid >= LU_W && tid < LU_W + w) T_s[tid - LU_W] = __ldcg(&sl.top[set * LU_W + tid - LU_W]);
         __syncthreads();
         const double pivot = P_s[j];
         if (pr != j) {                               // rows j and pr change places, each owner taking the other's published copy
             if (g == wc && tid < w) S[(size_t)(pr - r0) * SW + tid] = T_s[tid];
-            if (g == 0 && tid >= 32 && tid < 32 + w) S[j * SW + tid - 32] = P_s[tid - 32];
+            if (g == 0 && tid >= LU_W && tid < LU_W + w) S[j * SW + tid - LU_W] = P_s[tid - LU_W];
         }
         if (g == 0 && tid == 0) {
             ipiv_out[j] = row_base + pr;
@@ -140,19 +144,23 @@ getrf_panel_kernel(double* __restrict__ A, long long lda, long long m, int w, in
         }
         __syncthreads();
         if (pivot != 0.0) {                          // a zero pivot: the column is zero from row j down, nothing to eliminate
+            // the multipliers, one thread per row (IEEE division, as the definition: 256 divisions in flight, not a chain per warp) ...
             for (int r = tid; r < nloc; r += LU_T)
-                if (r0 + r > j) S[r * SW + j] = S[r * SW + j] / pivot;            // IEEE division, as the definition
+                if (r0 + r > j) S[r * SW + j] = S[r * SW + j] / pivot;
             __syncthreads();
-            if (lane > j && lane < w) {
-                const double pc = P_s[lane];
-                for (int r = warp; r < nloc; r += LU_T / 32)
-                    if (r0 + r > j) S[r * SW + lane] = __dsub_rn(S[r * SW + lane], __dmul_rn(S[r * SW + j], pc));
+            // ... then one warp per row: the row's columns past j, 32 at a time
+#pragma unroll 4
+            for (int r = warp; r < nloc; r += LU_T / 32) {
+                if (r0 + r > j) {
+                    const double l = S[r * SW + j];
+                    for (int c = j + 1 + lane; c < w; c += 32) S[r * SW + c] = __dsub_rn(S[r * SW + c], __dmul_rn(l, P_s[c]));
+                }
             }
         }
         __syncthreads();
     }
     for (int r = warp; r < nloc; r += LU_T / 32)
-        if (lane < w) A[(r0 + r) * lda + lane] = S[r * SW + lane];
+        for (int c = lane; c < w; c += 32) A[(r0 + r) * lda + c] = S[r * SW + c];
 }
 
 // rows on grid.x (as many as a permutation touches), 256 columns per CTA on grid.y
@@ -178,11 +186,11 @@ row_scatter_kernel(double* __restrict__ X, long long ld, int ncols, const int* _
 
 // device scratch of the panel kernel for launches of at most gcap CTAs: [counter 64 B][top][cval][ccont][crow]
 size_t getrf_slot_bytes(int gcap) {
-    return 64 + (size_t)LU_W * LU_W * 8 + (size_t)LU_W * gcap * 8 + (size_t)LU_W * gcap * LU_W * 8 + (size_t)LU_W * gcap * 4 + 64;
+    return 64 + (size_t)2 * LU_W * 8 + (size_t)2 * gcap * 8 + (size_t)2 * gcap * LU_W * 8 + (size_t)2 * gcap * 4 + 64;
 }
 
-// Panel width the kernel can take for m rows on this device (32, or less when a CTA's slab of a very tall panel would not fit
-// its shared memory), the CTAs it will use and their rows; 0 if even 8 columns do not fit.
+// Panel width the kernel can take for m rows on this device (128, or less when a CTA's slab of a tall panel would not fit
+// its shared memory: 64 from ~32000 rows, 32 from ~63000), the CTAs it will use and their rows; 0 if even 8 columns do not fit.
 int getrf_panel_shape(long long m, int* G_out, int* rpc_out) {
     static int sms = 0, smem_max = 0, coop = 0;
     if (!sms) {
@@ -195,7 +203,9 @@ int getrf_panel_shape(long long m, int* G_out, int* rpc_out) {
     static const int g_env = [] { const char* e = getenv("HCLOOC_GETRF_MAXG"); const int v = e ? atoi(e) : 0; return v > 0 ? v : LU_MAXG; }();   // experiment knob
     const int maxg = std::min(sms < LU_MAXG ? sms : LU_MAXG, g_env);
     const size_t avail = (size_t)smem_max - 4096;                 // static shared memory and the runtime's share
+    static const int w_env = [] { const char* e = getenv("HCLOOC_GETRF_BW"); const int v = e ? atoi(e) : 0; return v >= 8 ? v : LU_W; }();     // experiment knob
     for (int w = LU_W; w >= 8; w >>= 1) {
+        if (w > w_env) continue;
         long long G = (m + 127) / 128;
         if (G > maxg) G = maxg;
         if (G < 1) G = 1;
@@ -231,9 +241,9 @@ int launch_getrf_panel(double* dA, int64_t lda, int64_t m, int w, long long* ipi
     PanelSlots sl;
     uint8_t* p = (uint8_t*)slots;
     sl.counter = (unsigned long long*)p;  p += 64;
-    sl.top = (double*)p;                  p += (size_t)LU_W * LU_W * 8;
-    sl.cval = (double*)p;                 p += (size_t)LU_W * gcap * 8;
-    sl.ccont = (double*)p;                p += (size_t)LU_W * gcap * LU_W * 8;
+    sl.top = (double*)p;                  p += (size_t)2 * LU_W * 8;
+    sl.cval = (double*)p;                 p += (size_t)2 * gcap * 8;
+    sl.ccont = (double*)p;                p += (size_t)2 * gcap * LU_W * 8;
     sl.crow = (int*)p;
     long long lda_ll = lda, m_ll = m;
     unsigned long long base = *bar_base;

@@ -408,7 +408,11 @@ extern "C" int hclooc_dgetrf(hclooc_ctx* ctx, int64_t M, int64_t N, double* A, i
         if (cudaSetDevice(ctx->device) != cudaSuccess) return HCLOOC_ERR_CUDA;
         const int64_t c0 = bj * NB, nbj = width(bj);
         int e = HCLOOC_OK;
-        if (c0 < n) e = dev_getrf(W, dPan[buf] + c0 * ldp, ldp, M - c0, nbj, c0, c0);
+        if (c0 < n) {
+            int g2, r2;
+            W.bw = getrf_panel_shape(M - c0, &g2, &r2);           // shorter panels take wider leaves
+            e = dev_getrf(W, dPan[buf] + c0 * ldp, ldp, M - c0, nbj, c0, c0);
+        }
         if (e) return e;
         HCL_CUDA(cudaEventRecord(ev_fact, s_fact));
         HCL_CUDA(cudaStreamWaitEvent(s_down, ev_fact, 0));
