@@ -417,7 +417,7 @@ int hclooc_dpotrf_plan(int64_t N, size_t device_budget_bytes, int64_t* NB, uint6
  * block column before it, it takes that block's interchanges, a device DTRSM against the block's unit lower triangle and one
  * out-of-core DGEMM (L streamed from the host, the panel in device memory); then its rows from the diagonal down are factored in
  * device memory (recursive halving: tile-kernel DGEMMs and DTRSMs; at the bottom a cooperative multi-CTA kernel that keeps a
- * 32-column panel in shared memory and pays one grid barrier per column).  The host matrix sees no row interchange until a final
+ * panel of up to 128 columns in shared memory and pays one grid barrier per column).  The host matrix sees no row interchange until a final
  * pass brings every block column of L into the final order.  Look-ahead of one panel: the call starts ONE worker thread per panel
  * (joined before it returns) that drives the device factorization of panel j on a stream of its own while the calling thread drives the
  * out-of-core updates of panel j+1; three panels stay resident where they fit 7/8 of the budget, else two in 5/8 (knobs:
