@@ -183,6 +183,34 @@ def test_dgetrf_large(H, dist):
         check_float(M, N, A0, got, ipiv, info, full_oracle=False)
 
 
+@pytest.mark.parametrize("M,N,dist", [(40000, 200, "exact"), (40000, 200, "uniform"), (70000, 96, "exact"), (70000, 96, "uniform"),
+                                      (120000, 64, "exact"), (120000, 40, "uniform")])
+def test_dgetrf_tall_panels_take_narrower_leaves(H, M, N, dist):
+    """The panel kernel keeps a CTA's slab of rows in shared memory: 128-column leaves up to ~32000 rows, 64 up to ~63000, 32 up to
+    ~112000, 16 beyond (getrf_panel_shape).  Every width against the oracle on one resident panel."""
+    if dist == "exact":
+        vals, F_want, ipiv_want = exact_lu_case(M, N, M + N)
+    else:
+        vals = synthgen.fill_numpy(M, N, 37, "A", "uniform")
+    A = host_matrix(H, vals, 0)
+    A0 = A.view.copy()
+    ipiv, info, st = H.hclooc_dgetrf(None, M, N, A, A.ld, 512 * MiB)
+    got = A.view.copy()
+    assert st.plan.n_steps == 1 and info == 0
+    ref = A0.copy()
+    ipiv_ref, info_ref = oracle.dgetrf(ref)
+    assert info_ref == 0 and np.array_equal(ipiv, ipiv_ref), f"first differing interchange at step {int(np.argmax(ipiv != ipiv_ref))}"
+    if dist == "exact":
+        assert np.array_equal(ipiv, ipiv_want) and np.array_equal(got, F_want) and np.array_equal(ref, F_want)
+    else:
+        rng = np.random.default_rng(9)
+        rows = np.unique(np.concatenate([[0, 1, N - 1, N, M - 1], rng.integers(0, M, 200)]))
+        res, den = oracle.dgetrf_residual(A0, got, ipiv, rows, None)
+        assert (res <= oracle.dgetrf_gate(N) * den).all()
+        assert (np.abs(np.tril(got[:, :N], -1)) <= 1.0).all()
+        assert np.abs(got - ref).max() <= 1e-9 * np.abs(np.triu(ref[:N])).max()
+
+
 @pytest.mark.parametrize("panels", [2, 3])
 def test_dgetrf_two_and_three_resident_panels(H, panels, monkeypatch):
     """HCLOOC_GETRF_PANELS caps the resident panels: with two, the next panel's upload follows the freshest update range by range
