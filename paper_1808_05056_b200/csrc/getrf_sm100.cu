@@ -144,16 +144,16 @@ getrf_panel_kernel(double* __restrict__ A, long long lda, long long m, int w, in
         }
         __syncthreads();
         if (pivot != 0.0) {                          // a zero pivot: the column is zero from row j down, nothing to eliminate
-            // the multipliers, one thread per row (IEEE division, as the definition: 256 divisions in flight, not a chain per warp) ...
-            for (int r = tid; r < nloc; r += LU_T)
-                if (r0 + r > j) S[r * SW + j] = S[r * SW + j] / pivot;
-            __syncthreads();
-            // ... then one warp per row: the row's columns past j, 32 at a time
-#pragma unroll 4
-            for (int r = warp; r < nloc; r += LU_T / 32) {
+            // one thread per row: the multiplier (IEEE division, as the definition) stays in a register, then the row's columns past
+            // j one after the other -- the lanes of a warp walk 32 consecutive rows (odd stride: no bank conflict), the pivot row's
+            // element is a broadcast, and the iterations of a thread are independent, so the loads run ahead of the arithmetic
+            for (int r = tid; r < nloc; r += LU_T) {
                 if (r0 + r > j) {
-                    const double l = S[r * SW + j];
-                    for (int c = j + 1 + lane; c < w; c += 32) S[r * SW + c] = __dsub_rn(S[r * SW + c], __dmul_rn(l, P_s[c]));
+                    double* __restrict__ row = S + (size_t)r * SW;
+                    const double l = row[j] / pivot;
+                    row[j] = l;
+#pragma unroll 8
+                    for (int c = j + 1; c < w; ++c) row[c] = __dsub_rn(row[c], __dmul_rn(l, P_s[c]));
                 }
             }
         }
