@@ -68,17 +68,17 @@ getrf_panel_kernel(double* __restrict__ A, long long lda, long long m, int w, in
         for (int c = lane; c < w; c += 32) S[r * SW + c] = A[(r0 + r) * lda + c];
     __syncthreads();
     const int nsteps = (int)(m < (long long)w ? m : (long long)w);
+    // this thread's candidate for the pivot of the NEXT column: found at the end of a column's elimination, in the rows the thread
+    // has just updated (column 0: here)
+    double best = -1.0;
+    int brow = 0x7fffffff;
+    for (int r = tid; r < nloc; r += LU_T) {
+        const double v = fabs(S[r * SW]);
+        if (v > best) { best = v; brow = (int)(r0 + r); }
+    }
     for (int j = 0; j < nsteps; ++j) {
         const int set = j & 1;
         // ---- this CTA's candidate for the pivot of column j
-        double best = -1.0;
-        int brow = 0x7fffffff;
-        for (int r = tid; r < nloc; r += LU_T) {
-            if (r0 + r >= j) {
-                const double v = fabs(S[r * SW + j]);
-                if (v > best) { best = v; brow = (int)(r0 + r); }
-            }
-        }
 #pragma unroll
         for (int off = 16; off; off >>= 1) {
             const double ov = lu_shfl_down(best, off);
@@ -87,13 +87,10 @@ getrf_panel_kernel(double* __restrict__ A, long long lda, long long m, int w, in
         }
         if (lane == 0) { red_v[warp] = best; red_r[warp] = brow; }
         __syncthreads();
-        if (tid == 0) {
-            for (int k = 1; k < LU_T / 32; ++k)
-                if (lu_better(red_v[k], red_r[k], best, brow)) { best = red_v[k]; brow = red_r[k]; }
-            red_v[0] = best; red_r[0] = brow;
-        }
-        __syncthreads();
         best = red_v[0]; brow = red_r[0];
+#pragma unroll
+        for (int k = 1; k < LU_T / 32; ++k)
+            if (lu_better(red_v[k], red_r[k], best, brow)) { best = red_v[k]; brow = red_r[k]; }
         const size_t slot = (size_t)set * G + g;
         if (tid == 0) { sl.cval[slot] = best; sl.crow[slot] = brow; }
         if (tid < w && best >= 0.0) sl.ccont[slot * LU_W + tid] = S[(size_t)(brow - r0) * SW + tid];
@@ -107,7 +104,7 @@ getrf_panel_kernel(double* __restrict__ A, long long lda, long long m, int w, in
             while (ld_acquire_u64(sl.counter) < target) { }
         }
         __syncthreads();
-        // ---- the same winner in every CTA
+        // ---- the same winner in every CTA: warp 0 picks it and fetches the two rows that change places
         if (warp == 0) {
             double bv = -2.0;
             int br = 0x7fffffff, bc = -1;
@@ -123,16 +120,25 @@ getrf_panel_kernel(double* __restrict__ A, long long lda, long long m, int w, in
                 const int oc = __shfl_down_sync(0xffffffffu, bc, off);
                 if (lu_better(ov, orow, bv, br)) { bv = ov; br = orow; bc = oc; }
             }
-            if (lane == 0) {
-                if (!(bv >= 0.0)) { br = j; bc = -1; }      // nothing comparable in the column (NaN): no interchange
-                win_cta = bc; win_row = br;
+            if (!(bv >= 0.0)) { br = j; bc = -1; }          // nothing comparable in the column (NaN): no interchange
+            br = __shfl_sync(0xffffffffu, br, 0);
+            bc = __shfl_sync(0xffffffffu, bc, 0);
+            double tv[LU_W / 32], pv[LU_W / 32];          // all loads in flight before the first use: one L2 round trip, not four
+#pragma unroll
+            for (int i = 0; i < LU_W / 32; ++i) {
+                const int c = lane + 32 * i;
+                tv[i] = c < w ? __ldcg(&sl.top[set * LU_W + c]) : 0.0;
+                pv[i] = c < w && bc >= 0 ? __ldcg(&sl.ccont[((size_t)set * G + bc) * LU_W + c]) : 0.0;
             }
+#pragma unroll
+            for (int i = 0; i < LU_W / 32; ++i) {
+                const int c = lane + 32 * i;
+                if (c < w) { T_s[c] = tv[i]; P_s[c] = bc < 0 ? tv[i] : pv[i]; }
+            }
+            if (lane == 0) { win_cta = bc; win_row = br; }
         }
         __syncthreads();
         const int wc = win_cta, pr = win_row;
-        if (tid < w) P_s[tid] = wc < 0 ? __ldcg(&sl.top[set * LU_W + tid]) : __ldcg(&sl.ccont[((size_t)set * G + wc) * LU_W + tid]);
-        else if (tid >= LU_W && tid < LU_W + w) T_s[tid - LU_W] = __ldcg(&sl.top[set * LU_W + tid - LU_W]);
-        __syncthreads();
         const double pivot = P_s[j];
         if (pr != j) {                               // rows j and pr change places, each owner taking the other's published copy
             if (g == wc && tid < w) S[(size_t)(pr - r0) * SW + tid] = T_s[tid];
@@ -143,22 +149,31 @@ getrf_panel_kernel(double* __restrict__ A, long long lda, long long m, int w, in
             if (pivot == 0.0) atomicCAS((unsigned long long*)info, 0ULL, (unsigned long long)(info_base + j + 1));
         }
         __syncthreads();
-        if (pivot != 0.0) {                          // a zero pivot: the column is zero from row j down, nothing to eliminate
-            // one thread per row: the multiplier (IEEE division, as the definition) stays in a register, then the row's columns past
-            // j one after the other -- the lanes of a warp walk 32 consecutive rows (odd stride: no bank conflict), the pivot row's
-            // element is a broadcast, and the iterations of a thread are independent, so the loads run ahead of the arithmetic
-            for (int r = tid; r < nloc; r += LU_T) {
-                if (r0 + r > j) {
-                    double* __restrict__ row = S + (size_t)r * SW;
+        // ---- elimination, one thread per row: the multiplier (IEEE division, as the definition) stays in a register, then the
+        // row's columns past j one after the other -- the lanes of a warp walk 32 consecutive rows (odd stride: no bank conflict),
+        // the pivot row's element is a broadcast, and the iterations of a thread are independent, so the loads run ahead of the
+        // arithmetic.  A zero pivot: the column is zero from row j down, nothing to eliminate.  The thread then looks at its rows'
+        // entries in column j+1, which it has just written: its candidate for the next pivot (no barrier needed until the CTA
+        // reduction at the top of the loop, which also orders these writes before anybody else's reads).
+        best = -1.0;
+        brow = 0x7fffffff;
+        for (int r = tid; r < nloc; r += LU_T) {
+            if (r0 + r > j) {
+                double* __restrict__ row = S + (size_t)r * SW;
+                if (pivot != 0.0) {
                     const double l = row[j] / pivot;
                     row[j] = l;
 #pragma unroll 8
                     for (int c = j + 1; c < w; ++c) row[c] = __dsub_rn(row[c], __dmul_rn(l, P_s[c]));
                 }
+                if (j + 1 < nsteps) {
+                    const double v = fabs(row[j + 1]);
+                    if (v > best) { best = v; brow = (int)(r0 + r); }
+                }
             }
         }
-        __syncthreads();
     }
+    __syncthreads();
     for (int r = warp; r < nloc; r += LU_T / 32)
         for (int c = lane; c < w; c += 32) A[(r0 + r) * lda + c] = S[r * SW + c];
 }
