@@ -27,7 +27,7 @@ configs[4] (beyond-HBM: M = N = 163840, K = 8192, budget = all free HBM) scaled 
 `--impl reference` times the oracle (the reference arm of this tier) under the same metric string and
 workload name.  Under torchrun the problem grows to world*M rows cut into one row band of C per GPU
 (independent bands, B on every rank, no collective: weak scaling).
-`--op dsyrk|dtrsm|dpotrf` and `--sweep transition` time the other product paths (one JSON line each).
+`--op dsyrk|dtrsm|dpotrf|dgetrf` (and the `_dev` device phases) and `--sweep transition` time the other product paths (one JSON line each).
 """
 import argparse
 import json
@@ -660,7 +660,7 @@ class Bench:
 
 # ---------------------------------------------------------------------------------------------- the other product paths
 def run_op(args):
-    """`--op dsyrk|dsyr2k|dtrsm|dtrsm_right|dpotrf`: the routines built on the out-of-core DGEMM, timed like the
+    """`--op dsyrk|dsyr2k|dtrsm|dtrsm_right|dpotrf|dgetrf`: the routines built on the out-of-core DGEMM, timed like the
     DGEMM -- pinned host operands, a context created beforehand, wall time inside the call -- against the roofline of the call
     (the slower of its flops at the FP64 peak and its own bytes at the link rates measured here).  One JSON line."""
     import torch
@@ -852,7 +852,7 @@ def run_cublasxt(args):
 
 
 def run_dev_op(args, H, torch):
-    """`--op dtrsm_dev|dtrsm_right_dev|dpotrf_dev`: the DEVICE phases alone (hclDtrsmAsync / hclDpotrfAsync on device-resident operands:
+    """`--op dtrsm_dev|dtrsm_right_dev|dpotrf_dev|dgetrf_dev`: the DEVICE phases alone (hclDtrsmAsync / hclDpotrfAsync / hclDgetrf on device-resident operands:
     recursive halving down to the 128 x 128 block kernels), CUDA events on the launching stream, median of --steps launches.  With
     --m 128 (dtrsm_dev) / --n 128 (the others) the call is ONE launch of the block kernel."""
     op, M, N = args.op, args.m, args.n
