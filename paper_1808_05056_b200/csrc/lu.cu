@@ -491,10 +491,14 @@ extern "C" int hclooc_dgetrf(hclooc_ctx* ctx, int64_t M, int64_t N, double* A, i
         // ---- panel bj is factored by the worker ...
         HCL_CUDA(cudaStreamWaitEvent(s_fact, ev_fresh, 0));
         worker.rc = HCLOOC_OK;
+        bool spawned = false;
         if (lookahead) {
-            worker.active = true;
-            worker.th = std::thread([&worker, &factor_panel, bj, cur] { worker.rc = factor_panel(bj, cur); });
-        } else if ((rc = factor_panel(bj, cur))) return rc;
+            try {                                                // nothing throws across this ABI: no thread to be had -> factor in line
+                worker.th = std::thread([&worker, &factor_panel, bj, cur] { worker.rc = factor_panel(bj, cur); });
+                worker.active = spawned = true;
+            } catch (...) { spawned = false; }
+        }
+        if (!spawned && (rc = factor_panel(bj, cur))) return rc;
         // ---- ... while panel bj+1 comes up and receives the updates of the blocks BEFORE bj through the pipeline (L from the host)
         if (next && !next_up) {
             HCL_CUDA(cudaStreamWaitEvent(s_up, ev_fresh, 0));                        // nothing of this call still reads the buffer's previous tenant
