@@ -431,7 +431,7 @@ int hclooc_dpotrf_plan(int64_t N, size_t device_budget_bytes, int64_t* NB, uint6
  * panels and their scratch do not fit 5/8 of the budget (about 2 * M * 256 bytes + 1/4 MiB); the HCLOOC_ERR_* codes of hclooc_dgemm.  Knob: HCLOOC_GETRF_NB=n.     */
 int hclooc_dgetrf(hclooc_ctx* ctx, int64_t M, int64_t N, double* A, int64_t lda, int64_t* ipiv, size_t device_budget_bytes,
                   int64_t* info, hclooc_stats* stats_out);
-/* The panel width hclooc_dgetrf works with (pure host arithmetic) and the device bytes it keeps for itself (two panels, two
+/* The panel width hclooc_dgetrf works with (pure host arithmetic) and the device bytes it keeps for itself (two or three panels, two
  * diagonal blocks, scratch).  Errors: -1 M < 1, -2 N < 1, -4 NULL output, HCLOOC_ERR_BUDGET.                                 */
 int hclooc_dgetrf_plan(int64_t M, int64_t N, size_t device_budget_bytes, int64_t* NB, uint64_t* reserved_bytes);
 /* The device phase on its own: P A = L U of an M x N row-major matrix in DEVICE memory (16-byte aligned, lda even), in place, on
